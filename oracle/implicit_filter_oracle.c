@@ -1,0 +1,337 @@
+/*
+ * ORACLE -- test infrastructure, not product code.
+ *
+ * A plain, slow, fp64 CPU statement of what the hot path of arXiv 2404.07398 computes, written
+ * from the paper (citations "PAPER.md:NN" = /root/reference/PAPER.md line NN) with the readings
+ * listed in DESIGN.md.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may call it.  It shares no code with paper_2404_07398_b200/ (the CUDA
+ * library) and must never be used as a fallback for it.
+ *
+ * What is computed (notation of BASELINE.json: S = P1 stiffness, M = diag(A_v) lumped mass):
+ *   geometry   PAPER.md:57-61   S_vv' = integral grad N_v . grad N_v' dS  (closed form: -1/2 cot of the
+ *                               angle opposite edge vv', summed over the triangles sharing the edge);
+ *                               boundary term dropped = no-normal-flux condition
+ *   mass       PAPER.md:61      M^L = diag(A_v), A_v = median-dual area = sum of area_t/3 (Fig. 1a, :41)
+ *   operator   PAPER.md:61,:63  A_l = M + gamma l^2 S           (n = 1)
+ *                               A_l = M + gamma l^4 S M^-1 S    (n = 2)      gamma = 1/2
+ *   solve      PAPER.md:113     conjugate gradients on A_l x = M phi started from x0 = phi (the
+ *                               Guedot subtraction), Jacobi preconditioner (reading A8),
+ *                               stop at ||r||_2 <= tol ||M phi||_2 (reading A6; tol 1e-13 by default)
+ *   energy     PAPER.md:31      e_l = 1/2 sum_v A_v x_v^2 / sum_v A_v   ("second moment")
+ *   spectrum   PAPER.md:31,:209 k_l = 1/l ; E_j = (e_j - e_j+1)/(k_j - k_j+1) at sqrt(k_j k_j+1) (reading A4)
+ *   dense      BASELINE.json    Cholesky solve of the dense A_l for small meshes (cross-check of CG)
+ *
+ * Pins (tests/test_oracle_pins.py): P1-gradient definition of S by quadrature-free element matrices,
+ * 5-point stencil on the uniform grid, equilateral lattice, plane-wave closed form,
+ * dense solve, mean conservation, energy monotonicity, icosphere eigenvalues l(l+1).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    int64_t nv;       /* vertices */
+    int64_t nnz;      /* stored entries of S, diagonal included */
+    int64_t *rowptr;  /* [nv+1] */
+    int32_t *col;     /* [nnz] ascending within a row */
+    double *val;      /* [nnz] */
+    double *area;     /* [nv] A_v */
+    double *gdiag;    /* [nv] diag(S M^-1 S)_v = sum_j S_vj^2 / A_j */
+    double *sdiag;    /* [nv] S_vv */
+} orc_mesh;
+
+static void edge_vec(const double *coords, int dim, const double *period, int64_t from, int64_t to,
+                     double e[3]) {
+    /* e = x_to - x_from, minimum image on periodic axes: d -= P round(d/P) */
+    e[0] = e[1] = e[2] = 0.0;
+    for (int d = 0; d < dim; ++d) {
+        double v = coords[to * dim + d] - coords[from * dim + d];
+        if (period && period[d] > 0.0) v -= period[d] * nearbyint(v / period[d]);
+        e[d] = v;
+    }
+}
+
+void orc_free(orc_mesh *m) {
+    if (!m) return;
+    free(m->rowptr); free(m->col); free(m->val); free(m->area); free(m->gdiag); free(m->sdiag);
+    free(m);
+}
+
+/* Build S (CSR) and A_v.  Returns NULL and sets *err: 1 bad index, 2 degenerate triangle,
+ * 3 vertex in no triangle (A_v = 0), 4 out of memory. */
+orc_mesh *orc_build(const double *coords, int dim, int64_t nv, const int32_t *tri, int64_t nt,
+                    const double *period, int *err) {
+    *err = 0;
+    orc_mesh *m = (orc_mesh *)calloc(1, sizeof(orc_mesh));
+    int64_t *cap = (int64_t *)calloc((size_t)nv + 1, sizeof(int64_t));
+    if (!m || !cap) { *err = 4; free(cap); orc_free(m); return NULL; }
+    m->nv = nv;
+    /* capacity: every triangle adds two off-diagonal contributions to each of its three rows */
+    for (int64_t t = 0; t < nt; ++t)
+        for (int c = 0; c < 3; ++c) {
+            int64_t v = tri[3 * t + c];
+            if (v < 0 || v >= nv) { *err = 1; free(cap); orc_free(m); return NULL; }
+            cap[v + 1] += 2;
+        }
+    for (int64_t t = 0; t < nt; ++t)
+        if (tri[3 * t] == tri[3 * t + 1] || tri[3 * t] == tri[3 * t + 2] || tri[3 * t + 1] == tri[3 * t + 2]) {
+            *err = 1; free(cap); orc_free(m); return NULL;
+        }
+    for (int64_t v = 0; v < nv; ++v) cap[v + 1] += cap[v] + 1; /* +1: the diagonal */
+    int64_t total = cap[nv];
+    int32_t *tc = (int32_t *)malloc((size_t)total * sizeof(int32_t));
+    double *tv = (double *)malloc((size_t)total * sizeof(double));
+    int64_t *fill = (int64_t *)calloc((size_t)nv, sizeof(int64_t));
+    m->area = (double *)calloc((size_t)nv, sizeof(double));
+    if (!tc || !tv || !fill || !m->area) { *err = 4; goto fail; }
+
+    for (int64_t t = 0; t < nt; ++t) {
+        double tarea = 0.0;
+        for (int c = 0; c < 3; ++c) {
+            /* corner c, the other two vertices a, b: the angle at c is opposite edge ab */
+            int64_t vc = tri[3 * t + c], va = tri[3 * t + (c + 1) % 3], vb = tri[3 * t + (c + 2) % 3];
+            double e1[3], e2[3];
+            edge_vec(coords, dim, period, vc, va, e1);
+            edge_vec(coords, dim, period, vc, vb, e2);
+            double cx = e1[1] * e2[2] - e1[2] * e2[1];
+            double cy = e1[2] * e2[0] - e1[0] * e2[2];
+            double cz = e1[0] * e2[1] - e1[1] * e2[0];
+            double cr = sqrt(cx * cx + cy * cy + cz * cz);          /* = 2 * area, unsigned */
+            double dot = e1[0] * e2[0] + e1[1] * e2[1] + e1[2] * e2[2];
+            double n1 = e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2];
+            double n2 = e2[0] * e2[0] + e2[1] * e2[1] + e2[2] * e2[2];
+            if (!(cr > 1e-14 * (n1 + n2))) { *err = 2; goto fail; }
+            double w = -0.5 * dot / cr;                              /* -1/2 cot(angle at c) */
+            tc[cap[va] + fill[va]] = (int32_t)vb; tv[cap[va] + fill[va]] = w; fill[va]++;
+            tc[cap[vb] + fill[vb]] = (int32_t)va; tv[cap[vb] + fill[vb]] = w; fill[vb]++;
+            if (c == 0) tarea = 0.5 * cr;
+        }
+        for (int c = 0; c < 3; ++c) m->area[tri[3 * t + c]] += tarea / 3.0;
+    }
+    for (int64_t v = 0; v < nv; ++v)
+        if (!(m->area[v] > 0.0)) { *err = 3; goto fail; }
+
+    /* per row: sort by column, merge duplicates, add the diagonal S_vv = -sum of off-diagonals */
+    m->rowptr = (int64_t *)calloc((size_t)nv + 1, sizeof(int64_t));
+    if (!m->rowptr) { *err = 4; goto fail; }
+    for (int64_t v = 0; v < nv; ++v) {
+        int64_t b = cap[v], n = fill[v];
+        for (int64_t i = 1; i < n; ++i) {          /* insertion sort, stable */
+            int32_t c = tc[b + i]; double x = tv[b + i]; int64_t j = i;
+            while (j > 0 && tc[b + j - 1] > c) { tc[b + j] = tc[b + j - 1]; tv[b + j] = tv[b + j - 1]; --j; }
+            tc[b + j] = c; tv[b + j] = x;
+        }
+        int64_t u = 0;
+        for (int64_t i = 0; i < n; ++i) {
+            if (u > 0 && tc[b + u - 1] == tc[b + i]) tv[b + u - 1] += tv[b + i];
+            else { tc[b + u] = tc[b + i]; tv[b + u] = tv[b + i]; ++u; }
+        }
+        fill[v] = u;
+        m->rowptr[v + 1] = m->rowptr[v] + u + 1;
+    }
+    m->nnz = m->rowptr[nv];
+    m->col = (int32_t *)malloc((size_t)m->nnz * sizeof(int32_t));
+    m->val = (double *)malloc((size_t)m->nnz * sizeof(double));
+    m->sdiag = (double *)malloc((size_t)nv * sizeof(double));
+    m->gdiag = (double *)malloc((size_t)nv * sizeof(double));
+    if (!m->col || !m->val || !m->sdiag || !m->gdiag) { *err = 4; goto fail; }
+    for (int64_t v = 0; v < nv; ++v) {
+        int64_t b = cap[v], n = fill[v], o = m->rowptr[v];
+        double diag = 0.0;
+        for (int64_t i = 0; i < n; ++i) diag -= tv[b + i];
+        int placed = 0;
+        for (int64_t i = 0; i < n; ++i) {
+            if (!placed && tc[b + i] > v) { m->col[o] = (int32_t)v; m->val[o] = diag; ++o; placed = 1; }
+            m->col[o] = tc[b + i]; m->val[o] = tv[b + i]; ++o;
+        }
+        if (!placed) { m->col[o] = (int32_t)v; m->val[o] = diag; ++o; }
+        m->sdiag[v] = diag;
+    }
+    for (int64_t v = 0; v < nv; ++v) {
+        double g = 0.0;
+        for (int64_t i = m->rowptr[v]; i < m->rowptr[v + 1]; ++i)
+            g += m->val[i] * m->val[i] / m->area[m->col[i]];
+        m->gdiag[v] = g;
+    }
+    free(tc); free(tv); free(fill); free(cap);
+    return m;
+fail:
+    free(tc); free(tv); free(fill); free(cap); orc_free(m);
+    return NULL;
+}
+
+int64_t orc_nv(const orc_mesh *m) { return m->nv; }
+int64_t orc_nnz(const orc_mesh *m) { return m->nnz; }
+void orc_get_csr(const orc_mesh *m, int64_t *rowptr, int32_t *col, double *val) {
+    memcpy(rowptr, m->rowptr, (size_t)(m->nv + 1) * sizeof(int64_t));
+    memcpy(col, m->col, (size_t)m->nnz * sizeof(int32_t));
+    memcpy(val, m->val, (size_t)m->nnz * sizeof(double));
+}
+void orc_get_area(const orc_mesh *m, double *area) { memcpy(area, m->area, (size_t)m->nv * sizeof(double)); }
+
+/* y = S p */
+void orc_apply_S(const orc_mesh *m, const double *p, double *y) {
+#pragma omp parallel for schedule(static)
+    for (int64_t v = 0; v < m->nv; ++v) {
+        double s = 0.0;
+        for (int64_t i = m->rowptr[v]; i < m->rowptr[v + 1]; ++i) s += m->val[i] * p[m->col[i]];
+        y[v] = s;
+    }
+}
+
+/* out = A_l p,  A_l = M + gamma l^(2n) S (M^-1 S)^(n-1)   (PAPER.md:61 n=1, PAPER.md:63 n=2).
+ * tmp: scratch [nv], used for n = 2 only. */
+void orc_apply(const orc_mesh *m, double ell, int n, double gamma, const double *p, double *out, double *tmp) {
+    const double c = gamma * pow(ell, 2.0 * n);
+    if (n == 1) {
+        orc_apply_S(m, p, out);
+#pragma omp parallel for schedule(static)
+        for (int64_t v = 0; v < m->nv; ++v) out[v] = m->area[v] * p[v] + c * out[v];
+    } else {
+        orc_apply_S(m, p, tmp);                                   /* M psi = S p */
+#pragma omp parallel for schedule(static)
+        for (int64_t v = 0; v < m->nv; ++v) tmp[v] /= m->area[v];
+        orc_apply_S(m, tmp, out);
+#pragma omp parallel for schedule(static)
+        for (int64_t v = 0; v < m->nv; ++v) out[v] = m->area[v] * p[v] + c * out[v];
+    }
+}
+
+static double dot(int64_t n, const double *a, const double *b) {
+    double s = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : s)
+    for (int64_t i = 0; i < n; ++i) s += a[i] * b[i];
+    return s;
+}
+
+/* Jacobi-preconditioned CG on A_l x = M phi from x0 = phi.
+ * Stops when the recursive residual satisfies ||r||_2 <= tol ||M phi||_2, or at max_iter.
+ * Outputs: x [nv]; *iters; *rec_res = ||r||/||M phi|| (recursive); *true_res = ||M phi - A_l x||/||M phi||.
+ * Returns 0 converged, 1 iteration cap, 2 breakdown (p.Ap <= 0 or non-finite), 4 out of memory. */
+int orc_solve(const orc_mesh *m, const double *phi, double ell, int n, double gamma, double tol,
+              int64_t max_iter, double *x, int64_t *iters, double *rec_res, double *true_res) {
+    const int64_t nv = m->nv;
+    const double c = gamma * pow(ell, 2.0 * n);
+    double *b = (double *)malloc((size_t)nv * sizeof(double));
+    double *r = (double *)malloc((size_t)nv * sizeof(double));
+    double *z = (double *)malloc((size_t)nv * sizeof(double));
+    double *p = (double *)malloc((size_t)nv * sizeof(double));
+    double *q = (double *)malloc((size_t)nv * sizeof(double));
+    double *d = (double *)malloc((size_t)nv * sizeof(double));
+    double *tmp = (double *)malloc((size_t)nv * sizeof(double));
+    int status = 1;
+    if (!b || !r || !z || !p || !q || !d || !tmp) { status = 4; goto done; }
+    for (int64_t v = 0; v < nv; ++v) {
+        b[v] = m->area[v] * phi[v];
+        x[v] = phi[v];
+        d[v] = m->area[v] + c * (n == 1 ? m->sdiag[v] : m->gdiag[v]);   /* diag(A_l) */
+    }
+    orc_apply(m, ell, n, gamma, x, q, tmp);
+    for (int64_t v = 0; v < nv; ++v) { r[v] = b[v] - q[v]; z[v] = r[v] / d[v]; p[v] = z[v]; }
+    double bb = dot(nv, b, b);
+    double rho = dot(nv, r, z);
+    double rr = dot(nv, r, r);
+    int64_t it = 0;
+    if (rr <= tol * tol * bb) status = 0;
+    while (status == 1 && it < max_iter) {
+        orc_apply(m, ell, n, gamma, p, q, tmp);
+        double pq = dot(nv, p, q);
+        if (!(pq > 0.0) || !isfinite(pq)) { status = 2; break; }
+        double alpha = rho / pq;
+#pragma omp parallel for schedule(static)
+        for (int64_t v = 0; v < nv; ++v) { x[v] += alpha * p[v]; r[v] -= alpha * q[v]; z[v] = r[v] / d[v]; }
+        double rho_new = dot(nv, r, z);
+        rr = dot(nv, r, r);
+        ++it;
+        if (rr <= tol * tol * bb) { status = 0; break; }
+        double beta = rho_new / rho;
+        rho = rho_new;
+#pragma omp parallel for schedule(static)
+        for (int64_t v = 0; v < nv; ++v) p[v] = z[v] + beta * p[v];
+    }
+    *iters = it;
+    *rec_res = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+    orc_apply(m, ell, n, gamma, x, q, tmp);
+    for (int64_t v = 0; v < nv; ++v) q[v] = b[v] - q[v];
+    *true_res = bb > 0.0 ? sqrt(dot(nv, q, q) / bb) : 0.0;
+done:
+    free(b); free(r); free(z); free(p); free(q); free(d); free(tmp);
+    return status;
+}
+
+/* e = 1/2 sum_v A_v x_v^2 / sum_v A_v  ("second moment"; reading A4) */
+double orc_energy(const orc_mesh *m, const double *x) {
+    double s = 0.0, a = 0.0;
+    for (int64_t v = 0; v < m->nv; ++v) { s += m->area[v] * x[v] * x[v]; a += m->area[v]; }
+    return 0.5 * s / a;
+}
+
+/* k_j = 1/l_j; E_j = (e_j - e_j+1)/(k_j - k_j+1), k_mid_j = sqrt(k_j k_j+1), j < L-1 */
+void orc_spectrum(const double *ells, const double *e, int L, double *k_mid, double *E) {
+    for (int j = 0; j + 1 < L; ++j) {
+        double k0 = 1.0 / ells[j], k1 = 1.0 / ells[j + 1];
+        E[j] = (e[j] - e[j + 1]) / (k0 - k1);
+        k_mid[j] = sqrt(k0 * k1);
+    }
+}
+
+/* Dense check path: build A_l densely, Cholesky-factorise, solve A_l x = M phi.  O(nv^3): small meshes only.
+ * Returns 0 ok, 2 not positive definite, 4 out of memory. */
+int orc_dense_solve(const orc_mesh *m, const double *phi, double ell, int n, double gamma, double *x) {
+    const int64_t nv = m->nv;
+    const double c = gamma * pow(ell, 2.0 * n);
+    double *Sd = (double *)calloc((size_t)(nv * nv), sizeof(double));
+    double *A = (double *)calloc((size_t)(nv * nv), sizeof(double));
+    if (!Sd || !A) { free(Sd); free(A); return 4; }
+    for (int64_t v = 0; v < nv; ++v)
+        for (int64_t i = m->rowptr[v]; i < m->rowptr[v + 1]; ++i) Sd[v * nv + m->col[i]] = m->val[i];
+    if (n == 1) {
+        for (int64_t i = 0; i < nv * nv; ++i) A[i] = c * Sd[i];
+    } else {
+        for (int64_t i = 0; i < nv; ++i)
+            for (int64_t k = 0; k < nv; ++k) {
+                double sik = Sd[i * nv + k];
+                if (sik == 0.0) continue;
+                double f = c * sik / m->area[k];
+                for (int64_t j = 0; j < nv; ++j) A[i * nv + j] += f * Sd[k * nv + j];
+            }
+    }
+    for (int64_t v = 0; v < nv; ++v) A[v * nv + v] += m->area[v];
+    /* Cholesky A = L L^T, lower triangle in place */
+    for (int64_t j = 0; j < nv; ++j) {
+        double s = A[j * nv + j];
+        for (int64_t k = 0; k < j; ++k) s -= A[j * nv + k] * A[j * nv + k];
+        if (!(s > 0.0)) { free(Sd); free(A); return 2; }
+        double ljj = sqrt(s);
+        A[j * nv + j] = ljj;
+        for (int64_t i = j + 1; i < nv; ++i) {
+            double t = A[i * nv + j];
+            for (int64_t k = 0; k < j; ++k) t -= A[i * nv + k] * A[j * nv + k];
+            A[i * nv + j] = t / ljj;
+        }
+    }
+    for (int64_t i = 0; i < nv; ++i) {              /* L y = M phi */
+        double t = m->area[i] * phi[i];
+        for (int64_t k = 0; k < i; ++k) t -= A[i * nv + k] * x[k];
+        x[i] = t / A[i * nv + i];
+    }
+    for (int64_t i = nv - 1; i >= 0; --i) {         /* L^T x = y */
+        double t = x[i];
+        for (int64_t k = i + 1; k < nv; ++k) t -= A[k * nv + i] * x[k];
+        x[i] = t / A[i * nv + i];
+    }
+    free(Sd); free(A);
+    return 0;
+}
+
+int orc_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
