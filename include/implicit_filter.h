@@ -1,0 +1,136 @@
+/*
+ * implicit_filter.h -- C ABI of the B200-native implicit-filter hot path (arXiv 2404.07398).
+ *
+ * Citations: "PAPER.md:NN" = line NN of the paper text this library was written from.
+ *
+ * The paper splits the computation into a mesh-only preparation phase and a solving phase
+ * (PAPER.md:105).  This boundary follows that split:
+ *
+ *   if_prepare   once per mesh: P1 stiffness S (cotangent weights) and median-dual areas A_v
+ *                (PAPER.md:57-61), space-filling-curve reordering, SELL-C-sigma packing.
+ *   if_filter    coarse-grained fields  phibar_l  for many fields and scales l:
+ *                    (M + gamma l^(2n) S (M^-1 S)^(n-1)) phibar_l = M phi        (eq.(1), :61, :63)
+ *                M = diag(A_v), gamma = 1/2, n = 1 harmonic / n = 2 biharmonic,
+ *                solved by Jacobi-preconditioned conjugate gradients started from phi.
+ *   if_spectrum  the same solves followed by e_l = 1/2 sum_v A_v phibar_l,v^2 / sum_v A_v  ("second moment
+ *                of the field over scales") and its differences over k_l = 1/l.
+ *   if_apply     the operator alone: out = (M + gamma l^(2n) S (M^-1 S)^(n-1)) phi  (residual checks).
+ *
+ * Conventions
+ *   - fp64 everywhere; vertex ids int32; all multi-dimensional arrays are C-contiguous.
+ *   - Every argument says whether it is a HOST or a DEVICE pointer.  The caller owns every buffer it
+ *     passes (inputs, outputs, workspace); the handle owns the device arrays it built and if_destroy frees
+ *     them.  The library keeps no caller pointer past return and never frees or resizes caller memory.
+ *   - Inputs and outputs use the CALLER's vertex numbering; the internal reordering is invisible.
+ *   - Work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).  Calls that
+ *     return host outputs (if_spectrum, or any call given a non-NULL if_stats) synchronise that stream
+ *     before returning; if_filter/if_apply with stats == NULL return after the last poll of the
+ *     convergence flag (the output is complete in stream order).
+ *   - Return value: 0 on success; negative IF_E* on error (outputs untouched, nothing thrown);
+ *     positive IF_WNOTCONVERGED when some right-hand side hit max_iter or broke down -- an expected outcome
+ *     for n = 2 at large l; outputs then hold the last iterate and if_stats says which.
+ *   - A handle is read-only after if_prepare: concurrent calls on one handle are safe if their workspaces
+ *     and streams differ.  There is no CPU fallback: without a CUDA device every call fails with IF_ECUDA.
+ */
+#ifndef IMPLICIT_FILTER_H
+#define IMPLICIT_FILTER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct if_mesh_s* if_handle; /* opaque; owns all device-resident mesh arrays */
+
+enum {
+    IF_OK = 0,
+    IF_WNOTCONVERGED = 1, /* some right-hand side stopped on max_iter or breakdown                         */
+    IF_EINVAL = -1,       /* null pointer, dim not 2|3, order_n not 1|2, l <= 0 or non-finite, too few scales */
+    IF_EINDEX = -2,       /* triangle vertex id out of range, or a vertex repeated inside a triangle       */
+    IF_EDEGENERATE = -3,  /* triangle with |e1 x e2| <= 1e-14 (|e1|^2 + |e2|^2)                             */
+    IF_EORPHAN = -4,      /* vertex in no triangle: A_v = 0, M singular                                    */
+    IF_ENOMEM = -5,       /* host or device allocation failed                                              */
+    IF_ECUDA = -6,        /* CUDA runtime error, or no device                                              */
+    IF_EWORKSPACE = -7    /* workspace smaller than if_workspace_bytes says                                */
+};
+
+enum {
+    IF_FLAG_KEEP_CSR = 1 /* if_prepare keeps the unpermuted CSR of S so if_mesh_export_csr works */
+};
+
+typedef struct {
+    double gamma;    /* 0 => 0.5                                                              */
+    double tol;      /* 0 => 1e-12; stop when ||r||_2 <= tol ||M phi||_2 (recursive residual; PAPER.md:113
+                        uses 1e-9)                                                                           */
+    int max_iter;    /* 0 => 200000 iterations per right-hand side                                          */
+    int check_every; /* 0 => 16; iterations per CUDA-graph launch = between two polls of the done flag     */
+    int batch;       /* right-hand sides per SpMM: 4, 8 or 16; 0 => 16                                      */
+    int sell_c;      /* SELL chunk height C (rows sharing one padded width): multiple of 32; 0 => 32        */
+    int sell_sigma;  /* SELL sorting window sigma (rows): multiple of sell_c; 0 => 256; == sell_c: no sort  */
+    int sfc_kind;    /* 0 => Morton order of the quantised coordinates; 1 => keep the caller's order        */
+    int flags;       /* IF_FLAG_*                                                                           */
+} if_options;
+
+typedef struct {
+    int32_t* iters;     /* HOST [n_fields*n_ells] or NULL: CG iterations of each right-hand side (f*L + j)  */
+    double* rel_res;    /* HOST [n_fields*n_ells] or NULL: final recursive ||r||_2/||M phi||_2              */
+    int32_t* status;    /* HOST [n_fields*n_ells] or NULL: 0 converged, 1 max_iter, 2 breakdown (p.Ap <= 0) */
+    double seconds;     /* out: device time of the call (CUDA events on the stream)                         */
+    int64_t batch_iters; /* out: fused SpMM+CG iterations launched, summed over batches                      */
+    int64_t rhs_iters;   /* out: sum over right-hand sides of their iterations                               */
+} if_stats;
+
+/* Preparation phase.  All pointers HOST.
+ *   coords  [n_vert][dim] vertex positions, dim = 2 (planar) or 3 (surface in space; triangles are flat)
+ *   tri     [n_tri][3]    vertex ids, any orientation
+ *   period  [dim] or NULL; period[d] > 0 makes axis d periodic (edge vectors use the minimum image)
+ *   opt     NULL => defaults;   out: receives the handle (device-resident mesh; the current CUDA device)
+ * Boundary edges (one adjacent triangle) get the natural no-normal-flux condition. */
+int if_prepare(const double* coords, int dim, int64_t n_vert, const int32_t* tri, int64_t n_tri,
+               const double* period, const if_options* opt, if_handle* out);
+
+/* Bytes of DEVICE workspace if_filter / if_spectrum / if_apply need for this order and batch (0 => default). */
+int if_workspace_bytes(if_handle h, int order_n, int batch, size_t* bytes);
+
+/* Solving phase.  d_fields DEVICE [n_fields][n_vert]; ells HOST [n_ells] (> 0, coordinate units, any order);
+ * order_n 1|2; d_out DEVICE [n_fields][n_ells][n_vert]; d_workspace DEVICE, ws_bytes >= if_workspace_bytes;
+ * opt NULL => the options given to if_prepare; stats NULL or HOST. */
+int if_filter(if_handle h, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
+              double* d_out, void* d_workspace, size_t ws_bytes, void* cuda_stream, const if_options* opt,
+              if_stats* stats);
+
+/* As if_filter, but only the scale spectrum is returned (no field output).  n_ells >= 2, ells strictly
+ * ascending.  HOST outputs: energy [n_fields][n_ells] = e_l; k_mid [n_ells-1] = sqrt(k_j k_j+1), k_j = 1/l_j;
+ * E [n_fields][n_ells-1] = (e_j - e_j+1)/(k_j - k_j+1).  Any of the three may be NULL. */
+int if_spectrum(if_handle h, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
+                double* energy, double* k_mid, double* E, void* d_workspace, size_t ws_bytes,
+                void* cuda_stream, const if_options* opt, if_stats* stats);
+
+/* Operator only: d_out[f][j] = (M + gamma l_j^(2n) S (M^-1 S)^(n-1)) d_fields[f].  Same layouts as if_filter. */
+int if_apply(if_handle h, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
+             double* d_out, void* d_workspace, size_t ws_bytes, void* cuda_stream, const if_options* opt);
+
+/* Mesh facts (all HOST, any may be NULL): vertices, stored entries of S (diagonal included), sum of A_v,
+ * mean edge length, padded SELL slots (off-diagonal entries incl. padding). */
+int if_mesh_info(if_handle h, int64_t* n_vert, int64_t* nnz, double* total_area, double* mean_edge,
+                 int64_t* sell_slots);
+
+/* Copy S (CSR, caller's numbering, columns ascending, diagonal included) and A_v to HOST arrays:
+ * rowptr [n_vert+1], col [nnz], val [nnz], area [n_vert]; any may be NULL.  Needs IF_FLAG_KEEP_CSR
+ * (else IF_EINVAL).  For checking the preparation phase against another assembly. */
+int if_mesh_export_csr(if_handle h, int64_t* rowptr, int32_t* col, double* val, double* area);
+
+/* Internal ordering (HOST [n_vert], may be NULL): perm[new] = caller id of internal row `new`. */
+int if_mesh_export_perm(if_handle h, int32_t* perm);
+
+void if_destroy(if_handle h);
+const char* if_strerror(int code);
+/* Kernels launched by this library in the calling process so far (bench.py's gpu_launches). */
+int64_t if_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IMPLICIT_FILTER_H */

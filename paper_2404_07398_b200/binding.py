@@ -1,0 +1,299 @@
+"""Thin Python face of the C-ABI library (include/implicit_filter.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libimplicit_filter.so; PyTorch is used here for device
+memory (fields, outputs, workspace) and streams.  There is no CPU path: if the library has not been built
+(python -m paper_2404_07398_b200.build) or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libimplicit_filter.so")
+
+IF_OK, IF_WNOTCONVERGED = 0, 1
+IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKSPACE = -1, -2, -3, -4, -5, -6, -7
+IF_FLAG_KEEP_CSR = 1
+
+EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_apply", "if_mesh_info",
+           "if_mesh_export_csr", "if_mesh_export_perm", "if_destroy", "if_strerror", "if_launch_count")
+
+
+class if_options(C.Structure):
+    _fields_ = [("gamma", C.c_double), ("tol", C.c_double), ("max_iter", C.c_int), ("check_every", C.c_int),
+                ("batch", C.c_int), ("sell_c", C.c_int), ("sell_sigma", C.c_int), ("sfc_kind", C.c_int),
+                ("flags", C.c_int)]
+
+
+class if_stats(C.Structure):
+    _fields_ = [("iters", C.POINTER(C.c_int32)), ("rel_res", C.POINTER(C.c_double)),
+                ("status", C.POINTER(C.c_int32)), ("seconds", C.c_double), ("batch_iters", C.c_int64),
+                ("rhs_iters", C.c_int64)]
+
+
+class ImplicitFilterError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {strerror(code)} ({code})")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree library and declare its signatures.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2404_07398_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, i32, dp = C.c_void_p, C.c_int64, C.c_int, C.POINTER(C.c_double)
+    L.if_prepare.restype = i32
+    L.if_prepare.argtypes = [vp, i32, i64, vp, i64, vp, C.POINTER(if_options), C.POINTER(vp)]
+    L.if_workspace_bytes.restype = i32
+    L.if_workspace_bytes.argtypes = [vp, i32, i32, C.POINTER(C.c_size_t)]
+    L.if_filter.restype = i32
+    L.if_filter.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, C.c_size_t, vp, C.POINTER(if_options),
+                            C.POINTER(if_stats)]
+    L.if_spectrum.restype = i32
+    L.if_spectrum.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, vp, vp, C.c_size_t, vp, C.POINTER(if_options),
+                              C.POINTER(if_stats)]
+    L.if_apply.restype = i32
+    L.if_apply.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, C.c_size_t, vp, C.POINTER(if_options)]
+    L.if_mesh_info.restype = i32
+    L.if_mesh_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), dp, dp, C.POINTER(i64)]
+    L.if_mesh_export_csr.restype = i32
+    L.if_mesh_export_csr.argtypes = [vp, vp, vp, vp, vp]
+    L.if_mesh_export_perm.restype = i32
+    L.if_mesh_export_perm.argtypes = [vp, vp]
+    L.if_destroy.restype = None
+    L.if_destroy.argtypes = [vp]
+    L.if_strerror.restype = C.c_char_p
+    L.if_strerror.argtypes = [i32]
+    L.if_launch_count.restype = i64
+    L.if_launch_count.argtypes = []
+    _lib = L
+    return L
+
+
+def strerror(code: int) -> str:
+    return load_library().if_strerror(int(code)).decode()
+
+
+def if_launch_count() -> int:
+    return int(load_library().if_launch_count())
+
+
+def _options(**kw) -> Optional[if_options]:
+    kw = {k: v for k, v in kw.items() if v is not None}
+    if not kw:
+        return None
+    o = if_options()
+    for k, v in kw.items():
+        if not hasattr(o, k):
+            raise TypeError(f"unknown option {k!r}")
+        setattr(o, k, v)
+    return o
+
+
+def _np_ptr(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class Handle:
+    """Owns an if_handle (device-resident prepared mesh) plus a side stream and a cached workspace."""
+
+    def __init__(self, ptr: int, device):
+        import torch
+        self._ptr = C.c_void_p(ptr)
+        self.device = device
+        self.stream = torch.cuda.Stream(device=device)
+        self._ws = None
+        nv, nnz, slots = C.c_int64(), C.c_int64(), C.c_int64()
+        ta, me = C.c_double(), C.c_double()
+        load_library().if_mesh_info(self._ptr, C.byref(nv), C.byref(nnz), C.byref(ta), C.byref(me), C.byref(slots))
+        self.n_vert, self.nnz, self.sell_slots = int(nv.value), int(nnz.value), int(slots.value)
+        self.total_area, self.mean_edge = float(ta.value), float(me.value)
+
+    def close(self):
+        if self._ptr is not None and self._ptr.value:
+            load_library().if_destroy(self._ptr)
+        self._ptr = None
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def workspace(self, order_n: int, batch: int = 0):
+        import torch
+        need = if_workspace_bytes(self, order_n, batch)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=self.device)
+        return self._ws
+
+
+def if_prepare(coords, tri, period=None, **options) -> Handle:
+    """Preparation phase: host arrays coords [V][dim] float64, tri [T][3] int32, period [dim] or None."""
+    import torch
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise ImplicitFilterError(IF_ECUDA, "if_prepare (no CUDA device; there is no CPU fallback)")
+    coords = np.ascontiguousarray(coords, dtype=np.float64)
+    tri = np.ascontiguousarray(tri, dtype=np.int32)
+    if coords.ndim != 2 or tri.ndim != 2 or tri.shape[1] != 3:
+        raise ValueError("coords must be [V][dim], tri [T][3]")
+    per = None if period is None else np.ascontiguousarray(period, dtype=np.float64)
+    opt = _options(**options)
+    out = C.c_void_p()
+    device = torch.device("cuda", torch.cuda.current_device())
+    torch.cuda.init()
+    torch.zeros(1, device=device)      # make sure the primary context exists
+    rc = L.if_prepare(_np_ptr(coords), coords.shape[1], coords.shape[0], _np_ptr(tri), tri.shape[0],
+                      None if per is None else _np_ptr(per), None if opt is None else C.byref(opt), C.byref(out))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_prepare")
+    return Handle(out.value, device)
+
+
+def if_workspace_bytes(h: Handle, order_n: int, batch: int = 0) -> int:
+    n = C.c_size_t()
+    rc = load_library().if_workspace_bytes(h._ptr, int(order_n), int(batch), C.byref(n))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_workspace_bytes")
+    return int(n.value)
+
+
+def _device_fields(h: Handle, fields):
+    import torch
+    t = fields if isinstance(fields, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(fields, dtype=np.float64))
+    if t.dim() == 1:
+        t = t[None, :]
+    t = t.to(device=h.device, dtype=torch.float64).contiguous()
+    if t.shape[1] != h.n_vert:
+        raise ValueError(f"fields must be [F][{h.n_vert}]")
+    return t
+
+
+class _Stats:
+    def __init__(self, n_rhs: int, shape):
+        self.iters = np.zeros(n_rhs, dtype=np.int32)
+        self.rel_res = np.zeros(n_rhs, dtype=np.float64)
+        self.status = np.zeros(n_rhs, dtype=np.int32)
+        self.shape = shape
+        self.c = if_stats(self.iters.ctypes.data_as(C.POINTER(C.c_int32)),
+                          self.rel_res.ctypes.data_as(C.POINTER(C.c_double)),
+                          self.status.ctypes.data_as(C.POINTER(C.c_int32)), 0.0, 0, 0)
+
+    def as_dict(self, rc: int):
+        return {"iters": self.iters.reshape(self.shape), "rel_res": self.rel_res.reshape(self.shape),
+                "status": self.status.reshape(self.shape), "seconds": float(self.c.seconds),
+                "batch_iters": int(self.c.batch_iters), "rhs_iters": int(self.c.rhs_iters), "code": int(rc)}
+
+
+def _run(h: Handle, what: str, call, stream):
+    """Run `call(stream_ptr)` on the handle's side stream (ordered after the caller's current stream)."""
+    import torch
+    cur = torch.cuda.current_stream(h.device)
+    st = h.stream if stream is None else stream
+    st.wait_stream(cur)
+    rc = call(C.c_void_p(st.cuda_stream))
+    cur.wait_stream(st)
+    if rc < 0:
+        raise ImplicitFilterError(rc, what)
+    return rc
+
+
+def if_filter(h: Handle, fields, ells: Sequence[float], order_n: int, out=None, workspace=None, stream=None,
+              **options):
+    """Filtered fields [F][L][V] (torch.float64 on the device, caller's vertex order) and a stats dict."""
+    import torch
+    L = load_library()
+    f = _device_fields(h, fields)
+    el = np.ascontiguousarray(ells, dtype=np.float64)
+    if out is None:
+        out = torch.empty((f.shape[0], el.shape[0], h.n_vert), dtype=torch.float64, device=h.device)
+    opt = _options(**options)
+    ws = h.workspace(order_n, options.get("batch") or 0) if workspace is None else workspace
+    st = _Stats(f.shape[0] * el.shape[0], (f.shape[0], el.shape[0]))
+    rc = _run(h, "if_filter", lambda s: L.if_filter(
+        h._ptr, C.c_void_p(f.data_ptr()), f.shape[0], _np_ptr(el), el.shape[0], int(order_n),
+        C.c_void_p(out.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), s,
+        None if opt is None else C.byref(opt), C.byref(st.c)), stream)
+    return out, st.as_dict(rc)
+
+
+def if_spectrum(h: Handle, fields, ells: Sequence[float], order_n: int, workspace=None, stream=None, **options):
+    """dict(energy [F][L], k_mid [L-1], E [F][L-1], stats) -- host numpy arrays."""
+    L = load_library()
+    f = _device_fields(h, fields)
+    el = np.ascontiguousarray(ells, dtype=np.float64)
+    Fn, Ln = f.shape[0], el.shape[0]
+    energy = np.zeros((Fn, Ln), dtype=np.float64)
+    k_mid = np.zeros(max(Ln - 1, 0), dtype=np.float64)
+    E = np.zeros((Fn, max(Ln - 1, 0)), dtype=np.float64)
+    opt = _options(**options)
+    ws = h.workspace(order_n, options.get("batch") or 0) if workspace is None else workspace
+    st = _Stats(Fn * Ln, (Fn, Ln))
+    rc = _run(h, "if_spectrum", lambda s: L.if_spectrum(
+        h._ptr, C.c_void_p(f.data_ptr()), Fn, _np_ptr(el), Ln, int(order_n), _np_ptr(energy), _np_ptr(k_mid),
+        _np_ptr(E), C.c_void_p(ws.data_ptr()), ws.numel(), s, None if opt is None else C.byref(opt),
+        C.byref(st.c)), stream)
+    return {"energy": energy, "k_mid": k_mid, "E": E, "stats": st.as_dict(rc)}
+
+
+def if_apply(h: Handle, fields, ells: Sequence[float], order_n: int, out=None, workspace=None, stream=None,
+             **options):
+    """out[f][j] = (M + gamma l_j^(2n) S (M^-1 S)^(n-1)) fields[f]  -> torch.float64 [F][L][V] on the device."""
+    import torch
+    L = load_library()
+    f = _device_fields(h, fields)
+    el = np.ascontiguousarray(ells, dtype=np.float64)
+    if out is None:
+        out = torch.empty((f.shape[0], el.shape[0], h.n_vert), dtype=torch.float64, device=h.device)
+    opt = _options(**options)
+    ws = h.workspace(order_n, options.get("batch") or 0) if workspace is None else workspace
+    _run(h, "if_apply", lambda s: L.if_apply(
+        h._ptr, C.c_void_p(f.data_ptr()), f.shape[0], _np_ptr(el), el.shape[0], int(order_n),
+        C.c_void_p(out.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), s,
+        None if opt is None else C.byref(opt)), stream)
+    return out
+
+
+def if_mesh_export_csr(h: Handle):
+    """(rowptr int64 [V+1], col int32 [nnz], val float64 [nnz], area float64 [V]) -- needs IF_FLAG_KEEP_CSR."""
+    rowptr = np.empty(h.n_vert + 1, dtype=np.int64)
+    col = np.empty(h.nnz, dtype=np.int32)
+    val = np.empty(h.nnz, dtype=np.float64)
+    area = np.empty(h.n_vert, dtype=np.float64)
+    rc = load_library().if_mesh_export_csr(h._ptr, _np_ptr(rowptr), _np_ptr(col), _np_ptr(val), _np_ptr(area))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_mesh_export_csr")
+    return rowptr, col, val, area
+
+
+def if_mesh_export_perm(h: Handle) -> np.ndarray:
+    perm = np.empty(h.n_vert, dtype=np.int32)
+    rc = load_library().if_mesh_export_perm(h._ptr, _np_ptr(perm))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_mesh_export_perm")
+    return perm
+
+
+def if_destroy(h: Handle) -> None:
+    h.close()

@@ -1,0 +1,83 @@
+// Shared declarations of the implicit-filter CUDA library (sm_100a).  See include/implicit_filter.h
+// for the C ABI and DESIGN.md for the data layout.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include <atomic>
+
+#include "implicit_filter.h"
+
+namespace ifl {
+
+extern std::atomic<long long> g_launches;   // kernels launched by this library (if_launch_count)
+
+#define IF_CUDA_TRY(expr)                                                                          \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            fprintf(stderr, "[implicit_filter] CUDA error %s at %s:%d: %s\n", cudaGetErrorName(e__), \
+                    __FILE__, __LINE__, cudaGetErrorString(e__));                                  \
+            return e__ == cudaErrorMemoryAllocation ? IF_ENOMEM : IF_ECUDA;                        \
+        }                                                                                          \
+    } while (0)
+
+#define IF_LAUNCH_CHECK()                        \
+    do {                                         \
+        ++::ifl::g_launches;                     \
+        IF_CUDA_TRY(cudaGetLastError());         \
+    } while (0)
+
+// Resolved options (defaults filled in).
+struct Options {
+    double gamma = 0.5;
+    double tol = 1e-12;
+    int max_iter = 200000;
+    int check_every = 16;
+    int batch = 16;
+    int sell_c = 32;
+    int sell_sigma = 256;
+    int sfc_kind = 0;
+    int flags = 0;
+};
+
+int resolve_options(const if_options* in, const Options* base, Options* out);
+
+}  // namespace ifl
+
+// Device-resident prepared mesh.  Rows are in the internal order (SFC + SELL window sort):
+// internal row r is caller vertex perm[r]; iperm[perm[r]] = r.
+struct if_mesh_s {
+    int device = 0;
+    int64_t n_vert = 0;
+    int64_t nnz = 0;          // entries of S incl. diagonal
+    int64_t n_chunks = 0;     // ceil(n_vert / sell_c)
+    int64_t sell_slots = 0;   // padded off-diagonal slots
+    int sell_c = 32;
+    double total_area = 0.0;
+    double mean_edge = 0.0;
+    int n_sm = 148;
+    ifl::Options opt;
+    // SELL-C-sigma, off-diagonal entries only; slice c holds rows [c*C, (c+1)*C), row-major [row][width_c],
+    // width_c even, padding = (col = own row, val = 0).
+    int64_t* chunk_ptr = nullptr;   // [n_chunks+1] slot offsets (even)
+    int32_t* sell_col = nullptr;    // [sell_slots] internal column ids
+    double* sell_val = nullptr;     // [sell_slots]
+    double* area = nullptr;         // [n_vert] A_v            (internal order)
+    double* inv_area = nullptr;     // [n_vert] 1/A_v
+    double* sdiag = nullptr;        // [n_vert] S_vv
+    double* gdiag = nullptr;        // [n_vert] sum_j S_vj^2/A_j = diag(S M^-1 S)
+    int32_t* perm = nullptr;        // [n_vert] internal -> caller
+    int32_t* iperm = nullptr;       // [n_vert] caller -> internal
+    // optional unpermuted CSR (IF_FLAG_KEEP_CSR), caller numbering
+    int64_t* csr_rowptr = nullptr;
+    int32_t* csr_col = nullptr;
+    double* csr_val = nullptr;
+    double* csr_area = nullptr;
+    // pinned host staging for per-call control data and read-back
+    void* h_pinned = nullptr;
+    size_t h_pinned_bytes = 0;
+    std::atomic<int> pinned_busy{0};   // 1 while a solve call uses h_pinned (others allocate their own)
+};

@@ -1,0 +1,581 @@
+// Preparation phase: mesh -> device-resident S (SELL-C-sigma), A_v and diagonals.
+//
+//   P1  triangle geometry: edge vectors (minimum image on periodic axes), |e1 x e2|, cotangents
+//       S_ab += -1/2 cot(angle opposite ab)   = integral grad N_a . grad N_b dS
+//   P2  half-edge assembly: 6 directed off-diagonal contributions + 3 area contributions per triangle,
+//       radix-sorted by (row, col) and summed by key; edges seen by one triangle only (boundary) keep the
+//       single contribution = natural no-normal-flux condition; S_vv = -sum_j S_vj
+//   P3  A_v = sum over triangles of area/3 (median-dual = lumped P1 mass, PAPER.md:41 Fig. 1a, :61)
+//   P4  Morton order of the quantised coordinates (space-filling curve) -> perm
+//   P5  SELL-C-sigma: rows sorted by length inside windows of sigma rows, slices of C rows padded to the
+//       slice maximum (rounded up to even so int2/double2 loads stay aligned), row-major inside a slice
+//   P6  Jacobi ingredients S_vv and g_v = sum_j S_vj^2/A_j = diag(S M^-1 S)
+#include <cub/cub.cuh>
+
+#include <cmath>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+namespace ifl {
+
+std::atomic<long long> g_launches{0};
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) {
+        if (p) { cudaFree(p); p = nullptr; }
+        return cudaMalloc(&p, bytes ? bytes : 1);
+    }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+    void* release() { void* q = p; p = nullptr; return q; }
+};
+
+enum { FLAG_INDEX = 1, FLAG_DEGENERATE = 2, FLAG_ORPHAN = 4 };
+
+struct Period { double p[3]; };
+
+__device__ inline void edge_vec(const double* __restrict__ coords, int dim, const Period& per, int64_t from,
+                                int64_t to, double e[3]) {
+    e[0] = e[1] = e[2] = 0.0;
+    for (int d = 0; d < dim; ++d) {
+        double v = coords[to * dim + d] - coords[from * dim + d];
+        if (per.p[d] > 0.0) v -= per.p[d] * rint(v / per.p[d]);
+        e[d] = v;
+    }
+}
+
+// P1 + P2 (emit): 9 keyed contributions per triangle.
+__global__ void k_tri_emit(const double* __restrict__ coords, int dim, int64_t nv, const int32_t* __restrict__ tri,
+                           int64_t nt, Period per, unsigned long long* __restrict__ keys, double* __restrict__ vals,
+                           int* __restrict__ flags) {
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nt) return;
+    int64_t v[3] = {tri[3 * t], tri[3 * t + 1], tri[3 * t + 2]};
+    int64_t base = 9 * t;
+    bool bad = false;
+    for (int c = 0; c < 3; ++c) bad |= (v[c] < 0 || v[c] >= nv);
+    bad |= (v[0] == v[1] || v[0] == v[2] || v[1] == v[2]);
+    if (bad) {
+        atomicOr(flags, FLAG_INDEX);
+        for (int i = 0; i < 9; ++i) { keys[base + i] = 0ull; vals[base + i] = 0.0; }
+        return;
+    }
+    double tarea = 0.0;
+    for (int c = 0; c < 3; ++c) {
+        int64_t vc = v[c], va = v[(c + 1) % 3], vb = v[(c + 2) % 3];
+        double e1[3], e2[3];
+        edge_vec(coords, dim, per, vc, va, e1);
+        edge_vec(coords, dim, per, vc, vb, e2);
+        double cx = e1[1] * e2[2] - e1[2] * e2[1];
+        double cy = e1[2] * e2[0] - e1[0] * e2[2];
+        double cz = e1[0] * e2[1] - e1[1] * e2[0];
+        double cr = sqrt(cx * cx + cy * cy + cz * cz);
+        double dt = e1[0] * e2[0] + e1[1] * e2[1] + e1[2] * e2[2];
+        double n1 = e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2];
+        double n2 = e2[0] * e2[0] + e2[1] * e2[1] + e2[2] * e2[2];
+        if (!(cr > 1e-14 * (n1 + n2))) { atomicOr(flags, FLAG_DEGENERATE); cr = 1.0; }
+        double w = -0.5 * dt / cr;
+        keys[base + 2 * c] = ((unsigned long long)va << 32) | (unsigned long long)vb;
+        vals[base + 2 * c] = w;
+        keys[base + 2 * c + 1] = ((unsigned long long)vb << 32) | (unsigned long long)va;
+        vals[base + 2 * c + 1] = w;
+        if (c == 0) tarea = 0.5 * cr;
+    }
+    for (int c = 0; c < 3; ++c) {
+        keys[base + 6 + c] = ((unsigned long long)v[c] << 32) | (unsigned long long)v[c];
+        vals[base + 6 + c] = tarea / 3.0;
+    }
+}
+
+// rowptr[r] = first unique entry whose row >= r.
+__global__ void k_rowptr(const unsigned long long* __restrict__ ukeys, int64_t nnz, int64_t nv,
+                         int64_t* __restrict__ rowptr) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > nnz) return;
+    int64_t row_i = i < nnz ? (int64_t)(ukeys[i] >> 32) : nv;
+    int64_t row_p = i > 0 ? (int64_t)(ukeys[i - 1] >> 32) : -1;
+    for (int64_t r = row_p + 1; r <= row_i; ++r) rowptr[r] = i;
+}
+
+// Per caller row: the keyed sum at (v,v) is A_v; replace it by S_vv = -sum of off-diagonals.
+__global__ void k_row_finish(const unsigned long long* __restrict__ ukeys, const int64_t* __restrict__ rowptr,
+                             int64_t nv, double* __restrict__ val, int32_t* __restrict__ col,
+                             double* __restrict__ area, double* __restrict__ sdiag, int32_t* __restrict__ len,
+                             int* __restrict__ flags) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nv) return;
+    int64_t b = rowptr[v], e = rowptr[v + 1];
+    double off = 0.0, a = 0.0;
+    int64_t dpos = -1;
+    for (int64_t i = b; i < e; ++i) {
+        int32_t c = (int32_t)(ukeys[i] & 0xffffffffull);
+        col[i] = c;
+        if (c == v) { dpos = i; a = val[i]; } else off += val[i];
+    }
+    if (dpos < 0 || !(a > 0.0)) { atomicOr(flags, FLAG_ORPHAN); area[v] = 1.0; sdiag[v] = 0.0; len[v] = 0; return; }
+    val[dpos] = -off;
+    area[v] = a;
+    sdiag[v] = -off;
+    len[v] = (int32_t)(e - b - 1);
+}
+
+__global__ void k_gdiag(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                        const double* __restrict__ val, const double* __restrict__ area, int64_t nv,
+                        double* __restrict__ gdiag) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nv) return;
+    double g = 0.0;
+    for (int64_t i = rowptr[v]; i < rowptr[v + 1]; ++i) g += val[i] * val[i] / area[col[i]];
+    gdiag[v] = g;
+}
+
+// length of each edge once (row < col), 0 elsewhere
+__global__ void k_edge_len(const double* __restrict__ coords, int dim, Period per, const int64_t* __restrict__ rowptr,
+                           const int32_t* __restrict__ col, int64_t nv, double* __restrict__ out) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nv) return;
+    for (int64_t i = rowptr[v]; i < rowptr[v + 1]; ++i) {
+        double l = 0.0;
+        if (col[i] > v) {
+            double e[3];
+            edge_vec(coords, dim, per, v, col[i], e);
+            l = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+        }
+        out[i] = l;
+    }
+}
+
+__device__ inline unsigned long long spread3(unsigned long long x) {   // 21 bits -> every third bit
+    x &= 0x1fffffull;
+    x = (x | x << 32) & 0x1f00000000ffffull;
+    x = (x | x << 16) & 0x1f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+__device__ inline unsigned long long spread2(unsigned long long x) {   // 31 bits -> every second bit
+    x &= 0x7fffffffull;
+    x = (x | x << 16) & 0x0000ffff0000ffffull;
+    x = (x | x << 8) & 0x00ff00ff00ff00ffull;
+    x = (x | x << 4) & 0x0f0f0f0f0f0f0f0full;
+    x = (x | x << 2) & 0x3333333333333333ull;
+    x = (x | x << 1) & 0x5555555555555555ull;
+    return x;
+}
+
+struct Box { double lo[3]; double scale[3]; };
+
+__global__ void k_morton(const double* __restrict__ coords, int dim, int64_t nv, Box box,
+                         unsigned long long* __restrict__ keys, int32_t* __restrict__ ids, int identity) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nv) return;
+    ids[v] = (int32_t)v;
+    if (identity) { keys[v] = (unsigned long long)v; return; }
+    unsigned long long q[3] = {0, 0, 0};
+    const double top = dim == 3 ? 2097151.0 : 2147483647.0;
+    for (int d = 0; d < dim; ++d) {
+        double s = (coords[v * dim + d] - box.lo[d]) * box.scale[d] * top;
+        s = fmin(fmax(s, 0.0), top);
+        q[d] = (unsigned long long)s;
+    }
+    keys[v] = dim == 3 ? (spread3(q[0]) | spread3(q[1]) << 1 | spread3(q[2]) << 2)
+                       : (spread2(q[0]) | spread2(q[1]) << 1);
+}
+
+// sigma-window key: rows of one window sorted by descending length (stable)
+__global__ void k_sigma_key(const int32_t* __restrict__ order0, const int32_t* __restrict__ len, int64_t nv,
+                            int sigma, unsigned long long* __restrict__ keys) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= nv) return;
+    int l = len[order0[r]];
+    l = l > 255 ? 255 : l;
+    keys[r] = ((unsigned long long)(r / sigma) << 8) | (unsigned long long)(255 - l);
+}
+
+__global__ void k_invert_perm(const int32_t* __restrict__ perm, int64_t nv, int32_t* __restrict__ iperm) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < nv) iperm[perm[r]] = (int32_t)r;
+}
+
+// slots of slice c = C * even(max row length in the slice)
+__global__ void k_chunk_slots(const int32_t* __restrict__ perm, const int32_t* __restrict__ len, int64_t nv,
+                              int64_t n_chunks, int C, int64_t* __restrict__ slots) {
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c > n_chunks) return;
+    if (c == n_chunks) { slots[c] = 0; return; }
+    int w = 0;
+    for (int i = 0; i < C; ++i) {
+        int64_t r = c * C + i;
+        if (r < nv) w = max(w, len[perm[r]]);
+    }
+    w = (w + 1) & ~1;
+    slots[c] = (int64_t)w * C;
+}
+
+__global__ void k_sell_fill(const int32_t* __restrict__ perm, const int32_t* __restrict__ iperm,
+                            const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                            const double* __restrict__ val, const double* __restrict__ area_u,
+                            const double* __restrict__ sdiag_u, const double* __restrict__ gdiag_u, int64_t nv,
+                            int64_t n_chunks, int C, const int64_t* __restrict__ chunk_ptr,
+                            int32_t* __restrict__ sell_col, double* __restrict__ sell_val, double* __restrict__ area,
+                            double* __restrict__ inv_area, double* __restrict__ sdiag, double* __restrict__ gdiag) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_chunks * C) return;
+    int64_t c = r / C;
+    int64_t w = (chunk_ptr[c + 1] - chunk_ptr[c]) / C;
+    int64_t o = chunk_ptr[c] + (r - c * C) * w;
+    int64_t k = 0;
+    int32_t self = (int32_t)(r < nv ? r : nv - 1);
+    if (r < nv) {
+        int64_t u = perm[r];
+        for (int64_t i = rowptr[u]; i < rowptr[u + 1]; ++i) {
+            if (col[i] == u) continue;
+            sell_col[o + k] = iperm[col[i]];
+            sell_val[o + k] = val[i];
+            ++k;
+        }
+        area[r] = area_u[u];
+        inv_area[r] = 1.0 / area_u[u];
+        sdiag[r] = sdiag_u[u];
+        gdiag[r] = gdiag_u[u];
+    }
+    for (; k < w; ++k) { sell_col[o + k] = self; sell_val[o + k] = 0.0; }
+}
+
+inline unsigned grid_for(int64_t n, int block = 256) { return (unsigned)((n + block - 1) / block); }
+inline int bits_for(uint64_t n) { int b = 1; while ((1ull << b) < n && b < 63) ++b; return b; }
+
+}  // namespace
+
+int resolve_options(const if_options* in, const Options* base, Options* out) {
+    Options o = base ? *base : Options();
+    if (in) {
+        if (in->gamma != 0.0) o.gamma = in->gamma;
+        if (in->tol != 0.0) o.tol = in->tol;
+        if (in->max_iter != 0) o.max_iter = in->max_iter;
+        if (in->check_every != 0) o.check_every = in->check_every;
+        if (in->batch != 0) o.batch = in->batch;
+        if (!base) {   // mesh-layout options are fixed at if_prepare
+            if (in->sell_c != 0) o.sell_c = in->sell_c;
+            if (in->sell_sigma != 0) o.sell_sigma = in->sell_sigma;
+            o.sfc_kind = in->sfc_kind;
+            o.flags = in->flags;
+        }
+    }
+    if (!(o.gamma > 0.0) || !std::isfinite(o.gamma) || !(o.tol > 0.0) || !std::isfinite(o.tol)) return IF_EINVAL;
+    if (o.max_iter < 1 || o.check_every < 1) return IF_EINVAL;
+    if (o.batch != 4 && o.batch != 8 && o.batch != 16) return IF_EINVAL;
+    if (o.sell_c < 32 || o.sell_c % 32 != 0 || o.sell_c > 1024) return IF_EINVAL;
+    if (o.sell_sigma < o.sell_c || o.sell_sigma % o.sell_c != 0) return IF_EINVAL;
+    if (o.sfc_kind != 0 && o.sfc_kind != 1) return IF_EINVAL;
+    o.check_every = (o.check_every + 1) & ~1;   // even: the search direction is double-buffered
+    *out = o;
+    return IF_OK;
+}
+
+}  // namespace ifl
+
+using namespace ifl;
+
+extern "C" void if_destroy(if_handle h) {
+    if (!h) return;
+    int prev = 0;
+    cudaGetDevice(&prev);
+    cudaSetDevice(h->device);
+    cudaFree(h->chunk_ptr); cudaFree(h->sell_col); cudaFree(h->sell_val); cudaFree(h->area);
+    cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->perm); cudaFree(h->iperm);
+    cudaFree(h->csr_rowptr); cudaFree(h->csr_col); cudaFree(h->csr_val); cudaFree(h->csr_area);
+    if (h->h_pinned) cudaFreeHost(h->h_pinned);
+    cudaSetDevice(prev);
+    delete h;
+}
+
+static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t* tri, int64_t nt,
+                        const double* period, const Options& opt, if_mesh_s* h) {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return IF_ECUDA;
+    IF_CUDA_TRY(cudaGetDevice(&h->device));
+    IF_CUDA_TRY(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
+    h->n_vert = nv;
+    h->opt = opt;
+    h->sell_c = opt.sell_c;
+    cudaStream_t st = 0;
+
+    Period per{{0.0, 0.0, 0.0}};
+    if (period)
+        for (int d = 0; d < dim; ++d) {
+            if (!(period[d] >= 0.0) || !std::isfinite(period[d])) return IF_EINVAL;
+            per.p[d] = period[d];
+        }
+    // bounding box for the space-filling curve (host pass over the caller's coordinates)
+    Box box;
+    for (int d = 0; d < 3; ++d) { box.lo[d] = 0.0; box.scale[d] = 0.0; }
+    {
+        double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+        for (int64_t v = 0; v < nv; ++v)
+            for (int d = 0; d < dim; ++d) {
+                double x = coords[v * dim + d];
+                if (!std::isfinite(x)) return IF_EINVAL;
+                lo[d] = x < lo[d] ? x : lo[d];
+                hi[d] = x > hi[d] ? x : hi[d];
+            }
+        double ext = 0.0;
+        for (int d = 0; d < dim; ++d) ext = hi[d] - lo[d] > ext ? hi[d] - lo[d] : ext;
+        for (int d = 0; d < dim; ++d) { box.lo[d] = lo[d]; box.scale[d] = ext > 0.0 ? 1.0 / ext : 0.0; }
+    }
+
+    DevBuf d_coords, d_tri, d_flags;
+    IF_CUDA_TRY(d_coords.alloc((size_t)nv * dim * sizeof(double)));
+    IF_CUDA_TRY(d_tri.alloc((size_t)nt * 3 * sizeof(int32_t)));
+    IF_CUDA_TRY(d_flags.alloc(sizeof(int)));
+    IF_CUDA_TRY(cudaMemcpyAsync(d_coords.p, coords, (size_t)nv * dim * sizeof(double), cudaMemcpyHostToDevice, st));
+    IF_CUDA_TRY(cudaMemcpyAsync(d_tri.p, tri, (size_t)nt * 3 * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    IF_CUDA_TRY(cudaMemsetAsync(d_flags.p, 0, sizeof(int), st));
+
+    // ---- P1/P2: emit, sort by (row, col), sum by key
+    const int64_t n_emit = 9 * nt;
+    DevBuf k0, k1, v0, v1, tmp, d_nruns;
+    IF_CUDA_TRY(k0.alloc((size_t)n_emit * 8));
+    IF_CUDA_TRY(k1.alloc((size_t)n_emit * 8));
+    IF_CUDA_TRY(v0.alloc((size_t)n_emit * 8));
+    IF_CUDA_TRY(v1.alloc((size_t)n_emit * 8));
+    IF_CUDA_TRY(d_nruns.alloc(sizeof(int64_t)));
+    k_tri_emit<<<grid_for(nt), 256, 0, st>>>(d_coords.as<double>(), dim, nv, d_tri.as<int32_t>(), nt, per,
+                                            k0.as<unsigned long long>(), v0.as<double>(), d_flags.as<int>());
+    IF_LAUNCH_CHECK();
+    int flags = 0;
+    IF_CUDA_TRY(cudaMemcpyAsync(&flags, d_flags.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    if (flags & FLAG_INDEX) return IF_EINDEX;
+    if (flags & FLAG_DEGENERATE) return IF_EDEGENERATE;
+
+    const int key_bits = 32 + bits_for((uint64_t)nv);
+    size_t tb = 0;
+    IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tb, k0.as<unsigned long long>(), k1.as<unsigned long long>(),
+                                                v0.as<double>(), v1.as<double>(), n_emit, 0, key_bits, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tb, k0.as<unsigned long long>(), k1.as<unsigned long long>(),
+                                                v0.as<double>(), v1.as<double>(), n_emit, 0, key_bits, st));
+    ++g_launches;
+    tb = 0;
+    IF_CUDA_TRY(cub::DeviceReduce::ReduceByKey(nullptr, tb, k1.as<unsigned long long>(), k0.as<unsigned long long>(),
+                                               v1.as<double>(), v0.as<double>(), d_nruns.as<int64_t>(), cub::Sum(),
+                                               n_emit, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceReduce::ReduceByKey(tmp.p, tb, k1.as<unsigned long long>(), k0.as<unsigned long long>(),
+                                               v1.as<double>(), v0.as<double>(), d_nruns.as<int64_t>(), cub::Sum(),
+                                               n_emit, st));
+    ++g_launches;
+    int64_t nnz = 0;
+    IF_CUDA_TRY(cudaMemcpyAsync(&nnz, d_nruns.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    h->nnz = nnz;
+    k1.alloc(0); v1.alloc(0);   // sorted copies no longer needed
+    // now: k0 = unique keys [nnz], v0 = summed values [nnz]
+
+    // ---- CSR in the caller's numbering, A_v, S_vv, g_v
+    DevBuf rowptr, ccol, area_u, sdiag_u, gdiag_u, len;
+    IF_CUDA_TRY(rowptr.alloc((size_t)(nv + 1) * sizeof(int64_t)));
+    IF_CUDA_TRY(ccol.alloc((size_t)nnz * sizeof(int32_t)));
+    IF_CUDA_TRY(area_u.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(sdiag_u.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(gdiag_u.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(len.alloc((size_t)nv * 4));
+    k_rowptr<<<grid_for(nnz + 1), 256, 0, st>>>(k0.as<unsigned long long>(), nnz, nv, rowptr.as<int64_t>());
+    IF_LAUNCH_CHECK();
+    k_row_finish<<<grid_for(nv), 256, 0, st>>>(k0.as<unsigned long long>(), rowptr.as<int64_t>(), nv, v0.as<double>(),
+                                              ccol.as<int32_t>(), area_u.as<double>(), sdiag_u.as<double>(),
+                                              len.as<int32_t>(), d_flags.as<int>());
+    IF_LAUNCH_CHECK();
+    IF_CUDA_TRY(cudaMemcpyAsync(&flags, d_flags.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    if (flags & FLAG_ORPHAN) return IF_EORPHAN;
+    k_gdiag<<<grid_for(nv), 256, 0, st>>>(rowptr.as<int64_t>(), ccol.as<int32_t>(), v0.as<double>(),
+                                         area_u.as<double>(), nv, gdiag_u.as<double>());
+    IF_LAUNCH_CHECK();
+
+    // total area and mean edge length (deterministic device reductions)
+    {
+        DevBuf d_sum, elen;
+        IF_CUDA_TRY(d_sum.alloc(2 * sizeof(double)));
+        IF_CUDA_TRY(elen.alloc((size_t)nnz * 8));
+        k_edge_len<<<grid_for(nv), 256, 0, st>>>(d_coords.as<double>(), dim, per, rowptr.as<int64_t>(),
+                                                ccol.as<int32_t>(), nv, elen.as<double>());
+        IF_LAUNCH_CHECK();
+        tb = 0;
+        IF_CUDA_TRY(cub::DeviceReduce::Sum(nullptr, tb, elen.as<double>(), d_sum.as<double>(), nnz, st));
+        IF_CUDA_TRY(tmp.alloc(tb));
+        IF_CUDA_TRY(cub::DeviceReduce::Sum(tmp.p, tb, area_u.as<double>(), d_sum.as<double>(), nv, st));
+        IF_CUDA_TRY(cub::DeviceReduce::Sum(tmp.p, tb, elen.as<double>(), d_sum.as<double>() + 1, nnz, st));
+        g_launches += 2;
+        double s[2] = {0.0, 0.0};
+        IF_CUDA_TRY(cudaMemcpyAsync(s, d_sum.p, sizeof(s), cudaMemcpyDeviceToHost, st));
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        h->total_area = s[0];
+        int64_t n_edges = (nnz - nv) / 2;
+        h->mean_edge = n_edges > 0 ? s[1] / (double)n_edges : 0.0;
+    }
+
+    // ---- P4: space-filling-curve order; P5: sigma-window sort by row length
+    DevBuf mk0, mk1, id0, id1, perm, iperm;
+    IF_CUDA_TRY(mk0.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(mk1.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(id0.alloc((size_t)nv * 4));
+    IF_CUDA_TRY(id1.alloc((size_t)nv * 4));
+    IF_CUDA_TRY(perm.alloc((size_t)nv * 4));
+    IF_CUDA_TRY(iperm.alloc((size_t)nv * 4));
+    k_morton<<<grid_for(nv), 256, 0, st>>>(d_coords.as<double>(), dim, nv, box, mk0.as<unsigned long long>(),
+                                          id0.as<int32_t>(), opt.sfc_kind == 1);
+    IF_LAUNCH_CHECK();
+    tb = 0;
+    IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tb, mk0.as<unsigned long long>(), mk1.as<unsigned long long>(),
+                                                id0.as<int32_t>(), id1.as<int32_t>(), nv, 0, 64, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tb, mk0.as<unsigned long long>(), mk1.as<unsigned long long>(),
+                                                id0.as<int32_t>(), id1.as<int32_t>(), nv, 0, 64, st));
+    ++g_launches;
+    // id1 = SFC order (rank -> caller id)
+    if (opt.sell_sigma > opt.sell_c) {
+        k_sigma_key<<<grid_for(nv), 256, 0, st>>>(id1.as<int32_t>(), len.as<int32_t>(), nv, opt.sell_sigma,
+                                                 mk0.as<unsigned long long>());
+        IF_LAUNCH_CHECK();
+        const int sb = 8 + bits_for((uint64_t)(nv / opt.sell_sigma + 1));
+        IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tb, mk0.as<unsigned long long>(),
+                                                    mk1.as<unsigned long long>(), id1.as<int32_t>(),
+                                                    perm.as<int32_t>(), nv, 0, sb, st));
+        ++g_launches;
+    } else {
+        IF_CUDA_TRY(cudaMemcpyAsync(perm.p, id1.p, (size_t)nv * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    k_invert_perm<<<grid_for(nv), 256, 0, st>>>(perm.as<int32_t>(), nv, iperm.as<int32_t>());
+    IF_LAUNCH_CHECK();
+
+    const int C = opt.sell_c;
+    const int64_t n_chunks = (nv + C - 1) / C;
+    h->n_chunks = n_chunks;
+    DevBuf slots, chunk_ptr;
+    IF_CUDA_TRY(slots.alloc((size_t)(n_chunks + 1) * 8));
+    IF_CUDA_TRY(chunk_ptr.alloc((size_t)(n_chunks + 1) * 8));
+    k_chunk_slots<<<grid_for(n_chunks + 1), 256, 0, st>>>(perm.as<int32_t>(), len.as<int32_t>(), nv, n_chunks, C,
+                                                         slots.as<int64_t>());
+    IF_LAUNCH_CHECK();
+    tb = 0;
+    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(nullptr, tb, slots.as<int64_t>(), chunk_ptr.as<int64_t>(),
+                                              n_chunks + 1, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(tmp.p, tb, slots.as<int64_t>(), chunk_ptr.as<int64_t>(), n_chunks + 1,
+                                              st));
+    ++g_launches;
+    int64_t sell_slots = 0;
+    IF_CUDA_TRY(cudaMemcpyAsync(&sell_slots, chunk_ptr.as<int64_t>() + n_chunks, 8, cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    h->sell_slots = sell_slots;
+
+    DevBuf scol, sval, area, inv_area, sdiag, gdiag;
+    IF_CUDA_TRY(scol.alloc((size_t)sell_slots * 4 + 16));
+    IF_CUDA_TRY(sval.alloc((size_t)sell_slots * 8 + 16));
+    IF_CUDA_TRY(area.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(inv_area.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(sdiag.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(gdiag.alloc((size_t)nv * 8));
+    k_sell_fill<<<grid_for(n_chunks * C), 256, 0, st>>>(
+        perm.as<int32_t>(), iperm.as<int32_t>(), rowptr.as<int64_t>(), ccol.as<int32_t>(), v0.as<double>(),
+        area_u.as<double>(), sdiag_u.as<double>(), gdiag_u.as<double>(), nv, n_chunks, C, chunk_ptr.as<int64_t>(),
+        scol.as<int32_t>(), sval.as<double>(), area.as<double>(), inv_area.as<double>(), sdiag.as<double>(),
+        gdiag.as<double>());
+    IF_LAUNCH_CHECK();
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+
+    if (opt.flags & IF_FLAG_KEEP_CSR) {
+        // v0 holds [9 n_tri] doubles; keep a right-sized copy instead
+        DevBuf cval;
+        IF_CUDA_TRY(cval.alloc((size_t)nnz * 8));
+        IF_CUDA_TRY(cudaMemcpy(cval.p, v0.p, (size_t)nnz * 8, cudaMemcpyDeviceToDevice));
+        h->csr_rowptr = (int64_t*)rowptr.release();
+        h->csr_col = (int32_t*)ccol.release();
+        h->csr_val = (double*)cval.release();
+        h->csr_area = (double*)area_u.release();
+    }
+    h->chunk_ptr = (int64_t*)chunk_ptr.release();
+    h->sell_col = (int32_t*)scol.release();
+    h->sell_val = (double*)sval.release();
+    h->area = (double*)area.release();
+    h->inv_area = (double*)inv_area.release();
+    h->sdiag = (double*)sdiag.release();
+    h->gdiag = (double*)gdiag.release();
+    h->perm = (int32_t*)perm.release();
+    h->iperm = (int32_t*)iperm.release();
+
+    h->h_pinned_bytes = 1 << 20;
+    IF_CUDA_TRY(cudaHostAlloc(&h->h_pinned, h->h_pinned_bytes, cudaHostAllocDefault));
+    return IF_OK;
+}
+
+extern "C" int if_prepare(const double* coords, int dim, int64_t n_vert, const int32_t* tri, int64_t n_tri,
+                          const double* period, const if_options* opt, if_handle* out) {
+    if (!coords || !tri || !out || (dim != 2 && dim != 3) || n_vert < 3 || n_tri < 1) return IF_EINVAL;
+    if (n_vert > 0x7fffffffLL || n_tri > 0x7fffffffLL / 9) return IF_EINVAL;
+    Options o;
+    int rc = resolve_options(opt, nullptr, &o);
+    if (rc != IF_OK) return rc;
+    if_mesh_s* h = new (std::nothrow) if_mesh_s();
+    if (!h) return IF_ENOMEM;
+    rc = prepare_impl(coords, dim, n_vert, tri, n_tri, period, o, h);
+    if (rc != IF_OK) {
+        if_destroy(h);
+        return rc;
+    }
+    *out = h;
+    return IF_OK;
+}
+
+extern "C" int if_mesh_info(if_handle h, int64_t* n_vert, int64_t* nnz, double* total_area, double* mean_edge,
+                            int64_t* sell_slots) {
+    if (!h) return IF_EINVAL;
+    if (n_vert) *n_vert = h->n_vert;
+    if (nnz) *nnz = h->nnz;
+    if (total_area) *total_area = h->total_area;
+    if (mean_edge) *mean_edge = h->mean_edge;
+    if (sell_slots) *sell_slots = h->sell_slots;
+    return IF_OK;
+}
+
+extern "C" int if_mesh_export_csr(if_handle h, int64_t* rowptr, int32_t* col, double* val, double* area) {
+    if (!h || !h->csr_rowptr) return IF_EINVAL;
+    IF_CUDA_TRY(cudaSetDevice(h->device));
+    if (rowptr) IF_CUDA_TRY(cudaMemcpy(rowptr, h->csr_rowptr, (size_t)(h->n_vert + 1) * 8, cudaMemcpyDeviceToHost));
+    if (col) IF_CUDA_TRY(cudaMemcpy(col, h->csr_col, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
+    if (val) IF_CUDA_TRY(cudaMemcpy(val, h->csr_val, (size_t)h->nnz * 8, cudaMemcpyDeviceToHost));
+    if (area) IF_CUDA_TRY(cudaMemcpy(area, h->csr_area, (size_t)h->n_vert * 8, cudaMemcpyDeviceToHost));
+    return IF_OK;
+}
+
+extern "C" int if_mesh_export_perm(if_handle h, int32_t* perm) {
+    if (!h) return IF_EINVAL;
+    IF_CUDA_TRY(cudaSetDevice(h->device));
+    if (perm) IF_CUDA_TRY(cudaMemcpy(perm, h->perm, (size_t)h->n_vert * 4, cudaMemcpyDeviceToHost));
+    return IF_OK;
+}
+
+extern "C" const char* if_strerror(int code) {
+    switch (code) {
+        case IF_OK: return "ok";
+        case IF_WNOTCONVERGED: return "some right-hand sides did not converge (max_iter or breakdown)";
+        case IF_EINVAL: return "invalid argument";
+        case IF_EINDEX: return "triangle vertex id out of range or repeated";
+        case IF_EDEGENERATE: return "degenerate triangle";
+        case IF_EORPHAN: return "vertex in no triangle";
+        case IF_ENOMEM: return "out of memory";
+        case IF_ECUDA: return "CUDA error or no device";
+        case IF_EWORKSPACE: return "workspace too small";
+        default: return "unknown error";
+    }
+}
+
+extern "C" int64_t if_launch_count(void) { return (int64_t)ifl::g_launches.load(); }

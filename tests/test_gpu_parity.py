@@ -1,0 +1,218 @@
+"""GPU parity: the CUDA path, called through the C ABI (paper_2404_07398_b200.binding -> libimplicit_filter.so),
+against the CPU oracle, element by element on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): relative L2 <= 1e-7 per filtered field, <= 1e-6 per spectrum bin.
+Assembly (integer structure) is compared exactly; fp64 values of S, A_v and of the operator to 1e-12, which is
+the rounding of differently ordered sums of <= 10 terms ("tolerances").
+"""
+import numpy as np
+import pytest
+
+from workloads import grid_mesh, make_config
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD = 1e-7
+TOL_BIN = 1e-6
+
+
+@pytest.fixture(scope="module")
+def ifl():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2404_07398_b200 as lib
+    lib.load_library()          # fails loudly if the extension is missing
+    return lib
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / max(np.linalg.norm(np.asarray(b)), 1e-300))
+
+
+SMALL = {
+    "cfg1": lambda: make_config(1),
+    "cfg2_n96": lambda: make_config(2, n=96, n_ells=6, ell_max=24.0),
+    "cfg3_L4": lambda: make_config(3, level=4, n_ells=5, ell_max=6.0),
+    "cfg4_L5": lambda: make_config(4, level=5, n_ells=7),
+    "cfg5_L4": lambda: make_config(5, level=4, n_fields=3, n_ells=4, ell_max=5.0),
+}
+
+
+# ------------------------------------------------------------------------------------------ preparation
+@pytest.mark.parametrize("name", list(SMALL))
+def test_prepare_matches_oracle_assembly(ifl, oracle_mod, name):
+    w = SMALL[name]()
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period, flags=ifl.IF_FLAG_KEEP_CSR)
+    rp, col, val, area = ifl.if_mesh_export_csr(h)
+    orp, ocol, oval = om.csr()
+    assert h.n_vert == om.nv and h.nnz == om.nnz
+    assert np.array_equal(rp, orp)                      # bit-exact structure
+    assert np.array_equal(col, ocol)
+    assert np.abs(val - oval).max() <= 1e-12 * np.abs(oval).max()
+    assert np.abs(area - om.area()).max() <= 1e-13 * om.area().max()
+    assert abs(h.total_area - om.area().sum()) <= 1e-12 * om.area().sum()
+    perm = ifl.if_mesh_export_perm(h)
+    assert np.array_equal(np.sort(perm), np.arange(om.nv))
+    assert h.sell_slots >= h.nnz - h.n_vert and h.sell_slots % 2 == 0
+    h.close()
+
+
+@pytest.mark.parametrize("opts", [dict(sfc_kind=1), dict(sell_sigma=32), dict(sell_c=64, sell_sigma=512),
+                                  dict(sell_c=128, sell_sigma=128)])
+def test_layout_options_do_not_change_results(ifl, oracle_mod, opts):
+    w = SMALL["cfg4_L5"]()
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, **opts)
+    ells = w.ells[[0, 3]]
+    out = ifl.if_apply(h, w.fields, ells, 1).cpu().numpy()
+    for f in range(w.fields.shape[0]):
+        for j, ell in enumerate(ells):
+            assert rel(out[f, j], om.apply(w.fields[f], ell, 1)) <= 1e-12
+    h.close()
+
+
+def test_prepare_error_codes(ifl):
+    coords = np.array([[0.0, 0.0], [1.0, 0.0], [0.0, 1.0], [5.0, 5.0]])
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_prepare(coords, np.array([[0, 1, 2]], dtype=np.int32))
+    assert e.value.code == -4                                        # orphan vertex 3
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_prepare(coords[:3], np.array([[0, 1, 3]], dtype=np.int32))
+    assert e.value.code == -2
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_prepare(coords[:3], np.array([[0, 1, 1]], dtype=np.int32))
+    assert e.value.code == -2
+    flat = np.array([[0.0, 0.0], [1.0, 0.0], [2.0, 0.0]])
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_prepare(flat, np.array([[0, 1, 2]], dtype=np.int32))
+    assert e.value.code == -3
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_prepare(coords[:3], np.array([[0, 1, 2]], dtype=np.int32), sell_c=48)
+    assert e.value.code == -1
+
+
+# ------------------------------------------------------------------------------------------ operator (SpMM)
+@pytest.mark.parametrize("name", list(SMALL))
+@pytest.mark.parametrize("order_n", [1, 2])
+def test_apply_matches_oracle_operator(ifl, oracle_mod, name, order_n):
+    w = SMALL[name]()
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    out = ifl.if_apply(h, w.fields, w.ells, order_n).cpu().numpy()
+    for f in range(w.fields.shape[0]):
+        for j, ell in enumerate(w.ells):
+            assert rel(out[f, j], om.apply(w.fields[f], ell, order_n)) <= 1e-12, (f, j)
+    h.close()
+
+
+# ------------------------------------------------------------------------------------------ filter + spectrum
+def check_workload(ifl, oracle_mod, w, order_n=None, **options):
+    order_n = w.order_n if order_n is None else order_n
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    ref, en, k_mid, E, infos = oracle_mod.filter_and_spectrum(om, w.fields, w.ells, order_n)
+    assert all(i["status"] == 0 for row in infos for i in row)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    out, st = ifl.if_filter(h, w.fields, w.ells, order_n, **options)
+    out = out.cpu().numpy()
+    assert st["code"] == 0 and np.all(st["status"] == 0)
+    for f in range(w.fields.shape[0]):
+        for j in range(w.ells.shape[0]):
+            assert rel(out[f, j], ref[f, j]) <= TOL_FIELD, (f, j, rel(out[f, j], ref[f, j]))
+    sp = ifl.if_spectrum(h, w.fields, w.ells, order_n, **options)
+    assert sp["stats"]["code"] == 0
+    assert np.abs(sp["energy"] - en).max() <= TOL_BIN * np.abs(en).max()
+    assert np.all(np.abs(sp["E"] - E) <= TOL_BIN * np.abs(E)), np.abs(sp["E"] / E - 1).max()
+    assert np.allclose(sp["k_mid"], k_mid, rtol=1e-14)
+    h.close()
+    return out, sp, st
+
+
+@pytest.mark.parametrize("name", list(SMALL))
+def test_filter_and_spectrum_match_oracle(ifl, oracle_mod, name):
+    check_workload(ifl, oracle_mod, SMALL[name]())
+
+
+def test_config1_closed_form_on_gpu(ifl):
+    """Config 1 against the plane-wave closed form directly (no oracle in between), and the golden energies."""
+    import os
+    w = make_config(1)
+    N = 64
+    wv = w.waves[0]
+    lam = 4.0 - 2.0 * np.cos(2 * np.pi * wv.k[:, 0] / N) - 2.0 * np.cos(2 * np.pi * wv.k[:, 1] / N)
+    basis = np.cos(w.mesh.coords @ (wv.k.T * wv.scale) + wv.theta)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    out, st = ifl.if_filter(h, w.fields, w.ells, 1)
+    out = out.cpu().numpy()
+    for j, ell in enumerate(w.ells):
+        ref = basis @ (wv.amp / (1.0 + 0.5 * ell ** 2 * lam))
+        assert rel(out[0, j], ref) <= TOL_FIELD
+    sp = ifl.if_spectrum(h, w.fields, w.ells, 1)
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "config1_closed_form.txt"), comments="#")
+    assert np.abs(sp["energy"][0] - gold[:, 1]).max() <= TOL_BIN * gold[:, 1].max()
+    h.close()
+
+
+@pytest.mark.parametrize("batch", [4, 8, 16])
+@pytest.mark.parametrize("n_ells", [1, 5, 9])
+def test_batch_sizes_and_ragged_tails(ifl, oracle_mod, batch, n_ells):
+    """R = 2 fields x n_ells right-hand sides never fills the last batch: unused columns must stay inert."""
+    w = make_config(2, n=48, n_ells=max(n_ells, 2), ell_max=12.0)
+    w.ells = w.ells[:n_ells] if n_ells > 1 else w.ells[1:2]
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    out, st = ifl.if_filter(h, w.fields, w.ells, 1, batch=batch)
+    out = out.cpu().numpy()
+    for f in range(2):
+        for j, ell in enumerate(w.ells):
+            x, _ = om.solve(w.fields[f], ell, 1)
+            assert rel(out[f, j], x) <= TOL_FIELD
+    h.close()
+
+
+def test_degenerate_inputs(ifl, oracle_mod):
+    w = make_config(4, level=4, n_fields=1, n_ells=3)
+    V = w.mesh.n_vert
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    fields = np.stack([np.full(V, 2.5), np.zeros(V), w.fields[0]])
+    out, st = ifl.if_filter(h, fields, w.ells, 1)
+    out = out.cpu().numpy()
+    assert st["code"] == 0
+    assert np.all(st["iters"][0] <= 1) and np.all(st["iters"][1] == 0)
+    assert np.abs(out[0] - 2.5).max() <= 1e-12            # constants are fixed points (S 1 = 0)
+    assert np.all(out[1] == 0.0)
+    # iteration cap: a status, not a hang (convergence may be lost)
+    out2, st2 = ifl.if_filter(h, w.fields, w.ells[-1:], 2, max_iter=4, check_every=2)
+    assert st2["code"] == 1 and st2["status"][0, 0] == 1 and st2["iters"][0, 0] == 4
+    assert np.all(np.isfinite(out2.cpu().numpy()))
+    # argument errors
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_filter(h, w.fields, [1.0, -1.0], 1)
+    assert e.value.code == -1
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_filter(h, w.fields, [1.0], 3)
+    assert e.value.code == -1
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_spectrum(h, w.fields, [2.0, 1.0], 1)
+    assert e.value.code == -1
+    import torch
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_filter(h, w.fields, [1.0], 1, workspace=torch.empty(1024, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == -7
+    h.close()
+
+
+def test_tolerance_and_paper_setting(ifl, oracle_mod):
+    """tol = 1e-9 stops earlier than the default and still lands within 1e-6 of the oracle."""
+    w = make_config(2, n=64, n_ells=3, ell_max=16.0)
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    o9, s9 = ifl.if_filter(h, w.fields[:1], w.ells, 1, tol=1e-9)
+    o12, s12 = ifl.if_filter(h, w.fields[:1], w.ells, 1)
+    assert np.all(s9["iters"] <= s12["iters"]) and s9["iters"].sum() < s12["iters"].sum()
+    assert np.all(s12["rel_res"] <= 1e-12) and np.all(s9["rel_res"] <= 1e-9)
+    for j, ell in enumerate(w.ells):
+        x, _ = om.solve(w.fields[0], ell, 1)
+        assert rel(o9[0, j].cpu().numpy(), x) <= 1e-6
+    h.close()
