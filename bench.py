@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py -- the implicit-filter hot path on B200, one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4] [--level L]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: ingest -> fused SELL SpMM +
+Jacobi-PCG iteration loop (CUDA graph) for every (field, scale) right-hand side -> energy reduction -> spectrum,
+i.e. one if_spectrum call on BASELINE.json config 4 (masked level-10 icosphere, 2 fields x 40 scales, n = 1),
+with the mesh prepared once (if_prepare, reported separately as the paper does).
+
+metric  = CG iterations per second summed over right-hand sides ("RHS-iterations/s"); the 40-scale spectrum time
+          is ms_per_step.  value: fields resident in HBM.  e2e: fields start in pinned HOST memory, results end
+          in host memory, copies inside the timed region.
+N > 1   = one process per GPU (torchrun); right-hand sides are independent, so every rank solves its own
+          2 fields x 40 scales on its own replica of the prepared mesh; no data-path collective ("weak").
+--impl reference = the CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cg_rhs_iterations_per_second"
+UNIT = "RHS-iterations/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 = the metric's")
+    ap.add_argument("--level", type=int, default=None, help="icosphere level override (smaller = quick check)")
+    ap.add_argument("--n", type=int, default=None, help="grid size override for configs 1-2")
+    ap.add_argument("--n-ells", type=int, default=None)
+    ap.add_argument("--tol", type=float, default=0.0, help="0 = library default 1e-12")
+    ap.add_argument("--batch", type=int, default=0)
+    ap.add_argument("--check-every", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-sample-iters", type=int, default=60)
+    return ap.parse_args()
+
+
+def workload_name(w, args):
+    V, T = w.mesh.n_vert, w.mesh.n_tri
+    return (f"config{w.config}: {w.note}, V={V} T={T}, {w.fields.shape[0]} fields x {w.ells.shape[0]} scales "
+            f"= {w.n_rhs} RHS, n={w.order_n}, l/h in [{w.ells[0] / w.mesh.h:.3g}, {w.ells[-1] / w.mesh.h:.4g}]")
+
+
+def build_workload(args, n_fields_total=None):
+    from workloads import make_config
+    kw = {}
+    if args.level is not None:
+        kw["level"] = args.level
+    if args.n is not None:
+        kw["n"] = args.n
+    if args.n_ells is not None:
+        kw["n_ells"] = args.n_ells
+    if n_fields_total is not None:
+        kw["n_fields"] = n_fields_total
+    return make_config(args.config, **kw)
+
+
+# ----------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons of one GPU, sampled every 200 ms while running."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        fd, self.path = tempfile.mkstemp(suffix=".csv")
+        os.close(fd)
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.path)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ----------------------------------------------------------------------------------------- byte model
+def algorithmic_bytes(V, nnz, K, order_n):
+    """Algorithmic HBM bytes of ONE launch of each iteration kernel:
+    every vector element and every matrix entry read or written once; gathers of neighbour rows are re-reads
+    of lines already counted (served by L1/L2), SELL padding is not algorithmic."""
+    offdiag = nnz - V
+    matrix = offdiag * 12 + V * 16          # int32 col + fp64 val per entry; S_vv|g_v and A_v (or 1/A_v) per row
+    if order_n == 1:
+        spmm = V * K * 8 * 6 + matrix       # read z, p, x ; write x, p', q
+    else:
+        spmm = V * K * 8 * 6 + matrix + V * K * 8 * 3 + matrix   # pass A as above (t for q) + pass B: read t, p', write q
+    update = V * K * 8 * 3 + V * 16         # read z, q ; write z ; A_v and diagonal per row
+    return {"spmm": spmm, "update": update, "iteration": spmm + update}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------------------- reference arm (oracle)
+def oracle_sample(w, n_iters, steps, warmup):
+    """The CPU oracle as it stands on a bounded sample of the workload: its mesh assembly once, then per step the
+    first `n_iters` PCG iterations of (field 0, middle scale).  Returns (RHS-iterations/s, ms per step, info)."""
+    import oracle
+    oracle.build()
+    t0 = time.perf_counter()
+    om = oracle.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    t_asm = time.perf_counter() - t0
+    j = w.ells.shape[0] // 2
+    times, its = [], 0
+    for s in range(warmup + steps):
+        t0 = time.perf_counter()
+        _, info = om.solve(w.fields[0], float(w.ells[j]), w.order_n, max_iter=n_iters)
+        dt = time.perf_counter() - t0
+        if s >= warmup:
+            times.append(dt)
+            its += info["iters"]
+    total = float(sum(times))
+    sample = (f"oracle PCG, field 0, scale index {j} (l/h={w.ells[j] / w.mesh.h:.3g}), first {n_iters} iterations "
+              f"per step on the full mesh (V={w.mesh.n_vert}); oracle assembly {t_asm:.1f} s not included")
+    return its / total, 1e3 * total / max(len(times), 1), {"cores": oracle.threads(), "sample": sample}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = build_workload(args)
+    warm = min(args.warmup, 1)
+    val, ms, info = oracle_sample(w, args.cpu_sample_iters, args.steps, warm)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": warm, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(w, args)},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
+                             "sample": info["sample"]},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2404_07398_b200 import build as libbuild
+    if rank == 0:
+        libbuild.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2404_07398_b200 as lib
+    from paper_2404_07398_b200.sharding import rank_fields
+    lib.load_library()
+
+    # every rank solves its own fields on its own replica of the mesh (weak scaling, no data-path collective)
+    w = build_workload(args)
+    base_fields = w.fields.shape[0]
+    if world > 1:
+        w = build_workload(args, n_fields_total=base_fields * world)
+        w.fields = w.fields[rank_fields(base_fields * world, world, rank)]
+    V = w.mesh.n_vert
+    R = w.n_rhs
+    opts = {}
+    if args.tol:
+        opts["tol"] = args.tol
+    if args.batch:
+        opts["batch"] = args.batch
+    if args.check_every:
+        opts["check_every"] = args.check_every
+    K = args.batch or 16
+
+    t0 = time.perf_counter()
+    h = lib.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    torch.cuda.synchronize()
+    t_prepare = time.perf_counter() - t0
+
+    stream = torch.cuda.Stream(device=dev)
+    ws = h.workspace(w.order_n, args.batch)
+    h_fields = torch.from_numpy(np.ascontiguousarray(w.fields)).pin_memory()
+    d_fields = h_fields.to(dev)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(from_host: bool):
+        with torch.cuda.stream(stream):
+            if from_host:
+                d_fields.copy_(h_fields, non_blocking=True)
+            return lib.if_spectrum(h, d_fields, w.ells, w.order_n, workspace=ws, stream=stream, **opts)
+
+    def timed(n_steps: int, from_host: bool):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        launches0 = lib.if_launch_count()
+        e0.record(stream)
+        res = [step(from_host) for _ in range(n_steps)]
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, res, lib.if_launch_count() - launches0
+
+    for _ in range(max(args.warmup, 0)):
+        sp = step(False)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms, res, launches = timed(args.steps, False)
+    clocks = sampler.stop()
+    stats = [r["stats"] for r in res]
+    rhs_iters = sum(s["rhs_iters"] for s in stats)
+    batch_iters = sum(s["batch_iters"] for s in stats)
+    codes = sorted({s["code"] for s in stats})
+    if world > 1:
+        t = torch.tensor([rhs_iters, batch_iters], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        rhs_iters_all, batch_iters_all = float(t[0].item()), float(t[1].item())
+    else:
+        rhs_iters_all, batch_iters_all = float(rhs_iters), float(batch_iters)
+    value = rhs_iters_all / (ms * 1e-3)
+
+    e2e = None
+    if not args.no_e2e:
+        ms_e, res_e, _ = timed(args.steps, True)
+        it_e = sum(r["stats"]["rhs_iters"] for r in res_e)
+        if world > 1:
+            t = torch.tensor([it_e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+            it_e = float(t.item())
+        L = w.ells.shape[0]
+        F = w.fields.shape[0]
+        d2h = R * 8 + (L - 1) * 8 + F * (L - 1) * 8 + R * (4 + 4 + 8)
+        e2e = {"value": it_e / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h_fields.numel() * 8),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e / args.steps}
+
+    # roofline of the dominant kernel (fused SpMM): live per-launch time from the library's event samples
+    nsamp = sum(s["kernel_samples"] for s in stats)
+    spmm_s = sum(s["spmm_seconds"] * s["kernel_samples"] for s in stats) / max(nsamp, 1)
+    upd_s = sum(s["update_seconds"] * s["kernel_samples"] for s in stats) / max(nsamp, 1)
+    ab = algorithmic_bytes(V, h.nnz, K, w.order_n)
+    peak, peak_src = measured_peaks()
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(f"config{w.config}_V{V}_spmm_bytes_per_launch")
+        except Exception:
+            traffic = None
+    achieved = ab["spmm"] / spmm_s / 1e9 if spmm_s > 0 else None
+    roofline = {"bound": "hbm", "kernel": f"k_spmm<{K},CG{'1' if w.order_n == 1 else '2A+2B'}>",
+                "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["spmm"],
+                "launch_seconds": spmm_s, "samples": nsamp,
+                "update_kernel": {"achieved": ab["update"] / upd_s / 1e9 if upd_s > 0 else None,
+                                  "algorithmic_bytes_per_launch": ab["update"], "launch_seconds": upd_s},
+                "iteration": {"achieved": ab["iteration"] / (spmm_s + upd_s) / 1e9 if spmm_s > 0 else None,
+                              "frac": ab["iteration"] / (spmm_s + upd_s) / 1e9 / peak if spmm_s > 0 else None,
+                              "frac_of_8TBs_nominal": ab["iteration"] / (spmm_s + upd_s) / 8e12 if spmm_s > 0 else None}}
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, _, info = oracle_sample(w, args.cpu_sample_iters, 3, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": info["cores"], "kind": "oracle", "sample": info["sample"]}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(w, args), "batch_rhs_per_spmm": K,
+                       "tol": args.tol or 1e-12, "l2": "work vectors (5 x V x 16 x 8 B) exceed L2; no flush needed",
+                       "parallelism": f"rhs-replicas x{world}"},
+            "spectrum_seconds": ms * 1e-3 / args.steps, "prepare_seconds": t_prepare,
+            "rhs_iterations_per_step": rhs_iters_all / args.steps / world,
+            "batch_iterations_per_second": batch_iters_all / (ms * 1e-3),
+            "solver_codes": codes, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -80,6 +80,11 @@ typedef struct {
     double seconds;     /* out: device time of the call (CUDA events on the stream)                         */
     int64_t batch_iters; /* out: fused SpMM+CG iterations launched, summed over batches                      */
     int64_t rhs_iters;   /* out: sum over right-hand sides of their iterations                               */
+    double spmm_seconds;   /* out: mean device time of ONE operator application inside the iteration loop (the
+                              fused SpMM kernel; for n = 2 its two launches), CUDA events on the stream, sampled
+                              once per check_every iterations; 0 if nothing was sampled                       */
+    double update_seconds; /* out: the same for ONE fused vector-update kernel                               */
+    int64_t kernel_samples; /* out: number of samples behind the two means                                   */
 } if_stats;
 
 /* Preparation phase.  All pointers HOST.

@@ -486,10 +486,30 @@ struct Run {
     Options opt;
 };
 
+// Events recorded (as external event-record nodes) around one SpMM and one update launch of a captured graph,
+// so that the per-launch duration of both kernels is measured live on the launching stream (if_stats).
+struct TimingEvents {
+    cudaEvent_t s0 = nullptr, s1 = nullptr, u1 = nullptr;   // before SpMM, after SpMM (= before update), after update
+    int create() {
+        IF_CUDA_TRY(cudaEventCreate(&s0));
+        IF_CUDA_TRY(cudaEventCreate(&s1));
+        IF_CUDA_TRY(cudaEventCreate(&u1));
+        return IF_OK;
+    }
+    void destroy() {
+        if (s0) cudaEventDestroy(s0);
+        if (s1) cudaEventDestroy(s1);
+        if (u1) cudaEventDestroy(u1);
+        s0 = s1 = u1 = nullptr;
+    }
+};
+
 template <int K>
-int enqueue_two_iterations(const Run& r, const Geo& g) {
+int enqueue_two_iterations(const Run& r, const Geo& g, const TimingEvents* tev = nullptr) {
     // iteration with p0 -> p1, then p1 -> p0
     for (int half = 0; half < 2; ++half) {
+        const bool timed = tev && half == 0;
+        if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s0, r.st, cudaEventRecordExternal));
         const double* pold = half == 0 ? r.w.p0 : r.w.p1;
         double* pnew = half == 0 ? r.w.p1 : r.w.p0;
         if (r.order_n == 1) {
@@ -504,12 +524,26 @@ int enqueue_two_iterations(const Run& r, const Geo& g) {
             k_spmm<K, MODE_CG2B><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, b, g.rows_per_block);
             IF_LAUNCH_CHECK();
         }
+        if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s1, r.st, cudaEventRecordExternal));
         k_update<K><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.z, r.w.q, r.order_n,
                                                 g.rows_per_block);
         IF_LAUNCH_CHECK();
+        if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->u1, r.st, cudaEventRecordExternal));
     }
     return IF_OK;
 }
+
+// Two instantiations of the iteration graph, launched alternately: while one runs, the host reads the timing
+// events of the other (an event must not be re-recorded while it is being read).
+struct GraphSet {
+    cudaGraphExec_t exec[2] = {nullptr, nullptr};
+    TimingEvents tev[2];
+    ~GraphSet() {
+        for (int i = 0; i < 2; ++i) { if (exec[i]) cudaGraphExecDestroy(exec[i]); tev[i].destroy(); }
+    }
+};
+
+struct KernelTimes { double spmm_ms = 0.0, update_ms = 0.0; int64_t samples = 0; };
 
 struct PollState {
     int* flags = nullptr;          // pinned [4]
@@ -525,8 +559,8 @@ struct PollState {
 
 template <int K>
 int solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, size_t first, size_t count,
-                int n_ells, double* d_out, PollState& poll, int blocks_per_sm, cudaGraphExec_t* graph_cache,
-                int64_t* batch_iters) {
+                int n_ells, double* d_out, PollState& poll, int blocks_per_sm, GraphSet* graph_cache,
+                int64_t* batch_iters, KernelTimes* times) {
     const if_mesh_s* h = r.h;
     const Geo g = geometry(h->n_vert, K, h->n_sm, blocks_per_sm);
     Ctrl hc;
@@ -583,26 +617,32 @@ int solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
     // the iteration loop: `check_every` iterations per CUDA graph launch, flag polled one launch behind
     const int pairs = r.opt.check_every / 2;
     const int launches_per_graph = pairs * 2 * (r.order_n == 1 ? 2 : 3);
-    cudaGraphExec_t& gexec = *graph_cache;
-    if (!gexec && r.st != nullptr && r.st != cudaStreamLegacy) {
-        cudaGraph_t graph = nullptr;
-        if (cudaStreamBeginCapture(r.st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+    GraphSet& gs = *graph_cache;
+    if (!gs.exec[0] && r.st != nullptr && r.st != cudaStreamLegacy) {
+        for (int gi = 0; gi < 2; ++gi) {
+            if (gs.tev[gi].create() != IF_OK) return IF_ECUDA;
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(r.st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+                cudaGetLastError();   // stream cannot be captured: fall through to direct launches
+                break;
+            }
             int rc = IF_OK;
-            for (int i = 0; i < pairs && rc == IF_OK; ++i) rc = enqueue_two_iterations<K>(r, g);
+            const int timed_pair = pairs > 1 ? 1 : 0;
+            for (int i = 0; i < pairs && rc == IF_OK; ++i)
+                rc = enqueue_two_iterations<K>(r, g, i == timed_pair ? &gs.tev[gi] : nullptr);
             g_launches -= (long long)launches_per_graph;   // captured, not launched
             cudaError_t e = cudaStreamEndCapture(r.st, &graph);
             if (rc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
-            e = cudaGraphInstantiate(&gexec, graph, 0);
+            e = cudaGraphInstantiate(&gs.exec[gi], graph, 0);
             cudaGraphDestroy(graph);
-            if (e != cudaSuccess) { gexec = nullptr; cudaGetLastError(); return IF_ECUDA; }
-        } else {
-            cudaGetLastError();   // stream cannot be captured: fall through to direct launches
+            if (e != cudaSuccess) { gs.exec[gi] = nullptr; cudaGetLastError(); return IF_ECUDA; }
         }
     }
+    const bool use_graph = gs.exec[0] && gs.exec[1];
     const int64_t max_loops = (r.opt.max_iter + r.opt.check_every - 1) / r.opt.check_every + 2;
     for (int64_t it = 0; it < max_loops; ++it) {
-        if (gexec) {
-            IF_CUDA_TRY(cudaGraphLaunch(gexec, r.st));
+        if (use_graph) {
+            IF_CUDA_TRY(cudaGraphLaunch(gs.exec[it & 1], r.st));
             g_launches += (long long)launches_per_graph;
         } else {
             for (int i = 0; i < pairs; ++i) {
@@ -617,6 +657,17 @@ int solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
         if (it >= 1) {
             const int prev = (int)((it - 1) & 3);
             IF_CUDA_TRY(cudaEventSynchronize(poll.ev[prev]));
+            if (use_graph && !poll.flags[prev]) {
+                // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
+                const TimingEvents& te = gs.tev[(it - 1) & 1];
+                float a = 0.f, b = 0.f;
+                if (cudaEventElapsedTime(&a, te.s0, te.s1) == cudaSuccess &&
+                    cudaEventElapsedTime(&b, te.s1, te.u1) == cudaSuccess) {
+                    times->spmm_ms += a; times->update_ms += b; times->samples += 1;
+                } else {
+                    cudaGetLastError();
+                }
+            }
             if (poll.flags[prev]) break;
         }
     }
@@ -635,12 +686,12 @@ int solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
 }
 
 int dispatch_batch(int K, Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, size_t first,
-                   size_t count, int n_ells, double* d_out, PollState& poll, int bps, cudaGraphExec_t* cache,
-                   int64_t* bi) {
+                   size_t count, int n_ells, double* d_out, PollState& poll, int bps, GraphSet* cache,
+                   int64_t* bi, KernelTimes* kt) {
     switch (K) {
-        case 4: return solve_batch<4>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[0], bi);
-        case 8: return solve_batch<8>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[1], bi);
-        default: return solve_batch<16>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[2], bi);
+        case 4: return solve_batch<4>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[0], bi, kt);
+        case 8: return solve_batch<8>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[1], bi, kt);
+        default: return solve_batch<16>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[2], bi, kt);
     }
 }
 
@@ -706,8 +757,8 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (job != JOB_APPLY)
         std::stable_sort(rhs.begin(), rhs.end(), [](const Rhs& a, const Rhs& b) { return a.ell < b.ell; });
 
-    cudaGraphExec_t cache[3] = {nullptr, nullptr, nullptr};
-    struct GraphGuard { cudaGraphExec_t* c; ~GraphGuard() { for (int i = 0; i < 3; ++i) if (c[i]) cudaGraphExecDestroy(c[i]); } } gg{cache};
+    GraphSet cache[3];
+    KernelTimes ktimes;
     std::vector<std::pair<size_t, size_t>> batches;
     int64_t launched_iters = 0;
     size_t first = 0;
@@ -716,7 +767,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
         int K = r.opt.batch;
         while (K > 4 && remaining <= (size_t)K / 2) K /= 2;
         const size_t count = remaining < (size_t)K ? remaining : (size_t)K;
-        rc = dispatch_batch(K, r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, cache, &launched_iters);
+        rc = dispatch_batch(K, r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, cache, &launched_iters, &ktimes);
         if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
         batches.emplace_back(first, count);
         first += count;
@@ -751,6 +802,9 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
         stats->seconds = ms * 1e-3;
         stats->batch_iters = 0;
         stats->rhs_iters = 0;
+        stats->spmm_seconds = ktimes.samples ? 1e-3 * ktimes.spmm_ms / (double)ktimes.samples : 0.0;
+        stats->update_seconds = ktimes.samples ? 1e-3 * ktimes.update_ms / (double)ktimes.samples : 0.0;
+        stats->kernel_samples = ktimes.samples;
         for (auto& b : batches) {
             int mx = 0;
             for (size_t i = 0; i < b.second; ++i) {
