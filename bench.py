@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--tol", type=float, default=0.0, help="0 = library default 1e-12")
     ap.add_argument("--batch", type=int, default=0)
     ap.add_argument("--check-every", type=int, default=0)
+    ap.add_argument("--max-iter", type=int, default=0, help="iteration cap per RHS (profiling runs only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-iters", type=int, default=60)
@@ -234,6 +235,8 @@ def run_ours(args):
         opts["batch"] = args.batch
     if args.check_every:
         opts["check_every"] = args.check_every
+    if args.max_iter:
+        opts["max_iter"] = args.max_iter
     K = args.batch or 16
 
     t0 = time.perf_counter()
