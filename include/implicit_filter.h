@@ -67,7 +67,7 @@ typedef struct {
     int max_iter;    /* 0 => 200000 iterations per right-hand side                                          */
     int check_every; /* 0 => 16; iterations per CUDA-graph launch = between two polls of the done flag     */
     int batch;       /* right-hand sides per SpMM: 4, 8 or 16; 0 => 16                                      */
-    int sell_c;      /* SELL chunk height C (rows sharing one padded width): multiple of 32; 0 => 32        */
+    int sell_c;      /* SELL chunk height C (rows sharing one padded width): 32, 64 or 128; 0 => 32          */
     int sell_sigma;  /* SELL sorting window sigma (rows): multiple of sell_c; 0 => 256; == sell_c: no sort  */
     int sfc_kind;    /* 0 => Morton order of the quantised coordinates; 1 => keep the caller's order        */
     int flags;       /* IF_FLAG_*                                                                           */

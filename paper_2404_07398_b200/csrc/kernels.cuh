@@ -1,0 +1,586 @@
+// Device code of the solving phase: batched multi-right-hand-side Jacobi-PCG on
+//     A_c x_c = M phi_c,   A_c = M + c_c S (M^-1 S)^(n-1),   c_c = gamma l_c^(2n)
+// for K = 4, 8 or 16 columns c at once, every column with its own scale l_c, field, alpha, beta and stop time.
+//
+// Layout: work vectors are [row][K] fp64 (K = 16: one 128-byte line per row), rows in the internal order.
+// A row is handled by K/2 threads, each owning two adjacent columns (double2 = 16-byte accesses), so a warp
+// covers 64/K rows and every gather of a neighbour row is one contiguous K*8-byte segment.
+//
+// CG is carried in the preconditioned residual z = r/d (d = diag(A_c), Jacobi):
+//   kernel A (k_spmm, fused):  p' = z + beta p ;  x += alpha_prev p ;  q = A_c p' ;  partial p'.q
+//   kernel B (k_update):       z -= alpha q/d ;  partial rho' = sum d z^2 = r.z  and  ||r||^2 = sum (d z)^2
+// Per-column scalars (alpha, beta, rho, done flags) live in a device control block and are produced by the
+// last block to finish each kernel (single-pass, fixed-order, deterministic grid reduction).
+//
+// Kernel A is tiled for sm_100a: a persistent CTA walks tiles of T consecutive rows.  Per tile one thread issues
+// bulk async copies (TMA, cp.async.bulk + mbarrier complete_tx) that land the tile of z, p, x and the tile's
+// slice of the SELL matrix in shared memory; the CTA forms p' in place, hands x and p' back to global memory
+// with bulk stores, and gathers the neighbours' p' from the shared tile (rows are in space-filling-curve
+// order, so most neighbours are in the tile); only out-of-tile neighbours touch L2.
+#pragma once
+
+#include "common.cuh"
+
+namespace ifl {
+namespace {
+
+constexpr int KMAX = 16;
+constexpr int BLOCK = 256;
+constexpr int WCAP = 8;   // SELL slots per row that fit the shared-memory matrix slice (wider tiles read global)
+
+struct MeshView {
+    const int64_t* __restrict__ chunk_ptr;
+    const int32_t* __restrict__ col;
+    const double* __restrict__ val;
+    const double* __restrict__ area;
+    const double* __restrict__ inv_area;
+    const double* __restrict__ sdiag;
+    const double* __restrict__ gdiag;
+    const int32_t* __restrict__ perm;
+    int64_t nv;
+    int64_t n_chunks;
+    int log2c;
+};
+
+struct Ctrl {
+    double c[KMAX];       // gamma l^(2n)
+    double alpha[KMAX];
+    double beta[KMAX];
+    double rho[KMAX];
+    double bb[KMAX];      // ||M phi||^2
+    double rr[KMAX];      // ||r||^2 (recursive)
+    int field[KMAX];      // field of the column, -1 = empty column
+    int rhs[KMAX];        // f * n_ells + j of the column
+    int done[KMAX];
+    int epoch[KMAX];      // bumped every time a column is (re)started: lets the host match a snapshot to a RHS
+    int status[KMAX];
+    int iters[KMAX];
+    int all_done;
+    int cur_p;            // which direction buffer the last kernel A wrote
+    int max_iter;
+    int pad_;
+    double tol2;
+    long long total_iters;   // fused iterations executed while some column was active
+    unsigned int ticket[4];
+};
+
+// what the host reads back every check_every iterations
+struct Snapshot {
+    int done[KMAX];
+    int epoch[KMAX];
+};
+
+// per-column parameters of a (re)start, passed by value to k_init
+struct StartParams {
+    double c[KMAX];
+    int field[KMAX];
+    int rhs[KMAX];
+};
+
+enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3 };
+
+__device__ __forceinline__ double2 ld2(const double* __restrict__ p, int64_t i) {
+    return *reinterpret_cast<const double2*>(p + i);
+}
+__device__ __forceinline__ void st2(double* __restrict__ p, int64_t i, double2 v) {
+    *reinterpret_cast<double2*>(p + i) = v;
+}
+
+// ---- bulk async copy (TMA) and mbarrier wrappers (PTX ISA: cp.async.bulk, mbarrier)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    const uint32_t addr = smem_u32(bar);
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void bulk_load(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* dst_gmem, const void* src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)),
+                 "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+// Fixed-order block reduction of NV double2 accumulators per thread over the threads owning the same column
+// pair, then a ticket: the last block to arrive sums all blocks' partials in block order.
+// Returns true in the last block, with the totals of value set j, column c in tot[j*KMAX + c] (shared memory).
+template <int K, int NV>
+__device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __restrict__ partials,
+                                            unsigned int* ticket, double* tot /* shared [NV*KMAX] */) {
+    constexpr int TPR = K / 2;
+    __shared__ double2 red[BLOCK];
+    __shared__ bool is_last;
+    const int tid = threadIdx.x;
+    for (int j = 0; j < NV; ++j) {
+        red[tid] = acc[j];
+        __syncthreads();
+        if (tid < TPR) {
+            double2 s = red[tid];
+            for (int i = tid + TPR; i < BLOCK; i += TPR) { s.x += red[i].x; s.y += red[i].y; }
+            partials[((size_t)j * gridDim.x + blockIdx.x) * K + 2 * tid] = s.x;
+            partials[((size_t)j * gridDim.x + blockIdx.x) * K + 2 * tid + 1] = s.y;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        __threadfence();
+        unsigned int t = atomicAdd(ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    __threadfence();
+    double* redd = reinterpret_cast<double*>(red);   // [BLOCK] doubles (uses half of red)
+    constexpr int LANES = BLOCK / K;                  // threads per column
+    for (int j = 0; j < NV; ++j) {
+        const int c = tid % K, lane = tid / K;
+        double s = 0.0;
+        for (unsigned b = lane; b < gridDim.x; b += LANES)
+            s += __ldcg(&partials[((size_t)j * gridDim.x + b) * K + c]);
+        redd[tid] = s;
+        __syncthreads();
+        if (tid < K) {
+            double t = 0.0;
+            for (int i = 0; i < LANES; ++i) t += redd[i * K + tid];
+            tot[j * KMAX + tid] = t;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) *ticket = 0u;
+    return true;
+}
+
+// ------------------------------------------------------------------------------------------- kernel A
+struct SpmmArgs {
+    const double* in0;   // PLAIN: x        CG1/CG2A: z        CG2B: t            (the gathered vector)
+    const double* in1;   //                 CG1/CG2A: p_old    CG2B: p (current)
+    double* x;           //                 CG1/CG2A: x (in place)
+    double* out0;        // PLAIN: y        CG1: q             CG2A: t            CG2B: q
+    double* out1;        //                 CG1/CG2A: p_new
+    int scale_inv_area;  // PLAIN: multiply the row result by 1/A_v
+    int out_idx;         // CG1/CG2A: index of the direction buffer written (recorded in ctrl->cur_p)
+};
+
+template <int K> struct TileRows { static constexpr int T = K == 16 ? 128 : 256; };
+
+// dynamic shared memory of k_spmm: [vec a | vec b | vec c][val slice][col slice][chunk offsets][mbarrier]
+template <int K, int MODE> struct TileSmem {
+    static constexpr int T = TileRows<K>::T;
+    static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : (MODE == MODE_CG2B ? 2 : 3);
+    static constexpr size_t vec_bytes = (size_t)T * K * sizeof(double);
+    static constexpr size_t off_val = NVEC * vec_bytes;
+    static constexpr size_t off_col = off_val + (size_t)T * WCAP * sizeof(double);
+    static constexpr size_t off_cp = off_col + (size_t)T * WCAP * sizeof(int32_t);
+    static constexpr size_t off_bar = off_cp + 64 * sizeof(int32_t);
+    static constexpr size_t bytes = off_bar + 16;
+};
+
+template <int K, int MODE>
+__global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+                                                SpmmArgs a) {
+    using SM = TileSmem<K, MODE>;
+    constexpr int T = SM::T;
+    constexpr int TPR = K / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    constexpr bool CG_A = (MODE == MODE_CG1 || MODE == MODE_CG2A);
+    if (MODE != MODE_PLAIN && ctrl->all_done) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    double2* sa = reinterpret_cast<double2*>(smem);                        // gathered vector (z -> p', x, t)
+    double2* sb = reinterpret_cast<double2*>(smem + SM::vec_bytes);        // p_old, or own p' (CG2B)
+    double2* sc = reinterpret_cast<double2*>(smem + 2 * SM::vec_bytes);    // x
+    const double* sval = reinterpret_cast<const double*>(smem + SM::off_val);
+    const int32_t* scol = reinterpret_cast<const int32_t*>(smem + SM::off_col);
+    int32_t* scp = reinterpret_cast<int32_t*>(smem + SM::off_cp);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + SM::off_bar);
+
+    const int tid = threadIdx.x;
+    const int l = tid % TPR;
+    double2 beta = {0.0, 0.0}, alpha = {0.0, 0.0}, cc = {0.0, 0.0};
+    if (MODE != MODE_PLAIN) {
+        beta = ld2(ctrl->beta, 2 * l);
+        alpha = ld2(ctrl->alpha, 2 * l);
+        cc = ld2(ctrl->c, 2 * l);
+    }
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        fence_proxy_async();
+    }
+    uint32_t parity = 0;
+    double2 acc[1] = {{0.0, 0.0}};
+    const int C = 1 << m.log2c;
+    const int64_t ntiles = (m.nv + T - 1) / T;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int64_t row0 = tile * T;
+        const int nrows = (int)min((int64_t)T, m.nv - row0);
+        const uint32_t vbytes = (uint32_t)nrows * K * sizeof(double);
+        const int64_t ch0 = row0 >> m.log2c;
+        const int nch = (nrows + C - 1) >> m.log2c;
+        const int64_t cp_first = m.chunk_ptr[ch0];
+        const int64_t slots = m.chunk_ptr[ch0 + nch] - cp_first;
+        const bool msm = slots <= (int64_t)T * WCAP;       // the tile's SELL slice fits shared memory
+        __syncthreads();   // everyone is done reading the previous tile (and the barrier is initialised)
+        if (tid == 0) {
+            bulk_wait_read0();   // the previous tile's bulk stores have finished reading sa / sc
+            mbar_expect_tx(bar, vbytes * SM::NVEC + (msm ? (uint32_t)slots * 12u : 0u));
+            bulk_load(sa, a.in0 + row0 * K, vbytes, bar);
+            if (SM::NVEC >= 2) bulk_load(sb, a.in1 + row0 * K, vbytes, bar);
+            if (SM::NVEC >= 3) bulk_load(sc, a.x + row0 * K, vbytes, bar);
+            if (msm) {
+                bulk_load(const_cast<double*>(sval), m.val + cp_first, (uint32_t)slots * 8u, bar);
+                bulk_load(const_cast<int32_t*>(scol), m.col + cp_first, (uint32_t)slots * 4u, bar);
+            }
+        }
+        if (tid <= nch) scp[tid] = (int32_t)(m.chunk_ptr[ch0 + tid] - cp_first);
+        mbar_wait(bar, parity);
+        parity ^= 1u;
+        if (CG_A) {
+            // p' = z + beta p (in place over z) ; x += alpha_prev p (in place) ; both go back with bulk stores
+            for (int e = tid; e < nrows * TPR; e += BLOCK) {
+                const double2 zv = sa[e], pv = sb[e];
+                double2 xv = sc[e];
+                double2 own;
+                own.x = fma(beta.x, pv.x, zv.x);
+                own.y = fma(beta.y, pv.y, zv.y);
+                xv.x = fma(alpha.x, pv.x, xv.x);
+                xv.y = fma(alpha.y, pv.y, xv.y);
+                sa[e] = own;
+                sc[e] = xv;
+            }
+            fence_proxy_async();
+        }
+        __syncthreads();
+        if (CG_A && tid == 0) {
+            bulk_store(a.out1 + row0 * K, sa, vbytes);
+            bulk_store(a.x + row0 * K, sc, vbytes);
+            bulk_commit();
+        }
+        for (int r = tid / TPR; r < nrows; r += ROWS) {
+            const int64_t row = row0 + r;
+            const int chl = r >> m.log2c;
+            const int cpr = scp[chl];
+            const int w = (scp[chl + 1] - cpr) >> m.log2c;
+            const int o = cpr + (r & (C - 1)) * w;
+            const double2 own = sa[r * TPR + l];
+            double2 s = {0.0, 0.0};
+            for (int k = 0; k < w; k += 2) {
+                int2 cj;
+                double2 vj;
+                if (msm) {
+                    cj = *reinterpret_cast<const int2*>(scol + o + k);
+                    vj = *reinterpret_cast<const double2*>(sval + o + k);
+                } else {
+                    cj = *reinterpret_cast<const int2*>(m.col + cp_first + o + k);
+                    vj = ld2(m.val, cp_first + o + k);
+                }
+                double2 g0, g1;
+                const unsigned j0 = (unsigned)(cj.x - (int)row0), j1 = (unsigned)(cj.y - (int)row0);
+                if (j0 < (unsigned)nrows) {
+                    g0 = sa[j0 * TPR + l];
+                } else if (CG_A) {
+                    const double2 z0 = ld2(a.in0, (int64_t)cj.x * K + 2 * l), p0 = ld2(a.in1, (int64_t)cj.x * K + 2 * l);
+                    g0.x = fma(beta.x, p0.x, z0.x); g0.y = fma(beta.y, p0.y, z0.y);
+                } else {
+                    g0 = ld2(a.in0, (int64_t)cj.x * K + 2 * l);
+                }
+                if (j1 < (unsigned)nrows) {
+                    g1 = sa[j1 * TPR + l];
+                } else if (CG_A) {
+                    const double2 z1 = ld2(a.in0, (int64_t)cj.y * K + 2 * l), p1 = ld2(a.in1, (int64_t)cj.y * K + 2 * l);
+                    g1.x = fma(beta.x, p1.x, z1.x); g1.y = fma(beta.y, p1.y, z1.y);
+                } else {
+                    g1 = ld2(a.in0, (int64_t)cj.y * K + 2 * l);
+                }
+                s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
+                s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
+            }
+            const double sd = m.sdiag[row];
+            s.x = fma(sd, own.x, s.x);
+            s.y = fma(sd, own.y, s.y);          // s = (S v)_row
+            const int64_t ri = row * K + 2 * l;
+            if (MODE == MODE_PLAIN) {
+                if (a.scale_inv_area) { const double ia = m.inv_area[row]; s.x *= ia; s.y *= ia; }
+                st2(a.out0, ri, s);
+            } else if (MODE == MODE_CG2A) {
+                const double ia = m.inv_area[row];
+                s.x *= ia; s.y *= ia;            // t = M^-1 S p'
+                st2(a.out0, ri, s);
+            } else {
+                // q = A_v p + c (S v)_row ; v = p (n = 1) or t (n = 2)
+                const double av = m.area[row];
+                const double2 pv = (MODE == MODE_CG1) ? own : sb[r * TPR + l];
+                double2 q;
+                q.x = fma(cc.x, s.x, av * pv.x);
+                q.y = fma(cc.y, s.y, av * pv.y);
+                st2(a.out0, ri, q);
+                acc[0].x = fma(pv.x, q.x, acc[0].x);
+                acc[0].y = fma(pv.y, q.y, acc[0].y);
+            }
+        }
+    }
+    if (CG_A && tid == 0) bulk_wait0();
+    if (MODE == MODE_CG1 || MODE == MODE_CG2B) {
+        __shared__ double tot[KMAX];
+        if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[0], tot)) {
+            if (tid < K) {
+                const double pq = tot[tid];
+                double al = 0.0;
+                if (!ctrl->done[tid]) {
+                    if (pq > 0.0 && isfinite(pq)) al = ctrl->rho[tid] / pq;
+                    else { ctrl->done[tid] = 1; ctrl->status[tid] = 2; }
+                }
+                ctrl->alpha[tid] = al;
+            }
+        }
+    }
+    if (CG_A && blockIdx.x == 0 && tid == 0) ctrl->cur_p = a.out_idx;
+}
+
+// ------------------------------------------------------------------------------------------- start of a column
+// x[row][c] = field_c[perm[row]] for the columns in `mask`  (H0 ingest: gather through the permutation, transpose)
+template <int K>
+__global__ void __launch_bounds__(BLOCK) k_ingest(MeshView m, StartParams sp, unsigned mask,
+                                                  const double* __restrict__ fields, double* __restrict__ x) {
+    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
+    if (i >= m.nv * K) return;
+    const int64_t row = i / K;
+    const int c = (int)(i % K);
+    if (!((mask >> c) & 1u)) return;
+    const int f = sp.field[c];
+    x[i] = f >= 0 ? fields[(int64_t)f * m.nv + m.perm[row]] : 0.0;
+}
+
+// Start of CG from x0 = phi for the columns in `mask`: y = S (M^-1 S)^(n-1) phi is given;
+// r0 = M phi - A_c phi = -c y ;  z0 = r0/d ;  p = 0 ;  rho0 = r0.z0 ;  ||r0||^2 ;  ||M phi||^2.
+template <int K>
+__global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+                                                StartParams sp, unsigned mask, const double* __restrict__ x,
+                                                const double* __restrict__ y, double* __restrict__ z,
+                                                double* __restrict__ p0, double* __restrict__ p1, int order_n) {
+    constexpr int TPR = K / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    const int tid = threadIdx.x, l = tid % TPR;
+    const bool on0 = (mask >> (2 * l)) & 1u, on1 = (mask >> (2 * l + 1)) & 1u;
+    const double2 cc = {sp.c[2 * l], sp.c[2 * l + 1]};
+    const double* __restrict__ dg = order_n == 1 ? m.sdiag : m.gdiag;
+    double2 acc[3] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+    if (on0 || on1) {
+        for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < m.nv; row += (int64_t)gridDim.x * ROWS) {
+            const int64_t ri = row * K + 2 * l;
+            const double av = m.area[row], dv = dg[row];
+            const double2 d = {fma(cc.x, dv, av), fma(cc.y, dv, av)};
+            const double2 xv = ld2(x, ri), yv = ld2(y, ri);
+            double2 zv = ld2(z, ri), pa = ld2(p0, ri), pb = ld2(p1, ri);
+            const double2 r = {-cc.x * yv.x, -cc.y * yv.y};
+            const double2 b = {av * xv.x, av * xv.y};
+            if (on0) {
+                zv.x = r.x / d.x; pa.x = 0.0; pb.x = 0.0;
+                acc[0].x = fma(r.x, zv.x, acc[0].x); acc[1].x = fma(r.x, r.x, acc[1].x); acc[2].x = fma(b.x, b.x, acc[2].x);
+            }
+            if (on1) {
+                zv.y = r.y / d.y; pa.y = 0.0; pb.y = 0.0;
+                acc[0].y = fma(r.y, zv.y, acc[0].y); acc[1].y = fma(r.y, r.y, acc[1].y); acc[2].y = fma(b.y, b.y, acc[2].y);
+            }
+            st2(z, ri, zv);
+            st2(p0, ri, pa);
+            st2(p1, ri, pb);
+        }
+    }
+    __shared__ double tot[3 * KMAX];
+    if (grid_reduce<K, 3>(acc, partials, &ctrl->ticket[1], tot)) {
+        if (tid < K && ((mask >> tid) & 1u)) {
+            const double rho = tot[tid], rr = tot[KMAX + tid], bb = tot[2 * KMAX + tid];
+            ctrl->c[tid] = sp.c[tid]; ctrl->field[tid] = sp.field[tid]; ctrl->rhs[tid] = sp.rhs[tid];
+            ctrl->rho[tid] = rho; ctrl->rr[tid] = rr; ctrl->bb[tid] = bb;
+            ctrl->alpha[tid] = 0.0; ctrl->beta[tid] = 0.0; ctrl->iters[tid] = 0;
+            int st = 0;
+            int dn = (sp.field[tid] < 0) || (rr <= ctrl->tol2 * bb);
+            if (!isfinite(rr) || !isfinite(bb)) { dn = 1; st = 2; }
+            ctrl->status[tid] = st;
+            ctrl->epoch[tid] = ctrl->epoch[tid] + 1;
+            ctrl->done[tid] = dn;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int any = 0;
+            for (int c = 0; c < K; ++c) any |= !ctrl->done[c];
+            ctrl->all_done = !any;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------- kernel B
+// z -= alpha q/d ; rho' = sum d z^2 ; ||r||^2 = sum (d z)^2 ; then (last block) beta, stop tests.
+template <int K>
+__global__ void __launch_bounds__(BLOCK, 4) k_update(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+                                                     double* __restrict__ z, const double* __restrict__ q, int order_n) {
+    constexpr int TPR = K / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    constexpr int U = 4;
+    if (ctrl->all_done) return;
+    const int tid = threadIdx.x, l = tid % TPR;
+    const double2 cc = ld2(ctrl->c, 2 * l);
+    const double2 alpha = ld2(ctrl->alpha, 2 * l);
+    const double* __restrict__ dg = order_n == 1 ? m.sdiag : m.gdiag;
+    double2 acc[2] = {{0.0, 0.0}, {0.0, 0.0}};
+    const int64_t stride = (int64_t)gridDim.x * ROWS;
+    for (int64_t base = (int64_t)blockIdx.x * ROWS + tid / TPR; base < m.nv; base += U * stride) {
+        double2 zv[U], qv[U];
+        double av[U], dv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t row = base + u * stride;
+            if (row < m.nv) {
+                zv[u] = ld2(z, row * K + 2 * l);
+                qv[u] = ld2(q, row * K + 2 * l);
+                av[u] = m.area[row];
+                dv[u] = dg[row];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t row = base + u * stride;
+            if (row < m.nv) {
+                const double2 d = {fma(cc.x, dv[u], av[u]), fma(cc.y, dv[u], av[u])};
+                zv[u].x -= alpha.x * qv[u].x / d.x;
+                zv[u].y -= alpha.y * qv[u].y / d.y;
+                st2(z, row * K + 2 * l, zv[u]);
+                const double2 r = {d.x * zv[u].x, d.y * zv[u].y};
+                acc[0].x = fma(r.x, zv[u].x, acc[0].x); acc[0].y = fma(r.y, zv[u].y, acc[0].y);
+                acc[1].x = fma(r.x, r.x, acc[1].x);     acc[1].y = fma(r.y, r.y, acc[1].y);
+            }
+        }
+    }
+    __shared__ double tot[2 * KMAX];
+    if (grid_reduce<K, 2>(acc, partials, &ctrl->ticket[2], tot)) {
+        __shared__ int any_active;
+        if (tid == 0) any_active = 0;
+        __syncthreads();
+        if (tid < K) {
+            if (!ctrl->done[tid]) {
+                const double rho_new = tot[tid], rr = tot[KMAX + tid];
+                const int it = ctrl->iters[tid] + 1;
+                ctrl->iters[tid] = it;
+                ctrl->rr[tid] = rr;
+                double be = rho_new / ctrl->rho[tid];
+                ctrl->rho[tid] = rho_new;
+                int dn = 0;
+                if (!isfinite(rr)) { dn = 1; ctrl->status[tid] = 2; }
+                else if (rr <= ctrl->tol2 * ctrl->bb[tid]) { dn = 1; ctrl->status[tid] = 0; }
+                else if (!isfinite(be)) { dn = 1; ctrl->status[tid] = 2; }
+                else if (it >= ctrl->max_iter) { dn = 1; ctrl->status[tid] = 1; }
+                if (dn) { be = 0.0; ctrl->done[tid] = 1; }
+                ctrl->beta[tid] = be;
+                if (!dn) atomicOr(&any_active, 1);
+            } else {
+                ctrl->beta[tid] = 0.0;
+            }
+        }
+        __syncthreads();
+        if (tid == 0) { ctrl->all_done = !any_active; ctrl->total_iters += 1; }
+    }
+}
+
+// ------------------------------------------------------------------------------------------- end of a column
+// H6b for the columns in `mask`: x_final = x + alpha p (the update still pending, alpha = 0 once applied),
+// e_c = 1/2 sum_v A_v x_v^2 / sum_v A_v
+template <int K>
+__global__ void __launch_bounds__(BLOCK) k_energy(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+                                                  unsigned mask, const double* __restrict__ x,
+                                                  const double* __restrict__ pa, const double* __restrict__ pb,
+                                                  double total_area, double* __restrict__ energy) {
+    constexpr int TPR = K / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    const int tid = threadIdx.x, l = tid % TPR;
+    const double* __restrict__ p = ctrl->cur_p ? pb : pa;
+    const double2 alpha = ld2(ctrl->alpha, 2 * l);
+    double2 acc[1] = {{0.0, 0.0}};
+    if ((mask >> (2 * l)) & 3u) {
+        for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < m.nv; row += (int64_t)gridDim.x * ROWS) {
+            const int64_t ri = row * K + 2 * l;
+            const double av = m.area[row];
+            const double2 xv = ld2(x, ri), pv = ld2(p, ri);
+            const double2 xf = {fma(alpha.x, pv.x, xv.x), fma(alpha.y, pv.y, xv.y)};
+            acc[0].x = fma(av * xf.x, xf.x, acc[0].x);
+            acc[0].y = fma(av * xf.y, xf.y, acc[0].y);
+        }
+    }
+    __shared__ double tot[KMAX];
+    if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[3], tot)) {
+        if (tid < K && ((mask >> tid) & 1u) && ctrl->field[tid] >= 0)
+            energy[ctrl->rhs[tid]] = 0.5 * tot[tid] / total_area;
+    }
+}
+
+// H6a for the columns in `mask`: x_final scattered back to the caller's numbering: out[rhs][perm[row]]
+template <int K>
+__global__ void __launch_bounds__(BLOCK) k_scatter(MeshView m, const Ctrl* __restrict__ ctrl, unsigned mask,
+                                                   const double* __restrict__ x, const double* __restrict__ pa,
+                                                   const double* __restrict__ pb, int use_p, double* __restrict__ out) {
+    __shared__ double tile[K][33];
+    __shared__ int32_t dst[32];
+    const int tid = threadIdx.x;
+    const double* __restrict__ p = ctrl->cur_p ? pb : pa;
+    // BLOCK threads move 32 rows x K columns per step
+    for (int64_t base = (int64_t)blockIdx.x * 32; base < m.nv; base += (int64_t)gridDim.x * 32) {
+        for (int e = tid; e < 32 * K; e += BLOCK) {
+            const int r = e / K, c = e % K;
+            const int64_t row = base + r;
+            double v = 0.0;
+            if (row < m.nv && ((mask >> c) & 1u)) {
+                v = x[row * K + c];
+                if (use_p) v = fma(ctrl->alpha[c], p[row * K + c], v);
+            }
+            tile[c][r] = v;
+        }
+        if (tid < 32) dst[tid] = base + tid < m.nv ? m.perm[base + tid] : -1;
+        __syncthreads();
+        for (int e = tid; e < 32 * K; e += BLOCK) {
+            const int c = e / 32, r = e % 32;
+            if (((mask >> c) & 1u) && ctrl->field[c] >= 0 && dst[r] >= 0)
+                out[(int64_t)ctrl->rhs[c] * m.nv + dst[r]] = tile[c][r];
+        }
+        __syncthreads();
+    }
+}
+
+// per-right-hand-side results of the columns in `mask`
+__global__ void k_stats(const Ctrl* __restrict__ ctrl, int K, unsigned mask, int32_t* __restrict__ iters,
+                        int32_t* __restrict__ status, double* __restrict__ relres) {
+    const int c = threadIdx.x;
+    if (c < K && ((mask >> c) & 1u) && ctrl->field[c] >= 0) {
+        const int r = ctrl->rhs[c];
+        iters[r] = ctrl->iters[c];
+        status[r] = ctrl->status[c];
+        relres[r] = ctrl->bb[c] > 0.0 ? sqrt(ctrl->rr[c] / ctrl->bb[c]) : 0.0;
+    }
+}
+
+// H7: k_j = 1/l_j ; E_j = (e_j - e_j+1)/(k_j - k_j+1) ; k_mid_j = sqrt(k_j k_j+1)
+__global__ void k_spectrum(const double* __restrict__ energy, const double* __restrict__ ells, int n_fields, int n_ells,
+                           double* __restrict__ k_mid, double* __restrict__ E) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nb = n_ells - 1;
+    if (i >= n_fields * nb) return;
+    const int f = i / nb, j = i % nb;
+    const double k0 = 1.0 / ells[j], k1 = 1.0 / ells[j + 1];
+    E[i] = (energy[f * n_ells + j] - energy[f * n_ells + j + 1]) / (k0 - k1);
+    if (f == 0) k_mid[j] = sqrt(k0 * k1);
+}
+
+}  // namespace
+}  // namespace ifl

@@ -1,430 +1,20 @@
-// Solving phase: batched multi-right-hand-side Jacobi-PCG on
-//     A_c x_c = M phi_c,   A_c = M + c_c S (M^-1 S)^(n-1),   c_c = gamma l_c^(2n)
-// for K = 4, 8 or 16 columns c at once, every column with its own scale l_c, field, alpha, beta and stop time.
-//
-// Layout: work vectors are [row][K] fp64 (K = 16: one 128-byte line per row), rows in the internal order.
-// A row is handled by K/2 threads, each owning two adjacent columns (double2 = 16-byte loads/stores), so a warp
-// covers 64/K rows and every gather of a neighbour row is one contiguous K*8-byte segment.
-//
-// CG is carried in the preconditioned residual z = r/d (d = diag(A_c), Jacobi):
-//   kernel A (k_spmm, fused):  p' = z + beta p ;  x += alpha_prev p ;  q = A_c p' ;  partial p'.q
-//                              the gather recomputes p'_j = z_j + beta p_j at the neighbours, p is double-buffered
-//   kernel B (k_update):       z -= alpha q/d ;  partial rho' = sum d z^2 = r.z  and  ||r||^2 = sum (d z)^2
-// Per-column scalars (alpha, beta, rho, done flags) live in a device control block and are produced by the
-// last block to finish each kernel (single-pass, fixed-order, deterministic grid reduction); the host only polls
-// one flag every `check_every` iterations, one CUDA graph launch behind.
+// Solving phase, host side: queue of (field, scale) right-hand sides, K columns in flight,
+// CUDA-graph iteration loop polled every `check_every` iterations, converged columns finalised and refilled
+// from the queue.  The device code is in kernels.cuh.
 #include <algorithm>
 #include <cmath>
+#include <cstddef>
 #include <cstring>
 #include <vector>
 
-#include "common.cuh"
+#include "kernels.cuh"
 
 namespace ifl {
 namespace {
 
-constexpr int KMAX = 16;
-constexpr int BLOCK = 256;
 constexpr int MAX_RHS = 65536;
+constexpr int MAX_BLOCKS_PER_SM = 8;
 
-struct MeshView {
-    const int64_t* __restrict__ chunk_ptr;
-    const int32_t* __restrict__ col;
-    const double* __restrict__ val;
-    const double* __restrict__ area;
-    const double* __restrict__ inv_area;
-    const double* __restrict__ sdiag;
-    const double* __restrict__ gdiag;
-    const int32_t* __restrict__ perm;
-    int64_t nv;
-    int log2c;
-};
-
-struct Ctrl {
-    double c[KMAX];       // gamma l^(2n)
-    double alpha[KMAX];
-    double beta[KMAX];
-    double rho[KMAX];
-    double bb[KMAX];      // ||M phi||^2
-    double rr[KMAX];      // ||r||^2 (recursive)
-    int field[KMAX];      // field of the column, -1 = unused column
-    int rhs[KMAX];        // f * n_ells + j of the column
-    int done[KMAX];
-    int status[KMAX];
-    int iters[KMAX];
-    int all_done;
-    int cur_p;            // which direction buffer the last kernel A wrote
-    int max_iter;
-    int pad_;
-    double tol2;
-    unsigned int ticket[4];
-};
-
-enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3 };
-
-__device__ __forceinline__ double2 ld2(const double* __restrict__ p, int64_t i) {
-    return *reinterpret_cast<const double2*>(p + i);
-}
-__device__ __forceinline__ void st2(double* __restrict__ p, int64_t i, double2 v) {
-    *reinterpret_cast<double2*>(p + i) = v;
-}
-
-// Fixed-order block reduction of NV double2 accumulators per thread over the threads owning the same column
-// pair, then a ticket: the last block to arrive sums all blocks' partials in block order.
-// Returns true in the last block, with the totals of value set j, column c in tot[j*KMAX + c] (shared memory).
-template <int K, int NV>
-__device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __restrict__ partials,
-                                            unsigned int* ticket, double* tot /* shared [NV*KMAX] */) {
-    constexpr int TPR = K / 2;
-    __shared__ double2 red[BLOCK];
-    __shared__ bool is_last;
-    const int tid = threadIdx.x;
-    for (int j = 0; j < NV; ++j) {
-        red[tid] = acc[j];
-        __syncthreads();
-        if (tid < TPR) {
-            double2 s = red[tid];
-            for (int i = tid + TPR; i < BLOCK; i += TPR) { s.x += red[i].x; s.y += red[i].y; }
-            partials[((size_t)j * gridDim.x + blockIdx.x) * K + 2 * tid] = s.x;
-            partials[((size_t)j * gridDim.x + blockIdx.x) * K + 2 * tid + 1] = s.y;
-        }
-        __syncthreads();
-    }
-    if (tid == 0) {
-        __threadfence();
-        unsigned int t = atomicAdd(ticket, 1u);
-        is_last = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!is_last) return false;
-    __threadfence();
-    double* redd = reinterpret_cast<double*>(red);   // [BLOCK] doubles (uses half of red)
-    constexpr int LANES = BLOCK / K;                  // threads per column
-    for (int j = 0; j < NV; ++j) {
-        const int c = tid % K, lane = tid / K;
-        double s = 0.0;
-        for (unsigned b = lane; b < gridDim.x; b += LANES)
-            s += __ldcg(&partials[((size_t)j * gridDim.x + b) * K + c]);
-        redd[tid] = s;
-        __syncthreads();
-        if (tid < K) {
-            double t = 0.0;
-            for (int i = 0; i < LANES; ++i) t += redd[i * K + tid];
-            tot[j * KMAX + tid] = t;
-        }
-        __syncthreads();
-    }
-    if (tid == 0) *ticket = 0u;
-    return true;
-}
-
-struct SpmmArgs {
-    const double* in0;   // PLAIN: x        CG1/CG2A: z        CG2B: t
-    const double* in1;   //                 CG1/CG2A: p_old    CG2B: p (current)
-    double* x;           //                 CG1/CG2A: x (in place)
-    double* out0;        // PLAIN: y        CG1: q             CG2A: t            CG2B: q
-    double* out1;        //                 CG1/CG2A: p_new
-    int scale_inv_area;  // PLAIN: multiply the row result by 1/A_v
-    int out_idx;         // CG1/CG2A: index of the direction buffer written (recorded in ctrl->cur_p)
-};
-
-template <int K, int MODE>
-__global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
-                                                SpmmArgs a, int64_t rows_per_block) {
-    constexpr int TPR = K / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    if (MODE != MODE_PLAIN && ctrl->all_done) return;
-    const int tid = threadIdx.x;
-    const int l = tid % TPR;
-    const int64_t r0 = (int64_t)blockIdx.x * rows_per_block;
-    const int64_t r1 = min(r0 + rows_per_block, m.nv);
-    double2 beta = {0.0, 0.0}, alpha = {0.0, 0.0}, cc = {0.0, 0.0};
-    if (MODE != MODE_PLAIN) {
-        beta = ld2(ctrl->beta, 2 * l);
-        alpha = ld2(ctrl->alpha, 2 * l);
-        cc = ld2(ctrl->c, 2 * l);
-    }
-    double2 acc[1] = {{0.0, 0.0}};
-    const int C = 1 << m.log2c;
-    for (int64_t row = r0 + tid / TPR; row < r1; row += ROWS) {
-        const int64_t ch = row >> m.log2c;
-        const int64_t cp0 = m.chunk_ptr[ch];
-        const int w = (int)((m.chunk_ptr[ch + 1] - cp0) >> m.log2c);
-        const int64_t o = cp0 + (row & (C - 1)) * w;
-        const int64_t ri = row * K + 2 * l;
-        // own row
-        double2 own;   // the vector the operator is applied to, at this row
-        if (MODE == MODE_CG1 || MODE == MODE_CG2A) {
-            double2 zv = ld2(a.in0, ri), pv = ld2(a.in1, ri), xv = ld2(a.x, ri);
-            own.x = fma(beta.x, pv.x, zv.x);
-            own.y = fma(beta.y, pv.y, zv.y);
-            xv.x = fma(alpha.x, pv.x, xv.x);
-            xv.y = fma(alpha.y, pv.y, xv.y);
-            st2(a.x, ri, xv);
-            st2(a.out1, ri, own);
-        } else {
-            own = ld2(a.in0, ri);
-        }
-        // off-diagonal gather
-        double2 s = {0.0, 0.0};
-        for (int k = 0; k < w; k += 2) {
-            const int2 cj = *reinterpret_cast<const int2*>(m.col + o + k);
-            const double2 vj = ld2(m.val, o + k);
-            const int64_t j0 = (int64_t)cj.x * K + 2 * l, j1 = (int64_t)cj.y * K + 2 * l;
-            double2 g0, g1;
-            if (MODE == MODE_CG1 || MODE == MODE_CG2A) {
-                double2 z0 = ld2(a.in0, j0), p0 = ld2(a.in1, j0), z1 = ld2(a.in0, j1), p1 = ld2(a.in1, j1);
-                g0.x = fma(beta.x, p0.x, z0.x); g0.y = fma(beta.y, p0.y, z0.y);
-                g1.x = fma(beta.x, p1.x, z1.x); g1.y = fma(beta.y, p1.y, z1.y);
-            } else {
-                g0 = ld2(a.in0, j0);
-                g1 = ld2(a.in0, j1);
-            }
-            s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
-            s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
-        }
-        const double sd = m.sdiag[row];
-        s.x = fma(sd, own.x, s.x);
-        s.y = fma(sd, own.y, s.y);          // s = (S v)_row
-        if (MODE == MODE_PLAIN) {
-            if (a.scale_inv_area) { const double ia = m.inv_area[row]; s.x *= ia; s.y *= ia; }
-            st2(a.out0, ri, s);
-        } else if (MODE == MODE_CG2A) {
-            const double ia = m.inv_area[row];
-            s.x *= ia; s.y *= ia;            // t = M^-1 S p'
-            st2(a.out0, ri, s);
-        } else {
-            // q = A_v p + c (S v)_row ; v = p (n = 1) or t (n = 2)
-            const double av = m.area[row];
-            double2 pv = (MODE == MODE_CG1) ? own : ld2(a.in1, ri);
-            double2 q;
-            q.x = fma(cc.x, s.x, av * pv.x);
-            q.y = fma(cc.y, s.y, av * pv.y);
-            st2(a.out0, ri, q);
-            acc[0].x = fma(pv.x, q.x, acc[0].x);
-            acc[0].y = fma(pv.y, q.y, acc[0].y);
-        }
-    }
-    if (MODE == MODE_CG1 || MODE == MODE_CG2B) {
-        __shared__ double tot[KMAX];
-        if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[0], tot)) {
-            if (tid < K) {
-                const double pq = tot[tid];
-                double al = 0.0;
-                if (!ctrl->done[tid]) {
-                    if (pq > 0.0 && isfinite(pq)) al = ctrl->rho[tid] / pq;
-                    else { ctrl->done[tid] = 1; ctrl->status[tid] = 2; }
-                }
-                ctrl->alpha[tid] = al;
-            }
-        }
-    }
-    if ((MODE == MODE_CG1 || MODE == MODE_CG2A) && blockIdx.x == 0 && tid == 0) ctrl->cur_p = a.out_idx;
-}
-
-// x[row][c] = field_c[perm[row]]  (H0 ingest: gather through the permutation, replicate per scale, transpose)
-template <int K>
-__global__ void __launch_bounds__(BLOCK) k_ingest(MeshView m, const Ctrl* __restrict__ ctrl,
-                                                  const double* __restrict__ fields, double* __restrict__ x) {
-    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
-    if (i >= m.nv * K) return;
-    const int64_t row = i / K;
-    const int c = (int)(i % K);
-    const int f = ctrl->field[c];
-    x[i] = f >= 0 ? fields[(int64_t)f * m.nv + m.perm[row]] : 0.0;
-}
-
-// Start of CG from x0 = phi: y = S (M^-1 S)^(n-1) phi is given;
-// r0 = M phi - A_c phi = -c y ;  z0 = r0/d ;  p = 0 ;  rho0 = r0.z0 ;  ||r0||^2 ;  ||M phi||^2.
-template <int K>
-__global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
-                                                const double* __restrict__ x, const double* __restrict__ y,
-                                                double* __restrict__ z, double* __restrict__ p0, int order_n,
-                                                int64_t rows_per_block) {
-    constexpr int TPR = K / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    const int tid = threadIdx.x, l = tid % TPR;
-    const int64_t r0 = (int64_t)blockIdx.x * rows_per_block;
-    const int64_t r1 = min(r0 + rows_per_block, m.nv);
-    const double2 cc = ld2(ctrl->c, 2 * l);
-    const double* __restrict__ dg = order_n == 1 ? m.sdiag : m.gdiag;
-    double2 acc[3] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
-    for (int64_t row = r0 + tid / TPR; row < r1; row += ROWS) {
-        const int64_t ri = row * K + 2 * l;
-        const double av = m.area[row], dv = dg[row];
-        const double2 d = {fma(cc.x, dv, av), fma(cc.y, dv, av)};
-        const double2 xv = ld2(x, ri), yv = ld2(y, ri);
-        const double2 r = {-cc.x * yv.x, -cc.y * yv.y};
-        const double2 zv = {r.x / d.x, r.y / d.y};
-        st2(z, ri, zv);
-        st2(p0, ri, make_double2(0.0, 0.0));
-        acc[0].x = fma(r.x, zv.x, acc[0].x); acc[0].y = fma(r.y, zv.y, acc[0].y);
-        acc[1].x = fma(r.x, r.x, acc[1].x);  acc[1].y = fma(r.y, r.y, acc[1].y);
-        const double2 b = {av * xv.x, av * xv.y};
-        acc[2].x = fma(b.x, b.x, acc[2].x);  acc[2].y = fma(b.y, b.y, acc[2].y);
-    }
-    __shared__ double tot[3 * KMAX];
-    if (grid_reduce<K, 3>(acc, partials, &ctrl->ticket[1], tot)) {
-        __shared__ int any_active;
-        if (tid == 0) any_active = 0;
-        __syncthreads();
-        if (tid < K) {
-            const double rho = tot[tid], rr = tot[KMAX + tid], bb = tot[2 * KMAX + tid];
-            ctrl->rho[tid] = rho; ctrl->rr[tid] = rr; ctrl->bb[tid] = bb;
-            ctrl->alpha[tid] = 0.0; ctrl->beta[tid] = 0.0; ctrl->iters[tid] = 0;
-            int st = 0;
-            int dn = (ctrl->field[tid] < 0) || (rr <= ctrl->tol2 * bb);
-            if (!isfinite(rr) || !isfinite(bb)) { dn = 1; st = 2; }
-            ctrl->done[tid] = dn; ctrl->status[tid] = st;
-            if (!dn) atomicOr(&any_active, 1);
-        }
-        __syncthreads();
-        if (tid == 0) { ctrl->all_done = !any_active; ctrl->cur_p = 0; }
-    }
-}
-
-// kernel B: z -= alpha q/d ; rho' = sum d z^2 ; ||r||^2 = sum (d z)^2 ; then (last block) beta, stop tests.
-template <int K>
-__global__ void __launch_bounds__(BLOCK) k_update(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
-                                                  double* __restrict__ z, const double* __restrict__ q, int order_n,
-                                                  int64_t rows_per_block) {
-    constexpr int TPR = K / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    if (ctrl->all_done) return;
-    const int tid = threadIdx.x, l = tid % TPR;
-    const int64_t r0 = (int64_t)blockIdx.x * rows_per_block;
-    const int64_t r1 = min(r0 + rows_per_block, m.nv);
-    const double2 cc = ld2(ctrl->c, 2 * l);
-    const double2 alpha = ld2(ctrl->alpha, 2 * l);
-    const double* __restrict__ dg = order_n == 1 ? m.sdiag : m.gdiag;
-    double2 acc[2] = {{0.0, 0.0}, {0.0, 0.0}};
-#pragma unroll 2
-    for (int64_t row = r0 + tid / TPR; row < r1; row += ROWS) {
-        const int64_t ri = row * K + 2 * l;
-        const double av = m.area[row], dv = dg[row];
-        const double2 d = {fma(cc.x, dv, av), fma(cc.y, dv, av)};
-        double2 zv = ld2(z, ri);
-        const double2 qv = ld2(q, ri);
-        zv.x -= alpha.x * qv.x / d.x;
-        zv.y -= alpha.y * qv.y / d.y;
-        st2(z, ri, zv);
-        const double2 r = {d.x * zv.x, d.y * zv.y};
-        acc[0].x = fma(r.x, zv.x, acc[0].x); acc[0].y = fma(r.y, zv.y, acc[0].y);
-        acc[1].x = fma(r.x, r.x, acc[1].x);  acc[1].y = fma(r.y, r.y, acc[1].y);
-    }
-    __shared__ double tot[2 * KMAX];
-    if (grid_reduce<K, 2>(acc, partials, &ctrl->ticket[2], tot)) {
-        __shared__ int any_active;
-        if (tid == 0) any_active = 0;
-        __syncthreads();
-        if (tid < K) {
-            if (!ctrl->done[tid]) {
-                const double rho_new = tot[tid], rr = tot[KMAX + tid];
-                const int it = ctrl->iters[tid] + 1;
-                ctrl->iters[tid] = it;
-                ctrl->rr[tid] = rr;
-                double be = rho_new / ctrl->rho[tid];
-                ctrl->rho[tid] = rho_new;
-                int dn = 0;
-                if (!isfinite(rr)) { dn = 1; ctrl->status[tid] = 2; }
-                else if (rr <= ctrl->tol2 * ctrl->bb[tid]) { dn = 1; ctrl->status[tid] = 0; }
-                else if (!isfinite(be)) { dn = 1; ctrl->status[tid] = 2; }
-                else if (it >= ctrl->max_iter) { dn = 1; ctrl->status[tid] = 1; }
-                if (dn) { be = 0.0; ctrl->done[tid] = 1; }
-                ctrl->beta[tid] = be;
-                if (!dn) atomicOr(&any_active, 1);
-            } else {
-                ctrl->beta[tid] = 0.0;
-            }
-        }
-        __syncthreads();
-        if (tid == 0) ctrl->all_done = !any_active;
-    }
-}
-
-// H6b: x_final = x + alpha p (the update still pending), e_c = 1/2 sum_v A_v x_v^2 / sum_v A_v
-template <int K>
-__global__ void __launch_bounds__(BLOCK) k_energy(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
-                                                  const double* __restrict__ x, const double* __restrict__ pa,
-                                                  const double* __restrict__ pb, double total_area,
-                                                  double* __restrict__ energy, int64_t rows_per_block) {
-    constexpr int TPR = K / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    const int tid = threadIdx.x, l = tid % TPR;
-    const int64_t r0 = (int64_t)blockIdx.x * rows_per_block;
-    const int64_t r1 = min(r0 + rows_per_block, m.nv);
-    const double* __restrict__ p = ctrl->cur_p ? pb : pa;
-    const double2 alpha = ld2(ctrl->alpha, 2 * l);
-    double2 acc[1] = {{0.0, 0.0}};
-    for (int64_t row = r0 + tid / TPR; row < r1; row += ROWS) {
-        const int64_t ri = row * K + 2 * l;
-        const double av = m.area[row];
-        const double2 xv = ld2(x, ri), pv = ld2(p, ri);
-        const double2 xf = {fma(alpha.x, pv.x, xv.x), fma(alpha.y, pv.y, xv.y)};
-        acc[0].x = fma(av * xf.x, xf.x, acc[0].x);
-        acc[0].y = fma(av * xf.y, xf.y, acc[0].y);
-    }
-    __shared__ double tot[KMAX];
-    if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[3], tot)) {
-        if (tid < K && ctrl->field[tid] >= 0) energy[ctrl->rhs[tid]] = 0.5 * tot[tid] / total_area;
-    }
-}
-
-// H6a: x_final scattered back to the caller's numbering: out[rhs][perm[row]]
-template <int K>
-__global__ void __launch_bounds__(BLOCK) k_scatter(MeshView m, const Ctrl* __restrict__ ctrl,
-                                                   const double* __restrict__ x, const double* __restrict__ pa,
-                                                   const double* __restrict__ pb, int use_p, double* __restrict__ out) {
-    __shared__ double tile[K][33];
-    __shared__ int32_t dst[32];
-    const int tid = threadIdx.x;
-    const double* __restrict__ p = ctrl->cur_p ? pb : pa;
-    // BLOCK threads move 32 rows x K columns per step
-    for (int64_t base = (int64_t)blockIdx.x * 32; base < m.nv; base += (int64_t)gridDim.x * 32) {
-        for (int e = tid; e < 32 * K; e += BLOCK) {
-            const int r = e / K, c = e % K;
-            const int64_t row = base + r;
-            double v = 0.0;
-            if (row < m.nv) {
-                v = x[row * K + c];
-                if (use_p) v = fma(ctrl->alpha[c], p[row * K + c], v);
-            }
-            tile[c][r] = v;
-        }
-        if (tid < 32) dst[tid] = base + tid < m.nv ? m.perm[base + tid] : -1;
-        __syncthreads();
-        for (int e = tid; e < 32 * K; e += BLOCK) {
-            const int c = e / 32, r = e % 32;
-            if (ctrl->field[c] >= 0 && dst[r] >= 0) out[(int64_t)ctrl->rhs[c] * m.nv + dst[r]] = tile[c][r];
-        }
-        __syncthreads();
-    }
-}
-
-__global__ void k_stats(const Ctrl* __restrict__ ctrl, int K, int32_t* __restrict__ iters, int32_t* __restrict__ status,
-                        double* __restrict__ relres) {
-    const int c = threadIdx.x;
-    if (c < K && ctrl->field[c] >= 0) {
-        const int r = ctrl->rhs[c];
-        iters[r] = ctrl->iters[c];
-        status[r] = ctrl->status[c];
-        relres[r] = ctrl->bb[c] > 0.0 ? sqrt(ctrl->rr[c] / ctrl->bb[c]) : 0.0;
-    }
-}
-
-// H7: k_j = 1/l_j ; E_j = (e_j - e_j+1)/(k_j - k_j+1) ; k_mid_j = sqrt(k_j k_j+1)
-__global__ void k_spectrum(const double* __restrict__ energy, const double* __restrict__ ells, int n_fields, int n_ells,
-                           double* __restrict__ k_mid, double* __restrict__ E) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int nb = n_ells - 1;
-    if (i >= n_fields * nb) return;
-    const int f = i / nb, j = i % nb;
-    const double k0 = 1.0 / ells[j], k1 = 1.0 / ells[j + 1];
-    E[i] = (energy[f * n_ells + j] - energy[f * n_ells + j + 1]) / (k0 - k1);
-    if (f == 0) k_mid[j] = sqrt(k0 * k1);
-}
-
-// ------------------------------------------------------------------------------------------- host side
 struct Workspace {
     Ctrl* ctrl;
     double* partials;
@@ -442,7 +32,7 @@ Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* bas
     size_t off = 0;
     auto take = [&](size_t bytes) { void* r = p ? p + off : nullptr; off += align_up(bytes); return r; };
     const size_t vec = (size_t)h->n_vert * batch * sizeof(double);
-    const size_t gmax = (size_t)h->n_sm * 8;
+    const size_t gmax = (size_t)h->n_sm * MAX_BLOCKS_PER_SM;
     w.ctrl = (Ctrl*)take(sizeof(Ctrl));
     w.partials = (double*)take(3 * gmax * KMAX * sizeof(double));
     w.x = (double*)take(vec);
@@ -462,20 +52,12 @@ Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* bas
     return w;
 }
 
-struct Geo { int grid; int64_t rows_per_block; };
-
-Geo geometry(int64_t nv, int K, int n_sm, int blocks_per_sm) {
-    const int rows = BLOCK / (K / 2);
-    const int64_t nblk = (nv + rows - 1) / rows;
-    int64_t grid = std::min<int64_t>(nblk, (int64_t)n_sm * blocks_per_sm);
-    const int64_t rpb = (nblk + grid - 1) / grid * rows;
-    grid = (nv + rpb - 1) / rpb;
-    return Geo{(int)grid, rpb};
-}
-
 enum Job { JOB_FILTER, JOB_SPECTRUM, JOB_APPLY };
 
 struct Rhs { double ell; int f; int j; };
+
+// persistent grids: one wave of resident blocks, sized from the real occupancy of each kernel
+struct Grids { int plain, cga, cgb, update, stream; };
 
 struct Run {
     const if_mesh_s* h;
@@ -484,7 +66,49 @@ struct Run {
     cudaStream_t st;
     int order_n;
     Options opt;
+    Grids g;
 };
+
+template <class Kern>
+int resident_grid(Kern kern, size_t smem, int n_sm, int64_t work_items, int* grid) {
+    if (smem > 0)   // static + dynamic shared memory may pass 48 KB: always opt in
+        IF_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    IF_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLOCK, smem));
+    if (occ < 1) {
+        fprintf(stderr, "[implicit_filter] kernel does not fit an SM (dynamic shared memory %zu bytes)\n", smem);
+        return IF_ECUDA;
+    }
+    occ = std::min(occ, MAX_BLOCKS_PER_SM);
+    *grid = (int)std::max<int64_t>(1, std::min<int64_t>(work_items, (int64_t)n_sm * occ));
+    return IF_OK;
+}
+
+template <int K>
+int setup_grids(Run& r) {
+    const int64_t nv = r.h->n_vert;
+    const int n_sm = r.h->n_sm;
+    const int64_t tiles = (nv + TileRows<K>::T - 1) / TileRows<K>::T;
+    const int64_t passes = (nv + BLOCK / (K / 2) - 1) / (BLOCK / (K / 2));
+    int rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_PLAIN>, TileSmem<K, MODE_PLAIN>::bytes, n_sm, tiles, &r.g.plain))) return rc;
+    if (r.order_n == 1) {
+        if ((rc = resident_grid(k_spmm<K, MODE_CG1>, TileSmem<K, MODE_CG1>::bytes, n_sm, tiles, &r.g.cga))) return rc;
+    } else {
+        if ((rc = resident_grid(k_spmm<K, MODE_CG2A>, TileSmem<K, MODE_CG2A>::bytes, n_sm, tiles, &r.g.cga))) return rc;
+    }
+    if ((rc = resident_grid(k_spmm<K, MODE_CG2B>, TileSmem<K, MODE_CG2B>::bytes, n_sm, tiles, &r.g.cgb))) return rc;
+    if ((rc = resident_grid(k_update<K>, 0, n_sm, passes, &r.g.update))) return rc;
+    r.g.stream = (int)std::max<int64_t>(1, std::min<int64_t>(passes, (int64_t)n_sm * 4));
+    return IF_OK;
+}
+
+template <int K, int MODE>
+int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
+    k_spmm<K, MODE><<<grid, BLOCK, TileSmem<K, MODE>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
+    IF_LAUNCH_CHECK();
+    return IF_OK;
+}
 
 // Events recorded (as external event-record nodes) around one SpMM and one update launch of a captured graph,
 // so that the per-launch duration of both kernels is measured live on the launching stream (if_stats).
@@ -505,8 +129,9 @@ struct TimingEvents {
 };
 
 template <int K>
-int enqueue_two_iterations(const Run& r, const Geo& g, const TimingEvents* tev = nullptr) {
+int enqueue_two_iterations(const Run& r, const TimingEvents* tev = nullptr) {
     // iteration with p0 -> p1, then p1 -> p0
+    int rc;
     for (int half = 0; half < 2; ++half) {
         const bool timed = tev && half == 0;
         if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s0, r.st, cudaEventRecordExternal));
@@ -514,19 +139,15 @@ int enqueue_two_iterations(const Run& r, const Geo& g, const TimingEvents* tev =
         double* pnew = half == 0 ? r.w.p1 : r.w.p0;
         if (r.order_n == 1) {
             SpmmArgs a{r.w.z, pold, r.w.x, r.w.q, pnew, 0, half == 0 ? 1 : 0};
-            k_spmm<K, MODE_CG1><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, a, g.rows_per_block);
-            IF_LAUNCH_CHECK();
+            if ((rc = launch_spmm<K, MODE_CG1>(r, r.g.cga, a))) return rc;
         } else {
             SpmmArgs a{r.w.z, pold, r.w.x, r.w.t, pnew, 0, half == 0 ? 1 : 0};
-            k_spmm<K, MODE_CG2A><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, a, g.rows_per_block);
-            IF_LAUNCH_CHECK();
+            if ((rc = launch_spmm<K, MODE_CG2A>(r, r.g.cga, a))) return rc;
             SpmmArgs b{r.w.t, pnew, nullptr, r.w.q, nullptr, 0, 0};
-            k_spmm<K, MODE_CG2B><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, b, g.rows_per_block);
-            IF_LAUNCH_CHECK();
+            if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
         }
         if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s1, r.st, cudaEventRecordExternal));
-        k_update<K><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.z, r.w.q, r.order_n,
-                                                g.rows_per_block);
+        k_update<K><<<r.g.update, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.z, r.w.q, r.order_n);
         IF_LAUNCH_CHECK();
         if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->u1, r.st, cudaEventRecordExternal));
     }
@@ -546,153 +167,229 @@ struct GraphSet {
 struct KernelTimes { double spmm_ms = 0.0, update_ms = 0.0; int64_t samples = 0; };
 
 struct PollState {
-    int* flags = nullptr;          // pinned [4]
+    Snapshot* snap = nullptr;          // pinned [4]
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool own_pinned = false;
     if_mesh_s* h = nullptr;
     ~PollState() {
         for (auto& e : ev) if (e) cudaEventDestroy(e);
-        if (own_pinned && flags) cudaFreeHost(flags);
+        if (own_pinned && snap) cudaFreeHost(snap);
         else if (h) h->pinned_busy.store(0);
     }
 };
 
+// (Re)start the columns in `mask` from their right-hand sides: ingest, y = S (M^-1 S)^(n-1) phi, CG start.
 template <int K>
-int solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, size_t first, size_t count,
-                int n_ells, double* d_out, PollState& poll, int blocks_per_sm, GraphSet* graph_cache,
-                int64_t* batch_iters, KernelTimes* times) {
+int start_columns(const Run& r, unsigned mask, const StartParams& sp, const double* d_fields) {
     const if_mesh_s* h = r.h;
-    const Geo g = geometry(h->n_vert, K, h->n_sm, blocks_per_sm);
+    const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
+    int rc;
+    k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, sp, mask, d_fields, r.w.x);
+    IF_LAUNCH_CHECK();
+    if (r.order_n == 1) {
+        SpmmArgs a{r.w.x, nullptr, nullptr, r.w.q, nullptr, 0, 0};
+        if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, a))) return rc;
+    } else {
+        SpmmArgs a{r.w.x, nullptr, nullptr, r.w.t, nullptr, 1, 0};
+        if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, a))) return rc;
+        SpmmArgs b{r.w.t, nullptr, nullptr, r.w.q, nullptr, 0, 0};
+        if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, b))) return rc;
+    }
+    k_init<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, r.w.x, r.w.q, r.w.z, r.w.p0,
+                                              r.w.p1, r.order_n);
+    IF_LAUNCH_CHECK();
+    return IF_OK;
+}
+
+// The columns in `mask` have stopped: energy or scatter of x, and the per-right-hand-side results.
+template <int K>
+int finalize_columns(const Run& r, Job job, unsigned mask, double* d_out) {
+    const if_mesh_s* h = r.h;
+    if (job == JOB_SPECTRUM) {
+        k_energy<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, mask, r.w.x, r.w.p0, r.w.p1,
+                                                    h->total_area, r.w.energy);
+        IF_LAUNCH_CHECK();
+    } else {
+        const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
+        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, mask, r.w.x, r.w.p0, r.w.p1, 1, d_out);
+        IF_LAUNCH_CHECK();
+    }
+    k_stats<<<1, 32, 0, r.st>>>(r.w.ctrl, K, mask, r.w.iters, r.w.status, r.w.relres);
+    IF_LAUNCH_CHECK();
+    return IF_OK;
+}
+
+Ctrl fresh_ctrl(const Run& r) {
     Ctrl hc;
     memset(&hc, 0, sizeof(hc));
-    for (int c = 0; c < KMAX; ++c) { hc.field[c] = -1; hc.rhs[c] = 0; hc.done[c] = 1; }
-    for (size_t i = 0; i < count; ++i) {
-        const Rhs& q = rhs[first + i];
-        hc.c[i] = r.opt.gamma * std::pow(q.ell, 2.0 * r.order_n);
-        hc.field[i] = q.f;
-        hc.rhs[i] = q.f * n_ells + q.j;
-        hc.done[i] = 0;
-    }
+    for (int c = 0; c < KMAX; ++c) { hc.field[c] = -1; hc.done[c] = 1; }
+    hc.all_done = 1;
     hc.max_iter = r.opt.max_iter;
     hc.tol2 = r.opt.tol * r.opt.tol;
-    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
-    const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
-    k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, d_fields, r.w.x);
-    IF_LAUNCH_CHECK();
+    return hc;
+}
 
-    if (job == JOB_APPLY) {
+// if_apply: out = A_c phi for every right-hand side, K at a time (no iteration).
+template <int K>
+int apply_all(Run& r, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out) {
+    const if_mesh_s* h = r.h;
+    int rc;
+    if ((rc = setup_grids<K>(r))) return rc;
+    for (size_t first = 0; first < rhs.size(); first += K) {
+        const size_t count = std::min<size_t>(K, rhs.size() - first);
+        Ctrl hc = fresh_ctrl(r);
+        StartParams sp;
+        memset(&sp, 0, sizeof(sp));
+        for (int c = 0; c < KMAX; ++c) sp.field[c] = -1;
+        for (size_t i = 0; i < count; ++i) {
+            const Rhs& q = rhs[first + i];
+            hc.c[i] = sp.c[i] = r.opt.gamma * std::pow(q.ell, 2.0 * r.order_n);
+            hc.field[i] = sp.field[i] = q.f;
+            hc.rhs[i] = sp.rhs[i] = q.f * n_ells + q.j;
+        }
+        hc.all_done = 0;
+        IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
+        const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
+        k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, sp, (1u << K) - 1u, d_fields, r.w.x);
+        IF_LAUNCH_CHECK();
         const double* v = r.w.x;
         if (r.order_n == 2) {
             SpmmArgs a{r.w.x, nullptr, nullptr, r.w.t, nullptr, 1, 0};
-            k_spmm<K, MODE_PLAIN><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, a, g.rows_per_block);
-            IF_LAUNCH_CHECK();
+            if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, a))) return rc;
             v = r.w.t;
         }
         SpmmArgs b{v, r.w.x, nullptr, r.w.q, nullptr, 0, 0};
-        k_spmm<K, MODE_CG2B><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, b, g.rows_per_block);
-        IF_LAUNCH_CHECK();
-        k_scatter<K><<<std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8), BLOCK, 0, r.st>>>(
-            r.m, r.w.ctrl, r.w.q, r.w.p0, r.w.p1, 0, d_out);
-        IF_LAUNCH_CHECK();
-        return IF_OK;
-    }
-
-    // y = S (M^-1 S)^(n-1) phi  -> q
-    if (r.order_n == 1) {
-        SpmmArgs a{r.w.x, nullptr, nullptr, r.w.q, nullptr, 0, 0};
-        k_spmm<K, MODE_PLAIN><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, a, g.rows_per_block);
-        IF_LAUNCH_CHECK();
-    } else {
-        SpmmArgs a{r.w.x, nullptr, nullptr, r.w.t, nullptr, 1, 0};
-        k_spmm<K, MODE_PLAIN><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, a, g.rows_per_block);
-        IF_LAUNCH_CHECK();
-        SpmmArgs b{r.w.t, nullptr, nullptr, r.w.q, nullptr, 0, 0};
-        k_spmm<K, MODE_PLAIN><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, b, g.rows_per_block);
+        if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
+        const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
+        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, (1u << K) - 1u, r.w.q, r.w.p0, r.w.p1, 0, d_out);
         IF_LAUNCH_CHECK();
     }
-    k_init<K><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.x, r.w.q, r.w.z, r.w.p0, r.order_n,
-                                          g.rows_per_block);
-    IF_LAUNCH_CHECK();
+    return IF_OK;
+}
 
-    // the iteration loop: `check_every` iterations per CUDA graph launch, flag polled one launch behind
+// if_filter / if_spectrum: all right-hand sides through K columns with refill.
+template <int K>
+int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
+              PollState& poll, KernelTimes* times, int64_t* batch_iters) {
+    int rc;
+    if ((rc = setup_grids<K>(r))) return rc;
+    const size_t R = rhs.size();
+    Ctrl hc = fresh_ctrl(r);
+    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
+
+    int col_rhs[KMAX], host_epoch[KMAX];
+    size_t next = 0;
+    int active = 0;
+    auto assign = [&](unsigned mask, StartParams* sp, unsigned* started) {
+        memset(sp, 0, sizeof(*sp));
+        for (int c = 0; c < KMAX; ++c) sp->field[c] = -1;
+        *started = 0;
+        for (int c = 0; c < K; ++c) {
+            if (!((mask >> c) & 1u)) continue;
+            if (next < R) {
+                const Rhs& q = rhs[next];
+                sp->c[c] = r.opt.gamma * std::pow(q.ell, 2.0 * r.order_n);
+                sp->field[c] = q.f;
+                sp->rhs[c] = q.f * n_ells + q.j;
+                col_rhs[c] = (int)next++;
+                ++active;
+            } else {
+                col_rhs[c] = -1;
+            }
+            *started |= 1u << c;
+            host_epoch[c] += 1;
+        }
+    };
+    for (int c = 0; c < KMAX; ++c) { col_rhs[c] = -1; host_epoch[c] = 0; }
+    StartParams sp;
+    unsigned started = 0;
+    assign((1u << K) - 1u, &sp, &started);          // empty columns are started too (zeroed, done at once)
+    if ((rc = start_columns<K>(r, started, sp, d_fields))) return rc;
+
+    // the iteration loop: `check_every` iterations per CUDA graph launch, snapshot polled one launch behind
     const int pairs = r.opt.check_every / 2;
     const int launches_per_graph = pairs * 2 * (r.order_n == 1 ? 2 : 3);
-    GraphSet& gs = *graph_cache;
-    if (!gs.exec[0] && r.st != nullptr && r.st != cudaStreamLegacy) {
+    GraphSet gs;
+    if (r.st != nullptr && r.st != cudaStreamLegacy) {
         for (int gi = 0; gi < 2; ++gi) {
             if (gs.tev[gi].create() != IF_OK) return IF_ECUDA;
             cudaGraph_t graph = nullptr;
             if (cudaStreamBeginCapture(r.st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
-                cudaGetLastError();   // stream cannot be captured: fall through to direct launches
+                cudaGetLastError();   // stream cannot be captured: direct launches below
                 break;
             }
-            int rc = IF_OK;
+            int rcc = IF_OK;
             const int timed_pair = pairs > 1 ? 1 : 0;
-            for (int i = 0; i < pairs && rc == IF_OK; ++i)
-                rc = enqueue_two_iterations<K>(r, g, i == timed_pair ? &gs.tev[gi] : nullptr);
+            for (int i = 0; i < pairs && rcc == IF_OK; ++i)
+                rcc = enqueue_two_iterations<K>(r, i == timed_pair ? &gs.tev[gi] : nullptr);
             g_launches -= (long long)launches_per_graph;   // captured, not launched
             cudaError_t e = cudaStreamEndCapture(r.st, &graph);
-            if (rc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
+            if (rcc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
             e = cudaGraphInstantiate(&gs.exec[gi], graph, 0);
             cudaGraphDestroy(graph);
             if (e != cudaSuccess) { gs.exec[gi] = nullptr; cudaGetLastError(); return IF_ECUDA; }
         }
     }
     const bool use_graph = gs.exec[0] && gs.exec[1];
-    const int64_t max_loops = (r.opt.max_iter + r.opt.check_every - 1) / r.opt.check_every + 2;
-    for (int64_t it = 0; it < max_loops; ++it) {
+    const int64_t per_rhs = (r.opt.max_iter + r.opt.check_every - 1) / r.opt.check_every + 3;
+    const int64_t max_loops = ((int64_t)(R + K - 1) / K + 1) * per_rhs + 8;
+    for (int64_t it = 0; it < max_loops && active > 0; ++it) {
         if (use_graph) {
             IF_CUDA_TRY(cudaGraphLaunch(gs.exec[it & 1], r.st));
             g_launches += (long long)launches_per_graph;
         } else {
-            for (int i = 0; i < pairs; ++i) {
-                int rc = enqueue_two_iterations<K>(r, g);
-                if (rc != IF_OK) return rc;
-            }
+            for (int i = 0; i < pairs; ++i)
+                if ((rc = enqueue_two_iterations<K>(r))) return rc;
         }
-        *batch_iters += r.opt.check_every;
         const int slot = (int)(it & 3);
-        IF_CUDA_TRY(cudaMemcpyAsync(&poll.flags[slot], &r.w.ctrl->all_done, sizeof(int), cudaMemcpyDeviceToHost, r.st));
+        IF_CUDA_TRY(cudaMemcpyAsync(&poll.snap[slot], reinterpret_cast<const char*>(r.w.ctrl) + offsetof(Ctrl, done),
+                                    sizeof(Snapshot), cudaMemcpyDeviceToHost, r.st));
         IF_CUDA_TRY(cudaEventRecord(poll.ev[slot], r.st));
-        if (it >= 1) {
-            const int prev = (int)((it - 1) & 3);
-            IF_CUDA_TRY(cudaEventSynchronize(poll.ev[prev]));
-            if (use_graph && !poll.flags[prev]) {
-                // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
-                const TimingEvents& te = gs.tev[(it - 1) & 1];
-                float a = 0.f, b = 0.f;
-                if (cudaEventElapsedTime(&a, te.s0, te.s1) == cudaSuccess &&
-                    cudaEventElapsedTime(&b, te.s1, te.u1) == cudaSuccess) {
-                    times->spmm_ms += a; times->update_ms += b; times->samples += 1;
-                } else {
-                    cudaGetLastError();
-                }
+        if (it == 0) continue;
+        const int prev = (int)((it - 1) & 3);
+        IF_CUDA_TRY(cudaEventSynchronize(poll.ev[prev]));
+        const Snapshot& s = poll.snap[prev];
+        unsigned fin = 0;
+        bool any_running = false;
+        for (int c = 0; c < K; ++c) {
+            if (col_rhs[c] < 0 || s.epoch[c] != host_epoch[c]) continue;
+            if (s.done[c]) fin |= 1u << c; else any_running = true;
+        }
+        if (use_graph && any_running) {
+            // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
+            const TimingEvents& te = gs.tev[(it - 1) & 1];
+            float a = 0.f, b = 0.f;
+            if (cudaEventElapsedTime(&a, te.s0, te.s1) == cudaSuccess &&
+                cudaEventElapsedTime(&b, te.s1, te.u1) == cudaSuccess) {
+                times->spmm_ms += a; times->update_ms += b; times->samples += 1;
+            } else {
+                cudaGetLastError();
             }
-            if (poll.flags[prev]) break;
+        }
+        if (fin) {
+            // these columns stopped before launch it-1 ended and stayed frozen through launch it
+            if ((rc = finalize_columns<K>(r, job, fin, d_out))) return rc;
+            for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) --active;
+            if (next < R) {
+                assign(fin, &sp, &started);
+                if ((rc = start_columns<K>(r, started, sp, d_fields))) return rc;
+            } else {
+                for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) col_rhs[c] = -1;
+            }
         }
     }
-    const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
-    if (job == JOB_SPECTRUM) {
-        k_energy<K><<<g.grid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.x, r.w.p0, r.w.p1, h->total_area,
-                                                r.w.energy, g.rows_per_block);
-        IF_LAUNCH_CHECK();
-    } else {
-        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.x, r.w.p0, r.w.p1, 1, d_out);
-        IF_LAUNCH_CHECK();
-    }
-    k_stats<<<1, 32, 0, r.st>>>(r.w.ctrl, K, r.w.iters, r.w.status, r.w.relres);
-    IF_LAUNCH_CHECK();
+    if (active > 0) return IF_ECUDA;   // cannot happen: every column stops at max_iter
+    long long total = 0;
+    IF_CUDA_TRY(cudaMemcpyAsync(&total, &r.w.ctrl->total_iters, sizeof(long long), cudaMemcpyDeviceToHost, r.st));
+    IF_CUDA_TRY(cudaStreamSynchronize(r.st));
+    *batch_iters = (int64_t)total;
     return IF_OK;
 }
 
-int dispatch_batch(int K, Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, size_t first,
-                   size_t count, int n_ells, double* d_out, PollState& poll, int bps, GraphSet* cache,
-                   int64_t* bi, KernelTimes* kt) {
-    switch (K) {
-        case 4: return solve_batch<4>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[0], bi, kt);
-        case 8: return solve_batch<8>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[1], bi, kt);
-        default: return solve_batch<16>(r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, &cache[2], bi, kt);
-    }
+int pick_k(int batch, size_t R) {
+    int K = batch;
+    while (K > 4 && R <= (size_t)K / 2) K /= 2;   // few right-hand sides: narrower columns, less wasted bandwidth
+    return K;
 }
 
 int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
@@ -722,15 +419,15 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     int log2c = 0;
     while ((1 << log2c) < h->sell_c) ++log2c;
     r.m = MeshView{h->chunk_ptr, h->sell_col, h->sell_val, h->area, h->inv_area, h->sdiag, h->gdiag, h->perm,
-                   h->n_vert, log2c};
+                   h->n_vert, h->n_chunks, log2c};
 
     PollState poll;
     int expected = 0;
     if (h->h_pinned && h->pinned_busy.compare_exchange_strong(expected, 1)) {
-        poll.flags = static_cast<int*>(h->h_pinned);
+        poll.snap = static_cast<Snapshot*>(h->h_pinned);
         poll.h = h;
     } else {
-        IF_CUDA_TRY(cudaHostAlloc((void**)&poll.flags, 4 * sizeof(int), cudaHostAllocDefault));
+        IF_CUDA_TRY(cudaHostAlloc((void**)&poll.snap, 4 * sizeof(Snapshot), cudaHostAllocDefault));
         poll.own_pinned = true;
     }
     for (auto& e : poll.ev) IF_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -740,38 +437,27 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     struct EvGuard { cudaEvent_t a, b; ~EvGuard() { cudaEventDestroy(a); cudaEventDestroy(b); } } evg{t0, t1};
     IF_CUDA_TRY(cudaEventRecord(t0, r.st));
 
-    int bps = 4;
-    {
-        int occ = 0;
-        cudaError_t e = order_n == 1
-            ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_spmm<16, MODE_CG1>, BLOCK, 0)
-            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_spmm<16, MODE_CG2A>, BLOCK, 0);
-        if (e == cudaSuccess && occ > 0) bps = occ > 8 ? 8 : occ; else cudaGetLastError();
-    }
-
-    // right-hand sides sorted by scale so the columns of a batch need similar iteration counts
+    // queue of right-hand sides: largest scale (most iterations) first, so that the short solves fill the tail
     std::vector<Rhs> rhs;
     rhs.reserve((size_t)R);
     for (int f = 0; f < n_fields; ++f)
         for (int j = 0; j < n_ells; ++j) rhs.push_back(Rhs{ells[j], f, j});
     if (job != JOB_APPLY)
-        std::stable_sort(rhs.begin(), rhs.end(), [](const Rhs& a, const Rhs& b) { return a.ell < b.ell; });
+        std::stable_sort(rhs.begin(), rhs.end(), [](const Rhs& a, const Rhs& b) { return a.ell > b.ell; });
 
-    GraphSet cache[3];
     KernelTimes ktimes;
-    std::vector<std::pair<size_t, size_t>> batches;
-    int64_t launched_iters = 0;
-    size_t first = 0;
-    while (first < (size_t)R) {
-        const size_t remaining = (size_t)R - first;
-        int K = r.opt.batch;
-        while (K > 4 && remaining <= (size_t)K / 2) K /= 2;
-        const size_t count = remaining < (size_t)K ? remaining : (size_t)K;
-        rc = dispatch_batch(K, r, job, d_fields, rhs, first, count, n_ells, d_out, poll, bps, cache, &launched_iters, &ktimes);
-        if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
-        batches.emplace_back(first, count);
-        first += count;
+    int64_t batch_iters = 0;
+    const int K = pick_k(r.opt.batch, (size_t)R);
+    if (job == JOB_APPLY) {
+        rc = K == 4 ? apply_all<4>(r, d_fields, rhs, n_ells, d_out)
+           : K == 8 ? apply_all<8>(r, d_fields, rhs, n_ells, d_out)
+                    : apply_all<16>(r, d_fields, rhs, n_ells, d_out);
+    } else {
+        rc = K == 4 ? solve_all<4>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &batch_iters)
+           : K == 8 ? solve_all<8>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &batch_iters)
+                    : solve_all<16>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &batch_iters);
     }
+    if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
     if (job == JOB_SPECTRUM) {
         IF_CUDA_TRY(cudaMemcpyAsync(r.w.ells, ells, (size_t)n_ells * sizeof(double), cudaMemcpyHostToDevice, r.st));
         const int nb = n_fields * (n_ells - 1);
@@ -800,19 +486,11 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
         float ms = 0.f;
         IF_CUDA_TRY(cudaEventElapsedTime(&ms, t0, t1));
         stats->seconds = ms * 1e-3;
-        stats->batch_iters = 0;
+        stats->batch_iters = batch_iters;
         stats->rhs_iters = 0;
         stats->spmm_seconds = ktimes.samples ? 1e-3 * ktimes.spmm_ms / (double)ktimes.samples : 0.0;
         stats->update_seconds = ktimes.samples ? 1e-3 * ktimes.update_ms / (double)ktimes.samples : 0.0;
         stats->kernel_samples = ktimes.samples;
-        for (auto& b : batches) {
-            int mx = 0;
-            for (size_t i = 0; i < b.second; ++i) {
-                const Rhs& q = rhs[b.first + i];
-                mx = std::max(mx, (int)h_iters[(size_t)q.f * n_ells + q.j]);
-            }
-            stats->batch_iters += mx;
-        }
         for (int64_t i = 0; i < R; ++i) {
             stats->rhs_iters += h_iters[(size_t)i];
             if (stats->iters) stats->iters[i] = h_iters[(size_t)i];
