@@ -185,7 +185,9 @@ template <int K, int MODE> struct TileSmem {
     static constexpr size_t vec_bytes = (size_t)T * K * sizeof(double);
     static constexpr size_t off_val = NVEC * vec_bytes;
     static constexpr size_t off_col = off_val + (size_t)T * WCAP * sizeof(double);
-    static constexpr size_t off_cp = off_col + (size_t)T * WCAP * sizeof(int32_t);
+    static constexpr size_t off_dg = off_col + (size_t)T * WCAP * sizeof(int32_t);   // S_vv of the tile's rows
+    static constexpr size_t off_ar = off_dg + (size_t)T * sizeof(double);            // A_v or 1/A_v
+    static constexpr size_t off_cp = off_ar + (size_t)T * sizeof(double);
     static constexpr size_t off_bar = off_cp + 64 * sizeof(int32_t);
     static constexpr size_t bytes = off_bar + 16;
 };
@@ -205,7 +207,11 @@ __global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ c
     double2* sc = reinterpret_cast<double2*>(smem + 2 * SM::vec_bytes);    // x
     const double* sval = reinterpret_cast<const double*>(smem + SM::off_val);
     const int32_t* scol = reinterpret_cast<const int32_t*>(smem + SM::off_col);
+    const double* sdg = reinterpret_cast<const double*>(smem + SM::off_dg);
+    const double* sar = reinterpret_cast<const double*>(smem + SM::off_ar);
     int32_t* scp = reinterpret_cast<int32_t*>(smem + SM::off_cp);
+    // the per-row factor next to S_vv: A_v for q = A_v p + c S v, 1/A_v for t = M^-1 S v
+    const double* __restrict__ rowfac = (MODE == MODE_CG2A || (MODE == MODE_PLAIN && a.scale_inv_area)) ? m.inv_area : m.area;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + SM::off_bar);
 
     const int tid = threadIdx.x;
@@ -236,7 +242,10 @@ __global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ c
         __syncthreads();   // everyone is done reading the previous tile (and the barrier is initialised)
         if (tid == 0) {
             bulk_wait_read0();   // the previous tile's bulk stores have finished reading sa / sc
-            mbar_expect_tx(bar, vbytes * SM::NVEC + (msm ? (uint32_t)slots * 12u : 0u));
+            const uint32_t dbytes = ((uint32_t)nrows * 8u + 15u) & ~15u;   // the arrays are padded by 16 bytes
+            mbar_expect_tx(bar, vbytes * SM::NVEC + 2u * dbytes + (msm ? (uint32_t)slots * 12u : 0u));
+            bulk_load(const_cast<double*>(sdg), m.sdiag + row0, dbytes, bar);
+            bulk_load(const_cast<double*>(sar), rowfac + row0, dbytes, bar);
             bulk_load(sa, a.in0 + row0 * K, vbytes, bar);
             if (SM::NVEC >= 2) bulk_load(sb, a.in1 + row0 * K, vbytes, bar);
             if (SM::NVEC >= 3) bulk_load(sc, a.x + row0 * K, vbytes, bar);
@@ -308,20 +317,20 @@ __global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ c
                 s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
                 s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
             }
-            const double sd = m.sdiag[row];
+            const double sd = sdg[r];
             s.x = fma(sd, own.x, s.x);
             s.y = fma(sd, own.y, s.y);          // s = (S v)_row
             const int64_t ri = row * K + 2 * l;
             if (MODE == MODE_PLAIN) {
-                if (a.scale_inv_area) { const double ia = m.inv_area[row]; s.x *= ia; s.y *= ia; }
+                if (a.scale_inv_area) { const double ia = sar[r]; s.x *= ia; s.y *= ia; }
                 st2(a.out0, ri, s);
             } else if (MODE == MODE_CG2A) {
-                const double ia = m.inv_area[row];
+                const double ia = sar[r];
                 s.x *= ia; s.y *= ia;            // t = M^-1 S p'
                 st2(a.out0, ri, s);
             } else {
                 // q = A_v p + c (S v)_row ; v = p (n = 1) or t (n = 2)
-                const double av = m.area[row];
+                const double av = sar[r];
                 const double2 pv = (MODE == MODE_CG1) ? own : sb[r * TPR + l];
                 double2 q;
                 q.x = fma(cc.x, s.x, av * pv.x);

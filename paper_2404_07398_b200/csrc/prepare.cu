@@ -480,10 +480,14 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     DevBuf scol, sval, area, inv_area, sdiag, gdiag;
     IF_CUDA_TRY(scol.alloc((size_t)sell_slots * 4 + 16));
     IF_CUDA_TRY(sval.alloc((size_t)sell_slots * 8 + 16));
-    IF_CUDA_TRY(area.alloc((size_t)nv * 8));
-    IF_CUDA_TRY(inv_area.alloc((size_t)nv * 8));
-    IF_CUDA_TRY(sdiag.alloc((size_t)nv * 8));
-    IF_CUDA_TRY(gdiag.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(area.alloc((size_t)nv * 8 + 16));   // +16: the SpMM kernel bulk-copies 16-byte multiples
+    IF_CUDA_TRY(cudaMemsetAsync(area.p, 0, (size_t)nv * 8 + 16, st));
+    IF_CUDA_TRY(inv_area.alloc((size_t)nv * 8 + 16));   // +16: the SpMM kernel bulk-copies 16-byte multiples
+    IF_CUDA_TRY(cudaMemsetAsync(inv_area.p, 0, (size_t)nv * 8 + 16, st));
+    IF_CUDA_TRY(sdiag.alloc((size_t)nv * 8 + 16));   // +16: the SpMM kernel bulk-copies 16-byte multiples
+    IF_CUDA_TRY(cudaMemsetAsync(sdiag.p, 0, (size_t)nv * 8 + 16, st));
+    IF_CUDA_TRY(gdiag.alloc((size_t)nv * 8 + 16));   // +16: the SpMM kernel bulk-copies 16-byte multiples
+    IF_CUDA_TRY(cudaMemsetAsync(gdiag.p, 0, (size_t)nv * 8 + 16, st));
     k_sell_fill<<<grid_for(n_chunks * C), 256, 0, st>>>(
         perm.as<int32_t>(), iperm.as<int32_t>(), rowptr.as<int64_t>(), ccol.as<int32_t>(), v0.as<double>(),
         area_u.as<double>(), sdiag_u.as<double>(), gdiag_u.as<double>(), nv, n_chunks, C, chunk_ptr.as<int64_t>(),
