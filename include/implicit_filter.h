@@ -122,6 +122,11 @@ int if_apply(if_handle h, const double* d_fields, int n_fields, const double* el
 int if_mesh_info(if_handle h, int64_t* n_vert, int64_t* nnz, double* total_area, double* mean_edge,
                  int64_t* sell_slots);
 
+/* Row tiling of the fused SpMM kernel (all HOST, any may be NULL): tiles of 128 consecutive internal rows, total
+ * and largest number of out-of-tile rows ("halo") the tiles gather from, and tiles left unstaged because their
+ * halo or row width exceeds the shared-memory caps (they take the slower global-gather path). */
+int if_mesh_tile_info(if_handle h, int64_t* n_tiles, int64_t* halo_rows, int64_t* halo_max, int64_t* unstaged_tiles);
+
 /* Copy S (CSR, caller's numbering, columns ascending, diagonal included) and A_v to HOST arrays:
  * rowptr [n_vert+1], col [nnz], val [nnz], area [n_vert]; any may be NULL.  Needs IF_FLAG_KEEP_CSR
  * (else IF_EINVAL).  For checking the preparation phase against another assembly. */

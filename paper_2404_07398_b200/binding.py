@@ -19,7 +19,7 @@ IF_OK, IF_WNOTCONVERGED = 0, 1
 IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKSPACE = -1, -2, -3, -4, -5, -6, -7
 IF_FLAG_KEEP_CSR = 1
 
-EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_apply", "if_mesh_info",
+EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_apply", "if_mesh_info", "if_mesh_tile_info",
            "if_mesh_export_csr", "if_mesh_export_perm", "if_destroy", "if_strerror", "if_launch_count")
 
 
@@ -69,6 +69,8 @@ def load_library():
     L.if_apply.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, C.c_size_t, vp, C.POINTER(if_options)]
     L.if_mesh_info.restype = i32
     L.if_mesh_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), dp, dp, C.POINTER(i64)]
+    L.if_mesh_tile_info.restype = i32
+    L.if_mesh_tile_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
     L.if_mesh_export_csr.restype = i32
     L.if_mesh_export_csr.argtypes = [vp, vp, vp, vp, vp]
     L.if_mesh_export_perm.restype = i32
@@ -121,6 +123,10 @@ class Handle:
         load_library().if_mesh_info(self._ptr, C.byref(nv), C.byref(nnz), C.byref(ta), C.byref(me), C.byref(slots))
         self.n_vert, self.nnz, self.sell_slots = int(nv.value), int(nnz.value), int(slots.value)
         self.total_area, self.mean_edge = float(ta.value), float(me.value)
+        nt, hr, hm, ut = C.c_int64(), C.c_int64(), C.c_int64(), C.c_int64()
+        load_library().if_mesh_tile_info(self._ptr, C.byref(nt), C.byref(hr), C.byref(hm), C.byref(ut))
+        self.n_tiles, self.halo_rows, self.halo_max, self.unstaged_tiles = (int(nt.value), int(hr.value),
+                                                                            int(hm.value), int(ut.value))
 
     def close(self):
         if self._ptr is not None and self._ptr.value:

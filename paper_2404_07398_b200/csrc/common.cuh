@@ -12,6 +12,11 @@
 
 namespace ifl {
 
+// Row tile of the fused SpMM kernel and the most out-of-tile rows ("halo") a tile may stage in shared memory.
+// if_prepare builds tile-local column ids and halo lists for exactly this tile height.
+constexpr int TILE_ROWS = 128;
+constexpr int HALO_CAP = 128;
+
 extern std::atomic<long long> g_launches;   // kernels launched by this library (if_launch_count)
 
 #define IF_CUDA_TRY(expr)                                                                          \
@@ -65,6 +70,16 @@ struct if_mesh_s {
     int64_t* chunk_ptr = nullptr;   // [n_chunks+1] slot offsets (even)
     int32_t* sell_col = nullptr;    // [sell_slots] internal column ids
     double* sell_val = nullptr;     // [sell_slots]
+    // per row tile of TILE_ROWS rows: the out-of-tile rows it gathers from (sorted, unique) and the same matrix
+    // with tile-local column ids (tile row r -> r, halo slot s -> TILE_ROWS + s); halo_n = -1: tile not staged
+    int32_t* sell_lcol = nullptr;   // [sell_slots]
+    int32_t* halo_n = nullptr;      // [n_tiles]
+    int64_t* halo_ptr = nullptr;    // [n_tiles+1]
+    int32_t* halo_rows = nullptr;   // [halo_ptr[n_tiles]]
+    int64_t n_tiles = 0;
+    int64_t halo_total = 0;
+    int64_t halo_max = 0;         // largest staged halo
+    int64_t unstaged_tiles = 0;   // tiles whose halo or row width exceeds the shared-memory caps
     double* area = nullptr;         // [n_vert] A_v            (internal order)
     double* inv_area = nullptr;     // [n_vert] 1/A_v
     double* sdiag = nullptr;        // [n_vert] S_vv

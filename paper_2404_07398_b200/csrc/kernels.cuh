@@ -12,11 +12,13 @@
 // Per-column scalars (alpha, beta, rho, done flags) live in a device control block and are produced by the
 // last block to finish each kernel (single-pass, fixed-order, deterministic grid reduction).
 //
-// Kernel A is tiled for sm_100a: a persistent CTA walks tiles of T consecutive rows.  Per tile one thread issues
-// bulk async copies (TMA, cp.async.bulk + mbarrier complete_tx) that land the tile of z, p, x and the tile's
-// slice of the SELL matrix in shared memory; the CTA forms p' in place, hands x and p' back to global memory
-// with bulk stores, and gathers the neighbours' p' from the shared tile (rows are in space-filling-curve
-// order, so most neighbours are in the tile); only out-of-tile neighbours touch L2.
+// Kernel A is tiled for sm_100a: a persistent CTA walks tiles of TILE_ROWS consecutive rows.  Per tile one thread
+// issues bulk async copies (TMA, cp.async.bulk + mbarrier complete_tx) that land the tile of z and p, the tile's
+// slice of the SELL matrix (with tile-local column ids built by if_prepare) and its diagonals in shared memory;
+// meanwhile all threads fetch the tile's halo (the out-of-tile neighbour rows, listed by if_prepare) from L2
+// into the same shared array and x into registers.  The CTA forms p' in place, hands it back with a bulk store,
+// and the gather of the neighbours' p' is then branch-free shared-memory traffic (rows are in
+// space-filling-curve order, so the halo is small).
 #pragma once
 
 #include "common.cuh"
@@ -37,6 +39,10 @@ struct MeshView {
     const double* __restrict__ sdiag;
     const double* __restrict__ gdiag;
     const int32_t* __restrict__ perm;
+    const int32_t* __restrict__ lcol;       // tile-local column ids (tile row, or TILE_ROWS + halo slot)
+    const int32_t* __restrict__ halo_n;     // [tiles] halo rows of the tile, -1: not staged (use col)
+    const int64_t* __restrict__ halo_ptr;   // [tiles+1]
+    const int32_t* __restrict__ halo_rows;  // out-of-tile rows each tile gathers from, ascending per tile
     int64_t nv;
     int64_t n_chunks;
     int log2c;
@@ -176,43 +182,46 @@ struct SpmmArgs {
     int out_idx;         // CG1/CG2A: index of the direction buffer written (recorded in ctrl->cur_p)
 };
 
-template <int K> struct TileRows { static constexpr int T = K == 16 ? 128 : 256; };
-
-// dynamic shared memory of k_spmm: [vec a | vec b | vec c][val slice][col slice][chunk offsets][mbarrier]
+// dynamic shared memory of k_spmm:
+//   [gathered vector: T tile rows + HALO_CAP halo rows][second vector: T rows][val slice][col slice]
+//   [S_vv][A_v | 1/A_v][chunk offsets][mbarrier]
 template <int K, int MODE> struct TileSmem {
-    static constexpr int T = TileRows<K>::T;
-    static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : (MODE == MODE_CG2B ? 2 : 3);
+    static constexpr int T = TILE_ROWS;
+    static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // vectors that arrive by bulk copy
     static constexpr size_t vec_bytes = (size_t)T * K * sizeof(double);
-    static constexpr size_t off_val = NVEC * vec_bytes;
+    static constexpr size_t off_b = (size_t)(T + HALO_CAP) * K * sizeof(double);
+    static constexpr size_t off_val = off_b + (NVEC - 1) * vec_bytes;
     static constexpr size_t off_col = off_val + (size_t)T * WCAP * sizeof(double);
     static constexpr size_t off_dg = off_col + (size_t)T * WCAP * sizeof(int32_t);   // S_vv of the tile's rows
     static constexpr size_t off_ar = off_dg + (size_t)T * sizeof(double);            // A_v or 1/A_v
     static constexpr size_t off_cp = off_ar + (size_t)T * sizeof(double);
-    static constexpr size_t off_bar = off_cp + 64 * sizeof(int32_t);
+    static constexpr size_t off_bar = off_cp + 16 * sizeof(int32_t);
     static constexpr size_t bytes = off_bar + 16;
 };
 
 template <int K, int MODE>
-__global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+__global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
                                                 SpmmArgs a) {
     using SM = TileSmem<K, MODE>;
     constexpr int T = SM::T;
     constexpr int TPR = K / 2;
     constexpr int ROWS = BLOCK / TPR;
+    constexpr int XPT = T * TPR / BLOCK;                 // double2 elements of a tile vector per thread
+    constexpr int HPT = (HALO_CAP + ROWS - 1) / ROWS;    // halo rows per thread group
     constexpr bool CG_A = (MODE == MODE_CG1 || MODE == MODE_CG2A);
     if (MODE != MODE_PLAIN && ctrl->all_done) return;
     extern __shared__ __align__(128) unsigned char smem[];
-    double2* sa = reinterpret_cast<double2*>(smem);                        // gathered vector (z -> p', x, t)
-    double2* sb = reinterpret_cast<double2*>(smem + SM::vec_bytes);        // p_old, or own p' (CG2B)
-    double2* sc = reinterpret_cast<double2*>(smem + 2 * SM::vec_bytes);    // x
+    double2* sa = reinterpret_cast<double2*>(smem);                  // gathered vector (z -> p', x, t): tile + halo
+    double2* sb = reinterpret_cast<double2*>(smem + SM::off_b);      // p_old, or own p' (CG2B)
     const double* sval = reinterpret_cast<const double*>(smem + SM::off_val);
     const int32_t* scol = reinterpret_cast<const int32_t*>(smem + SM::off_col);
     const double* sdg = reinterpret_cast<const double*>(smem + SM::off_dg);
     const double* sar = reinterpret_cast<const double*>(smem + SM::off_ar);
     int32_t* scp = reinterpret_cast<int32_t*>(smem + SM::off_cp);
-    // the per-row factor next to S_vv: A_v for q = A_v p + c S v, 1/A_v for t = M^-1 S v
-    const double* __restrict__ rowfac = (MODE == MODE_CG2A || (MODE == MODE_PLAIN && a.scale_inv_area)) ? m.inv_area : m.area;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + SM::off_bar);
+    // the per-row factor next to S_vv: A_v for q = A_v p + c S v, 1/A_v for t = M^-1 S v
+    const double* __restrict__ rowfac =
+        (MODE == MODE_CG2A || (MODE == MODE_PLAIN && a.scale_inv_area)) ? m.inv_area : m.area;
 
     const int tid = threadIdx.x;
     const int l = tid % TPR;
@@ -238,44 +247,78 @@ __global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ c
         const int nch = (nrows + C - 1) >> m.log2c;
         const int64_t cp_first = m.chunk_ptr[ch0];
         const int64_t slots = m.chunk_ptr[ch0 + nch] - cp_first;
-        const bool msm = slots <= (int64_t)T * WCAP;       // the tile's SELL slice fits shared memory
+        const int nh = m.halo_n[tile];
+        // staged tile: matrix slice and halo fit shared memory, columns are tile-local indices, no branches
+        const bool staged = nh >= 0 && slots <= (int64_t)T * WCAP;
         __syncthreads();   // everyone is done reading the previous tile (and the barrier is initialised)
         if (tid == 0) {
-            bulk_wait_read0();   // the previous tile's bulk stores have finished reading sa / sc
+            bulk_wait_read0();   // the previous tile's bulk store has finished reading sa
             const uint32_t dbytes = ((uint32_t)nrows * 8u + 15u) & ~15u;   // the arrays are padded by 16 bytes
-            mbar_expect_tx(bar, vbytes * SM::NVEC + 2u * dbytes + (msm ? (uint32_t)slots * 12u : 0u));
-            bulk_load(const_cast<double*>(sdg), m.sdiag + row0, dbytes, bar);
-            bulk_load(const_cast<double*>(sar), rowfac + row0, dbytes, bar);
+            mbar_expect_tx(bar, vbytes * SM::NVEC + 2u * dbytes + (staged ? (uint32_t)slots * 12u : 0u));
             bulk_load(sa, a.in0 + row0 * K, vbytes, bar);
             if (SM::NVEC >= 2) bulk_load(sb, a.in1 + row0 * K, vbytes, bar);
-            if (SM::NVEC >= 3) bulk_load(sc, a.x + row0 * K, vbytes, bar);
-            if (msm) {
+            bulk_load(const_cast<double*>(sdg), m.sdiag + row0, dbytes, bar);
+            bulk_load(const_cast<double*>(sar), rowfac + row0, dbytes, bar);
+            if (staged) {
                 bulk_load(const_cast<double*>(sval), m.val + cp_first, (uint32_t)slots * 8u, bar);
-                bulk_load(const_cast<int32_t*>(scol), m.col + cp_first, (uint32_t)slots * 4u, bar);
+                bulk_load(const_cast<int32_t*>(scol), m.lcol + cp_first, (uint32_t)slots * 4u, bar);
             }
         }
         if (tid <= nch) scp[tid] = (int32_t)(m.chunk_ptr[ch0 + tid] - cp_first);
+        // while the bulk copies fly: x of the tile into registers, the halo rows into shared memory
+        double2 xv[XPT];
+        if (CG_A) {
+#pragma unroll
+            for (int i = 0; i < XPT; ++i) {
+                const int e = tid + i * BLOCK;
+                if (e < nrows * TPR) xv[i] = ld2(a.x, row0 * K + 2 * (int64_t)e);
+            }
+        }
+        if (staged) {
+            const int64_t hp = m.halo_ptr[tile];
+            double2 h0[HPT], h1[HPT];
+#pragma unroll
+            for (int i = 0; i < HPT; ++i) {
+                const int hh = tid / TPR + i * ROWS;
+                if (hh < nh) {
+                    const int64_t j = m.halo_rows[hp + hh];
+                    h0[i] = ld2(a.in0, j * K + 2 * l);
+                    if (CG_A) h1[i] = ld2(a.in1, j * K + 2 * l);
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < HPT; ++i) {
+                const int hh = tid / TPR + i * ROWS;
+                if (hh < nh) {
+                    double2 g = h0[i];
+                    if (CG_A) { g.x = fma(beta.x, h1[i].x, g.x); g.y = fma(beta.y, h1[i].y, g.y); }
+                    sa[(T + hh) * TPR + l] = g;
+                }
+            }
+        }
         mbar_wait(bar, parity);
         parity ^= 1u;
         if (CG_A) {
-            // p' = z + beta p (in place over z) ; x += alpha_prev p (in place) ; both go back with bulk stores
-            for (int e = tid; e < nrows * TPR; e += BLOCK) {
-                const double2 zv = sa[e], pv = sb[e];
-                double2 xv = sc[e];
-                double2 own;
-                own.x = fma(beta.x, pv.x, zv.x);
-                own.y = fma(beta.y, pv.y, zv.y);
-                xv.x = fma(alpha.x, pv.x, xv.x);
-                xv.y = fma(alpha.y, pv.y, xv.y);
-                sa[e] = own;
-                sc[e] = xv;
+            // p' = z + beta p (in place over z, goes back with a bulk store) ; x += alpha_prev p
+#pragma unroll
+            for (int i = 0; i < XPT; ++i) {
+                const int e = tid + i * BLOCK;
+                if (e < nrows * TPR) {
+                    const double2 zv = sa[e], pv = sb[e];
+                    double2 own;
+                    own.x = fma(beta.x, pv.x, zv.x);
+                    own.y = fma(beta.y, pv.y, zv.y);
+                    xv[i].x = fma(alpha.x, pv.x, xv[i].x);
+                    xv[i].y = fma(alpha.y, pv.y, xv[i].y);
+                    sa[e] = own;
+                    st2(a.x, row0 * K + 2 * (int64_t)e, xv[i]);
+                }
             }
             fence_proxy_async();
         }
         __syncthreads();
         if (CG_A && tid == 0) {
             bulk_store(a.out1 + row0 * K, sa, vbytes);
-            bulk_store(a.x + row0 * K, sc, vbytes);
             bulk_commit();
         }
         for (int r = tid / TPR; r < nrows; r += ROWS) {
@@ -286,36 +329,45 @@ __global__ void __launch_bounds__(BLOCK) k_spmm(MeshView m, Ctrl* __restrict__ c
             const int o = cpr + (r & (C - 1)) * w;
             const double2 own = sa[r * TPR + l];
             double2 s = {0.0, 0.0};
-            for (int k = 0; k < w; k += 2) {
-                int2 cj;
-                double2 vj;
-                if (msm) {
-                    cj = *reinterpret_cast<const int2*>(scol + o + k);
-                    vj = *reinterpret_cast<const double2*>(sval + o + k);
-                } else {
-                    cj = *reinterpret_cast<const int2*>(m.col + cp_first + o + k);
-                    vj = ld2(m.val, cp_first + o + k);
+            if (staged) {
+                // every neighbour (tile or halo) is in shared memory under its tile-local index
+                double2 s1 = {0.0, 0.0};
+                for (int k = 0; k < w; k += 2) {
+                    const int2 cj = *reinterpret_cast<const int2*>(scol + o + k);
+                    const double2 vj = *reinterpret_cast<const double2*>(sval + o + k);
+                    const double2 g0 = sa[cj.x * TPR + l], g1 = sa[cj.y * TPR + l];
+                    s.x = fma(vj.x, g0.x, s.x);   s.y = fma(vj.x, g0.y, s.y);
+                    s1.x = fma(vj.y, g1.x, s1.x); s1.y = fma(vj.y, g1.y, s1.y);
                 }
-                double2 g0, g1;
-                const unsigned j0 = (unsigned)(cj.x - (int)row0), j1 = (unsigned)(cj.y - (int)row0);
-                if (j0 < (unsigned)nrows) {
-                    g0 = sa[j0 * TPR + l];
-                } else if (CG_A) {
-                    const double2 z0 = ld2(a.in0, (int64_t)cj.x * K + 2 * l), p0 = ld2(a.in1, (int64_t)cj.x * K + 2 * l);
-                    g0.x = fma(beta.x, p0.x, z0.x); g0.y = fma(beta.y, p0.y, z0.y);
-                } else {
-                    g0 = ld2(a.in0, (int64_t)cj.x * K + 2 * l);
+                s.x += s1.x; s.y += s1.y;
+            } else {
+                // fallback (wide rows or a halo beyond HALO_CAP): global column ids, out-of-tile rows from L2
+                for (int k = 0; k < w; k += 2) {
+                    const int2 cj = *reinterpret_cast<const int2*>(m.col + cp_first + o + k);
+                    const double2 vj = ld2(m.val, cp_first + o + k);
+                    double2 g0, g1;
+                    const unsigned j0 = (unsigned)(cj.x - (int)row0), j1 = (unsigned)(cj.y - (int)row0);
+                    if (j0 < (unsigned)nrows) {
+                        g0 = sa[j0 * TPR + l];
+                    } else {
+                        g0 = ld2(a.in0, (int64_t)cj.x * K + 2 * l);
+                        if (CG_A) {
+                            const double2 p0 = ld2(a.in1, (int64_t)cj.x * K + 2 * l);
+                            g0.x = fma(beta.x, p0.x, g0.x); g0.y = fma(beta.y, p0.y, g0.y);
+                        }
+                    }
+                    if (j1 < (unsigned)nrows) {
+                        g1 = sa[j1 * TPR + l];
+                    } else {
+                        g1 = ld2(a.in0, (int64_t)cj.y * K + 2 * l);
+                        if (CG_A) {
+                            const double2 p1 = ld2(a.in1, (int64_t)cj.y * K + 2 * l);
+                            g1.x = fma(beta.x, p1.x, g1.x); g1.y = fma(beta.y, p1.y, g1.y);
+                        }
+                    }
+                    s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
+                    s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
                 }
-                if (j1 < (unsigned)nrows) {
-                    g1 = sa[j1 * TPR + l];
-                } else if (CG_A) {
-                    const double2 z1 = ld2(a.in0, (int64_t)cj.y * K + 2 * l), p1 = ld2(a.in1, (int64_t)cj.y * K + 2 * l);
-                    g1.x = fma(beta.x, p1.x, z1.x); g1.y = fma(beta.y, p1.y, z1.y);
-                } else {
-                    g1 = ld2(a.in0, (int64_t)cj.y * K + 2 * l);
-                }
-                s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
-                s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
             }
             const double sd = sdg[r];
             s.x = fma(sd, own.x, s.x);
@@ -433,13 +485,26 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
 }
 
 // ------------------------------------------------------------------------------------------- kernel B
+// 1/d for d > 0 in the normal range: hardware seed (2^-23) and two Newton steps (full fp64 precision, ~1 ulp).
+// A fp64 division costs about five times as many instructions and made this streaming kernel issue-bound.
+__device__ __forceinline__ double rcp_pos(double d) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    double e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-d, r, 1.0);
+    return fma(r, e, r);
+}
+
 // z -= alpha q/d ; rho' = sum d z^2 ; ||r||^2 = sum (d z)^2 ; then (last block) beta, stop tests.
+// Pure streaming: every thread keeps U = 8 rows (16 independent 16-byte loads) in flight, two blocks per SM --
+// measured on B200 this reaches the copy bandwidth, while more resident warps with fewer loads each do not.
 template <int K>
-__global__ void __launch_bounds__(BLOCK, 4) k_update(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+__global__ void __launch_bounds__(BLOCK, 2) k_update(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
                                                      double* __restrict__ z, const double* __restrict__ q, int order_n) {
     constexpr int TPR = K / 2;
     constexpr int ROWS = BLOCK / TPR;
-    constexpr int U = 4;
+    constexpr int U = 8;
     if (ctrl->all_done) return;
     const int tid = threadIdx.x, l = tid % TPR;
     const double2 cc = ld2(ctrl->c, 2 * l);
@@ -465,8 +530,8 @@ __global__ void __launch_bounds__(BLOCK, 4) k_update(MeshView m, Ctrl* __restric
             const int64_t row = base + u * stride;
             if (row < m.nv) {
                 const double2 d = {fma(cc.x, dv[u], av[u]), fma(cc.y, dv[u], av[u])};
-                zv[u].x -= alpha.x * qv[u].x / d.x;
-                zv[u].y -= alpha.y * qv[u].y / d.y;
+                zv[u].x = fma(-alpha.x * qv[u].x, rcp_pos(d.x), zv[u].x);
+                zv[u].y = fma(-alpha.y * qv[u].y, rcp_pos(d.y), zv[u].y);
                 st2(z, row * K + 2 * l, zv[u]);
                 const double2 r = {d.x * zv[u].x, d.y * zv[u].y};
                 acc[0].x = fma(r.x, zv[u].x, acc[0].x); acc[0].y = fma(r.y, zv[u].y, acc[0].y);

@@ -248,6 +248,91 @@ __global__ void k_sell_fill(const int32_t* __restrict__ perm, const int32_t* __r
     for (; k < w; ++k) { sell_col[o + k] = self; sell_val[o + k] = 0.0; }
 }
 
+
+// Per row tile of TILE_ROWS rows (one block each): the sorted, unique out-of-tile columns ("halo") and the SELL
+// columns rewritten as tile-local ids.  Pass 1 (write = 0) only counts; pass 2 fills halo_rows and lcol.
+constexpr int ECAP = 1024;   // out-of-tile references a tile may have before it is left unstaged
+__global__ void __launch_bounds__(128) k_tile_halo(const int64_t* __restrict__ chunk_ptr, const int32_t* __restrict__ col,
+                                                   int64_t nv, int log2c, int write, int32_t* __restrict__ halo_n,
+                                                   int64_t* __restrict__ halo_cnt, const int64_t* __restrict__ halo_ptr,
+                                                   int32_t* __restrict__ halo_rows, int32_t* __restrict__ lcol) {
+    __shared__ int ext[ECAP];
+    __shared__ int n_ext, n_uniq;
+    const int tid = threadIdx.x;
+    const int64_t tile = blockIdx.x;
+    const int64_t row0 = tile * TILE_ROWS;
+    const int nrows = (int)min((int64_t)TILE_ROWS, nv - row0);
+    const int C = 1 << log2c;
+    const int64_t ch0 = row0 >> log2c;
+    const int nch = (nrows + C - 1) >> log2c;
+    const int64_t cp_first = chunk_ptr[ch0];
+    const int64_t slots = chunk_ptr[ch0 + nch] - cp_first;
+    if (tid == 0) { n_ext = 0; n_uniq = 0; }
+    __syncthreads();
+    for (int64_t s = tid; s < slots; s += 128) {
+        const int64_t c = col[cp_first + s];
+        if (c < row0 || c >= row0 + nrows) {
+            const int i = atomicAdd(&n_ext, 1);
+            if (i < ECAP) ext[i] = (int)c;
+        }
+    }
+    __syncthreads();
+    const int ne = n_ext;
+    bool over = ne > ECAP;
+    if (!over) {
+        int np2 = 1;
+        while (np2 < ne) np2 <<= 1;
+        for (int i = ne + tid; i < np2; i += 128) ext[i] = 0x7fffffff;
+        __syncthreads();
+        for (int k = 2; k <= np2; k <<= 1)
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                for (int i = tid; i < np2; i += 128) {
+                    const int ixj = i ^ j;
+                    if (ixj > i) {
+                        const bool up = (i & k) == 0;
+                        const int a = ext[i], b = ext[ixj];
+                        if ((a > b) == up) { ext[i] = b; ext[ixj] = a; }
+                    }
+                }
+                __syncthreads();
+            }
+        if (tid == 0) {
+            int nu = 0;
+            for (int i = 0; i < ne; ++i)
+                if (i == 0 || ext[i] != ext[i - 1]) ext[nu++] = ext[i];
+            n_uniq = nu;
+        }
+        __syncthreads();
+        over = n_uniq > HALO_CAP;
+    }
+    const int nu = over ? -1 : n_uniq;
+    if (!write) {
+        if (tid == 0) { halo_n[tile] = nu; halo_cnt[tile] = nu > 0 ? nu : 0; }
+        return;
+    }
+    if (nu < 0) {
+        for (int64_t s = tid; s < slots; s += 128) lcol[cp_first + s] = 0;
+        return;
+    }
+    const int64_t hp = halo_ptr[tile];
+    for (int i = tid; i < nu; i += 128) halo_rows[hp + i] = ext[i];
+    for (int64_t s = tid; s < slots; s += 128) {
+        const int64_t c = col[cp_first + s];
+        int lc;
+        if (c >= row0 && c < row0 + nrows) {
+            lc = (int)(c - row0);
+        } else {
+            int lo = 0, hi = nu - 1;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (ext[mid] < (int)c) lo = mid + 1; else hi = mid;
+            }
+            lc = TILE_ROWS + lo;
+        }
+        lcol[cp_first + s] = lc;
+    }
+}
+
 inline unsigned grid_for(int64_t n, int block = 256) { return (unsigned)((n + block - 1) / block); }
 inline int bits_for(uint64_t n) { int b = 1; while ((1ull << b) < n && b < 63) ++b; return b; }
 
@@ -290,6 +375,7 @@ extern "C" void if_destroy(if_handle h) {
     cudaSetDevice(h->device);
     cudaFree(h->chunk_ptr); cudaFree(h->sell_col); cudaFree(h->sell_val); cudaFree(h->area);
     cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->perm); cudaFree(h->iperm);
+    cudaFree(h->sell_lcol); cudaFree(h->halo_n); cudaFree(h->halo_ptr); cudaFree(h->halo_rows);
     cudaFree(h->csr_rowptr); cudaFree(h->csr_col); cudaFree(h->csr_val); cudaFree(h->csr_area);
     if (h->h_pinned) cudaFreeHost(h->h_pinned);
     cudaSetDevice(prev);
@@ -496,6 +582,51 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     IF_LAUNCH_CHECK();
     IF_CUDA_TRY(cudaStreamSynchronize(st));
 
+    // ---- row tiles of the SpMM kernel: halo lists and tile-local column ids
+    const int64_t n_tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
+    h->n_tiles = n_tiles;
+    int log2c = 0;
+    while ((1 << log2c) < C) ++log2c;
+    DevBuf halo_n, halo_cnt, halo_ptr, halo_rows, lcol;
+    IF_CUDA_TRY(halo_n.alloc((size_t)n_tiles * 4));
+    IF_CUDA_TRY(halo_cnt.alloc((size_t)(n_tiles + 1) * 8));
+    IF_CUDA_TRY(halo_ptr.alloc((size_t)(n_tiles + 1) * 8));
+    IF_CUDA_TRY(lcol.alloc((size_t)sell_slots * 4 + 16));
+    IF_CUDA_TRY(cudaMemsetAsync(halo_cnt.p, 0, (size_t)(n_tiles + 1) * 8, st));
+    k_tile_halo<<<(unsigned)n_tiles, 128, 0, st>>>(chunk_ptr.as<int64_t>(), scol.as<int32_t>(), nv, log2c, 0,
+                                                   halo_n.as<int32_t>(), halo_cnt.as<int64_t>(), nullptr, nullptr,
+                                                   nullptr);
+    IF_LAUNCH_CHECK();
+    tb = 0;
+    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(nullptr, tb, halo_cnt.as<int64_t>(), halo_ptr.as<int64_t>(),
+                                              n_tiles + 1, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(tmp.p, tb, halo_cnt.as<int64_t>(), halo_ptr.as<int64_t>(), n_tiles + 1,
+                                              st));
+    ++g_launches;
+    int64_t halo_total = 0;
+    IF_CUDA_TRY(cudaMemcpyAsync(&halo_total, halo_ptr.as<int64_t>() + n_tiles, 8, cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    h->halo_total = halo_total;
+    IF_CUDA_TRY(halo_rows.alloc((size_t)halo_total * 4 + 16));
+    k_tile_halo<<<(unsigned)n_tiles, 128, 0, st>>>(chunk_ptr.as<int64_t>(), scol.as<int32_t>(), nv, log2c, 1,
+                                                   halo_n.as<int32_t>(), halo_cnt.as<int64_t>(),
+                                                   halo_ptr.as<int64_t>(), halo_rows.as<int32_t>(),
+                                                   lcol.as<int32_t>());
+    IF_LAUNCH_CHECK();
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    {
+        std::vector<int32_t> hn((size_t)n_tiles);
+        IF_CUDA_TRY(cudaMemcpy(hn.data(), halo_n.p, (size_t)n_tiles * 4, cudaMemcpyDeviceToHost));
+        h->unstaged_tiles = 0;
+        h->halo_max = 0;
+        for (int32_t v : hn) { if (v < 0) ++h->unstaged_tiles; else if (v > h->halo_max) h->halo_max = v; }
+    }
+    h->sell_lcol = (int32_t*)lcol.release();
+    h->halo_n = (int32_t*)halo_n.release();
+    h->halo_ptr = (int64_t*)halo_ptr.release();
+    h->halo_rows = (int32_t*)halo_rows.release();
+
     if (opt.flags & IF_FLAG_KEEP_CSR) {
         // v0 holds [9 n_tri] doubles; keep a right-sized copy instead
         DevBuf cval;
@@ -547,6 +678,16 @@ extern "C" int if_mesh_info(if_handle h, int64_t* n_vert, int64_t* nnz, double* 
     if (total_area) *total_area = h->total_area;
     if (mean_edge) *mean_edge = h->mean_edge;
     if (sell_slots) *sell_slots = h->sell_slots;
+    return IF_OK;
+}
+
+extern "C" int if_mesh_tile_info(if_handle h, int64_t* n_tiles, int64_t* halo_rows, int64_t* halo_max,
+                                 int64_t* unstaged_tiles) {
+    if (!h) return IF_EINVAL;
+    if (n_tiles) *n_tiles = h->n_tiles;
+    if (halo_rows) *halo_rows = h->halo_total;
+    if (halo_max) *halo_max = h->halo_max;
+    if (unstaged_tiles) *unstaged_tiles = h->unstaged_tiles;
     return IF_OK;
 }
 

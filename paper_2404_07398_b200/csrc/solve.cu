@@ -88,7 +88,7 @@ template <int K>
 int setup_grids(Run& r) {
     const int64_t nv = r.h->n_vert;
     const int n_sm = r.h->n_sm;
-    const int64_t tiles = (nv + TileRows<K>::T - 1) / TileRows<K>::T;
+    const int64_t tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
     const int64_t passes = (nv + BLOCK / (K / 2) - 1) / (BLOCK / (K / 2));
     int rc;
     if ((rc = resident_grid(k_spmm<K, MODE_PLAIN>, TileSmem<K, MODE_PLAIN>::bytes, n_sm, tiles, &r.g.plain))) return rc;
@@ -419,7 +419,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     int log2c = 0;
     while ((1 << log2c) < h->sell_c) ++log2c;
     r.m = MeshView{h->chunk_ptr, h->sell_col, h->sell_val, h->area, h->inv_area, h->sdiag, h->gdiag, h->perm,
-                   h->n_vert, h->n_chunks, log2c};
+                   h->sell_lcol, h->halo_n, h->halo_ptr, h->halo_rows, h->n_vert, h->n_chunks, log2c};
 
     PollState poll;
     int expected = 0;
