@@ -68,7 +68,8 @@ typedef struct {
     int check_every; /* 0 => 16; iterations per CUDA-graph launch = between two polls of the done flag     */
     int batch;       /* right-hand sides per SpMM: 4, 8 or 16; 0 => 16                                      */
     int sell_c;      /* SELL chunk height C (rows sharing one padded width): 32, 64 or 128; 0 => 32          */
-    int sell_sigma;  /* SELL sorting window sigma (rows): multiple of sell_c; 0 => 256; == sell_c: no sort  */
+    int sell_sigma;  /* SELL sorting window sigma (rows): multiple of sell_c; 0 => 128 (the SpMM row tile; a
+                        larger window scatters a tile over the window and defeats the halo staging)         */
     int sfc_kind;    /* 0 => Morton order of the quantised coordinates; 1 => keep the caller's order        */
     int flags;       /* IF_FLAG_*                                                                           */
 } if_options;

@@ -43,7 +43,7 @@ struct Options {
     int check_every = 16;
     int batch = 16;
     int sell_c = 32;
-    int sell_sigma = 256;
+    int sell_sigma = 128;   // = TILE_ROWS: sorting inside a row tile keeps the tile spatially compact
     int sfc_kind = 0;
     int flags = 0;
 };
@@ -74,8 +74,8 @@ struct if_mesh_s {
     // with tile-local column ids (tile row r -> r, halo slot s -> TILE_ROWS + s); halo_n = -1: tile not staged
     int32_t* sell_lcol = nullptr;   // [sell_slots]
     int32_t* halo_n = nullptr;      // [n_tiles]
-    int64_t* halo_ptr = nullptr;    // [n_tiles+1]
-    int32_t* halo_rows = nullptr;   // [halo_ptr[n_tiles]]
+    int32_t* halo_rows = nullptr;   // [n_tiles][HALO_CAP], unused entries = the tile's first row
+    int32_t* tile_desc = nullptr;   // [n_tiles+1][16] per-tile descriptor (see k_tile_halo)
     int64_t n_tiles = 0;
     int64_t halo_total = 0;
     int64_t halo_max = 0;         // largest staged halo

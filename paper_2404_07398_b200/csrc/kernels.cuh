@@ -40,9 +40,8 @@ struct MeshView {
     const double* __restrict__ gdiag;
     const int32_t* __restrict__ perm;
     const int32_t* __restrict__ lcol;       // tile-local column ids (tile row, or TILE_ROWS + halo slot)
-    const int32_t* __restrict__ halo_n;     // [tiles] halo rows of the tile, -1: not staged (use col)
-    const int64_t* __restrict__ halo_ptr;   // [tiles+1]
-    const int32_t* __restrict__ halo_rows;  // out-of-tile rows each tile gathers from, ascending per tile
+    const int32_t* __restrict__ halo_rows;  // [tiles][HALO_CAP] out-of-tile rows each tile gathers from
+    const int32_t* __restrict__ tile_desc;  // [tiles+1][16] first slot, slots, halo rows | -1, slice offsets
     int64_t nv;
     int64_t n_chunks;
     int log2c;
@@ -184,7 +183,7 @@ struct SpmmArgs {
 
 // dynamic shared memory of k_spmm:
 //   [gathered vector: T tile rows + HALO_CAP halo rows][second vector: T rows][val slice][col slice]
-//   [S_vv][A_v | 1/A_v][chunk offsets][mbarrier]
+//   [S_vv][A_v | 1/A_v][two tile descriptors][mbarrier]
 template <int K, int MODE> struct TileSmem {
     static constexpr int T = TILE_ROWS;
     static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // vectors that arrive by bulk copy
@@ -195,7 +194,7 @@ template <int K, int MODE> struct TileSmem {
     static constexpr size_t off_dg = off_col + (size_t)T * WCAP * sizeof(int32_t);   // S_vv of the tile's rows
     static constexpr size_t off_ar = off_dg + (size_t)T * sizeof(double);            // A_v or 1/A_v
     static constexpr size_t off_cp = off_ar + (size_t)T * sizeof(double);
-    static constexpr size_t off_bar = off_cp + 16 * sizeof(int32_t);
+    static constexpr size_t off_bar = off_cp + 32 * sizeof(int32_t);
     static constexpr size_t bytes = off_bar + 16;
 };
 
@@ -217,7 +216,7 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
     const int32_t* scol = reinterpret_cast<const int32_t*>(smem + SM::off_col);
     const double* sdg = reinterpret_cast<const double*>(smem + SM::off_dg);
     const double* sar = reinterpret_cast<const double*>(smem + SM::off_ar);
-    int32_t* scp = reinterpret_cast<int32_t*>(smem + SM::off_cp);
+    int32_t* sdesc = reinterpret_cast<int32_t*>(smem + SM::off_cp);   // [2][16] tile descriptors
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + SM::off_bar);
     // the per-row factor next to S_vv: A_v for q = A_v p + c S v, 1/A_v for t = M^-1 S v
     const double* __restrict__ rowfac =
@@ -239,18 +238,28 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
     double2 acc[1] = {{0.0, 0.0}};
     const int C = 1 << m.log2c;
     const int64_t ntiles = (m.nv + T - 1) / T;
-    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    // Tile descriptors (first slot, slots, halo rows, slice offsets) and the halo row ids are fetched one tile
+    // ahead, so that at the top of a tile every load it needs can be issued at once, with no dependent chain.
+    int64_t tile = blockIdx.x;
+    int hidx[HPT];
+    if (tile < ntiles) {
+        if (tid < 16) sdesc[tid] = m.tile_desc[tile * 16 + tid];
+#pragma unroll
+        for (int i = 0; i < HPT; ++i) hidx[i] = m.halo_rows[tile * HALO_CAP + tid / TPR + i * ROWS];
+    }
+    int par = 0;
+    for (; tile < ntiles; tile += gridDim.x) {
         const int64_t row0 = tile * T;
         const int nrows = (int)min((int64_t)T, m.nv - row0);
         const uint32_t vbytes = (uint32_t)nrows * K * sizeof(double);
-        const int64_t ch0 = row0 >> m.log2c;
-        const int nch = (nrows + C - 1) >> m.log2c;
-        const int64_t cp_first = m.chunk_ptr[ch0];
-        const int64_t slots = m.chunk_ptr[ch0 + nch] - cp_first;
-        const int nh = m.halo_n[tile];
+        __syncthreads();   // everyone is done reading the previous tile; this tile's descriptor is visible
+        const int32_t* d = sdesc + par * 16;
+        const int64_t cp_first = (int64_t)(uint32_t)d[0] | ((int64_t)d[1] << 32);
+        const int slots = d[2];
+        const int nh = d[3];
+        const int32_t* scp = d + 4;
         // staged tile: matrix slice and halo fit shared memory, columns are tile-local indices, no branches
-        const bool staged = nh >= 0 && slots <= (int64_t)T * WCAP;
-        __syncthreads();   // everyone is done reading the previous tile (and the barrier is initialised)
+        const bool staged = nh >= 0 && slots <= T * WCAP;
         if (tid == 0) {
             bulk_wait_read0();   // the previous tile's bulk store has finished reading sa
             const uint32_t dbytes = ((uint32_t)nrows * 8u + 15u) & ~15u;   // the arrays are padded by 16 bytes
@@ -264,8 +273,18 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
                 bulk_load(const_cast<int32_t*>(scol), m.lcol + cp_first, (uint32_t)slots * 4u, bar);
             }
         }
-        if (tid <= nch) scp[tid] = (int32_t)(m.chunk_ptr[ch0 + tid] - cp_first);
-        // while the bulk copies fly: x of the tile into registers, the halo rows into shared memory
+        // while the bulk copies fly: the halo rows (from L2) and x of the tile into registers ...
+        double2 h0[HPT], h1[HPT];
+        if (staged) {
+#pragma unroll
+            for (int i = 0; i < HPT; ++i) {
+                if (tid / TPR + i * ROWS < nh) {
+                    const int64_t j = hidx[i];
+                    h0[i] = ld2(a.in0, j * K + 2 * l);
+                    if (CG_A) h1[i] = ld2(a.in1, j * K + 2 * l);
+                }
+            }
+        }
         double2 xv[XPT];
         if (CG_A) {
 #pragma unroll
@@ -274,18 +293,16 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
                 if (e < nrows * TPR) xv[i] = ld2(a.x, row0 * K + 2 * (int64_t)e);
             }
         }
-        if (staged) {
-            const int64_t hp = m.halo_ptr[tile];
-            double2 h0[HPT], h1[HPT];
+        // ... and the next tile's descriptor and halo row ids (used one iteration later)
+        const int64_t ntile = tile + gridDim.x;
+        int dnext = 0;
+        int hnext[HPT];
+        if (ntile < ntiles) {
+            if (tid < 16) dnext = m.tile_desc[ntile * 16 + tid];
 #pragma unroll
-            for (int i = 0; i < HPT; ++i) {
-                const int hh = tid / TPR + i * ROWS;
-                if (hh < nh) {
-                    const int64_t j = m.halo_rows[hp + hh];
-                    h0[i] = ld2(a.in0, j * K + 2 * l);
-                    if (CG_A) h1[i] = ld2(a.in1, j * K + 2 * l);
-                }
-            }
+            for (int i = 0; i < HPT; ++i) hnext[i] = m.halo_rows[ntile * HALO_CAP + tid / TPR + i * ROWS];
+        }
+        if (staged) {
 #pragma unroll
             for (int i = 0; i < HPT; ++i) {
                 const int hh = tid / TPR + i * ROWS;
@@ -392,6 +409,10 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
                 acc[0].y = fma(pv.y, q.y, acc[0].y);
             }
         }
+        if (tid < 16) sdesc[(par ^ 1) * 16 + tid] = dnext;
+#pragma unroll
+        for (int i = 0; i < HPT; ++i) hidx[i] = hnext[i];
+        par ^= 1;
     }
     if (CG_A && tid == 0) bulk_wait0();
     if (MODE == MODE_CG1 || MODE == MODE_CG2B) {

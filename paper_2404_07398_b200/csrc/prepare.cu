@@ -249,13 +249,16 @@ __global__ void k_sell_fill(const int32_t* __restrict__ perm, const int32_t* __r
 }
 
 
-// Per row tile of TILE_ROWS rows (one block each): the sorted, unique out-of-tile columns ("halo") and the SELL
-// columns rewritten as tile-local ids.  Pass 1 (write = 0) only counts; pass 2 fills halo_rows and lcol.
+// Per row tile of TILE_ROWS rows (one block each): the sorted, unique out-of-tile columns ("halo", stored with a
+// fixed stride of HALO_CAP per tile, unused entries = the tile's first row), the SELL columns rewritten as
+// tile-local ids, and a 64-byte descriptor the SpMM kernel prefetches one tile ahead:
+//   desc[0..1] first SELL slot of the tile (int64), [2] slots, [3] halo rows or -1 (tile not staged),
+//   desc[4..12] slot offset of each SELL slice of the tile relative to the first (TILE_ROWS/C + 1 entries)
 constexpr int ECAP = 1024;   // out-of-tile references a tile may have before it is left unstaged
 __global__ void __launch_bounds__(128) k_tile_halo(const int64_t* __restrict__ chunk_ptr, const int32_t* __restrict__ col,
-                                                   int64_t nv, int log2c, int write, int32_t* __restrict__ halo_n,
-                                                   int64_t* __restrict__ halo_cnt, const int64_t* __restrict__ halo_ptr,
-                                                   int32_t* __restrict__ halo_rows, int32_t* __restrict__ lcol) {
+                                                   int64_t nv, int log2c, int32_t* __restrict__ halo_n,
+                                                   int32_t* __restrict__ halo_rows, int32_t* __restrict__ lcol,
+                                                   int32_t* __restrict__ desc) {
     __shared__ int ext[ECAP];
     __shared__ int n_ext, n_uniq;
     const int tid = threadIdx.x;
@@ -306,28 +309,31 @@ __global__ void __launch_bounds__(128) k_tile_halo(const int64_t* __restrict__ c
         over = n_uniq > HALO_CAP;
     }
     const int nu = over ? -1 : n_uniq;
-    if (!write) {
-        if (tid == 0) { halo_n[tile] = nu; halo_cnt[tile] = nu > 0 ? nu : 0; }
-        return;
+    if (tid == 0) halo_n[tile] = nu;
+    if (tid < 16) {
+        int v = 0;
+        if (tid == 0) v = (int)(cp_first & 0xffffffffll);
+        else if (tid == 1) v = (int)(cp_first >> 32);
+        else if (tid == 2) v = (int)slots;
+        else if (tid == 3) v = nu;
+        else if (tid - 4 <= nch) v = (int)(chunk_ptr[ch0 + tid - 4] - cp_first);
+        desc[tile * 16 + tid] = v;
     }
-    if (nu < 0) {
-        for (int64_t s = tid; s < slots; s += 128) lcol[cp_first + s] = 0;
-        return;
-    }
-    const int64_t hp = halo_ptr[tile];
-    for (int i = tid; i < nu; i += 128) halo_rows[hp + i] = ext[i];
+    for (int i = tid; i < HALO_CAP; i += 128) halo_rows[tile * HALO_CAP + i] = (nu > 0 && i < nu) ? ext[i] : (int)row0;
     for (int64_t s = tid; s < slots; s += 128) {
-        const int64_t c = col[cp_first + s];
-        int lc;
-        if (c >= row0 && c < row0 + nrows) {
-            lc = (int)(c - row0);
-        } else {
-            int lo = 0, hi = nu - 1;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (ext[mid] < (int)c) lo = mid + 1; else hi = mid;
+        int lc = 0;
+        if (nu >= 0) {
+            const int64_t c = col[cp_first + s];
+            if (c >= row0 && c < row0 + nrows) {
+                lc = (int)(c - row0);
+            } else {
+                int lo = 0, hi = nu - 1;
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (ext[mid] < (int)c) lo = mid + 1; else hi = mid;
+                }
+                lc = TILE_ROWS + lo;
             }
-            lc = TILE_ROWS + lo;
         }
         lcol[cp_first + s] = lc;
     }
@@ -375,7 +381,7 @@ extern "C" void if_destroy(if_handle h) {
     cudaSetDevice(h->device);
     cudaFree(h->chunk_ptr); cudaFree(h->sell_col); cudaFree(h->sell_val); cudaFree(h->area);
     cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->perm); cudaFree(h->iperm);
-    cudaFree(h->sell_lcol); cudaFree(h->halo_n); cudaFree(h->halo_ptr); cudaFree(h->halo_rows);
+    cudaFree(h->sell_lcol); cudaFree(h->halo_n); cudaFree(h->tile_desc); cudaFree(h->halo_rows);
     cudaFree(h->csr_rowptr); cudaFree(h->csr_col); cudaFree(h->csr_val); cudaFree(h->csr_area);
     if (h->h_pinned) cudaFreeHost(h->h_pinned);
     cudaSetDevice(prev);
@@ -587,32 +593,15 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     h->n_tiles = n_tiles;
     int log2c = 0;
     while ((1 << log2c) < C) ++log2c;
-    DevBuf halo_n, halo_cnt, halo_ptr, halo_rows, lcol;
+    DevBuf halo_n, halo_rows, lcol, tile_desc;
     IF_CUDA_TRY(halo_n.alloc((size_t)n_tiles * 4));
-    IF_CUDA_TRY(halo_cnt.alloc((size_t)(n_tiles + 1) * 8));
-    IF_CUDA_TRY(halo_ptr.alloc((size_t)(n_tiles + 1) * 8));
+    IF_CUDA_TRY(halo_rows.alloc((size_t)n_tiles * HALO_CAP * 4));
+    IF_CUDA_TRY(tile_desc.alloc((size_t)(n_tiles + 1) * 64));
+    IF_CUDA_TRY(cudaMemsetAsync(tile_desc.p, 0, (size_t)(n_tiles + 1) * 64, st));
     IF_CUDA_TRY(lcol.alloc((size_t)sell_slots * 4 + 16));
-    IF_CUDA_TRY(cudaMemsetAsync(halo_cnt.p, 0, (size_t)(n_tiles + 1) * 8, st));
-    k_tile_halo<<<(unsigned)n_tiles, 128, 0, st>>>(chunk_ptr.as<int64_t>(), scol.as<int32_t>(), nv, log2c, 0,
-                                                   halo_n.as<int32_t>(), halo_cnt.as<int64_t>(), nullptr, nullptr,
-                                                   nullptr);
-    IF_LAUNCH_CHECK();
-    tb = 0;
-    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(nullptr, tb, halo_cnt.as<int64_t>(), halo_ptr.as<int64_t>(),
-                                              n_tiles + 1, st));
-    IF_CUDA_TRY(tmp.alloc(tb));
-    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(tmp.p, tb, halo_cnt.as<int64_t>(), halo_ptr.as<int64_t>(), n_tiles + 1,
-                                              st));
-    ++g_launches;
-    int64_t halo_total = 0;
-    IF_CUDA_TRY(cudaMemcpyAsync(&halo_total, halo_ptr.as<int64_t>() + n_tiles, 8, cudaMemcpyDeviceToHost, st));
-    IF_CUDA_TRY(cudaStreamSynchronize(st));
-    h->halo_total = halo_total;
-    IF_CUDA_TRY(halo_rows.alloc((size_t)halo_total * 4 + 16));
-    k_tile_halo<<<(unsigned)n_tiles, 128, 0, st>>>(chunk_ptr.as<int64_t>(), scol.as<int32_t>(), nv, log2c, 1,
-                                                   halo_n.as<int32_t>(), halo_cnt.as<int64_t>(),
-                                                   halo_ptr.as<int64_t>(), halo_rows.as<int32_t>(),
-                                                   lcol.as<int32_t>());
+    k_tile_halo<<<(unsigned)n_tiles, 128, 0, st>>>(chunk_ptr.as<int64_t>(), scol.as<int32_t>(), nv, log2c,
+                                                   halo_n.as<int32_t>(), halo_rows.as<int32_t>(), lcol.as<int32_t>(),
+                                                   tile_desc.as<int32_t>());
     IF_LAUNCH_CHECK();
     IF_CUDA_TRY(cudaStreamSynchronize(st));
     {
@@ -620,11 +609,16 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
         IF_CUDA_TRY(cudaMemcpy(hn.data(), halo_n.p, (size_t)n_tiles * 4, cudaMemcpyDeviceToHost));
         h->unstaged_tiles = 0;
         h->halo_max = 0;
-        for (int32_t v : hn) { if (v < 0) ++h->unstaged_tiles; else if (v > h->halo_max) h->halo_max = v; }
+        h->halo_total = 0;
+        for (int32_t v : hn) {
+            if (v < 0) { ++h->unstaged_tiles; continue; }
+            h->halo_total += v;
+            if (v > h->halo_max) h->halo_max = v;
+        }
     }
     h->sell_lcol = (int32_t*)lcol.release();
     h->halo_n = (int32_t*)halo_n.release();
-    h->halo_ptr = (int64_t*)halo_ptr.release();
+    h->tile_desc = (int32_t*)tile_desc.release();
     h->halo_rows = (int32_t*)halo_rows.release();
 
     if (opt.flags & IF_FLAG_KEEP_CSR) {

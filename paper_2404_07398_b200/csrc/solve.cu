@@ -419,7 +419,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     int log2c = 0;
     while ((1 << log2c) < h->sell_c) ++log2c;
     r.m = MeshView{h->chunk_ptr, h->sell_col, h->sell_val, h->area, h->inv_area, h->sdiag, h->gdiag, h->perm,
-                   h->sell_lcol, h->halo_n, h->halo_ptr, h->halo_rows, h->n_vert, h->n_chunks, log2c};
+                   h->sell_lcol, h->halo_rows, h->tile_desc, h->n_vert, h->n_chunks, log2c};
 
     PollState poll;
     int expected = 0;
