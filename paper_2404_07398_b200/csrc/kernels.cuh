@@ -124,11 +124,11 @@ __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_
 // Fixed-order block reduction of NV double2 accumulators per thread over the threads owning the same column
 // pair, then a ticket: the last block to arrive sums all blocks' partials in block order.
 // Returns true in the last block, with the totals of value set j, column c in tot[j*KMAX + c] (shared memory).
-template <int K, int NV>
+template <int K, int NV, int NT = BLOCK>
 __device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __restrict__ partials,
                                             unsigned int* ticket, double* tot /* shared [NV*KMAX] */) {
     constexpr int TPR = K / 2;
-    __shared__ double2 red[BLOCK];
+    __shared__ double2 red[NT];
     __shared__ bool is_last;
     const int tid = threadIdx.x;
     for (int j = 0; j < NV; ++j) {
@@ -136,7 +136,7 @@ __device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __
         __syncthreads();
         if (tid < TPR) {
             double2 s = red[tid];
-            for (int i = tid + TPR; i < BLOCK; i += TPR) { s.x += red[i].x; s.y += red[i].y; }
+            for (int i = tid + TPR; i < NT; i += TPR) { s.x += red[i].x; s.y += red[i].y; }
             partials[((size_t)j * gridDim.x + blockIdx.x) * K + 2 * tid] = s.x;
             partials[((size_t)j * gridDim.x + blockIdx.x) * K + 2 * tid + 1] = s.y;
         }
@@ -150,8 +150,8 @@ __device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __
     __syncthreads();
     if (!is_last) return false;
     __threadfence();
-    double* redd = reinterpret_cast<double*>(red);   // [BLOCK] doubles (uses half of red)
-    constexpr int LANES = BLOCK / K;                  // threads per column
+    double* redd = reinterpret_cast<double*>(red);   // [NT] doubles (uses half of red)
+    constexpr int LANES = NT / K;                  // threads per column
     for (int j = 0; j < NV; ++j) {
         const int c = tid % K, lane = tid / K;
         double s = 0.0;
@@ -181,9 +181,11 @@ struct SpmmArgs {
     int out_idx;         // CG1/CG2A: index of the direction buffer written (recorded in ctrl->cur_p)
 };
 
-// dynamic shared memory of k_spmm:
-//   [gathered vector: T tile rows + HALO_CAP halo rows][second vector: T rows][val slice][col slice]
-//   [S_vv][A_v | 1/A_v][two tile descriptors][mbarrier]
+// dynamic shared memory of k_spmm: SPMM_STAGES stages of
+//   [gathered vector: T tile rows + HALO_CAP halo rows][second vector: T rows][val slice][col slice][S_vv][A_v | 1/A_v]
+// then a ring of four tile descriptors and one mbarrier per stage
+constexpr int SPMM_BLOCK = 512;
+constexpr int SPMM_STAGES = 3;
 template <int K, int MODE> struct TileSmem {
     static constexpr int T = TILE_ROWS;
     static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // vectors that arrive by bulk copy
@@ -193,67 +195,151 @@ template <int K, int MODE> struct TileSmem {
     static constexpr size_t off_col = off_val + (size_t)T * WCAP * sizeof(double);
     static constexpr size_t off_dg = off_col + (size_t)T * WCAP * sizeof(int32_t);   // S_vv of the tile's rows
     static constexpr size_t off_ar = off_dg + (size_t)T * sizeof(double);            // A_v or 1/A_v
-    static constexpr size_t off_cp = off_ar + (size_t)T * sizeof(double);
-    static constexpr size_t off_bar = off_cp + 32 * sizeof(int32_t);
-    static constexpr size_t bytes = off_bar + 16;
+    static constexpr size_t stage_bytes = off_ar + (size_t)T * sizeof(double);
+    static constexpr size_t off_desc = SPMM_STAGES * stage_bytes;
+    static constexpr size_t off_bar = off_desc + 4 * 16 * sizeof(int32_t);
+    static constexpr size_t bytes = off_bar + 8 * SPMM_STAGES + 8;
 };
 
+// What one thread needs to issue the bulk copies of a tile (kept in registers by the issuing thread).
+struct TileIssue { int64_t cp_first; int slots; int nh; };
+__device__ __forceinline__ TileIssue load_issue(const int32_t* __restrict__ desc, int64_t tile) {
+    const int4 v = *reinterpret_cast<const int4*>(desc + tile * 16);
+    TileIssue t;
+    t.cp_first = (int64_t)(uint32_t)v.x | ((int64_t)v.y << 32);
+    t.slots = v.z;
+    t.nh = v.w;
+    return t;
+}
+
+// Software pipeline of one persistent CTA per SM (tile i being computed):
+//   bulk copies (TMA) of tiles i+1 and i+2 are in flight into the other two stages,
+//   x and the halo rows of tile i+1 are in flight into registers,
+//   descriptors and halo row ids are fetched two tiles ahead.
+// About 130 KB of loads per SM are outstanding at all times, which is what the loaded HBM latency of B200 needs.
 template <int K, int MODE>
-__global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
-                                                SpmmArgs a) {
+__global__ void __launch_bounds__(SPMM_BLOCK, 1) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
+                                                        double* __restrict__ partials, SpmmArgs a) {
     using SM = TileSmem<K, MODE>;
     constexpr int T = SM::T;
+    constexpr int NT = SPMM_BLOCK;
     constexpr int TPR = K / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    constexpr int XPT = T * TPR / BLOCK;                 // double2 elements of a tile vector per thread
+    constexpr int ROWS = NT / TPR;
+    constexpr int XPT = (T * TPR + NT - 1) / NT;         // double2 elements of a tile vector per thread
     constexpr int HPT = (HALO_CAP + ROWS - 1) / ROWS;    // halo rows per thread group
     constexpr bool CG_A = (MODE == MODE_CG1 || MODE == MODE_CG2A);
     if (MODE != MODE_PLAIN && ctrl->all_done) return;
     extern __shared__ __align__(128) unsigned char smem[];
-    double2* sa = reinterpret_cast<double2*>(smem);                  // gathered vector (z -> p', x, t): tile + halo
-    double2* sb = reinterpret_cast<double2*>(smem + SM::off_b);      // p_old, or own p' (CG2B)
-    const double* sval = reinterpret_cast<const double*>(smem + SM::off_val);
-    const int32_t* scol = reinterpret_cast<const int32_t*>(smem + SM::off_col);
-    const double* sdg = reinterpret_cast<const double*>(smem + SM::off_dg);
-    const double* sar = reinterpret_cast<const double*>(smem + SM::off_ar);
-    int32_t* sdesc = reinterpret_cast<int32_t*>(smem + SM::off_cp);   // [2][16] tile descriptors
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + SM::off_bar);
+    int32_t* sdesc = reinterpret_cast<int32_t*>(smem + SM::off_desc);   // [4][16] tile descriptors (ring)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::off_bar);   // one per stage
     // the per-row factor next to S_vv: A_v for q = A_v p + c S v, 1/A_v for t = M^-1 S v
     const double* __restrict__ rowfac =
         (MODE == MODE_CG2A || (MODE == MODE_PLAIN && a.scale_inv_area)) ? m.inv_area : m.area;
 
     const int tid = threadIdx.x;
     const int l = tid % TPR;
+    const int rg = tid / TPR;                            // row group of the thread
     double2 beta = {0.0, 0.0}, alpha = {0.0, 0.0}, cc = {0.0, 0.0};
     if (MODE != MODE_PLAIN) {
         beta = ld2(ctrl->beta, 2 * l);
         alpha = ld2(ctrl->alpha, 2 * l);
         cc = ld2(ctrl->c, 2 * l);
     }
-    if (tid == 0) {
-        mbar_init(bar, 1);
-        fence_proxy_async();
-    }
-    uint32_t parity = 0;
-    double2 acc[1] = {{0.0, 0.0}};
     const int C = 1 << m.log2c;
     const int64_t ntiles = (m.nv + T - 1) / T;
-    // Tile descriptors (first slot, slots, halo rows, slice offsets) and the halo row ids are fetched one tile
-    // ahead, so that at the top of a tile every load it needs can be issued at once, with no dependent chain.
-    int64_t tile = blockIdx.x;
-    int hidx[HPT];
-    if (tile < ntiles) {
-        if (tid < 16) sdesc[tid] = m.tile_desc[tile * 16 + tid];
-#pragma unroll
-        for (int i = 0; i < HPT; ++i) hidx[i] = m.halo_rows[tile * HALO_CAP + tid / TPR + i * ROWS];
-    }
-    int par = 0;
-    for (; tile < ntiles; tile += gridDim.x) {
+    const int64_t G = gridDim.x;
+    const int64_t tile0 = blockIdx.x;
+
+    auto issue = [&](int64_t tile, int stage, const TileIssue& ti) {   // thread 0 only
+        unsigned char* st = smem + (size_t)stage * SM::stage_bytes;
         const int64_t row0 = tile * T;
         const int nrows = (int)min((int64_t)T, m.nv - row0);
         const uint32_t vbytes = (uint32_t)nrows * K * sizeof(double);
-        __syncthreads();   // everyone is done reading the previous tile; this tile's descriptor is visible
-        const int32_t* d = sdesc + par * 16;
+        const uint32_t dbytes = ((uint32_t)nrows * 8u + 15u) & ~15u;   // the arrays are padded by 16 bytes
+        const bool staged = ti.nh >= 0 && ti.slots <= T * WCAP;
+        uint64_t* bar = &bars[stage];
+        mbar_expect_tx(bar, vbytes * SM::NVEC + 2u * dbytes + (staged ? (uint32_t)ti.slots * 12u : 0u));
+        bulk_load(st, a.in0 + row0 * K, vbytes, bar);
+        if (SM::NVEC >= 2) bulk_load(st + SM::off_b, a.in1 + row0 * K, vbytes, bar);
+        bulk_load(st + SM::off_dg, m.sdiag + row0, dbytes, bar);
+        bulk_load(st + SM::off_ar, rowfac + row0, dbytes, bar);
+        if (staged) {
+            bulk_load(st + SM::off_val, m.val + ti.cp_first, (uint32_t)ti.slots * 8u, bar);
+            bulk_load(st + SM::off_col, m.lcol + ti.cp_first, (uint32_t)ti.slots * 4u, bar);
+        }
+    };
+    auto load_halo = [&](const int (&idx)[HPT], int nh, double2 (&h0)[HPT], double2 (&h1)[HPT]) {
+#pragma unroll
+        for (int i = 0; i < HPT; ++i) {
+            if (rg + i * ROWS < nh) {
+                const int64_t j = idx[i];
+                h0[i] = ld2(a.in0, j * K + 2 * l);
+                if (CG_A) h1[i] = ld2(a.in1, j * K + 2 * l);
+            }
+        }
+    };
+    auto load_hidx = [&](int64_t tile, int (&idx)[HPT]) {
+#pragma unroll
+        for (int i = 0; i < HPT; ++i) {
+            const int hh = rg + i * ROWS;
+            idx[i] = (tile < ntiles && hh < HALO_CAP) ? m.halo_rows[tile * HALO_CAP + hh] : 0;
+        }
+    };
+    auto load_x = [&](int64_t tile, double2 (&xv)[XPT]) {
+        if (tile >= ntiles) return;
+        const int64_t row0 = tile * T;
+        const int nrows = (int)min((int64_t)T, m.nv - row0);
+#pragma unroll
+        for (int i = 0; i < XPT; ++i) {
+            const int e = tid + i * NT;
+            if (e < nrows * TPR) xv[i] = ld2(a.x, row0 * K + 2 * (int64_t)e);
+        }
+    };
+    if (tid == 0) {
+        for (int s = 0; s < SPMM_STAGES; ++s) mbar_init(&bars[s], 1);
+        fence_proxy_async();
+    }
+    // prologue: descriptors of the first two tiles, their bulk copies, halo and x of the first tile
+    if (tid < 32) {
+        const int64_t t = tile0 + (tid / 16) * G;
+        sdesc[tid] = t < ntiles ? m.tile_desc[t * 16 + tid % 16] : 0;
+    }
+    __syncthreads();
+    TileIssue tq{0, 0, -1};   // thread 0: what it needs to issue the tile two ahead
+    if (tid == 0) {
+        for (int k = 0; k < 2; ++k) {
+            const int64_t t = tile0 + k * G;
+            if (t < ntiles) issue(t, k, load_issue(m.tile_desc, t));
+        }
+        if (tile0 + 2 * G < ntiles) tq = load_issue(m.tile_desc, tile0 + 2 * G);
+    }
+    int hid_n[HPT];
+    double2 h0[HPT], h1[HPT], xv[XPT];
+    int dnext = 0;
+    if (tile0 < ntiles) {
+        int hid[HPT];
+        load_hidx(tile0, hid);
+        if (sdesc[3] >= 0 && sdesc[2] <= T * WCAP) load_halo(hid, sdesc[3], h0, h1);
+        if (CG_A) load_x(tile0, xv);
+        load_hidx(tile0 + G, hid_n);
+    }
+    double2 acc[1] = {{0.0, 0.0}};
+    int64_t tile = tile0;
+    for (int64_t it = 0; tile < ntiles; ++it, tile += G) {
+        const int stage = (int)(it % SPMM_STAGES);
+        const uint32_t parity = (uint32_t)(it / SPMM_STAGES) & 1u;
+        unsigned char* st = smem + (size_t)stage * SM::stage_bytes;
+        double2* sa = reinterpret_cast<double2*>(st);                    // gathered vector: tile + halo
+        double2* sb = reinterpret_cast<double2*>(st + SM::off_b);        // p_old, or own p' (CG2B)
+        const double* sval = reinterpret_cast<const double*>(st + SM::off_val);
+        const int32_t* scol = reinterpret_cast<const int32_t*>(st + SM::off_col);
+        const double* sdg = reinterpret_cast<const double*>(st + SM::off_dg);
+        const double* sar = reinterpret_cast<const double*>(st + SM::off_ar);
+        const int64_t row0 = tile * T;
+        const int nrows = (int)min((int64_t)T, m.nv - row0);
+        const uint32_t vbytes = (uint32_t)nrows * K * sizeof(double);
+        __syncthreads();   // tile it-1 is fully consumed; the descriptor of tile it+1 is visible
+        const int32_t* d = sdesc + (it & 3) * 16;
         const int64_t cp_first = (int64_t)(uint32_t)d[0] | ((int64_t)d[1] << 32);
         const int slots = d[2];
         const int nh = d[3];
@@ -261,51 +347,18 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
         // staged tile: matrix slice and halo fit shared memory, columns are tile-local indices, no branches
         const bool staged = nh >= 0 && slots <= T * WCAP;
         if (tid == 0) {
-            bulk_wait_read0();   // the previous tile's bulk store has finished reading sa
-            const uint32_t dbytes = ((uint32_t)nrows * 8u + 15u) & ~15u;   // the arrays are padded by 16 bytes
-            mbar_expect_tx(bar, vbytes * SM::NVEC + 2u * dbytes + (staged ? (uint32_t)slots * 12u : 0u));
-            bulk_load(sa, a.in0 + row0 * K, vbytes, bar);
-            if (SM::NVEC >= 2) bulk_load(sb, a.in1 + row0 * K, vbytes, bar);
-            bulk_load(const_cast<double*>(sdg), m.sdiag + row0, dbytes, bar);
-            bulk_load(const_cast<double*>(sar), rowfac + row0, dbytes, bar);
-            if (staged) {
-                bulk_load(const_cast<double*>(sval), m.val + cp_first, (uint32_t)slots * 8u, bar);
-                bulk_load(const_cast<int32_t*>(scol), m.lcol + cp_first, (uint32_t)slots * 4u, bar);
+            const int64_t t2 = tile + 2 * G;
+            if (t2 < ntiles) {
+                bulk_wait_read0();   // the stage of tile it-1 is free once its bulk store has been read
+                issue(t2, (int)((it + 2) % SPMM_STAGES), tq);
             }
+            if (t2 + G < ntiles) tq = load_issue(m.tile_desc, t2 + G);
         }
-        // while the bulk copies fly: the halo rows (from L2) and x of the tile into registers ...
-        double2 h0[HPT], h1[HPT];
+        // halo of this tile: registers -> shared memory
         if (staged) {
 #pragma unroll
             for (int i = 0; i < HPT; ++i) {
-                if (tid / TPR + i * ROWS < nh) {
-                    const int64_t j = hidx[i];
-                    h0[i] = ld2(a.in0, j * K + 2 * l);
-                    if (CG_A) h1[i] = ld2(a.in1, j * K + 2 * l);
-                }
-            }
-        }
-        double2 xv[XPT];
-        if (CG_A) {
-#pragma unroll
-            for (int i = 0; i < XPT; ++i) {
-                const int e = tid + i * BLOCK;
-                if (e < nrows * TPR) xv[i] = ld2(a.x, row0 * K + 2 * (int64_t)e);
-            }
-        }
-        // ... and the next tile's descriptor and halo row ids (used one iteration later)
-        const int64_t ntile = tile + gridDim.x;
-        int dnext = 0;
-        int hnext[HPT];
-        if (ntile < ntiles) {
-            if (tid < 16) dnext = m.tile_desc[ntile * 16 + tid];
-#pragma unroll
-            for (int i = 0; i < HPT; ++i) hnext[i] = m.halo_rows[ntile * HALO_CAP + tid / TPR + i * ROWS];
-        }
-        if (staged) {
-#pragma unroll
-            for (int i = 0; i < HPT; ++i) {
-                const int hh = tid / TPR + i * ROWS;
+                const int hh = rg + i * ROWS;
                 if (hh < nh) {
                     double2 g = h0[i];
                     if (CG_A) { g.x = fma(beta.x, h1[i].x, g.x); g.y = fma(beta.y, h1[i].y, g.y); }
@@ -313,13 +366,19 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
                 }
             }
         }
-        mbar_wait(bar, parity);
-        parity ^= 1u;
+        // next tile: its halo rows into registers; two ahead: halo row ids and descriptor
+        {
+            const int32_t* d1 = sdesc + ((it + 1) & 3) * 16;
+            if (tile + G < ntiles && d1[3] >= 0 && d1[2] <= T * WCAP) load_halo(hid_n, d1[3], h0, h1);
+            load_hidx(tile + 2 * G, hid_n);
+            if (tid < 16) dnext = tile + 2 * G < ntiles ? m.tile_desc[(tile + 2 * G) * 16 + tid] : 0;
+        }
+        mbar_wait(&bars[stage], parity);
         if (CG_A) {
             // p' = z + beta p (in place over z, goes back with a bulk store) ; x += alpha_prev p
 #pragma unroll
             for (int i = 0; i < XPT; ++i) {
-                const int e = tid + i * BLOCK;
+                const int e = tid + i * NT;
                 if (e < nrows * TPR) {
                     const double2 zv = sa[e], pv = sb[e];
                     double2 own;
@@ -331,6 +390,7 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
                     st2(a.x, row0 * K + 2 * (int64_t)e, xv[i]);
                 }
             }
+            load_x(tile + G, xv);   // x of the next tile flies during the gather
             fence_proxy_async();
         }
         __syncthreads();
@@ -338,7 +398,7 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
             bulk_store(a.out1 + row0 * K, sa, vbytes);
             bulk_commit();
         }
-        for (int r = tid / TPR; r < nrows; r += ROWS) {
+        for (int r = rg; r < nrows; r += ROWS) {
             const int64_t row = row0 + r;
             const int chl = r >> m.log2c;
             const int cpr = scp[chl];
@@ -409,15 +469,12 @@ __global__ void __launch_bounds__(BLOCK, 2) k_spmm(MeshView m, Ctrl* __restrict_
                 acc[0].y = fma(pv.y, q.y, acc[0].y);
             }
         }
-        if (tid < 16) sdesc[(par ^ 1) * 16 + tid] = dnext;
-#pragma unroll
-        for (int i = 0; i < HPT; ++i) hidx[i] = hnext[i];
-        par ^= 1;
+        if (tid < 16) sdesc[((it + 2) & 3) * 16 + tid] = dnext;
     }
     if (CG_A && tid == 0) bulk_wait0();
     if (MODE == MODE_CG1 || MODE == MODE_CG2B) {
         __shared__ double tot[KMAX];
-        if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[0], tot)) {
+        if (grid_reduce<K, 1, NT>(acc, partials, &ctrl->ticket[0], tot)) {
             if (tid < K) {
                 const double pq = tot[tid];
                 double al = 0.0;

@@ -70,11 +70,11 @@ struct Run {
 };
 
 template <class Kern>
-int resident_grid(Kern kern, size_t smem, int n_sm, int64_t work_items, int* grid) {
+int resident_grid(Kern kern, size_t smem, int n_sm, int64_t work_items, int* grid, int block = BLOCK) {
     if (smem > 0)   // static + dynamic shared memory may pass 48 KB: always opt in
         IF_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    IF_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLOCK, smem));
+    IF_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, block, smem));
     if (occ < 1) {
         fprintf(stderr, "[implicit_filter] kernel does not fit an SM (dynamic shared memory %zu bytes)\n", smem);
         return IF_ECUDA;
@@ -91,13 +91,13 @@ int setup_grids(Run& r) {
     const int64_t tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
     const int64_t passes = (nv + BLOCK / (K / 2) - 1) / (BLOCK / (K / 2));
     int rc;
-    if ((rc = resident_grid(k_spmm<K, MODE_PLAIN>, TileSmem<K, MODE_PLAIN>::bytes, n_sm, tiles, &r.g.plain))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_PLAIN>, TileSmem<K, MODE_PLAIN>::bytes, n_sm, tiles, &r.g.plain, SPMM_BLOCK))) return rc;
     if (r.order_n == 1) {
-        if ((rc = resident_grid(k_spmm<K, MODE_CG1>, TileSmem<K, MODE_CG1>::bytes, n_sm, tiles, &r.g.cga))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_CG1>, TileSmem<K, MODE_CG1>::bytes, n_sm, tiles, &r.g.cga, SPMM_BLOCK))) return rc;
     } else {
-        if ((rc = resident_grid(k_spmm<K, MODE_CG2A>, TileSmem<K, MODE_CG2A>::bytes, n_sm, tiles, &r.g.cga))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_CG2A>, TileSmem<K, MODE_CG2A>::bytes, n_sm, tiles, &r.g.cga, SPMM_BLOCK))) return rc;
     }
-    if ((rc = resident_grid(k_spmm<K, MODE_CG2B>, TileSmem<K, MODE_CG2B>::bytes, n_sm, tiles, &r.g.cgb))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_CG2B>, TileSmem<K, MODE_CG2B>::bytes, n_sm, tiles, &r.g.cgb, SPMM_BLOCK))) return rc;
     if ((rc = resident_grid(k_update<K>, 0, n_sm, passes, &r.g.update))) return rc;
     r.g.stream = (int)std::max<int64_t>(1, std::min<int64_t>(passes, (int64_t)n_sm * 4));
     return IF_OK;
@@ -105,7 +105,7 @@ int setup_grids(Run& r) {
 
 template <int K, int MODE>
 int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
-    k_spmm<K, MODE><<<grid, BLOCK, TileSmem<K, MODE>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
+    k_spmm<K, MODE><<<grid, SPMM_BLOCK, TileSmem<K, MODE>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
     IF_LAUNCH_CHECK();
     return IF_OK;
 }
