@@ -181,6 +181,35 @@ struct SpmmArgs {
     int out_idx;         // CG1/CG2A: index of the direction buffer written (recorded in ctrl->cur_p)
 };
 
+// One row of the staged SpMM: all column ids and values of the row first, then all W gathers from the shared
+// tile, then the multiply-adds on two accumulators -- one shared-memory latency per phase instead of one per entry.
+template <int W, int TPR>
+__device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_row, const double* __restrict__ sval_row,
+                                              const double2* __restrict__ sa, int l) {
+    int2 cj[W / 2];
+    double2 vj[W / 2];
+#pragma unroll
+    for (int k = 0; k < W / 2; ++k) {
+        cj[k] = reinterpret_cast<const int2*>(scol_row)[k];
+        vj[k] = reinterpret_cast<const double2*>(sval_row)[k];
+    }
+    double2 g[W];
+#pragma unroll
+    for (int k = 0; k < W / 2; ++k) {
+        g[2 * k] = sa[cj[k].x * TPR + l];
+        g[2 * k + 1] = sa[cj[k].y * TPR + l];
+    }
+    double2 s0 = {0.0, 0.0}, s1 = {0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < W / 2; ++k) {
+        s0.x = fma(vj[k].x, g[2 * k].x, s0.x);     s0.y = fma(vj[k].x, g[2 * k].y, s0.y);
+        s1.x = fma(vj[k].y, g[2 * k + 1].x, s1.x); s1.y = fma(vj[k].y, g[2 * k + 1].y, s1.y);
+    }
+    s0.x += s1.x;
+    s0.y += s1.y;
+    return s0;
+}
+
 // dynamic shared memory of k_spmm: SPMM_STAGES stages of
 //   [gathered vector: T tile rows + HALO_CAP halo rows][second vector: T rows][val slice][col slice][S_vv][A_v | 1/A_v]
 // then a ring of four tile descriptors and one mbarrier per stage
@@ -408,15 +437,14 @@ __global__ void __launch_bounds__(SPMM_BLOCK, 1) k_spmm(MeshView m, Ctrl* __rest
             double2 s = {0.0, 0.0};
             if (staged) {
                 // every neighbour (tile or halo) is in shared memory under its tile-local index
-                double2 s1 = {0.0, 0.0};
-                for (int k = 0; k < w; k += 2) {
-                    const int2 cj = *reinterpret_cast<const int2*>(scol + o + k);
-                    const double2 vj = *reinterpret_cast<const double2*>(sval + o + k);
-                    const double2 g0 = sa[cj.x * TPR + l], g1 = sa[cj.y * TPR + l];
-                    s.x = fma(vj.x, g0.x, s.x);   s.y = fma(vj.x, g0.y, s.y);
-                    s1.x = fma(vj.y, g1.x, s1.x); s1.y = fma(vj.y, g1.y, s1.y);
+                // the width is the same for all rows of a SELL slice, hence warp-uniform: fully unrolled rows
+                switch (w) {
+                    case 2: s = gather_row<2, TPR>(scol + o, sval + o, sa, l); break;
+                    case 4: s = gather_row<4, TPR>(scol + o, sval + o, sa, l); break;
+                    case 6: s = gather_row<6, TPR>(scol + o, sval + o, sa, l); break;
+                    case 8: s = gather_row<8, TPR>(scol + o, sval + o, sa, l); break;
+                    default: break;   // w == 0 (staged tiles have w <= WCAP = 8, always even)
                 }
-                s.x += s1.x; s.y += s1.y;
             } else {
                 // fallback (wide rows or a halo beyond HALO_CAP): global column ids, out-of-tile rows from L2
                 for (int k = 0; k < w; k += 2) {
