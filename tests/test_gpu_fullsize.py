@@ -1,0 +1,101 @@
+"""Full-size checks on BASELINE.json config 4 in the launch configuration bench.py times (K = 16 columns, refill,
+default tolerance): sampled right-hand sides against the oracle where it finishes in seconds, and properties that
+hold at any size where it does not.  Needs a B200-class GPU (about 6 GB) and a few minutes."""
+import numpy as np
+import pytest
+
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD = 1e-7
+TOL_BIN = 1e-6
+
+
+@pytest.fixture(scope="module")
+def full():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    if torch.cuda.get_device_properties(0).total_memory < 16e9:
+        pytest.skip("needs 16 GB of device memory")
+    import paper_2404_07398_b200 as lib
+    lib.load_library()
+    w = make_config(4)
+    h = lib.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    yield lib, w, h
+    h.close()
+
+
+@pytest.fixture(scope="module")
+def oracle_mesh(full, oracle_mod):
+    _, w, _ = full
+    return oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+
+
+def rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def test_full_mesh_is_the_named_workload(full):
+    lib, w, h = full
+    assert w.mesh.n_vert == 7340033 and w.mesh.n_tri == 14664875      # 10 485 762 vertices minus the land mask
+    assert h.n_vert == w.mesh.n_vert and w.n_rhs == 80 and w.order_n == 1
+    assert abs(w.ells[-1] / w.mesh.h - 1000.0) < 1e-9 and abs(w.ells[0] / w.mesh.h - 1.0) < 1e-12
+    # the tiled SpMM stages (nearly) every tile in shared memory on the space-filling-curve order
+    assert h.n_tiles == (h.n_vert + 127) // 128 and h.unstaged_tiles <= 0.05 * h.n_tiles
+
+
+def test_spectrum_full_size_properties_and_sampled_energies(full, oracle_mesh):
+    """The bench step itself: all 80 right-hand sides.  e_l monotone, E >= 0, every solve converged; the energies of
+    sampled right-hand sides (those the oracle finishes in seconds) to 1e-6."""
+    lib, w, h = full
+    sp = lib.if_spectrum(h, w.fields, w.ells, 1)
+    st = sp["stats"]
+    assert st["code"] == 0 and np.all(st["status"] == 0) and np.all(st["rel_res"] <= 1e-12)
+    assert np.all(np.diff(sp["energy"], axis=1) < 0.0)                  # strictly decreasing in l
+    assert np.all(sp["E"] > 0.0)
+    k = 1.0 / w.ells
+    assert np.allclose(sp["k_mid"], np.sqrt(k[:-1] * k[1:]), rtol=1e-14)
+    for f in range(2):                                                   # telescoping sum of the bins
+        tele = np.sum(sp["E"][f] * (k[:-1] - k[1:]))
+        assert abs(tele - (sp["energy"][f, 0] - sp["energy"][f, -1])) <= 1e-12 * sp["energy"][f, 0]
+    for f, j in ((0, 0), (0, 8), (1, 4), (0, 16)):
+        x, info = oracle_mesh.solve(w.fields[f], float(w.ells[j]), 1)
+        assert info["status"] == 0
+        e = oracle_mesh.energy(x)
+        assert abs(sp["energy"][f, j] - e) <= TOL_BIN * e, (f, j)
+
+
+def test_filter_full_size_sampled_fields(full, oracle_mesh):
+    """16 right-hand sides (2 fields x the 8 smallest scales) in one K = 16 batch; three of them against the oracle."""
+    lib, w, h = full
+    ells = w.ells[:8]
+    out, st = lib.if_filter(h, w.fields, ells, 1)
+    assert st["code"] == 0
+    for f, j in ((0, 0), (1, 3), (0, 7)):
+        x, info = oracle_mesh.solve(w.fields[f], float(ells[j]), 1)
+        assert info["status"] == 0
+        assert rel(out[f, j].cpu().numpy(), x) <= TOL_FIELD, (f, j)
+
+
+def test_filter_full_size_largest_scales_properties(full, oracle_mesh):
+    """The longest solves (l up to 1000 h, ~1e4 iterations): true residual through if_apply, mean conservation,
+    energy identity phi^T M x = x^T A_l x >= x^T M x.  The oracle would need minutes per solve here."""
+    import torch
+    lib, w, h = full
+    ells = w.ells[-8:]
+    out, st = lib.if_filter(h, w.fields, ells, 1)
+    assert st["code"] == 0 and st["iters"].max() > 2000
+    area = torch.from_numpy(oracle_mesh.area()).to(out.device)
+    fields = torch.from_numpy(w.fields).to(out.device)
+    for f, j in ((0, 7), (1, 7), (0, 0)):
+        x = out[f, j]
+        b = area * fields[f]
+        ax = lib.if_apply(h, x[None, :], ells[j:j + 1], 1)[0, 0]
+        true_res = float(torch.linalg.norm(b - ax) / torch.linalg.norm(b))
+        assert true_res <= 1e-9, (f, j, true_res)                        # recursive 1e-12; true floors near u*kappa
+        mean_in, mean_out = float((area * fields[f]).sum()), float((area * x).sum())
+        assert abs(mean_out - mean_in) <= 1e-9 * float((area * fields[f].abs()).sum())
+        lhs, mid, low = float((b * x).sum()), float((x * ax).sum()), float((area * x * x).sum())
+        assert abs(lhs - mid) <= 1e-8 * abs(lhs) and mid >= low * (1 - 1e-12)
