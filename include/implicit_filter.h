@@ -114,6 +114,13 @@ int if_spectrum(if_handle h, const double* d_fields, int n_fields, const double*
                 double* energy, double* k_mid, double* E, void* d_workspace, size_t ws_bytes,
                 void* cuda_stream, const if_options* opt, if_stats* stats);
 
+/* if_spectrum for callers whose fields live in HOST memory (pinned memory makes the copy asynchronous): the fields
+ * are copied to the device inside the call, into the tail of the workspace, which must therefore hold
+ * if_workspace_bytes(...) + n_fields * n_vert * 8 bytes.  Everything else as if_spectrum. */
+int if_spectrum_host(if_handle h, const double* h_fields, int n_fields, const double* ells, int n_ells, int order_n,
+                     double* energy, double* k_mid, double* E, void* d_workspace, size_t ws_bytes,
+                     void* cuda_stream, const if_options* opt, if_stats* stats);
+
 /* Operator only: d_out[f][j] = (M + gamma l_j^(2n) S (M^-1 S)^(n-1)) d_fields[f].  Same layouts as if_filter. */
 int if_apply(if_handle h, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
              double* d_out, void* d_workspace, size_t ws_bytes, void* cuda_stream, const if_options* opt);

@@ -19,7 +19,7 @@ IF_OK, IF_WNOTCONVERGED = 0, 1
 IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKSPACE = -1, -2, -3, -4, -5, -6, -7
 IF_FLAG_KEEP_CSR = 1
 
-EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_apply", "if_mesh_info", "if_mesh_tile_info",
+EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_spectrum_host", "if_apply", "if_mesh_info", "if_mesh_tile_info",
            "if_mesh_export_csr", "if_mesh_export_perm", "if_destroy", "if_strerror", "if_launch_count")
 
 
@@ -65,6 +65,8 @@ def load_library():
     L.if_spectrum.restype = i32
     L.if_spectrum.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, vp, vp, C.c_size_t, vp, C.POINTER(if_options),
                               C.POINTER(if_stats)]
+    L.if_spectrum_host.restype = i32
+    L.if_spectrum_host.argtypes = L.if_spectrum.argtypes
     L.if_apply.restype = i32
     L.if_apply.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, C.c_size_t, vp, C.POINTER(if_options)]
     L.if_mesh_info.restype = i32
@@ -262,6 +264,36 @@ def if_spectrum(h: Handle, fields, ells: Sequence[float], order_n: int, workspac
     rc = _run(h, "if_spectrum", lambda s: L.if_spectrum(
         h._ptr, C.c_void_p(f.data_ptr()), Fn, _np_ptr(el), Ln, int(order_n), _np_ptr(energy), _np_ptr(k_mid),
         _np_ptr(E), C.c_void_p(ws.data_ptr()), ws.numel(), s, None if opt is None else C.byref(opt),
+        C.byref(st.c)), stream)
+    return {"energy": energy, "k_mid": k_mid, "E": E, "stats": st.as_dict(rc)}
+
+
+def if_spectrum_host(h: Handle, fields, ells: Sequence[float], order_n: int, workspace=None, stream=None, **options):
+    """if_spectrum with the fields in HOST memory (numpy array or CPU torch tensor, ideally pinned): the C call copies
+    them to the device itself.  Returns the same dict as if_spectrum."""
+    import torch
+    L = load_library()
+    t = fields if isinstance(fields, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(fields, dtype=np.float64))
+    if t.dim() == 1:
+        t = t[None, :]
+    if t.device.type != "cpu" or t.dtype != torch.float64 or not t.is_contiguous() or t.shape[1] != h.n_vert:
+        raise ValueError(f"fields must be a contiguous float64 HOST array [F][{h.n_vert}]")
+    el = np.ascontiguousarray(ells, dtype=np.float64)
+    Fn, Ln = t.shape[0], el.shape[0]
+    energy = np.zeros((Fn, Ln), dtype=np.float64)
+    k_mid = np.zeros(max(Ln - 1, 0), dtype=np.float64)
+    E = np.zeros((Fn, max(Ln - 1, 0)), dtype=np.float64)
+    opt = _options(**options)
+    need = if_workspace_bytes(h, order_n, options.get("batch") or 0) + Fn * h.n_vert * 8
+    if workspace is None:
+        if h._ws is None or h._ws.numel() < need:
+            h._ws = None
+            h._ws = torch.empty(need, dtype=torch.uint8, device=h.device)
+        workspace = h._ws
+    st = _Stats(Fn * Ln, (Fn, Ln))
+    rc = _run(h, "if_spectrum_host", lambda s: L.if_spectrum_host(
+        h._ptr, C.c_void_p(t.data_ptr()), Fn, _np_ptr(el), Ln, int(order_n), _np_ptr(energy), _np_ptr(k_mid),
+        _np_ptr(E), C.c_void_p(workspace.data_ptr()), workspace.numel(), s, None if opt is None else C.byref(opt),
         C.byref(st.c)), stream)
     return {"energy": energy, "k_mid": k_mid, "E": E, "stats": st.as_dict(rc)}
 

@@ -30,7 +30,8 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
+        extra = os.environ.get("IF_NVCC_EXTRA", "").split()      # e.g. -DIF_TILE_ROWS=64 (tuning experiments)
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
         subprocess.run(cmd, check=True)
     return LIB
 

@@ -14,8 +14,14 @@ namespace ifl {
 
 // Row tile of the fused SpMM kernel and the most out-of-tile rows ("halo") a tile may stage in shared memory.
 // if_prepare builds tile-local column ids and halo lists for exactly this tile height.
-constexpr int TILE_ROWS = 128;
-constexpr int HALO_CAP = 128;
+#ifndef IF_TILE_ROWS
+#define IF_TILE_ROWS 128
+#endif
+#ifndef IF_HALO_CAP
+#define IF_HALO_CAP 128
+#endif
+constexpr int TILE_ROWS = IF_TILE_ROWS;   // 64 or 128
+constexpr int HALO_CAP = IF_HALO_CAP;     // multiple of 32
 
 extern std::atomic<long long> g_launches;   // kernels launched by this library (if_launch_count)
 
@@ -43,7 +49,7 @@ struct Options {
     int check_every = 16;
     int batch = 16;
     int sell_c = 32;
-    int sell_sigma = 128;   // = TILE_ROWS: sorting inside a row tile keeps the tile spatially compact
+    int sell_sigma = TILE_ROWS;   // sorting inside a row tile keeps the tile spatially compact
     int sfc_kind = 0;
     int flags = 0;
 };

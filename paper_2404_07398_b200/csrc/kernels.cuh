@@ -213,8 +213,17 @@ __device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_r
 // dynamic shared memory of k_spmm: SPMM_STAGES stages of
 //   [gathered vector: T tile rows + HALO_CAP halo rows][second vector: T rows][val slice][col slice][S_vv][A_v | 1/A_v]
 // then a ring of four tile descriptors and one mbarrier per stage
-constexpr int SPMM_BLOCK = 512;
-constexpr int SPMM_STAGES = 3;
+#ifndef IF_SPMM_BLOCK
+#define IF_SPMM_BLOCK 512
+#endif
+#ifndef IF_SPMM_STAGES
+#define IF_SPMM_STAGES 3
+#endif
+#ifndef IF_SPMM_MINB
+#define IF_SPMM_MINB 1
+#endif
+constexpr int SPMM_BLOCK = IF_SPMM_BLOCK;
+constexpr int SPMM_STAGES = IF_SPMM_STAGES;
 template <int K, int MODE> struct TileSmem {
     static constexpr int T = TILE_ROWS;
     static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // vectors that arrive by bulk copy
@@ -247,7 +256,7 @@ __device__ __forceinline__ TileIssue load_issue(const int32_t* __restrict__ desc
 //   descriptors and halo row ids are fetched two tiles ahead.
 // About 130 KB of loads per SM are outstanding at all times, which is what the loaded HBM latency of B200 needs.
 template <int K, int MODE>
-__global__ void __launch_bounds__(SPMM_BLOCK, 1) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
+__global__ void __launch_bounds__(SPMM_BLOCK, IF_SPMM_MINB) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
                                                         double* __restrict__ partials, SpmmArgs a) {
     using SM = TileSmem<K, MODE>;
     constexpr int T = SM::T;
@@ -324,12 +333,50 @@ __global__ void __launch_bounds__(SPMM_BLOCK, 1) k_spmm(MeshView m, Ctrl* __rest
             if (e < nrows * TPR) xv[i] = ld2(a.x, row0 * K + 2 * (int64_t)e);
         }
     };
+    // stage views
+    auto stage_ptr = [&](int64_t it) { return smem + (size_t)(it % SPMM_STAGES) * SM::stage_bytes; };
+    // halo of a tile: registers -> shared memory behind the tile rows (p' = z + beta p for the CG passes)
+    auto halo_to_smem = [&](unsigned char* st, int nh, const double2 (&h0)[HPT], const double2 (&h1)[HPT]) {
+        double2* sa = reinterpret_cast<double2*>(st);
+#pragma unroll
+        for (int i = 0; i < HPT; ++i) {
+            const int hh = rg + i * ROWS;
+            if (hh < nh) {
+                double2 g = h0[i];
+                if (CG_A) { g.x = fma(beta.x, h1[i].x, g.x); g.y = fma(beta.y, h1[i].y, g.y); }
+                sa[(T + hh) * TPR + l] = g;
+            }
+        }
+    };
+    // p' = z + beta p in place over the z tile ; x += alpha_prev p (x comes from and goes to global memory)
+    auto elementwise = [&](unsigned char* st, int64_t tile, double2 (&xv)[XPT]) {
+        double2* sa = reinterpret_cast<double2*>(st);
+        const double2* sb = reinterpret_cast<const double2*>(st + SM::off_b);
+        const int64_t row0 = tile * T;
+        const int nrows = (int)min((int64_t)T, m.nv - row0);
+#pragma unroll
+        for (int i = 0; i < XPT; ++i) {
+            const int e = tid + i * NT;
+            if (e < nrows * TPR) {
+                const double2 zv = sa[e], pv = sb[e];
+                double2 own;
+                own.x = fma(beta.x, pv.x, zv.x);
+                own.y = fma(beta.y, pv.y, zv.y);
+                xv[i].x = fma(alpha.x, pv.x, xv[i].x);
+                xv[i].y = fma(alpha.y, pv.y, xv[i].y);
+                sa[e] = own;
+                st2(a.x, row0 * K + 2 * (int64_t)e, xv[i]);
+            }
+        }
+    };
+    auto is_staged = [&](const int32_t* d) { return d[3] >= 0 && d[2] <= T * WCAP; };
+
     if (tid == 0) {
         for (int s = 0; s < SPMM_STAGES; ++s) mbar_init(&bars[s], 1);
         fence_proxy_async();
     }
-    // prologue: descriptors of the first two tiles, their bulk copies, halo and x of the first tile
-    if (tid < 32) {
+    // ---- prologue: descriptors of tiles 0..2, bulk copies of tiles 0 and 1, tile 0 made ready for its gather
+    if (tid < 48) {
         const int64_t t = tile0 + (tid / 16) * G;
         sdesc[tid] = t < ntiles ? m.tile_desc[t * 16 + tid % 16] : 0;
     }
@@ -346,87 +393,55 @@ __global__ void __launch_bounds__(SPMM_BLOCK, 1) k_spmm(MeshView m, Ctrl* __rest
     double2 h0[HPT], h1[HPT], xv[XPT];
     int dnext = 0;
     if (tile0 < ntiles) {
-        int hid[HPT];
-        load_hidx(tile0, hid);
-        if (sdesc[3] >= 0 && sdesc[2] <= T * WCAP) load_halo(hid, sdesc[3], h0, h1);
+        load_hidx(tile0, hid_n);
+        if (is_staged(sdesc)) load_halo(hid_n, sdesc[3], h0, h1);
         if (CG_A) load_x(tile0, xv);
+        if (is_staged(sdesc)) halo_to_smem(smem, sdesc[3], h0, h1);
         load_hidx(tile0 + G, hid_n);
+        if (tile0 + G < ntiles && is_staged(sdesc + 16)) load_halo(hid_n, sdesc[16 + 3], h0, h1);
+        load_hidx(tile0 + 2 * G, hid_n);
+        if (tid < 16) dnext = tile0 + 3 * G < ntiles ? m.tile_desc[(tile0 + 3 * G) * 16 + tid] : 0;
+        mbar_wait(&bars[0], 0u);
+        if (CG_A) {
+            elementwise(smem, tile0, xv);
+            load_x(tile0 + G, xv);
+            fence_proxy_async();
+        }
     }
     double2 acc[1] = {{0.0, 0.0}};
     int64_t tile = tile0;
+    // ---- main loop.  Iteration `it` gathers tile it (made ready one iteration earlier) and then makes tile it+1
+    // ready; one block barrier per tile.
     for (int64_t it = 0; tile < ntiles; ++it, tile += G) {
-        const int stage = (int)(it % SPMM_STAGES);
-        const uint32_t parity = (uint32_t)(it / SPMM_STAGES) & 1u;
-        unsigned char* st = smem + (size_t)stage * SM::stage_bytes;
-        double2* sa = reinterpret_cast<double2*>(st);                    // gathered vector: tile + halo
-        double2* sb = reinterpret_cast<double2*>(st + SM::off_b);        // p_old, or own p' (CG2B)
+        unsigned char* st = stage_ptr(it);
+        const double2* sa = reinterpret_cast<const double2*>(st);          // gathered vector: tile + halo
+        const double2* sb = reinterpret_cast<const double2*>(st + SM::off_b);   // own p' (CG2B)
         const double* sval = reinterpret_cast<const double*>(st + SM::off_val);
         const int32_t* scol = reinterpret_cast<const int32_t*>(st + SM::off_col);
         const double* sdg = reinterpret_cast<const double*>(st + SM::off_dg);
         const double* sar = reinterpret_cast<const double*>(st + SM::off_ar);
         const int64_t row0 = tile * T;
         const int nrows = (int)min((int64_t)T, m.nv - row0);
-        const uint32_t vbytes = (uint32_t)nrows * K * sizeof(double);
-        __syncthreads();   // tile it-1 is fully consumed; the descriptor of tile it+1 is visible
+        __syncthreads();   // tile it is ready in its stage; tile it-1 is fully consumed
         const int32_t* d = sdesc + (it & 3) * 16;
         const int64_t cp_first = (int64_t)(uint32_t)d[0] | ((int64_t)d[1] << 32);
-        const int slots = d[2];
-        const int nh = d[3];
         const int32_t* scp = d + 4;
-        // staged tile: matrix slice and halo fit shared memory, columns are tile-local indices, no branches
-        const bool staged = nh >= 0 && slots <= T * WCAP;
+        const bool staged = is_staged(d);
         if (tid == 0) {
             const int64_t t2 = tile + 2 * G;
-            if (t2 < ntiles) {
-                bulk_wait_read0();   // the stage of tile it-1 is free once its bulk store has been read
-                issue(t2, (int)((it + 2) % SPMM_STAGES), tq);
+            bulk_wait_read0();   // the stage of tile it-1 is free once its bulk store has been read
+            if (t2 < ntiles) issue(t2, (int)((it + 2) % SPMM_STAGES), tq);
+            if (CG_A) {
+                bulk_store(a.out1 + row0 * K, sa, (uint32_t)nrows * K * sizeof(double));
+                bulk_commit();
             }
             if (t2 + G < ntiles) tq = load_issue(m.tile_desc, t2 + G);
         }
-        // halo of this tile: registers -> shared memory
-        if (staged) {
-#pragma unroll
-            for (int i = 0; i < HPT; ++i) {
-                const int hh = rg + i * ROWS;
-                if (hh < nh) {
-                    double2 g = h0[i];
-                    if (CG_A) { g.x = fma(beta.x, h1[i].x, g.x); g.y = fma(beta.y, h1[i].y, g.y); }
-                    sa[(T + hh) * TPR + l] = g;
-                }
-            }
+        if (tid < 16) {   // descriptor ring: tile it+3 in, tile it+4 on its way
+            sdesc[((it + 3) & 3) * 16 + tid] = dnext;
+            dnext = tile + 4 * G < ntiles ? m.tile_desc[(tile + 4 * G) * 16 + tid] : 0;
         }
-        // next tile: its halo rows into registers; two ahead: halo row ids and descriptor
-        {
-            const int32_t* d1 = sdesc + ((it + 1) & 3) * 16;
-            if (tile + G < ntiles && d1[3] >= 0 && d1[2] <= T * WCAP) load_halo(hid_n, d1[3], h0, h1);
-            load_hidx(tile + 2 * G, hid_n);
-            if (tid < 16) dnext = tile + 2 * G < ntiles ? m.tile_desc[(tile + 2 * G) * 16 + tid] : 0;
-        }
-        mbar_wait(&bars[stage], parity);
-        if (CG_A) {
-            // p' = z + beta p (in place over z, goes back with a bulk store) ; x += alpha_prev p
-#pragma unroll
-            for (int i = 0; i < XPT; ++i) {
-                const int e = tid + i * NT;
-                if (e < nrows * TPR) {
-                    const double2 zv = sa[e], pv = sb[e];
-                    double2 own;
-                    own.x = fma(beta.x, pv.x, zv.x);
-                    own.y = fma(beta.y, pv.y, zv.y);
-                    xv[i].x = fma(alpha.x, pv.x, xv[i].x);
-                    xv[i].y = fma(alpha.y, pv.y, xv[i].y);
-                    sa[e] = own;
-                    st2(a.x, row0 * K + 2 * (int64_t)e, xv[i]);
-                }
-            }
-            load_x(tile + G, xv);   // x of the next tile flies during the gather
-            fence_proxy_async();
-        }
-        __syncthreads();
-        if (CG_A && tid == 0) {
-            bulk_store(a.out1 + row0 * K, sa, vbytes);
-            bulk_commit();
-        }
+
         for (int r = rg; r < nrows; r += ROWS) {
             const int64_t row = row0 + r;
             const int chl = r >> m.log2c;
@@ -497,7 +512,21 @@ __global__ void __launch_bounds__(SPMM_BLOCK, 1) k_spmm(MeshView m, Ctrl* __rest
                 acc[0].y = fma(pv.y, q.y, acc[0].y);
             }
         }
-        if (tid < 16) sdesc[((it + 2) & 3) * 16 + tid] = dnext;
+        // ---- make tile it+1 ready: halo into its stage, wait for its bulk copies, form p', update x
+        if (tile + G < ntiles) {
+            unsigned char* st1 = stage_ptr(it + 1);
+            const int32_t* d1 = sdesc + ((it + 1) & 3) * 16;
+            const int32_t* d2 = sdesc + ((it + 2) & 3) * 16;
+            if (is_staged(d1)) halo_to_smem(st1, d1[3], h0, h1);
+            if (tile + 2 * G < ntiles && is_staged(d2)) load_halo(hid_n, d2[3], h0, h1);
+            load_hidx(tile + 3 * G, hid_n);
+            mbar_wait(&bars[(it + 1) % SPMM_STAGES], (uint32_t)((it + 1) / SPMM_STAGES) & 1u);
+            if (CG_A) {
+                elementwise(st1, tile + G, xv);
+                load_x(tile + 2 * G, xv);
+                fence_proxy_async();
+            }
+        }
     }
     if (CG_A && tid == 0) bulk_wait0();
     if (MODE == MODE_CG1 || MODE == MODE_CG2B) {

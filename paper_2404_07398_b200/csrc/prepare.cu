@@ -362,7 +362,7 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
     if (!(o.gamma > 0.0) || !std::isfinite(o.gamma) || !(o.tol > 0.0) || !std::isfinite(o.tol)) return IF_EINVAL;
     if (o.max_iter < 1 || o.check_every < 1) return IF_EINVAL;
     if (o.batch != 4 && o.batch != 8 && o.batch != 16) return IF_EINVAL;
-    if (o.sell_c != 32 && o.sell_c != 64 && o.sell_c != 128) return IF_EINVAL;   // must divide the SpMM row tile
+    if ((o.sell_c != 32 && o.sell_c != 64 && o.sell_c != 128) || TILE_ROWS % o.sell_c != 0) return IF_EINVAL;   // must divide the SpMM row tile
     if (o.sell_sigma < o.sell_c || o.sell_sigma % o.sell_c != 0) return IF_EINVAL;
     if (o.sfc_kind != 0 && o.sfc_kind != 1) return IF_EINVAL;
     o.check_every = (o.check_every + 1) & ~1;   // even: the search direction is double-buffered

@@ -528,6 +528,23 @@ extern "C" int if_spectrum(if_handle h, const double* d_fields, int n_fields, co
                    ws_bytes, cuda_stream, opt, stats);
 }
 
+extern "C" int if_spectrum_host(if_handle h, const double* h_fields, int n_fields, const double* ells, int n_ells,
+                                int order_n, double* energy, double* k_mid, double* E, void* d_workspace,
+                                size_t ws_bytes, void* cuda_stream, const if_options* opt, if_stats* stats) {
+    if (!h || !h_fields || n_fields < 1 || !d_workspace || (order_n != 1 && order_n != 2)) return IF_EINVAL;
+    Options o;
+    int rc = resolve_options(opt, &h->opt, &o);
+    if (rc != IF_OK) return rc;
+    const size_t base = layout_workspace(h, order_n, o.batch, nullptr).bytes;
+    const size_t fbytes = (size_t)n_fields * (size_t)h->n_vert * sizeof(double);
+    if (ws_bytes < base + fbytes) return IF_EWORKSPACE;
+    double* d_fields = reinterpret_cast<double*>(static_cast<char*>(d_workspace) + base);
+    IF_CUDA_TRY(cudaMemcpyAsync(d_fields, h_fields, fbytes, cudaMemcpyHostToDevice,
+                                static_cast<cudaStream_t>(cuda_stream)));
+    return run_job(h, JOB_SPECTRUM, d_fields, n_fields, ells, n_ells, order_n, nullptr, energy, k_mid, E, d_workspace,
+                   base, cuda_stream, opt, stats);
+}
+
 extern "C" int if_apply(if_handle h, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
                         double* d_out, void* d_workspace, size_t ws_bytes, void* cuda_stream, const if_options* opt) {
     return run_job(h, JOB_APPLY, d_fields, n_fields, ells, n_ells, order_n, d_out, nullptr, nullptr, nullptr,

@@ -216,3 +216,20 @@ def test_tolerance_and_paper_setting(ifl, oracle_mod):
         x, _ = om.solve(w.fields[0], ell, 1)
         assert rel(o9[0, j].cpu().numpy(), x) <= 1e-6
     h.close()
+
+
+def test_spectrum_from_host_buffers(ifl, oracle_mod):
+    """if_spectrum_host: fields in host memory, copied inside the C call; same numbers as the device-pointer call."""
+    import torch
+    w = make_config(4, level=5, n_ells=7)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    a = ifl.if_spectrum(h, w.fields, w.ells, 1)
+    pinned = torch.from_numpy(w.fields).pin_memory()
+    b = ifl.if_spectrum_host(h, pinned, w.ells, 1)
+    c = ifl.if_spectrum_host(h, w.fields, w.ells, 1)                     # pageable numpy memory works too
+    assert b["stats"]["code"] == 0 and np.array_equal(a["energy"], b["energy"]) and np.array_equal(a["E"], c["E"])
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_spectrum_host(h, pinned, w.ells, 1, workspace=torch.empty(ifl.if_workspace_bytes(h, 1), dtype=torch.uint8,
+                                                                         device="cuda"))
+    assert e.value.code == -7                                            # no room for the fields in the workspace
+    h.close()
