@@ -62,7 +62,7 @@ def workload_name(w, args):
             f"= {w.n_rhs} RHS, n={w.order_n}, l/h in [{w.ells[0] / w.mesh.h:.3g}, {w.ells[-1] / w.mesh.h:.4g}]")
 
 
-def build_workload(args, n_fields_total=None):
+def build_workload(args, field_offset=0):
     from workloads import make_config
     kw = {}
     if args.level is not None:
@@ -71,9 +71,7 @@ def build_workload(args, n_fields_total=None):
         kw["n"] = args.n
     if args.n_ells is not None:
         kw["n_ells"] = args.n_ells
-    if n_fields_total is not None:
-        kw["n_fields"] = n_fields_total
-    return make_config(args.config, **kw)
+    return make_config(args.config, field_offset=field_offset, **kw)
 
 
 # ----------------------------------------------------------------------------------------- clocks
@@ -205,11 +203,18 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    n_dev = torch.cuda.device_count()
+    local = local % n_dev
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    rdev = dev                       # where the few scalars that are reduced over ranks live
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+        if n_dev >= world:
+            dist.init_process_group("nccl", device_id=dev)
+        else:                        # more ranks than GPUs (a dry run of the N > 1 logic on a 1-GPU box): gloo
+            dist.init_process_group("gloo")
+            rdev = torch.device("cpu")
 
     from paper_2404_07398_b200 import build as libbuild
     if rank == 0:
@@ -221,11 +226,8 @@ def run_ours(args):
     lib.load_library()
 
     # every rank solves its own fields on its own replica of the mesh (weak scaling, no data-path collective)
-    w = build_workload(args)
-    base_fields = w.fields.shape[0]
-    if world > 1:
-        w = build_workload(args, n_fields_total=base_fields * world)
-        w.fields = w.fields[rank_fields(base_fields * world, world, rank)]
+    n_base = {1: 1, 2: 2, 3: 1, 4: 2, 5: 8}[args.config]
+    w = build_workload(args, field_offset=rank_fields(n_base * world, world, rank).start)
     V = w.mesh.n_vert
     R = w.n_rhs
     opts = {}
@@ -273,7 +275,7 @@ def run_ours(args):
         barrier()
         ms = e0.elapsed_time(e1)
         if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            t = torch.tensor([ms], dtype=torch.float64, device=rdev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
         return ms, res, lib.if_launch_count() - launches0
@@ -289,7 +291,7 @@ def run_ours(args):
     batch_iters = sum(s["batch_iters"] for s in stats)
     codes = sorted({s["code"] for s in stats})
     if world > 1:
-        t = torch.tensor([rhs_iters, batch_iters], dtype=torch.float64, device=dev)
+        t = torch.tensor([rhs_iters, batch_iters], dtype=torch.float64, device=rdev)
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         rhs_iters_all, batch_iters_all = float(t[0].item()), float(t[1].item())
     else:
@@ -301,7 +303,7 @@ def run_ours(args):
         ms_e, res_e, _ = timed(args.steps, True)
         it_e = sum(r["stats"]["rhs_iters"] for r in res_e)
         if world > 1:
-            t = torch.tensor([it_e], dtype=torch.float64, device=dev)
+            t = torch.tensor([it_e], dtype=torch.float64, device=rdev)
             dist.all_reduce(t, op=dist.ReduceOp.SUM)
             it_e = float(t.item())
         L = w.ells.shape[0]

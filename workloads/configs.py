@@ -33,19 +33,22 @@ class Workload:
         return int(self.fields.shape[0] * self.ells.shape[0])
 
 
-def _streams(config: int, n_fields: int):
+def _streams(config: int, n_fields: int, offset: int = 0):
     ss = np.random.SeedSequence(BASE_SEED + config)
-    kids = ss.spawn(2 + n_fields)
+    kids = ss.spawn(2 + offset + n_fields)
+    kids = kids[:2] + kids[2 + offset:]
     return [np.random.default_rng(k) for k in kids]
 
 
 def make_config(config: int, *, n: Optional[int] = None, level: Optional[int] = None,
                 n_fields: Optional[int] = None, n_ells: Optional[int] = None,
-                ell_max: Optional[float] = None) -> Workload:
+                ell_max: Optional[float] = None, field_offset: int = 0) -> Workload:
+    """`field_offset` skips that many field streams: fields [offset, offset + n_fields) of the same seeded sequence
+    (what rank r of a multi-GPU run generates for itself)."""
     if config == 1:
         n = 64 if n is None else n
         nf = 1 if n_fields is None else n_fields
-        rs = _streams(1, nf)
+        rs = _streams(1, nf, field_offset)
         mesh = M.grid_mesh(n, periodic=True, rng=rs[0])
         fl, wv = zip(*[F.planar_wave_field(mesh.coords, n, n // 2, min(128, 2 * n), rs[2 + i])
                        for i in range(nf)])
@@ -55,7 +58,7 @@ def make_config(config: int, *, n: Optional[int] = None, level: Optional[int] = 
     if config == 2:
         n = 512 if n is None else n
         nf = 2 if n_fields is None else n_fields
-        rs = _streams(2, nf)
+        rs = _streams(2, nf, field_offset)
         mesh = M.grid_mesh(n, periodic=True, jitter=0.3, random_diagonals=True, rng=rs[0])
         fl, wv = zip(*[F.planar_wave_field(mesh.coords, n, n // 2, 128, rs[2 + i]) for i in range(nf)])
         ells = F.log_spaced(1.0, float(n // 2) if ell_max is None else ell_max,
@@ -64,7 +67,7 @@ def make_config(config: int, *, n: Optional[int] = None, level: Optional[int] = 
     if config == 3:
         level = 9 if level is None else level
         nf = 1 if n_fields is None else n_fields
-        rs = _streams(3, nf)
+        rs = _streams(3, nf, field_offset)
         mesh = M.jitter_sphere(M.icosphere(level), 0.25, rs[0])
         kmax = max(4, int(round(400 * 2.0 ** (level - 9))))
         fl, wv = zip(*[F.sphere_wave_field(mesh.coords, kmax, 512, rs[2 + i]) for i in range(nf)])
@@ -80,7 +83,7 @@ def make_config(config: int, *, n: Optional[int] = None, level: Optional[int] = 
         base = M.icosphere(level)
         jit = M.jitter_sphere(base, 0.25, rs_mesh[0])
         mesh = M.land_mask(jit, base.coords, 0.30, rs_mesh[1])
-        rs = _streams(config, nf)
+        rs = _streams(config, nf, field_offset)
         kmax = max(4, int(round(800 * 2.0 ** (level - 10))))
         fl, wv = zip(*[F.sphere_wave_field(mesh.coords, kmax, 512, rs[2 + i]) for i in range(nf)])
         if config == 4:
