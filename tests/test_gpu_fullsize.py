@@ -99,3 +99,73 @@ def test_filter_full_size_largest_scales_properties(full, oracle_mesh):
         assert abs(mean_out - mean_in) <= 1e-9 * float((area * fields[f].abs()).sum())
         lhs, mid, low = float((b * x).sum()), float((x * ax).sum()), float((area * x * x).sum())
         assert abs(lhs - mid) <= 1e-8 * abs(lhs) and mid >= low * (1 - 1e-12)
+
+
+# ------------------------------------------------------------------------------------------ the other full-size configs
+def test_config2_full_size_sampled(oracle_mod):
+    """Config 2 at full size (512 x 512 jittered periodic grid with slivers, 2 fields x 20 scales): all 40 solves
+    on the GPU, a sample of them (including the largest scale of each field) against the oracle."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2404_07398_b200 as lib
+    w = make_config(2)
+    assert w.mesh.n_vert == 262144 and w.n_rhs == 40
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    h = lib.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    assert h.unstaged_tiles == 0                      # 2-D Morton order: every tile staged in shared memory
+    out, st = lib.if_filter(h, w.fields, w.ells, 1)
+    sp = lib.if_spectrum(h, w.fields, w.ells, 1)
+    assert st["code"] == 0 and sp["stats"]["code"] == 0
+    assert np.all(np.diff(sp["energy"], axis=1) < 0.0)
+    for f, j in ((0, 0), (1, 6), (0, 12), (0, 19), (1, 19)):
+        x, info = om.solve(w.fields[f], float(w.ells[j]), 1)
+        assert info["status"] == 0
+        assert rel(out[f, j].cpu().numpy(), x) <= TOL_FIELD, (f, j)
+        e = om.energy(x)
+        assert abs(sp["energy"][f, j] - e) <= TOL_BIN * e, (f, j)
+    h.close()
+
+
+def test_config3_full_size_biharmonic_sampled(oracle_mod):
+    """Config 3 at full size (icosphere level 9, n = 2): the smallest scales against the oracle (the oracle needs
+    minutes to hours beyond l ~ 4 h), a mid scale through its true residual and the energy identity."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2404_07398_b200 as lib
+    w = make_config(3)
+    assert w.mesh.n_vert == 2621442 and w.order_n == 2 and w.n_rhs == 20
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    h = lib.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    ells = w.ells[:12]                                # 1 ... 7.4 h: up to ~5e3 iterations
+    out, st = lib.if_filter(h, w.fields, ells, 2)
+    assert st["code"] == 0
+    for j in (0, 3, 5):
+        x, info = om.solve(w.fields[0], float(ells[j]), 2)
+        assert info["status"] == 0
+        assert rel(out[0, j].cpu().numpy(), x) <= TOL_FIELD, j
+    area = torch.from_numpy(om.area()).to(out.device)
+    phi = torch.from_numpy(w.fields[0]).to(out.device)
+    j = 11
+    x = out[0, j]
+    ax = lib.if_apply(h, x[None, :], ells[j:j + 1], 2)[0, 0]
+    b = area * phi
+    assert float(torch.linalg.norm(b - ax) / torch.linalg.norm(b)) <= 1e-8
+    assert abs(float((area * x).sum()) - float(b.sum())) <= 1e-9 * float(b.abs().sum())
+    h.close()
+
+
+def test_config5_full_size_biharmonic_batches(full, oracle_mesh, oracle_mod):
+    """Config 5 = config 4's mesh (one if_prepare), 8 fields, n = 2, batches of 16: 8 fields x the 4 smallest scales
+    = 32 right-hand sides through the refill path; two of them against the oracle."""
+    lib, w4, h = full
+    w = make_config(5)
+    assert w.fields.shape[0] == 8 and w.order_n == 2 and np.array_equal(w.mesh.tri, w4.mesh.tri)
+    ells = w.ells[:4]
+    out, st = lib.if_filter(h, w.fields, ells, 2)
+    assert st["code"] == 0 and st["iters"].shape == (8, 4)
+    for f, j in ((0, 0), (7, 3)):
+        x, info = oracle_mesh.solve(w.fields[f], float(ells[j]), 2)
+        assert info["status"] == 0
+        assert rel(out[f, j].cpu().numpy(), x) <= TOL_FIELD, (f, j)
