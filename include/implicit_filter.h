@@ -53,11 +53,14 @@ enum {
     IF_EORPHAN = -4,      /* vertex in no triangle: A_v = 0, M singular                                    */
     IF_ENOMEM = -5,       /* host or device allocation failed                                              */
     IF_ECUDA = -6,        /* CUDA runtime error, or no device                                              */
-    IF_EWORKSPACE = -7    /* workspace smaller than if_workspace_bytes says                                */
+    IF_EWORKSPACE = -7,   /* workspace smaller than if_workspace_bytes says                                */
+    IF_EIO = -8           /* if_save / if_load: file cannot be written / read, or is not a prepared mesh   */
 };
 
 enum {
-    IF_FLAG_KEEP_CSR = 1 /* if_prepare keeps the unpermuted CSR of S so if_mesh_export_csr works */
+    IF_FLAG_KEEP_CSR = 1, /* if_prepare keeps the unpermuted CSR of S so if_mesh_export_csr works */
+    IF_FLAG_HIGHPASS = 2  /* if_filter (per call): write the high-pass field phi - phibar_l (PAPER.md:143-147,
+                             Fig. 3) instead of phibar_l                                                    */
 };
 
 typedef struct {
@@ -142,6 +145,13 @@ int if_mesh_export_csr(if_handle h, int64_t* rowptr, int32_t* col, double* val, 
 
 /* Internal ordering (HOST [n_vert], may be NULL): perm[new] = caller id of internal row `new`. */
 int if_mesh_export_perm(if_handle h, int32_t* perm);
+
+/* The prepared mesh is independent of the scales and can be kept on disk and reused.
+ * if_save writes every device array of the handle to `path` (HOST string); if_load rebuilds a handle on the current
+ * CUDA device from such a file (same library build: the row-tile constants are checked).  The optional CSR copy of
+ * IF_FLAG_KEEP_CSR is not saved.  IF_EIO on any file problem. */
+int if_save(if_handle h, const char* path);
+int if_load(const char* path, if_handle* out);
 
 void if_destroy(if_handle h);
 const char* if_strerror(int code);

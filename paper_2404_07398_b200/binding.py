@@ -16,11 +16,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libimplicit_filter.so")
 
 IF_OK, IF_WNOTCONVERGED = 0, 1
-IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKSPACE = -1, -2, -3, -4, -5, -6, -7
+IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKSPACE, IF_EIO = -1, -2, -3, -4, -5, -6, -7, -8
 IF_FLAG_KEEP_CSR = 1
+IF_FLAG_HIGHPASS = 2
 
 EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_spectrum_host", "if_apply", "if_mesh_info", "if_mesh_tile_info",
-           "if_mesh_export_csr", "if_mesh_export_perm", "if_destroy", "if_strerror", "if_launch_count")
+           "if_mesh_export_csr", "if_mesh_export_perm", "if_save", "if_load", "if_destroy", "if_strerror", "if_launch_count")
 
 
 class if_options(C.Structure):
@@ -77,6 +78,10 @@ def load_library():
     L.if_mesh_export_csr.argtypes = [vp, vp, vp, vp, vp]
     L.if_mesh_export_perm.restype = i32
     L.if_mesh_export_perm.argtypes = [vp, vp]
+    L.if_save.restype = i32
+    L.if_save.argtypes = [vp, C.c_char_p]
+    L.if_load.restype = i32
+    L.if_load.argtypes = [C.c_char_p, C.POINTER(vp)]
     L.if_destroy.restype = None
     L.if_destroy.argtypes = [vp]
     L.if_strerror.restype = C.c_char_p
@@ -334,6 +339,27 @@ def if_mesh_export_perm(h: Handle) -> np.ndarray:
     if rc != IF_OK:
         raise ImplicitFilterError(rc, "if_mesh_export_perm")
     return perm
+
+
+def if_save(h: Handle, path: str) -> None:
+    """Write the prepared mesh to `path` (the auxiliary arrays are reusable)."""
+    rc = load_library().if_save(h._ptr, os.fsencode(path))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_save")
+
+
+def if_load(path: str) -> Handle:
+    """A handle on the current CUDA device from a file written by if_save."""
+    import torch
+    if not torch.cuda.is_available():
+        raise ImplicitFilterError(IF_ECUDA, "if_load (no CUDA device; there is no CPU fallback)")
+    device = torch.device("cuda", torch.cuda.current_device())
+    torch.zeros(1, device=device)
+    out = C.c_void_p()
+    rc = load_library().if_load(os.fsencode(path), C.byref(out))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_load")
+    return Handle(out.value, device)
 
 
 def if_destroy(h: Handle) -> None:

@@ -736,10 +736,12 @@ __global__ void __launch_bounds__(BLOCK) k_energy(MeshView m, Ctrl* __restrict__
 }
 
 // H6a for the columns in `mask`: x_final scattered back to the caller's numbering: out[rhs][perm[row]]
+// (or the high-pass field phi - x_final)
 template <int K>
 __global__ void __launch_bounds__(BLOCK) k_scatter(MeshView m, const Ctrl* __restrict__ ctrl, unsigned mask,
                                                    const double* __restrict__ x, const double* __restrict__ pa,
-                                                   const double* __restrict__ pb, int use_p, double* __restrict__ out) {
+                                                   const double* __restrict__ pb, int use_p, double* __restrict__ out,
+                                                   const double* __restrict__ fields, int highpass) {
     __shared__ double tile[K][33];
     __shared__ int32_t dst[32];
     const int tid = threadIdx.x;
@@ -760,8 +762,11 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(MeshView m, const Ctrl* __res
         __syncthreads();
         for (int e = tid; e < 32 * K; e += BLOCK) {
             const int c = e / 32, r = e % 32;
-            if (((mask >> c) & 1u) && ctrl->field[c] >= 0 && dst[r] >= 0)
-                out[(int64_t)ctrl->rhs[c] * m.nv + dst[r]] = tile[c][r];
+            if (((mask >> c) & 1u) && ctrl->field[c] >= 0 && dst[r] >= 0) {
+                double v = tile[c][r];
+                if (highpass) v = fields[(int64_t)ctrl->field[c] * m.nv + dst[r]] - v;   // phi - phibar
+                out[(int64_t)ctrl->rhs[c] * m.nv + dst[r]] = v;
+            }
         }
         __syncthreads();
     }

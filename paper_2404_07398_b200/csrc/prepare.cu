@@ -13,6 +13,8 @@
 #include <cub/cub.cuh>
 
 #include <cmath>
+#include <cstdio>
+#include <cstring>
 #include <new>
 #include <vector>
 
@@ -357,6 +359,8 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
             if (in->sell_sigma != 0) o.sell_sigma = in->sell_sigma;
             o.sfc_kind = in->sfc_kind;
             o.flags = in->flags;
+        } else {   // per-call flags
+            o.flags = (o.flags & ~IF_FLAG_HIGHPASS) | (in->flags & IF_FLAG_HIGHPASS);
         }
     }
     if (!(o.gamma > 0.0) || !std::isfinite(o.gamma) || !(o.tol > 0.0) || !std::isfinite(o.tol)) return IF_EINVAL;
@@ -702,6 +706,116 @@ extern "C" int if_mesh_export_perm(if_handle h, int32_t* perm) {
     return IF_OK;
 }
 
+// ------------------------------------------------------------------------------------------- save / load
+namespace {
+struct FileHeader {
+    char magic[8];            // "IFMESH01"
+    int32_t tile_rows, halo_cap, sell_c, pad_;
+    int64_t n_vert, nnz, n_chunks, sell_slots, n_tiles, halo_total, halo_max, unstaged_tiles;
+    double total_area, mean_edge;
+    ifl::Options opt;
+};
+
+int write_dev(FILE* f, const void* d, size_t bytes, std::vector<char>& buf) {
+    buf.resize(bytes);
+    if (bytes) IF_CUDA_TRY(cudaMemcpy(buf.data(), d, bytes, cudaMemcpyDeviceToHost));
+    return fwrite(buf.data(), 1, bytes, f) == bytes ? IF_OK : IF_EIO;
+}
+int read_dev(FILE* f, void** d, size_t bytes, size_t alloc_bytes, std::vector<char>& buf) {
+    buf.resize(bytes);
+    if (fread(buf.data(), 1, bytes, f) != bytes) return IF_EIO;
+    IF_CUDA_TRY(cudaMalloc(d, alloc_bytes ? alloc_bytes : 1));
+    IF_CUDA_TRY(cudaMemset(*d, 0, alloc_bytes ? alloc_bytes : 1));
+    if (bytes) IF_CUDA_TRY(cudaMemcpy(*d, buf.data(), bytes, cudaMemcpyHostToDevice));
+    return IF_OK;
+}
+}  // namespace
+
+extern "C" int if_save(if_handle h, const char* path) {
+    if (!h || !path) return IF_EINVAL;
+    IF_CUDA_TRY(cudaSetDevice(h->device));
+    FILE* f = fopen(path, "wb");
+    if (!f) return IF_EIO;
+    FileHeader hd;
+    memset(&hd, 0, sizeof(hd));
+    memcpy(hd.magic, "IFMESH01", 8);
+    hd.tile_rows = TILE_ROWS; hd.halo_cap = HALO_CAP; hd.sell_c = h->sell_c;
+    hd.n_vert = h->n_vert; hd.nnz = h->nnz; hd.n_chunks = h->n_chunks; hd.sell_slots = h->sell_slots;
+    hd.n_tiles = h->n_tiles; hd.halo_total = h->halo_total; hd.halo_max = h->halo_max;
+    hd.unstaged_tiles = h->unstaged_tiles; hd.total_area = h->total_area; hd.mean_edge = h->mean_edge;
+    hd.opt = h->opt;
+    hd.opt.flags &= ~(IF_FLAG_KEEP_CSR | IF_FLAG_HIGHPASS);
+    std::vector<char> buf;
+    const size_t nv = (size_t)h->n_vert, ns = (size_t)h->sell_slots, nt = (size_t)h->n_tiles;
+    int rc = fwrite(&hd, sizeof(hd), 1, f) == 1 ? IF_OK : IF_EIO;
+    if (rc == IF_OK) rc = write_dev(f, h->chunk_ptr, (size_t)(h->n_chunks + 1) * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->sell_col, ns * 4, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->sell_val, ns * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->sell_lcol, ns * 4, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->area, nv * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->inv_area, nv * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->sdiag, nv * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->gdiag, nv * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->perm, nv * 4, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->iperm, nv * 4, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->halo_n, nt * 4, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->halo_rows, nt * HALO_CAP * 4, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->tile_desc, (nt + 1) * 64, buf);
+    if (fclose(f) != 0 && rc == IF_OK) rc = IF_EIO;
+    return rc;
+}
+
+extern "C" int if_load(const char* path, if_handle* out) {
+    if (!path || !out) return IF_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return IF_ECUDA; }
+    FILE* f = fopen(path, "rb");
+    if (!f) return IF_EIO;
+    FileHeader hd;
+    if (fread(&hd, sizeof(hd), 1, f) != 1 || memcmp(hd.magic, "IFMESH01", 8) != 0 || hd.tile_rows != TILE_ROWS ||
+        hd.halo_cap != HALO_CAP || hd.n_vert < 3 || hd.sell_slots < 0 || hd.n_tiles != (hd.n_vert + TILE_ROWS - 1) / TILE_ROWS) {
+        fclose(f);
+        return IF_EIO;
+    }
+    if_mesh_s* h = new (std::nothrow) if_mesh_s();
+    if (!h) { fclose(f); return IF_ENOMEM; }
+    auto fail = [&](int rc) { fclose(f); if_destroy(h); return rc; };
+    if (cudaGetDevice(&h->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess)
+        return fail(IF_ECUDA);
+    h->n_vert = hd.n_vert; h->nnz = hd.nnz; h->n_chunks = hd.n_chunks; h->sell_slots = hd.sell_slots;
+    h->n_tiles = hd.n_tiles; h->halo_total = hd.halo_total; h->halo_max = hd.halo_max;
+    h->unstaged_tiles = hd.unstaged_tiles; h->total_area = hd.total_area; h->mean_edge = hd.mean_edge;
+    h->opt = hd.opt; h->sell_c = hd.sell_c;
+    std::vector<char> buf;
+    const size_t nv = (size_t)h->n_vert, ns = (size_t)h->sell_slots, nt = (size_t)h->n_tiles;
+    int rc;
+    if ((rc = read_dev(f, (void**)&h->chunk_ptr, (size_t)(h->n_chunks + 1) * 8, (size_t)(h->n_chunks + 1) * 8, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->sell_col, ns * 4, ns * 4 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->sell_val, ns * 8, ns * 8 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->sell_lcol, ns * 4, ns * 4 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->area, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->inv_area, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->sdiag, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->gdiag, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->perm, nv * 4, nv * 4, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->iperm, nv * 4, nv * 4, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->halo_n, nt * 4, nt * 4, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->halo_rows, nt * HALO_CAP * 4, nt * HALO_CAP * 4, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->tile_desc, (nt + 1) * 64, (nt + 1) * 64, buf))) return fail(rc);
+    char extra;
+    if (fread(&extra, 1, 1, f) != 0) return fail(IF_EIO);   // trailing bytes: not a file of ours
+    fclose(f);
+    h->h_pinned_bytes = 1 << 20;
+    if (cudaHostAlloc(&h->h_pinned, h->h_pinned_bytes, cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError();
+        if_destroy(h);
+        return IF_ENOMEM;
+    }
+    *out = h;
+    return IF_OK;
+}
+
 extern "C" const char* if_strerror(int code) {
     switch (code) {
         case IF_OK: return "ok";
@@ -713,6 +827,7 @@ extern "C" const char* if_strerror(int code) {
         case IF_ENOMEM: return "out of memory";
         case IF_ECUDA: return "CUDA error or no device";
         case IF_EWORKSPACE: return "workspace too small";
+        case IF_EIO: return "file cannot be written or read, or is not a prepared mesh of this library build";
         default: return "unknown error";
     }
 }

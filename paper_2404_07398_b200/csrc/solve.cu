@@ -203,7 +203,7 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
 
 // The columns in `mask` have stopped: energy or scatter of x, and the per-right-hand-side results.
 template <int K>
-int finalize_columns(const Run& r, Job job, unsigned mask, double* d_out) {
+int finalize_columns(const Run& r, Job job, unsigned mask, double* d_out, const double* d_fields) {
     const if_mesh_s* h = r.h;
     if (job == JOB_SPECTRUM) {
         k_energy<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, mask, r.w.x, r.w.p0, r.w.p1,
@@ -211,7 +211,8 @@ int finalize_columns(const Run& r, Job job, unsigned mask, double* d_out) {
         IF_LAUNCH_CHECK();
     } else {
         const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
-        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, mask, r.w.x, r.w.p0, r.w.p1, 1, d_out);
+        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, mask, r.w.x, r.w.p0, r.w.p1, 1, d_out, d_fields,
+                                                (r.opt.flags & IF_FLAG_HIGHPASS) ? 1 : 0);
         IF_LAUNCH_CHECK();
     }
     k_stats<<<1, 32, 0, r.st>>>(r.w.ctrl, K, mask, r.w.iters, r.w.status, r.w.relres);
@@ -261,7 +262,7 @@ int apply_all(Run& r, const double* d_fields, const std::vector<Rhs>& rhs, int n
         SpmmArgs b{v, r.w.x, nullptr, r.w.q, nullptr, 0, 0};
         if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
         const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
-        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, (1u << K) - 1u, r.w.q, r.w.p0, r.w.p1, 0, d_out);
+        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, (1u << K) - 1u, r.w.q, r.w.p0, r.w.p1, 0, d_out, nullptr, 0);
         IF_LAUNCH_CHECK();
     }
     return IF_OK;
@@ -368,7 +369,7 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
         }
         if (fin) {
             // these columns stopped before launch it-1 ended and stayed frozen through launch it
-            if ((rc = finalize_columns<K>(r, job, fin, d_out))) return rc;
+            if ((rc = finalize_columns<K>(r, job, fin, d_out, d_fields))) return rc;
             for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) --active;
             if (next < R) {
                 assign(fin, &sp, &started);

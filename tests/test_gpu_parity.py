@@ -233,3 +233,44 @@ def test_spectrum_from_host_buffers(ifl, oracle_mod):
                                                                          device="cuda"))
     assert e.value.code == -7                                            # no room for the fields in the workspace
     h.close()
+
+
+def test_highpass_output(ifl, oracle_mod):
+    """IF_FLAG_HIGHPASS: if_filter returns phi - phibar_l (Fig. 3)."""
+    w = make_config(4, level=5, n_ells=5)
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    hp, st = ifl.if_filter(h, w.fields, w.ells, 1, flags=ifl.IF_FLAG_HIGHPASS)
+    lp, _ = ifl.if_filter(h, w.fields, w.ells, 1)                      # the flag is per call
+    hp, lp = hp.cpu().numpy(), lp.cpu().numpy()
+    assert st["code"] == 0
+    for f in range(2):
+        for j, ell in enumerate(w.ells):
+            x, _ = om.solve(w.fields[f], ell, 1)
+            assert rel(hp[f, j], w.fields[f] - x) <= TOL_FIELD
+            assert rel(lp[f, j], x) <= TOL_FIELD
+    h.close()
+
+
+def test_save_and_load_prepared_mesh(ifl, tmp_path):
+    """The prepared mesh is scale-independent and reusable from disk: bit-identical results."""
+    w = make_config(3, level=4, n_ells=4, ell_max=4.0)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    a, _ = ifl.if_filter(h, w.fields, w.ells, 2)
+    path = str(tmp_path / "mesh.ifm")
+    ifl.if_save(h, path)
+    h.close()
+    g = ifl.if_load(path)
+    assert (g.n_vert, g.n_tiles) == (w.mesh.n_vert, (w.mesh.n_vert + 127) // 128)
+    b, st = ifl.if_filter(g, w.fields, w.ells, 2)
+    assert st["code"] == 0 and bool((a == b).all())
+    assert np.array_equal(np.sort(ifl.if_mesh_export_perm(g)), np.arange(w.mesh.n_vert))
+    g.close()
+    with open(path, "r+b") as fh:
+        fh.write(b"garbage!")
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_load(path)
+    assert e.value.code == -8
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_load(str(tmp_path / "missing.ifm"))
+    assert e.value.code == -8
