@@ -796,5 +796,42 @@ __global__ void k_spectrum(const double* __restrict__ energy, const double* __re
     if (f == 0) k_mid[j] = sqrt(k0 * k1);
 }
 
+// ------------------------------------------------------------------------------------------- column compaction (H5)
+// When the queue is empty and at most half of the columns are still running, the survivors move to a narrower
+// layout ([row][KN] instead of [row][KW]) so that finished columns stop costing bandwidth.
+struct ColMap { int src[KMAX]; };   // new column j <- old column src[j]; -1 = empty
+
+template <int KW, int KN>
+__global__ void __launch_bounds__(BLOCK) k_repack(int64_t nv, ColMap map, const double* __restrict__ src,
+                                                  double* __restrict__ dst) {
+    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
+    if (i >= nv * KN) return;
+    const int64_t row = i / KN;
+    const int s = map.src[i % KN];
+    dst[i] = s >= 0 ? src[row * KW + s] : 0.0;
+}
+
+__global__ void k_compact_ctrl(Ctrl* __restrict__ ctrl, ColMap map, int KN) {
+    const int j = threadIdx.x;   // one block of KMAX threads
+    const int s = j < KN ? map.src[j] : -1;
+    double c = 0.0, al = 0.0, be = 0.0, rho = 0.0, bb = 0.0, rr = 0.0;
+    int field = -1, rhs = 0, done = 1, epoch = 0, status = 0, iters = 0;
+    if (s >= 0) {
+        c = ctrl->c[s]; al = ctrl->alpha[s]; be = ctrl->beta[s]; rho = ctrl->rho[s]; bb = ctrl->bb[s]; rr = ctrl->rr[s];
+        field = ctrl->field[s]; rhs = ctrl->rhs[s]; done = ctrl->done[s]; epoch = ctrl->epoch[s];
+        status = ctrl->status[s]; iters = ctrl->iters[s];
+    }
+    __syncthreads();
+    ctrl->c[j] = c; ctrl->alpha[j] = al; ctrl->beta[j] = be; ctrl->rho[j] = rho; ctrl->bb[j] = bb; ctrl->rr[j] = rr;
+    ctrl->field[j] = field; ctrl->rhs[j] = rhs; ctrl->done[j] = done; ctrl->epoch[j] = epoch;
+    ctrl->status[j] = status; ctrl->iters[j] = iters;
+    __syncthreads();
+    if (j == 0) {
+        int any = 0;
+        for (int k = 0; k < KMAX; ++k) any |= !ctrl->done[k];
+        ctrl->all_done = !any;
+    }
+}
+
 }  // namespace
 }  // namespace ifl

@@ -268,44 +268,54 @@ int apply_all(Run& r, const double* d_fields, const std::vector<Rhs>& rhs, int n
     return IF_OK;
 }
 
-// if_filter / if_spectrum: all right-hand sides through K columns with refill.
+// Host view of the K columns: which right-hand side each one runs, and the epoch the device should report for it.
+struct QueueState {
+    int col_rhs[KMAX];
+    int host_epoch[KMAX];
+    size_t next = 0;     // next right-hand side of the queue
+    int active = 0;      // columns running a right-hand side
+};
+
+// if_filter / if_spectrum: right-hand sides through K columns with refill.  With `first` the columns are started
+// from the queue; otherwise the state comes from a wider phase (compact_columns).  Returns when every column has
+// stopped, or -- if *compact_to is given -- when the queue is empty and at most K/2 columns are still running
+// (*compact_to = 4 or 8: the survivors should move to that many columns).
 template <int K>
-int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
-              PollState& poll, KernelTimes* times, int64_t* batch_iters) {
+int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
+                PollState& poll, KernelTimes* times, QueueState& q, bool first, int* compact_to) {
     int rc;
     if ((rc = setup_grids<K>(r))) return rc;
     const size_t R = rhs.size();
-    Ctrl hc = fresh_ctrl(r);
-    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
-
-    int col_rhs[KMAX], host_epoch[KMAX];
-    size_t next = 0;
-    int active = 0;
+    if (compact_to) *compact_to = 0;
     auto assign = [&](unsigned mask, StartParams* sp, unsigned* started) {
         memset(sp, 0, sizeof(*sp));
         for (int c = 0; c < KMAX; ++c) sp->field[c] = -1;
         *started = 0;
         for (int c = 0; c < K; ++c) {
             if (!((mask >> c) & 1u)) continue;
-            if (next < R) {
-                const Rhs& q = rhs[next];
-                sp->c[c] = r.opt.gamma * std::pow(q.ell, 2.0 * r.order_n);
-                sp->field[c] = q.f;
-                sp->rhs[c] = q.f * n_ells + q.j;
-                col_rhs[c] = (int)next++;
-                ++active;
+            if (q.next < R) {
+                const Rhs& s = rhs[q.next];
+                sp->c[c] = r.opt.gamma * std::pow(s.ell, 2.0 * r.order_n);
+                sp->field[c] = s.f;
+                sp->rhs[c] = s.f * n_ells + s.j;
+                q.col_rhs[c] = (int)q.next++;
+                ++q.active;
             } else {
-                col_rhs[c] = -1;
+                q.col_rhs[c] = -1;
             }
             *started |= 1u << c;
-            host_epoch[c] += 1;
+            q.host_epoch[c] += 1;
         }
     };
-    for (int c = 0; c < KMAX; ++c) { col_rhs[c] = -1; host_epoch[c] = 0; }
     StartParams sp;
     unsigned started = 0;
-    assign((1u << K) - 1u, &sp, &started);          // empty columns are started too (zeroed, done at once)
-    if ((rc = start_columns<K>(r, started, sp, d_fields))) return rc;
+    if (first) {
+        Ctrl hc = fresh_ctrl(r);
+        IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
+        for (int c = 0; c < KMAX; ++c) { q.col_rhs[c] = -1; q.host_epoch[c] = 0; }
+        assign((1u << K) - 1u, &sp, &started);          // empty columns are started too (zeroed, done at once)
+        if ((rc = start_columns<K>(r, started, sp, d_fields))) return rc;
+    }
 
     // the iteration loop: `check_every` iterations per CUDA graph launch, snapshot polled one launch behind
     const int pairs = r.opt.check_every / 2;
@@ -334,7 +344,7 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
     const bool use_graph = gs.exec[0] && gs.exec[1];
     const int64_t per_rhs = (r.opt.max_iter + r.opt.check_every - 1) / r.opt.check_every + 3;
     const int64_t max_loops = ((int64_t)(R + K - 1) / K + 1) * per_rhs + 8;
-    for (int64_t it = 0; it < max_loops && active > 0; ++it) {
+    for (int64_t it = 0; it < max_loops && q.active > 0; ++it) {
         if (use_graph) {
             IF_CUDA_TRY(cudaGraphLaunch(gs.exec[it & 1], r.st));
             g_launches += (long long)launches_per_graph;
@@ -353,10 +363,10 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
         unsigned fin = 0;
         bool any_running = false;
         for (int c = 0; c < K; ++c) {
-            if (col_rhs[c] < 0 || s.epoch[c] != host_epoch[c]) continue;
+            if (q.col_rhs[c] < 0 || s.epoch[c] != q.host_epoch[c]) continue;
             if (s.done[c]) fin |= 1u << c; else any_running = true;
         }
-        if (use_graph && any_running) {
+        if (times && use_graph && any_running) {
             // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
             const TimingEvents& te = gs.tev[(it - 1) & 1];
             float a = 0.f, b = 0.f;
@@ -370,16 +380,93 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
         if (fin) {
             // these columns stopped before launch it-1 ended and stayed frozen through launch it
             if ((rc = finalize_columns<K>(r, job, fin, d_out, d_fields))) return rc;
-            for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) --active;
-            if (next < R) {
+            for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) --q.active;
+            if (q.next < R) {
                 assign(fin, &sp, &started);
                 if ((rc = start_columns<K>(r, started, sp, d_fields))) return rc;
             } else {
-                for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) col_rhs[c] = -1;
+                for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) q.col_rhs[c] = -1;
             }
         }
+        if (compact_to && K > 4 && q.next >= R && q.active > 0 && q.active <= K / 2) {
+            *compact_to = (q.active <= 4) ? 4 : 8;
+            return IF_OK;   // the graph launch already enqueued runs first; the caller repacks after it
+        }
     }
-    if (active > 0) return IF_ECUDA;   // cannot happen: every column stops at max_iter
+    if (q.active > 0) return IF_ECUDA;   // cannot happen: every column stops at max_iter
+    return IF_OK;
+}
+
+// Move the running columns of a KW-wide phase into a KN-wide layout (KN <= KW/2).  The narrow vectors live in the
+// wide buffers that are dead at an iteration boundary: x, z -> the two halves of q; p0, p1 -> the halves of x;
+// q, t -> the halves of z.
+template <int KW, int KN>
+int compact_columns(Run& r, QueueState& q) {
+    static_assert(2 * KN <= KW, "compaction at least halves the width");
+    ColMap map;
+    QueueState nq = q;
+    int j = 0;
+    for (int c = 0; c < KMAX; ++c) { map.src[c] = -1; nq.col_rhs[c] = -1; nq.host_epoch[c] = 0; }
+    for (int c = 0; c < KW; ++c)
+        if (q.col_rhs[c] >= 0) {
+            if (j >= KN) return IF_ECUDA;
+            map.src[j] = c;
+            nq.col_rhs[j] = q.col_rhs[c];
+            nq.host_epoch[j] = q.host_epoch[c];
+            ++j;
+        }
+    const int64_t nv = r.h->n_vert;
+    const size_t vn = (size_t)nv * KN;   // doubles per narrow vector
+    const unsigned g = (unsigned)((vn + BLOCK - 1) / BLOCK);
+    Workspace& w = r.w;
+    double* x2 = w.q;
+    double* z2 = w.q + vn;
+    k_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, map, w.x, x2);
+    IF_LAUNCH_CHECK();
+    k_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, map, w.z, z2);
+    IF_LAUNCH_CHECK();
+    double* p0_2 = w.x;
+    double* p1_2 = w.x + vn;
+    k_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, map, w.p0, p0_2);
+    IF_LAUNCH_CHECK();
+    k_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, map, w.p1, p1_2);
+    IF_LAUNCH_CHECK();
+    double* q2 = w.z;
+    double* t2 = w.z + vn;
+    k_compact_ctrl<<<1, KMAX, 0, r.st>>>(w.ctrl, map, KN);
+    IF_LAUNCH_CHECK();
+    w.x = x2; w.z = z2; w.p0 = p0_2; w.p1 = p1_2; w.q = q2;
+    if (r.order_n == 2) w.t = t2;
+    q = nq;
+    return IF_OK;
+}
+
+template <int K>
+int solve_from(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
+               PollState& poll, KernelTimes* times, QueueState& q, bool first) {
+    int to = 0;
+    int rc = solve_phase<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, q, first, K > 4 ? &to : nullptr);
+    if (rc != IF_OK || to == 0) return rc;
+    if constexpr (K == 16) {
+        if (to == 8) {
+            if ((rc = compact_columns<16, 8>(r, q))) return rc;
+            return solve_from<8>(r, job, d_fields, rhs, n_ells, d_out, poll, nullptr, q, false);
+        }
+        if ((rc = compact_columns<16, 4>(r, q))) return rc;
+        return solve_from<4>(r, job, d_fields, rhs, n_ells, d_out, poll, nullptr, q, false);
+    } else if constexpr (K == 8) {
+        if ((rc = compact_columns<8, 4>(r, q))) return rc;
+        return solve_from<4>(r, job, d_fields, rhs, n_ells, d_out, poll, nullptr, q, false);
+    }
+    return IF_ECUDA;
+}
+
+template <int K>
+int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
+              PollState& poll, KernelTimes* times, int64_t* batch_iters) {
+    QueueState q;
+    int rc = solve_from<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, q, true);
+    if (rc != IF_OK) return rc;
     long long total = 0;
     IF_CUDA_TRY(cudaMemcpyAsync(&total, &r.w.ctrl->total_iters, sizeof(long long), cudaMemcpyDeviceToHost, r.st));
     IF_CUDA_TRY(cudaStreamSynchronize(r.st));
