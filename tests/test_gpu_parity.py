@@ -274,3 +274,25 @@ def test_save_and_load_prepared_mesh(ifl, tmp_path):
     with pytest.raises(ifl.ImplicitFilterError) as e:
         ifl.if_load(str(tmp_path / "missing.ifm"))
     assert e.value.code == -8
+
+
+@pytest.mark.parametrize("n,periodic", [(8, True), (5, False), (12, False)])
+def test_meshes_smaller_than_one_row_tile(ifl, oracle_mod, n, periodic):
+    """Fewer vertices than one 128-row SpMM tile (64, 36, 169 with a ragged second tile): the persistent kernels
+    see one or two tiles, most CTAs none; dense direct solve as the reference for the smallest."""
+    m = grid_mesh(n, periodic=periodic, jitter=0.2, random_diagonals=True, rng=np.random.default_rng(n))
+    rng = np.random.default_rng(100 + n)
+    fields = rng.standard_normal((3, m.n_vert))
+    ells = np.array([0.7, 2.0, 5.0])
+    om = oracle_mod.OracleMesh(m.coords, m.tri, m.period)
+    h = ifl.if_prepare(m.coords, m.tri, m.period)
+    assert h.n_tiles == (m.n_vert + 127) // 128
+    for order_n in (1, 2):
+        out, st = ifl.if_filter(h, fields, ells, order_n)
+        out = out.cpu().numpy()
+        assert st["code"] == 0
+        for f in range(3):
+            for j, ell in enumerate(ells):
+                ref = om.dense_solve(fields[f], ell, order_n) if m.n_vert <= 500 else om.solve(fields[f], ell, order_n)[0]
+                assert rel(out[f, j], ref) <= TOL_FIELD, (order_n, f, j)
+    h.close()
