@@ -223,6 +223,13 @@ __device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_r
 #define IF_SPMM_MINB 1
 #endif
 constexpr int SPMM_BLOCK = IF_SPMM_BLOCK;
+// threads per CTA and CTAs per SM of k_spmm: the 16-column layout fills an SM with one 512-thread CTA (186 KB of
+// stages); the 4-column layout of the compacted tail has stages a third of that size, and two 256-thread CTAs per
+// SM overlap each other's per-tile fixed costs
+template <int K> struct SpmmCfg {
+    static constexpr int NT = (K == 4) ? 256 : SPMM_BLOCK;
+    static constexpr int MINB = (K == 4) ? 2 : IF_SPMM_MINB;
+};
 constexpr int SPMM_STAGES = IF_SPMM_STAGES;
 template <int K, int MODE> struct TileSmem {
     static constexpr int T = TILE_ROWS;
@@ -256,11 +263,11 @@ __device__ __forceinline__ TileIssue load_issue(const int32_t* __restrict__ desc
 //   descriptors and halo row ids are fetched two tiles ahead.
 // About 130 KB of loads per SM are outstanding at all times, which is what the loaded HBM latency of B200 needs.
 template <int K, int MODE>
-__global__ void __launch_bounds__(SPMM_BLOCK, IF_SPMM_MINB) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
+__global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
                                                         double* __restrict__ partials, SpmmArgs a) {
     using SM = TileSmem<K, MODE>;
     constexpr int T = SM::T;
-    constexpr int NT = SPMM_BLOCK;
+    constexpr int NT = SpmmCfg<K>::NT;
     constexpr int TPR = K / 2;
     constexpr int ROWS = NT / TPR;
     constexpr int XPT = (T * TPR + NT - 1) / NT;         // double2 elements of a tile vector per thread
