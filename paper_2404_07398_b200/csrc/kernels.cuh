@@ -210,7 +210,7 @@ __device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_r
     return s0;
 }
 
-// dynamic shared memory of k_spmm: SPMM_STAGES stages of
+// dynamic shared memory of k_spmm: SpmmCfg<K>::STAGES stages of
 //   [gathered vector: T tile rows + HALO_CAP halo rows][second vector: T rows][val slice][col slice][S_vv][A_v | 1/A_v]
 // then a ring of four tile descriptors and one mbarrier per stage
 #ifndef IF_SPMM_BLOCK
@@ -223,14 +223,17 @@ __device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_r
 #define IF_SPMM_MINB 1
 #endif
 constexpr int SPMM_BLOCK = IF_SPMM_BLOCK;
-// threads per CTA and CTAs per SM of k_spmm: the 16-column layout fills an SM with one 512-thread CTA (186 KB of
-// stages); the 4-column layout of the compacted tail has stages a third of that size, and two 256-thread CTAs per
-// SM overlap each other's per-tile fixed costs
-template <int K> struct SpmmCfg {
-    static constexpr int NT = (K == 4) ? 256 : SPMM_BLOCK;
-    static constexpr int MINB = (K == 4) ? 2 : IF_SPMM_MINB;
-};
 constexpr int SPMM_STAGES = IF_SPMM_STAGES;
+// Threads per CTA, CTAs per SM and pipeline stages of k_spmm.  The 16-column layout fills an SM with one 512-thread
+// CTA and three stages (186 KB).  The narrower layouts of the compacted tail have smaller stages and are bound by
+// per-tile fixed costs, not by HBM: two 256-thread CTAs per SM overlap each other's stalls (K = 8 with two stages to
+// fit shared memory).
+template <int K> struct SpmmCfg {
+    static constexpr int NT = (K == 16) ? SPMM_BLOCK : 256;
+    static constexpr int MINB = (K == 16) ? IF_SPMM_MINB : 2;
+    static constexpr int STAGES = (K == 8) ? 2 : SPMM_STAGES;
+};
+
 template <int K, int MODE> struct TileSmem {
     static constexpr int T = TILE_ROWS;
     static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // vectors that arrive by bulk copy
@@ -241,9 +244,9 @@ template <int K, int MODE> struct TileSmem {
     static constexpr size_t off_dg = off_col + (size_t)T * WCAP * sizeof(int32_t);   // S_vv of the tile's rows
     static constexpr size_t off_ar = off_dg + (size_t)T * sizeof(double);            // A_v or 1/A_v
     static constexpr size_t stage_bytes = off_ar + (size_t)T * sizeof(double);
-    static constexpr size_t off_desc = SPMM_STAGES * stage_bytes;
+    static constexpr size_t off_desc = SpmmCfg<K>::STAGES * stage_bytes;
     static constexpr size_t off_bar = off_desc + 4 * 16 * sizeof(int32_t);
-    static constexpr size_t bytes = off_bar + 8 * SPMM_STAGES + 8;
+    static constexpr size_t bytes = off_bar + 8 * SpmmCfg<K>::STAGES + 8;
 };
 
 // What one thread needs to issue the bulk copies of a tile (kept in registers by the issuing thread).
@@ -268,6 +271,8 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     using SM = TileSmem<K, MODE>;
     constexpr int T = SM::T;
     constexpr int NT = SpmmCfg<K>::NT;
+    constexpr int NS = SpmmCfg<K>::STAGES;               // pipeline stages
+    constexpr int LA = NS - 1;                           // tiles the bulk copies run ahead of the gather
     constexpr int TPR = K / 2;
     constexpr int ROWS = NT / TPR;
     constexpr int XPT = (T * TPR + NT - 1) / NT;         // double2 elements of a tile vector per thread
@@ -341,7 +346,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
         }
     };
     // stage views
-    auto stage_ptr = [&](int64_t it) { return smem + (size_t)(it % SPMM_STAGES) * SM::stage_bytes; };
+    auto stage_ptr = [&](int64_t it) { return smem + (size_t)(it % NS) * SM::stage_bytes; };
     // halo of a tile: registers -> shared memory behind the tile rows (p' = z + beta p for the CG passes)
     auto halo_to_smem = [&](unsigned char* st, int nh, const double2 (&h0)[HPT], const double2 (&h1)[HPT]) {
         double2* sa = reinterpret_cast<double2*>(st);
@@ -379,10 +384,10 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     auto is_staged = [&](const int32_t* d) { return d[3] >= 0 && d[2] <= T * WCAP; };
 
     if (tid == 0) {
-        for (int s = 0; s < SPMM_STAGES; ++s) mbar_init(&bars[s], 1);
+        for (int s = 0; s < NS; ++s) mbar_init(&bars[s], 1);
         fence_proxy_async();
     }
-    // ---- prologue: descriptors of tiles 0..2, bulk copies of tiles 0 and 1, tile 0 made ready for its gather
+    // ---- prologue: descriptors of tiles 0..2, bulk copies of the first LA tiles, tile 0 made ready for its gather
     if (tid < 48) {
         const int64_t t = tile0 + (tid / 16) * G;
         sdesc[tid] = t < ntiles ? m.tile_desc[t * 16 + tid % 16] : 0;
@@ -390,11 +395,11 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     __syncthreads();
     TileIssue tq{0, 0, -1};   // thread 0: what it needs to issue the tile two ahead
     if (tid == 0) {
-        for (int k = 0; k < 2; ++k) {
+        for (int k = 0; k < LA; ++k) {
             const int64_t t = tile0 + k * G;
             if (t < ntiles) issue(t, k, load_issue(m.tile_desc, t));
         }
-        if (tile0 + 2 * G < ntiles) tq = load_issue(m.tile_desc, tile0 + 2 * G);
+        if (tile0 + LA * G < ntiles) tq = load_issue(m.tile_desc, tile0 + LA * G);
     }
     int hid_n[HPT];
     double2 h0[HPT], h1[HPT], xv[XPT];
@@ -435,9 +440,9 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
         const int32_t* scp = d + 4;
         const bool staged = is_staged(d);
         if (tid == 0) {
-            const int64_t t2 = tile + 2 * G;
+            const int64_t t2 = tile + LA * G;
             bulk_wait_read0();   // the stage of tile it-1 is free once its bulk store has been read
-            if (t2 < ntiles) issue(t2, (int)((it + 2) % SPMM_STAGES), tq);
+            if (t2 < ntiles) issue(t2, (int)((it + LA) % NS), tq);
             if (CG_A) {
                 bulk_store(a.out1 + row0 * K, sa, (uint32_t)nrows * K * sizeof(double));
                 bulk_commit();
@@ -527,7 +532,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             if (is_staged(d1)) halo_to_smem(st1, d1[3], h0, h1);
             if (tile + 2 * G < ntiles && is_staged(d2)) load_halo(hid_n, d2[3], h0, h1);
             load_hidx(tile + 3 * G, hid_n);
-            mbar_wait(&bars[(it + 1) % SPMM_STAGES], (uint32_t)((it + 1) / SPMM_STAGES) & 1u);
+            mbar_wait(&bars[(it + 1) % NS], (uint32_t)((it + 1) / NS) & 1u);
             if (CG_A) {
                 elementwise(st1, tile + G, xv);
                 load_x(tile + 2 * G, xv);
