@@ -59,6 +59,8 @@ enum {
 
 enum {
     IF_FLAG_KEEP_CSR = 1, /* if_prepare keeps the unpermuted CSR of S so if_mesh_export_csr works */
+    IF_FLAG_MULTIGRID = 4, /* if_prepare also builds the smoothed-aggregation hierarchy that if_options.solver = 1 needs
+                              (about 3 x the memory of the prepared mesh, a second or two of device time)          */
     IF_FLAG_HIGHPASS = 2  /* if_filter (per call): write the high-pass field phi - phibar_l (PAPER.md:143-147,
                              Fig. 3) instead of phibar_l                                                    */
 };
@@ -75,6 +77,13 @@ typedef struct {
                         larger window scatters a tile over the window and defeats the halo staging)         */
     int sfc_kind;    /* 0 => Morton order of the quantised coordinates; 1 => keep the caller's order        */
     int flags;       /* IF_FLAG_*                                                                           */
+    int solver;      /* 0 => Jacobi-preconditioned CG for every right-hand side.  1 => right-hand sides with
+                        l >= mg_min_ell mean edge lengths are solved by multigrid-preconditioned CG (one V(1,1)
+                        cycle of a smoothed-aggregation hierarchy per iteration; n = 1, batch = 16 and a handle
+                        prepared with IF_FLAG_MULTIGRID, else ignored), the rest by Jacobi-PCG.  Same systems,
+                        same stop test, same answers within the tolerance (PAPER.md:207 names the convergence of
+                        plain CG at large scales as the open problem)                                           */
+    double mg_min_ell; /* 0 => 6 (in mean edge lengths; below that Jacobi-PCG needs fewer bytes)                */
 } if_options;
 
 typedef struct {

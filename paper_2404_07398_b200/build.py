@@ -12,7 +12,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
-SRC = [os.path.join(HERE, "csrc", f) for f in ("prepare.cu", "solve.cu")]
+SRC = [os.path.join(HERE, "csrc", f) for f in ("prepare.cu", "solve.cu", "mg.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "common.cuh"), os.path.join(HERE, "csrc", "kernels.cuh"), os.path.join(ROOT, "include", "implicit_filter.h")]
 LIB = os.path.join(HERE, "libimplicit_filter.so")
 

@@ -52,9 +52,38 @@ struct Options {
     int sell_sigma = TILE_ROWS;   // sorting inside a row tile keeps the tile spatially compact
     int sfc_kind = 0;
     int flags = 0;
+    int solver = 0;
+    double mg_min_ell = 6.0;
 };
 
 int resolve_options(const if_options* in, const Options* base, Options* out);
+}  // namespace ifl
+struct if_mesh_s;
+namespace ifl {
+int mg_build(if_mesh_s* h);    // mg.cu: builds h->mg from the SELL matrix and the areas
+void mg_free(if_mesh_s* h);
+
+// ---- multigrid hierarchy (optional, IF_FLAG_MULTIGRID): smoothed aggregation on the internal row order.
+// Level 0 is the mesh itself; level l+1 has one unknown per MG_AGG consecutive rows of level l.  Every level stores
+// the pair (S_l, M_l) on one sparsity pattern, so that A_l = M_l + c S_l is applied matrix-free for any scale.
+constexpr int MG_MAX_LEVELS = 12;
+constexpr int MG_AGG = 8;          // rows per aggregate (consecutive rows of the space-filling-curve order)
+constexpr int MG_COARSEST = 64;    // the hierarchy stops at a level with at most this many unknowns (dense solve)
+struct MgLevel {
+    int64_t n = 0, nnz = 0;
+    int64_t* rowptr = nullptr;   // [n+1]
+    int32_t* col = nullptr;      // [nnz]
+    double2* sm = nullptr;       // [nnz]  (S_ij, M_ij)
+    double2* diag = nullptr;     // [n]    (S_ii, M_ii)
+    // transfer to level l+1 (absent on the coarsest level): P [n x n_coarse] by rows, R = P^T by rows
+    int64_t n_coarse = 0, p_nnz = 0;
+    int64_t* p_rowptr = nullptr;
+    int32_t* p_col = nullptr;
+    double* p_val = nullptr;
+    int64_t* r_rowptr = nullptr;
+    int32_t* r_col = nullptr;
+    double* r_val = nullptr;
+};
 
 }  // namespace ifl
 
@@ -97,6 +126,9 @@ struct if_mesh_s {
     int32_t* csr_col = nullptr;
     double* csr_val = nullptr;
     double* csr_area = nullptr;
+    // multigrid hierarchy (IF_FLAG_MULTIGRID), see MgLevel
+    ifl::MgLevel mg[ifl::MG_MAX_LEVELS];
+    int mg_levels = 0;              // 0: no hierarchy
     // pinned host staging for per-call control data and read-back
     void* h_pinned = nullptr;
     size_t h_pinned_bytes = 0;

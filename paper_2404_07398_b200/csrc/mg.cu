@@ -1,0 +1,389 @@
+// Multigrid hierarchy for the n = 1 systems (M + c S) x = M phi at large scales (the cost and the
+// loss of convergence of plain CG at large l are the paper's stated open problem).
+//
+// Smoothed aggregation on the internal (space-filling-curve) row order:
+//   aggregates      MG_AGG consecutive rows                      (tentative prolongator P_t: piecewise constant)
+//   prolongator     P = (I - omega D_S^-1 S) P_t, omega = 2/3    (smoothed with the stiffness only, so P does not
+//                                                                 depend on the scale)
+//   coarse pair     S_c = P^T S P ,  M_c = P^T M P               (Galerkin; A_c = M_c + c S_c for every column)
+// All sparse products are built as "emit (key, value) triples -> radix sort -> reduce by key", the pattern the
+// assembly of S already uses (prepare.cu).  Built once per mesh by if_prepare(IF_FLAG_MULTIGRID).
+#include <cub/cub.cuh>
+
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+namespace ifl {
+namespace {
+
+constexpr double MG_OMEGA_P = 2.0 / 3.0;
+
+struct DBuf {
+    void* p = nullptr;
+    ~DBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) {
+        if (p) { cudaFree(p); p = nullptr; }
+        return cudaMalloc(&p, bytes ? bytes : 1);
+    }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+    void* release() { void* q = p; p = nullptr; return q; }
+};
+
+struct Add2 {
+    __device__ __forceinline__ double2 operator()(const double2& a, const double2& b) const {
+        return make_double2(a.x + b.x, a.y + b.y);
+    }
+};
+
+typedef unsigned long long u64;
+inline unsigned gridf(int64_t n, int block = 256) { return (unsigned)((n + block - 1) / block); }
+inline int bitsf(uint64_t n) { int b = 1; while ((1ull << b) < n && b < 63) ++b; return b; }
+
+// rowptr[r] = first sorted key whose row (high 32 bits) >= r
+__global__ void k_mg_rowptr(const u64* __restrict__ keys, int64_t nnz, int64_t n, int64_t* __restrict__ rowptr) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > nnz) return;
+    int64_t row_i = i < nnz ? (int64_t)(keys[i] >> 32) : n;
+    int64_t row_p = i > 0 ? (int64_t)(keys[i - 1] >> 32) : -1;
+    for (int64_t r = row_p + 1; r <= row_i; ++r) rowptr[r] = i;
+}
+__global__ void k_mg_cols(const u64* __restrict__ keys, int64_t nnz, int32_t* __restrict__ col) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < nnz) col[i] = (int32_t)(keys[i] & 0xffffffffull);
+}
+
+// level 0 from the SELL matrix: row lengths (diagonal + off-diagonals that are not padding), then the entries
+__global__ void k_mg_l0_len(const int64_t* __restrict__ chunk_ptr, const int32_t* __restrict__ scol, int log2c,
+                            int64_t nv, int64_t* __restrict__ len) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r > nv) return;
+    if (r == nv) { len[r] = 0; return; }
+    const int C = 1 << log2c;
+    const int64_t ch = r >> log2c, cp0 = chunk_ptr[ch];
+    const int w = (int)((chunk_ptr[ch + 1] - cp0) >> log2c);
+    const int64_t o = cp0 + (r & (C - 1)) * w;
+    int n = 1;
+    for (int k = 0; k < w; ++k) n += (scol[o + k] != (int32_t)r);
+    len[r] = n;
+}
+__global__ void k_mg_l0_fill(const int64_t* __restrict__ chunk_ptr, const int32_t* __restrict__ scol,
+                             const double* __restrict__ sval, const double* __restrict__ sdiag,
+                             const double* __restrict__ area, int log2c, int64_t nv,
+                             const int64_t* __restrict__ rowptr, int32_t* __restrict__ col, double2* __restrict__ sm,
+                             double2* __restrict__ diag) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= nv) return;
+    const int C = 1 << log2c;
+    const int64_t ch = r >> log2c, cp0 = chunk_ptr[ch];
+    const int w = (int)((chunk_ptr[ch + 1] - cp0) >> log2c);
+    const int64_t o = cp0 + (r & (C - 1)) * w;
+    int64_t e = rowptr[r];
+    col[e] = (int32_t)r;
+    sm[e] = make_double2(sdiag[r], area[r]);
+    ++e;
+    for (int k = 0; k < w; ++k) {
+        const int32_t c = scol[o + k];
+        if (c == (int32_t)r) continue;
+        col[e] = c;
+        sm[e] = make_double2(sval[o + k], 0.0);
+        ++e;
+    }
+    diag[r] = make_double2(sdiag[r], area[r]);
+}
+
+// P = (I - omega D_S^-1 S) P_t : one triple per matrix entry, keyed (row, aggregate of the column)
+__global__ void k_mg_emit_p(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                            const double2* __restrict__ sm, const double2* __restrict__ diag, int64_t n,
+                            u64* __restrict__ keys, double* __restrict__ vals) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double sii = diag[i].x;
+    const double f = sii > 0.0 ? -MG_OMEGA_P / sii : 0.0;
+    const int64_t b = rowptr[i], e = rowptr[i + 1];
+    const int64_t o = b + i;   // one extra triple per row (the tentative prolongator)
+    keys[o] = ((u64)i << 32) | (u64)(i / MG_AGG);
+    vals[o] = 1.0;
+    for (int64_t k = b; k < e; ++k) {
+        keys[o + 1 + (k - b)] = ((u64)i << 32) | (u64)(col[k] / MG_AGG);
+        vals[o + 1 + (k - b)] = f * sm[k].x;
+    }
+}
+
+// triples of P with swapped key (aggregate, row): sorted they are R = P^T by rows
+__global__ void k_mg_swap_keys(const int64_t* __restrict__ p_rowptr, const int32_t* __restrict__ p_col, int64_t n,
+                               u64* __restrict__ keys) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    for (int64_t k = p_rowptr[i]; k < p_rowptr[i + 1]; ++k) keys[k] = ((u64)p_col[k] << 32) | (u64)i;
+}
+
+// T = G P (G = the level's (S, M) pair): counts per row, then the triples keyed (row, aggregate)
+__global__ void k_mg_count_t(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                             const int64_t* __restrict__ p_rowptr, int64_t n, int64_t* __restrict__ cnt) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    int64_t c = 0;
+    if (i < n)
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) c += p_rowptr[col[k] + 1] - p_rowptr[col[k]];
+    cnt[i] = c;
+}
+__global__ void k_mg_emit_t(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                            const double2* __restrict__ sm, const int64_t* __restrict__ p_rowptr,
+                            const int32_t* __restrict__ p_col, const double* __restrict__ p_val, int64_t n,
+                            const int64_t* __restrict__ off, u64* __restrict__ keys, double2* __restrict__ vals) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int64_t o = off[i];
+    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+        const int64_t j = col[k];
+        const double2 g = sm[k];
+        for (int64_t q = p_rowptr[j]; q < p_rowptr[j + 1]; ++q) {
+            keys[o] = ((u64)i << 32) | (u64)p_col[q];
+            vals[o] = make_double2(g.x * p_val[q], g.y * p_val[q]);
+            ++o;
+        }
+    }
+}
+
+// G_c = P^T T : counts per fine row, then the triples keyed (aggregate a, aggregate b)
+__global__ void k_mg_count_c(const int64_t* __restrict__ p_rowptr, const int64_t* __restrict__ t_rowptr, int64_t n,
+                             int64_t* __restrict__ cnt) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    cnt[i] = i < n ? (p_rowptr[i + 1] - p_rowptr[i]) * (t_rowptr[i + 1] - t_rowptr[i]) : 0;
+}
+__global__ void k_mg_emit_c(const int64_t* __restrict__ p_rowptr, const int32_t* __restrict__ p_col,
+                            const double* __restrict__ p_val, const int64_t* __restrict__ t_rowptr,
+                            const int32_t* __restrict__ t_col, const double2* __restrict__ t_sm, int64_t n,
+                            const int64_t* __restrict__ off, u64* __restrict__ keys, double2* __restrict__ vals) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int64_t o = off[i];
+    for (int64_t q = p_rowptr[i]; q < p_rowptr[i + 1]; ++q) {
+        const u64 a = (u64)p_col[q];
+        const double pv = p_val[q];
+        for (int64_t k = t_rowptr[i]; k < t_rowptr[i + 1]; ++k) {
+            keys[o] = (a << 32) | (u64)t_col[k];
+            vals[o] = make_double2(pv * t_sm[k].x, pv * t_sm[k].y);
+            ++o;
+        }
+    }
+}
+
+__global__ void k_mg_diag(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                          const double2* __restrict__ sm, int64_t n, double2* __restrict__ diag) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double2 d = make_double2(0.0, 0.0);
+    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k)
+        if (col[k] == (int32_t)i) { d.x += sm[k].x; d.y += sm[k].y; }
+    diag[i] = d;
+}
+
+// sort (key, value) pairs by key and add the values of equal keys; the inputs are released
+template <class V, class Op>
+int sort_reduce(DBuf& keys, DBuf& vals, int64_t n, int key_bits, Op op, DBuf& ukeys, DBuf& uvals, int64_t* n_unique,
+                cudaStream_t st) {
+    DBuf k1, v1, tmp, d_n;
+    IF_CUDA_TRY(k1.alloc((size_t)n * sizeof(u64)));
+    IF_CUDA_TRY(v1.alloc((size_t)n * sizeof(V)));
+    size_t tb = 0;
+    IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tb, keys.as<u64>(), k1.as<u64>(), vals.as<V>(), v1.as<V>(), n, 0,
+                                                key_bits, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tb, keys.as<u64>(), k1.as<u64>(), vals.as<V>(), v1.as<V>(), n, 0,
+                                                key_bits, st));
+    ++g_launches;
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    keys.alloc(0);
+    vals.alloc(0);
+    IF_CUDA_TRY(ukeys.alloc((size_t)n * sizeof(u64)));
+    IF_CUDA_TRY(uvals.alloc((size_t)n * sizeof(V)));
+    IF_CUDA_TRY(d_n.alloc(sizeof(int64_t)));
+    tb = 0;
+    IF_CUDA_TRY(cub::DeviceReduce::ReduceByKey(nullptr, tb, k1.as<u64>(), ukeys.as<u64>(), v1.as<V>(), uvals.as<V>(),
+                                               d_n.as<int64_t>(), op, n, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceReduce::ReduceByKey(tmp.p, tb, k1.as<u64>(), ukeys.as<u64>(), v1.as<V>(), uvals.as<V>(),
+                                               d_n.as<int64_t>(), op, n, st));
+    ++g_launches;
+    IF_CUDA_TRY(cudaMemcpyAsync(n_unique, d_n.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    return IF_OK;
+}
+
+// CSR (rowptr, col) from sorted unique keys (row << 32 | col)
+int csr_from_keys(const u64* ukeys, int64_t nnz, int64_t n_rows, DBuf& rowptr, DBuf& col, cudaStream_t st) {
+    IF_CUDA_TRY(rowptr.alloc((size_t)(n_rows + 1) * sizeof(int64_t)));
+    IF_CUDA_TRY(col.alloc((size_t)nnz * sizeof(int32_t)));
+    k_mg_rowptr<<<gridf(nnz + 1), 256, 0, st>>>(ukeys, nnz, n_rows, rowptr.as<int64_t>());
+    IF_LAUNCH_CHECK();
+    k_mg_cols<<<gridf(nnz), 256, 0, st>>>(ukeys, nnz, col.as<int32_t>());
+    IF_LAUNCH_CHECK();
+    return IF_OK;
+}
+
+int exclusive_scan(int64_t* d_in, int64_t* d_out, int64_t n, int64_t* total, cudaStream_t st) {
+    DBuf tmp;
+    size_t tb = 0;
+    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(nullptr, tb, d_in, d_out, n, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    IF_CUDA_TRY(cub::DeviceScan::ExclusiveSum(tmp.p, tb, d_in, d_out, n, st));
+    ++g_launches;
+    IF_CUDA_TRY(cudaMemcpyAsync(total, d_out + (n - 1), sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    return IF_OK;
+}
+
+// transfer operators and the Galerkin pair of level `f` -> fills f.p_*, f.r_* and the matrix of level c
+int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
+    const int64_t n = f.n, nc = (n + MG_AGG - 1) / MG_AGG;
+    int rc;
+    // ---- P
+    {
+        const int64_t ne = f.nnz + n;
+        DBuf keys, vals, uk, uv;
+        IF_CUDA_TRY(keys.alloc((size_t)ne * sizeof(u64)));
+        IF_CUDA_TRY(vals.alloc((size_t)ne * sizeof(double)));
+        k_mg_emit_p<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, n, keys.as<u64>(), vals.as<double>());
+        IF_LAUNCH_CHECK();
+        int64_t pn = 0;
+        if ((rc = sort_reduce<double>(keys, vals, ne, 32 + bitsf((uint64_t)n), cub::Sum(), uk, uv, &pn, st))) return rc;
+        DBuf prow, pcol, pval;
+        if ((rc = csr_from_keys(uk.as<u64>(), pn, n, prow, pcol, st))) return rc;
+        IF_CUDA_TRY(pval.alloc((size_t)pn * sizeof(double)));
+        IF_CUDA_TRY(cudaMemcpyAsync(pval.p, uv.p, (size_t)pn * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        f.n_coarse = nc; f.p_nnz = pn;
+        f.p_rowptr = (int64_t*)prow.release(); f.p_col = (int32_t*)pcol.release(); f.p_val = (double*)pval.release();
+    }
+    // ---- R = P^T
+    {
+        DBuf keys, vals, k1, v1, tmp;
+        IF_CUDA_TRY(keys.alloc((size_t)f.p_nnz * sizeof(u64)));
+        IF_CUDA_TRY(k1.alloc((size_t)f.p_nnz * sizeof(u64)));
+        IF_CUDA_TRY(v1.alloc((size_t)f.p_nnz * sizeof(double)));
+        k_mg_swap_keys<<<gridf(n), 256, 0, st>>>(f.p_rowptr, f.p_col, n, keys.as<u64>());
+        IF_LAUNCH_CHECK();
+        size_t tb = 0;
+        IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tb, keys.as<u64>(), k1.as<u64>(), f.p_val, v1.as<double>(),
+                                                    f.p_nnz, 0, 32 + bitsf((uint64_t)nc), st));
+        IF_CUDA_TRY(tmp.alloc(tb));
+        IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tb, keys.as<u64>(), k1.as<u64>(), f.p_val, v1.as<double>(),
+                                                    f.p_nnz, 0, 32 + bitsf((uint64_t)nc), st));
+        ++g_launches;
+        DBuf rrow, rcol;
+        if ((rc = csr_from_keys(k1.as<u64>(), f.p_nnz, nc, rrow, rcol, st))) return rc;
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        f.r_rowptr = (int64_t*)rrow.release(); f.r_col = (int32_t*)rcol.release(); f.r_val = (double*)v1.release();
+    }
+    // ---- T = G P
+    DBuf trow, tcol, tsm;
+    int64_t tn = 0;
+    {
+        DBuf cnt, off;
+        IF_CUDA_TRY(cnt.alloc((size_t)(n + 1) * sizeof(int64_t)));
+        IF_CUDA_TRY(off.alloc((size_t)(n + 1) * sizeof(int64_t)));
+        k_mg_count_t<<<gridf(n + 1), 256, 0, st>>>(f.rowptr, f.col, f.p_rowptr, n, cnt.as<int64_t>());
+        IF_LAUNCH_CHECK();
+        int64_t ne = 0;
+        if ((rc = exclusive_scan(cnt.as<int64_t>(), off.as<int64_t>(), n + 1, &ne, st))) return rc;
+        DBuf keys, vals, uk, uv;
+        IF_CUDA_TRY(keys.alloc((size_t)ne * sizeof(u64)));
+        IF_CUDA_TRY(vals.alloc((size_t)ne * sizeof(double2)));
+        k_mg_emit_t<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.p_rowptr, f.p_col, f.p_val, n, off.as<int64_t>(),
+                                             keys.as<u64>(), vals.as<double2>());
+        IF_LAUNCH_CHECK();
+        if ((rc = sort_reduce<double2>(keys, vals, ne, 32 + bitsf((uint64_t)n), Add2(), uk, uv, &tn, st))) return rc;
+        if ((rc = csr_from_keys(uk.as<u64>(), tn, n, trow, tcol, st))) return rc;
+        IF_CUDA_TRY(tsm.alloc((size_t)tn * sizeof(double2)));
+        IF_CUDA_TRY(cudaMemcpyAsync(tsm.p, uv.p, (size_t)tn * sizeof(double2), cudaMemcpyDeviceToDevice, st));
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    // ---- G_c = P^T T
+    {
+        DBuf cnt, off;
+        IF_CUDA_TRY(cnt.alloc((size_t)(n + 1) * sizeof(int64_t)));
+        IF_CUDA_TRY(off.alloc((size_t)(n + 1) * sizeof(int64_t)));
+        k_mg_count_c<<<gridf(n + 1), 256, 0, st>>>(f.p_rowptr, trow.as<int64_t>(), n, cnt.as<int64_t>());
+        IF_LAUNCH_CHECK();
+        int64_t ne = 0;
+        if ((rc = exclusive_scan(cnt.as<int64_t>(), off.as<int64_t>(), n + 1, &ne, st))) return rc;
+        DBuf keys, vals, uk, uv;
+        IF_CUDA_TRY(keys.alloc((size_t)ne * sizeof(u64)));
+        IF_CUDA_TRY(vals.alloc((size_t)ne * sizeof(double2)));
+        k_mg_emit_c<<<gridf(n), 256, 0, st>>>(f.p_rowptr, f.p_col, f.p_val, trow.as<int64_t>(), tcol.as<int32_t>(),
+                                             tsm.as<double2>(), n, off.as<int64_t>(), keys.as<u64>(), vals.as<double2>());
+        IF_LAUNCH_CHECK();
+        int64_t cn = 0;
+        if ((rc = sort_reduce<double2>(keys, vals, ne, 32 + bitsf((uint64_t)nc), Add2(), uk, uv, &cn, st))) return rc;
+        DBuf crow, ccol, csm, cdiag;
+        if ((rc = csr_from_keys(uk.as<u64>(), cn, nc, crow, ccol, st))) return rc;
+        IF_CUDA_TRY(csm.alloc((size_t)cn * sizeof(double2)));
+        IF_CUDA_TRY(cudaMemcpyAsync(csm.p, uv.p, (size_t)cn * sizeof(double2), cudaMemcpyDeviceToDevice, st));
+        IF_CUDA_TRY(cdiag.alloc((size_t)nc * sizeof(double2)));
+        k_mg_diag<<<gridf(nc), 256, 0, st>>>(crow.as<int64_t>(), ccol.as<int32_t>(), csm.as<double2>(), nc,
+                                            cdiag.as<double2>());
+        IF_LAUNCH_CHECK();
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        c.n = nc; c.nnz = cn;
+        c.rowptr = (int64_t*)crow.release(); c.col = (int32_t*)ccol.release();
+        c.sm = (double2*)csm.release(); c.diag = (double2*)cdiag.release();
+    }
+    return IF_OK;
+}
+
+}  // namespace
+
+void mg_free(if_mesh_s* h) {
+    for (int l = 0; l < MG_MAX_LEVELS; ++l) {
+        MgLevel& g = h->mg[l];
+        cudaFree(g.rowptr); cudaFree(g.col); cudaFree(g.sm); cudaFree(g.diag);
+        cudaFree(g.p_rowptr); cudaFree(g.p_col); cudaFree(g.p_val);
+        cudaFree(g.r_rowptr); cudaFree(g.r_col); cudaFree(g.r_val);
+        g = MgLevel();
+    }
+    h->mg_levels = 0;
+}
+
+int mg_build(if_mesh_s* h) {
+    cudaStream_t st = 0;
+    const int64_t nv = h->n_vert;
+    int log2c = 0;
+    while ((1 << log2c) < h->sell_c) ++log2c;
+    // level 0: the (S, M) pair in CSR, internal order, diagonal first in every row
+    {
+        DBuf len, rowptr, col, sm, diag;
+        IF_CUDA_TRY(len.alloc((size_t)(nv + 1) * sizeof(int64_t)));
+        IF_CUDA_TRY(rowptr.alloc((size_t)(nv + 1) * sizeof(int64_t)));
+        k_mg_l0_len<<<gridf(nv + 1), 256, 0, st>>>(h->chunk_ptr, h->sell_col, log2c, nv, len.as<int64_t>());
+        IF_LAUNCH_CHECK();
+        int64_t nnz = 0;
+        int rc = exclusive_scan(len.as<int64_t>(), rowptr.as<int64_t>(), nv + 1, &nnz, st);
+        if (rc) return rc;
+        IF_CUDA_TRY(col.alloc((size_t)nnz * sizeof(int32_t)));
+        IF_CUDA_TRY(sm.alloc((size_t)nnz * sizeof(double2)));
+        IF_CUDA_TRY(diag.alloc((size_t)nv * sizeof(double2)));
+        k_mg_l0_fill<<<gridf(nv), 256, 0, st>>>(h->chunk_ptr, h->sell_col, h->sell_val, h->sdiag, h->area, log2c, nv,
+                                               rowptr.as<int64_t>(), col.as<int32_t>(), sm.as<double2>(),
+                                               diag.as<double2>());
+        IF_LAUNCH_CHECK();
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        MgLevel& g = h->mg[0];
+        g.n = nv; g.nnz = nnz;
+        g.rowptr = (int64_t*)rowptr.release(); g.col = (int32_t*)col.release();
+        g.sm = (double2*)sm.release(); g.diag = (double2*)diag.release();
+    }
+    int L = 1;
+    while (h->mg[L - 1].n > MG_COARSEST && L < MG_MAX_LEVELS) {
+        int rc = build_next_level(h->mg[L - 1], h->mg[L], st);
+        if (rc != IF_OK) { mg_free(h); return rc; }
+        ++L;
+    }
+    h->mg_levels = L;
+    return IF_OK;
+}
+
+}  // namespace ifl

@@ -1,0 +1,392 @@
+// Multigrid-preconditioned CG for the n = 1 systems at large scales (included by solve.cu).
+//
+//   PCG on (M + c S) x = M phi, x0 = phi, preconditioner B = one V(1,1) cycle of the smoothed-
+//   aggregation hierarchy of mg.cu with damped Jacobi smoothing and a dense Cholesky solve on the coarsest level.
+//   B is symmetric positive definite and fixed per column, so plain PCG applies.  16 columns at a time, every
+//   column with its own c, alpha, beta and stop time; the scalars are formed on the host from device dot products
+//   (an iteration costs milliseconds, two small read-backs per iteration do not matter here).
+// The stop test is the same as in the Jacobi path: recursive ||r||_2 <= tol ||M phi||_2.
+#pragma once
+
+namespace ifl {
+namespace {
+
+constexpr int MGK = 16;               // columns of the multigrid path
+constexpr double MG_OMEGA = 0.7;      // Jacobi damping of the smoother
+
+struct MgCols {                       // per-column scalars, passed by value
+    double c[MGK];
+    double a[MGK];
+    double b[MGK];
+};
+
+struct MgMat {                        // one level's (S, M) pair
+    const int64_t* __restrict__ rowptr;
+    const int32_t* __restrict__ col;
+    const double2* __restrict__ sm;
+    const double2* __restrict__ diag;
+    int64_t n;
+};
+
+// MODE 0: y = A x ;  MODE 1: y = r - A x ;  MODE 2: y = x + omega (r - A x) / d        with A = M + c S per column
+template <int MODE>
+__global__ void __launch_bounds__(BLOCK) k_mg_apply(MgMat g, MgCols cs, const double* __restrict__ x,
+                                                    const double* __restrict__ r, double* __restrict__ y) {
+    constexpr int TPR = MGK / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    const int l = threadIdx.x % TPR;
+    const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
+    for (int64_t row = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; row < g.n; row += (int64_t)gridDim.x * ROWS) {
+        double2 s = {0.0, 0.0};
+        for (int64_t k = g.rowptr[row]; k < g.rowptr[row + 1]; ++k) {
+            const double2 w = g.sm[k];
+            const double2 v = ld2(x, (int64_t)g.col[k] * MGK + 2 * l);
+            s.x = fma(fma(cc.x, w.x, w.y), v.x, s.x);
+            s.y = fma(fma(cc.y, w.x, w.y), v.y, s.y);
+        }
+        const int64_t ri = row * MGK + 2 * l;
+        if (MODE == 0) {
+            st2(y, ri, s);
+        } else {
+            const double2 rv = ld2(r, ri);
+            double2 t = {rv.x - s.x, rv.y - s.y};
+            if (MODE == 2) {
+                const double2 d = g.diag[row];
+                const double2 xv = ld2(x, ri);
+                t.x = fma(MG_OMEGA * t.x, 1.0 / fma(cc.x, d.x, d.y), xv.x);
+                t.y = fma(MG_OMEGA * t.y, 1.0 / fma(cc.y, d.x, d.y), xv.y);
+            }
+            st2(y, ri, t);
+        }
+    }
+}
+
+// e = omega r / d  (Jacobi sweep from a zero initial guess)
+__global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, MgCols cs, const double* __restrict__ r,
+                                                      double* __restrict__ e) {
+    constexpr int TPR = MGK / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    const int l = threadIdx.x % TPR;
+    const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
+    for (int64_t row = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; row < g.n; row += (int64_t)gridDim.x * ROWS) {
+        const int64_t ri = row * MGK + 2 * l;
+        const double2 d = g.diag[row];
+        const double2 rv = ld2(r, ri);
+        st2(e, ri, make_double2(MG_OMEGA * rv.x / fma(cc.x, d.x, d.y), MG_OMEGA * rv.y / fma(cc.y, d.x, d.y)));
+    }
+}
+
+// y (+)= B x for a scalar CSR matrix (restriction R, prolongation P)
+template <int ACC>
+__global__ void __launch_bounds__(BLOCK) k_mg_csr(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                                                  const double* __restrict__ val, int64_t n,
+                                                  const double* __restrict__ x, double* __restrict__ y) {
+    constexpr int TPR = MGK / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    const int l = threadIdx.x % TPR;
+    for (int64_t row = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; row < n; row += (int64_t)gridDim.x * ROWS) {
+        double2 s = {0.0, 0.0};
+        for (int64_t k = rowptr[row]; k < rowptr[row + 1]; ++k) {
+            const double w = val[k];
+            const double2 v = ld2(x, (int64_t)col[k] * MGK + 2 * l);
+            s.x = fma(w, v.x, s.x);
+            s.y = fma(w, v.y, s.y);
+        }
+        const int64_t ri = row * MGK + 2 * l;
+        if (ACC) { const double2 o = ld2(y, ri); s.x += o.x; s.y += o.y; }
+        st2(y, ri, s);
+    }
+}
+
+// coarsest level: dense Cholesky of A = M + c S per column (one block per column), then the two triangular solves
+__global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, MgCols cs, const double* __restrict__ r, double* __restrict__ e) {
+    __shared__ double a[MG_COARSEST][MG_COARSEST + 1];
+    __shared__ double v[MG_COARSEST];
+    const int c = blockIdx.x, t = threadIdx.x, n = (int)g.n;
+    const double cc = cs.c[c];
+    for (int i = t; i < n; i += 64) {
+        for (int j = 0; j < n; ++j) a[i][j] = 0.0;
+        v[i] = r[(int64_t)i * MGK + c];
+    }
+    __syncthreads();
+    for (int i = t; i < n; i += 64)
+        for (int64_t k = g.rowptr[i]; k < g.rowptr[i + 1]; ++k) a[i][g.col[k]] += fma(cc, g.sm[k].x, g.sm[k].y);
+    __syncthreads();
+    for (int k = 0; k < n; ++k) {                 // right-looking Cholesky, lower triangle
+        if (t == 0) a[k][k] = sqrt(a[k][k]);
+        __syncthreads();
+        for (int i = k + 1 + t; i < n; i += 64) a[i][k] /= a[k][k];
+        __syncthreads();
+        for (int i = k + 1 + t; i < n; i += 64)
+            for (int j = k + 1; j <= i; ++j) a[i][j] -= a[i][k] * a[j][k];
+        __syncthreads();
+    }
+    if (t == 0) {                                 // L y = v ; L^T x = y  (n <= 64: one thread is enough)
+        for (int i = 0; i < n; ++i) {
+            double s = v[i];
+            for (int j = 0; j < i; ++j) s -= a[i][j] * v[j];
+            v[i] = s / a[i][i];
+        }
+        for (int i = n - 1; i >= 0; --i) {
+            double s = v[i];
+            for (int j = i + 1; j < n; ++j) s -= a[j][i] * v[j];
+            v[i] = s / a[i][i];
+        }
+    }
+    __syncthreads();
+    for (int i = t; i < n; i += 64) e[(int64_t)i * MGK + c] = v[i];
+}
+
+// ---- PCG vector kernels on [row][16]
+// out = area * x
+__global__ void __launch_bounds__(BLOCK) k_mg_mass(const double* __restrict__ area, int64_t n, const double* __restrict__ x,
+                                                   double* __restrict__ out) {
+    constexpr int TPR = MGK / 2;
+    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
+    if (i >= n * TPR) return;
+    const double av = area[i / TPR];
+    const double2 xv = ld2(x, 2 * i);
+    st2(out, 2 * i, make_double2(av * xv.x, av * xv.y));
+}
+// x += a p ; r -= a q
+__global__ void __launch_bounds__(BLOCK) k_mg_axpy2(MgCols cs, int64_t n, double* __restrict__ x,
+                                                    const double* __restrict__ p, double* __restrict__ r,
+                                                    const double* __restrict__ q) {
+    constexpr int TPR = MGK / 2;
+    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
+    if (i >= n * TPR) return;
+    const int l = (int)(i % TPR);
+    const double2 al = {cs.a[2 * l], cs.a[2 * l + 1]};
+    double2 xv = ld2(x, 2 * i), rv = ld2(r, 2 * i);
+    const double2 pv = ld2(p, 2 * i), qv = ld2(q, 2 * i);
+    xv.x = fma(al.x, pv.x, xv.x); xv.y = fma(al.y, pv.y, xv.y);
+    rv.x = fma(-al.x, qv.x, rv.x); rv.y = fma(-al.y, qv.y, rv.y);
+    st2(x, 2 * i, xv);
+    st2(r, 2 * i, rv);
+}
+// p = z + b p
+__global__ void __launch_bounds__(BLOCK) k_mg_xpby(MgCols cs, int64_t n, const double* __restrict__ z, double* __restrict__ p) {
+    constexpr int TPR = MGK / 2;
+    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
+    if (i >= n * TPR) return;
+    const int l = (int)(i % TPR);
+    const double2 be = {cs.b[2 * l], cs.b[2 * l + 1]};
+    const double2 zv = ld2(z, 2 * i);
+    double2 pv = ld2(p, 2 * i);
+    pv.x = fma(be.x, pv.x, zv.x); pv.y = fma(be.y, pv.y, zv.y);
+    st2(p, 2 * i, pv);
+}
+// per-block partial sums of a.b and a.c per column (fixed order); k_mg_dot_final adds the blocks in order
+__global__ void __launch_bounds__(BLOCK) k_mg_dot(int64_t n, const double* __restrict__ a, const double* __restrict__ b,
+                                                  const double* __restrict__ c, double* __restrict__ partials) {
+    constexpr int TPR = MGK / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    __shared__ double2 red[2][BLOCK];
+    const int tid = threadIdx.x, l = tid % TPR;
+    double2 s0 = {0.0, 0.0}, s1 = {0.0, 0.0};
+    for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < n; row += (int64_t)gridDim.x * ROWS) {
+        const int64_t ri = row * MGK + 2 * l;
+        const double2 av = ld2(a, ri), bv = ld2(b, ri), cv = ld2(c, ri);
+        s0.x = fma(av.x, bv.x, s0.x); s0.y = fma(av.y, bv.y, s0.y);
+        s1.x = fma(av.x, cv.x, s1.x); s1.y = fma(av.y, cv.y, s1.y);
+    }
+    red[0][tid] = s0;
+    red[1][tid] = s1;
+    __syncthreads();
+    if (tid < 2 * TPR) {
+        const int j = tid / TPR, ll = tid % TPR;
+        double2 s = red[j][ll];
+        for (int i = ll + TPR; i < BLOCK; i += TPR) { s.x += red[j][i].x; s.y += red[j][i].y; }
+        partials[((size_t)blockIdx.x * 2 + j) * MGK + 2 * ll] = s.x;
+        partials[((size_t)blockIdx.x * 2 + j) * MGK + 2 * ll + 1] = s.y;
+    }
+}
+__global__ void k_mg_dot_final(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
+    const int t = threadIdx.x;   // 2 * MGK threads
+    if (t >= 2 * MGK) return;
+    double s = 0.0;
+    for (int b = 0; b < nblocks; ++b) s += partials[(size_t)b * 2 * MGK + t];
+    out[t] = s;
+}
+
+// ------------------------------------------------------------------------------------------- host side
+struct MgBuffers {
+    double *x, *r, *p, *q, *za, *zb;            // level 0, [n][16]
+    double* lev[MG_MAX_LEVELS][4];              // levels >= 1: R, E, T, E2
+    double* partials;                           // [grid][2][16]
+    double* dots;                               // [32]
+    int dot_grid;
+};
+
+inline size_t mg_extra_bytes(const if_mesh_s* h) {
+    if (h->mg_levels < 2) return 0;
+    size_t b = align_up((size_t)h->n_vert * MGK * sizeof(double));            // zb (the sixth level-0 vector)
+    for (int l = 1; l < h->mg_levels; ++l) b += 4 * align_up((size_t)h->mg[l].n * MGK * sizeof(double));
+    b += align_up((size_t)h->n_sm * 4 * 2 * MGK * sizeof(double)) + align_up(2 * MGK * sizeof(double));
+    return b;
+}
+
+inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) {
+    MgBuffers m{};
+    m.x = w.x; m.r = w.z; m.p = w.p0; m.q = w.q; m.za = w.p1;
+    char* p = static_cast<char*>(extra);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { void* r = p + off; off += align_up(bytes); return r; };
+    m.zb = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
+    for (int l = 1; l < h->mg_levels; ++l)
+        for (int k = 0; k < 4; ++k) m.lev[l][k] = (double*)take((size_t)h->mg[l].n * MGK * sizeof(double));
+    m.dot_grid = h->n_sm * 4;
+    m.partials = (double*)take((size_t)m.dot_grid * 2 * MGK * sizeof(double));
+    m.dots = (double*)take(2 * MGK * sizeof(double));
+    return m;
+}
+
+inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n}; }
+inline int mg_grid(const if_mesh_s* h, int64_t n) {
+    const int64_t rows = BLOCK / (MGK / 2);
+    return (int)std::max<int64_t>(1, std::min<int64_t>((n + rows - 1) / rows, (int64_t)h->n_sm * 8));
+}
+
+// one V(1,1) cycle: returns the buffer that holds e = B r on level l
+int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double* R, double* E, double* T, double* E2,
+              double** result) {
+    const if_mesh_s* h = r.h;
+    const MgLevel& g = h->mg[l];
+    const MgMat gm = mg_mat(g);
+    if (l == h->mg_levels - 1) {
+        k_mg_coarse<<<MGK, 64, 0, r.st>>>(gm, cs, R, E);
+        IF_LAUNCH_CHECK();
+        *result = E;
+        return IF_OK;
+    }
+    const int grid = mg_grid(h, g.n), gridc = mg_grid(h, g.n_coarse);
+    k_mg_jacobi0<<<grid, BLOCK, 0, r.st>>>(gm, cs, R, E);
+    IF_LAUNCH_CHECK();
+    k_mg_apply<1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T);
+    IF_LAUNCH_CHECK();
+    double* const* nb = b.lev[l + 1];
+    k_mg_csr<0><<<gridc, BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
+    IF_LAUNCH_CHECK();
+    double* ec = nullptr;
+    int rc = mg_vcycle(r, b, cs, l + 1, nb[0], nb[1], nb[2], nb[3], &ec);
+    if (rc != IF_OK) return rc;
+    k_mg_csr<1><<<grid, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
+    IF_LAUNCH_CHECK();
+    k_mg_apply<2><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2);
+    IF_LAUNCH_CHECK();
+    *result = E2;
+    return IF_OK;
+}
+
+// host copies of (a.b, a.c) per column
+int mg_dots(const Run& r, const MgBuffers& b, const double* a, const double* bb, const double* cc, double* h_out /*[32] pinned*/) {
+    k_mg_dot<<<b.dot_grid, BLOCK, 0, r.st>>>(r.h->n_vert, a, bb, cc, b.partials);
+    IF_LAUNCH_CHECK();
+    k_mg_dot_final<<<1, 2 * MGK, 0, r.st>>>(b.partials, b.dot_grid, b.dots);
+    IF_LAUNCH_CHECK();
+    IF_CUDA_TRY(cudaMemcpyAsync(h_out, b.dots, 2 * MGK * sizeof(double), cudaMemcpyDeviceToHost, r.st));
+    IF_CUDA_TRY(cudaStreamSynchronize(r.st));
+    return IF_OK;
+}
+
+// Up to 16 right-hand sides rhs[first .. first+count) by multigrid-preconditioned CG; results are finalised like in
+// the Jacobi path (energy or scatter, per-RHS stats).
+int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, size_t first, size_t count,
+                   int n_ells, double* d_out, void* mg_extra, double* h_dots /*pinned [32]*/, int64_t* iters_total) {
+    const if_mesh_s* h = r.h;
+    const int64_t nv = h->n_vert;
+    int rc;
+    MgBuffers b = mg_layout(h, r.w, mg_extra);
+    Ctrl hc = fresh_ctrl(r);
+    StartParams sp;
+    MgCols cs;
+    memset(&sp, 0, sizeof(sp));
+    memset(&cs, 0, sizeof(cs));
+    for (int c = 0; c < KMAX; ++c) sp.field[c] = -1;
+    for (size_t i = 0; i < count; ++i) {
+        const Rhs& q = rhs[first + i];
+        cs.c[i] = sp.c[i] = hc.c[i] = r.opt.gamma * q.ell * q.ell;
+        sp.field[i] = hc.field[i] = q.f;
+        sp.rhs[i] = hc.rhs[i] = q.f * n_ells + q.j;
+    }
+    const unsigned eg = (unsigned)((nv * MGK + BLOCK - 1) / BLOCK);
+    const unsigned vg = (unsigned)((nv * (MGK / 2) + BLOCK - 1) / BLOCK);
+    const MgMat g0 = mg_mat(h->mg[0]);
+    const int grid0 = mg_grid(h, nv);
+    k_ingest<MGK><<<eg, BLOCK, 0, r.st>>>(r.m, sp, 0xffffu, d_fields, b.x);
+    IF_LAUNCH_CHECK();
+    k_mg_mass<<<vg, BLOCK, 0, r.st>>>(h->area, nv, b.x, b.za);               // b = M phi
+    IF_LAUNCH_CHECK();
+    k_mg_apply<1><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.x, b.za, b.r);        // r = b - A x0
+    IF_LAUNCH_CHECK();
+    if ((rc = mg_dots(r, b, b.za, b.za, b.za, h_dots))) return rc;
+    double bb[MGK], rr[MGK], rz[MGK];
+    int iters[MGK], status[MGK];
+    bool active[MGK];
+    for (int c = 0; c < MGK; ++c) { bb[c] = h_dots[c]; iters[c] = 0; status[c] = 0; }
+    double* z = nullptr;
+    if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z))) return rc;
+    if ((rc = mg_dots(r, b, b.r, b.r, z, h_dots))) return rc;
+    for (int c = 0; c < MGK; ++c) { rr[c] = h_dots[c]; rz[c] = h_dots[MGK + c]; }
+    IF_CUDA_TRY(cudaMemcpyAsync(b.p, z, (size_t)nv * MGK * sizeof(double), cudaMemcpyDeviceToDevice, r.st));
+    const double tol2 = r.opt.tol * r.opt.tol;
+    int64_t loops = 0;
+    for (;;) {
+        bool any = false;
+        for (int c = 0; c < MGK; ++c) {
+            active[c] = (size_t)c < count && status[c] == 0 && rr[c] > tol2 * bb[c] && iters[c] < r.opt.max_iter;
+            if ((size_t)c < count && status[c] == 0 && !(rr[c] > tol2 * bb[c]) && !std::isfinite(rr[c])) status[c] = 2;
+            any |= active[c];
+        }
+        if (!any) break;
+        k_mg_apply<0><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.p, nullptr, b.q);  // q = A p
+        IF_LAUNCH_CHECK();
+        if ((rc = mg_dots(r, b, b.p, b.q, b.q, h_dots))) return rc;
+        for (int c = 0; c < MGK; ++c) {
+            cs.a[c] = 0.0;
+            if (!active[c]) continue;
+            const double pq = h_dots[c];
+            if (pq > 0.0 && std::isfinite(pq)) cs.a[c] = rz[c] / pq;
+            else { status[c] = 2; active[c] = false; }
+        }
+        k_mg_axpy2<<<vg, BLOCK, 0, r.st>>>(cs, nv, b.x, b.p, b.r, b.q);
+        IF_LAUNCH_CHECK();
+        if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z))) return rc;
+        if ((rc = mg_dots(r, b, b.r, b.r, z, h_dots))) return rc;
+        for (int c = 0; c < MGK; ++c) {
+            cs.b[c] = 0.0;
+            if (!active[c]) continue;
+            iters[c] += 1;
+            rr[c] = h_dots[c];
+            const double rzn = h_dots[MGK + c];
+            cs.b[c] = rzn / rz[c];
+            rz[c] = rzn;
+            if (!std::isfinite(rr[c]) || !std::isfinite(cs.b[c])) { status[c] = 2; cs.b[c] = 0.0; }
+        }
+        k_mg_xpby<<<vg, BLOCK, 0, r.st>>>(cs, nv, z, b.p);
+        IF_LAUNCH_CHECK();
+        ++loops;
+    }
+    *iters_total += loops;
+    // hand the columns to the common finalisation (alpha = 0: nothing pending)
+    for (size_t c = 0; c < count; ++c) {
+        if (status[c] == 0 && rr[c] > tol2 * bb[c]) status[c] = 1;   // stopped by max_iter
+        hc.iters[c] = iters[c];
+        hc.status[c] = status[c];
+        hc.rr[c] = rr[c];
+        hc.bb[c] = bb[c];
+        hc.done[c] = 1;
+    }
+    hc.cur_p = 0;
+    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
+    Run fr = r;
+    fr.w.x = b.x;
+    fr.w.p0 = fr.w.p1 = b.p;
+    fr.g.stream = (int)std::max<int64_t>(1, std::min<int64_t>((nv + 31) / 32, (int64_t)h->n_sm * 4));
+    if ((rc = finalize_columns<MGK>(fr, job, (count >= 16 ? 0xffffu : ((1u << count) - 1u)), d_out, d_fields))) return rc;
+    IF_CUDA_TRY(cudaStreamSynchronize(r.st));   // hc lives on this stack frame
+    return IF_OK;
+}
+
+}  // namespace
+}  // namespace ifl

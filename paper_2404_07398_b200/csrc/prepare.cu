@@ -354,6 +354,8 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
         if (in->max_iter != 0) o.max_iter = in->max_iter;
         if (in->check_every != 0) o.check_every = in->check_every;
         if (in->batch != 0) o.batch = in->batch;
+        if (in->solver != 0) o.solver = in->solver;
+        if (in->mg_min_ell != 0.0) o.mg_min_ell = in->mg_min_ell;
         if (!base) {   // mesh-layout options are fixed at if_prepare
             if (in->sell_c != 0) o.sell_c = in->sell_c;
             if (in->sell_sigma != 0) o.sell_sigma = in->sell_sigma;
@@ -369,6 +371,7 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
     if ((o.sell_c != 32 && o.sell_c != 64 && o.sell_c != 128) || TILE_ROWS % o.sell_c != 0) return IF_EINVAL;   // must divide the SpMM row tile
     if (o.sell_sigma < o.sell_c || o.sell_sigma % o.sell_c != 0) return IF_EINVAL;
     if (o.sfc_kind != 0 && o.sfc_kind != 1) return IF_EINVAL;
+    if ((o.solver != 0 && o.solver != 1) || !(o.mg_min_ell > 0.0)) return IF_EINVAL;
     o.check_every = (o.check_every + 1) & ~1;   // even: the search direction is double-buffered
     *out = o;
     return IF_OK;
@@ -386,6 +389,7 @@ extern "C" void if_destroy(if_handle h) {
     cudaFree(h->chunk_ptr); cudaFree(h->sell_col); cudaFree(h->sell_val); cudaFree(h->area);
     cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->perm); cudaFree(h->iperm);
     cudaFree(h->sell_lcol); cudaFree(h->halo_n); cudaFree(h->tile_desc); cudaFree(h->halo_rows);
+    ifl::mg_free(h);
     cudaFree(h->csr_rowptr); cudaFree(h->csr_col); cudaFree(h->csr_val); cudaFree(h->csr_area);
     if (h->h_pinned) cudaFreeHost(h->h_pinned);
     cudaSetDevice(prev);
@@ -647,6 +651,10 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
 
     h->h_pinned_bytes = 1 << 20;
     IF_CUDA_TRY(cudaHostAlloc(&h->h_pinned, h->h_pinned_bytes, cudaHostAllocDefault));
+    if (opt.flags & IF_FLAG_MULTIGRID) {
+        int rc = mg_build(h);
+        if (rc != IF_OK) return rc;
+    }
     return IF_OK;
 }
 
@@ -811,6 +819,10 @@ extern "C" int if_load(const char* path, if_handle* out) {
         cudaGetLastError();
         if_destroy(h);
         return IF_ENOMEM;
+    }
+    if (h->opt.flags & IF_FLAG_MULTIGRID) {   // the hierarchy is not stored: rebuild it
+        int rc = mg_build(h);
+        if (rc != IF_OK) { if_destroy(h); return rc; }
     }
     *out = h;
     return IF_OK;

@@ -21,10 +21,12 @@ struct Workspace {
     double *x, *z, *p0, *p1, *q, *t;
     double *energy, *relres, *ells, *k_mid, *E;
     int32_t *iters, *status;
+    void* mg_extra;   // buffers of the multigrid path (mg_solve.cuh), NULL if the handle has no hierarchy
     size_t bytes;
 };
 
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+inline size_t mg_extra_bytes(const if_mesh_s* h);   // mg_solve.cuh
 
 Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* base) {
     Workspace w{};
@@ -48,6 +50,8 @@ Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* bas
     w.E = (double*)take(MAX_RHS * sizeof(double));
     w.iters = (int32_t*)take(MAX_RHS * sizeof(int32_t));
     w.status = (int32_t*)take(MAX_RHS * sizeof(int32_t));
+    w.mg_extra = nullptr;
+    if (order_n == 1 && batch == KMAX && h->mg_levels > 1) w.mg_extra = take(mg_extra_bytes(h));
     w.bytes = off;
     return w;
 }
@@ -474,6 +478,12 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
     return IF_OK;
 }
 
+}  // namespace
+}  // namespace ifl
+#include "mg_solve.cuh"
+namespace ifl {
+namespace {
+
 int pick_k(int batch, size_t R) {
     int K = batch;
     while (K > 4 && R <= (size_t)K / 2) K /= 2;   // few right-hand sides: narrower columns, less wasted bandwidth
@@ -515,7 +525,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
         poll.snap = static_cast<Snapshot*>(h->h_pinned);
         poll.h = h;
     } else {
-        IF_CUDA_TRY(cudaHostAlloc((void**)&poll.snap, 4 * sizeof(Snapshot), cudaHostAllocDefault));
+        IF_CUDA_TRY(cudaHostAlloc((void**)&poll.snap, 4 * sizeof(Snapshot) + 512, cudaHostAllocDefault));
         poll.own_pinned = true;
     }
     for (auto& e : poll.ev) IF_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -535,15 +545,31 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
 
     KernelTimes ktimes;
     int64_t batch_iters = 0;
-    const int K = pick_k(r.opt.batch, (size_t)R);
+    // large scales by multigrid-preconditioned CG (option solver = 1), 16 right-hand sides at a time
+    if (job != JOB_APPLY && r.opt.solver == 1 && order_n == 1 && r.w.mg_extra && h->mean_edge > 0.0) {
+        size_t n_big = 0;
+        while (n_big < rhs.size() && rhs[n_big].ell >= r.opt.mg_min_ell * h->mean_edge) ++n_big;
+        if (n_big > 0) {
+            double* h_dots = reinterpret_cast<double*>(reinterpret_cast<char*>(poll.snap) + 4 * sizeof(Snapshot));
+            for (size_t first = 0; first < n_big; first += MGK) {
+                rc = mg_solve_batch(r, job, d_fields, rhs, first, std::min<size_t>(MGK, n_big - first), n_ells, d_out,
+                                    r.w.mg_extra, h_dots, &batch_iters);
+                if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
+            }
+            rhs.erase(rhs.begin(), rhs.begin() + (ptrdiff_t)n_big);
+        }
+    }
+    const int K = pick_k(r.opt.batch, rhs.size());
     if (job == JOB_APPLY) {
         rc = K == 4 ? apply_all<4>(r, d_fields, rhs, n_ells, d_out)
            : K == 8 ? apply_all<8>(r, d_fields, rhs, n_ells, d_out)
                     : apply_all<16>(r, d_fields, rhs, n_ells, d_out);
-    } else {
-        rc = K == 4 ? solve_all<4>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &batch_iters)
-           : K == 8 ? solve_all<8>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &batch_iters)
-                    : solve_all<16>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &batch_iters);
+    } else if (!rhs.empty()) {
+        int64_t jac_iters = 0;
+        rc = K == 4 ? solve_all<4>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &jac_iters)
+           : K == 8 ? solve_all<8>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &jac_iters)
+                    : solve_all<16>(r, job, d_fields, rhs, n_ells, d_out, poll, &ktimes, &jac_iters);
+        batch_iters += jac_iters;
     }
     if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
     if (job == JOB_SPECTRUM) {
