@@ -296,3 +296,44 @@ def test_meshes_smaller_than_one_row_tile(ifl, oracle_mod, n, periodic):
                 ref = om.dense_solve(fields[f], ell, order_n) if m.n_vert <= 500 else om.solve(fields[f], ell, order_n)[0]
                 assert rel(out[f, j], ref) <= TOL_FIELD, (order_n, f, j)
     h.close()
+
+
+# ------------------------------------------------------------------------------------------ multigrid-preconditioned CG
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_n96", "cfg4_L5"])
+def test_multigrid_solver_matches_oracle(ifl, oracle_mod, name):
+    """solver = 1: the large scales go through the smoothed-aggregation V-cycle PCG, the small ones through
+    Jacobi-PCG; same systems, same answers (1e-7 per field, 1e-6 per bin), far fewer iterations at large l."""
+    w = SMALL[name]()
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    ref, en, k_mid, E, _ = oracle_mod.filter_and_spectrum(om, w.fields, w.ells, 1)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period, flags=ifl.IF_FLAG_MULTIGRID)
+    out, st = ifl.if_filter(h, w.fields, w.ells, 1, solver=1, mg_min_ell=2.0)
+    jac, stj = ifl.if_filter(h, w.fields, w.ells, 1)
+    out = out.cpu().numpy()
+    assert st["code"] == 0 and np.all(st["rel_res"] <= 1e-12)
+    for f in range(w.fields.shape[0]):
+        for j in range(w.ells.shape[0]):
+            assert rel(out[f, j], ref[f, j]) <= TOL_FIELD, (f, j)
+    big = w.ells >= 2.0 * h.mean_edge
+    assert big.any() and st["iters"][:, big].sum() < stj["iters"][:, big].sum()
+    # small scales take the Jacobi path (another column width may move a stop by an iteration)
+    assert np.abs(st["iters"][:, ~big] - stj["iters"][:, ~big]).max(initial=0) <= 2
+    sp = ifl.if_spectrum(h, w.fields, w.ells, 1, solver=1, mg_min_ell=2.0)
+    assert np.all(np.abs(sp["E"] - E) <= TOL_BIN * np.abs(E))
+    h.close()
+
+
+def test_multigrid_option_is_ignored_where_it_does_not_apply(ifl, oracle_mod):
+    """n = 2, a handle without hierarchy, or a narrower batch: solver = 1 silently means Jacobi-PCG."""
+    w = SMALL["cfg4_L5"]()
+    h0 = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    h1 = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    a, sa = ifl.if_filter(h0, w.fields, w.ells, 1)
+    for h, kw in ((h0, dict(solver=1)), (h1, dict(solver=1, batch=8))):
+        b, sb = ifl.if_filter(h, w.fields, w.ells, 1, **kw)
+        assert np.abs(sa["iters"] - sb["iters"]).max() <= 2
+        assert float((a - b).abs().max()) <= 1e-9 * float(a.abs().max())
+    c, sc = ifl.if_filter(h1, w.fields, w.ells[:3], 2, solver=1)
+    d, sd = ifl.if_filter(h0, w.fields, w.ells[:3], 2)
+    assert np.abs(sc["iters"] - sd["iters"]).max() <= 2
+    h0.close(); h1.close()
