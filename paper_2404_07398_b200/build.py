@@ -13,7 +13,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SRC = [os.path.join(HERE, "csrc", f) for f in ("prepare.cu", "solve.cu", "mg.cu")]
-DEPS = SRC + [os.path.join(HERE, "csrc", "common.cuh"), os.path.join(HERE, "csrc", "kernels.cuh"), os.path.join(ROOT, "include", "implicit_filter.h")]
+DEPS = ([os.path.join(HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(HERE, "csrc")))]
+        + [os.path.join(ROOT, "include", "implicit_filter.h")])
 LIB = os.path.join(HERE, "libimplicit_filter.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

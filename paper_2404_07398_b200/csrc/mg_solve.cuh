@@ -28,22 +28,31 @@ struct MgMat {                        // one level's (S, M) pair
     int64_t n;
 };
 
+// A row is handled by 8 * SL threads: column pair l = tid % 8, entry slice sl = (tid / 8) % SL.  SL = 1 for the
+// short rows of the fine levels; SL = 4 (one row per warp, slices added with two shuffles) for the coarse levels
+// whose rows have hundreds of entries and would otherwise be walked serially.
 // MODE 0: y = A x ;  MODE 1: y = r - A x ;  MODE 2: y = x + omega (r - A x) / d        with A = M + c S per column
-template <int MODE>
+template <int MODE, int SL>
 __global__ void __launch_bounds__(BLOCK) k_mg_apply(MgMat g, MgCols cs, const double* __restrict__ x,
                                                     const double* __restrict__ r, double* __restrict__ y) {
-    constexpr int TPR = MGK / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    const int l = threadIdx.x % TPR;
+    constexpr int WPB = BLOCK / (8 * SL);
+    const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
     const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
-    for (int64_t row = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; row < g.n; row += (int64_t)gridDim.x * ROWS) {
+    // (rows are padded to whole warps by the loop bound: every lane of a warp takes part in the shuffles)
+    const int64_t n_pad = (g.n + 3) / 4 * 4;
+    for (int64_t row = (int64_t)blockIdx.x * WPB + threadIdx.x / (8 * SL); row < n_pad; row += (int64_t)gridDim.x * WPB) {
         double2 s = {0.0, 0.0};
-        for (int64_t k = g.rowptr[row]; k < g.rowptr[row + 1]; ++k) {
+        const bool live = row < g.n;
+        const int64_t k1 = live ? g.rowptr[row + 1] : 0;
+        for (int64_t k = live ? g.rowptr[row] + sl : 0; k < k1; k += SL) {
             const double2 w = g.sm[k];
             const double2 v = ld2(x, (int64_t)g.col[k] * MGK + 2 * l);
             s.x = fma(fma(cc.x, w.x, w.y), v.x, s.x);
             s.y = fma(fma(cc.y, w.x, w.y), v.y, s.y);
         }
+        if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 8);  s.y += __shfl_xor_sync(0xffffffffu, s.y, 8); }
+        if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 16); s.y += __shfl_xor_sync(0xffffffffu, s.y, 16); }
+        if (sl != 0 || !live) continue;
         const int64_t ri = row * MGK + 2 * l;
         if (MODE == 0) {
             st2(y, ri, s);
@@ -76,22 +85,27 @@ __global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, MgCols cs, const 
     }
 }
 
-// y (+)= B x for a scalar CSR matrix (restriction R, prolongation P)
-template <int ACC>
+// y (+)= B x for a scalar CSR matrix (restriction R, prolongation P); thread mapping as above
+template <int ACC, int SL>
 __global__ void __launch_bounds__(BLOCK) k_mg_csr(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                                                   const double* __restrict__ val, int64_t n,
                                                   const double* __restrict__ x, double* __restrict__ y) {
-    constexpr int TPR = MGK / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    const int l = threadIdx.x % TPR;
-    for (int64_t row = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; row < n; row += (int64_t)gridDim.x * ROWS) {
+    constexpr int WPB = BLOCK / (8 * SL);
+    const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
+    const int64_t n_pad = (n + 3) / 4 * 4;
+    for (int64_t row = (int64_t)blockIdx.x * WPB + threadIdx.x / (8 * SL); row < n_pad; row += (int64_t)gridDim.x * WPB) {
         double2 s = {0.0, 0.0};
-        for (int64_t k = rowptr[row]; k < rowptr[row + 1]; ++k) {
+        const bool live = row < n;
+        const int64_t k1 = live ? rowptr[row + 1] : 0;
+        for (int64_t k = live ? rowptr[row] + sl : 0; k < k1; k += SL) {
             const double w = val[k];
             const double2 v = ld2(x, (int64_t)col[k] * MGK + 2 * l);
             s.x = fma(w, v.x, s.x);
             s.y = fma(w, v.y, s.y);
         }
+        if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 8);  s.y += __shfl_xor_sync(0xffffffffu, s.y, 8); }
+        if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 16); s.y += __shfl_xor_sync(0xffffffffu, s.y, 16); }
+        if (sl != 0 || !live) continue;
         const int64_t ri = row * MGK + 2 * l;
         if (ACC) { const double2 o = ld2(y, ri); s.x += o.x; s.y += o.y; }
         st2(y, ri, s);
@@ -242,8 +256,8 @@ inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) 
 }
 
 inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n}; }
-inline int mg_grid(const if_mesh_s* h, int64_t n) {
-    const int64_t rows = BLOCK / (MGK / 2);
+inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
+    const int64_t rows = BLOCK / (8 * sl);
     return (int)std::max<int64_t>(1, std::min<int64_t>((n + rows - 1) / rows, (int64_t)h->n_sm * 8));
 }
 
@@ -259,20 +273,27 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
         *result = E;
         return IF_OK;
     }
-    const int grid = mg_grid(h, g.n), gridc = mg_grid(h, g.n_coarse);
-    k_mg_jacobi0<<<grid, BLOCK, 0, r.st>>>(gm, cs, R, E);
+    // rows with many entries (coarse levels, restriction) are split over four entry slices
+    const bool wide = g.nnz >= 24 * g.n, wide_r = g.p_nnz >= 24 * g.n_coarse, wide_p = g.p_nnz >= 24 * g.n;
+    const int grid1 = mg_grid(h, g.n);
+    const int grid = mg_grid(h, g.n, wide ? 4 : 1);
+    k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, cs, R, E);
     IF_LAUNCH_CHECK();
-    k_mg_apply<1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T);
+    if (wide) k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T);
+    else k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T);
     IF_LAUNCH_CHECK();
     double* const* nb = b.lev[l + 1];
-    k_mg_csr<0><<<gridc, BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
+    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
+    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
     IF_LAUNCH_CHECK();
     double* ec = nullptr;
     int rc = mg_vcycle(r, b, cs, l + 1, nb[0], nb[1], nb[2], nb[3], &ec);
     if (rc != IF_OK) return rc;
-    k_mg_csr<1><<<grid, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
+    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
+    else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
     IF_LAUNCH_CHECK();
-    k_mg_apply<2><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2);
+    if (wide) k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2);
+    else k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2);
     IF_LAUNCH_CHECK();
     *result = E2;
     return IF_OK;
@@ -317,7 +338,7 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
     IF_LAUNCH_CHECK();
     k_mg_mass<<<vg, BLOCK, 0, r.st>>>(h->area, nv, b.x, b.za);               // b = M phi
     IF_LAUNCH_CHECK();
-    k_mg_apply<1><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.x, b.za, b.r);        // r = b - A x0
+    k_mg_apply<1, 1><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.x, b.za, b.r);     // r = b - A x0
     IF_LAUNCH_CHECK();
     if ((rc = mg_dots(r, b, b.za, b.za, b.za, h_dots))) return rc;
     double bb[MGK], rr[MGK], rz[MGK];
@@ -339,7 +360,7 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
             any |= active[c];
         }
         if (!any) break;
-        k_mg_apply<0><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.p, nullptr, b.q);  // q = A p
+        k_mg_apply<0, 1><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.p, nullptr, b.q);   // q = A p
         IF_LAUNCH_CHECK();
         if ((rc = mg_dots(r, b, b.p, b.q, b.q, h_dots))) return rc;
         for (int c = 0; c < MGK; ++c) {
