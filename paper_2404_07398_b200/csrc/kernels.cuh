@@ -82,7 +82,10 @@ struct StartParams {
     int rhs[KMAX];
 };
 
-enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3 };
+enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4 };
+// MODE_AX (multigrid path, level 0): v = in0 (gathered), r = in1 (own rows), A = M + c S per column, and with
+// SpmmArgs::scale_inv_area as the sub-mode:  0: out0 = A v ;  1: out0 = r - A v ;  2: out0 = v + omega (r - A v)/d
+constexpr double AX_OMEGA = 0.7;   // Jacobi damping of the multigrid smoother
 
 __device__ __forceinline__ double2 ld2(const double* __restrict__ p, int64_t i) {
     return *reinterpret_cast<const double2*>(p + i);
@@ -512,6 +515,18 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 const double ia = sar[r];
                 s.x *= ia; s.y *= ia;            // t = M^-1 S p'
                 st2(a.out0, ri, s);
+            } else if (MODE == MODE_AX) {
+                const double av = sar[r];
+                double2 o = {fma(cc.x, s.x, av * own.x), fma(cc.y, s.y, av * own.y)};   // A v
+                if (a.scale_inv_area >= 1) {
+                    const double2 rv = sb[r * TPR + l];
+                    o.x = rv.x - o.x; o.y = rv.y - o.y;                                  // r - A v
+                    if (a.scale_inv_area == 2) {
+                        o.x = fma(AX_OMEGA * o.x, 1.0 / fma(cc.x, sd, av), own.x);
+                        o.y = fma(AX_OMEGA * o.y, 1.0 / fma(cc.y, sd, av), own.y);
+                    }
+                }
+                st2(a.out0, ri, o);
             } else {
                 // q = A_v p + c (S v)_row ; v = p (n = 1) or t (n = 2)
                 const double av = sar[r];

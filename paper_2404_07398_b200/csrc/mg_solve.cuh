@@ -12,7 +12,7 @@ namespace ifl {
 namespace {
 
 constexpr int MGK = 16;               // columns of the multigrid path
-constexpr double MG_OMEGA = 0.7;      // Jacobi damping of the smoother
+constexpr double MG_OMEGA = AX_OMEGA;  // Jacobi damping of the smoother (level 0 runs in k_spmm<16, MODE_AX>)
 
 struct MgCols {                       // per-column scalars, passed by value
     double c[MGK];
@@ -230,6 +230,7 @@ struct MgBuffers {
     double* partials;                           // [grid][2][16]
     double* dots;                               // [32]
     int dot_grid;
+    int ax_grid;                                // persistent grid of k_spmm<16, MODE_AX> (level-0 operator)
 };
 
 inline size_t mg_extra_bytes(const if_mesh_s* h) {
@@ -273,15 +274,20 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
         *result = E;
         return IF_OK;
     }
+    // level 0: the tiled TMA kernel applies A = M + c S (c from the control block)
+    auto ax = [&](int sub, const double* v, const double* rr, double* out) {
+        SpmmArgs a{v, rr, nullptr, out, nullptr, sub, 0};
+        return launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a);
+    };
     // rows with many entries (coarse levels, restriction) are split over four entry slices
     const bool wide = g.nnz >= 24 * g.n, wide_r = g.p_nnz >= 24 * g.n_coarse, wide_p = g.p_nnz >= 24 * g.n;
     const int grid1 = mg_grid(h, g.n);
     const int grid = mg_grid(h, g.n, wide ? 4 : 1);
     k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, cs, R, E);
     IF_LAUNCH_CHECK();
-    if (wide) k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T);
-    else k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T);
-    IF_LAUNCH_CHECK();
+    if (l == 0) { int rc0 = ax(1, E, R, T); if (rc0) return rc0; }
+    else if (wide) { k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T); IF_LAUNCH_CHECK(); }
+    else { k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T); IF_LAUNCH_CHECK(); }
     double* const* nb = b.lev[l + 1];
     if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
     else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
@@ -292,9 +298,9 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
     if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
     else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
     IF_LAUNCH_CHECK();
-    if (wide) k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2);
-    else k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2);
-    IF_LAUNCH_CHECK();
+    if (l == 0) { int rc0 = ax(2, E, R, E2); if (rc0) return rc0; }
+    else if (wide) { k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2); IF_LAUNCH_CHECK(); }
+    else { k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2); IF_LAUNCH_CHECK(); }
     *result = E2;
     return IF_OK;
 }
@@ -330,6 +336,10 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
         sp.field[i] = hc.field[i] = q.f;
         sp.rhs[i] = hc.rhs[i] = q.f * n_ells + q.j;
     }
+    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm,
+                            (nv + TILE_ROWS - 1) / TILE_ROWS, &b.ax_grid, SpmmCfg<MGK>::NT))) return rc;
+    hc.all_done = 0;   // k_spmm reads c from the control block and returns at once when all_done is set
+    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
     const unsigned eg = (unsigned)((nv * MGK + BLOCK - 1) / BLOCK);
     const unsigned vg = (unsigned)((nv * (MGK / 2) + BLOCK - 1) / BLOCK);
     const MgMat g0 = mg_mat(h->mg[0]);
@@ -338,8 +348,10 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
     IF_LAUNCH_CHECK();
     k_mg_mass<<<vg, BLOCK, 0, r.st>>>(h->area, nv, b.x, b.za);               // b = M phi
     IF_LAUNCH_CHECK();
-    k_mg_apply<1, 1><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.x, b.za, b.r);     // r = b - A x0
-    IF_LAUNCH_CHECK();
+    {
+        SpmmArgs a{b.x, b.za, nullptr, b.r, nullptr, 1, 0};                   // r = b - A x0
+        if ((rc = launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a))) return rc;
+    }
     if ((rc = mg_dots(r, b, b.za, b.za, b.za, h_dots))) return rc;
     double bb[MGK], rr[MGK], rz[MGK];
     int iters[MGK], status[MGK];
@@ -360,8 +372,10 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
             any |= active[c];
         }
         if (!any) break;
-        k_mg_apply<0, 1><<<grid0, BLOCK, 0, r.st>>>(g0, cs, b.p, nullptr, b.q);   // q = A p
-        IF_LAUNCH_CHECK();
+        {
+            SpmmArgs a{b.p, b.p, nullptr, b.q, nullptr, 0, 0};                // q = A p
+            if ((rc = launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a))) return rc;
+        }
         if ((rc = mg_dots(r, b, b.p, b.q, b.q, h_dots))) return rc;
         for (int c = 0; c < MGK; ++c) {
             cs.a[c] = 0.0;
