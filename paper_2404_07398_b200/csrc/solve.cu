@@ -549,6 +549,8 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (job != JOB_APPLY && r.opt.solver == 1 && order_n == 1 && r.w.mg_extra && h->mean_edge > 0.0) {
         size_t n_big = 0;
         while (n_big < rhs.size() && rhs[n_big].ell >= r.opt.mg_min_ell * h->mean_edge) ++n_big;
+        // whole batches of 16: a ragged last batch costs a full one, its (smallest) scales are cheap for Jacobi-PCG
+        if (n_big > MGK && n_big % MGK != 0 && n_big % MGK < MGK / 2 && n_big < rhs.size()) n_big -= n_big % MGK;
         if (n_big > 0) {
             double* h_dots = reinterpret_cast<double*>(reinterpret_cast<char*>(poll.snap) + 4 * sizeof(Snapshot));
             for (size_t first = 0; first < n_big; first += MGK) {
