@@ -22,9 +22,16 @@ def full():
     import paper_2404_07398_b200 as lib
     lib.load_library()
     w = make_config(4)
-    h = lib.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    # as bench.py prepares it: with the multigrid hierarchy, which the default (Jacobi) solver does not touch
+    h = lib.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period, flags=lib.IF_FLAG_MULTIGRID)
     yield lib, w, h
     h.close()
+
+
+@pytest.fixture(scope="module")
+def jacobi_spectrum(full):
+    lib, w, h = full
+    return lib.if_spectrum(h, w.fields, w.ells, 1)
 
 
 @pytest.fixture(scope="module")
@@ -46,11 +53,11 @@ def test_full_mesh_is_the_named_workload(full):
     assert h.n_tiles == (h.n_vert + 127) // 128 and h.unstaged_tiles <= 0.05 * h.n_tiles
 
 
-def test_spectrum_full_size_properties_and_sampled_energies(full, oracle_mesh):
+def test_spectrum_full_size_properties_and_sampled_energies(full, oracle_mesh, jacobi_spectrum):
     """The bench step itself: all 80 right-hand sides.  e_l monotone, E >= 0, every solve converged; the energies of
     sampled right-hand sides (those the oracle finishes in seconds) to 1e-6."""
     lib, w, h = full
-    sp = lib.if_spectrum(h, w.fields, w.ells, 1)
+    sp = jacobi_spectrum
     st = sp["stats"]
     assert st["code"] == 0 and np.all(st["status"] == 0) and np.all(st["rel_res"] <= 1e-12)
     assert np.all(np.diff(sp["energy"], axis=1) < 0.0)                  # strictly decreasing in l
@@ -99,6 +106,36 @@ def test_filter_full_size_largest_scales_properties(full, oracle_mesh):
         assert abs(mean_out - mean_in) <= 1e-9 * float((area * fields[f].abs()).sum())
         lhs, mid, low = float((b * x).sum()), float((x * ax).sum()), float((area * x * x).sum())
         assert abs(lhs - mid) <= 1e-8 * abs(lhs) and mid >= low * (1 - 1e-12)
+
+
+def test_multigrid_spectrum_full_size(full, oracle_mesh, jacobi_spectrum):
+    """solver = 1 (smoothed-aggregation preconditioner on the scales >= 6 mean edges, Jacobi below) on the bench
+    step: the same energies as the Jacobi-preconditioned run, an order of magnitude fewer iterations on the large
+    scales, and the true residual of the largest scale through if_apply."""
+    import torch
+    lib, w, h = full
+    sp = lib.if_spectrum(h, w.fields, w.ells, 1, solver=1)
+    st, stj = sp["stats"], jacobi_spectrum["stats"]
+    assert st["code"] == 0 and np.all(st["status"] == 0) and np.all(st["rel_res"] <= 1e-12)
+    assert np.all(np.abs(sp["energy"] - jacobi_spectrum["energy"]) <= 1e-9 * jacobi_spectrum["energy"])
+    assert np.all(np.diff(sp["energy"], axis=1) < 0.0) and np.all(sp["E"] > 0.0)
+    big = w.ells >= 6.0 * w.mesh.h
+    assert st["iters"][:, big].max() < 200 and stj["iters"][:, big].max() > 5000
+    assert np.array_equal(st["iters"][:, ~big] > 0, stj["iters"][:, ~big] > 0)
+    assert np.all(np.abs(st["iters"][:, ~big] - stj["iters"][:, ~big]) <= 2)     # small scales: the Jacobi path
+    assert st["rhs_iters"] < 0.05 * stj["rhs_iters"]
+    for f, j in ((0, 16), (1, 12)):                                      # multigrid-solved, oracle in seconds
+        x, info = oracle_mesh.solve(w.fields[f], float(w.ells[j]), 1)
+        assert info["status"] == 0 and big[j]
+        e = oracle_mesh.energy(x)
+        assert abs(sp["energy"][f, j] - e) <= TOL_BIN * e, (f, j)
+    out, sf = lib.if_filter(h, w.fields[:1], w.ells[-1:], 1, solver=1)
+    assert sf["code"] == 0 and sf["iters"].max() < 200
+    area = torch.from_numpy(oracle_mesh.area()).to(out.device)
+    b = area * torch.from_numpy(w.fields[0]).to(out.device)
+    ax = lib.if_apply(h, out[0, 0][None, :], w.ells[-1:], 1)[0, 0]
+    assert float(torch.linalg.norm(b - ax) / torch.linalg.norm(b)) <= 1e-9
+    assert abs(float((area * out[0, 0]).sum()) - float(b.sum())) <= 1e-9 * float(b.abs().sum())
 
 
 # ------------------------------------------------------------------------------------------ the other full-size configs
