@@ -64,13 +64,17 @@ int mg_build(if_mesh_s* h);    // mg.cu: builds h->mg from the SELL matrix and t
 void mg_free(if_mesh_s* h);
 
 // ---- multigrid hierarchy (optional, IF_FLAG_MULTIGRID): smoothed aggregation on the internal row order.
-// Level 0 is the mesh itself; level l+1 has one unknown per MG_AGG consecutive rows of level l.  Every level stores
+// Level 0 is the mesh itself; level l+1 has one unknown per graph aggregate of level l (mg.cu).  Every level stores
 // the pair (S_l, M_l) on one sparsity pattern, so that A_l = M_l + c S_l is applied matrix-free for any scale.
 constexpr int MG_MAX_LEVELS = 12;
-constexpr int MG_AGG = 8;          // rows per aggregate (consecutive rows of the space-filling-curve order)
 constexpr int MG_COARSEST = 64;    // the hierarchy stops at a level with at most this many unknowns (dense solve)
+constexpr double MG_OMEGA_MAX = 0.9;   // Jacobi damping of the smoother, lowered where rho(D^-1 S) is large
+constexpr int MG_NU_COARSE = 3;    // smoothing sweeps before and after the coarse correction on levels >= 1
+                                   // (level 0, where a sweep costs a pass over the mesh, does one)
 struct MgLevel {
     int64_t n = 0, nnz = 0;
+    double rho = 2.0;            // estimate of rho(D_S^-1 S) (power iteration, with a safety factor)
+    double omega = 0.7;          // Jacobi damping of the smoother on this level: min(MG_OMEGA_MAX, 1.6 / rho)
     int64_t* rowptr = nullptr;   // [n+1]
     int32_t* col = nullptr;      // [nnz]
     double2* sm = nullptr;       // [nnz]  (S_ij, M_ij)

@@ -85,7 +85,7 @@ struct StartParams {
 enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4 };
 // MODE_AX (multigrid path, level 0): v = in0 (gathered), r = in1 (own rows), A = M + c S per column, and with
 // SpmmArgs::scale_inv_area as the sub-mode:  0: out0 = A v ;  1: out0 = r - A v ;  2: out0 = v + omega (r - A v)/d
-constexpr double AX_OMEGA = 0.7;   // Jacobi damping of the multigrid smoother
+// (omega = SpmmArgs::omega, the Jacobi damping of the multigrid smoother on level 0)
 
 __device__ __forceinline__ double2 ld2(const double* __restrict__ p, int64_t i) {
     return *reinterpret_cast<const double2*>(p + i);
@@ -182,6 +182,7 @@ struct SpmmArgs {
     double* out1;        //                 CG1/CG2A: p_new
     int scale_inv_area;  // PLAIN: multiply the row result by 1/A_v
     int out_idx;         // CG1/CG2A: index of the direction buffer written (recorded in ctrl->cur_p)
+    double omega;        // AX, sub-mode 2: damping
 };
 
 // One row of the staged SpMM: all column ids and values of the row first, then all W gathers from the shared
@@ -522,8 +523,8 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                     const double2 rv = sb[r * TPR + l];
                     o.x = rv.x - o.x; o.y = rv.y - o.y;                                  // r - A v
                     if (a.scale_inv_area == 2) {
-                        o.x = fma(AX_OMEGA * o.x, 1.0 / fma(cc.x, sd, av), own.x);
-                        o.y = fma(AX_OMEGA * o.y, 1.0 / fma(cc.y, sd, av), own.y);
+                        o.x = fma(a.omega * o.x, 1.0 / fma(cc.x, sd, av), own.x);
+                        o.y = fma(a.omega * o.y, 1.0 / fma(cc.y, sd, av), own.y);
                     }
                 }
                 st2(a.out0, ri, o);

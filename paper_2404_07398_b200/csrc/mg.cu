@@ -2,14 +2,19 @@
 // loss of convergence of plain CG at large l are the paper's stated open problem).
 //
 // Smoothed aggregation on the internal (space-filling-curve) row order:
-//   aggregates      MG_AGG consecutive rows                      (tentative prolongator P_t: piecewise constant)
-//   prolongator     P = (I - omega D_S^-1 S) P_t, omega = 2/3    (smoothed with the stiffness only, so P does not
-//                                                                 depend on the scale)
+//   aggregates      greedy over the graph of S, in row order: a row whose neighbours are all free becomes a root
+//                   and takes them; leftovers join a neighbouring aggregate (tentative prolongator P_t: piecewise
+//                   constant).  Graph aggregates never join two connected components of the masked mesh, which
+//                   blocks of consecutive rows did; it is a serial sweep and runs on the host (once per mesh).
+//   prolongator     P = (I - omega_p D_S^-1 S) P_t, omega_p = 4 / (3 rho(D_S^-1 S)), rho by power iteration
+//                   (smoothed with the stiffness only, so P does not depend on the scale)
 //   coarse pair     S_c = P^T S P ,  M_c = P^T M P               (Galerkin; A_c = M_c + c S_c for every column)
 // All sparse products are built as "emit (key, value) triples -> radix sort -> reduce by key", the pattern the
 // assembly of S already uses (prepare.cu).  Built once per mesh by if_prepare(IF_FLAG_MULTIGRID).
 #include <cub/cub.cuh>
 
+#include <algorithm>
+#include <cmath>
 #include <new>
 #include <vector>
 
@@ -18,7 +23,8 @@
 namespace ifl {
 namespace {
 
-constexpr double MG_OMEGA_P = 2.0 / 3.0;
+constexpr int MG_POWER_ITERS = 24;     // power iteration for rho(D_S^-1 S)
+constexpr double MG_RHO_SAFETY = 1.05;  // the iteration approaches rho from below
 
 struct DBuf {
     void* p = nullptr;
@@ -95,18 +101,19 @@ __global__ void k_mg_l0_fill(const int64_t* __restrict__ chunk_ptr, const int32_
 
 // P = (I - omega D_S^-1 S) P_t : one triple per matrix entry, keyed (row, aggregate of the column)
 __global__ void k_mg_emit_p(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
-                            const double2* __restrict__ sm, const double2* __restrict__ diag, int64_t n,
+                            const double2* __restrict__ sm, const double2* __restrict__ diag,
+                            const int32_t* __restrict__ agg, double omega_p, int64_t n,
                             u64* __restrict__ keys, double* __restrict__ vals) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double sii = diag[i].x;
-    const double f = sii > 0.0 ? -MG_OMEGA_P / sii : 0.0;
+    const double f = sii > 0.0 ? -omega_p / sii : 0.0;
     const int64_t b = rowptr[i], e = rowptr[i + 1];
     const int64_t o = b + i;   // one extra triple per row (the tentative prolongator)
-    keys[o] = ((u64)i << 32) | (u64)(i / MG_AGG);
+    keys[o] = ((u64)i << 32) | (u64)agg[i];
     vals[o] = 1.0;
     for (int64_t k = b; k < e; ++k) {
-        keys[o + 1 + (k - b)] = ((u64)i << 32) | (u64)(col[k] / MG_AGG);
+        keys[o + 1 + (k - b)] = ((u64)i << 32) | (u64)agg[col[k]];
         vals[o + 1 + (k - b)] = f * sm[k].x;
     }
 }
@@ -237,17 +244,128 @@ int exclusive_scan(int64_t* d_in, int64_t* d_out, int64_t n, int64_t* total, cud
     return IF_OK;
 }
 
+// power iteration on D_S^-1 S: y = D_S^-1 S x, sq = y^2 ;  x = y / ||y||
+__global__ void k_mg_power_start(int64_t n, double* __restrict__ x) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u64 z = (u64)i * 0x9E3779B97F4A7C15ull + 0x632BE59BD9B4E019ull;   // splitmix64 finaliser: fixed pseudo-random signs
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    x[i] = (double)(z >> 11) * (2.0 / 9007199254740992.0) - 1.0;
+}
+__global__ void k_mg_power_apply(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                                 const double2* __restrict__ sm, const double2* __restrict__ diag, int64_t n,
+                                 const double* __restrict__ x, double* __restrict__ y, double* __restrict__ sq) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double s = 0.0;
+    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) s = fma(sm[k].x, x[col[k]], s);
+    const double d = diag[i].x;
+    s = d > 0.0 ? s / d : 0.0;
+    y[i] = s;
+    sq[i] = s * s;
+}
+__global__ void k_mg_power_scale(int64_t n, const double* __restrict__ y, const double* __restrict__ sumsq,
+                                 double* __restrict__ x) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double nrm = sqrt(*sumsq);
+    x[i] = nrm > 0.0 ? y[i] / nrm : 0.0;
+}
+
+// rho(D_S^-1 S) of a level (>= 1 is returned: the bound used for the damping must cover the mass part, whose
+// Jacobi-scaled spectrum lies near 1)
+int spectral_radius(const MgLevel& f, double* rho, cudaStream_t st) {
+    const int64_t n = f.n;
+    DBuf x, y, sq, sum, tmp;
+    IF_CUDA_TRY(x.alloc((size_t)n * sizeof(double)));
+    IF_CUDA_TRY(y.alloc((size_t)n * sizeof(double)));
+    IF_CUDA_TRY(sq.alloc((size_t)n * sizeof(double)));
+    IF_CUDA_TRY(sum.alloc(sizeof(double)));
+    size_t tb = 0;
+    IF_CUDA_TRY(cub::DeviceReduce::Sum(nullptr, tb, sq.as<double>(), sum.as<double>(), n, st));
+    IF_CUDA_TRY(tmp.alloc(tb));
+    k_mg_power_start<<<gridf(n), 256, 0, st>>>(n, y.as<double>());
+    IF_LAUNCH_CHECK();
+    double h_sum = (double)n;   // rough norm^2 of the start vector; from the second step on x has norm 1 exactly
+    IF_CUDA_TRY(cudaMemcpyAsync(sum.p, &h_sum, sizeof(double), cudaMemcpyHostToDevice, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    for (int it = 0; it < MG_POWER_ITERS; ++it) {
+        k_mg_power_scale<<<gridf(n), 256, 0, st>>>(n, y.as<double>(), sum.as<double>(), x.as<double>());
+        IF_LAUNCH_CHECK();
+        k_mg_power_apply<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, n, x.as<double>(), y.as<double>(),
+                                                  sq.as<double>());
+        IF_LAUNCH_CHECK();
+        IF_CUDA_TRY(cub::DeviceReduce::Sum(tmp.p, tb, sq.as<double>(), sum.as<double>(), n, st));
+        ++g_launches;
+    }
+    IF_CUDA_TRY(cudaMemcpyAsync(&h_sum, sum.p, sizeof(double), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    const double r = std::sqrt(h_sum) * MG_RHO_SAFETY;
+    *rho = (std::isfinite(r) && r > 1.0) ? r : 1.0;
+    return IF_OK;
+}
+
+// Greedy aggregation over the graph of the level's matrix, serial in row order (host).  agg[i] = aggregate of row
+// i, numbered in the order of their roots, so the coarse numbering follows the fine one along the curve.
+int aggregate_rows(const MgLevel& f, DBuf& d_agg, int64_t* n_agg, cudaStream_t st) {
+    const int64_t n = f.n;
+    std::vector<int64_t> rp;
+    std::vector<int32_t> cj, agg;
+    try {
+        rp.resize((size_t)n + 1);
+        cj.resize((size_t)f.nnz);
+        agg.assign((size_t)n, -1);
+    } catch (const std::bad_alloc&) { return IF_ENOMEM; }
+    IF_CUDA_TRY(cudaMemcpyAsync(rp.data(), f.rowptr, (size_t)(n + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaMemcpyAsync(cj.data(), f.col, (size_t)f.nnz * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    int32_t na = 0;
+    // pass 1: roots
+    for (int64_t i = 0; i < n; ++i) {
+        if (agg[i] >= 0) continue;
+        bool all_free = true;
+        for (int64_t k = rp[i]; k < rp[i + 1] && all_free; ++k) all_free = agg[cj[k]] < 0;
+        if (!all_free) continue;
+        for (int64_t k = rp[i]; k < rp[i + 1]; ++k) agg[cj[k]] = na;
+        agg[i] = na++;
+    }
+    // pass 2: a leftover joins the aggregate (as of pass 1) of its first aggregated neighbour; joined rows are
+    // marked -2 - a until the end of the pass so that leftovers do not chain onto each other
+    for (int64_t i = 0; i < n; ++i) {
+        if (agg[i] != -1) continue;
+        for (int64_t k = rp[i]; k < rp[i + 1]; ++k)
+            if (agg[cj[k]] >= 0) { agg[i] = -2 - agg[cj[k]]; break; }
+    }
+    // pass 3: what is still free (possible only in a component without a root) becomes its own aggregate
+    for (int64_t i = 0; i < n; ++i) {
+        if (agg[i] <= -2) agg[i] = -2 - agg[i];
+        else if (agg[i] == -1) agg[i] = na++;
+    }
+    IF_CUDA_TRY(d_agg.alloc((size_t)n * sizeof(int32_t)));
+    IF_CUDA_TRY(cudaMemcpyAsync(d_agg.p, agg.data(), (size_t)n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    *n_agg = na;
+    return IF_OK;
+}
+
 // transfer operators and the Galerkin pair of level `f` -> fills f.p_*, f.r_* and the matrix of level c
 int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
-    const int64_t n = f.n, nc = (n + MG_AGG - 1) / MG_AGG;
+    const int64_t n = f.n;
     int rc;
+    DBuf agg;
+    int64_t nc = 0;
+    if ((rc = aggregate_rows(f, agg, &nc, st))) return rc;
+    const double omega_p = 4.0 / (3.0 * f.rho);
     // ---- P
     {
         const int64_t ne = f.nnz + n;
         DBuf keys, vals, uk, uv;
         IF_CUDA_TRY(keys.alloc((size_t)ne * sizeof(u64)));
         IF_CUDA_TRY(vals.alloc((size_t)ne * sizeof(double)));
-        k_mg_emit_p<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, n, keys.as<u64>(), vals.as<double>());
+        k_mg_emit_p<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, agg.as<int32_t>(), omega_p, n,
+                                             keys.as<u64>(), vals.as<double>());
         IF_LAUNCH_CHECK();
         int64_t pn = 0;
         if ((rc = sort_reduce<double>(keys, vals, ne, 32 + bitsf((uint64_t)n), cub::Sum(), uk, uv, &pn, st))) return rc;
@@ -377,9 +495,15 @@ int mg_build(if_mesh_s* h) {
         g.sm = (double2*)sm.release(); g.diag = (double2*)diag.release();
     }
     int L = 1;
-    while (h->mg[L - 1].n > MG_COARSEST && L < MG_MAX_LEVELS) {
-        int rc = build_next_level(h->mg[L - 1], h->mg[L], st);
+    for (;;) {
+        MgLevel& g = h->mg[L - 1];
+        int rc = spectral_radius(g, &g.rho, st);
         if (rc != IF_OK) { mg_free(h); return rc; }
+        g.omega = std::min(MG_OMEGA_MAX, 1.6 / g.rho);
+        if (g.n <= MG_COARSEST || L >= MG_MAX_LEVELS) break;
+        rc = build_next_level(g, h->mg[L], st);
+        if (rc != IF_OK) { mg_free(h); return rc; }
+        if (h->mg[L].n >= g.n) break;            // no coarsening (a graph without edges): stop here
         ++L;
     }
     h->mg_levels = L;

@@ -1,7 +1,8 @@
 // Multigrid-preconditioned CG for the n = 1 systems at large scales (included by solve.cu).
 //
-//   PCG on (M + c S) x = M phi, x0 = phi, preconditioner B = one V(1,1) cycle of the smoothed-
-//   aggregation hierarchy of mg.cu with damped Jacobi smoothing and a dense Cholesky solve on the coarsest level.
+//   PCG on (M + c S) x = M phi, x0 = phi, preconditioner B = one V cycle of the smoothed-
+//   aggregation hierarchy of mg.cu with damped Jacobi smoothing (one sweep on the mesh, MG_NU_COARSE on the coarse
+//   levels) and a dense Cholesky solve on the coarsest level.
 //   B is symmetric positive definite and fixed per column, so plain PCG applies.  16 columns at a time, every
 //   column with its own c, alpha, beta and stop time; the scalars are formed on the host from device dot products
 //   (an iteration costs milliseconds, two small read-backs per iteration do not matter here).
@@ -12,7 +13,6 @@ namespace ifl {
 namespace {
 
 constexpr int MGK = 16;               // columns of the multigrid path
-constexpr double MG_OMEGA = AX_OMEGA;  // Jacobi damping of the smoother (level 0 runs in k_spmm<16, MODE_AX>)
 
 struct MgCols {                       // per-column scalars, passed by value
     double c[MGK];
@@ -26,6 +26,7 @@ struct MgMat {                        // one level's (S, M) pair
     const double2* __restrict__ sm;
     const double2* __restrict__ diag;
     int64_t n;
+    double omega;                     // Jacobi damping of the smoother on this level
 };
 
 // A row is handled by 8 * SL threads: column pair l = tid % 8, entry slice sl = (tid / 8) % SL.  SL = 1 for the
@@ -62,8 +63,8 @@ __global__ void __launch_bounds__(BLOCK) k_mg_apply(MgMat g, MgCols cs, const do
             if (MODE == 2) {
                 const double2 d = g.diag[row];
                 const double2 xv = ld2(x, ri);
-                t.x = fma(MG_OMEGA * t.x, 1.0 / fma(cc.x, d.x, d.y), xv.x);
-                t.y = fma(MG_OMEGA * t.y, 1.0 / fma(cc.y, d.x, d.y), xv.y);
+                t.x = fma(g.omega * t.x, 1.0 / fma(cc.x, d.x, d.y), xv.x);
+                t.y = fma(g.omega * t.y, 1.0 / fma(cc.y, d.x, d.y), xv.y);
             }
             st2(y, ri, t);
         }
@@ -81,7 +82,7 @@ __global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, MgCols cs, const 
         const int64_t ri = row * MGK + 2 * l;
         const double2 d = g.diag[row];
         const double2 rv = ld2(r, ri);
-        st2(e, ri, make_double2(MG_OMEGA * rv.x / fma(cc.x, d.x, d.y), MG_OMEGA * rv.y / fma(cc.y, d.x, d.y)));
+        st2(e, ri, make_double2(g.omega * rv.x / fma(cc.x, d.x, d.y), g.omega * rv.y / fma(cc.y, d.x, d.y)));
     }
 }
 
@@ -256,52 +257,75 @@ inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) 
     return m;
 }
 
-inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n}; }
+inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n, g.omega}; }
 inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
     const int64_t rows = BLOCK / (8 * sl);
     return (int)std::max<int64_t>(1, std::min<int64_t>((n + rows - 1) / rows, (int64_t)h->n_sm * 8));
 }
 
-// one V(1,1) cycle: returns the buffer that holds e = B r on level l
+// One V cycle on level l: e = B_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
+// nu = 1 on level 0 and MG_NU_COARSE below it.  R holds r and is not changed; E, T, E2 are work buffers of the
+// level; *result is the one that holds e.
 int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double* R, double* E, double* T, double* E2,
               double** result) {
     const if_mesh_s* h = r.h;
     const MgLevel& g = h->mg[l];
     const MgMat gm = mg_mat(g);
-    if (l == h->mg_levels - 1) {
+    const bool last = l == h->mg_levels - 1;
+    if (last && g.n <= MG_COARSEST) {
         k_mg_coarse<<<MGK, 64, 0, r.st>>>(gm, cs, R, E);
         IF_LAUNCH_CHECK();
         *result = E;
         return IF_OK;
     }
-    // level 0: the tiled TMA kernel applies A = M + c S (c from the control block)
-    auto ax = [&](int sub, const double* v, const double* rr, double* out) {
-        SpmmArgs a{v, rr, nullptr, out, nullptr, sub, 0};
-        return launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a);
-    };
     // rows with many entries (coarse levels, restriction) are split over four entry slices
-    const bool wide = g.nnz >= 24 * g.n, wide_r = g.p_nnz >= 24 * g.n_coarse, wide_p = g.p_nnz >= 24 * g.n;
+    const bool wide = g.nnz >= 24 * g.n;
     const int grid1 = mg_grid(h, g.n);
     const int grid = mg_grid(h, g.n, wide ? 4 : 1);
-    k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, cs, R, E);
+    // sub 1: out = rr - A v ;  sub 2: out = v + omega (rr - A v) / d      (level 0: the tiled TMA kernel)
+    auto apply = [&](int sub, const double* v, double* out) -> int {
+        if (l == 0) {
+            SpmmArgs a{v, R, nullptr, out, nullptr, sub, 0, g.omega};
+            return launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a);
+        }
+        if (sub == 1) {
+            if (wide) k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
+            else k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
+        } else {
+            if (wide) k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
+            else k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
+        }
+        IF_LAUNCH_CHECK();
+        return IF_OK;
+    };
+    // a coarsest level too large for the dense solve (coarsening stalled): smoothing only
+    const int nu = last ? 4 * MG_NU_COARSE : (l == 0 ? 1 : MG_NU_COARSE);
+    int rc;
+    double* cur = E;
+    double* spare[2] = {E2, T};
+    k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, cs, R, cur);
     IF_LAUNCH_CHECK();
-    if (l == 0) { int rc0 = ax(1, E, R, T); if (rc0) return rc0; }
-    else if (wide) { k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T); IF_LAUNCH_CHECK(); }
-    else { k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, T); IF_LAUNCH_CHECK(); }
+    for (int k = 1; k < nu; ++k) {
+        if ((rc = apply(2, cur, spare[0]))) return rc;
+        std::swap(cur, spare[0]);
+    }
+    if (last) { *result = cur; return IF_OK; }
+    if ((rc = apply(1, cur, spare[1]))) return rc;                    // residual of the level
     double* const* nb = b.lev[l + 1];
-    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
-    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, T, nb[0]);
+    const bool wide_r = g.p_nnz >= 24 * g.n_coarse, wide_p = g.p_nnz >= 24 * g.n;
+    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, spare[1], nb[0]);
+    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, spare[1], nb[0]);
     IF_LAUNCH_CHECK();
     double* ec = nullptr;
-    int rc = mg_vcycle(r, b, cs, l + 1, nb[0], nb[1], nb[2], nb[3], &ec);
-    if (rc != IF_OK) return rc;
-    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
-    else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, E);
+    if ((rc = mg_vcycle(r, b, cs, l + 1, nb[0], nb[1], nb[2], nb[3], &ec))) return rc;
+    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
+    else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
     IF_LAUNCH_CHECK();
-    if (l == 0) { int rc0 = ax(2, E, R, E2); if (rc0) return rc0; }
-    else if (wide) { k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2); IF_LAUNCH_CHECK(); }
-    else { k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, E, R, E2); IF_LAUNCH_CHECK(); }
-    *result = E2;
+    for (int k = 0; k < nu; ++k) {
+        if ((rc = apply(2, cur, spare[k & 1]))) return rc;
+        std::swap(cur, spare[k & 1]);
+    }
+    *result = cur;
     return IF_OK;
 }
 
