@@ -85,7 +85,9 @@ struct StartParams {
 enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4 };
 // MODE_AX (multigrid path, level 0): v = in0 (gathered), r = in1 (own rows), A = M + c S per column, and with
 // SpmmArgs::scale_inv_area as the sub-mode:  0: out0 = A v ;  1: out0 = r - A v ;  2: out0 = v + omega (r - A v)/d
-// (omega = SpmmArgs::omega, the Jacobi damping of the multigrid smoother on level 0)
+// (omega = SpmmArgs::omega, the Jacobi damping of the multigrid smoother on level 0);  3: as 2, the last sweep of
+// the preconditioner z = B r, plus the CG bookkeeping of kernel B (rho' = r.z, ||r||^2, beta, stop test);  4: as 3
+// at the start of a batch (rho = r.z, beta = 0, no iteration counted).
 
 __device__ __forceinline__ double2 ld2(const double* __restrict__ p, int64_t i) {
     return *reinterpret_cast<const double2*>(p + i);
@@ -171,6 +173,40 @@ __device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __
     }
     if (tid == 0) *ticket = 0u;
     return true;
+}
+
+// CG bookkeeping after z = B r (run by the last block of a grid reduction; tot = rho' per column, then ||r||^2):
+// beta = rho'/rho, stop test, iteration count -- the same rules as the tail of k_update.  `start`: first
+// preconditioner application of a batch (rho = rho', beta = alpha = 0, nothing counted).
+template <int K>
+__device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const double* tot, bool start) {
+    __shared__ int any_active;
+    const int tid = threadIdx.x;
+    if (tid == 0) any_active = 0;
+    __syncthreads();
+    if (tid < K) {
+        if (!ctrl->done[tid]) {
+            const double rho_new = tot[tid], rr = tot[KMAX + tid];
+            const int it = start ? 0 : ctrl->iters[tid] + 1;
+            ctrl->iters[tid] = it;
+            ctrl->rr[tid] = rr;
+            double be = start ? 0.0 : rho_new / ctrl->rho[tid];
+            ctrl->rho[tid] = rho_new;
+            int dn = 0;
+            if (!isfinite(rr)) { dn = 1; ctrl->status[tid] = 2; }
+            else if (rr <= ctrl->tol2 * ctrl->bb[tid]) { dn = 1; ctrl->status[tid] = 0; }
+            else if (!isfinite(be) || !(rho_new > 0.0)) { dn = 1; ctrl->status[tid] = 2; }
+            else if (it >= ctrl->max_iter) { dn = 1; ctrl->status[tid] = 1; }
+            if (dn) { be = 0.0; ctrl->done[tid] = 1; }
+            ctrl->beta[tid] = be;
+            if (start) ctrl->alpha[tid] = 0.0;
+            if (!dn) atomicOr(&any_active, 1);
+        } else {
+            ctrl->beta[tid] = 0.0;
+        }
+    }
+    __syncthreads();
+    if (tid == 0) { ctrl->all_done = !any_active; if (!start) ctrl->total_iters += 1; }
 }
 
 // ------------------------------------------------------------------------------------------- kernel A
@@ -424,7 +460,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             fence_proxy_async();
         }
     }
-    double2 acc[1] = {{0.0, 0.0}};
+    double2 acc[MODE == MODE_AX ? 2 : 1] = {};
     int64_t tile = tile0;
     // ---- main loop.  Iteration `it` gathers tile it (made ready one iteration earlier) and then makes tile it+1
     // ready; one block barrier per tile.
@@ -522,9 +558,12 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 if (a.scale_inv_area >= 1) {
                     const double2 rv = sb[r * TPR + l];
                     o.x = rv.x - o.x; o.y = rv.y - o.y;                                  // r - A v
-                    if (a.scale_inv_area == 2) {
+                    if (a.scale_inv_area >= 2) {
                         o.x = fma(a.omega * o.x, 1.0 / fma(cc.x, sd, av), own.x);
                         o.y = fma(a.omega * o.y, 1.0 / fma(cc.y, sd, av), own.y);
+                        acc[0].x = fma(rv.x, o.x, acc[0].x);  acc[0].y = fma(rv.y, o.y, acc[0].y);     // r.z
+                        acc[MODE == MODE_AX ? 1 : 0].x = fma(rv.x, rv.x, acc[MODE == MODE_AX ? 1 : 0].x);
+                        acc[MODE == MODE_AX ? 1 : 0].y = fma(rv.y, rv.y, acc[MODE == MODE_AX ? 1 : 0].y);
                     }
                 }
                 st2(a.out0, ri, o);
@@ -559,7 +598,8 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     if (CG_A && tid == 0) bulk_wait0();
     if (MODE == MODE_CG1 || MODE == MODE_CG2B) {
         __shared__ double tot[KMAX];
-        if (grid_reduce<K, 1, NT>(acc, partials, &ctrl->ticket[0], tot)) {
+        const double2 acc1[1] = {acc[0]};
+        if (grid_reduce<K, 1, NT>(acc1, partials, &ctrl->ticket[0], tot)) {
             if (tid < K) {
                 const double pq = tot[tid];
                 double al = 0.0;
@@ -570,6 +610,12 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 ctrl->alpha[tid] = al;
             }
         }
+    }
+    if (MODE == MODE_AX && a.scale_inv_area >= 3) {
+        __shared__ double tot2[2 * KMAX];
+        const double2 acc2[2] = {acc[0], acc[MODE == MODE_AX ? 1 : 0]};
+        if (grid_reduce<K, 2, NT>(acc2, partials, &ctrl->ticket[2], tot2))
+            cg_bookkeeping<K>(ctrl, tot2, a.scale_inv_area == 4);
     }
     if (CG_A && blockIdx.x == 0 && tid == 0) ctrl->cur_p = a.out_idx;
 }

@@ -4,8 +4,13 @@
 //   aggregation hierarchy of mg.cu with damped Jacobi smoothing (one sweep on the mesh, MG_NU_COARSE on the coarse
 //   levels) and a dense Cholesky solve on the coarsest level.
 //   B is symmetric positive definite and fixed per column, so plain PCG applies.  16 columns at a time, every
-//   column with its own c, alpha, beta and stop time; the scalars are formed on the host from device dot products
-//   (an iteration costs milliseconds, two small read-backs per iteration do not matter here).
+//   column with its own c, alpha, beta and stop time.  As in the Jacobi path all CG scalars live in the device
+//   control block: the iteration is
+//       k_spmm<16, CG1>      p' = z + beta p ; x += alpha p ; q = A p' ; alpha' = rho / p'.q         (kernel A)
+//       k_mg_rupdate         r -= alpha' q ; e = omega r / d                     (first sweep of B on level 0)
+//       k_spmm<16, AX> sub 1 residual, then restriction, the coarse levels, prolongation
+//       k_spmm<16, AX> sub 3 z = last sweep ; rho' = r.z ; ||r||^2 ; beta ; stop test        (CG bookkeeping)
+//   and the host reads the control block once per iteration to see whether every column has stopped.
 // The stop test is the same as in the Jacobi path: recursive ||r||_2 <= tol ||M phi||_2.
 #pragma once
 
@@ -163,33 +168,35 @@ __global__ void __launch_bounds__(BLOCK) k_mg_mass(const double* __restrict__ ar
     const double2 xv = ld2(x, 2 * i);
     st2(out, 2 * i, make_double2(av * xv.x, av * xv.y));
 }
-// x += a p ; r -= a q
-__global__ void __launch_bounds__(BLOCK) k_mg_axpy2(MgCols cs, int64_t n, double* __restrict__ x,
-                                                    const double* __restrict__ p, double* __restrict__ r,
-                                                    const double* __restrict__ q) {
+// r -= alpha q (alpha from the control block) ; e = omega r / d : the residual update of CG and the first Jacobi
+// sweep (from a zero guess) of the preconditioner on level 0 in one pass
+__global__ void __launch_bounds__(BLOCK, 2) k_mg_rupdate(MgMat g, const Ctrl* __restrict__ ctrl, double* __restrict__ r,
+                                                         const double* __restrict__ q, double* __restrict__ e) {
     constexpr int TPR = MGK / 2;
-    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
-    if (i >= n * TPR) return;
-    const int l = (int)(i % TPR);
-    const double2 al = {cs.a[2 * l], cs.a[2 * l + 1]};
-    double2 xv = ld2(x, 2 * i), rv = ld2(r, 2 * i);
-    const double2 pv = ld2(p, 2 * i), qv = ld2(q, 2 * i);
-    xv.x = fma(al.x, pv.x, xv.x); xv.y = fma(al.y, pv.y, xv.y);
-    rv.x = fma(-al.x, qv.x, rv.x); rv.y = fma(-al.y, qv.y, rv.y);
-    st2(x, 2 * i, xv);
-    st2(r, 2 * i, rv);
-}
-// p = z + b p
-__global__ void __launch_bounds__(BLOCK) k_mg_xpby(MgCols cs, int64_t n, const double* __restrict__ z, double* __restrict__ p) {
-    constexpr int TPR = MGK / 2;
-    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
-    if (i >= n * TPR) return;
-    const int l = (int)(i % TPR);
-    const double2 be = {cs.b[2 * l], cs.b[2 * l + 1]};
-    const double2 zv = ld2(z, 2 * i);
-    double2 pv = ld2(p, 2 * i);
-    pv.x = fma(be.x, pv.x, zv.x); pv.y = fma(be.y, pv.y, zv.y);
-    st2(p, 2 * i, pv);
+    constexpr int ROWS = BLOCK / TPR;
+    constexpr int U = 4;
+    const int l = threadIdx.x % TPR;
+    const double2 cc = ld2(ctrl->c, 2 * l), al = ld2(ctrl->alpha, 2 * l);
+    const int64_t stride = (int64_t)gridDim.x * ROWS;
+    for (int64_t base = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; base < g.n; base += U * stride) {
+        double2 rv[U], qv[U], dv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t row = base + u * stride;
+            if (row < g.n) { rv[u] = ld2(r, row * MGK + 2 * l); qv[u] = ld2(q, row * MGK + 2 * l); dv[u] = g.diag[row]; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t row = base + u * stride;
+            if (row < g.n) {
+                rv[u].x = fma(-al.x, qv[u].x, rv[u].x);
+                rv[u].y = fma(-al.y, qv[u].y, rv[u].y);
+                st2(r, row * MGK + 2 * l, rv[u]);
+                st2(e, row * MGK + 2 * l, make_double2(g.omega * rv[u].x * rcp_pos(fma(cc.x, dv[u].x, dv[u].y)),
+                                                       g.omega * rv[u].y * rcp_pos(fma(cc.y, dv[u].x, dv[u].y))));
+            }
+        }
+    }
 }
 // per-block partial sums of a.b and a.c per column (fixed order); k_mg_dot_final adds the blocks in order
 __global__ void __launch_bounds__(BLOCK) k_mg_dot(int64_t n, const double* __restrict__ a, const double* __restrict__ b,
@@ -226,7 +233,7 @@ __global__ void k_mg_dot_final(const double* __restrict__ partials, int nblocks,
 
 // ------------------------------------------------------------------------------------------- host side
 struct MgBuffers {
-    double *x, *r, *p, *q, *za, *zb;            // level 0, [n][16]
+    double *x, *r, *p[2], *q, *za, *zb;         // level 0, [n][16]
     double* lev[MG_MAX_LEVELS][4];              // levels >= 1: R, E, T, E2
     double* partials;                           // [grid][2][16]
     double* dots;                               // [32]
@@ -236,7 +243,7 @@ struct MgBuffers {
 
 inline size_t mg_extra_bytes(const if_mesh_s* h) {
     if (h->mg_levels < 2) return 0;
-    size_t b = align_up((size_t)h->n_vert * MGK * sizeof(double));            // zb (the sixth level-0 vector)
+    size_t b = 2 * align_up((size_t)h->n_vert * MGK * sizeof(double));        // za, zb (level-0 vectors 6 and 7)
     for (int l = 1; l < h->mg_levels; ++l) b += 4 * align_up((size_t)h->mg[l].n * MGK * sizeof(double));
     b += align_up((size_t)h->n_sm * 4 * 2 * MGK * sizeof(double)) + align_up(2 * MGK * sizeof(double));
     return b;
@@ -244,10 +251,11 @@ inline size_t mg_extra_bytes(const if_mesh_s* h) {
 
 inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) {
     MgBuffers m{};
-    m.x = w.x; m.r = w.z; m.p = w.p0; m.q = w.q; m.za = w.p1;
+    m.x = w.x; m.r = w.z; m.p[0] = w.p0; m.p[1] = w.p1; m.q = w.q;
     char* p = static_cast<char*>(extra);
     size_t off = 0;
     auto take = [&](size_t bytes) { void* r = p + off; off += align_up(bytes); return r; };
+    m.za = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
     m.zb = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
     for (int l = 1; l < h->mg_levels; ++l)
         for (int k = 0; k < 4; ++k) m.lev[l][k] = (double*)take((size_t)h->mg[l].n * MGK * sizeof(double));
@@ -266,8 +274,10 @@ inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
 // One V cycle on level l: e = B_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
 // nu = 1 on level 0 and MG_NU_COARSE below it.  R holds r and is not changed; E, T, E2 are work buffers of the
 // level; *result is the one that holds e.
+// On level 0 the caller may have done the first sweep already (first_done: E = omega r / d) and chooses the
+// sub-mode of the last sweep (final_sub 3 / 4: with the CG bookkeeping, see kernels.cuh).
 int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double* R, double* E, double* T, double* E2,
-              double** result) {
+              double** result, int final_sub = 2, bool first_done = false) {
     const if_mesh_s* h = r.h;
     const MgLevel& g = h->mg[l];
     const MgMat gm = mg_mat(g);
@@ -303,8 +313,10 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
     int rc;
     double* cur = E;
     double* spare[2] = {E2, T};
-    k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, cs, R, cur);
-    IF_LAUNCH_CHECK();
+    if (!(l == 0 && first_done)) {
+        k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, cs, R, cur);
+        IF_LAUNCH_CHECK();
+    }
     for (int k = 1; k < nu; ++k) {
         if ((rc = apply(2, cur, spare[0]))) return rc;
         std::swap(cur, spare[0]);
@@ -322,7 +334,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
     else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
     IF_LAUNCH_CHECK();
     for (int k = 0; k < nu; ++k) {
-        if ((rc = apply(2, cur, spare[k & 1]))) return rc;
+        if ((rc = apply((l == 0 && k == nu - 1) ? final_sub : 2, cur, spare[k & 1]))) return rc;
         std::swap(cur, spare[k & 1]);
     }
     *result = cur;
@@ -360,87 +372,64 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
         sp.field[i] = hc.field[i] = q.f;
         sp.rhs[i] = hc.rhs[i] = q.f * n_ells + q.j;
     }
-    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm,
-                            (nv + TILE_ROWS - 1) / TILE_ROWS, &b.ax_grid, SpmmCfg<MGK>::NT))) return rc;
+    const int64_t tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
+    int cg_grid = 0;
+    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &b.ax_grid,
+                            SpmmCfg<MGK>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<MGK, MODE_CG1>, TileSmem<MGK, MODE_CG1>::bytes, h->n_sm, tiles, &cg_grid,
+                            SpmmCfg<MGK>::NT))) return rc;
     hc.all_done = 0;   // k_spmm reads c from the control block and returns at once when all_done is set
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
     const unsigned eg = (unsigned)((nv * MGK + BLOCK - 1) / BLOCK);
     const unsigned vg = (unsigned)((nv * (MGK / 2) + BLOCK - 1) / BLOCK);
     const MgMat g0 = mg_mat(h->mg[0]);
-    const int grid0 = mg_grid(h, nv);
+    const int ru_grid = (int)std::max<int64_t>(1, std::min<int64_t>((nv + 15) / 16, (int64_t)h->n_sm * 8));
     k_ingest<MGK><<<eg, BLOCK, 0, r.st>>>(r.m, sp, 0xffffu, d_fields, b.x);
     IF_LAUNCH_CHECK();
     k_mg_mass<<<vg, BLOCK, 0, r.st>>>(h->area, nv, b.x, b.za);               // b = M phi
     IF_LAUNCH_CHECK();
     {
-        SpmmArgs a{b.x, b.za, nullptr, b.r, nullptr, 1, 0};                   // r = b - A x0
+        SpmmArgs a{b.x, b.za, nullptr, b.r, nullptr, 1, 0, 0.0};              // r = b - A x0
         if ((rc = launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a))) return rc;
     }
-    if ((rc = mg_dots(r, b, b.za, b.za, b.za, h_dots))) return rc;
-    double bb[MGK], rr[MGK], rz[MGK];
-    int iters[MGK], status[MGK];
-    bool active[MGK];
-    for (int c = 0; c < MGK; ++c) { bb[c] = h_dots[c]; iters[c] = 0; status[c] = 0; }
+    IF_CUDA_TRY(cudaMemsetAsync(b.p[0], 0, (size_t)nv * MGK * sizeof(double), r.st));
+    if ((rc = mg_dots(r, b, b.za, b.za, b.za, h_dots))) return rc;            // ||M phi||^2 (host sync)
+    // the control block of the batch: unused columns stay done, the others start with rho, beta set by the first
+    // preconditioner application (sub-mode 4)
+    for (int c = 0; c < MGK; ++c) {
+        hc.bb[c] = h_dots[c];
+        hc.done[c] = (size_t)c < count ? 0 : 1;
+    }
+    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
     double* z = nullptr;
-    if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z))) return rc;
-    if ((rc = mg_dots(r, b, b.r, b.r, z, h_dots))) return rc;
-    for (int c = 0; c < MGK; ++c) { rr[c] = h_dots[c]; rz[c] = h_dots[MGK + c]; }
-    IF_CUDA_TRY(cudaMemcpyAsync(b.p, z, (size_t)nv * MGK * sizeof(double), cudaMemcpyDeviceToDevice, r.st));
-    const double tol2 = r.opt.tol * r.opt.tol;
+    if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z, 4, false))) return rc;
+    int* h_flag = reinterpret_cast<int*>(h_dots);
+    auto all_done = [&](bool* out) -> int {
+        IF_CUDA_TRY(cudaMemcpyAsync(h_flag, &r.w.ctrl->all_done, sizeof(int), cudaMemcpyDeviceToHost, r.st));
+        IF_CUDA_TRY(cudaStreamSynchronize(r.st));
+        *out = *h_flag != 0;
+        return IF_OK;
+    };
+    bool stop = false;
+    if ((rc = all_done(&stop))) return rc;
     int64_t loops = 0;
-    for (;;) {
-        bool any = false;
-        for (int c = 0; c < MGK; ++c) {
-            active[c] = (size_t)c < count && status[c] == 0 && rr[c] > tol2 * bb[c] && iters[c] < r.opt.max_iter;
-            if ((size_t)c < count && status[c] == 0 && !(rr[c] > tol2 * bb[c]) && !std::isfinite(rr[c])) status[c] = 2;
-            any |= active[c];
-        }
-        if (!any) break;
+    int cur = 0;
+    while (!stop) {
         {
-            SpmmArgs a{b.p, b.p, nullptr, b.q, nullptr, 0, 0};                // q = A p
-            if ((rc = launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a))) return rc;
+            SpmmArgs a{z, b.p[cur], b.x, b.q, b.p[cur ^ 1], 0, cur ^ 1, 0.0};  // kernel A of the Jacobi path
+            if ((rc = launch_spmm<MGK, MODE_CG1>(r, cg_grid, a))) return rc;
         }
-        if ((rc = mg_dots(r, b, b.p, b.q, b.q, h_dots))) return rc;
-        for (int c = 0; c < MGK; ++c) {
-            cs.a[c] = 0.0;
-            if (!active[c]) continue;
-            const double pq = h_dots[c];
-            if (pq > 0.0 && std::isfinite(pq)) cs.a[c] = rz[c] / pq;
-            else { status[c] = 2; active[c] = false; }
-        }
-        k_mg_axpy2<<<vg, BLOCK, 0, r.st>>>(cs, nv, b.x, b.p, b.r, b.q);
+        cur ^= 1;
+        k_mg_rupdate<<<ru_grid, BLOCK, 0, r.st>>>(g0, r.w.ctrl, b.r, b.q, b.za);
         IF_LAUNCH_CHECK();
-        if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z))) return rc;
-        if ((rc = mg_dots(r, b, b.r, b.r, z, h_dots))) return rc;
-        for (int c = 0; c < MGK; ++c) {
-            cs.b[c] = 0.0;
-            if (!active[c]) continue;
-            iters[c] += 1;
-            rr[c] = h_dots[c];
-            const double rzn = h_dots[MGK + c];
-            cs.b[c] = rzn / rz[c];
-            rz[c] = rzn;
-            if (!std::isfinite(rr[c]) || !std::isfinite(cs.b[c])) { status[c] = 2; cs.b[c] = 0.0; }
-        }
-        k_mg_xpby<<<vg, BLOCK, 0, r.st>>>(cs, nv, z, b.p);
-        IF_LAUNCH_CHECK();
+        if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z, 3, true))) return rc;
         ++loops;
+        if ((rc = all_done(&stop))) return rc;
     }
     *iters_total += loops;
-    // hand the columns to the common finalisation (alpha = 0: nothing pending)
-    for (size_t c = 0; c < count; ++c) {
-        if (status[c] == 0 && rr[c] > tol2 * bb[c]) status[c] = 1;   // stopped by max_iter
-        hc.iters[c] = iters[c];
-        hc.status[c] = status[c];
-        hc.rr[c] = rr[c];
-        hc.bb[c] = bb[c];
-        hc.done[c] = 1;
-    }
-    hc.cur_p = 0;
-    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
+    // the columns are finalised from the device control block (pending alpha p included, as in the Jacobi path)
     Run fr = r;
     fr.w.x = b.x;
-    fr.w.p0 = fr.w.p1 = b.p;
     fr.g.stream = (int)std::max<int64_t>(1, std::min<int64_t>((nv + 31) / 32, (int64_t)h->n_sm * 4));
     if ((rc = finalize_columns<MGK>(fr, job, (count >= 16 ? 0xffffu : ((1u << count) - 1u)), d_out, d_fields))) return rc;
     IF_CUDA_TRY(cudaStreamSynchronize(r.st));   // hc lives on this stack frame
