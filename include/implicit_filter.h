@@ -78,12 +78,12 @@ typedef struct {
     int sfc_kind;    /* 0 => Morton order of the quantised coordinates; 1 => keep the caller's order        */
     int flags;       /* IF_FLAG_*                                                                           */
     int solver;      /* 0 => Jacobi-preconditioned CG for every right-hand side.  1 => right-hand sides with
-                        l >= mg_min_ell mean edge lengths are solved by multigrid-preconditioned CG (one V(1,1)
+                        l >= mg_min_ell mean edge lengths are solved by multigrid-preconditioned CG (one V
                         cycle of a smoothed-aggregation hierarchy per iteration; n = 1, batch = 16 and a handle
                         prepared with IF_FLAG_MULTIGRID, else ignored), the rest by Jacobi-PCG.  Same systems,
                         same stop test, same answers within the tolerance (PAPER.md:207 names the convergence of
                         plain CG at large scales as the open problem)                                           */
-    double mg_min_ell; /* 0 => 6 (in mean edge lengths; below that Jacobi-PCG needs fewer bytes)                */
+    double mg_min_ell; /* 0 => 4 (in mean edge lengths; below that Jacobi-PCG needs fewer bytes)                */
 } if_options;
 
 typedef struct {

@@ -53,7 +53,7 @@ struct Options {
     int sfc_kind = 0;
     int flags = 0;
     int solver = 0;
-    double mg_min_ell = 6.0;
+    double mg_min_ell = 4.0;
 };
 
 int resolve_options(const if_options* in, const Options* base, Options* out);

@@ -18,6 +18,16 @@ namespace ifl {
 namespace {
 
 constexpr int MGK = 16;               // columns of the multigrid path
+constexpr int MG_UB = 4;              // matrix entries a thread has in flight in the CSR kernels of the hierarchy
+#ifndef IF_MG_BPS
+#define IF_MG_BPS 6                   // blocks per SM of the CSR kernels (what their registers allow: one full wave)
+#endif
+#ifndef IF_MG_MINB
+#define IF_MG_MINB 6
+#endif
+#ifndef IF_MG_WIDE
+#define IF_MG_WIDE 24                 // mean row length from which a row is split over four entry slices
+#endif
 
 struct MgCols {                       // per-column scalars, passed by value
     double c[MGK];
@@ -39,22 +49,38 @@ struct MgMat {                        // one level's (S, M) pair
 // whose rows have hundreds of entries and would otherwise be walked serially.
 // MODE 0: y = A x ;  MODE 1: y = r - A x ;  MODE 2: y = x + omega (r - A x) / d        with A = M + c S per column
 template <int MODE, int SL>
-__global__ void __launch_bounds__(BLOCK) k_mg_apply(MgMat g, MgCols cs, const double* __restrict__ x,
+__global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, MgCols cs, const double* __restrict__ x,
                                                     const double* __restrict__ r, double* __restrict__ y) {
     constexpr int WPB = BLOCK / (8 * SL);
     const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
     const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
     // (rows are padded to whole warps by the loop bound: every lane of a warp takes part in the shuffles)
-    const int64_t n_pad = (g.n + 3) / 4 * 4;
-    for (int64_t row = (int64_t)blockIdx.x * WPB + threadIdx.x / (8 * SL); row < n_pad; row += (int64_t)gridDim.x * WPB) {
+    // a block walks a contiguous range of rows, WPB at a time: neighbouring rows gather the same rows of x, which
+    // the L1 then serves (a grid-stride assignment sends every gather to the L2)
+    const int64_t per_block = ((g.n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;
+    const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, (g.n + 3) / 4 * 4);
+    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / (8 * SL); row < row_end; row += WPB) {
         double2 s = {0.0, 0.0};
         const bool live = row < g.n;
         const int64_t k1 = live ? g.rowptr[row + 1] : 0;
-        for (int64_t k = live ? g.rowptr[row] + sl : 0; k < k1; k += SL) {
-            const double2 w = g.sm[k];
-            const double2 v = ld2(x, (int64_t)g.col[k] * MGK + 2 * l);
-            s.x = fma(fma(cc.x, w.x, w.y), v.x, s.x);
-            s.y = fma(fma(cc.y, w.x, w.y), v.y, s.y);
+        // MG_UB entries at a time: their column ids and values first, then the gathers, then the multiply-adds
+        for (int64_t k = live ? g.rowptr[row] + sl : 0; k < k1; k += MG_UB * SL) {
+            double2 w[MG_UB], v[MG_UB];
+            int32_t cj[MG_UB];
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j) {
+                const int64_t kk = k + j * SL < k1 ? k + j * SL : k;
+                cj[j] = g.col[kk];
+                w[j] = g.sm[kk];
+            }
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * MGK + 2 * l);
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j)
+                if (k + j * SL < k1) {
+                    s.x = fma(fma(cc.x, w[j].x, w[j].y), v[j].x, s.x);
+                    s.y = fma(fma(cc.y, w[j].x, w[j].y), v[j].y, s.y);
+                }
         }
         if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 8);  s.y += __shfl_xor_sync(0xffffffffu, s.y, 8); }
         if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 16); s.y += __shfl_xor_sync(0xffffffffu, s.y, 16); }
@@ -93,21 +119,35 @@ __global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, MgCols cs, const 
 
 // y (+)= B x for a scalar CSR matrix (restriction R, prolongation P); thread mapping as above
 template <int ACC, int SL>
-__global__ void __launch_bounds__(BLOCK) k_mg_csr(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+__global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                                                   const double* __restrict__ val, int64_t n,
                                                   const double* __restrict__ x, double* __restrict__ y) {
     constexpr int WPB = BLOCK / (8 * SL);
     const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
-    const int64_t n_pad = (n + 3) / 4 * 4;
-    for (int64_t row = (int64_t)blockIdx.x * WPB + threadIdx.x / (8 * SL); row < n_pad; row += (int64_t)gridDim.x * WPB) {
+    const int64_t per_block = ((n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;   // contiguous rows per block
+    const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, (n + 3) / 4 * 4);
+    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / (8 * SL); row < row_end; row += WPB) {
         double2 s = {0.0, 0.0};
         const bool live = row < n;
         const int64_t k1 = live ? rowptr[row + 1] : 0;
-        for (int64_t k = live ? rowptr[row] + sl : 0; k < k1; k += SL) {
-            const double w = val[k];
-            const double2 v = ld2(x, (int64_t)col[k] * MGK + 2 * l);
-            s.x = fma(w, v.x, s.x);
-            s.y = fma(w, v.y, s.y);
+        for (int64_t k = live ? rowptr[row] + sl : 0; k < k1; k += MG_UB * SL) {
+            double w[MG_UB];
+            double2 v[MG_UB];
+            int32_t cj[MG_UB];
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j) {
+                const int64_t kk = k + j * SL < k1 ? k + j * SL : k;
+                cj[j] = col[kk];
+                w[j] = val[kk];
+            }
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * MGK + 2 * l);
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j)
+                if (k + j * SL < k1) {
+                    s.x = fma(w[j], v[j].x, s.x);
+                    s.y = fma(w[j], v[j].y, s.y);
+                }
         }
         if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 8);  s.y += __shfl_xor_sync(0xffffffffu, s.y, 8); }
         if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 16); s.y += __shfl_xor_sync(0xffffffffu, s.y, 16); }
@@ -268,7 +308,7 @@ inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) 
 inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n, g.omega}; }
 inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
     const int64_t rows = BLOCK / (8 * sl);
-    return (int)std::max<int64_t>(1, std::min<int64_t>((n + rows - 1) / rows, (int64_t)h->n_sm * 8));
+    return (int)std::max<int64_t>(1, std::min<int64_t>((n + rows - 1) / rows, (int64_t)h->n_sm * IF_MG_BPS));
 }
 
 // One V cycle on level l: e = B_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
@@ -289,7 +329,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
         return IF_OK;
     }
     // rows with many entries (coarse levels, restriction) are split over four entry slices
-    const bool wide = g.nnz >= 24 * g.n;
+    const bool wide = g.nnz >= IF_MG_WIDE * g.n;
     const int grid1 = mg_grid(h, g.n);
     const int grid = mg_grid(h, g.n, wide ? 4 : 1);
     // sub 1: out = rr - A v ;  sub 2: out = v + omega (rr - A v) / d      (level 0: the tiled TMA kernel)
@@ -324,7 +364,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
     if (last) { *result = cur; return IF_OK; }
     if ((rc = apply(1, cur, spare[1]))) return rc;                    // residual of the level
     double* const* nb = b.lev[l + 1];
-    const bool wide_r = g.p_nnz >= 24 * g.n_coarse, wide_p = g.p_nnz >= 24 * g.n;
+    const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse, wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
     if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, spare[1], nb[0]);
     else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, spare[1], nb[0]);
     IF_LAUNCH_CHECK();

@@ -109,28 +109,29 @@ def test_filter_full_size_largest_scales_properties(full, oracle_mesh):
 
 
 def test_multigrid_spectrum_full_size(full, oracle_mesh, jacobi_spectrum):
-    """solver = 1 (smoothed-aggregation preconditioner on the scales >= 6 mean edges, Jacobi below) on the bench
+    """solver = 1 (smoothed-aggregation preconditioner on the scales >= 4 mean edges, Jacobi below) on the bench
     step: the same energies as the Jacobi-preconditioned run, an order of magnitude fewer iterations on the large
     scales, and the true residual of the largest scale through if_apply."""
     import torch
     lib, w, h = full
-    sp = lib.if_spectrum(h, w.fields, w.ells, 1, solver=1)
+    sp = lib.if_spectrum(h, w.fields, w.ells, 1, solver=1, mg_min_ell=4.0)
     st, stj = sp["stats"], jacobi_spectrum["stats"]
     assert st["code"] == 0 and np.all(st["status"] == 0) and np.all(st["rel_res"] <= 1e-12)
     assert np.all(np.abs(sp["energy"] - jacobi_spectrum["energy"]) <= 1e-9 * jacobi_spectrum["energy"])
     assert np.all(np.diff(sp["energy"], axis=1) < 0.0) and np.all(sp["E"] > 0.0)
-    big = w.ells >= 6.0 * w.mesh.h
-    assert st["iters"][:, big].max() < 200 and stj["iters"][:, big].max() > 5000
+    big = w.ells >= 4.0 * h.mean_edge
+    assert int(big.sum()) * 2 % 16 == 0                                  # whole batches: no remainder moved
+    assert st["iters"][:, big].max() < 100 and stj["iters"][:, big].max() > 5000
     assert np.array_equal(st["iters"][:, ~big] > 0, stj["iters"][:, ~big] > 0)
     assert np.all(np.abs(st["iters"][:, ~big] - stj["iters"][:, ~big]) <= 2)     # small scales: the Jacobi path
-    assert st["rhs_iters"] < 0.05 * stj["rhs_iters"]
+    assert st["rhs_iters"] < 0.02 * stj["rhs_iters"]
     for f, j in ((0, 16), (1, 12)):                                      # multigrid-solved, oracle in seconds
         x, info = oracle_mesh.solve(w.fields[f], float(w.ells[j]), 1)
         assert info["status"] == 0 and big[j]
         e = oracle_mesh.energy(x)
         assert abs(sp["energy"][f, j] - e) <= TOL_BIN * e, (f, j)
     out, sf = lib.if_filter(h, w.fields[:1], w.ells[-1:], 1, solver=1)
-    assert sf["code"] == 0 and sf["iters"].max() < 200
+    assert sf["code"] == 0 and sf["iters"].max() < 100
     area = torch.from_numpy(oracle_mesh.area()).to(out.device)
     b = area * torch.from_numpy(w.fields[0]).to(out.device)
     ax = lib.if_apply(h, out[0, 0][None, :], w.ells[-1:], 1)[0, 0]
