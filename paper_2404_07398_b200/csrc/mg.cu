@@ -15,6 +15,8 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <new>
 #include <vector>
 
@@ -507,6 +509,11 @@ int mg_build(if_mesh_s* h) {
         ++L;
     }
     h->mg_levels = L;
+    if (getenv("IF_VERBOSE"))
+        for (int l = 0; l < L; ++l)
+            fprintf(stderr, "[implicit_filter] multigrid level %d: %lld rows, %.1f entries per row, rho %.3f, omega %.3f, "
+                            "P %.1f entries per row\n", l, (long long)h->mg[l].n, (double)h->mg[l].nnz / (double)h->mg[l].n,
+                    h->mg[l].rho, h->mg[l].omega, h->mg[l].n ? (double)h->mg[l].p_nnz / (double)h->mg[l].n : 0.0);
     return IF_OK;
 }
 

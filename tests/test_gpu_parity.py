@@ -337,3 +337,64 @@ def test_multigrid_option_is_ignored_where_it_does_not_apply(ifl, oracle_mod):
     d, sd = ifl.if_filter(h0, w.fields, w.ells[:3], 2)
     assert np.abs(sc["iters"] - sd["iters"]).max() <= 2
     h0.close(); h1.close()
+
+
+def test_multigrid_on_disconnected_and_degenerate_inputs(ifl, oracle_mod):
+    """Three components (two jittered 40 x 40 grids and a lone triangle), scales far above their size: the filter
+    tends to each component's own area-weighted mean, which the graph aggregates must respect.  Also constants and
+    zeros (no iteration), the iteration cap (a status), high-pass output and host buffers with solver = 1."""
+    a = grid_mesh(40, periodic=False, jitter=0.25, random_diagonals=True, rng=np.random.default_rng(5))
+    b = grid_mesh(40, periodic=False, jitter=0.25, random_diagonals=True, rng=np.random.default_rng(6))
+    lone = np.array([[200.0, 0.0], [201.0, 0.1], [200.4, 0.9]])
+    coords = np.concatenate([a.coords, b.coords + np.array([60.0, 3.0]), lone])
+    tri = np.concatenate([a.tri, b.tri + a.n_vert, np.array([[0, 1, 2]], dtype=np.int32) + 2 * a.n_vert]).astype(np.int32)
+    V = coords.shape[0]
+    rng = np.random.default_rng(77)
+    fields = np.stack([rng.standard_normal(V), np.full(V, -1.5), np.zeros(V)])
+    ells = np.array([1.0, 6.0, 40.0, 400.0])
+    om = oracle_mod.OracleMesh(coords, tri, None)
+    h = ifl.if_prepare(coords, tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    out, st = ifl.if_filter(h, fields, ells, 1, solver=1, mg_min_ell=2.0)
+    jac, stj = ifl.if_filter(h, fields, ells, 1)
+    out = out.cpu().numpy()
+    assert st["code"] == 0 and np.all(st["rel_res"] <= 1e-12)
+    for j, ell in enumerate(ells):
+        x, info = om.solve(fields[0], float(ell), 1)
+        assert info["status"] == 0 and rel(out[0, j], x) <= TOL_FIELD, j
+    assert st["iters"][0, 1:].max() < 80 and stj["iters"][0, 3] > 10 * st["iters"][0, 3]
+    area = om.area()
+    for lo, hi in ((0, a.n_vert), (a.n_vert, 2 * a.n_vert), (2 * a.n_vert, V)):      # per-component means at l = 400
+        mean = float((area[lo:hi] * fields[0, lo:hi]).sum() / area[lo:hi].sum())
+        assert np.abs(out[0, 3, lo:hi] - mean).max() <= 2e-2 * np.abs(fields[0]).max()
+        assert abs(float((area[lo:hi] * out[0, 3, lo:hi]).sum() / area[lo:hi].sum()) - mean) <= 1e-10
+    # a constant is a fixed point (S 1 = 0): nothing to do but to clean up the rounding of c S 1 at l = 400
+    assert np.all(st["iters"][1, :3] <= 1) and st["iters"][1, 3] <= 8 and np.all(st["iters"][2] == 0)
+    assert np.abs(out[1] + 1.5).max() <= 1e-9 and np.all(out[2] == 0.0)     # (the lone triangle is the loosest)
+    # iteration cap inside the multigrid path
+    o2, s2 = ifl.if_filter(h, fields[:1], ells[-1:], 1, solver=1, mg_min_ell=2.0, max_iter=3)
+    assert s2["code"] == 1 and s2["status"][0, 0] == 1 and s2["iters"][0, 0] == 3
+    assert np.all(np.isfinite(o2.cpu().numpy()))
+    # high-pass output and host buffers
+    hp, _ = ifl.if_filter(h, fields[:1], ells, 1, solver=1, mg_min_ell=2.0, flags=ifl.IF_FLAG_HIGHPASS)
+    assert rel(hp[0].cpu().numpy(), fields[0][None, :] - out[0]) <= 1e-10
+    sp_d = ifl.if_spectrum(h, fields[:1], ells, 1, solver=1, mg_min_ell=2.0)
+    sp_h = ifl.if_spectrum_host(h, fields[:1], ells, 1, solver=1, mg_min_ell=2.0)
+    assert np.array_equal(sp_d["energy"], sp_h["energy"])
+    en = np.array([om.energy(om.solve(fields[0], float(l), 1)[0]) for l in ells])
+    assert np.all(np.abs(sp_d["energy"][0] - en) <= TOL_BIN * en)
+    h.close()
+
+
+def test_multigrid_hierarchy_survives_save_and_load(ifl, tmp_path):
+    """if_save / if_load of a handle prepared with IF_FLAG_MULTIGRID: the loaded handle solves with solver = 1 and
+    gives the same iteration counts and bits (the hierarchy is rebuilt deterministically on load)."""
+    w = make_config(4, level=5, n_ells=7)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    a, sa = ifl.if_filter(h, w.fields, w.ells, 1, solver=1, mg_min_ell=2.0)
+    path = str(tmp_path / "mesh_mg.bin")
+    ifl.if_save(h, path)
+    h2 = ifl.if_load(path)
+    b, sb = ifl.if_filter(h2, w.fields, w.ells, 1, solver=1, mg_min_ell=2.0)
+    assert np.array_equal(sa["iters"], sb["iters"]) and sa["iters"].max() < 60
+    assert bool((a == b).all())
+    h.close(); h2.close()
