@@ -82,18 +82,33 @@ struct StartParams {
     int rhs[KMAX];
 };
 
-enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4 };
+enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4, MODE_MGR = 5 };
 // MODE_AX (multigrid path, level 0): v = in0 (gathered), r = in1 (own rows), A = M + c S per column, and with
 // SpmmArgs::scale_inv_area as the sub-mode:  0: out0 = A v ;  1: out0 = r - A v ;  2: out0 = v + omega (r - A v)/d
 // (omega = SpmmArgs::omega, the Jacobi damping of the multigrid smoother on level 0);  3: as 2, the last sweep of
 // the preconditioner z = B r, plus the CG bookkeeping of kernel B (rho' = r.z, ||r||^2, beta, stop test);  4: as 3
 // at the start of a batch (rho = r.z, beta = 0, no iteration counted).
+// MODE_MGR (multigrid path, level 0): the residual update of CG, the first Jacobi sweep of the preconditioner (from a
+// zero guess) and the residual of that sweep in one pass.  in0 = r, in1 = q (both gathered: tile by bulk copy, halo
+// rows from L2), alpha from the control block:  r' = r - alpha q -> x ;  e = omega r'/d -> out1 ;  t = r' - A e -> out0.
+// r' goes to a second buffer (x), not over r: other blocks still read r and q for their halo rows.
 
 __device__ __forceinline__ double2 ld2(const double* __restrict__ p, int64_t i) {
     return *reinterpret_cast<const double2*>(p + i);
 }
 __device__ __forceinline__ void st2(double* __restrict__ p, int64_t i, double2 v) {
     *reinterpret_cast<double2*>(p + i) = v;
+}
+
+// 1/d for d > 0 in the normal range: hardware seed (2^-23) and two Newton steps (full fp64 precision, ~1 ulp).
+// A fp64 division costs about five times as many instructions and made the streaming update kernel (kernel B) issue-bound.
+__device__ __forceinline__ double rcp_pos(double d) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    double e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-d, r, 1.0);
+    return fma(r, e, r);
 }
 
 // ---- bulk async copy (TMA) and mbarrier wrappers (PTX ISA: cp.async.bulk, mbarrier)
@@ -213,7 +228,7 @@ __device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const do
 struct SpmmArgs {
     const double* in0;   // PLAIN: x        CG1/CG2A: z        CG2B: t            (the gathered vector)
     const double* in1;   //                 CG1/CG2A: p_old    CG2B: p (current)
-    double* x;           //                 CG1/CG2A: x (in place)
+    double* x;           //                 CG1/CG2A: x (in place)                        MGR: r' (new residual)
     double* out0;        // PLAIN: y        CG1: q             CG2A: t            CG2B: q
     double* out1;        //                 CG1/CG2A: p_new
     int scale_inv_area;  // PLAIN: multiply the row result by 1/A_v
@@ -318,6 +333,8 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     constexpr int XPT = (T * TPR + NT - 1) / NT;         // double2 elements of a tile vector per thread
     constexpr int HPT = (HALO_CAP + ROWS - 1) / ROWS;    // halo rows per thread group
     constexpr bool CG_A = (MODE == MODE_CG1 || MODE == MODE_CG2A);
+    constexpr bool MGR = (MODE == MODE_MGR);
+    constexpr bool AXE = (MODE == MODE_AX || MODE == MODE_MGR);   // epilogue with A = M + c S
     if (MODE != MODE_PLAIN && ctrl->all_done) return;
     extern __shared__ __align__(128) unsigned char smem[];
     int32_t* sdesc = reinterpret_cast<int32_t*>(smem + SM::off_desc);   // [4][16] tile descriptors (ring)
@@ -358,13 +375,15 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             bulk_load(st + SM::off_col, m.lcol + ti.cp_first, (uint32_t)ti.slots * 4u, bar);
         }
     };
+    double2 hd[MGR ? HPT : 1];   // MGR: (S_vv, A_v) of the halo rows in flight
     auto load_halo = [&](const int (&idx)[HPT], int nh, double2 (&h0)[HPT], double2 (&h1)[HPT]) {
 #pragma unroll
         for (int i = 0; i < HPT; ++i) {
             if (rg + i * ROWS < nh) {
                 const int64_t j = idx[i];
                 h0[i] = ld2(a.in0, j * K + 2 * l);
-                if (CG_A) h1[i] = ld2(a.in1, j * K + 2 * l);
+                if (CG_A || MGR) h1[i] = ld2(a.in1, j * K + 2 * l);
+                if (MGR) hd[MGR ? i : 0] = make_double2(m.sdiag[j], m.area[j]);
             }
         }
     };
@@ -396,6 +415,11 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             if (hh < nh) {
                 double2 g = h0[i];
                 if (CG_A) { g.x = fma(beta.x, h1[i].x, g.x); g.y = fma(beta.y, h1[i].y, g.y); }
+                if (MGR) {   // e = omega (r - alpha q) / d of the halo row
+                    const double2 dd = hd[MGR ? i : 0];
+                    g.x = a.omega * fma(-alpha.x, h1[i].x, g.x) * rcp_pos(fma(cc.x, dd.x, dd.y));
+                    g.y = a.omega * fma(-alpha.y, h1[i].y, g.y) * rcp_pos(fma(cc.y, dd.x, dd.y));
+                }
                 sa[(T + hh) * TPR + l] = g;
             }
         }
@@ -418,6 +442,28 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 xv[i].y = fma(alpha.y, pv.y, xv[i].y);
                 sa[e] = own;
                 st2(a.x, row0 * K + 2 * (int64_t)e, xv[i]);
+            }
+        }
+    };
+    // MGR: r' = r - alpha q over the q tile, e = omega r'/d over the r tile
+    auto elementwise_mgr = [&](unsigned char* st, int64_t tile) {
+        double2* sa = reinterpret_cast<double2*>(st);
+        double2* sb = reinterpret_cast<double2*>(st + SM::off_b);
+        const double* sdg = reinterpret_cast<const double*>(st + SM::off_dg);
+        const double* sar = reinterpret_cast<const double*>(st + SM::off_ar);
+        const int nrows = (int)min((int64_t)T, m.nv - tile * T);
+#pragma unroll
+        for (int i = 0; i < XPT; ++i) {
+            const int e = tid + i * NT;
+            if (e < nrows * TPR) {
+                const int rr = e / TPR;
+                const double2 rv = sa[e], qv = sb[e];
+                const double sd = sdg[rr], av = sar[rr];
+                double2 rn;
+                rn.x = fma(-alpha.x, qv.x, rv.x);
+                rn.y = fma(-alpha.y, qv.y, rv.y);
+                sb[e] = rn;
+                sa[e] = make_double2(a.omega * rn.x * rcp_pos(fma(cc.x, sd, av)), a.omega * rn.y * rcp_pos(fma(cc.y, sd, av)));
             }
         }
     };
@@ -459,6 +505,10 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             load_x(tile0 + G, xv);
             fence_proxy_async();
         }
+        if (MGR) {
+            elementwise_mgr(smem, tile0);
+            fence_proxy_async();
+        }
     }
     double2 acc[MODE == MODE_AX ? 2 : 1] = {};
     int64_t tile = tile0;
@@ -483,8 +533,9 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             const int64_t t2 = tile + LA * G;
             bulk_wait_read0();   // the stage of tile it-1 is free once its bulk store has been read
             if (t2 < ntiles) issue(t2, (int)((it + LA) % NS), tq);
-            if (CG_A) {
+            if (CG_A || MGR) {
                 bulk_store(a.out1 + row0 * K, sa, (uint32_t)nrows * K * sizeof(double));
+                if (MGR) bulk_store(a.x + row0 * K, sb, (uint32_t)nrows * K * sizeof(double));
                 bulk_commit();
             }
             if (t2 + G < ntiles) tq = load_issue(m.tile_desc, t2 + G);
@@ -527,6 +578,12 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                             const double2 p0 = ld2(a.in1, (int64_t)cj.x * K + 2 * l);
                             g0.x = fma(beta.x, p0.x, g0.x); g0.y = fma(beta.y, p0.y, g0.y);
                         }
+                        if (MGR) {
+                            const double2 p0 = ld2(a.in1, (int64_t)cj.x * K + 2 * l);
+                            const double sj = m.sdiag[cj.x], aj = m.area[cj.x];
+                            g0.x = a.omega * fma(-alpha.x, p0.x, g0.x) * rcp_pos(fma(cc.x, sj, aj));
+                            g0.y = a.omega * fma(-alpha.y, p0.y, g0.y) * rcp_pos(fma(cc.y, sj, aj));
+                        }
                     }
                     if (j1 < (unsigned)nrows) {
                         g1 = sa[j1 * TPR + l];
@@ -535,6 +592,12 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                         if (CG_A) {
                             const double2 p1 = ld2(a.in1, (int64_t)cj.y * K + 2 * l);
                             g1.x = fma(beta.x, p1.x, g1.x); g1.y = fma(beta.y, p1.y, g1.y);
+                        }
+                        if (MGR) {
+                            const double2 p1 = ld2(a.in1, (int64_t)cj.y * K + 2 * l);
+                            const double sj = m.sdiag[cj.y], aj = m.area[cj.y];
+                            g1.x = a.omega * fma(-alpha.x, p1.x, g1.x) * rcp_pos(fma(cc.x, sj, aj));
+                            g1.y = a.omega * fma(-alpha.y, p1.y, g1.y) * rcp_pos(fma(cc.y, sj, aj));
                         }
                     }
                     s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
@@ -552,15 +615,18 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 const double ia = sar[r];
                 s.x *= ia; s.y *= ia;            // t = M^-1 S p'
                 st2(a.out0, ri, s);
-            } else if (MODE == MODE_AX) {
+            } else if (AXE) {
+                const int sub = MGR ? 1 : a.scale_inv_area;
                 const double av = sar[r];
                 double2 o = {fma(cc.x, s.x, av * own.x), fma(cc.y, s.y, av * own.y)};   // A v
-                if (a.scale_inv_area >= 1) {
+                if (sub >= 1) {
                     const double2 rv = sb[r * TPR + l];
                     o.x = rv.x - o.x; o.y = rv.y - o.y;                                  // r - A v
-                    if (a.scale_inv_area >= 2) {
-                        o.x = fma(a.omega * o.x, 1.0 / fma(cc.x, sd, av), own.x);
-                        o.y = fma(a.omega * o.y, 1.0 / fma(cc.y, sd, av), own.y);
+                    if (sub >= 2) {
+                        // (rcp_pos as in the first sweep: the same D^-1 on both sides of the cycle, and a fifth of
+                        // this kernel's instructions less than two fp64 divisions)
+                        o.x = fma(a.omega * o.x, rcp_pos(fma(cc.x, sd, av)), own.x);
+                        o.y = fma(a.omega * o.y, rcp_pos(fma(cc.y, sd, av)), own.y);
                         acc[0].x = fma(rv.x, o.x, acc[0].x);  acc[0].y = fma(rv.y, o.y, acc[0].y);     // r.z
                         acc[MODE == MODE_AX ? 1 : 0].x = fma(rv.x, rv.x, acc[MODE == MODE_AX ? 1 : 0].x);
                         acc[MODE == MODE_AX ? 1 : 0].y = fma(rv.y, rv.y, acc[MODE == MODE_AX ? 1 : 0].y);
@@ -593,9 +659,13 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 load_x(tile + 2 * G, xv);
                 fence_proxy_async();
             }
+            if (MGR) {
+                elementwise_mgr(st1, tile + G);
+                fence_proxy_async();
+            }
         }
     }
-    if (CG_A && tid == 0) bulk_wait0();
+    if ((CG_A || MGR) && tid == 0) bulk_wait0();
     if (MODE == MODE_CG1 || MODE == MODE_CG2B) {
         __shared__ double tot[KMAX];
         const double2 acc1[1] = {acc[0]};
@@ -694,17 +764,6 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
 }
 
 // ------------------------------------------------------------------------------------------- kernel B
-// 1/d for d > 0 in the normal range: hardware seed (2^-23) and two Newton steps (full fp64 precision, ~1 ulp).
-// A fp64 division costs about five times as many instructions and made this streaming kernel issue-bound.
-__device__ __forceinline__ double rcp_pos(double d) {
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
-    double e = fma(-d, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-d, r, 1.0);
-    return fma(r, e, r);
-}
-
 // z -= alpha q/d ; rho' = sum d z^2 ; ||r||^2 = sum (d z)^2 ; then (last block) beta, stop tests.
 // Pure streaming: every thread keeps U = 8 rows (16 independent 16-byte loads) in flight, two blocks per SM --
 // measured on B200 this reaches the copy bandwidth, while more resident warps with fewer loads each do not.

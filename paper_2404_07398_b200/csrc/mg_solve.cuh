@@ -7,8 +7,8 @@
 //   column with its own c, alpha, beta and stop time.  As in the Jacobi path all CG scalars live in the device
 //   control block: the iteration is
 //       k_spmm<16, CG1>      p' = z + beta p ; x += alpha p ; q = A p' ; alpha' = rho / p'.q         (kernel A)
-//       k_mg_rupdate         r -= alpha' q ; e = omega r / d                     (first sweep of B on level 0)
-//       k_spmm<16, AX> sub 1 residual, then restriction, the coarse levels, prolongation
+//       k_spmm<16, MGR>      r' = r - alpha' q ; e = omega r'/d ; t = r' - A e     (residual update, first sweep of B
+//                            on level 0 and its residual in one pass), then restriction, coarse levels, prolongation
 //       k_spmm<16, AX> sub 3 z = last sweep ; rho' = r.z ; ||r||^2 ; beta ; stop test        (CG bookkeeping)
 //   and the host reads the control block once per iteration to see whether every column has stopped.
 // The stop test is the same as in the Jacobi path: recursive ||r||_2 <= tol ||M phi||_2.
@@ -208,36 +208,6 @@ __global__ void __launch_bounds__(BLOCK) k_mg_mass(const double* __restrict__ ar
     const double2 xv = ld2(x, 2 * i);
     st2(out, 2 * i, make_double2(av * xv.x, av * xv.y));
 }
-// r -= alpha q (alpha from the control block) ; e = omega r / d : the residual update of CG and the first Jacobi
-// sweep (from a zero guess) of the preconditioner on level 0 in one pass
-__global__ void __launch_bounds__(BLOCK, 2) k_mg_rupdate(MgMat g, const Ctrl* __restrict__ ctrl, double* __restrict__ r,
-                                                         const double* __restrict__ q, double* __restrict__ e) {
-    constexpr int TPR = MGK / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    constexpr int U = 4;
-    const int l = threadIdx.x % TPR;
-    const double2 cc = ld2(ctrl->c, 2 * l), al = ld2(ctrl->alpha, 2 * l);
-    const int64_t stride = (int64_t)gridDim.x * ROWS;
-    for (int64_t base = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; base < g.n; base += U * stride) {
-        double2 rv[U], qv[U], dv[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int64_t row = base + u * stride;
-            if (row < g.n) { rv[u] = ld2(r, row * MGK + 2 * l); qv[u] = ld2(q, row * MGK + 2 * l); dv[u] = g.diag[row]; }
-        }
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int64_t row = base + u * stride;
-            if (row < g.n) {
-                rv[u].x = fma(-al.x, qv[u].x, rv[u].x);
-                rv[u].y = fma(-al.y, qv[u].y, rv[u].y);
-                st2(r, row * MGK + 2 * l, rv[u]);
-                st2(e, row * MGK + 2 * l, make_double2(g.omega * rv[u].x * rcp_pos(fma(cc.x, dv[u].x, dv[u].y)),
-                                                       g.omega * rv[u].y * rcp_pos(fma(cc.y, dv[u].x, dv[u].y))));
-            }
-        }
-    }
-}
 // per-block partial sums of a.b and a.c per column (fixed order); k_mg_dot_final adds the blocks in order
 __global__ void __launch_bounds__(BLOCK) k_mg_dot(int64_t n, const double* __restrict__ a, const double* __restrict__ b,
                                                   const double* __restrict__ c, double* __restrict__ partials) {
@@ -273,7 +243,7 @@ __global__ void k_mg_dot_final(const double* __restrict__ partials, int nblocks,
 
 // ------------------------------------------------------------------------------------------- host side
 struct MgBuffers {
-    double *x, *r, *p[2], *q, *za, *zb;         // level 0, [n][16]
+    double *x, *r[2], *p[2], *q, *za, *zb, *t;  // level 0, [n][16]; r is double-buffered (k_spmm<16, MGR>)
     double* lev[MG_MAX_LEVELS][4];              // levels >= 1: R, E, T, E2
     double* partials;                           // [grid][2][16]
     double* dots;                               // [32]
@@ -283,7 +253,7 @@ struct MgBuffers {
 
 inline size_t mg_extra_bytes(const if_mesh_s* h) {
     if (h->mg_levels < 2) return 0;
-    size_t b = 2 * align_up((size_t)h->n_vert * MGK * sizeof(double));        // za, zb (level-0 vectors 6 and 7)
+    size_t b = 4 * align_up((size_t)h->n_vert * MGK * sizeof(double));        // za, zb, t, second r (level-0 vectors 6 to 9)
     for (int l = 1; l < h->mg_levels; ++l) b += 4 * align_up((size_t)h->mg[l].n * MGK * sizeof(double));
     b += align_up((size_t)h->n_sm * 4 * 2 * MGK * sizeof(double)) + align_up(2 * MGK * sizeof(double));
     return b;
@@ -291,12 +261,14 @@ inline size_t mg_extra_bytes(const if_mesh_s* h) {
 
 inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) {
     MgBuffers m{};
-    m.x = w.x; m.r = w.z; m.p[0] = w.p0; m.p[1] = w.p1; m.q = w.q;
+    m.x = w.x; m.r[0] = w.z; m.p[0] = w.p0; m.p[1] = w.p1; m.q = w.q;
     char* p = static_cast<char*>(extra);
     size_t off = 0;
     auto take = [&](size_t bytes) { void* r = p + off; off += align_up(bytes); return r; };
     m.za = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
     m.zb = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
+    m.t = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
+    m.r[1] = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
     for (int l = 1; l < h->mg_levels; ++l)
         for (int k = 0; k < 4; ++k) m.lev[l][k] = (double*)take((size_t)h->mg[l].n * MGK * sizeof(double));
     m.dot_grid = h->n_sm * 4;
@@ -314,8 +286,9 @@ inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
 // One V cycle on level l: e = B_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
 // nu = 1 on level 0 and MG_NU_COARSE below it.  R holds r and is not changed; E, T, E2 are work buffers of the
 // level; *result is the one that holds e.
-// On level 0 the caller may have done the first sweep already (first_done: E = omega r / d) and chooses the
-// sub-mode of the last sweep (final_sub 3 / 4: with the CG bookkeeping, see kernels.cuh).
+// On level 0 the caller may have done the first sweep and its residual already (first_done: E = omega r / d,
+// T = r - A E, both by k_spmm<16, MGR>) and chooses the sub-mode of the last sweep (final_sub 3 / 4: with the CG
+// bookkeeping, see kernels.cuh).
 int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double* R, double* E, double* T, double* E2,
               double** result, int final_sub = 2, bool first_done = false) {
     const if_mesh_s* h = r.h;
@@ -349,7 +322,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
         return IF_OK;
     };
     // a coarsest level too large for the dense solve (coarsening stalled): smoothing only
-    const int nu = last ? 4 * MG_NU_COARSE : (l == 0 ? 1 : MG_NU_COARSE);
+    const int nu = last ? 4 * MG_NU_COARSE : (l == 0 ? 1 : (l == 1 ? MG_NU_L1 : MG_NU_COARSE));
     int rc;
     double* cur = E;
     double* spare[2] = {E2, T};
@@ -362,7 +335,8 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
         std::swap(cur, spare[0]);
     }
     if (last) { *result = cur; return IF_OK; }
-    if ((rc = apply(1, cur, spare[1]))) return rc;                    // residual of the level
+    if (!(l == 0 && first_done && nu == 1))
+        if ((rc = apply(1, cur, spare[1]))) return rc;                // residual of the level
     double* const* nb = b.lev[l + 1];
     const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse, wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
     if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, spare[1], nb[0]);
@@ -423,13 +397,15 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
     const unsigned eg = (unsigned)((nv * MGK + BLOCK - 1) / BLOCK);
     const unsigned vg = (unsigned)((nv * (MGK / 2) + BLOCK - 1) / BLOCK);
     const MgMat g0 = mg_mat(h->mg[0]);
-    const int ru_grid = (int)std::max<int64_t>(1, std::min<int64_t>((nv + 15) / 16, (int64_t)h->n_sm * 8));
     k_ingest<MGK><<<eg, BLOCK, 0, r.st>>>(r.m, sp, 0xffffu, d_fields, b.x);
     IF_LAUNCH_CHECK();
     k_mg_mass<<<vg, BLOCK, 0, r.st>>>(h->area, nv, b.x, b.za);               // b = M phi
     IF_LAUNCH_CHECK();
+    int mgr_grid = 0;
+    if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &mgr_grid,
+                            SpmmCfg<MGK>::NT))) return rc;
     {
-        SpmmArgs a{b.x, b.za, nullptr, b.r, nullptr, 1, 0, 0.0};              // r = b - A x0
+        SpmmArgs a{b.x, b.za, nullptr, b.r[0], nullptr, 1, 0, 0.0};           // r = b - A x0
         if ((rc = launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a))) return rc;
     }
     IF_CUDA_TRY(cudaMemsetAsync(b.p[0], 0, (size_t)nv * MGK * sizeof(double), r.st));
@@ -442,7 +418,7 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
     }
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
     double* z = nullptr;
-    if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z, 4, false))) return rc;
+    if ((rc = mg_vcycle(r, b, cs, 0, b.r[0], b.za, b.t, b.zb, &z, 4, false))) return rc;
     int* h_flag = reinterpret_cast<int*>(h_dots);
     auto all_done = [&](bool* out) -> int {
         IF_CUDA_TRY(cudaMemcpyAsync(h_flag, &r.w.ctrl->all_done, sizeof(int), cudaMemcpyDeviceToHost, r.st));
@@ -453,20 +429,26 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
     bool stop = false;
     if ((rc = all_done(&stop))) return rc;
     int64_t loops = 0;
-    int cur = 0;
+    int cur = 0, cr = 0;
     while (!stop) {
         {
             SpmmArgs a{z, b.p[cur], b.x, b.q, b.p[cur ^ 1], 0, cur ^ 1, 0.0};  // kernel A of the Jacobi path
             if ((rc = launch_spmm<MGK, MODE_CG1>(r, cg_grid, a))) return rc;
         }
         cur ^= 1;
-        k_mg_rupdate<<<ru_grid, BLOCK, 0, r.st>>>(g0, r.w.ctrl, b.r, b.q, b.za);
-        IF_LAUNCH_CHECK();
-        if ((rc = mg_vcycle(r, b, cs, 0, b.r, b.za, b.q, b.zb, &z, 3, true))) return rc;
+        {
+            SpmmArgs a{b.r[cr], b.q, b.r[cr ^ 1], b.t, b.za, 0, 0, g0.omega};
+            if ((rc = launch_spmm<MGK, MODE_MGR>(r, mgr_grid, a))) return rc;
+        }
+        cr ^= 1;
+        if ((rc = mg_vcycle(r, b, cs, 0, b.r[cr], b.za, b.t, b.zb, &z, 3, true))) return rc;
         ++loops;
         if ((rc = all_done(&stop))) return rc;
     }
     *iters_total += loops;
+    if (getenv("IF_VERBOSE"))
+        fprintf(stderr, "[implicit_filter] multigrid batch: largest scale %.4g, %zu columns, %lld iterations\n",
+                rhs[first].ell, count, (long long)loops);
     // the columns are finalised from the device control block (pending alpha p included, as in the Jacobi path)
     Run fr = r;
     fr.w.x = b.x;

@@ -385,6 +385,40 @@ def test_multigrid_on_disconnected_and_degenerate_inputs(ifl, oracle_mod):
     h.close()
 
 
+def test_multigrid_fused_residual_kernel_on_unstaged_tiles(ifl, oracle_mod):
+    """k_spmm<16, MGR> (r' = r - alpha q, e = omega r'/d, t = r' - A e in one pass) has two gather paths: tiles whose
+    halo fits the shared-memory stage and tiles that read their out-of-tile rows from global memory.  A shuffled
+    vertex order kept as it is (sfc_kind = 1) makes every tile of the second kind; both orders must give the oracle's
+    fields, and the iteration counts may differ only by what another summation order moves a stop."""
+    w = SMALL["cfg4_L5"]()
+    V = w.mesh.n_vert
+    rng = np.random.default_rng(11)
+    new_of_old = rng.permutation(V)
+    coords = np.empty_like(w.mesh.coords)
+    coords[new_of_old] = w.mesh.coords
+    tri = new_of_old[w.mesh.tri].astype(np.int32)
+    fields = np.empty_like(w.fields)
+    fields[:, new_of_old] = w.fields
+    ells = w.ells[-3:]
+    om = oracle_mod.OracleMesh(coords, tri, None)
+    h_sfc = ifl.if_prepare(coords, tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    h_raw = ifl.if_prepare(coords, tri, None, flags=ifl.IF_FLAG_MULTIGRID, sfc_kind=1)
+    # (the ragged last tile has few rows and may still fit)
+    assert h_raw.unstaged_tiles >= h_raw.n_tiles - 1 and h_sfc.unstaged_tiles < h_sfc.n_tiles // 2
+    a, sa = ifl.if_filter(h_sfc, fields, ells, 1, solver=1, mg_min_ell=1.0)
+    b, sb = ifl.if_filter(h_raw, fields, ells, 1, solver=1, mg_min_ell=1.0)
+    jac, sj = ifl.if_filter(h_raw, fields, ells, 1)
+    assert sa["code"] == 0 and sb["code"] == 0
+    assert sb["iters"].sum() < sj["iters"].sum()          # the multigrid path did run
+    a, b = a.cpu().numpy(), b.cpu().numpy()
+    for f in range(fields.shape[0]):
+        for j, ell in enumerate(ells):
+            x, info = om.solve(fields[f], float(ell), 1)
+            assert info["status"] == 0
+            assert rel(a[f, j], x) <= TOL_FIELD and rel(b[f, j], x) <= TOL_FIELD, (f, j)
+    h_sfc.close(); h_raw.close()
+
+
 def test_multigrid_hierarchy_survives_save_and_load(ifl, tmp_path):
     """if_save / if_load of a handle prepared with IF_FLAG_MULTIGRID: the loaded handle solves with solver = 1 and
     gives the same iteration counts and bits (the hierarchy is rebuilt deterministically on load)."""
