@@ -68,11 +68,28 @@ void mg_free(if_mesh_s* h);
 // the pair (S_l, M_l) on one sparsity pattern, so that A_l = M_l + c S_l is applied matrix-free for any scale.
 constexpr int MG_MAX_LEVELS = 12;
 constexpr int MG_COARSEST = 64;    // the hierarchy stops at a level with at most this many unknowns (dense solve)
+// Cycle and aggregation parameters (macros: the tuning runs of DESIGN.md section 9b rebuild with -DIF_MG_...).
+#ifndef IF_MG_THETA
+#define IF_MG_THETA 0.08
+#endif
+#ifndef IF_MG_NU_L1
+#define IF_MG_NU_L1 1
+#endif
+#ifndef IF_MG_NU_COARSE
+#define IF_MG_NU_COARSE 2
+#endif
+// strength of connection for the aggregates: |S_ij| >= theta sqrt(S_ii S_jj); 0 = the whole graph
+constexpr double MG_THETA = IF_MG_THETA;
+// a level whose strong graph coarsens by less than this uses the whole graph (small aggregates + a prolongator
+// smoothed with the whole matrix = fill-in on the next level)
+constexpr double MG_MIN_COARSENING = 6.0;
 constexpr double MG_OMEGA_MAX = 0.9;   // Jacobi damping of the smoother, lowered where rho(D^-1 S) is large
-constexpr int MG_NU_L1 = 2;        // smoothing sweeps before and after the coarse correction on level 1 (a ninth of
-                                   // the mesh: its sweeps are a fifth of the cycle), MG_NU_COARSE on levels >= 2
-constexpr int MG_NU_COARSE = 4;    // (cheap); level 0, where a sweep costs a pass over the mesh, does one.  Measured
-                                   // on config 4: (3, 3) 1.207 s, (2, 3) 1.133 s, (2, 4) 1.104 s, (1, 3) 1.176 s
+// smoothing sweeps before and after the coarse correction: one on level 0 (a sweep there is a pass over the mesh),
+// MG_NU_L1 on level 1 (an eighth of the mesh: its sweeps are a fifth of the cycle), MG_NU_COARSE below (cheap).
+// Config 4, whole spectrum: with theta = 0.08 (1, 1) 0.925 s, (1, 2) 0.932 s, (2, 2) 0.981 s, (2, 4) 1.031 s;
+// with theta = 0 (2, 4) 1.072 s, (3, 3) 1.18 s, (1, 3) 1.15 s.
+constexpr int MG_NU_L1 = IF_MG_NU_L1;
+constexpr int MG_NU_COARSE = IF_MG_NU_COARSE;
 struct MgLevel {
     int64_t n = 0, nnz = 0;
     double rho = 2.0;            // estimate of rho(D_S^-1 S) (power iteration, with a safety factor)

@@ -309,42 +309,87 @@ int spectral_radius(const MgLevel& f, double* rho, cudaStream_t st) {
     return IF_OK;
 }
 
+// strength of connection: keep[k] = 1 for the diagonal and for the entries with S_ij^2 >= theta^2 S_ii S_jj
+__global__ void k_mg_strong(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                            const double2* __restrict__ sm, const double2* __restrict__ diag, double theta2, int64_t n,
+                            uint8_t* __restrict__ keep) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double sii = diag[i].x;
+    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+        const int32_t j = col[k];
+        const double sij = sm[k].x;
+        keep[k] = (j == i || sij * sij >= theta2 * sii * diag[j].x) ? 1 : 0;
+    }
+}
+
 // Greedy aggregation over the graph of the level's matrix, serial in row order (host).  agg[i] = aggregate of row
 // i, numbered in the order of their roots, so the coarse numbering follows the fine one along the curve.
+// The graph is that of the strong connections (MG_THETA): weak ones -- across a sliver, or the small entries the
+// Galerkin products accumulate on the coarse levels -- do not pull a row into an aggregate.  Should the filtered
+// graph coarsen by less than MG_MIN_COARSENING (the prolongator is smoothed with the whole matrix, so small
+// aggregates mean fill-in on the next level), the level falls back to the whole graph.
 int aggregate_rows(const MgLevel& f, DBuf& d_agg, int64_t* n_agg, cudaStream_t st) {
     const int64_t n = f.n;
-    std::vector<int64_t> rp;
-    std::vector<int32_t> cj, agg;
+    std::vector<int64_t> rp, rps;
+    std::vector<int32_t> cj, cjs, agg;
+    std::vector<uint8_t> keep;
     try {
         rp.resize((size_t)n + 1);
         cj.resize((size_t)f.nnz);
-        agg.assign((size_t)n, -1);
+        if (MG_THETA > 0.0) { keep.resize((size_t)f.nnz); rps.resize((size_t)n + 1); cjs.reserve((size_t)f.nnz); }
     } catch (const std::bad_alloc&) { return IF_ENOMEM; }
     IF_CUDA_TRY(cudaMemcpyAsync(rp.data(), f.rowptr, (size_t)(n + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
     IF_CUDA_TRY(cudaMemcpyAsync(cj.data(), f.col, (size_t)f.nnz * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    if (MG_THETA > 0.0) {
+        DBuf d_keep;
+        IF_CUDA_TRY(d_keep.alloc((size_t)f.nnz));
+        k_mg_strong<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, MG_THETA * MG_THETA, n, d_keep.as<uint8_t>());
+        IF_LAUNCH_CHECK();
+        IF_CUDA_TRY(cudaMemcpyAsync(keep.data(), d_keep.p, (size_t)f.nnz, cudaMemcpyDeviceToHost, st));
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        for (int64_t i = 0; i < n; ++i) {
+            rps[(size_t)i] = (int64_t)cjs.size();
+            for (int64_t k = rp[i]; k < rp[i + 1]; ++k)
+                if (keep[(size_t)k]) cjs.push_back(cj[(size_t)k]);
+        }
+        rps[(size_t)n] = (int64_t)cjs.size();
+    }
     IF_CUDA_TRY(cudaStreamSynchronize(st));
-    int32_t na = 0;
-    // pass 1: roots
-    for (int64_t i = 0; i < n; ++i) {
-        if (agg[i] >= 0) continue;
-        bool all_free = true;
-        for (int64_t k = rp[i]; k < rp[i + 1] && all_free; ++k) all_free = agg[cj[k]] < 0;
-        if (!all_free) continue;
-        for (int64_t k = rp[i]; k < rp[i + 1]; ++k) agg[cj[k]] = na;
-        agg[i] = na++;
-    }
-    // pass 2: a leftover joins the aggregate (as of pass 1) of its first aggregated neighbour; joined rows are
-    // marked -2 - a until the end of the pass so that leftovers do not chain onto each other
-    for (int64_t i = 0; i < n; ++i) {
-        if (agg[i] != -1) continue;
-        for (int64_t k = rp[i]; k < rp[i + 1]; ++k)
-            if (agg[cj[k]] >= 0) { agg[i] = -2 - agg[cj[k]]; break; }
-    }
-    // pass 3: what is still free (possible only in a component without a root) becomes its own aggregate
-    for (int64_t i = 0; i < n; ++i) {
-        if (agg[i] <= -2) agg[i] = -2 - agg[i];
-        else if (agg[i] == -1) agg[i] = na++;
-    }
+    auto greedy = [&](const std::vector<int64_t>& rp, const std::vector<int32_t>& cj) -> int32_t {
+        agg.assign((size_t)n, -1);
+        int32_t na = 0;
+        // pass 1: roots
+        for (int64_t i = 0; i < n; ++i) {
+            if (agg[i] >= 0) continue;
+            bool all_free = true;
+            for (int64_t k = rp[i]; k < rp[i + 1] && all_free; ++k) all_free = agg[cj[k]] < 0;
+            if (!all_free) continue;
+            for (int64_t k = rp[i]; k < rp[i + 1]; ++k) agg[cj[k]] = na;
+            agg[i] = na++;
+        }
+        // pass 2: a leftover joins the aggregate (as of pass 1) of its first aggregated neighbour; joined rows are
+        // marked -2 - a until the end of the pass so that leftovers do not chain onto each other
+        for (int64_t i = 0; i < n; ++i) {
+            if (agg[i] != -1) continue;
+            for (int64_t k = rp[i]; k < rp[i + 1]; ++k)
+                if (agg[cj[k]] >= 0) { agg[i] = -2 - agg[cj[k]]; break; }
+        }
+        // pass 3: what is still free (possible only in a component without a root) becomes its own aggregate
+        for (int64_t i = 0; i < n; ++i) {
+            if (agg[i] <= -2) agg[i] = -2 - agg[i];
+            else if (agg[i] == -1) agg[i] = na++;
+        }
+        return na;
+    };
+    int32_t na = -1;
+    try {
+        if (MG_THETA > 0.0) {
+            na = greedy(rps, cjs);
+            if ((double)na * MG_MIN_COARSENING > (double)n) na = -1;
+        }
+        if (na < 0) na = greedy(rp, cj);
+    } catch (const std::bad_alloc&) { return IF_ENOMEM; }
     IF_CUDA_TRY(d_agg.alloc((size_t)n * sizeof(int32_t)));
     IF_CUDA_TRY(cudaMemcpyAsync(d_agg.p, agg.data(), (size_t)n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     IF_CUDA_TRY(cudaStreamSynchronize(st));
