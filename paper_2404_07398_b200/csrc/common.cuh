@@ -93,7 +93,8 @@ constexpr int MG_NU_COARSE = IF_MG_NU_COARSE;
 struct MgLevel {
     int64_t n = 0, nnz = 0;
     double rho = 2.0;            // estimate of rho(D_S^-1 S) (power iteration, with a safety factor)
-    double omega = 0.7;          // Jacobi damping of the smoother on this level: min(MG_OMEGA_MAX, 1.6 / rho)
+    double rho_m = 1.0;          // the same for D_M^-1 M (1 on the mesh, where M is diagonal)
+    double omega = 0.7;          // Jacobi damping of the smoother on this level: min(MG_OMEGA_MAX, 1.6 / max(rho, rho_m))
     int64_t* rowptr = nullptr;   // [n+1]
     int32_t* col = nullptr;      // [nnz]
     double2* sm = nullptr;       // [nnz]  (S_ij, M_ij)

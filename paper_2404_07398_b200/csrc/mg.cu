@@ -2,9 +2,9 @@
 // loss of convergence of plain CG at large l are the paper's stated open problem).
 //
 // Smoothed aggregation on the internal (space-filling-curve) row order:
-//   aggregates      greedy over the graph of S, in row order: a row whose neighbours are all free becomes a root
-//                   and takes them; leftovers join a neighbouring aggregate (tentative prolongator P_t: piecewise
-//                   constant).  Graph aggregates never join two connected components of the masked mesh, which
+//   aggregates      greedy over the graph of the strong connections of S (|S_ij| >= MG_THETA sqrt(S_ii S_jj)), in
+//                   row order: a row whose neighbours are all free becomes a root and takes them; leftovers join a
+//                   neighbouring aggregate (tentative prolongator P_t: piecewise constant).  Graph aggregates never join two connected components of the masked mesh, which
 //                   blocks of consecutive rows did; it is a serial sweep and runs on the host (once per mesh).
 //   prolongator     P = (I - omega_p D_S^-1 S) P_t, omega_p = 4 / (3 rho(D_S^-1 S)), rho by power iteration
 //                   (smoothed with the stiffness only, so P does not depend on the scale)
@@ -246,7 +246,7 @@ int exclusive_scan(int64_t* d_in, int64_t* d_out, int64_t n, int64_t* total, cud
     return IF_OK;
 }
 
-// power iteration on D_S^-1 S: y = D_S^-1 S x, sq = y^2 ;  x = y / ||y||
+// power iteration on D_S^-1 S (part 0) or D_M^-1 M (part 1): y = D^-1 B x, sq = y^2 ;  x = y / ||y||
 __global__ void k_mg_power_start(int64_t n, double* __restrict__ x) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -257,13 +257,13 @@ __global__ void k_mg_power_start(int64_t n, double* __restrict__ x) {
     x[i] = (double)(z >> 11) * (2.0 / 9007199254740992.0) - 1.0;
 }
 __global__ void k_mg_power_apply(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
-                                 const double2* __restrict__ sm, const double2* __restrict__ diag, int64_t n,
+                                 const double2* __restrict__ sm, const double2* __restrict__ diag, int part, int64_t n,
                                  const double* __restrict__ x, double* __restrict__ y, double* __restrict__ sq) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double s = 0.0;
-    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) s = fma(sm[k].x, x[col[k]], s);
-    const double d = diag[i].x;
+    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) s = fma(part ? sm[k].y : sm[k].x, x[col[k]], s);
+    const double d = part ? diag[i].y : diag[i].x;
     s = d > 0.0 ? s / d : 0.0;
     y[i] = s;
     sq[i] = s * s;
@@ -276,9 +276,11 @@ __global__ void k_mg_power_scale(int64_t n, const double* __restrict__ y, const 
     x[i] = nrm > 0.0 ? y[i] / nrm : 0.0;
 }
 
-// rho(D_S^-1 S) of a level (>= 1 is returned: the bound used for the damping must cover the mass part, whose
-// Jacobi-scaled spectrum lies near 1)
-int spectral_radius(const MgLevel& f, double* rho, cudaStream_t st) {
+// rho(D_S^-1 S) (part 0) or rho(D_M^-1 M) (part 1) of a level; >= 1 is returned.  The mass part is diagonal on the
+// mesh (rho = 1) but not below it: M_l = P^T M P has positive off-diagonal entries and its Jacobi-scaled spectrum
+// reaches 2-3, with the smooth vectors on top -- the damping of the smoother must cover both parts, since the
+// Rayleigh quotients of D^-1 (M_l + c S_l) lie between those of the two parts for every c.
+int spectral_radius(const MgLevel& f, int part, double* rho, cudaStream_t st) {
     const int64_t n = f.n;
     DBuf x, y, sq, sum, tmp;
     IF_CUDA_TRY(x.alloc((size_t)n * sizeof(double)));
@@ -296,7 +298,7 @@ int spectral_radius(const MgLevel& f, double* rho, cudaStream_t st) {
     for (int it = 0; it < MG_POWER_ITERS; ++it) {
         k_mg_power_scale<<<gridf(n), 256, 0, st>>>(n, y.as<double>(), sum.as<double>(), x.as<double>());
         IF_LAUNCH_CHECK();
-        k_mg_power_apply<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, n, x.as<double>(), y.as<double>(),
+        k_mg_power_apply<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, part, n, x.as<double>(), y.as<double>(),
                                                   sq.as<double>());
         IF_LAUNCH_CHECK();
         IF_CUDA_TRY(cub::DeviceReduce::Sum(tmp.p, tb, sq.as<double>(), sum.as<double>(), n, st));
@@ -544,9 +546,10 @@ int mg_build(if_mesh_s* h) {
     int L = 1;
     for (;;) {
         MgLevel& g = h->mg[L - 1];
-        int rc = spectral_radius(g, &g.rho, st);
+        int rc = spectral_radius(g, 0, &g.rho, st);
+        if (rc == IF_OK && L > 1) rc = spectral_radius(g, 1, &g.rho_m, st);
         if (rc != IF_OK) { mg_free(h); return rc; }
-        g.omega = std::min(MG_OMEGA_MAX, 1.6 / g.rho);
+        g.omega = std::min(MG_OMEGA_MAX, 1.6 / std::max(g.rho, g.rho_m));
         if (g.n <= MG_COARSEST || L >= MG_MAX_LEVELS) break;
         rc = build_next_level(g, h->mg[L], st);
         if (rc != IF_OK) { mg_free(h); return rc; }
@@ -556,9 +559,10 @@ int mg_build(if_mesh_s* h) {
     h->mg_levels = L;
     if (getenv("IF_VERBOSE"))
         for (int l = 0; l < L; ++l)
-            fprintf(stderr, "[implicit_filter] multigrid level %d: %lld rows, %.1f entries per row, rho %.3f, omega %.3f, "
-                            "P %.1f entries per row\n", l, (long long)h->mg[l].n, (double)h->mg[l].nnz / (double)h->mg[l].n,
-                    h->mg[l].rho, h->mg[l].omega, h->mg[l].n ? (double)h->mg[l].p_nnz / (double)h->mg[l].n : 0.0);
+            fprintf(stderr, "[implicit_filter] multigrid level %d: %lld rows, %.1f entries per row, rho(S) %.3f, rho(M) %.3f, "
+                            "omega %.3f, P %.1f entries per row\n", l, (long long)h->mg[l].n,
+                    (double)h->mg[l].nnz / (double)h->mg[l].n, h->mg[l].rho, h->mg[l].rho_m, h->mg[l].omega,
+                    h->mg[l].n ? (double)h->mg[l].p_nnz / (double)h->mg[l].n : 0.0);
     return IF_OK;
 }
 

@@ -1,8 +1,8 @@
 // Multigrid-preconditioned CG for the n = 1 systems at large scales (included by solve.cu).
 //
 //   PCG on (M + c S) x = M phi, x0 = phi, preconditioner B = one V cycle of the smoothed-
-//   aggregation hierarchy of mg.cu with damped Jacobi smoothing (one sweep on the mesh, MG_NU_COARSE on the coarse
-//   levels) and a dense Cholesky solve on the coarsest level.
+//   aggregation hierarchy of mg.cu with damped Jacobi smoothing (one sweep on the mesh, MG_NU_L1 on level 1,
+//   MG_NU_COARSE on the coarser levels) and a dense Cholesky solve on the coarsest level.
 //   B is symmetric positive definite and fixed per column, so plain PCG applies.  16 columns at a time, every
 //   column with its own c, alpha, beta and stop time.  As in the Jacobi path all CG scalars live in the device
 //   control block: the iteration is
@@ -284,7 +284,7 @@ inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
 }
 
 // One V cycle on level l: e = B_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
-// nu = 1 on level 0 and MG_NU_COARSE below it.  R holds r and is not changed; E, T, E2 are work buffers of the
+// nu = 1 on level 0, MG_NU_L1 on level 1 and MG_NU_COARSE below.  R holds r and is not changed; E, T, E2 are work buffers of the
 // level; *result is the one that holds e.
 // On level 0 the caller may have done the first sweep and its residual already (first_done: E = omega r / d,
 // T = r - A E, both by k_spmm<16, MGR>) and chooses the sub-mode of the last sweep (final_sub 3 / 4: with the CG
