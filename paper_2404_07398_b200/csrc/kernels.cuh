@@ -90,7 +90,8 @@ enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX 
 // at the start of a batch (rho = r.z, beta = 0, no iteration counted).
 // MODE_MGR (multigrid path, level 0): the residual update of CG, the first Jacobi sweep of the preconditioner (from a
 // zero guess) and the residual of that sweep in one pass.  in0 = r, in1 = q (both gathered: tile by bulk copy, halo
-// rows from L2), alpha from the control block:  r' = r - alpha q -> x ;  e = omega r'/d -> out1 ;  t = r' - A e -> out0.
+// rows from L2), alpha from the control block:  r' = r - alpha q -> x ;  e = omega r'/d -> out1 (unless out1 is
+// null: k_mg_prolong0 forms it again) ;  t = r' - A e -> out0.
 // r' goes to a second buffer (x), not over r: other blocks still read r and q for their halo rows.
 
 __device__ __forceinline__ double2 ld2(const double* __restrict__ p, int64_t i) {
@@ -534,7 +535,8 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             bulk_wait_read0();   // the stage of tile it-1 is free once its bulk store has been read
             if (t2 < ntiles) issue(t2, (int)((it + LA) % NS), tq);
             if (CG_A || MGR) {
-                bulk_store(a.out1 + row0 * K, sa, (uint32_t)nrows * K * sizeof(double));
+                // (MGR with out1 == nullptr: e is not stored, the prolongation kernel forms it again from r')
+                if (!MGR || a.out1) bulk_store(a.out1 + row0 * K, sa, (uint32_t)nrows * K * sizeof(double));
                 if (MGR) bulk_store(a.x + row0 * K, sb, (uint32_t)nrows * K * sizeof(double));
                 bulk_commit();
             }

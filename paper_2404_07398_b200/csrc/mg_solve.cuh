@@ -158,6 +158,51 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __r
     }
 }
 
+// Prolongation onto the mesh fused with the first sweep:  e = omega r / d + P e_c  (8 threads per row as above; the
+// prolongator has 2.6 entries per row).  k_spmm<16, MGR> then does not store its e = omega r'/d, and this kernel
+// reads r' where k_mg_csr<1, 1> would read e back: one pass over a [V][16] vector less per iteration.
+__global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_prolong0(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                                                       const double* __restrict__ val, MgMat g, MgCols cs,
+                                                       const double* __restrict__ x, const double* __restrict__ r,
+                                                       double* __restrict__ y) {
+    constexpr int WPB = BLOCK / 8;
+    const int l = threadIdx.x % 8;
+    const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
+    const int64_t n = g.n;
+    const int64_t per_block = ((n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;   // contiguous rows per block
+    const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, n);
+    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / 8; row < row_end; row += WPB) {
+        const int64_t ri = row * MGK + 2 * l;
+        const double2 rv = ld2(r, ri);
+        const double2 d = g.diag[row];
+        double2 s = {0.0, 0.0};
+        const int64_t k1 = rowptr[row + 1];
+        for (int64_t k = rowptr[row]; k < k1; k += MG_UB) {
+            double w[MG_UB];
+            double2 v[MG_UB];
+            int32_t cj[MG_UB];
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j) {
+                const int64_t kk = k + j < k1 ? k + j : k;
+                cj[j] = col[kk];
+                w[j] = val[kk];
+            }
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * MGK + 2 * l);
+#pragma unroll
+            for (int j = 0; j < MG_UB; ++j)
+                if (k + j < k1) {
+                    s.x = fma(w[j], v[j].x, s.x);
+                    s.y = fma(w[j], v[j].y, s.y);
+                }
+        }
+        // the same arithmetic as the e of k_spmm<16, MGR> (rcp_pos, this order of the products)
+        s.x += g.omega * rv.x * rcp_pos(fma(cc.x, d.x, d.y));
+        s.y += g.omega * rv.y * rcp_pos(fma(cc.y, d.x, d.y));
+        st2(y, ri, s);
+    }
+}
+
 // coarsest level: dense Cholesky of A = M + c S per column (one block per column), then the two triangular solves
 __global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, MgCols cs, const double* __restrict__ r, double* __restrict__ e) {
     __shared__ double a[MG_COARSEST][MG_COARSEST + 1];
@@ -277,6 +322,8 @@ inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) 
     return m;
 }
 
+// level 0: the prolongation kernel can form e = omega r'/d itself (short prolongator rows only)
+inline bool mg_fused_prolongation(const MgLevel& g) { return g.p_nnz < IF_MG_WIDE * g.n; }
 inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n, g.omega}; }
 inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
     const int64_t rows = BLOCK / (8 * sl);
@@ -344,7 +391,9 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
     IF_LAUNCH_CHECK();
     double* ec = nullptr;
     if ((rc = mg_vcycle(r, b, cs, l + 1, nb[0], nb[1], nb[2], nb[3], &ec))) return rc;
-    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
+    if (l == 0 && first_done && nu == 1 && mg_fused_prolongation(g))   // cur = omega R / d has not been stored
+        k_mg_prolong0<<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, gm, cs, ec, R, cur);
+    else if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
     else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
     IF_LAUNCH_CHECK();
     for (int k = 0; k < nu; ++k) {
@@ -437,7 +486,7 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
         }
         cur ^= 1;
         {
-            SpmmArgs a{b.r[cr], b.q, b.r[cr ^ 1], b.t, b.za, 0, 0, g0.omega};
+            SpmmArgs a{b.r[cr], b.q, b.r[cr ^ 1], b.t, mg_fused_prolongation(h->mg[0]) ? nullptr : b.za, 0, 0, g0.omega};
             if ((rc = launch_spmm<MGK, MODE_MGR>(r, mgr_grid, a))) return rc;
         }
         cr ^= 1;
