@@ -61,7 +61,7 @@ struct Ctrl {
     int status[KMAX];
     int iters[KMAX];
     int all_done;
-    int cur_p;            // which direction buffer the last kernel A wrote
+    int cur_p;            // which direction buffer holds the current direction (flipped at the end of every iteration)
     int max_iter;
     int pad_;
     double tol2;
@@ -222,7 +222,7 @@ __device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const do
         }
     }
     __syncthreads();
-    if (tid == 0) { ctrl->all_done = !any_active; if (!start) ctrl->total_iters += 1; }
+    if (tid == 0) { ctrl->all_done = !any_active; if (!start) { ctrl->total_iters += 1; ctrl->cur_p ^= 1; } }
 }
 
 // ------------------------------------------------------------------------------------------- kernel A
@@ -233,7 +233,9 @@ struct SpmmArgs {
     double* out0;        // PLAIN: y        CG1: q             CG2A: t            CG2B: q
     double* out1;        //                 CG1/CG2A: p_new
     int scale_inv_area;  // PLAIN: multiply the row result by 1/A_v
-    int out_idx;         // CG1/CG2A: index of the direction buffer written (recorded in ctrl->cur_p)
+    int p_select;        // CG1/CG2A/CG2B inside the iteration: in1 and out1 are the two direction buffers p[0], p[1] and
+                         // the kernel picks old/new from ctrl->cur_p (the buffer holding the current direction), so a
+                         // captured graph stays valid whatever iteration it resumes at
     double omega;        // AX, sub-mode 2: damping
 };
 
@@ -323,7 +325,7 @@ __device__ __forceinline__ TileIssue load_issue(const int32_t* __restrict__ desc
 // About 130 KB of loads per SM are outstanding at all times, which is what the loaded HBM latency of B200 needs.
 template <int K, int MODE>
 __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
-                                                        double* __restrict__ partials, SpmmArgs a) {
+                                                        double* __restrict__ partials, SpmmArgs a_in) {
     using SM = TileSmem<K, MODE>;
     constexpr int T = SM::T;
     constexpr int NT = SpmmCfg<K>::NT;
@@ -337,6 +339,15 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     constexpr bool MGR = (MODE == MODE_MGR);
     constexpr bool AXE = (MODE == MODE_AX || MODE == MODE_MGR);   // epilogue with A = M + c S
     if (MODE != MODE_PLAIN && ctrl->all_done) return;
+    SpmmArgs a = a_in;
+    if ((CG_A || MODE == MODE_CG2B) && a.p_select) {
+        // direction buffers by the device-side index: p[cur_p] is the current direction, kernel A writes the other one
+        // (cur_p flips at the end of the iteration, in the last block of k_update / cg_bookkeeping)
+        double* const pb[2] = {const_cast<double*>(a_in.in1), a_in.out1};
+        const int cp = ctrl->cur_p;
+        a.in1 = pb[CG_A ? cp : cp ^ 1];
+        a.out1 = CG_A ? pb[cp ^ 1] : nullptr;
+    }
     extern __shared__ __align__(128) unsigned char smem[];
     int32_t* sdesc = reinterpret_cast<int32_t*>(smem + SM::off_desc);   // [4][16] tile descriptors (ring)
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::off_bar);   // one per stage
@@ -563,7 +574,17 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                     case 4: s = gather_row<4, TPR>(scol + o, sval + o, sa, l); break;
                     case 6: s = gather_row<6, TPR>(scol + o, sval + o, sa, l); break;
                     case 8: s = gather_row<8, TPR>(scol + o, sval + o, sa, l); break;
-                    default: break;   // w == 0 (staged tiles have w <= WCAP = 8, always even)
+                    default:
+                        // a slice wider than 8 (a vertex of valence 9 or more in its 32 rows): the tile's slots still
+                        // fit the shared slice (is_staged checks the total), so the same gather as a plain loop
+                        for (int k = 0; k < w; k += 2) {
+                            const int2 cj = *reinterpret_cast<const int2*>(scol + o + k);
+                            const double2 vj = *reinterpret_cast<const double2*>(sval + o + k);
+                            const double2 g0 = sa[cj.x * TPR + l], g1 = sa[cj.y * TPR + l];
+                            s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
+                            s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
+                        }
+                        break;
                 }
             } else {
                 // fallback (wide rows or a halo beyond HALO_CAP): global column ids, out-of-tile rows from L2
@@ -689,7 +710,6 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
         if (grid_reduce<K, 2, NT>(acc2, partials, &ctrl->ticket[2], tot2))
             cg_bookkeeping<K>(ctrl, tot2, a.scale_inv_area == 4);
     }
-    if (CG_A && blockIdx.x == 0 && tid == 0) ctrl->cur_p = a.out_idx;
 }
 
 // ------------------------------------------------------------------------------------------- start of a column
@@ -835,7 +855,7 @@ __global__ void __launch_bounds__(BLOCK, 2) k_update(MeshView m, Ctrl* __restric
             }
         }
         __syncthreads();
-        if (tid == 0) { ctrl->all_done = !any_active; ctrl->total_iters += 1; }
+        if (tid == 0) { ctrl->all_done = !any_active; ctrl->total_iters += 1; ctrl->cur_p ^= 1; }
     }
 }
 

@@ -458,6 +458,7 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
         if ((rc = launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a))) return rc;
     }
     IF_CUDA_TRY(cudaMemsetAsync(b.p[0], 0, (size_t)nv * MGK * sizeof(double), r.st));
+    IF_CUDA_TRY(cudaMemsetAsync(b.p[1], 0, (size_t)nv * MGK * sizeof(double), r.st));
     if ((rc = mg_dots(r, b, b.za, b.za, b.za, h_dots))) return rc;            // ||M phi||^2 (host sync)
     // the control block of the batch: unused columns stay done, the others start with rho, beta set by the first
     // preconditioner application (sub-mode 4)
@@ -478,13 +479,12 @@ int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rh
     bool stop = false;
     if ((rc = all_done(&stop))) return rc;
     int64_t loops = 0;
-    int cur = 0, cr = 0;
+    int cr = 0;
     while (!stop) {
         {
-            SpmmArgs a{z, b.p[cur], b.x, b.q, b.p[cur ^ 1], 0, cur ^ 1, 0.0};  // kernel A of the Jacobi path
+            SpmmArgs a{z, b.p[0], b.x, b.q, b.p[1], 0, 1, 0.0};  // kernel A of the Jacobi path
             if ((rc = launch_spmm<MGK, MODE_CG1>(r, cg_grid, a))) return rc;
         }
-        cur ^= 1;
         {
             SpmmArgs a{b.r[cr], b.q, b.r[cr ^ 1], b.t, mg_fused_prolongation(h->mg[0]) ? nullptr : b.za, 0, 0, g0.omega};
             if ((rc = launch_spmm<MGK, MODE_MGR>(r, mgr_grid, a))) return rc;

@@ -372,7 +372,6 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
     if (o.sell_sigma < o.sell_c || o.sell_sigma % o.sell_c != 0) return IF_EINVAL;
     if (o.sfc_kind != 0 && o.sfc_kind != 1) return IF_EINVAL;
     if ((o.solver != 0 && o.solver != 1) || !(o.mg_min_ell > 0.0)) return IF_EINVAL;
-    o.check_every = (o.check_every + 1) & ~1;   // even: the search direction is double-buffered
     *out = o;
     return IF_OK;
 }

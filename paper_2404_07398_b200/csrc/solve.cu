@@ -132,29 +132,25 @@ struct TimingEvents {
     }
 };
 
+// One CG iteration: kernel A (two launches for n = 2) and kernel B.  The direction buffers are picked on the device
+// from ctrl->cur_p, so every iteration is the same launch sequence and a graph may resume at any iteration.
 template <int K>
-int enqueue_two_iterations(const Run& r, const TimingEvents* tev = nullptr) {
-    // iteration with p0 -> p1, then p1 -> p0
+int enqueue_iteration(const Run& r, const TimingEvents* tev = nullptr) {
     int rc;
-    for (int half = 0; half < 2; ++half) {
-        const bool timed = tev && half == 0;
-        if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s0, r.st, cudaEventRecordExternal));
-        const double* pold = half == 0 ? r.w.p0 : r.w.p1;
-        double* pnew = half == 0 ? r.w.p1 : r.w.p0;
-        if (r.order_n == 1) {
-            SpmmArgs a{r.w.z, pold, r.w.x, r.w.q, pnew, 0, half == 0 ? 1 : 0};
-            if ((rc = launch_spmm<K, MODE_CG1>(r, r.g.cga, a))) return rc;
-        } else {
-            SpmmArgs a{r.w.z, pold, r.w.x, r.w.t, pnew, 0, half == 0 ? 1 : 0};
-            if ((rc = launch_spmm<K, MODE_CG2A>(r, r.g.cga, a))) return rc;
-            SpmmArgs b{r.w.t, pnew, nullptr, r.w.q, nullptr, 0, 0};
-            if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
-        }
-        if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s1, r.st, cudaEventRecordExternal));
-        k_update<K><<<r.g.update, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.z, r.w.q, r.order_n);
-        IF_LAUNCH_CHECK();
-        if (timed) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->u1, r.st, cudaEventRecordExternal));
+    if (tev) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s0, r.st, cudaEventRecordExternal));
+    if (r.order_n == 1) {
+        SpmmArgs a{r.w.z, r.w.p0, r.w.x, r.w.q, r.w.p1, 0, 1};
+        if ((rc = launch_spmm<K, MODE_CG1>(r, r.g.cga, a))) return rc;
+    } else {
+        SpmmArgs a{r.w.z, r.w.p0, r.w.x, r.w.t, r.w.p1, 0, 1};
+        if ((rc = launch_spmm<K, MODE_CG2A>(r, r.g.cga, a))) return rc;
+        SpmmArgs b{r.w.t, r.w.p0, nullptr, r.w.q, r.w.p1, 0, 1};
+        if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
     }
+    if (tev) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s1, r.st, cudaEventRecordExternal));
+    k_update<K><<<r.g.update, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.z, r.w.q, r.order_n);
+    IF_LAUNCH_CHECK();
+    if (tev) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->u1, r.st, cudaEventRecordExternal));
     return IF_OK;
 }
 
@@ -322,8 +318,8 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
     }
 
     // the iteration loop: `check_every` iterations per CUDA graph launch, snapshot polled one launch behind
-    const int pairs = r.opt.check_every / 2;
-    const int launches_per_graph = pairs * 2 * (r.order_n == 1 ? 2 : 3);
+    const int per_graph = r.opt.check_every;
+    const int launches_per_graph = per_graph * (r.order_n == 1 ? 2 : 3);
     GraphSet gs;
     if (r.st != nullptr && r.st != cudaStreamLegacy) {
         for (int gi = 0; gi < 2; ++gi) {
@@ -334,9 +330,9 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
                 break;
             }
             int rcc = IF_OK;
-            const int timed_pair = pairs > 1 ? 1 : 0;
-            for (int i = 0; i < pairs && rcc == IF_OK; ++i)
-                rcc = enqueue_two_iterations<K>(r, i == timed_pair ? &gs.tev[gi] : nullptr);
+            const int timed_it = per_graph > 2 ? 2 : 0;
+            for (int i = 0; i < per_graph && rcc == IF_OK; ++i)
+                rcc = enqueue_iteration<K>(r, i == timed_it ? &gs.tev[gi] : nullptr);
             g_launches -= (long long)launches_per_graph;   // captured, not launched
             cudaError_t e = cudaStreamEndCapture(r.st, &graph);
             if (rcc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
@@ -353,8 +349,8 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
             IF_CUDA_TRY(cudaGraphLaunch(gs.exec[it & 1], r.st));
             g_launches += (long long)launches_per_graph;
         } else {
-            for (int i = 0; i < pairs; ++i)
-                if ((rc = enqueue_two_iterations<K>(r))) return rc;
+            for (int i = 0; i < per_graph; ++i)
+                if ((rc = enqueue_iteration<K>(r))) return rc;
         }
         const int slot = (int)(it & 3);
         IF_CUDA_TRY(cudaMemcpyAsync(&poll.snap[slot], reinterpret_cast<const char*>(r.w.ctrl) + offsetof(Ctrl, done),

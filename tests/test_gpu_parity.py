@@ -453,3 +453,182 @@ def test_multigrid_hierarchy_survives_save_and_load(ifl, tmp_path):
     assert np.array_equal(sa["iters"], sb["iters"]) and sa["iters"].max() < 60
     assert bool((a == b).all())
     h.close(); h2.close()
+
+
+# ------------------------------------------------------------------------------------------ n = 2 at the top of its range
+def true_residual(ifl, h, x, phi, area, ell, order_n):
+    """||M phi - A_l x||_2 / ||M phi||_2 with A_l x from the library's if_apply (x: device tensor [V])."""
+    import torch
+    b = torch.from_numpy(area * phi).to(x.device)
+    ax = ifl.if_apply(h, x[None, :], np.array([ell]), order_n)[0, 0]
+    return float(torch.linalg.norm(b - ax) / torch.linalg.norm(b))
+
+
+def parity_tolerance(area, phi, x_ref, res_a, res_b):
+    """Tolerance for the relative L2 difference of two approximate solutions of A x = M phi, A = M + c S M^-1 S
+    ("n = 2 at large scales"): x_a - x_b = A^-1 (r_b - r_a) and A >= M (S M^-1 S is positive
+    semidefinite), so ||x_a - x_b|| <= (res_a + res_b) ||M phi|| / min A_v with res = TRUE relative residuals.
+    1e-7 (north_star) wherever that bound supports it, the bound itself elsewhere."""
+    bound = (res_a + res_b) * np.linalg.norm(area * phi) / area.min() / np.linalg.norm(x_ref)
+    return max(TOL_FIELD, float(bound))
+
+
+LARGE_N2 = {
+    "cfg3_L4": lambda: make_config(3, level=4, n_ells=6, ell_max=32.0),
+    "cfg3_L5": lambda: make_config(3, level=5, n_ells=6, ell_max=32.0),
+    "cfg5_L5": lambda: make_config(5, level=5, n_fields=3, n_ells=6, ell_max=32.0),
+}
+
+
+@pytest.mark.parametrize("name", list(LARGE_N2))
+def test_biharmonic_up_to_32_edge_lengths_matches_oracle(ifl, oracle_mod, name):
+    """Reading A16 sets the n = 2 range to [1, 32] h; kappa ~ 1/2 (l^2 lambda_max)^2 reaches 1e8 at the top, where the
+    true residual of any fp64 CG floors near u kappa (oracle: 1e-8 to 5e-8 at 32 h).  Scales 1, 2, 4, 8, 16, 32 h,
+    every field element by element against the oracle, tolerance from the recorded true residuals of BOTH sides."""
+    w = LARGE_N2[name]()
+    assert abs(w.ells[-1] / w.mesh.h - 32.0) < 1e-9
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    area = om.area()
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    out, st = ifl.if_filter(h, w.fields, w.ells, 2)
+    assert st["code"] == 0 and np.all(st["status"] == 0)
+    sp = ifl.if_spectrum(h, w.fields, w.ells, 2)
+    worst = 0.0
+    for f in range(w.fields.shape[0]):
+        en = []
+        for j, ell in enumerate(w.ells):
+            x, info = om.solve(w.fields[f], float(ell), 2)
+            assert info["status"] == 0
+            res_gpu = true_residual(ifl, h, out[f, j], w.fields[f], area, float(ell), 2)
+            tol = parity_tolerance(area, w.fields[f], x, res_gpu, info["true_res"])
+            err = rel(out[f, j].cpu().numpy(), x)
+            assert err <= tol, (f, j, err, tol, res_gpu, info["true_res"])
+            assert res_gpu <= 20.0 * max(info["true_res"], 1e-12), (f, j, res_gpu, info["true_res"])
+            worst = max(worst, err)
+            en.append(om.energy(x))
+        en = np.array(en)
+        k_mid, E = oracle_mod.spectrum(w.ells, en)
+        assert np.all(np.abs(sp["energy"][f] - en) <= TOL_BIN * en)
+        assert np.all(np.abs(sp["E"][f] - E) <= TOL_BIN * np.abs(E)), (f, np.abs(sp["E"][f] / E - 1).max())
+    print(f"{name}: worst relative L2 difference from the oracle {worst:.2e}")
+    h.close()
+
+
+def test_biharmonic_32_edge_lengths_against_dense_direct_solve(ifl, oracle_mod):
+    """The same top-of-range solves against numpy's dense LU of A = M + c S M^-1 S built from the oracle's CSR
+    (2 562 vertices): neither CG is the reference here."""
+    w = LARGE_N2["cfg3_L4"]()
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    rp, col, val = om.csr()
+    V = om.nv
+    S = np.zeros((V, V))
+    for v in range(V):
+        S[v, col[rp[v]:rp[v + 1]]] = val[rp[v]:rp[v + 1]]
+    area = om.area()
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    ells = w.ells[-3:]
+    out, st = ifl.if_filter(h, w.fields, ells, 2)
+    assert st["code"] == 0
+    for j, ell in enumerate(ells):
+        A = np.diag(area) + 0.5 * ell ** 4 * (S @ (S / area[:, None]))
+        x = np.linalg.solve(A, area * w.fields[0])
+        assert rel(out[0, j].cpu().numpy(), x) <= TOL_FIELD, (j, rel(out[0, j].cpu().numpy(), x))
+    h.close()
+
+
+def test_biharmonic_beyond_its_range_returns_a_status(ifl):
+    """for the biharmonic filter "the convergence can be lost for large l".  l = 400 h on a
+    level-5 sphere (kappa ~ 1e12-1e13, far beyond reading A16's range) with the default iteration cap: the call must
+    come back -- per-right-hand-side status, finite output, every column stopped by the cap or converged -- not hang."""
+    w = make_config(5, level=5, n_fields=2, n_ells=2, ell_max=2.0)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    ells = w.mesh.h * np.array([2.0, 400.0])
+    out, st = ifl.if_filter(h, w.fields, ells, 2, max_iter=60000)
+    assert np.all(st["status"][:, 0] == 0)
+    assert st["code"] in (0, 1) and np.all(np.isin(st["status"][:, 1], (0, 1, 2)))
+    assert st["code"] == (1 if np.any(st["status"] != 0) else 0)
+    capped = st["status"][:, 1] == 1
+    assert np.all(st["iters"][capped, 1] == 60000)
+    assert bool(out.isfinite().all())
+    print("l = 400 h: status", st["status"][:, 1], "iterations", st["iters"][:, 1], "residual", st["rel_res"][:, 1])
+    h.close()
+
+
+def test_breakdown_status_is_per_column(ifl, oracle_mod):
+    """status 2 (breakdown): a right-hand side whose arithmetic leaves the finite range stops with status 2 and does
+    not disturb the other columns of its batch.  (a) a field holding a NaN; (b) l = 1e60 with n = 2: c = l^4 / 2
+    overflows ||r0||^2."""
+    w = make_config(4, level=4, n_fields=2, n_ells=3)
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
+    fields = w.fields.copy()
+    fields[1, 17] = np.nan
+    out, st = ifl.if_filter(h, fields, w.ells, 1)
+    assert st["code"] == 1 and np.all(st["status"][1] == 2) and np.all(st["status"][0] == 0)
+    for j, ell in enumerate(w.ells):
+        x, _ = om.solve(fields[0], float(ell), 1)
+        assert rel(out[0, j].cpu().numpy(), x) <= TOL_FIELD
+    ells = np.array([w.ells[0], 1e60])
+    out, st = ifl.if_filter(h, w.fields, ells, 2)
+    assert st["code"] == 1 and np.all(st["status"][:, 1] == 2) and np.all(st["status"][:, 0] == 0)
+    for f in range(2):
+        x, _ = om.solve(w.fields[f], float(ells[0]), 2)
+        assert rel(out[f, 0].cpu().numpy(), x) <= TOL_FIELD
+    h.close()
+
+
+# ------------------------------------------------------------------------------------------ general unstructured meshes
+@pytest.mark.parametrize("sell_c", [32, 64])
+def test_rows_wider_than_eight_entries(ifl, oracle_mod, sell_c):
+    """A Delaunay mesh with valences 3 to 14: SELL slices wider than the 8 slots the unrolled gather of the staged
+    tiles handles.  Operator and solves (n = 1, 2, and the multigrid path, whose level 0 is the same kernel) against
+    the oracle."""
+    from workloads import delaunay_mesh
+    m = delaunay_mesh(48, np.random.default_rng(3))
+    om = oracle_mod.OracleMesh(m.coords, m.tri, None)
+    rp, _, _ = om.csr()
+    assert (np.diff(rp) - 1).max() >= 12
+    rng = np.random.default_rng(4)
+    fields = rng.standard_normal((3, m.n_vert))
+    ells = np.array([0.8, 3.0, 9.0])
+    h = ifl.if_prepare(m.coords, m.tri, None, sell_c=sell_c, flags=ifl.IF_FLAG_MULTIGRID)
+    assert h.unstaged_tiles < h.n_tiles            # the wide rows sit in staged tiles
+    for order_n in (1, 2):
+        ap = ifl.if_apply(h, fields, ells, order_n).cpu().numpy()
+        for f in range(3):
+            for j, ell in enumerate(ells):
+                assert rel(ap[f, j], om.apply(fields[f], float(ell), order_n)) <= 1e-12, (order_n, f, j)
+    for order_n, kw in ((1, {}), (2, {}), (1, dict(solver=1, mg_min_ell=1.0))):
+        out, st = ifl.if_filter(h, fields, ells[:2] if order_n == 2 else ells, order_n, **kw)
+        assert st["code"] == 0
+        out = out.cpu().numpy()
+        for f in range(3):
+            for j in range(out.shape[1]):
+                x, info = om.solve(fields[f], float(ells[j]), order_n)
+                assert info["status"] == 0 and rel(out[f, j], x) <= TOL_FIELD, (order_n, kw, f, j)
+    h.close()
+
+
+@pytest.mark.parametrize("check_every", [1, 3, 16])
+def test_refill_while_other_columns_have_a_pending_step(ifl, oracle_mod, check_every):
+    """4 columns, 27 short solves at a loose tolerance, graph launches of 1, 3 or 16 iterations: columns stop on odd and
+    even iterations while the queue is not empty, so refilled columns restart next to columns whose last step
+    x += alpha p is still pending.  At the same iteration count the CG iterate is the oracle's up to rounding."""
+    w = make_config(2, n=48, n_fields=3, n_ells=9, ell_max=6.0)
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    for order_n in (1, 2):
+        out, st = ifl.if_filter(h, w.fields, w.ells, order_n, batch=4, tol=1e-4, check_every=check_every)
+        out = out.cpu().numpy()
+        assert st["code"] == 0
+        same = 0
+        for f in range(3):
+            for j, ell in enumerate(w.ells):
+                x, info = om.solve(w.fields[f], float(ell), order_n, tol=1e-4)
+                if info["iters"] == st["iters"][f, j]:
+                    same += 1
+                    assert rel(out[f, j], x) <= 1e-9, (order_n, f, j, rel(out[f, j], x))
+                else:
+                    assert abs(info["iters"] - st["iters"][f, j]) <= 1 and rel(out[f, j], x) <= 1e-3
+        assert same >= 24
+    h.close()

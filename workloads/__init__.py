@@ -6,9 +6,9 @@ arithmetic (stiffness, areas, solves, spectra) lives here; the oracle (oracle/) 
 """
 from .configs import Workload, make_config
 from .fields import Waves, log_spaced, planar_wave_field, sphere_wave_field
-from .meshes import (Mesh, equilateral_mesh, grid_mesh, icosphere, icosphere_edge, jitter_sphere,
+from .meshes import (Mesh, delaunay_mesh, equilateral_mesh, grid_mesh, icosphere, icosphere_edge, jitter_sphere,
                      land_mask)
 
 __all__ = ["Workload", "make_config", "Waves", "log_spaced", "planar_wave_field", "sphere_wave_field",
-           "Mesh", "equilateral_mesh", "grid_mesh", "icosphere", "icosphere_edge", "jitter_sphere",
+           "Mesh", "delaunay_mesh", "equilateral_mesh", "grid_mesh", "icosphere", "icosphere_edge", "jitter_sphere",
            "land_mask"]

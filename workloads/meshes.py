@@ -213,3 +213,27 @@ def land_mask(mesh: Mesh, positions: np.ndarray, fraction: float, rng: np.random
     tri = new_id[tri].astype(np.int32)
     return Mesh(coords=np.ascontiguousarray(mesh.coords[used]), tri=np.ascontiguousarray(tri),
                 period=None, h=mesh.h, name=mesh.name + "m")
+
+
+# --------------------------------------------------------------------------- unstructured planar (Delaunay)
+def delaunay_mesh(n: int, rng: np.random.Generator, hubs: int = 3, hub_valence: int = 14) -> Mesh:
+    """Non-periodic planar mesh of the square [0, n]^2 with unit point density: a regular boundary (spacing 1),
+    uniformly random interior points and `hubs` hub vertices, each the centre of a circle of `hub_valence` points
+    with nothing else inside (so the hub has exactly that many neighbours), triangulated by scipy's Delaunay.
+    Vertex valences spread from 3 to hub_valence -- unlike the grids and icospheres, whose rows never exceed 8
+    entries -- which is what a general unstructured mesh looks like to the SELL packing."""
+    from scipy.spatial import Delaunay
+    t = np.arange(n, dtype=np.float64)
+    border = np.concatenate([np.stack([t, np.zeros(n)], 1), np.stack([np.full(n, float(n)), t], 1),
+                             np.stack([n - t, np.full(n, float(n))], 1), np.stack([np.zeros(n), n - t], 1)])
+    inner = rng.uniform(0.7, n - 0.7, size=((n - 1) * (n - 1), 2))
+    centres = rng.uniform(0.25 * n, 0.75 * n, size=(hubs, 2))
+    rad = 1.5
+    for c in centres:
+        inner = inner[np.linalg.norm(inner - c, axis=1) > rad + 0.35]
+    ang = 2.0 * np.pi * np.arange(hub_valence) / hub_valence
+    rings = [c + rad * np.stack([np.cos(ang + 0.1 * i), np.sin(ang + 0.1 * i)], 1) for i, c in enumerate(centres)]
+    pts = np.concatenate([border, inner, centres] + rings)
+    tri = Delaunay(pts).simplices.astype(np.int32)
+    return Mesh(coords=np.ascontiguousarray(pts), tri=np.ascontiguousarray(tri), period=None, h=1.0,
+                name=f"delaunay{n}")
