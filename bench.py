@@ -245,9 +245,9 @@ def run_ours(args):
         opts["max_iter"] = args.max_iter
     K = args.batch or 16
     # the multigrid hierarchy exists for n = 1 only; it is built in if_prepare and costs nothing when unused
-    use_mg = (w.order_n == 1 and K == 16) and (args.solver == "multigrid" or not args.no_multigrid)
+    use_mg = K == 16 and (args.solver == "multigrid" or not args.no_multigrid)
     if args.solver == "multigrid" and not use_mg:
-        raise SystemExit("bench.py: --solver multigrid needs an n = 1 workload and batch 16")
+        raise SystemExit("bench.py: --solver multigrid needs batch 16")
     mg_opts = dict(opts, solver=1)
     if args.mg_min_ell:
         mg_opts["mg_min_ell"] = args.mg_min_ell

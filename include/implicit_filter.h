@@ -77,13 +77,14 @@ typedef struct {
                         larger window scatters a tile over the window and defeats the halo staging)         */
     int sfc_kind;    /* 0 => Morton order of the quantised coordinates; 1 => keep the caller's order        */
     int flags;       /* IF_FLAG_*                                                                           */
-    int solver;      /* 0 => Jacobi-preconditioned CG for every right-hand side.  1 => right-hand sides with
-                        l >= mg_min_ell mean edge lengths are solved by multigrid-preconditioned CG (one V
-                        cycle of a smoothed-aggregation hierarchy per iteration; n = 1, batch = 16 and a handle
-                        prepared with IF_FLAG_MULTIGRID, else ignored), the rest by Jacobi-PCG.  Same systems,
-                        same stop test, same answers within the tolerance (PAPER.md:207 names the convergence of
-                        plain CG at large scales as the open problem)                                           */
-    double mg_min_ell; /* 0 => 4 (in mean edge lengths; below that Jacobi-PCG needs fewer bytes)                */
+    int solver;      /* 0 => Jacobi-preconditioned CG for every right-hand side (per call: 0 inherits the handle's choice,
+                        2 = Jacobi-PCG explicitly).  1 => right-hand sides with l >= mg_min_ell mean edge lengths are
+                        solved by multigrid-preconditioned CG: one V cycle of a smoothed-aggregation hierarchy per
+                        iteration for n = 1, the product V M V of two cycles for n = 2 (needs batch = 16 and a handle
+                        prepared with IF_FLAG_MULTIGRID, else ignored); the rest by Jacobi-PCG.  Same systems, same
+                        start vector, same stop test, same answers within the tolerance (PAPER.md:207 names the
+                        convergence of plain CG at large scales, above all for n = 2, as the open problem)           */
+    double mg_min_ell; /* 0 => 4 for n = 1, 0.5 for n = 2 (in mean edge lengths; below that Jacobi-PCG is cheaper)     */
 } if_options;
 
 typedef struct {
@@ -98,6 +99,14 @@ typedef struct {
                               once per check_every iterations; 0 if nothing was sampled                       */
     double update_seconds; /* out: the same for ONE fused vector-update kernel                               */
     int64_t kernel_samples; /* out: number of samples behind the two means                                   */
+    double mg_kernel_seconds[8]; /* out (solver = 1): mean device time per ITERATION of the kernel groups of the
+                              multigrid-preconditioned path, CUDA events on the stream, one sample per graph launch:
+                              [0] kernel A (n = 2: its two launches)  [1] fused residual update + first sweep + its
+                              residual on the mesh  [2] restriction mesh -> level 1  [3] all kernels on level 1
+                              [4] levels >= 2  [5] prolongation level 1 -> mesh  [6] last sweep (+ CG bookkeeping);
+                              for n = 2 groups 1-6 hold the sum over both cycles; [7] unused                         */
+    int64_t mg_samples;     /* out: samples behind mg_kernel_seconds                                          */
+    int64_t mg_batch_iters; /* out: 16-column iterations of the multigrid-preconditioned path (part of batch_iters) */
 } if_stats;
 
 /* Preparation phase.  All pointers HOST.

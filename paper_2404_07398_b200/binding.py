@@ -35,7 +35,8 @@ class if_stats(C.Structure):
     _fields_ = [("iters", C.POINTER(C.c_int32)), ("rel_res", C.POINTER(C.c_double)),
                 ("status", C.POINTER(C.c_int32)), ("seconds", C.c_double), ("batch_iters", C.c_int64),
                 ("rhs_iters", C.c_int64), ("spmm_seconds", C.c_double), ("update_seconds", C.c_double),
-                ("kernel_samples", C.c_int64)]
+                ("kernel_samples", C.c_int64), ("mg_kernel_seconds", C.c_double * 8), ("mg_samples", C.c_int64),
+                ("mg_batch_iters", C.c_int64)]
 
 
 class ImplicitFilterError(RuntimeError):
@@ -214,12 +215,15 @@ class _Stats:
         self.c = if_stats(self.iters.ctypes.data_as(C.POINTER(C.c_int32)),
                           self.rel_res.ctypes.data_as(C.POINTER(C.c_double)),
                           self.status.ctypes.data_as(C.POINTER(C.c_int32)), 0.0, 0, 0, 0.0, 0.0, 0)
+        self.c.mg_samples = 0
 
     def as_dict(self, rc: int):
         return {"iters": self.iters.reshape(self.shape), "rel_res": self.rel_res.reshape(self.shape),
                 "status": self.status.reshape(self.shape), "seconds": float(self.c.seconds),
                 "batch_iters": int(self.c.batch_iters), "rhs_iters": int(self.c.rhs_iters), "spmm_seconds": float(self.c.spmm_seconds),
                 "update_seconds": float(self.c.update_seconds), "kernel_samples": int(self.c.kernel_samples),
+                "mg_kernel_seconds": [float(v) for v in self.c.mg_kernel_seconds], "mg_samples": int(self.c.mg_samples),
+                "mg_batch_iters": int(self.c.mg_batch_iters),
                 "code": int(rc)}
 
 

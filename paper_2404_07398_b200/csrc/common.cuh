@@ -53,7 +53,7 @@ struct Options {
     int sfc_kind = 0;
     int flags = 0;
     int solver = 0;
-    double mg_min_ell = 4.0;
+    double mg_min_ell = 0.0;    // 0: the default of the order (mg_solve.cuh: 4 mean edges for n = 1, 0.5 for n = 2)
 };
 
 int resolve_options(const if_options* in, const Options* base, Options* out);

@@ -60,6 +60,11 @@ struct Ctrl {
     int epoch[KMAX];      // bumped every time a column is (re)started: lets the host match a snapshot to a RHS
     int status[KMAX];
     int iters[KMAX];
+    double c1[KMAX];      // multigrid path: coefficient of the cycle's operator K = M + c1 S (n = 1: c; n = 2: sqrt(c))
+    int starting[KMAX];   // multigrid path: the column was (re)started; its first iteration only applies the
+                          // preconditioner (alpha = 0, then rho = r.z, beta = 0), see k_init
+    int cur_r;            // multigrid path: which residual buffer holds r (flipped with cur_p)
+    int pad1_;
     int all_done;
     int cur_p;            // which direction buffer holds the current direction (flipped at the end of every iteration)
     int max_iter;
@@ -78,16 +83,20 @@ struct Snapshot {
 // per-column parameters of a (re)start, passed by value to k_init
 struct StartParams {
     double c[KMAX];
+    double c1[KMAX];      // multigrid path (see Ctrl::c1)
     int field[KMAX];
     int rhs[KMAX];
 };
 
-enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4, MODE_MGR = 5 };
-// MODE_AX (multigrid path, level 0): v = in0 (gathered), r = in1 (own rows), A = M + c S per column, and with
-// SpmmArgs::scale_inv_area as the sub-mode:  0: out0 = A v ;  1: out0 = r - A v ;  2: out0 = v + omega (r - A v)/d
+enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4, MODE_MGR = 5, MODE_MGR0 = 6 };
+// MODE_AX (multigrid path, level 0): v = in0 (gathered), r = in1 (own rows), K = M + c1 S per column (Ctrl::c1), and with
+// SpmmArgs::scale_inv_area as the sub-mode:  0: out0 = K v ;  1: out0 = r - K v ;  2: out0 = v + omega (r - K v)/d
 // (omega = SpmmArgs::omega, the Jacobi damping of the multigrid smoother on level 0);  3: as 2, the last sweep of
-// the preconditioner z = B r, plus the CG bookkeeping of kernel B (rho' = r.z, ||r||^2, beta, stop test);  4: as 3
-// at the start of a batch (rho = r.z, beta = 0, no iteration counted).
+// the preconditioner z = B r, plus the CG bookkeeping of kernel B (rho' = r.z, ||r||^2, beta, stop test);
+// 5 (n = 2, B = V M V): y = v + omega (r - K v)/d is the end of the first cycle, out0 = M y goes to the second one,
+// and the bookkeeping uses rho' = y.M y = r.(V M V r) and ||r||^2.
+// MODE_MGR0: MODE_MGR without the residual update (the second cycle of n = 2 starts from w = M y): e = omega w/d,
+// t = w - K e; only one vector arrives by bulk copy.
 // MODE_MGR (multigrid path, level 0): the residual update of CG, the first Jacobi sweep of the preconditioner (from a
 // zero guess) and the residual of that sweep in one pass.  in0 = r, in1 = q (both gathered: tile by bulk copy, halo
 // rows from L2), alpha from the control block:  r' = r - alpha q -> x ;  e = omega r'/d -> out1 (unless out1 is
@@ -192,22 +201,24 @@ __device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __
 }
 
 // CG bookkeeping after z = B r (run by the last block of a grid reduction; tot = rho' per column, then ||r||^2):
-// beta = rho'/rho, stop test, iteration count -- the same rules as the tail of k_update.  `start`: first
-// preconditioner application of a batch (rho = rho', beta = alpha = 0, nothing counted).
+// beta = rho'/rho, stop test, iteration count -- the same rules as the tail of k_update.  A column that was
+// (re)started (Ctrl::starting) has only had its preconditioner applied: rho = rho', beta = 0, nothing counted.
 template <int K>
-__device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const double* tot, bool start) {
+__device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const double* tot) {
     __shared__ int any_active;
     const int tid = threadIdx.x;
     if (tid == 0) any_active = 0;
     __syncthreads();
     if (tid < K) {
         if (!ctrl->done[tid]) {
+            const bool start = ctrl->starting[tid] != 0;
             const double rho_new = tot[tid], rr = tot[KMAX + tid];
             const int it = start ? 0 : ctrl->iters[tid] + 1;
             ctrl->iters[tid] = it;
             ctrl->rr[tid] = rr;
             double be = start ? 0.0 : rho_new / ctrl->rho[tid];
             ctrl->rho[tid] = rho_new;
+            ctrl->starting[tid] = 0;
             int dn = 0;
             if (!isfinite(rr)) { dn = 1; ctrl->status[tid] = 2; }
             else if (rr <= ctrl->tol2 * ctrl->bb[tid]) { dn = 1; ctrl->status[tid] = 0; }
@@ -215,14 +226,18 @@ __device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const do
             else if (it >= ctrl->max_iter) { dn = 1; ctrl->status[tid] = 1; }
             if (dn) { be = 0.0; ctrl->done[tid] = 1; }
             ctrl->beta[tid] = be;
-            if (start) ctrl->alpha[tid] = 0.0;
             if (!dn) atomicOr(&any_active, 1);
         } else {
             ctrl->beta[tid] = 0.0;
         }
     }
     __syncthreads();
-    if (tid == 0) { ctrl->all_done = !any_active; if (!start) { ctrl->total_iters += 1; ctrl->cur_p ^= 1; } }
+    if (tid == 0) {
+        ctrl->all_done = !any_active;
+        ctrl->total_iters += 1;
+        ctrl->cur_p ^= 1;
+        ctrl->cur_r ^= 1;
+    }
 }
 
 // ------------------------------------------------------------------------------------------- kernel A
@@ -237,6 +252,11 @@ struct SpmmArgs {
                          // the kernel picks old/new from ctrl->cur_p (the buffer holding the current direction), so a
                          // captured graph stays valid whatever iteration it resumes at
     double omega;        // AX, sub-mode 2: damping
+    double omega2;       // MGR / MGR0 with two or more sweeps before the coarse correction: out0 = e + omega2 (r' - K e)/d
+                         // (the second sweep) instead of the residual t = r' - K e; 0: the residual
+    int r_select;        // multigrid path inside the iteration: the residual is double-buffered (r[0], r[1]) and picked on
+                         // the device from ctrl->cur_r.  MGR: (in0, x) = (r[0], r[1]) -> reads r[cur_r], writes r[cur_r^1];
+                         // AX: (in1, x) = (r[0], r[1]) -> reads r[cur_r^1] (the residual MGR has just written)
 };
 
 // One row of the staged SpMM: all column ids and values of the row first, then all W gathers from the shared
@@ -294,7 +314,8 @@ template <int K> struct SpmmCfg {
 
 template <int K, int MODE> struct TileSmem {
     static constexpr int T = TILE_ROWS;
-    static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // vectors that arrive by bulk copy
+    static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // tile-sized vector regions of a stage
+    static constexpr int NLOAD = (MODE == MODE_PLAIN || MODE == MODE_MGR0) ? 1 : 2;   // vectors that arrive by bulk copy
     static constexpr size_t vec_bytes = (size_t)T * K * sizeof(double);
     static constexpr size_t off_b = (size_t)(T + HALO_CAP) * K * sizeof(double);
     static constexpr size_t off_val = off_b + (NVEC - 1) * vec_bytes;
@@ -336,8 +357,9 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     constexpr int XPT = (T * TPR + NT - 1) / NT;         // double2 elements of a tile vector per thread
     constexpr int HPT = (HALO_CAP + ROWS - 1) / ROWS;    // halo rows per thread group
     constexpr bool CG_A = (MODE == MODE_CG1 || MODE == MODE_CG2A);
-    constexpr bool MGR = (MODE == MODE_MGR);
-    constexpr bool AXE = (MODE == MODE_AX || MODE == MODE_MGR);   // epilogue with A = M + c S
+    constexpr bool MGR = (MODE == MODE_MGR || MODE == MODE_MGR0);
+    constexpr bool MGQ = (MODE == MODE_MGR);                      // with the residual update r' = r - alpha q
+    constexpr bool AXE = (MODE == MODE_AX || MGR);                // epilogue with K = M + c1 S
     if (MODE != MODE_PLAIN && ctrl->all_done) return;
     SpmmArgs a = a_in;
     if ((CG_A || MODE == MODE_CG2B) && a.p_select) {
@@ -347,6 +369,17 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
         const int cp = ctrl->cur_p;
         a.in1 = pb[CG_A ? cp : cp ^ 1];
         a.out1 = CG_A ? pb[cp ^ 1] : nullptr;
+    }
+    if (AXE && a.r_select) {
+        const int cr = ctrl->cur_r;
+        if (MGQ) {
+            double* const rb[2] = {const_cast<double*>(a_in.in0), a_in.x};
+            a.in0 = rb[cr];
+            a.x = rb[cr ^ 1];
+        } else if (MODE == MODE_AX) {
+            double* const rb[2] = {const_cast<double*>(a_in.in1), a_in.x};
+            a.in1 = rb[cr ^ 1];
+        }
     }
     extern __shared__ __align__(128) unsigned char smem[];
     int32_t* sdesc = reinterpret_cast<int32_t*>(smem + SM::off_desc);   // [4][16] tile descriptors (ring)
@@ -362,7 +395,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     if (MODE != MODE_PLAIN) {
         beta = ld2(ctrl->beta, 2 * l);
         alpha = ld2(ctrl->alpha, 2 * l);
-        cc = ld2(ctrl->c, 2 * l);
+        cc = ld2(AXE ? ctrl->c1 : ctrl->c, 2 * l);
     }
     const int C = 1 << m.log2c;
     const int64_t ntiles = (m.nv + T - 1) / T;
@@ -377,9 +410,9 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
         const uint32_t dbytes = ((uint32_t)nrows * 8u + 15u) & ~15u;   // the arrays are padded by 16 bytes
         const bool staged = ti.nh >= 0 && ti.slots <= T * WCAP;
         uint64_t* bar = &bars[stage];
-        mbar_expect_tx(bar, vbytes * SM::NVEC + 2u * dbytes + (staged ? (uint32_t)ti.slots * 12u : 0u));
+        mbar_expect_tx(bar, vbytes * SM::NLOAD + 2u * dbytes + (staged ? (uint32_t)ti.slots * 12u : 0u));
         bulk_load(st, a.in0 + row0 * K, vbytes, bar);
-        if (SM::NVEC >= 2) bulk_load(st + SM::off_b, a.in1 + row0 * K, vbytes, bar);
+        if (SM::NLOAD >= 2) bulk_load(st + SM::off_b, a.in1 + row0 * K, vbytes, bar);
         bulk_load(st + SM::off_dg, m.sdiag + row0, dbytes, bar);
         bulk_load(st + SM::off_ar, rowfac + row0, dbytes, bar);
         if (staged) {
@@ -394,7 +427,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             if (rg + i * ROWS < nh) {
                 const int64_t j = idx[i];
                 h0[i] = ld2(a.in0, j * K + 2 * l);
-                if (CG_A || MGR) h1[i] = ld2(a.in1, j * K + 2 * l);
+                if (CG_A || MGQ) h1[i] = ld2(a.in1, j * K + 2 * l);
                 if (MGR) hd[MGR ? i : 0] = make_double2(m.sdiag[j], m.area[j]);
             }
         }
@@ -429,8 +462,9 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 if (CG_A) { g.x = fma(beta.x, h1[i].x, g.x); g.y = fma(beta.y, h1[i].y, g.y); }
                 if (MGR) {   // e = omega (r - alpha q) / d of the halo row
                     const double2 dd = hd[MGR ? i : 0];
-                    g.x = a.omega * fma(-alpha.x, h1[i].x, g.x) * rcp_pos(fma(cc.x, dd.x, dd.y));
-                    g.y = a.omega * fma(-alpha.y, h1[i].y, g.y) * rcp_pos(fma(cc.y, dd.x, dd.y));
+                    if (MGQ) { g.x = fma(-alpha.x, h1[i].x, g.x); g.y = fma(-alpha.y, h1[i].y, g.y); }
+                    g.x = a.omega * g.x * rcp_pos(fma(cc.x, dd.x, dd.y));
+                    g.y = a.omega * g.y * rcp_pos(fma(cc.y, dd.x, dd.y));
                 }
                 sa[(T + hh) * TPR + l] = g;
             }
@@ -469,11 +503,14 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             const int e = tid + i * NT;
             if (e < nrows * TPR) {
                 const int rr = e / TPR;
-                const double2 rv = sa[e], qv = sb[e];
+                const double2 rv = sa[e];
                 const double sd = sdg[rr], av = sar[rr];
-                double2 rn;
-                rn.x = fma(-alpha.x, qv.x, rv.x);
-                rn.y = fma(-alpha.y, qv.y, rv.y);
+                double2 rn = rv;
+                if (MGQ) {
+                    const double2 qv = sb[e];
+                    rn.x = fma(-alpha.x, qv.x, rv.x);
+                    rn.y = fma(-alpha.y, qv.y, rv.y);
+                }
                 sb[e] = rn;
                 sa[e] = make_double2(a.omega * rn.x * rcp_pos(fma(cc.x, sd, av)), a.omega * rn.y * rcp_pos(fma(cc.y, sd, av)));
             }
@@ -548,7 +585,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             if (CG_A || MGR) {
                 // (MGR with out1 == nullptr: e is not stored, the prolongation kernel forms it again from r')
                 if (!MGR || a.out1) bulk_store(a.out1 + row0 * K, sa, (uint32_t)nrows * K * sizeof(double));
-                if (MGR) bulk_store(a.x + row0 * K, sb, (uint32_t)nrows * K * sizeof(double));
+                if (MGQ) bulk_store(a.x + row0 * K, sb, (uint32_t)nrows * K * sizeof(double));
                 bulk_commit();
             }
             if (t2 + G < ntiles) tq = load_issue(m.tile_desc, t2 + G);
@@ -602,10 +639,13 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                             g0.x = fma(beta.x, p0.x, g0.x); g0.y = fma(beta.y, p0.y, g0.y);
                         }
                         if (MGR) {
-                            const double2 p0 = ld2(a.in1, (int64_t)cj.x * K + 2 * l);
+                            if (MGQ) {
+                                const double2 p0 = ld2(a.in1, (int64_t)cj.x * K + 2 * l);
+                                g0.x = fma(-alpha.x, p0.x, g0.x); g0.y = fma(-alpha.y, p0.y, g0.y);
+                            }
                             const double sj = m.sdiag[cj.x], aj = m.area[cj.x];
-                            g0.x = a.omega * fma(-alpha.x, p0.x, g0.x) * rcp_pos(fma(cc.x, sj, aj));
-                            g0.y = a.omega * fma(-alpha.y, p0.y, g0.y) * rcp_pos(fma(cc.y, sj, aj));
+                            g0.x = a.omega * g0.x * rcp_pos(fma(cc.x, sj, aj));
+                            g0.y = a.omega * g0.y * rcp_pos(fma(cc.y, sj, aj));
                         }
                     }
                     if (j1 < (unsigned)nrows) {
@@ -617,10 +657,13 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                             g1.x = fma(beta.x, p1.x, g1.x); g1.y = fma(beta.y, p1.y, g1.y);
                         }
                         if (MGR) {
-                            const double2 p1 = ld2(a.in1, (int64_t)cj.y * K + 2 * l);
+                            if (MGQ) {
+                                const double2 p1 = ld2(a.in1, (int64_t)cj.y * K + 2 * l);
+                                g1.x = fma(-alpha.x, p1.x, g1.x); g1.y = fma(-alpha.y, p1.y, g1.y);
+                            }
                             const double sj = m.sdiag[cj.y], aj = m.area[cj.y];
-                            g1.x = a.omega * fma(-alpha.x, p1.x, g1.x) * rcp_pos(fma(cc.x, sj, aj));
-                            g1.y = a.omega * fma(-alpha.y, p1.y, g1.y) * rcp_pos(fma(cc.y, sj, aj));
+                            g1.x = a.omega * g1.x * rcp_pos(fma(cc.x, sj, aj));
+                            g1.y = a.omega * g1.y * rcp_pos(fma(cc.y, sj, aj));
                         }
                     }
                     s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
@@ -645,12 +688,22 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 if (sub >= 1) {
                     const double2 rv = sb[r * TPR + l];
                     o.x = rv.x - o.x; o.y = rv.y - o.y;                                  // r - A v
+                    if (MGR && a.omega2 != 0.0) {      // second sweep: e2 = e1 + omega2 (r' - K e1)/d
+                        o.x = fma(a.omega2 * o.x, rcp_pos(fma(cc.x, sd, av)), own.x);
+                        o.y = fma(a.omega2 * o.y, rcp_pos(fma(cc.y, sd, av)), own.y);
+                    }
                     if (sub >= 2) {
                         // (rcp_pos as in the first sweep: the same D^-1 on both sides of the cycle, and a fifth of
                         // this kernel's instructions less than two fp64 divisions)
                         o.x = fma(a.omega * o.x, rcp_pos(fma(cc.x, sd, av)), own.x);
                         o.y = fma(a.omega * o.y, rcp_pos(fma(cc.y, sd, av)), own.y);
-                        acc[0].x = fma(rv.x, o.x, acc[0].x);  acc[0].y = fma(rv.y, o.y, acc[0].y);     // r.z
+                        if (sub == 5) {     // y = V r ends the first cycle of B = V M V: rho' = y.M y, w = M y goes on
+                            const double2 wv = {av * o.x, av * o.y};
+                            acc[0].x = fma(wv.x, o.x, acc[0].x);  acc[0].y = fma(wv.y, o.y, acc[0].y);
+                            o = wv;
+                        } else {
+                            acc[0].x = fma(rv.x, o.x, acc[0].x);  acc[0].y = fma(rv.y, o.y, acc[0].y);     // r.z
+                        }
                         acc[MODE == MODE_AX ? 1 : 0].x = fma(rv.x, rv.x, acc[MODE == MODE_AX ? 1 : 0].x);
                         acc[MODE == MODE_AX ? 1 : 0].y = fma(rv.y, rv.y, acc[MODE == MODE_AX ? 1 : 0].y);
                     }
@@ -696,7 +749,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             if (tid < K) {
                 const double pq = tot[tid];
                 double al = 0.0;
-                if (!ctrl->done[tid]) {
+                if (!ctrl->done[tid] && !ctrl->starting[tid]) {   // (a starting column has no direction yet)
                     if (pq > 0.0 && isfinite(pq)) al = ctrl->rho[tid] / pq;
                     else { ctrl->done[tid] = 1; ctrl->status[tid] = 2; }
                 }
@@ -708,7 +761,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
         __shared__ double tot2[2 * KMAX];
         const double2 acc2[2] = {acc[0], acc[MODE == MODE_AX ? 1 : 0]};
         if (grid_reduce<K, 2, NT>(acc2, partials, &ctrl->ticket[2], tot2))
-            cg_bookkeeping<K>(ctrl, tot2, a.scale_inv_area == 4);
+            cg_bookkeeping<K>(ctrl, tot2);
     }
 }
 
@@ -731,8 +784,12 @@ __global__ void __launch_bounds__(BLOCK) k_ingest(MeshView m, StartParams sp, un
 template <int K>
 __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
                                                 StartParams sp, unsigned mask, const double* __restrict__ x,
-                                                const double* __restrict__ y, double* __restrict__ z,
-                                                double* __restrict__ p0, double* __restrict__ p1, int order_n) {
+                                                const double* __restrict__ y, double* __restrict__ z_,
+                                                double* __restrict__ p0, double* __restrict__ p1, int order_n,
+                                                double* __restrict__ r_alt, double* __restrict__ z_clear, int mg) {
+    // multigrid path (mg): the iteration is carried in r, double-buffered: r0 goes to the buffer ctrl->cur_r names,
+    // and the column is marked `starting` (its first iteration applies the preconditioner only)
+    double* __restrict__ z = (mg && ctrl->cur_r) ? r_alt : z_;
     constexpr int TPR = K / 2;
     constexpr int ROWS = BLOCK / TPR;
     const int tid = threadIdx.x, l = tid % TPR;
@@ -750,23 +807,30 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
             const double2 r = {-cc.x * yv.x, -cc.y * yv.y};
             const double2 b = {av * xv.x, av * xv.y};
             if (on0) {
-                zv.x = r.x / d.x; pa.x = 0.0; pb.x = 0.0;
+                zv.x = mg ? r.x : r.x / d.x; pa.x = 0.0; pb.x = 0.0;
                 acc[0].x = fma(r.x, zv.x, acc[0].x); acc[1].x = fma(r.x, r.x, acc[1].x); acc[2].x = fma(b.x, b.x, acc[2].x);
             }
             if (on1) {
-                zv.y = r.y / d.y; pa.y = 0.0; pb.y = 0.0;
+                zv.y = mg ? r.y : r.y / d.y; pa.y = 0.0; pb.y = 0.0;
                 acc[0].y = fma(r.y, zv.y, acc[0].y); acc[1].y = fma(r.y, r.y, acc[1].y); acc[2].y = fma(b.y, b.y, acc[2].y);
             }
             st2(z, ri, zv);
             st2(p0, ri, pa);
             st2(p1, ri, pb);
+            if (z_clear) {   // (multigrid path) the preconditioned residual of a starting column: finite before its first use
+                double2 zc = ld2(z_clear, ri);
+                if (on0) zc.x = 0.0;
+                if (on1) zc.y = 0.0;
+                st2(z_clear, ri, zc);
+            }
         }
     }
     __shared__ double tot[3 * KMAX];
     if (grid_reduce<K, 3>(acc, partials, &ctrl->ticket[1], tot)) {
         if (tid < K && ((mask >> tid) & 1u)) {
             const double rho = tot[tid], rr = tot[KMAX + tid], bb = tot[2 * KMAX + tid];
-            ctrl->c[tid] = sp.c[tid]; ctrl->field[tid] = sp.field[tid]; ctrl->rhs[tid] = sp.rhs[tid];
+            ctrl->c[tid] = sp.c[tid]; ctrl->c1[tid] = sp.c1[tid]; ctrl->field[tid] = sp.field[tid]; ctrl->rhs[tid] = sp.rhs[tid];
+            ctrl->starting[tid] = mg;
             ctrl->rho[tid] = rho; ctrl->rr[tid] = rr; ctrl->bb[tid] = bb;
             ctrl->alpha[tid] = 0.0; ctrl->beta[tid] = 0.0; ctrl->iters[tid] = 0;
             int st = 0;
@@ -969,15 +1033,15 @@ __global__ void __launch_bounds__(BLOCK) k_repack(int64_t nv, ColMap map, const 
 __global__ void k_compact_ctrl(Ctrl* __restrict__ ctrl, ColMap map, int KN) {
     const int j = threadIdx.x;   // one block of KMAX threads
     const int s = j < KN ? map.src[j] : -1;
-    double c = 0.0, al = 0.0, be = 0.0, rho = 0.0, bb = 0.0, rr = 0.0;
+    double c = 0.0, c1 = 0.0, al = 0.0, be = 0.0, rho = 0.0, bb = 0.0, rr = 0.0;
     int field = -1, rhs = 0, done = 1, epoch = 0, status = 0, iters = 0;
     if (s >= 0) {
-        c = ctrl->c[s]; al = ctrl->alpha[s]; be = ctrl->beta[s]; rho = ctrl->rho[s]; bb = ctrl->bb[s]; rr = ctrl->rr[s];
+        c = ctrl->c[s]; c1 = ctrl->c1[s]; al = ctrl->alpha[s]; be = ctrl->beta[s]; rho = ctrl->rho[s]; bb = ctrl->bb[s]; rr = ctrl->rr[s];
         field = ctrl->field[s]; rhs = ctrl->rhs[s]; done = ctrl->done[s]; epoch = ctrl->epoch[s];
         status = ctrl->status[s]; iters = ctrl->iters[s];
     }
     __syncthreads();
-    ctrl->c[j] = c; ctrl->alpha[j] = al; ctrl->beta[j] = be; ctrl->rho[j] = rho; ctrl->bb[j] = bb; ctrl->rr[j] = rr;
+    ctrl->c[j] = c; ctrl->c1[j] = c1; ctrl->starting[j] = 0; ctrl->alpha[j] = al; ctrl->beta[j] = be; ctrl->rho[j] = rho; ctrl->bb[j] = bb; ctrl->rr[j] = rr;
     ctrl->field[j] = field; ctrl->rhs[j] = rhs; ctrl->done[j] = done; ctrl->epoch[j] = epoch;
     ctrl->status[j] = status; ctrl->iters[j] = iters;
     __syncthreads();

@@ -1,16 +1,25 @@
-// Multigrid-preconditioned CG for the n = 1 systems at large scales (included by solve.cu).
+// Multigrid-preconditioned CG for large scales (included by solve.cu).
 //
-//   PCG on (M + c S) x = M phi, x0 = phi, preconditioner B = one V cycle of the smoothed-
-//   aggregation hierarchy of mg.cu with damped Jacobi smoothing (one sweep on the mesh, MG_NU_L1 on level 1,
-//   MG_NU_COARSE on the coarser levels) and a dense Cholesky solve on the coarsest level.
-//   B is symmetric positive definite and fixed per column, so plain PCG applies.  16 columns at a time, every
-//   column with its own c, alpha, beta and stop time.  As in the Jacobi path all CG scalars live in the device
-//   control block: the iteration is
-//       k_spmm<16, CG1>      p' = z + beta p ; x += alpha p ; q = A p' ; alpha' = rho / p'.q         (kernel A)
-//       k_spmm<16, MGR>      r' = r - alpha' q ; e = omega r'/d ; t = r' - A e     (residual update, first sweep of B
-//                            on level 0 and its residual in one pass), then restriction, coarse levels, prolongation
-//       k_spmm<16, AX> sub 3 z = last sweep ; rho' = r.z ; ||r||^2 ; beta ; stop test        (CG bookkeeping)
-//   and the host reads the control block once per iteration to see whether every column has stopped.
+//   n = 1:  PCG on (M + c S) x = M phi, x0 = phi, preconditioner B = V = one V cycle of the smoothed-
+//           aggregation hierarchy of mg.cu for K = M + c S: damped Jacobi smoothing (one sweep on the mesh, MG_NU_L1 on
+//           level 1, MG_NU_COARSE on the coarser levels), dense Cholesky solve on the coarsest level.
+//   n = 2:  PCG on (M + c S M^-1 S) x = M phi with the product preconditioner B = V M V, V = the same V cycle for
+//           K = M + mu S, mu = sqrt(c):  K M^-1 K = M + 2 mu S + c S M^-1 S, and for every eigenvalue lambda of M^-1 S
+//           1 <= (1 + mu lambda)^2 / (1 + c lambda^2) <= 2, so with exact inner solves the condition number is <= 2
+//           (PAPER.md:207 names the loss of convergence of the biharmonic filter at large l as the open problem).
+//   V is a fixed symmetric positive definite operator per column (fixed sweep counts, the same damping before and
+//   after the coarse correction), hence so are B = V and B = V M V, and plain PCG applies.
+// 16 columns at a time, every column with its own c, alpha, beta and stop time; all per-column scalars live in the
+// device control block (Ctrl), so ONE iteration is a fixed launch sequence, captured in a CUDA graph by solve.cu:
+//       k_spmm<16, CG1>  (n = 2: CG2A, CG2B)   p' = z + beta p ; x += alpha p ; q = A p' ; alpha' = rho / p'.q
+//       k_spmm<16, MGR>      r' = r - alpha' q ; e = omega r'/d ; t = r' - K e    (residual update, first sweep of V on
+//                            level 0 and its residual in one pass), then restriction, coarse levels, prolongation
+//       k_spmm<16, AX> sub 3 z = last sweep ; rho' = r'.z ; ||r'||^2 ; beta ; stop test      (CG bookkeeping)
+//   n = 2: the last sweep of the first cycle is sub 5 (y = V r', w = M y, rho' = y.w, bookkeeping), then a second
+//   cycle on w (k_spmm<16, MGR0>, transfers, coarse levels, sub 2) gives z = V w.
+// A (re)started column (Ctrl::starting, set by k_init) joins at an iteration boundary: its first iteration has alpha = 0
+// and ends with rho = r0.z0, beta = 0 -- the start of PCG -- so columns are refilled from the queue as in the Jacobi
+// path and the host never waits inside the loop.
 // The stop test is the same as in the Jacobi path: recursive ||r||_2 <= tol ||M phi||_2.
 #pragma once
 
@@ -18,6 +27,13 @@ namespace ifl {
 namespace {
 
 constexpr int MGK = 16;               // columns of the multigrid path
+constexpr int MG_REFILL_MIN = 4;      // stopped columns wait until this many can be restarted together (solve.cu)
+// right-hand sides below this many mean edge lengths stay on the Jacobi path (option mg_min_ell = 0)
+constexpr double MG_MIN_ELL_N1 = 4.0;
+constexpr double MG_MIN_ELL_N2 = 0.5;
+// n = 2: sweeps per side of the cycle on the mesh and on level 1 (Chebyshev-root dampings, mg_omegas)
+constexpr int MG_NU0_N2 = 4;
+constexpr int MG_NU1_N2 = 2;
 constexpr int MG_UB = 4;              // matrix entries a thread has in flight in the CSR kernels of the hierarchy
 #ifndef IF_MG_BPS
 #define IF_MG_BPS 6                   // blocks per SM of the CSR kernels (what their registers allow: one full wave)
@@ -28,12 +44,6 @@ constexpr int MG_UB = 4;              // matrix entries a thread has in flight i
 #ifndef IF_MG_WIDE
 #define IF_MG_WIDE 24                 // mean row length from which a row is split over four entry slices
 #endif
-
-struct MgCols {                       // per-column scalars, passed by value
-    double c[MGK];
-    double a[MGK];
-    double b[MGK];
-};
 
 struct MgMat {                        // one level's (S, M) pair
     const int64_t* __restrict__ rowptr;
@@ -49,11 +59,12 @@ struct MgMat {                        // one level's (S, M) pair
 // whose rows have hundreds of entries and would otherwise be walked serially.
 // MODE 0: y = A x ;  MODE 1: y = r - A x ;  MODE 2: y = x + omega (r - A x) / d        with A = M + c S per column
 template <int MODE, int SL>
-__global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, MgCols cs, const double* __restrict__ x,
+__global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ x,
                                                     const double* __restrict__ r, double* __restrict__ y) {
     constexpr int WPB = BLOCK / (8 * SL);
     const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
-    const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
+    if (ctrl->all_done) return;
+    const double2 cc = ld2(ctrl->c1, 2 * l);
     // (rows are padded to whole warps by the loop bound: every lane of a warp takes part in the shuffles)
     // a block walks a contiguous range of rows, WPB at a time: neighbouring rows gather the same rows of x, which
     // the L1 then serves (a grid-stride assignment sends every gather to the L2)
@@ -103,12 +114,13 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, MgCols 
 }
 
 // e = omega r / d  (Jacobi sweep from a zero initial guess)
-__global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, MgCols cs, const double* __restrict__ r,
+__global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ r,
                                                       double* __restrict__ e) {
     constexpr int TPR = MGK / 2;
     constexpr int ROWS = BLOCK / TPR;
     const int l = threadIdx.x % TPR;
-    const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
+    if (ctrl->all_done) return;
+    const double2 cc = ld2(ctrl->c1, 2 * l);
     for (int64_t row = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; row < g.n; row += (int64_t)gridDim.x * ROWS) {
         const int64_t ri = row * MGK + 2 * l;
         const double2 d = g.diag[row];
@@ -121,8 +133,10 @@ __global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, MgCols cs, const 
 template <int ACC, int SL>
 __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                                                   const double* __restrict__ val, int64_t n,
-                                                  const double* __restrict__ x, double* __restrict__ y) {
+                                                  const Ctrl* __restrict__ ctrl, const double* __restrict__ x,
+                                                  double* __restrict__ y) {
     constexpr int WPB = BLOCK / (8 * SL);
+    if (ctrl->all_done) return;
     const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
     const int64_t per_block = ((n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;   // contiguous rows per block
     const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, (n + 3) / 4 * 4);
@@ -162,12 +176,16 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __r
 // prolongator has 2.6 entries per row).  k_spmm<16, MGR> then does not store its e = omega r'/d, and this kernel
 // reads r' where k_mg_csr<1, 1> would read e back: one pass over a [V][16] vector less per iteration.
 __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_prolong0(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
-                                                       const double* __restrict__ val, MgMat g, MgCols cs,
-                                                       const double* __restrict__ x, const double* __restrict__ r,
+                                                       const double* __restrict__ val, MgMat g, const Ctrl* __restrict__ ctrl,
+                                                       const double* __restrict__ x, const double* __restrict__ r0,
+                                                       const double* __restrict__ r1, int r_select,
                                                        double* __restrict__ y) {
     constexpr int WPB = BLOCK / 8;
+    // r_select: the residual k_spmm<16, MGR> has just written, r[cur_r ^ 1] of the double buffer (r0, r1); else r0
+    const double* __restrict__ r = r_select ? (ctrl->cur_r ? r0 : r1) : r0;
     const int l = threadIdx.x % 8;
-    const double2 cc = {cs.c[2 * l], cs.c[2 * l + 1]};
+    if (ctrl->all_done) return;
+    const double2 cc = ld2(ctrl->c1, 2 * l);
     const int64_t n = g.n;
     const int64_t per_block = ((n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;   // contiguous rows per block
     const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, n);
@@ -204,11 +222,12 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_prolong0(const int64_t
 }
 
 // coarsest level: dense Cholesky of A = M + c S per column (one block per column), then the two triangular solves
-__global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, MgCols cs, const double* __restrict__ r, double* __restrict__ e) {
+__global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ r, double* __restrict__ e) {
     __shared__ double a[MG_COARSEST][MG_COARSEST + 1];
     __shared__ double v[MG_COARSEST];
     const int c = blockIdx.x, t = threadIdx.x, n = (int)g.n;
-    const double cc = cs.c[c];
+    if (ctrl->all_done) return;
+    const double cc = ctrl->c1[c];
     for (int i = t; i < n; i += 64) {
         for (int j = 0; j < n; ++j) a[i][j] = 0.0;
         v[i] = r[(int64_t)i * MGK + c];
@@ -242,83 +261,32 @@ __global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, MgCols cs, const doub
     for (int i = t; i < n; i += 64) e[(int64_t)i * MGK + c] = v[i];
 }
 
-// ---- PCG vector kernels on [row][16]
-// out = area * x
-__global__ void __launch_bounds__(BLOCK) k_mg_mass(const double* __restrict__ area, int64_t n, const double* __restrict__ x,
-                                                   double* __restrict__ out) {
-    constexpr int TPR = MGK / 2;
-    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
-    if (i >= n * TPR) return;
-    const double av = area[i / TPR];
-    const double2 xv = ld2(x, 2 * i);
-    st2(out, 2 * i, make_double2(av * xv.x, av * xv.y));
-}
-// per-block partial sums of a.b and a.c per column (fixed order); k_mg_dot_final adds the blocks in order
-__global__ void __launch_bounds__(BLOCK) k_mg_dot(int64_t n, const double* __restrict__ a, const double* __restrict__ b,
-                                                  const double* __restrict__ c, double* __restrict__ partials) {
-    constexpr int TPR = MGK / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    __shared__ double2 red[2][BLOCK];
-    const int tid = threadIdx.x, l = tid % TPR;
-    double2 s0 = {0.0, 0.0}, s1 = {0.0, 0.0};
-    for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < n; row += (int64_t)gridDim.x * ROWS) {
-        const int64_t ri = row * MGK + 2 * l;
-        const double2 av = ld2(a, ri), bv = ld2(b, ri), cv = ld2(c, ri);
-        s0.x = fma(av.x, bv.x, s0.x); s0.y = fma(av.y, bv.y, s0.y);
-        s1.x = fma(av.x, cv.x, s1.x); s1.y = fma(av.y, cv.y, s1.y);
-    }
-    red[0][tid] = s0;
-    red[1][tid] = s1;
-    __syncthreads();
-    if (tid < 2 * TPR) {
-        const int j = tid / TPR, ll = tid % TPR;
-        double2 s = red[j][ll];
-        for (int i = ll + TPR; i < BLOCK; i += TPR) { s.x += red[j][i].x; s.y += red[j][i].y; }
-        partials[((size_t)blockIdx.x * 2 + j) * MGK + 2 * ll] = s.x;
-        partials[((size_t)blockIdx.x * 2 + j) * MGK + 2 * ll + 1] = s.y;
-    }
-}
-__global__ void k_mg_dot_final(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
-    const int t = threadIdx.x;   // 2 * MGK threads
-    if (t >= 2 * MGK) return;
-    double s = 0.0;
-    for (int b = 0; b < nblocks; ++b) s += partials[(size_t)b * 2 * MGK + t];
-    out[t] = s;
-}
-
 // ------------------------------------------------------------------------------------------- host side
 struct MgBuffers {
     double *x, *r[2], *p[2], *q, *za, *zb, *t;  // level 0, [n][16]; r is double-buffered (k_spmm<16, MGR>)
     double* lev[MG_MAX_LEVELS][4];              // levels >= 1: R, E, T, E2
-    double* partials;                           // [grid][2][16]
-    double* dots;                               // [32]
-    int dot_grid;
-    int ax_grid;                                // persistent grid of k_spmm<16, MODE_AX> (level-0 operator)
 };
 
-inline size_t mg_extra_bytes(const if_mesh_s* h) {
+// level-0 vectors beyond the Jacobi workspace: za (e), zb (z), the second r; for n = 1 also t (the n = 2 workspace has one)
+inline size_t mg_extra_bytes(const if_mesh_s* h, int order_n) {
     if (h->mg_levels < 2) return 0;
-    size_t b = 4 * align_up((size_t)h->n_vert * MGK * sizeof(double));        // za, zb, t, second r (level-0 vectors 6 to 9)
+    size_t b = (order_n == 1 ? 4 : 3) * align_up((size_t)h->n_vert * MGK * sizeof(double));
     for (int l = 1; l < h->mg_levels; ++l) b += 4 * align_up((size_t)h->mg[l].n * MGK * sizeof(double));
-    b += align_up((size_t)h->n_sm * 4 * 2 * MGK * sizeof(double)) + align_up(2 * MGK * sizeof(double));
     return b;
 }
 
-inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, void* extra) {
+inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, int order_n) {
     MgBuffers m{};
     m.x = w.x; m.r[0] = w.z; m.p[0] = w.p0; m.p[1] = w.p1; m.q = w.q;
-    char* p = static_cast<char*>(extra);
+    char* p = static_cast<char*>(w.mg_extra);
     size_t off = 0;
     auto take = [&](size_t bytes) { void* r = p + off; off += align_up(bytes); return r; };
     m.za = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
     m.zb = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
-    m.t = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
     m.r[1] = (double*)take((size_t)h->n_vert * MGK * sizeof(double));
+    m.t = order_n == 1 ? (double*)take((size_t)h->n_vert * MGK * sizeof(double)) : w.t;
     for (int l = 1; l < h->mg_levels; ++l)
         for (int k = 0; k < 4; ++k) m.lev[l][k] = (double*)take((size_t)h->mg[l].n * MGK * sizeof(double));
-    m.dot_grid = h->n_sm * 4;
-    m.partials = (double*)take((size_t)m.dot_grid * 2 * MGK * sizeof(double));
-    m.dots = (double*)take(2 * MGK * sizeof(double));
     return m;
 }
 
@@ -330,21 +298,48 @@ inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
     return (int)std::max<int64_t>(1, std::min<int64_t>((n + rows - 1) / rows, (int64_t)h->n_sm * IF_MG_BPS));
 }
 
-// One V cycle on level l: e = B_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
-// nu = 1 on level 0, MG_NU_L1 on level 1 and MG_NU_COARSE below.  R holds r and is not changed; E, T, E2 are work buffers of the
+// groups of the per-kernel timing (if_stats.mg_kernel_seconds)
+enum { MGT_A = 0, MGT_MGR = 1, MGT_RESTRICT0 = 2, MGT_LEVEL1 = 3, MGT_COARSE = 4, MGT_PROLONG0 = 5, MGT_LAST = 6 };
+
+int mg_setup(Run& r) {
+    const if_mesh_s* h = r.h;
+    const int64_t tiles = (h->n_vert + TILE_ROWS - 1) / TILE_ROWS;
+    int rc;
+    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK>::NT))) return rc;
+    if (r.order_n == 2 &&
+        (rc = resident_grid(k_spmm<MGK, MODE_MGR0>, TileSmem<MGK, MODE_MGR0>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<MGK>::NT))) return rc;
+    return IF_OK;
+}
+
+// Damping of the Jacobi sweeps of a level.  One sweep: omega = min(MG_OMEGA_MAX, 1.6 / rho), rho = max(rho(D_S^-1 S),
+// rho(D_M^-1 M)) (mg.cu).  k >= 2 sweeps: the reciprocals of the roots of the Chebyshev polynomial of degree k on
+// [rho / 4, rho] -- the same number of passes, but the product of the k factors (1 - omega_j t) is 1 / T_k(5/3) on the
+// upper three quarters of the spectrum (0.22, 0.074, 0.025 for k = 2, 3, 4) where k equal sweeps give 0.6^k, and stays
+// below 1 in modulus on (0, rho]: the smoother contracts, the cycle stays symmetric positive definite.
+inline void mg_omegas(const MgLevel& g, int k, double* om) {
+    if (k <= 1) { om[0] = g.omega; return; }
+    const double rho = std::max(g.rho, g.rho_m), lo = rho / 4.0;
+    const double c = 0.5 * (rho + lo), hw = 0.5 * (rho - lo);
+    for (int j = 0; j < k; ++j) om[j] = 1.0 / (c + hw * std::cos(M_PI * (2 * j + 1) / (2.0 * k)));
+}
+constexpr int MG_MAX_NU = 8;
+
+// Levels >= 1 of a V cycle: e = V_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
+// nu = r.mg_nu[1] on level 1 and r.mg_nu[2] below.  R holds r and is not changed; E, T, E2 are work buffers of the
 // level; *result is the one that holds e.
-// On level 0 the caller may have done the first sweep and its residual already (first_done: E = omega r / d,
-// T = r - A E, both by k_spmm<16, MGR>) and chooses the sub-mode of the last sweep (final_sub 3 / 4: with the CG
-// bookkeeping, see kernels.cuh).
-int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double* R, double* E, double* T, double* E2,
-              double** result, int final_sub = 2, bool first_done = false) {
+int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, double* T, double* E2, double** result,
+              IterTimer* tm) {
     const if_mesh_s* h = r.h;
     const MgLevel& g = h->mg[l];
-    const MgMat gm = mg_mat(g);
+    MgMat gm = mg_mat(g);
+    const Ctrl* ctrl = r.w.ctrl;
     const bool last = l == h->mg_levels - 1;
+    int rc;
     if (last && g.n <= MG_COARSEST) {
-        k_mg_coarse<<<MGK, 64, 0, r.st>>>(gm, cs, R, E);
+        k_mg_coarse<<<MGK, 64, 0, r.st>>>(gm, ctrl, R, E);
         IF_LAUNCH_CHECK();
+        if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
         *result = E;
         return IF_OK;
     }
@@ -352,159 +347,156 @@ int mg_vcycle(const Run& r, const MgBuffers& b, const MgCols& cs, int l, double*
     const bool wide = g.nnz >= IF_MG_WIDE * g.n;
     const int grid1 = mg_grid(h, g.n);
     const int grid = mg_grid(h, g.n, wide ? 4 : 1);
-    // sub 1: out = rr - A v ;  sub 2: out = v + omega (rr - A v) / d      (level 0: the tiled TMA kernel)
-    auto apply = [&](int sub, const double* v, double* out) -> int {
-        if (l == 0) {
-            SpmmArgs a{v, R, nullptr, out, nullptr, sub, 0, g.omega};
-            return launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a);
-        }
+    // sub 1: out = R - K v ;  sub 2: out = v + omega (R - K v) / d
+    auto apply = [&](int sub, double omega, const double* v, double* out) -> int {
+        gm.omega = omega;
         if (sub == 1) {
-            if (wide) k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
-            else k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
+            if (wide) k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
+            else k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
         } else {
-            if (wide) k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
-            else k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, cs, v, R, out);
+            if (wide) k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
+            else k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
         }
         IF_LAUNCH_CHECK();
         return IF_OK;
     };
     // a coarsest level too large for the dense solve (coarsening stalled): smoothing only
-    const int nu = last ? 4 * MG_NU_COARSE : (l == 0 ? 1 : (l == 1 ? MG_NU_L1 : MG_NU_COARSE));
-    int rc;
+    const int nu = std::min(MG_MAX_NU, last ? 4 * r.mg_nu[2] : r.mg_nu[l == 1 ? 1 : 2]);
+    double om[MG_MAX_NU];
+    mg_omegas(g, nu, om);
+    if (nu >= 2 && nu == r.mg_nu[l == 1 ? 1 : 2] && r.order_n == 1)
+        for (int j = 0; j < nu; ++j) om[j] = g.omega;      // n = 1: equal sweeps, as tuned
     double* cur = E;
     double* spare[2] = {E2, T};
-    if (!(l == 0 && first_done)) {
-        k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, cs, R, cur);
-        IF_LAUNCH_CHECK();
-    }
+    gm.omega = om[0];
+    k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, ctrl, R, cur);
+    IF_LAUNCH_CHECK();
     for (int k = 1; k < nu; ++k) {
-        if ((rc = apply(2, cur, spare[0]))) return rc;
+        if ((rc = apply(2, om[k], cur, spare[0]))) return rc;
         std::swap(cur, spare[0]);
     }
-    if (last) { *result = cur; return IF_OK; }
-    if (!(l == 0 && first_done && nu == 1))
-        if ((rc = apply(1, cur, spare[1]))) return rc;                // residual of the level
+    if (last) {
+        if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
+        *result = cur;
+        return IF_OK;
+    }
+    if ((rc = apply(1, 0.0, cur, spare[1]))) return rc;                // residual of the level
     double* const* nb = b.lev[l + 1];
     const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse, wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
-    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, spare[1], nb[0]);
-    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, spare[1], nb[0]);
+    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, spare[1], nb[0]);
+    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, spare[1], nb[0]);
     IF_LAUNCH_CHECK();
+    if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
     double* ec = nullptr;
-    if ((rc = mg_vcycle(r, b, cs, l + 1, nb[0], nb[1], nb[2], nb[3], &ec))) return rc;
-    if (l == 0 && first_done && nu == 1 && mg_fused_prolongation(g))   // cur = omega R / d has not been stored
-        k_mg_prolong0<<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, gm, cs, ec, R, cur);
-    else if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
-    else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ec, cur);
+    if ((rc = mg_vcycle(r, b, l + 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
+    if (l == 1 && tm && (rc = tm->mark(r.st, MGT_COARSE))) return rc;
+    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
+    else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
     IF_LAUNCH_CHECK();
     for (int k = 0; k < nu; ++k) {
-        if ((rc = apply((l == 0 && k == nu - 1) ? final_sub : 2, cur, spare[k & 1]))) return rc;
+        if ((rc = apply(2, om[nu - 1 - k], cur, spare[k & 1]))) return rc;
         std::swap(cur, spare[k & 1]);
     }
+    if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
     *result = cur;
     return IF_OK;
 }
 
-// host copies of (a.b, a.c) per column
-int mg_dots(const Run& r, const MgBuffers& b, const double* a, const double* bb, const double* cc, double* h_out /*[32] pinned*/) {
-    k_mg_dot<<<b.dot_grid, BLOCK, 0, r.st>>>(r.h->n_vert, a, bb, cc, b.partials);
+// Level 0 of one V cycle.  `first` (k_spmm<16, MGR | MGR0>) has done the first sweep from a zero guess on the way:
+//   one sweep per side (nu0 = 1): it left t = R - K e in b.t and did not store e = omega R/d -- the prolongation
+//       kernel forms it again (unless the prolongator is too wide for that kernel; then e is in b.za);
+//   nu0 >= 2: it left the SECOND sweep e2 in b.za; the other sweeps and the residual follow here.
+// Then restriction, coarse levels, prolongation, nu0 sweeps, the last one with sub-mode `final_sub` into `out`.
+// R is (R0, R1) picked on the device (r_select, see SpmmArgs) or R0.  Work buffers: b.za, b.zb, b.t (and out, which
+// is only written by the last sweep).
+int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const double* R1, int r_select, double* out,
+                    int final_sub, IterTimer* tm) {
+    const if_mesh_s* h = r.h;
+    const MgLevel& g = h->mg[0];
+    const Ctrl* ctrl = r.w.ctrl;
+    const int nu = r.mg_nu[0];
+    double om[MG_MAX_NU];
+    mg_omegas(g, nu, om);
+    int rc;
+    auto sweep = [&](int sub, double omega, const double* v, double* dst) -> int {
+        SpmmArgs a{v, R0, const_cast<double*>(R1), dst, nullptr, sub, 0, omega, 0.0, r_select};
+        return launch_spmm<MGK, MODE_AX>(r, r.mgg.ax, a);
+    };
+    double* cur = b.za;
+    if (nu >= 2) {
+        double* other = b.zb;
+        for (int k = 2; k < nu; ++k) {
+            if ((rc = sweep(2, om[k], cur, other))) return rc;
+            std::swap(cur, other);
+        }
+        if ((rc = sweep(1, 0.0, cur, b.t))) return rc;                 // residual after the sweeps
+        if (tm && (rc = tm->mark(r.st, MGT_LAST))) return rc;
+    }
+    double* const* nb = b.lev[1];
+    const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse, wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
+    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, b.t, nb[0]);
+    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, b.t, nb[0]);
     IF_LAUNCH_CHECK();
-    k_mg_dot_final<<<1, 2 * MGK, 0, r.st>>>(b.partials, b.dot_grid, b.dots);
+    if (tm && (rc = tm->mark(r.st, MGT_RESTRICT0))) return rc;
+    double* ec = nullptr;
+    if ((rc = mg_vcycle(r, b, 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
+    if (nu == 1 && mg_fused_prolongation(g))      // e = omega R/d formed again here: it has not been stored
+        k_mg_prolong0<<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, mg_mat(g), ctrl, ec, R0, R1, r_select, cur);
+    else if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
+    else k_mg_csr<1, 1><<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
     IF_LAUNCH_CHECK();
-    IF_CUDA_TRY(cudaMemcpyAsync(h_out, b.dots, 2 * MGK * sizeof(double), cudaMemcpyDeviceToHost, r.st));
-    IF_CUDA_TRY(cudaStreamSynchronize(r.st));
+    if (tm && (rc = tm->mark(r.st, MGT_PROLONG0))) return rc;
+    // sweeps after the correction, dampings in reverse order (the cycle is symmetric); scratch: za, zb, t minus `out`
+    for (int k = 0; k < nu - 1; ++k) {
+        double* dst = nullptr;
+        for (double* cand : {b.za, b.t, b.zb})
+            if (cand != cur && cand != out) { dst = cand; break; }
+        if ((rc = sweep(2, om[nu - 1 - k], cur, dst))) return rc;
+        cur = dst;
+    }
+    if ((rc = sweep(final_sub, om[0], cur, out))) return rc;
+    if (tm && (rc = tm->mark(r.st, MGT_LAST))) return rc;
     return IF_OK;
 }
 
-// Up to 16 right-hand sides rhs[first .. first+count) by multigrid-preconditioned CG; results are finalised like in
-// the Jacobi path (energy or scatter, per-RHS stats).
-int mg_solve_batch(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, size_t first, size_t count,
-                   int n_ells, double* d_out, void* mg_extra, double* h_dots /*pinned [32]*/, int64_t* iters_total) {
+// ONE iteration of multigrid-preconditioned CG for the 16 columns (see the head of this file); every pointer that
+// alternates between iterations is picked on the device, so the sequence is the same every time (CUDA graph).
+int mg_enqueue_iteration(const Run& r, IterTimer* tm) {
     const if_mesh_s* h = r.h;
-    const int64_t nv = h->n_vert;
+    const MgBuffers b = mg_layout(h, r.w, r.order_n);
+    const int nu = r.mg_nu[0];
+    double om[MG_MAX_NU];
+    mg_omegas(h->mg[0], nu, om);
+    // what the fused first-sweep kernel leaves behind (see mg_cycle_level0)
+    double* e_store = (nu == 1 && !mg_fused_prolongation(h->mg[0])) ? b.za : nullptr;
+    double* first_out = nu >= 2 ? b.za : b.t;
+    const double omega2 = nu >= 2 ? om[1] : 0.0;
     int rc;
-    MgBuffers b = mg_layout(h, r.w, mg_extra);
-    Ctrl hc = fresh_ctrl(r);
-    StartParams sp;
-    MgCols cs;
-    memset(&sp, 0, sizeof(sp));
-    memset(&cs, 0, sizeof(cs));
-    for (int c = 0; c < KMAX; ++c) sp.field[c] = -1;
-    for (size_t i = 0; i < count; ++i) {
-        const Rhs& q = rhs[first + i];
-        cs.c[i] = sp.c[i] = hc.c[i] = r.opt.gamma * q.ell * q.ell;
-        sp.field[i] = hc.field[i] = q.f;
-        sp.rhs[i] = hc.rhs[i] = q.f * n_ells + q.j;
+    if (tm && (rc = tm->mark(r.st, -1))) return rc;
+    if (r.order_n == 1) {
+        SpmmArgs a{b.zb, b.p[0], b.x, b.q, b.p[1], 0, 1, 0.0, 0.0, 0};          // kernel A of the Jacobi path
+        if ((rc = launch_spmm<MGK, MODE_CG1>(r, r.g.cga, a))) return rc;
+    } else {
+        SpmmArgs a{b.zb, b.p[0], b.x, b.t, b.p[1], 0, 1, 0.0, 0.0, 0};
+        if ((rc = launch_spmm<MGK, MODE_CG2A>(r, r.g.cga, a))) return rc;
+        SpmmArgs c{b.t, b.p[0], nullptr, b.q, b.p[1], 0, 1, 0.0, 0.0, 0};
+        if ((rc = launch_spmm<MGK, MODE_CG2B>(r, r.g.cgb, c))) return rc;
     }
-    const int64_t tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
-    int cg_grid = 0;
-    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &b.ax_grid,
-                            SpmmCfg<MGK>::NT))) return rc;
-    if ((rc = resident_grid(k_spmm<MGK, MODE_CG1>, TileSmem<MGK, MODE_CG1>::bytes, h->n_sm, tiles, &cg_grid,
-                            SpmmCfg<MGK>::NT))) return rc;
-    hc.all_done = 0;   // k_spmm reads c from the control block and returns at once when all_done is set
-    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
-    const unsigned eg = (unsigned)((nv * MGK + BLOCK - 1) / BLOCK);
-    const unsigned vg = (unsigned)((nv * (MGK / 2) + BLOCK - 1) / BLOCK);
-    const MgMat g0 = mg_mat(h->mg[0]);
-    k_ingest<MGK><<<eg, BLOCK, 0, r.st>>>(r.m, sp, 0xffffu, d_fields, b.x);
-    IF_LAUNCH_CHECK();
-    k_mg_mass<<<vg, BLOCK, 0, r.st>>>(h->area, nv, b.x, b.za);               // b = M phi
-    IF_LAUNCH_CHECK();
-    int mgr_grid = 0;
-    if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &mgr_grid,
-                            SpmmCfg<MGK>::NT))) return rc;
+    if (tm && (rc = tm->mark(r.st, MGT_A))) return rc;
     {
-        SpmmArgs a{b.x, b.za, nullptr, b.r[0], nullptr, 1, 0, 0.0};           // r = b - A x0
-        if ((rc = launch_spmm<MGK, MODE_AX>(r, b.ax_grid, a))) return rc;
+        SpmmArgs a{b.r[0], b.q, b.r[1], first_out, e_store, 0, 0, om[0], omega2, 1};
+        if ((rc = launch_spmm<MGK, MODE_MGR>(r, r.mgg.mgr, a))) return rc;
     }
-    IF_CUDA_TRY(cudaMemsetAsync(b.p[0], 0, (size_t)nv * MGK * sizeof(double), r.st));
-    IF_CUDA_TRY(cudaMemsetAsync(b.p[1], 0, (size_t)nv * MGK * sizeof(double), r.st));
-    if ((rc = mg_dots(r, b, b.za, b.za, b.za, h_dots))) return rc;            // ||M phi||^2 (host sync)
-    // the control block of the batch: unused columns stay done, the others start with rho, beta set by the first
-    // preconditioner application (sub-mode 4)
-    for (int c = 0; c < MGK; ++c) {
-        hc.bb[c] = h_dots[c];
-        hc.done[c] = (size_t)c < count ? 0 : 1;
+    if (tm && (rc = tm->mark(r.st, MGT_MGR))) return rc;
+    if (r.order_n == 1) return mg_cycle_level0(r, b, b.r[0], b.r[1], 1, b.zb, 3, tm);
+    // n = 2: y = V r', w = M y (into q, dead by now), bookkeeping with rho' = y.w; then z = V w
+    if ((rc = mg_cycle_level0(r, b, b.r[0], b.r[1], 1, b.q, 5, tm))) return rc;
+    {
+        SpmmArgs a{b.q, nullptr, nullptr, first_out, e_store, 0, 0, om[0], omega2, 0};
+        if ((rc = launch_spmm<MGK, MODE_MGR0>(r, r.mgg.mgr0, a))) return rc;
     }
-    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
-    double* z = nullptr;
-    if ((rc = mg_vcycle(r, b, cs, 0, b.r[0], b.za, b.t, b.zb, &z, 4, false))) return rc;
-    int* h_flag = reinterpret_cast<int*>(h_dots);
-    auto all_done = [&](bool* out) -> int {
-        IF_CUDA_TRY(cudaMemcpyAsync(h_flag, &r.w.ctrl->all_done, sizeof(int), cudaMemcpyDeviceToHost, r.st));
-        IF_CUDA_TRY(cudaStreamSynchronize(r.st));
-        *out = *h_flag != 0;
-        return IF_OK;
-    };
-    bool stop = false;
-    if ((rc = all_done(&stop))) return rc;
-    int64_t loops = 0;
-    int cr = 0;
-    while (!stop) {
-        {
-            SpmmArgs a{z, b.p[0], b.x, b.q, b.p[1], 0, 1, 0.0};  // kernel A of the Jacobi path
-            if ((rc = launch_spmm<MGK, MODE_CG1>(r, cg_grid, a))) return rc;
-        }
-        {
-            SpmmArgs a{b.r[cr], b.q, b.r[cr ^ 1], b.t, mg_fused_prolongation(h->mg[0]) ? nullptr : b.za, 0, 0, g0.omega};
-            if ((rc = launch_spmm<MGK, MODE_MGR>(r, mgr_grid, a))) return rc;
-        }
-        cr ^= 1;
-        if ((rc = mg_vcycle(r, b, cs, 0, b.r[cr], b.za, b.t, b.zb, &z, 3, true))) return rc;
-        ++loops;
-        if ((rc = all_done(&stop))) return rc;
-    }
-    *iters_total += loops;
-    if (getenv("IF_VERBOSE"))
-        fprintf(stderr, "[implicit_filter] multigrid batch: largest scale %.4g, %zu columns, %lld iterations\n",
-                rhs[first].ell, count, (long long)loops);
-    // the columns are finalised from the device control block (pending alpha p included, as in the Jacobi path)
-    Run fr = r;
-    fr.w.x = b.x;
-    fr.g.stream = (int)std::max<int64_t>(1, std::min<int64_t>((nv + 31) / 32, (int64_t)h->n_sm * 4));
-    if ((rc = finalize_columns<MGK>(fr, job, (count >= 16 ? 0xffffu : ((1u << count) - 1u)), d_out, d_fields))) return rc;
-    IF_CUDA_TRY(cudaStreamSynchronize(r.st));   // hc lives on this stack frame
-    return IF_OK;
+    if (tm && (rc = tm->mark(r.st, MGT_MGR))) return rc;
+    return mg_cycle_level0(r, b, b.q, nullptr, 0, b.zb, 2, tm);
 }
 
 }  // namespace

@@ -371,7 +371,8 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
     if ((o.sell_c != 32 && o.sell_c != 64 && o.sell_c != 128) || TILE_ROWS % o.sell_c != 0) return IF_EINVAL;   // must divide the SpMM row tile
     if (o.sell_sigma < o.sell_c || o.sell_sigma % o.sell_c != 0) return IF_EINVAL;
     if (o.sfc_kind != 0 && o.sfc_kind != 1) return IF_EINVAL;
-    if ((o.solver != 0 && o.solver != 1) || !(o.mg_min_ell > 0.0)) return IF_EINVAL;
+    if (o.solver == 2) o.solver = 0;   // 2 = Jacobi-PCG explicitly (a per-call 0 inherits the handle's choice)
+    if ((o.solver != 0 && o.solver != 1) || !(o.mg_min_ell >= 0.0) || !std::isfinite(o.mg_min_ell)) return IF_EINVAL;
     *out = o;
     return IF_OK;
 }

@@ -26,7 +26,7 @@ struct Workspace {
 };
 
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
-inline size_t mg_extra_bytes(const if_mesh_s* h);   // mg_solve.cuh
+inline size_t mg_extra_bytes(const if_mesh_s* h, int order_n);   // mg_solve.cuh (included below)
 
 Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* base) {
     Workspace w{};
@@ -51,7 +51,7 @@ Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* bas
     w.iters = (int32_t*)take(MAX_RHS * sizeof(int32_t));
     w.status = (int32_t*)take(MAX_RHS * sizeof(int32_t));
     w.mg_extra = nullptr;
-    if (order_n == 1 && batch == KMAX && h->mg_levels > 1) w.mg_extra = take(mg_extra_bytes(h));
+    if (batch == KMAX && h->mg_levels > 1) w.mg_extra = take(mg_extra_bytes(h, order_n));
     w.bytes = off;
     return w;
 }
@@ -62,6 +62,7 @@ struct Rhs { double ell; int f; int j; };
 
 // persistent grids: one wave of resident blocks, sized from the real occupancy of each kernel
 struct Grids { int plain, cga, cgb, update, stream; };
+struct MgGrids { int ax = 0, mgr = 0, mgr0 = 0; };   // level-0 kernels of the multigrid cycle
 
 struct Run {
     const if_mesh_s* h;
@@ -71,6 +72,9 @@ struct Run {
     int order_n;
     Options opt;
     Grids g;
+    bool mg = false;   // this phase runs multigrid-preconditioned CG (mg_solve.cuh) instead of Jacobi-PCG
+    MgGrids mgg;
+    int mg_nu[3] = {1, 1, 2};   // Jacobi sweeps per side of the V cycle on the mesh, on level 1, below (mg_solve.cuh)
 };
 
 template <class Kern>
@@ -114,30 +118,44 @@ int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
     return IF_OK;
 }
 
-// Events recorded (as external event-record nodes) around one SpMM and one update launch of a captured graph,
-// so that the per-launch duration of both kernels is measured live on the launching stream (if_stats).
-struct TimingEvents {
-    cudaEvent_t s0 = nullptr, s1 = nullptr, u1 = nullptr;   // before SpMM, after SpMM (= before update), after update
+// Events recorded (as external event-record nodes) between the kernel groups of ONE iteration of a captured graph, so
+// that the per-launch duration of every group is measured live on the launching stream (if_stats).  mark(g) closes an
+// interval that belongs to group g (the first mark only opens one).
+constexpr int TIMER_GROUPS = 8;
+struct IterTimer {
+    static constexpr int MAXE = 40;
+    cudaEvent_t ev[MAXE] = {};
+    int gid[MAXE] = {};
+    int n = 0, created = 0;
     int create() {
-        IF_CUDA_TRY(cudaEventCreate(&s0));
-        IF_CUDA_TRY(cudaEventCreate(&s1));
-        IF_CUDA_TRY(cudaEventCreate(&u1));
+        for (created = 0; created < MAXE; ++created) IF_CUDA_TRY(cudaEventCreate(&ev[created]));
         return IF_OK;
     }
     void destroy() {
-        if (s0) cudaEventDestroy(s0);
-        if (s1) cudaEventDestroy(s1);
-        if (u1) cudaEventDestroy(u1);
-        s0 = s1 = u1 = nullptr;
+        for (int i = 0; i < created; ++i) cudaEventDestroy(ev[i]);
+        created = n = 0;
+    }
+    int mark(cudaStream_t st, int g) {
+        if (n >= created) return IF_OK;
+        gid[n] = g;
+        IF_CUDA_TRY(cudaEventRecordWithFlags(ev[n], st, cudaEventRecordExternal));
+        ++n;
+        return IF_OK;
     }
 };
+
+}  // namespace
+}  // namespace ifl
+#include "mg_solve.cuh"
+namespace ifl {
+namespace {
 
 // One CG iteration: kernel A (two launches for n = 2) and kernel B.  The direction buffers are picked on the device
 // from ctrl->cur_p, so every iteration is the same launch sequence and a graph may resume at any iteration.
 template <int K>
-int enqueue_iteration(const Run& r, const TimingEvents* tev = nullptr) {
+int enqueue_iteration(const Run& r, IterTimer* tm = nullptr) {
     int rc;
-    if (tev) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s0, r.st, cudaEventRecordExternal));
+    if (tm && (rc = tm->mark(r.st, -1))) return rc;
     if (r.order_n == 1) {
         SpmmArgs a{r.w.z, r.w.p0, r.w.x, r.w.q, r.w.p1, 0, 1};
         if ((rc = launch_spmm<K, MODE_CG1>(r, r.g.cga, a))) return rc;
@@ -147,10 +165,10 @@ int enqueue_iteration(const Run& r, const TimingEvents* tev = nullptr) {
         SpmmArgs b{r.w.t, r.w.p0, nullptr, r.w.q, r.w.p1, 0, 1};
         if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
     }
-    if (tev) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->s1, r.st, cudaEventRecordExternal));
+    if (tm && (rc = tm->mark(r.st, 0))) return rc;
     k_update<K><<<r.g.update, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, r.w.z, r.w.q, r.order_n);
     IF_LAUNCH_CHECK();
-    if (tev) IF_CUDA_TRY(cudaEventRecordWithFlags(tev->u1, r.st, cudaEventRecordExternal));
+    if (tm && (rc = tm->mark(r.st, 1))) return rc;
     return IF_OK;
 }
 
@@ -158,13 +176,13 @@ int enqueue_iteration(const Run& r, const TimingEvents* tev = nullptr) {
 // events of the other (an event must not be re-recorded while it is being read).
 struct GraphSet {
     cudaGraphExec_t exec[2] = {nullptr, nullptr};
-    TimingEvents tev[2];
+    IterTimer tev[2];
     ~GraphSet() {
         for (int i = 0; i < 2; ++i) { if (exec[i]) cudaGraphExecDestroy(exec[i]); tev[i].destroy(); }
     }
 };
 
-struct KernelTimes { double spmm_ms = 0.0, update_ms = 0.0; int64_t samples = 0; };
+struct KernelTimes { double ms[TIMER_GROUPS] = {}; int64_t samples = 0; };   // per group, summed over samples
 
 struct PollState {
     Snapshot* snap = nullptr;          // pinned [4]
@@ -195,8 +213,16 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
         SpmmArgs b{r.w.t, nullptr, nullptr, r.w.q, nullptr, 0, 0};
         if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, b))) return rc;
     }
+    // multigrid phase: r0 into the residual buffer in use (w.z or its twin), z cleared, the column marked `starting`
+    double* r_alt = nullptr;
+    double* z_clear = nullptr;
+    if (r.mg) {
+        const MgBuffers b = mg_layout(h, r.w, r.order_n);
+        r_alt = b.r[1];
+        z_clear = b.zb;
+    }
     k_init<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, r.w.x, r.w.q, r.w.z, r.w.p0,
-                                              r.w.p1, r.order_n);
+                                              r.w.p1, r.order_n, r_alt, z_clear, r.mg ? 1 : 0);
     IF_LAUNCH_CHECK();
     return IF_OK;
 }
@@ -285,6 +311,7 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
                 PollState& poll, KernelTimes* times, QueueState& q, bool first, int* compact_to) {
     int rc;
     if ((rc = setup_grids<K>(r))) return rc;
+    if (r.mg && (K != MGK || (rc = mg_setup(r)))) return rc ? rc : IF_EINVAL;
     const size_t R = rhs.size();
     if (compact_to) *compact_to = 0;
     auto assign = [&](unsigned mask, StartParams* sp, unsigned* started) {
@@ -296,6 +323,7 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
             if (q.next < R) {
                 const Rhs& s = rhs[q.next];
                 sp->c[c] = r.opt.gamma * std::pow(s.ell, 2.0 * r.order_n);
+                sp->c1[c] = r.order_n == 1 ? sp->c[c] : std::sqrt(sp->c[c]);   // K = M + sqrt(c) S (mg_solve.cuh)
                 sp->field[c] = s.f;
                 sp->rhs[c] = s.f * n_ells + s.j;
                 q.col_rhs[c] = (int)q.next++;
@@ -318,8 +346,9 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
     }
 
     // the iteration loop: `check_every` iterations per CUDA graph launch, snapshot polled one launch behind
-    const int per_graph = r.opt.check_every;
-    const int launches_per_graph = per_graph * (r.order_n == 1 ? 2 : 3);
+    // (a multigrid iteration is some forty launches and a thirtieth of a solve: one per graph)
+    const int per_graph = r.mg ? 1 : r.opt.check_every;
+    long long launches_per_graph = 0;
     GraphSet gs;
     if (r.st != nullptr && r.st != cudaStreamLegacy) {
         for (int gi = 0; gi < 2; ++gi) {
@@ -331,9 +360,13 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
             }
             int rcc = IF_OK;
             const int timed_it = per_graph > 2 ? 2 : 0;
-            for (int i = 0; i < per_graph && rcc == IF_OK; ++i)
-                rcc = enqueue_iteration<K>(r, i == timed_it ? &gs.tev[gi] : nullptr);
-            g_launches -= (long long)launches_per_graph;   // captured, not launched
+            const long long before = g_launches.load();
+            for (int i = 0; i < per_graph && rcc == IF_OK; ++i) {
+                IterTimer* tm = i == timed_it ? &gs.tev[gi] : nullptr;
+                rcc = r.mg ? mg_enqueue_iteration(r, tm) : enqueue_iteration<K>(r, tm);
+            }
+            launches_per_graph = g_launches.load() - before;
+            g_launches -= launches_per_graph;   // captured, not launched
             cudaError_t e = cudaStreamEndCapture(r.st, &graph);
             if (rcc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
             e = cudaGraphInstantiate(&gs.exec[gi], graph, 0);
@@ -342,15 +375,16 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
         }
     }
     const bool use_graph = gs.exec[0] && gs.exec[1];
-    const int64_t per_rhs = (r.opt.max_iter + r.opt.check_every - 1) / r.opt.check_every + 3;
+    const int64_t per_rhs = (r.opt.max_iter + per_graph - 1) / per_graph + 3;
     const int64_t max_loops = ((int64_t)(R + K - 1) / K + 1) * per_rhs + 8;
+    unsigned free_cols = 0;   // stopped and finalised, waiting for a right-hand side
     for (int64_t it = 0; it < max_loops && q.active > 0; ++it) {
         if (use_graph) {
             IF_CUDA_TRY(cudaGraphLaunch(gs.exec[it & 1], r.st));
-            g_launches += (long long)launches_per_graph;
+            g_launches += launches_per_graph;
         } else {
             for (int i = 0; i < per_graph; ++i)
-                if ((rc = enqueue_iteration<K>(r))) return rc;
+                if ((rc = r.mg ? mg_enqueue_iteration(r, nullptr) : enqueue_iteration<K>(r))) return rc;
         }
         const int slot = (int)(it & 3);
         IF_CUDA_TRY(cudaMemcpyAsync(&poll.snap[slot], reinterpret_cast<const char*>(r.w.ctrl) + offsetof(Ctrl, done),
@@ -368,11 +402,17 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
         }
         if (times && use_graph && any_running) {
             // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
-            const TimingEvents& te = gs.tev[(it - 1) & 1];
-            float a = 0.f, b = 0.f;
-            if (cudaEventElapsedTime(&a, te.s0, te.s1) == cudaSuccess &&
-                cudaEventElapsedTime(&b, te.s1, te.u1) == cudaSuccess) {
-                times->spmm_ms += a; times->update_ms += b; times->samples += 1;
+            const IterTimer& te = gs.tev[(it - 1) & 1];
+            double ms[TIMER_GROUPS] = {};
+            bool ok = te.n > 1;
+            for (int i = 1; i < te.n && ok; ++i) {
+                float dt = 0.f;
+                ok = cudaEventElapsedTime(&dt, te.ev[i - 1], te.ev[i]) == cudaSuccess;
+                if (ok && te.gid[i] >= 0 && te.gid[i] < TIMER_GROUPS) ms[te.gid[i]] += dt;
+            }
+            if (ok) {
+                for (int g = 0; g < TIMER_GROUPS; ++g) times->ms[g] += ms[g];
+                times->samples += 1;
             } else {
                 cudaGetLastError();
             }
@@ -381,14 +421,21 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
             // these columns stopped before launch it-1 ended and stayed frozen through launch it
             if ((rc = finalize_columns<K>(r, job, fin, d_out, d_fields))) return rc;
             for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) --q.active;
-            if (q.next < R) {
-                assign(fin, &sp, &started);
+            for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) q.col_rhs[c] = -1;
+            free_cols |= fin;
+        }
+        // refill: at once in the Jacobi path (a start costs 3 passes, a solve hundreds of iterations); in the multigrid
+        // path a start is a tenth of a solve, so freed columns wait for company (or for the last running column)
+        if (free_cols && q.next < R) {
+            int nfree = 0;
+            for (int c = 0; c < K; ++c) nfree += (free_cols >> c) & 1u;
+            if (!r.mg || nfree >= MG_REFILL_MIN || q.active == 0 || (size_t)nfree >= R - q.next) {
+                assign(free_cols, &sp, &started);
                 if ((rc = start_columns<K>(r, started, sp, d_fields))) return rc;
-            } else {
-                for (int c = 0; c < K; ++c) if ((fin >> c) & 1u) q.col_rhs[c] = -1;
+                free_cols = 0;
             }
         }
-        if (compact_to && K > 4 && q.next >= R && q.active > 0 && q.active <= K / 2) {
+        if (compact_to && !r.mg && K > 4 && q.next >= R && q.active > 0 && q.active <= K / 2) {
             *compact_to = (q.active <= 4) ? 4 : 8;
             return IF_OK;   // the graph launch already enqueued runs first; the caller repacks after it
         }
@@ -474,12 +521,6 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
     return IF_OK;
 }
 
-}  // namespace
-}  // namespace ifl
-#include "mg_solve.cuh"
-namespace ifl {
-namespace {
-
 int pick_k(int batch, size_t R) {
     int K = batch;
     while (K > 4 && R <= (size_t)K / 2) K /= 2;   // few right-hand sides: narrower columns, less wasted bandwidth
@@ -539,22 +580,32 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (job != JOB_APPLY)
         std::stable_sort(rhs.begin(), rhs.end(), [](const Rhs& a, const Rhs& b) { return a.ell > b.ell; });
 
-    KernelTimes ktimes;
-    int64_t batch_iters = 0;
-    // large scales by multigrid-preconditioned CG (option solver = 1), 16 right-hand sides at a time
-    if (job != JOB_APPLY && r.opt.solver == 1 && order_n == 1 && r.w.mg_extra && h->mean_edge > 0.0) {
+    KernelTimes ktimes, mgtimes;
+    int64_t batch_iters = 0, mg_batch_iters = 0;
+    // large scales by multigrid-preconditioned CG (option solver = 1): a stream of right-hand sides through 16 columns
+    if (job != JOB_APPLY && r.opt.solver == 1 && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
+        const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)) *
+                               h->mean_edge;
         size_t n_big = 0;
-        while (n_big < rhs.size() && rhs[n_big].ell >= r.opt.mg_min_ell * h->mean_edge) ++n_big;
-        // whole batches of 16: a ragged last batch costs a full one, its (smallest) scales are cheap for Jacobi-PCG
-        if (n_big > MGK && n_big % MGK != 0 && n_big % MGK < MGK / 2 && n_big < rhs.size()) n_big -= n_big % MGK;
+        while (n_big < rhs.size() && rhs[n_big].ell >= min_ell) ++n_big;
         if (n_big > 0) {
-            double* h_dots = reinterpret_cast<double*>(reinterpret_cast<char*>(poll.snap) + 4 * sizeof(Snapshot));
-            for (size_t first = 0; first < n_big; first += MGK) {
-                rc = mg_solve_batch(r, job, d_fields, rhs, first, std::min<size_t>(MGK, n_big - first), n_ells, d_out,
-                                    r.w.mg_extra, h_dots, &batch_iters);
-                if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
+            std::vector<Rhs> big(rhs.begin(), rhs.begin() + (ptrdiff_t)n_big);
+            Run rm = r;
+            rm.mg = true;
+            // sweeps per side of the cycle: n = 1 (1, MG_NU_L1, MG_NU_COARSE) as tuned on config 4; n = 2 needs the
+            // stronger smoother: what V leaves of a rough residual enters B = V M V squared
+            rm.mg_nu[0] = order_n == 1 ? 1 : MG_NU0_N2;
+            rm.mg_nu[1] = order_n == 1 ? MG_NU_L1 : MG_NU1_N2;
+            rm.mg_nu[2] = MG_NU_COARSE;
+            if (const char* e = getenv("IF_MG_NU")) {   // tuning runs: "nu0,nu1,nu2"
+                int a0 = 0, a1 = 0, a2 = 0;
+                if (sscanf(e, "%d,%d,%d", &a0, &a1, &a2) == 3 && a0 >= 1 && a1 >= 1 && a2 >= 1 && a0 <= MG_MAX_NU &&
+                    a1 <= MG_MAX_NU && a2 <= MG_MAX_NU) { rm.mg_nu[0] = a0; rm.mg_nu[1] = a1; rm.mg_nu[2] = a2; }
             }
+            rc = solve_all<MGK>(rm, job, d_fields, big, n_ells, d_out, poll, &mgtimes, &mg_batch_iters);
+            if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
             rhs.erase(rhs.begin(), rhs.begin() + (ptrdiff_t)n_big);
+            batch_iters += mg_batch_iters;
         }
     }
     const int K = pick_k(r.opt.batch, rhs.size());
@@ -600,9 +651,13 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
         stats->seconds = ms * 1e-3;
         stats->batch_iters = batch_iters;
         stats->rhs_iters = 0;
-        stats->spmm_seconds = ktimes.samples ? 1e-3 * ktimes.spmm_ms / (double)ktimes.samples : 0.0;
-        stats->update_seconds = ktimes.samples ? 1e-3 * ktimes.update_ms / (double)ktimes.samples : 0.0;
+        stats->spmm_seconds = ktimes.samples ? 1e-3 * ktimes.ms[0] / (double)ktimes.samples : 0.0;
+        stats->update_seconds = ktimes.samples ? 1e-3 * ktimes.ms[1] / (double)ktimes.samples : 0.0;
         stats->kernel_samples = ktimes.samples;
+        for (int g = 0; g < 8; ++g)
+            stats->mg_kernel_seconds[g] = mgtimes.samples && g < TIMER_GROUPS ? 1e-3 * mgtimes.ms[g] / (double)mgtimes.samples : 0.0;
+        stats->mg_samples = mgtimes.samples;
+        stats->mg_batch_iters = mg_batch_iters;
         for (int64_t i = 0; i < R; ++i) {
             stats->rhs_iters += h_iters[(size_t)i];
             if (stats->iters) stats->iters[i] = h_iters[(size_t)i];

@@ -324,7 +324,8 @@ def test_multigrid_solver_matches_oracle(ifl, oracle_mod, name):
 
 
 def test_multigrid_option_is_ignored_where_it_does_not_apply(ifl, oracle_mod):
-    """n = 2, a handle without hierarchy, or a narrower batch: solver = 1 silently means Jacobi-PCG."""
+    """A handle without hierarchy, or a narrower batch: solver = 1 silently means Jacobi-PCG; solver = 2 asks for
+    Jacobi-PCG on a handle whose default is multigrid."""
     w = SMALL["cfg4_L5"]()
     h0 = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
     h1 = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
@@ -333,10 +334,11 @@ def test_multigrid_option_is_ignored_where_it_does_not_apply(ifl, oracle_mod):
         b, sb = ifl.if_filter(h, w.fields, w.ells, 1, **kw)
         assert np.abs(sa["iters"] - sb["iters"]).max() <= 2
         assert float((a - b).abs().max()) <= 1e-9 * float(a.abs().max())
-    c, sc = ifl.if_filter(h1, w.fields, w.ells[:3], 2, solver=1)
-    d, sd = ifl.if_filter(h0, w.fields, w.ells[:3], 2)
-    assert np.abs(sc["iters"] - sd["iters"]).max() <= 2
-    h0.close(); h1.close()
+    h2 = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID, solver=1)
+    c, sc = ifl.if_filter(h2, w.fields, w.ells, 1)              # the handle's default: multigrid
+    d, sd = ifl.if_filter(h2, w.fields, w.ells, 1, solver=2)    # explicitly Jacobi
+    assert sc["iters"].sum() < 0.5 * sa["iters"].sum() and np.abs(sd["iters"] - sa["iters"]).max() <= 2
+    h0.close(); h1.close(); h2.close()
 
 
 def test_multigrid_on_disconnected_and_degenerate_inputs(ifl, oracle_mod):
@@ -538,17 +540,19 @@ def test_biharmonic_32_edge_lengths_against_dense_direct_solve(ifl, oracle_mod):
 
 def test_biharmonic_beyond_its_range_returns_a_status(ifl):
     """for the biharmonic filter "the convergence can be lost for large l".  l = 400 h on a
-    level-5 sphere (kappa ~ 1e12-1e13, far beyond reading A16's range) with the default iteration cap: the call must
-    come back -- per-right-hand-side status, finite output, every column stopped by the cap or converged -- not hang."""
+    level-5 sphere (kappa ~ 1e12-1e13, far beyond reading A16's range): with a cap of 3 000 iterations the call must
+    come back with status 1 for exactly those right-hand sides (finite output = the last iterate, the in-range column
+    of the same batch converged); with the default cap it must come back as well, converged or not -- never hang."""
     w = make_config(5, level=5, n_fields=2, n_ells=2, ell_max=2.0)
     h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None)
     ells = w.mesh.h * np.array([2.0, 400.0])
-    out, st = ifl.if_filter(h, w.fields, ells, 2, max_iter=60000)
-    assert np.all(st["status"][:, 0] == 0)
-    assert st["code"] in (0, 1) and np.all(np.isin(st["status"][:, 1], (0, 1, 2)))
-    assert st["code"] == (1 if np.any(st["status"] != 0) else 0)
-    capped = st["status"][:, 1] == 1
-    assert np.all(st["iters"][capped, 1] == 60000)
+    out, st = ifl.if_filter(h, w.fields, ells, 2, max_iter=3000)
+    assert st["code"] == 1 and np.all(st["status"][:, 0] == 0) and np.all(st["status"][:, 1] == 1)
+    assert np.all(st["iters"][:, 1] == 3000) and np.all(st["rel_res"][:, 1] > 1e-12)
+    assert bool(out.isfinite().all())
+    out, st = ifl.if_filter(h, w.fields, ells, 2)
+    assert st["code"] in (0, 1) and np.all(np.isin(st["status"], (0, 1, 2)))
+    assert st["code"] == (1 if np.any(st["status"] != 0) else 0) and st["iters"].max() <= 200000
     assert bool(out.isfinite().all())
     print("l = 400 h: status", st["status"][:, 1], "iterations", st["iters"][:, 1], "residual", st["rel_res"][:, 1])
     h.close()
@@ -614,7 +618,13 @@ def test_refill_while_other_columns_have_a_pending_step(ifl, oracle_mod, check_e
     """4 columns, 27 short solves at a loose tolerance, graph launches of 1, 3 or 16 iterations: columns stop on odd and
     even iterations while the queue is not empty, so refilled columns restart next to columns whose last step
     x += alpha p is still pending.  At the same iteration count the CG iterate is the oracle's up to rounding."""
-    w = make_config(2, n=48, n_fields=3, n_ells=9, ell_max=6.0)
+    from workloads import log_spaced
+    # (mild jitter, no slivers: on config 2's literal mesh kappa amplifies the rounding of two CG implementations
+    # to 1e-7 within a few hundred iterations, which would hide the defect this test is about)
+    m = grid_mesh(48, periodic=True, jitter=0.2, random_diagonals=True, rng=np.random.default_rng(8))
+    fields = np.random.default_rng(9).standard_normal((3, m.n_vert))
+    ells = log_spaced(0.7, 4.0, 9)
+    w = type("W", (), dict(mesh=m, fields=fields, ells=ells))
     om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
     h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period)
     for order_n in (1, 2):
@@ -627,8 +637,75 @@ def test_refill_while_other_columns_have_a_pending_step(ifl, oracle_mod, check_e
                 x, info = om.solve(w.fields[f], float(ell), order_n, tol=1e-4)
                 if info["iters"] == st["iters"][f, j]:
                     same += 1
-                    assert rel(out[f, j], x) <= 1e-9, (order_n, f, j, rel(out[f, j], x))
+                    # n = 1: the two implementations agree to 1e-14 here; n = 2 (200-470 iterations on white noise)
+                    # amplifies their rounding to 6e-7 with or without refill -- a misapplied last step is >= 1e-5
+                    assert rel(out[f, j], x) <= (1e-12 if order_n == 1 else 5e-6), (order_n, f, j, rel(out[f, j], x))
                 else:
                     assert abs(info["iters"] - st["iters"][f, j]) <= 1 and rel(out[f, j], x) <= 1e-3
         assert same >= 24
+    h.close()
+
+
+# ------------------------------------------------------------------------------------------ n = 2 through the hierarchy
+@pytest.mark.parametrize("name", list(LARGE_N2))
+def test_biharmonic_multigrid_product_preconditioner_matches_oracle(ifl, oracle_mod, name):
+    """solver = 1 for n = 2: PCG on M + c S M^-1 S with B = V M V (V = one V cycle for M + sqrt(c) S).  Same systems,
+    same start vector, same stop test as the oracle's Jacobi-PCG: fields at 1 ... 32 h within the tolerance derived
+    from both true residuals, spectra to 1e-6, an order of magnitude fewer iterations at the large scales."""
+    w = LARGE_N2[name]()
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, w.mesh.period)
+    area = om.area()
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, w.mesh.period, flags=ifl.IF_FLAG_MULTIGRID)
+    out, st = ifl.if_filter(h, w.fields, w.ells, 2, solver=1, mg_min_ell=0.5)
+    jac, stj = ifl.if_filter(h, w.fields, w.ells, 2)
+    assert st["code"] == 0 and np.all(st["status"] == 0) and np.all(st["rel_res"] <= 1e-12)
+    print(name, "iterations multigrid", st["iters"][0], "Jacobi", stj["iters"][0])
+    assert st["iters"].max() < 200 and st["iters"][:, -1].max() * 10 < stj["iters"][:, -1].min()
+    sp = ifl.if_spectrum(h, w.fields, w.ells, 2, solver=1, mg_min_ell=0.5)
+    worst = 0.0
+    for f in range(w.fields.shape[0]):
+        en = []
+        for j, ell in enumerate(w.ells):
+            x, info = om.solve(w.fields[f], float(ell), 2)
+            assert info["status"] == 0
+            res_gpu = true_residual(ifl, h, out[f, j], w.fields[f], area, float(ell), 2)
+            tol = parity_tolerance(area, w.fields[f], x, res_gpu, info["true_res"])
+            err = rel(out[f, j].cpu().numpy(), x)
+            assert err <= tol, (f, j, err, tol, res_gpu, info["true_res"])
+            worst = max(worst, err)
+            en.append(om.energy(x))
+        en = np.array(en)
+        k_mid, E = oracle_mod.spectrum(w.ells, en)
+        assert np.all(np.abs(sp["energy"][f] - en) <= TOL_BIN * en)
+        assert np.all(np.abs(sp["E"][f] - E) <= TOL_BIN * np.abs(E))
+    print(f"{name}: worst relative L2 difference from the oracle {worst:.2e}")
+    h.close()
+
+
+@pytest.mark.parametrize("order_n", [1, 2])
+def test_multigrid_stream_refills_columns_and_is_deterministic(ifl, oracle_mod, order_n):
+    """More right-hand sides than columns (3 fields x 11 scales = 33 through 16 columns), very unequal scales: stopped
+    columns are restarted from the queue at iteration boundaries next to running ones.  The preconditioner is a fixed
+    operator per column, so two runs give the same iteration counts and the same bits; answers are the oracle's."""
+    w = make_config(5 if order_n == 2 else 4, level=5, n_fields=3, n_ells=11, ell_max=32.0)
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    area = om.area()
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    a, sa = ifl.if_filter(h, w.fields, w.ells, order_n, solver=1, mg_min_ell=0.5)
+    b, sb = ifl.if_filter(h, w.fields, w.ells, order_n, solver=1, mg_min_ell=0.5)
+    assert sa["code"] == 0 and np.array_equal(sa["iters"], sb["iters"]) and bool((a == b).all())
+    assert sa["mg_batch_iters"] > 0 and sa["mg_batch_iters"] == sa["batch_iters"]
+    assert sa["iters"].sum() <= 16 * sa["mg_batch_iters"]
+    for f in range(3):
+        for j in (0, 3, 5, 8, 10):
+            x, info = om.solve(w.fields[f], float(w.ells[j]), order_n)
+            res_gpu = true_residual(ifl, h, a[f, j], w.fields[f], area, float(w.ells[j]), order_n)
+            tol = parity_tolerance(area, w.fields[f], x, res_gpu, info["true_res"])
+            assert info["status"] == 0 and rel(a[f, j].cpu().numpy(), x) <= tol, (f, j)
+    # mixed: the smallest scales stay on the Jacobi path, and the iteration cap gives a status in the multigrid path
+    c, sc = ifl.if_filter(h, w.fields, w.ells, order_n, solver=1, mg_min_ell=3.0)
+    assert sc["code"] == 0 and 0 < sc["mg_batch_iters"] < sc["batch_iters"]
+    assert float((c - a).abs().max()) <= 1e-8 * float(a.abs().max())
+    d, sd = ifl.if_filter(h, w.fields[:1], w.ells[-1:], order_n, solver=1, max_iter=3)
+    assert sd["code"] == 1 and sd["status"][0, 0] == 1 and sd["iters"][0, 0] == 3 and bool(d.isfinite().all())
     h.close()
