@@ -57,6 +57,9 @@ def parse_args():
                     help="preconditioner of the timed headline run (the metric is quoted on jacobi)")
     ap.add_argument("--mg-min-ell", type=float, default=0.0, help="0 = library default (4 mean edge lengths)")
     ap.add_argument("--no-multigrid", action="store_true", help="skip the extra multigrid-preconditioned leg")
+    ap.add_argument("--budget-seconds", type=float, default=150.0,
+                    help="a timed leg stops adding steps once it has run this long (at least one step; the line "
+                         "reports the steps actually timed); 0 = no budget")
     return ap.parse_args()
 
 
@@ -142,6 +145,40 @@ def algorithmic_bytes(V, nnz, K, order_n):
         spmm = V * K * 8 * 6 + matrix + V * K * 8 * 3 + matrix   # pass A as above (t for q) + pass B: read t, p', write q
     update = V * K * 8 * 3 + V * 16         # read z, q ; write z ; A_v and diagonal per row
     return {"spmm": spmm, "update": update, "iteration": spmm + update}
+
+
+def mg_algorithmic_bytes(V, nnz, info, order_n):
+    """Algorithmic HBM bytes of ONE 16-column iteration of the multigrid-preconditioned path, by kernel group
+    (the groups of if_stats.mg_kernel_seconds): every [rows][16] vector and every matrix entry
+    a kernel reads or writes counted once per launch."""
+    nu0, nu1, nuc = info["sweeps"][order_n]
+    rows, lnnz, pnnz, L = info["rows"], info["nnz"], info["p_nnz"], info["levels"]
+    vec = V * 16 * 8
+    matrix = (nnz - V) * 12 + V * 16
+    sweep = 3 * vec + matrix                     # gathered vector, r in; out (also the residual pass)
+    g = {"A": 6 * vec + matrix if order_n == 1 else 9 * vec + 2 * matrix}
+    g.update(MGR=0, restrict0=0, level1=0, coarse=0, prolong0=0, last=0)
+
+    def level(l, nu):
+        n, v = rows[l], rows[l] * 128
+        if l == L - 1:
+            return 2 * v + 16 * lnnz[l] * 20     # dense solve per column
+        m = lnnz[l] * 20 + n * 16                # int32 column + (S, M) pair per entry, diagonal pair per row
+        b = 2 * v + n * 16                       # first sweep from a zero guess
+        b += 2 * nu * (3 * v + m)                # nu - 1 sweeps, the residual, nu sweeps
+        b += v + pnnz[l] * 12 + rows[l + 1] * 128        # restriction
+        b += 2 * v + pnnz[l] * 12 + rows[l + 1] * 128    # prolongation (accumulating)
+        return b
+
+    for cycle in range(1 if order_n == 1 else 2):
+        g["MGR"] += (4 if cycle == 0 else 2) * vec + matrix      # r, q in; r', t (or e2) out | w in; t (or e2) out
+        g["restrict0"] += vec + pnnz[0] * 12 + rows[1] * 128
+        g["level1"] += level(1, nu1) if L > 1 else 0
+        g["coarse"] += sum(level(l, nuc) for l in range(2, L))
+        g["prolong0"] += 2 * vec + pnnz[0] * 12 + rows[1] * 128 + (V * 16 if nu0 == 1 else 0)
+        g["last"] += sweep if nu0 == 1 else (2 * nu0 - 1) * sweep   # nu0 - 2 sweeps, residual, nu0 sweeps
+    g["iteration"] = sum(g.values())
+    return g
 
 
 def measured_peaks():
@@ -279,12 +316,30 @@ def run_ours(args):
                 return lib.if_spectrum_host(h, h_fields, w.ells, w.order_n, workspace=ws_host, stream=stream, **o)
             return lib.if_spectrum(h, d_fields, w.ells, w.order_n, workspace=ws, stream=stream, **o)
 
+    def over_budget(t_start):
+        """True once a leg has used its time budget (agreed over ranks, so that every rank times the same steps)."""
+        if args.budget_seconds <= 0:
+            return False
+        over = time.perf_counter() - t_start > args.budget_seconds
+        if world > 1:
+            t = torch.tensor([1.0 if over else 0.0], dtype=torch.float64, device=rdev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            over = bool(t.item() > 0)
+        return over
+
     def timed(n_steps: int, from_host: bool, o=None):
+        """(total ms, results, launches, steps timed): up to n_steps steps between two events on the stream; stops
+        early only when the leg's time budget is used up (a step of the Jacobi leg on config 4 takes 35 s)."""
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         launches0 = lib.if_launch_count()
+        t_start = time.perf_counter()
         e0.record(stream)
-        res = [step(from_host, o) for _ in range(n_steps)]
+        res = []
+        for _ in range(n_steps):
+            res.append(step(from_host, o))
+            if len(res) < n_steps and over_budget(t_start):
+                break
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
@@ -292,13 +347,18 @@ def run_ours(args):
             t = torch.tensor([ms], dtype=torch.float64, device=rdev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
-        return ms, res, lib.if_launch_count() - launches0
+        return ms, res, lib.if_launch_count() - launches0, len(res)
 
+    t_w = time.perf_counter()
+    n_warm = 0
     for _ in range(max(args.warmup, 0)):
         sp = step(False)
+        n_warm += 1
+        if n_warm >= 3 and over_budget(t_w):     # never fewer than 3 warm-up steps (if that many were asked for)
+            break
     sampler = ClockSampler(local)
     sampler.start()
-    ms, res, launches = timed(args.steps, False)
+    ms, res, launches, n_steps = timed(args.steps, False)
     clocks = sampler.stop()
     stats = [r["stats"] for r in res]
     rhs_iters = sum(s["rhs_iters"] for s in stats)
@@ -314,7 +374,7 @@ def run_ours(args):
 
     e2e = None
     if not args.no_e2e:
-        ms_e, res_e, _ = timed(args.steps, True)
+        ms_e, res_e, _, n_e = timed(args.steps, True)
         it_e = sum(r["stats"]["rhs_iters"] for r in res_e)
         if world > 1:
             t = torch.tensor([it_e], dtype=torch.float64, device=rdev)
@@ -324,31 +384,83 @@ def run_ours(args):
         F = w.fields.shape[0]
         d2h = R * 8 + (L - 1) * 8 + F * (L - 1) * 8 + R * (4 + 4 + 8)
         e2e = {"value": it_e / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h_fields.numel() * 8),
-               "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e / args.steps}
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e / n_e, "steps": n_e}
 
-    # the same spectrum with the smoothed-aggregation preconditioner on the large scales:
-    # a second reported time, not the headline metric (its iterations are not comparable one to one)
+    peak, peak_src = measured_peaks()
+    traffic_all = {}
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic_all = json.load(open(tpath))
+        except Exception:
+            traffic_all = {}
+
+    def mg_roofline(stats_list):
+        """Roofline record of the multigrid-preconditioned iteration: algorithmic bytes of each kernel group of one
+        16-column iteration (mg_algorithmic_bytes) over its live event time (if_stats.mg_kernel_seconds)."""
+        info = lib.if_mesh_multigrid_info(h)
+        ns = sum(s_["mg_samples"] for s_ in stats_list)
+        if info["levels"] < 2 or ns == 0:
+            return None
+        names = ["A", "MGR", "restrict0", "level1", "coarse", "prolong0", "last"]
+        secs = [sum(s_["mg_kernel_seconds"][i] * s_["mg_samples"] for s_ in stats_list) / ns for i in range(7)]
+        ab = mg_algorithmic_bytes(V, h.nnz, info, w.order_n)
+        groups = {}
+        for nm, sec in zip(names, secs):
+            gbs = ab[nm] / sec / 1e9 if sec > 0 else None
+            groups[nm] = {"algorithmic_bytes": int(ab[nm]), "seconds": sec, "achieved": gbs,
+                          "frac": gbs / peak if gbs else None}
+        it_s = sum(secs)
+        return {"bound": "hbm", "kernel": "one 16-column iteration of multigrid-preconditioned CG "
+                "(A = kernel A, MGR = fused residual update + first sweep, restrict0 / prolong0 = transfers mesh <-> "
+                "level 1, level1, coarse = levels >= 2, last = the other sweeps on the mesh + CG bookkeeping"
+                + ("; n = 2: both cycles of B = V M V)" if w.order_n == 2 else ")"),
+                "achieved": ab["iteration"] / it_s / 1e9, "peak": peak, "unit": "GB/s",
+                "frac": ab["iteration"] / it_s / 1e9 / peak, "traffic": traffic_all.get(f"config{w.config}_V{V}_mg_iteration_bytes"),
+                "peak_source": peak_src, "algorithmic_bytes_per_iteration": int(ab["iteration"]),
+                "iteration_seconds": it_s, "samples": ns, "groups": groups,
+                "hierarchy": {"rows": info["rows"], "entries": info["nnz"], "sweeps_per_side": info["sweeps"][w.order_n]}}
+
+    def mg_e2e(o):
+        ms_x, res_x, _, n_x = timed(args.steps, True, o)
+        it_x = sum(r_["stats"]["rhs_iters"] for r_ in res_x)
+        if world > 1:
+            t_ = torch.tensor([it_x], dtype=torch.float64, device=rdev)
+            dist.all_reduce(t_, op=dist.ReduceOp.SUM)
+            it_x = float(t_.item())
+        L_, F_ = w.ells.shape[0], w.fields.shape[0]
+        return {"value": it_x / (ms_x * 1e-3), "unit": UNIT, "spectrum_seconds": ms_x * 1e-3 / n_x, "steps": n_x,
+                "h2d_bytes_per_step": int(h_fields.numel() * 8),
+                "d2h_bytes_per_step": int(R * 8 + (L_ - 1) * 8 + F_ * (L_ - 1) * 8 + R * 16)}
+
+    # the same spectrum with the multigrid preconditioner on the large scales (DESIGN.md sections 9b, 9d): a second
+    # reported time, not the headline metric (its iterations are not comparable one to one)
     mg = None
     if use_mg and args.solver != "multigrid":
         step(False, mg_opts)
-        ms_m, res_m, launches_m = timed(args.steps, False, mg_opts)
+        ms_m, res_m, launches_m, n_m = timed(args.steps, False, mg_opts)
         e_j = np.asarray(res[-1]["energy"], dtype=np.float64)
         e_m = np.asarray(res_m[-1]["energy"], dtype=np.float64)
-        mg = {"spectrum_seconds": ms_m * 1e-3 / args.steps,
-              "rhs_iterations_per_step": sum(r["stats"]["rhs_iters"] for r in res_m) / args.steps,
-              "batch_iterations_per_step": sum(r["stats"]["batch_iters"] for r in res_m) / args.steps,
-              "mg_min_ell_in_mean_edges": args.mg_min_ell or 4.0, "gpu_launches": int(launches_m),
+        mg = {"spectrum_seconds": ms_m * 1e-3 / n_m, "steps": n_m,
+              "rhs_iterations_per_step": sum(r["stats"]["rhs_iters"] for r in res_m) / n_m,
+              "batch_iterations_per_step": sum(r["stats"]["batch_iters"] for r in res_m) / n_m,
+              "multigrid_batch_iterations_per_step": sum(r["stats"]["mg_batch_iters"] for r in res_m) / n_m,
+              "mg_min_ell_in_mean_edges": args.mg_min_ell or (4.0 if w.order_n == 1 else 0.5),
+              "gpu_launches": int(launches_m),
               "solver_codes": sorted({r["stats"]["code"] for r in res_m}),
-              "max_rel_energy_diff_vs_jacobi": float(np.max(np.abs(e_m - e_j) / np.abs(e_j)))}
+              "max_rel_energy_diff_vs_jacobi": float(np.max(np.abs(e_m - e_j) / np.abs(e_j))),
+              "roofline": mg_roofline([r["stats"] for r in res_m])}
+        if not args.no_e2e:
+            mg["e2e"] = mg_e2e(mg_opts)
         if not args.tol:
             # the same call at the paper's own solver tolerance (PAPER.md:113, 1e-9): context for its timings
             p_opts = dict(mg_opts, tol=1e-9)
             step(False, p_opts)
-            ms_p, res_p, _ = timed(args.steps, False, p_opts)
+            ms_p, res_p, _, n_p = timed(args.steps, False, p_opts)
             e_p = np.asarray(res_p[-1]["energy"], dtype=np.float64)
             mg["at_paper_tol_1e-9"] = {
-                "spectrum_seconds": ms_p * 1e-3 / args.steps,
-                "rhs_iterations_per_step": sum(r["stats"]["rhs_iters"] for r in res_p) / args.steps,
+                "spectrum_seconds": ms_p * 1e-3 / n_p,
+                "rhs_iterations_per_step": sum(r["stats"]["rhs_iters"] for r in res_p) / n_p,
                 "max_rel_energy_diff_vs_jacobi": float(np.max(np.abs(e_p - e_j) / np.abs(e_j)))}
 
     # roofline of the dominant kernel (fused SpMM): live per-launch time from the library's event samples
@@ -356,14 +468,7 @@ def run_ours(args):
     spmm_s = sum(s["spmm_seconds"] * s["kernel_samples"] for s in stats) / max(nsamp, 1)
     upd_s = sum(s["update_seconds"] * s["kernel_samples"] for s in stats) / max(nsamp, 1)
     ab = algorithmic_bytes(V, h.nnz, K, w.order_n)
-    peak, peak_src = measured_peaks()
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(f"config{w.config}_V{V}_spmm_bytes_per_launch")
-        except Exception:
-            traffic = None
+    traffic = traffic_all.get(f"config{w.config}_V{V}_spmm_bytes_per_launch")
     achieved = ab["spmm"] / spmm_s / 1e9 if spmm_s > 0 else None
     roofline = {"bound": "hbm", "kernel": f"k_spmm<{K},CG{'1' if w.order_n == 1 else '2A+2B'}>",
                 "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -375,6 +480,9 @@ def run_ours(args):
                 "iteration": {"achieved": ab["iteration"] / (spmm_s + upd_s) / 1e9 if spmm_s > 0 else None,
                               "frac": ab["iteration"] / (spmm_s + upd_s) / 1e9 / peak if spmm_s > 0 else None,
                               "frac_of_8TBs_nominal": ab["iteration"] / (spmm_s + upd_s) / 8e12 if spmm_s > 0 else None}}
+    if args.solver == "multigrid":      # the timed headline run was the multigrid path: its iteration is the record
+        roofline = mg_roofline(stats) or roofline
+    mg_info = lib.if_mesh_multigrid_info(h) if use_mg else None
 
     if rank != 0:
         if world > 1:
@@ -387,18 +495,21 @@ def run_ours(args):
         v, _, info = oracle_sample(w, args.cpu_sample_iters, 3, 1)
         cpu = {"value": v, "unit": UNIT, "cores": info["cores"], "kind": "oracle", "sample": info["sample"]}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": n_steps,
+            "warmup": n_warm, "ms_per_step": ms / n_steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(w, args), "batch_rhs_per_spmm": K,
                        "tol": args.tol or 1e-12, "l2": "work vectors (5 x V x 16 x 8 B) exceed L2; no flush needed",
-                       "parallelism": f"rhs-replicas x{world}"},
-            "spectrum_seconds": ms * 1e-3 / args.steps,
+                       "parallelism": f"rhs-replicas x{world}", "steps_asked": args.steps, "warmup_asked": args.warmup,
+                       "budget_seconds_per_leg": args.budget_seconds},
+            "spectrum_seconds": ms * 1e-3 / n_steps,
             # the same 40-scale spectrum, same tolerance, by the multigrid-preconditioned path (detail under "multigrid")
             "spectrum_seconds_multigrid": (mg or {}).get("spectrum_seconds") if args.solver != "multigrid"
-            else ms * 1e-3 / args.steps,
+            else ms * 1e-3 / n_steps,
             "prepare_seconds": t_prepare,
-            "rhs_iterations_per_step": rhs_iters_all / args.steps / world,
+            "prepare_split": {"mesh": t_prepare - mg_info["build_seconds"], "hierarchy": mg_info["build_seconds"]}
+            if mg_info else {"mesh": t_prepare, "hierarchy": 0.0},
+            "rhs_iterations_per_step": rhs_iters_all / n_steps / world,
             "batch_iterations_per_second": batch_iters_all / (ms * 1e-3),
             "solver": args.solver, "solver_codes": codes, "multigrid": mg, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu}

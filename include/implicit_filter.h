@@ -156,6 +156,13 @@ int if_mesh_info(if_handle h, int64_t* n_vert, int64_t* nnz, double* total_area,
  * halo or row width exceeds the shared-memory caps (they take the slower global-gather path). */
 int if_mesh_tile_info(if_handle h, int64_t* n_tiles, int64_t* halo_rows, int64_t* halo_max, int64_t* unstaged_tiles);
 
+/* The multigrid hierarchy of a handle prepared with IF_FLAG_MULTIGRID (all HOST, any may be NULL): number of levels
+ * (0: none; level 0 is the mesh), per level l < 12 its rows, stored entries of the (S_l, M_l) pair and entries of the
+ * prolongator to level l+1, the wall-clock seconds if_prepare spent building it, and the Jacobi sweeps per side of the
+ * V cycle, sweeps[n-1][0..2] = on the mesh, on level 1, below, for filter order n = 1, 2 (bench.py's byte model). */
+int if_mesh_multigrid_info(if_handle h, int* n_levels, int64_t* rows, int64_t* nnz, int64_t* p_nnz,
+                           double* build_seconds, int* sweeps);
+
 /* Copy S (CSR, caller's numbering, columns ascending, diagonal included) and A_v to HOST arrays:
  * rowptr [n_vert+1], col [nnz], val [nnz], area [n_vert]; any may be NULL.  Needs IF_FLAG_KEEP_CSR
  * (else IF_EINVAL).  For checking the preparation phase against another assembly. */

@@ -22,6 +22,7 @@ IF_FLAG_HIGHPASS = 2
 IF_FLAG_MULTIGRID = 4
 
 EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_spectrum_host", "if_apply", "if_mesh_info", "if_mesh_tile_info",
+           "if_mesh_multigrid_info",
            "if_mesh_export_csr", "if_mesh_export_perm", "if_save", "if_load", "if_destroy", "if_strerror", "if_launch_count")
 
 
@@ -76,6 +77,8 @@ def load_library():
     L.if_mesh_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), dp, dp, C.POINTER(i64)]
     L.if_mesh_tile_info.restype = i32
     L.if_mesh_tile_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
+    L.if_mesh_multigrid_info.restype = i32
+    L.if_mesh_multigrid_info.argtypes = [vp, C.POINTER(C.c_int), vp, vp, vp, dp, vp]
     L.if_mesh_export_csr.restype = i32
     L.if_mesh_export_csr.argtypes = [vp, vp, vp, vp, vp]
     L.if_mesh_export_perm.restype = i32
@@ -336,6 +339,21 @@ def if_mesh_export_csr(h: Handle):
     if rc != IF_OK:
         raise ImplicitFilterError(rc, "if_mesh_export_csr")
     return rowptr, col, val, area
+
+
+def if_mesh_multigrid_info(h: Handle) -> dict:
+    """Levels of the multigrid hierarchy (rows, entries, prolongator entries), its build time and the sweep counts."""
+    n = C.c_int(0)
+    rows, nnz, pnnz = (np.zeros(12, dtype=np.int64) for _ in range(3))
+    secs = C.c_double(0.0)
+    sweeps = np.zeros(6, dtype=np.int32)
+    rc = load_library().if_mesh_multigrid_info(h._ptr, C.byref(n), _np_ptr(rows), _np_ptr(nnz), _np_ptr(pnnz),
+                                               C.byref(secs), _np_ptr(sweeps))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_mesh_multigrid_info")
+    L = int(n.value)
+    return {"levels": L, "rows": rows[:L].tolist(), "nnz": nnz[:L].tolist(), "p_nnz": pnnz[:L].tolist(),
+            "build_seconds": float(secs.value), "sweeps": {1: sweeps[:3].tolist(), 2: sweeps[3:].tolist()}}
 
 
 def if_mesh_export_perm(h: Handle) -> np.ndarray:

@@ -153,6 +153,7 @@ struct if_mesh_s {
     // multigrid hierarchy (IF_FLAG_MULTIGRID), see MgLevel
     ifl::MgLevel mg[ifl::MG_MAX_LEVELS];
     int mg_levels = 0;              // 0: no hierarchy
+    double mg_build_seconds = 0.0;  // wall clock of mg_build
     // pinned host staging for per-call control data and read-back
     void* h_pinned = nullptr;
     size_t h_pinned_bytes = 0;

@@ -14,6 +14,7 @@
 #include <cub/cub.cuh>
 
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -516,6 +517,7 @@ void mg_free(if_mesh_s* h) {
 }
 
 int mg_build(if_mesh_s* h) {
+    const auto t_start = std::chrono::steady_clock::now();
     cudaStream_t st = 0;
     const int64_t nv = h->n_vert;
     int log2c = 0;
@@ -557,6 +559,8 @@ int mg_build(if_mesh_s* h) {
         ++L;
     }
     h->mg_levels = L;
+    IF_CUDA_TRY(cudaStreamSynchronize(st));
+    h->mg_build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
     if (getenv("IF_VERBOSE"))
         for (int l = 0; l < L; ++l)
             fprintf(stderr, "[implicit_filter] multigrid level %d: %lld rows, %.1f entries per row, rho(S) %.3f, rho(M) %.3f, "

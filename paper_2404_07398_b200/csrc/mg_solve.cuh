@@ -27,7 +27,7 @@ namespace ifl {
 namespace {
 
 constexpr int MGK = 16;               // columns of the multigrid path
-constexpr int MG_REFILL_MIN = 4;      // stopped columns wait until this many can be restarted together (solve.cu)
+constexpr int MG_REFILL_MIN = 1;      // stopped columns are restarted as soon as this many are free (solve.cu)
 // right-hand sides below this many mean edge lengths stay on the Jacobi path (option mg_min_ell = 0)
 constexpr double MG_MIN_ELL_N1 = 4.0;
 constexpr double MG_MIN_ELL_N2 = 0.5;
