@@ -14,6 +14,8 @@
  *   mass       PAPER.md:61      M^L = diag(A_v), A_v = median-dual area = sum of area_t/3 (Fig. 1a, :41)
  *   operator   PAPER.md:61,:63  A_l = M + gamma l^2 S           (n = 1)
  *                               A_l = M + gamma l^4 S M^-1 S    (n = 2)      gamma = 1/2
+ *                               A_l = M + gamma l^(2n) S (M^-1 S)^(n-1)  (n = 3, 4: "This procedure can be generalized
+ *                               to higher-order filters"; the four-Laplacian filter of PAPER.md:201-205)
  *   solve      PAPER.md:113     conjugate gradients on A_l x = M phi started from x0 = phi (the
  *                               Guedot subtraction), Jacobi preconditioner (reading A8),
  *                               stop at ||r||_2 <= tol ||M phi||_2 (reading A6; tol 1e-13 by default)
@@ -183,10 +185,24 @@ void orc_apply_S(const orc_mesh *m, const double *p, double *y) {
     }
 }
 
-/* out = A_l p,  A_l = M + gamma l^(2n) S (M^-1 S)^(n-1)   (PAPER.md:61 n=1, PAPER.md:63 n=2).
- * tmp: scratch [nv], used for n = 2 only. */
+/* out = A_l p,  A_l = M + gamma l^(2n) S (M^-1 S)^(n-1)   (PAPER.md:61 n=1, PAPER.md:63 n=2 and "higher-order").
+ * tmp: scratch [nv], used for n >= 2 only. */
 void orc_apply(const orc_mesh *m, double ell, int n, double gamma, const double *p, double *out, double *tmp) {
     const double c = gamma * pow(ell, 2.0 * n);
+    if (n > 2) {
+        /* the two-step derivation of PAPER.md:63 repeated: psi_1 = M^-1 S p, psi_k = M^-1 S psi_k-1, out = M p + c S psi_n-1 */
+        double *psi = (double *)malloc((size_t)m->nv * sizeof(double));
+        orc_apply_S(m, p, tmp);
+        for (int64_t v = 0; v < m->nv; ++v) psi[v] = tmp[v] / m->area[v];
+        for (int k = 2; k < n; ++k) {
+            orc_apply_S(m, psi, tmp);
+            for (int64_t v = 0; v < m->nv; ++v) psi[v] = tmp[v] / m->area[v];
+        }
+        orc_apply_S(m, psi, out);
+        for (int64_t v = 0; v < m->nv; ++v) out[v] = m->area[v] * p[v] + c * out[v];
+        free(psi);
+        return;
+    }
     if (n == 1) {
         orc_apply_S(m, p, out);
 #pragma omp parallel for schedule(static)
@@ -199,6 +215,34 @@ void orc_apply(const orc_mesh *m, double ell, int n, double gamma, const double 
 #pragma omp parallel for schedule(static)
         for (int64_t v = 0; v < m->nv; ++v) out[v] = m->area[v] * p[v] + c * out[v];
     }
+}
+
+/* diag(S (M^-1 S)^(n-1))_v for n >= 3, exactly: column v of the operator is built as a sparse vector, one factor at a
+ * time (u <- S u, u <- u / A), and its entry v is read off.  Plain and slow: a dense scratch vector with a list of the
+ * touched entries, O(ring size) per factor. */
+static double diag_higher(const orc_mesh *m, int64_t v, int n, double *u, double *w, int64_t *tu, int64_t *tw, char *mark) {
+    int64_t nu = 1;
+    u[v] = 1.0; tu[0] = v;
+    double result = 0.0;
+    for (int k = 0; k < n; ++k) {
+        /* w = S u */
+        int64_t nw = 0;
+        for (int64_t a = 0; a < nu; ++a) {
+            int64_t j = tu[a];
+            for (int64_t i = m->rowptr[j]; i < m->rowptr[j + 1]; ++i) {       /* S symmetric: column j = row j */
+                int64_t r = m->col[i];
+                if (!mark[r]) { mark[r] = 1; w[r] = 0.0; tw[nw++] = r; }
+                w[r] += m->val[i] * u[j];
+            }
+        }
+        for (int64_t a = 0; a < nu; ++a) u[tu[a]] = 0.0;
+        if (k == n - 1) result = mark[v] ? w[v] : 0.0;
+        /* u = M^-1 w */
+        for (int64_t a = 0; a < nw; ++a) { int64_t r = tw[a]; u[r] = w[r] / m->area[r]; tu[a] = r; mark[r] = 0; }
+        nu = nw;
+    }
+    for (int64_t a = 0; a < nu; ++a) u[tu[a]] = 0.0;
+    return result;
 }
 
 static double dot(int64_t n, const double *a, const double *b) {
@@ -229,6 +273,14 @@ int orc_solve(const orc_mesh *m, const double *phi, double ell, int n, double ga
         b[v] = m->area[v] * phi[v];
         x[v] = phi[v];
         d[v] = m->area[v] + c * (n == 1 ? m->sdiag[v] : m->gdiag[v]);   /* diag(A_l) */
+    }
+    if (n > 2) {   /* diag(A_l) for the higher orders, computed exactly row by row */
+        double *u = (double *)calloc((size_t)nv, sizeof(double)), *w = (double *)calloc((size_t)nv, sizeof(double));
+        int64_t *tu = (int64_t *)malloc((size_t)nv * sizeof(int64_t)), *tw = (int64_t *)malloc((size_t)nv * sizeof(int64_t));
+        char *mark = (char *)calloc((size_t)nv, 1);
+        if (!u || !w || !tu || !tw || !mark) { free(u); free(w); free(tu); free(tw); free(mark); status = 4; goto done; }
+        for (int64_t v = 0; v < nv; ++v) d[v] = m->area[v] + c * diag_higher(m, v, n, u, w, tu, tw, mark);
+        free(u); free(w); free(tu); free(tw); free(mark);
     }
     orc_apply(m, ell, n, gamma, x, q, tmp);
     for (int64_t v = 0; v < nv; ++v) { r[v] = b[v] - q[v]; z[v] = r[v] / d[v]; p[v] = z[v]; }
@@ -291,7 +343,7 @@ int orc_dense_solve(const orc_mesh *m, const double *phi, double ell, int n, dou
         for (int64_t i = m->rowptr[v]; i < m->rowptr[v + 1]; ++i) Sd[v * nv + m->col[i]] = m->val[i];
     if (n == 1) {
         for (int64_t i = 0; i < nv * nv; ++i) A[i] = c * Sd[i];
-    } else {
+    } else if (n == 2) {
         for (int64_t i = 0; i < nv; ++i)
             for (int64_t k = 0; k < nv; ++k) {
                 double sik = Sd[i * nv + k];
@@ -299,6 +351,25 @@ int orc_dense_solve(const orc_mesh *m, const double *phi, double ell, int n, dou
                 double f = c * sik / m->area[k];
                 for (int64_t j = 0; j < nv; ++j) A[i * nv + j] += f * Sd[k * nv + j];
             }
+    } else {
+        /* A = c S (M^-1 S)^(n-1): P <- S, then n-1 times P <- P M^-1 S */
+        double *P = (double *)malloc((size_t)(nv * nv) * sizeof(double));
+        double *Q = (double *)calloc((size_t)(nv * nv), sizeof(double));
+        if (!P || !Q) { free(P); free(Q); free(Sd); free(A); return 4; }
+        memcpy(P, Sd, (size_t)(nv * nv) * sizeof(double));
+        for (int f = 1; f < n; ++f) {
+            memset(Q, 0, (size_t)(nv * nv) * sizeof(double));
+            for (int64_t i = 0; i < nv; ++i)
+                for (int64_t k = 0; k < nv; ++k) {
+                    double pik = P[i * nv + k];
+                    if (pik == 0.0) continue;
+                    double g = pik / m->area[k];
+                    for (int64_t j = 0; j < nv; ++j) Q[i * nv + j] += g * Sd[k * nv + j];
+                }
+            double *T = P; P = Q; Q = T;
+        }
+        for (int64_t i = 0; i < nv * nv; ++i) A[i] = c * P[i];
+        free(P); free(Q);
     }
     for (int64_t v = 0; v < nv; ++v) A[v * nv + v] += m->area[v];
     /* Cholesky A = L L^T, lower triangle in place */
