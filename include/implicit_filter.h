@@ -10,7 +10,8 @@
  *                (PAPER.md:57-61), space-filling-curve reordering, SELL-C-sigma packing.
  *   if_filter    coarse-grained fields  phibar_l  for many fields and scales l:
  *                    (M + gamma l^(2n) S (M^-1 S)^(n-1)) phibar_l = M phi        (eq.(1), :61, :63)
- *                M = diag(A_v), gamma = 1/2, n = 1 harmonic / n = 2 biharmonic,
+ *                M = diag(A_v), gamma = 1/2, n = 1 harmonic / n = 2 biharmonic / n = 3, 4 ("can be
+ *                generalized to higher-order filters"; the four-Laplacian filter of PAPER.md:201-205),
  *                solved by Jacobi-preconditioned conjugate gradients started from phi.
  *   if_spectrum  the same solves followed by e_l = 1/2 sum_v A_v phibar_l,v^2 / sum_v A_v  ("second moment
  *                of the field over scales") and its differences over k_l = 1/l.
@@ -47,7 +48,7 @@ typedef struct if_mesh_s* if_handle; /* opaque; owns all device-resident mesh ar
 enum {
     IF_OK = 0,
     IF_WNOTCONVERGED = 1, /* some right-hand side stopped on max_iter or breakdown                         */
-    IF_EINVAL = -1,       /* null pointer, dim not 2|3, order_n not 1|2, l <= 0 or non-finite, too few scales */
+    IF_EINVAL = -1,       /* null pointer, dim not 2|3, order_n not 1..4, l <= 0 or non-finite, too few scales */
     IF_EINDEX = -2,       /* triangle vertex id out of range, or a vertex repeated inside a triangle       */
     IF_EDEGENERATE = -3,  /* triangle with |e1 x e2| <= 1e-14 (|e1|^2 + |e2|^2)                             */
     IF_EORPHAN = -4,      /* vertex in no triangle: A_v = 0, M singular                                    */
@@ -61,8 +62,12 @@ enum {
     IF_FLAG_KEEP_CSR = 1, /* if_prepare keeps the unpermuted CSR of S so if_mesh_export_csr works */
     IF_FLAG_MULTIGRID = 4, /* if_prepare also builds the smoothed-aggregation hierarchy that if_options.solver = 1 needs
                               (about 3 x the memory of the prepared mesh, a second or two of device time)          */
-    IF_FLAG_HIGHPASS = 2  /* if_filter (per call): write the high-pass field phi - phibar_l (PAPER.md:143-147,
+    IF_FLAG_HIGHPASS = 2, /* if_filter (per call): write the high-pass field phi - phibar_l (PAPER.md:143-147,
                              Fig. 3) instead of phibar_l                                                    */
+    IF_FLAG_PAIRS = 8     /* if_spectrum (per call): the fields are velocity components in pairs (u_0, v_0, u_1, v_1, ...)
+                             and the spectra of a pair are added (kinetic energy 1/2 <u^2 + v^2>, the quantity of
+                             PAPER.md:149-157): n_fields even; energy is [n_fields/2][n_ells], E [n_fields/2][n_ells-1];
+                             if_stats stays per field                                                           */
 };
 
 typedef struct {
@@ -118,11 +123,12 @@ typedef struct {
 int if_prepare(const double* coords, int dim, int64_t n_vert, const int32_t* tri, int64_t n_tri,
                const double* period, const if_options* opt, if_handle* out);
 
-/* Bytes of DEVICE workspace if_filter / if_spectrum / if_apply need for this order and batch (0 => default). */
+/* Bytes of DEVICE workspace if_filter / if_spectrum / if_apply need for this order (1..4) and batch (0 => default). */
 int if_workspace_bytes(if_handle h, int order_n, int batch, size_t* bytes);
 
 /* Solving phase.  d_fields DEVICE [n_fields][n_vert]; ells HOST [n_ells] (> 0, coordinate units, any order);
- * order_n 1|2; d_out DEVICE [n_fields][n_ells][n_vert]; d_workspace DEVICE, ws_bytes >= if_workspace_bytes;
+ * order_n 1..4 (the condition number grows like (l^2 lambda_max)^n: fp64 carries n = 3 to about 6 and n = 4 to about 2.5
+ * edge lengths, beyond that the call returns IF_WNOTCONVERGED like n = 2 beyond 32); d_out DEVICE [n_fields][n_ells][n_vert]; d_workspace DEVICE, ws_bytes >= if_workspace_bytes;
  * opt NULL => the options given to if_prepare; stats NULL or HOST. */
 int if_filter(if_handle h, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
               double* d_out, void* d_workspace, size_t ws_bytes, void* cuda_stream, const if_options* opt,

@@ -20,6 +20,7 @@ IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKS
 IF_FLAG_KEEP_CSR = 1
 IF_FLAG_HIGHPASS = 2
 IF_FLAG_MULTIGRID = 4
+IF_FLAG_PAIRS = 8
 
 EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_spectrum_host", "if_apply", "if_mesh_info", "if_mesh_tile_info",
            "if_mesh_multigrid_info",
@@ -268,9 +269,10 @@ def if_spectrum(h: Handle, fields, ells: Sequence[float], order_n: int, workspac
     f = _device_fields(h, fields)
     el = np.ascontiguousarray(ells, dtype=np.float64)
     Fn, Ln = f.shape[0], el.shape[0]
-    energy = np.zeros((Fn, Ln), dtype=np.float64)
+    Fo = Fn // 2 if (options.get("flags") or 0) & IF_FLAG_PAIRS else Fn     # velocity pairs: one spectrum per (u, v)
+    energy = np.zeros((Fo, Ln), dtype=np.float64)
     k_mid = np.zeros(max(Ln - 1, 0), dtype=np.float64)
-    E = np.zeros((Fn, max(Ln - 1, 0)), dtype=np.float64)
+    E = np.zeros((Fo, max(Ln - 1, 0)), dtype=np.float64)
     opt = _options(**options)
     ws = h.workspace(order_n, options.get("batch") or 0) if workspace is None else workspace
     st = _Stats(Fn * Ln, (Fn, Ln))
@@ -293,9 +295,10 @@ def if_spectrum_host(h: Handle, fields, ells: Sequence[float], order_n: int, wor
         raise ValueError(f"fields must be a contiguous float64 HOST array [F][{h.n_vert}]")
     el = np.ascontiguousarray(ells, dtype=np.float64)
     Fn, Ln = t.shape[0], el.shape[0]
-    energy = np.zeros((Fn, Ln), dtype=np.float64)
+    Fo = Fn // 2 if (options.get("flags") or 0) & IF_FLAG_PAIRS else Fn     # velocity pairs: one spectrum per (u, v)
+    energy = np.zeros((Fo, Ln), dtype=np.float64)
     k_mid = np.zeros(max(Ln - 1, 0), dtype=np.float64)
-    E = np.zeros((Fn, max(Ln - 1, 0)), dtype=np.float64)
+    E = np.zeros((Fo, max(Ln - 1, 0)), dtype=np.float64)
     opt = _options(**options)
     need = if_workspace_bytes(h, order_n, options.get("batch") or 0) + Fn * h.n_vert * 8
     if workspace is None:

@@ -143,6 +143,8 @@ struct if_mesh_s {
     double* inv_area = nullptr;     // [n_vert] 1/A_v
     double* sdiag = nullptr;        // [n_vert] S_vv
     double* gdiag = nullptr;        // [n_vert] sum_j S_vj^2/A_j = diag(S M^-1 S)
+    double* gdiag3 = nullptr;       // [n_vert] diag(S (M^-1 S)^2)   (filter order 3)
+    double* gdiag4 = nullptr;       // [n_vert] diag(S (M^-1 S)^3)   (filter order 4)
     int32_t* perm = nullptr;        // [n_vert] internal -> caller
     int32_t* iperm = nullptr;       // [n_vert] caller -> internal
     // optional unpermuted CSR (IF_FLAG_KEEP_CSR), caller numbering

@@ -38,6 +38,8 @@ struct MeshView {
     const double* __restrict__ inv_area;
     const double* __restrict__ sdiag;
     const double* __restrict__ gdiag;
+    const double* __restrict__ gdiag3;
+    const double* __restrict__ gdiag4;
     const int32_t* __restrict__ perm;
     const int32_t* __restrict__ lcol;       // tile-local column ids (tile row, or TILE_ROWS + halo slot)
     const int32_t* __restrict__ halo_rows;  // [tiles][HALO_CAP] out-of-tile rows each tile gathers from
@@ -46,6 +48,11 @@ struct MeshView {
     int64_t n_chunks;
     int log2c;
 };
+
+// diag(S (M^-1 S)^(n-1)) for the Jacobi preconditioner of order n
+__device__ __forceinline__ const double* jacobi_diag(const MeshView& m, int order_n) {
+    return order_n == 1 ? m.sdiag : order_n == 2 ? m.gdiag : order_n == 3 ? m.gdiag3 : m.gdiag4;
+}
 
 struct Ctrl {
     double c[KMAX];       // gamma l^(2n)
@@ -795,7 +802,7 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
     const int tid = threadIdx.x, l = tid % TPR;
     const bool on0 = (mask >> (2 * l)) & 1u, on1 = (mask >> (2 * l + 1)) & 1u;
     const double2 cc = {sp.c[2 * l], sp.c[2 * l + 1]};
-    const double* __restrict__ dg = order_n == 1 ? m.sdiag : m.gdiag;
+    const double* __restrict__ dg = jacobi_diag(m, order_n);
     double2 acc[3] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
     if (on0 || on1) {
         for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < m.nv; row += (int64_t)gridDim.x * ROWS) {
@@ -863,7 +870,7 @@ __global__ void __launch_bounds__(BLOCK, 2) k_update(MeshView m, Ctrl* __restric
     const int tid = threadIdx.x, l = tid % TPR;
     const double2 cc = ld2(ctrl->c, 2 * l);
     const double2 alpha = ld2(ctrl->alpha, 2 * l);
-    const double* __restrict__ dg = order_n == 1 ? m.sdiag : m.gdiag;
+    const double* __restrict__ dg = jacobi_diag(m, order_n);
     double2 acc[2] = {{0.0, 0.0}, {0.0, 0.0}};
     const int64_t stride = (int64_t)gridDim.x * ROWS;
     for (int64_t base = (int64_t)blockIdx.x * ROWS + tid / TPR; base < m.nv; base += U * stride) {
@@ -1001,6 +1008,14 @@ __global__ void k_stats(const Ctrl* __restrict__ ctrl, int K, unsigned mask, int
         status[r] = ctrl->status[c];
         relres[r] = ctrl->bb[c] > 0.0 ? sqrt(ctrl->rr[c] / ctrl->bb[c]) : 0.0;
     }
+}
+
+// velocity pairs (IF_FLAG_PAIRS): e_pair[i][j] = e[2i][j] + e[2i+1][j]   (1/2 <u^2 + v^2>: the two spectra add)
+__global__ void k_pair_sum(const double* __restrict__ energy, int n_pairs, int n_ells, double* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_pairs * n_ells) return;
+    const int p = i / n_ells, j = i % n_ells;
+    out[i] = energy[(2 * p) * n_ells + j] + energy[(2 * p + 1) * n_ells + j];
 }
 
 // H7: k_j = 1/l_j ; E_j = (e_j - e_j+1)/(k_j - k_j+1) ; k_mid_j = sqrt(k_j k_j+1)

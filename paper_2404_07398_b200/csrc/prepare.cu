@@ -136,6 +136,53 @@ __global__ void k_gdiag(const int64_t* __restrict__ rowptr, const int32_t* __res
     gdiag[v] = g;
 }
 
+// Jacobi diagonals of the higher orders ("can be generalized to higher-order filters"), exactly.
+// With y = column v of M^-1 S (the one-ring of v: y_j = S_vj / A_j, S symmetric):
+//   n = 3:  diag(S M^-1 S M^-1 S)_v = y^T S y = sum_j y_j sum_{k in row(j), k in row(v)} S_jk y_k
+//   n = 4:  diag(S (M^-1 S)^3)_v = z^T M^-1 z,  z = S y (the two-ring of v) = sum_k z_k^2 / A_k
+// Columns are ascending inside a CSR row, so membership in row(v) is a binary search; z is accumulated in a small
+// per-thread table (a two-ring beyond its capacity -- valences of several dozen -- falls back to the k = v term alone,
+// a positive lower bound: the preconditioner stays symmetric positive definite, only weaker for that row).
+constexpr int RING2_CAP = 192;
+__global__ void k_gdiag_higher(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                               const double* __restrict__ val, const double* __restrict__ area, int64_t nv,
+                               double* __restrict__ gdiag3, double* __restrict__ gdiag4) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nv) return;
+    const int64_t b = rowptr[v], e = rowptr[v + 1];
+    int32_t kk[RING2_CAP];
+    double zz[RING2_CAP];
+    int nz = 0;
+    bool overflow = false;
+    double d3 = 0.0, zv = 0.0;
+    for (int64_t a = b; a < e; ++a) {
+        const int64_t j = col[a];
+        const double yj = val[a] / area[j];
+        double sy = 0.0;                                   // (S y)_j restricted to row(v) -- y vanishes elsewhere
+        for (int64_t i = rowptr[j]; i < rowptr[j + 1]; ++i) {
+            const int32_t k = col[i];
+            const double sjk = val[i];
+            int64_t lo = b, hi = e - 1;                    // k in row(v)?
+            while (lo < hi) { const int64_t mid = (lo + hi) >> 1; if (col[mid] < k) lo = mid + 1; else hi = mid; }
+            if (col[lo] == k) sy += sjk * (val[lo] / area[k]);
+            // z_k += S_kj y_j
+            if (k == v) zv += sjk * yj;
+            int t = 0;
+            while (t < nz && kk[t] != k) ++t;
+            if (t == nz) {
+                if (nz < RING2_CAP) { kk[nz] = k; zz[nz] = 0.0; ++nz; } else { overflow = true; continue; }
+            }
+            zz[t] += sjk * yj;
+        }
+        d3 += yj * sy;
+    }
+    double d4 = 0.0;
+    if (overflow) d4 = zv * zv / area[v];
+    else for (int t = 0; t < nz; ++t) d4 += zz[t] * zz[t] / area[kk[t]];
+    gdiag3[v] = d3;
+    gdiag4[v] = d4;
+}
+
 // length of each edge once (row < col), 0 elsewhere
 __global__ void k_edge_len(const double* __restrict__ coords, int dim, Period per, const int64_t* __restrict__ rowptr,
                            const int32_t* __restrict__ col, int64_t nv, double* __restrict__ out) {
@@ -223,10 +270,12 @@ __global__ void k_chunk_slots(const int32_t* __restrict__ perm, const int32_t* _
 __global__ void k_sell_fill(const int32_t* __restrict__ perm, const int32_t* __restrict__ iperm,
                             const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                             const double* __restrict__ val, const double* __restrict__ area_u,
-                            const double* __restrict__ sdiag_u, const double* __restrict__ gdiag_u, int64_t nv,
+                            const double* __restrict__ sdiag_u, const double* __restrict__ gdiag_u,
+                            const double* __restrict__ g3_u, const double* __restrict__ g4_u, int64_t nv,
                             int64_t n_chunks, int C, const int64_t* __restrict__ chunk_ptr,
                             int32_t* __restrict__ sell_col, double* __restrict__ sell_val, double* __restrict__ area,
-                            double* __restrict__ inv_area, double* __restrict__ sdiag, double* __restrict__ gdiag) {
+                            double* __restrict__ inv_area, double* __restrict__ sdiag, double* __restrict__ gdiag,
+                            double* __restrict__ gdiag3, double* __restrict__ gdiag4) {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n_chunks * C) return;
     int64_t c = r / C;
@@ -246,6 +295,8 @@ __global__ void k_sell_fill(const int32_t* __restrict__ perm, const int32_t* __r
         inv_area[r] = 1.0 / area_u[u];
         sdiag[r] = sdiag_u[u];
         gdiag[r] = gdiag_u[u];
+        gdiag3[r] = g3_u[u];
+        gdiag4[r] = g4_u[u];
     }
     for (; k < w; ++k) { sell_col[o + k] = self; sell_val[o + k] = 0.0; }
 }
@@ -362,7 +413,7 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
             o.sfc_kind = in->sfc_kind;
             o.flags = in->flags;
         } else {   // per-call flags
-            o.flags = (o.flags & ~IF_FLAG_HIGHPASS) | (in->flags & IF_FLAG_HIGHPASS);
+            o.flags = (o.flags & ~(IF_FLAG_HIGHPASS | IF_FLAG_PAIRS)) | (in->flags & (IF_FLAG_HIGHPASS | IF_FLAG_PAIRS));
         }
     }
     if (!(o.gamma > 0.0) || !std::isfinite(o.gamma) || !(o.tol > 0.0) || !std::isfinite(o.tol)) return IF_EINVAL;
@@ -387,7 +438,7 @@ extern "C" void if_destroy(if_handle h) {
     cudaGetDevice(&prev);
     cudaSetDevice(h->device);
     cudaFree(h->chunk_ptr); cudaFree(h->sell_col); cudaFree(h->sell_val); cudaFree(h->area);
-    cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->perm); cudaFree(h->iperm);
+    cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->gdiag3); cudaFree(h->gdiag4); cudaFree(h->perm); cudaFree(h->iperm);
     cudaFree(h->sell_lcol); cudaFree(h->halo_n); cudaFree(h->tile_desc); cudaFree(h->halo_rows);
     ifl::mg_free(h);
     cudaFree(h->csr_rowptr); cudaFree(h->csr_col); cudaFree(h->csr_val); cudaFree(h->csr_area);
@@ -480,12 +531,14 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     // now: k0 = unique keys [nnz], v0 = summed values [nnz]
 
     // ---- CSR in the caller's numbering, A_v, S_vv, g_v
-    DevBuf rowptr, ccol, area_u, sdiag_u, gdiag_u, len;
+    DevBuf rowptr, ccol, area_u, sdiag_u, gdiag_u, g3_u, g4_u, len;
     IF_CUDA_TRY(rowptr.alloc((size_t)(nv + 1) * sizeof(int64_t)));
     IF_CUDA_TRY(ccol.alloc((size_t)nnz * sizeof(int32_t)));
     IF_CUDA_TRY(area_u.alloc((size_t)nv * 8));
     IF_CUDA_TRY(sdiag_u.alloc((size_t)nv * 8));
     IF_CUDA_TRY(gdiag_u.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(g3_u.alloc((size_t)nv * 8));
+    IF_CUDA_TRY(g4_u.alloc((size_t)nv * 8));
     IF_CUDA_TRY(len.alloc((size_t)nv * 4));
     k_rowptr<<<grid_for(nnz + 1), 256, 0, st>>>(k0.as<unsigned long long>(), nnz, nv, rowptr.as<int64_t>());
     IF_LAUNCH_CHECK();
@@ -498,6 +551,9 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     if (flags & FLAG_ORPHAN) return IF_EORPHAN;
     k_gdiag<<<grid_for(nv), 256, 0, st>>>(rowptr.as<int64_t>(), ccol.as<int32_t>(), v0.as<double>(),
                                          area_u.as<double>(), nv, gdiag_u.as<double>());
+    IF_LAUNCH_CHECK();
+    k_gdiag_higher<<<grid_for(nv, 128), 128, 0, st>>>(rowptr.as<int64_t>(), ccol.as<int32_t>(), v0.as<double>(),
+                                                      area_u.as<double>(), nv, g3_u.as<double>(), g4_u.as<double>());
     IF_LAUNCH_CHECK();
 
     // total area and mean edge length (deterministic device reductions)
@@ -577,7 +633,7 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     IF_CUDA_TRY(cudaStreamSynchronize(st));
     h->sell_slots = sell_slots;
 
-    DevBuf scol, sval, area, inv_area, sdiag, gdiag;
+    DevBuf scol, sval, area, inv_area, sdiag, gdiag, gdiag3, gdiag4;
     IF_CUDA_TRY(scol.alloc((size_t)sell_slots * 4 + 16));
     IF_CUDA_TRY(sval.alloc((size_t)sell_slots * 8 + 16));
     IF_CUDA_TRY(area.alloc((size_t)nv * 8 + 16));   // +16: the SpMM kernel bulk-copies 16-byte multiples
@@ -588,11 +644,15 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     IF_CUDA_TRY(cudaMemsetAsync(sdiag.p, 0, (size_t)nv * 8 + 16, st));
     IF_CUDA_TRY(gdiag.alloc((size_t)nv * 8 + 16));   // +16: the SpMM kernel bulk-copies 16-byte multiples
     IF_CUDA_TRY(cudaMemsetAsync(gdiag.p, 0, (size_t)nv * 8 + 16, st));
+    IF_CUDA_TRY(gdiag3.alloc((size_t)nv * 8 + 16));
+    IF_CUDA_TRY(cudaMemsetAsync(gdiag3.p, 0, (size_t)nv * 8 + 16, st));
+    IF_CUDA_TRY(gdiag4.alloc((size_t)nv * 8 + 16));
+    IF_CUDA_TRY(cudaMemsetAsync(gdiag4.p, 0, (size_t)nv * 8 + 16, st));
     k_sell_fill<<<grid_for(n_chunks * C), 256, 0, st>>>(
         perm.as<int32_t>(), iperm.as<int32_t>(), rowptr.as<int64_t>(), ccol.as<int32_t>(), v0.as<double>(),
-        area_u.as<double>(), sdiag_u.as<double>(), gdiag_u.as<double>(), nv, n_chunks, C, chunk_ptr.as<int64_t>(),
-        scol.as<int32_t>(), sval.as<double>(), area.as<double>(), inv_area.as<double>(), sdiag.as<double>(),
-        gdiag.as<double>());
+        area_u.as<double>(), sdiag_u.as<double>(), gdiag_u.as<double>(), g3_u.as<double>(), g4_u.as<double>(), nv,
+        n_chunks, C, chunk_ptr.as<int64_t>(), scol.as<int32_t>(), sval.as<double>(), area.as<double>(),
+        inv_area.as<double>(), sdiag.as<double>(), gdiag.as<double>(), gdiag3.as<double>(), gdiag4.as<double>());
     IF_LAUNCH_CHECK();
     IF_CUDA_TRY(cudaStreamSynchronize(st));
 
@@ -646,6 +706,8 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     h->inv_area = (double*)inv_area.release();
     h->sdiag = (double*)sdiag.release();
     h->gdiag = (double*)gdiag.release();
+    h->gdiag3 = (double*)gdiag3.release();
+    h->gdiag4 = (double*)gdiag4.release();
     h->perm = (int32_t*)perm.release();
     h->iperm = (int32_t*)iperm.release();
 
@@ -717,7 +779,7 @@ extern "C" int if_mesh_export_perm(if_handle h, int32_t* perm) {
 // ------------------------------------------------------------------------------------------- save / load
 namespace {
 struct FileHeader {
-    char magic[8];            // "IFMESH01"
+    char magic[8];            // "IFMESH02"
     int32_t tile_rows, halo_cap, sell_c, pad_;
     int64_t n_vert, nnz, n_chunks, sell_slots, n_tiles, halo_total, halo_max, unstaged_tiles;
     double total_area, mean_edge;
@@ -746,13 +808,14 @@ extern "C" int if_save(if_handle h, const char* path) {
     if (!f) return IF_EIO;
     FileHeader hd;
     memset(&hd, 0, sizeof(hd));
-    memcpy(hd.magic, "IFMESH01", 8);
+    memcpy(hd.magic, "IFMESH02", 8);
     hd.tile_rows = TILE_ROWS; hd.halo_cap = HALO_CAP; hd.sell_c = h->sell_c;
+    hd.pad_ = (int32_t)sizeof(ifl::Options);   // the options are stored raw: their layout is part of the format
     hd.n_vert = h->n_vert; hd.nnz = h->nnz; hd.n_chunks = h->n_chunks; hd.sell_slots = h->sell_slots;
     hd.n_tiles = h->n_tiles; hd.halo_total = h->halo_total; hd.halo_max = h->halo_max;
     hd.unstaged_tiles = h->unstaged_tiles; hd.total_area = h->total_area; hd.mean_edge = h->mean_edge;
     hd.opt = h->opt;
-    hd.opt.flags &= ~(IF_FLAG_KEEP_CSR | IF_FLAG_HIGHPASS);
+    hd.opt.flags &= ~(IF_FLAG_KEEP_CSR | IF_FLAG_HIGHPASS | IF_FLAG_PAIRS);
     std::vector<char> buf;
     const size_t nv = (size_t)h->n_vert, ns = (size_t)h->sell_slots, nt = (size_t)h->n_tiles;
     int rc = fwrite(&hd, sizeof(hd), 1, f) == 1 ? IF_OK : IF_EIO;
@@ -764,6 +827,8 @@ extern "C" int if_save(if_handle h, const char* path) {
     if (rc == IF_OK) rc = write_dev(f, h->inv_area, nv * 8, buf);
     if (rc == IF_OK) rc = write_dev(f, h->sdiag, nv * 8, buf);
     if (rc == IF_OK) rc = write_dev(f, h->gdiag, nv * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->gdiag3, nv * 8, buf);
+    if (rc == IF_OK) rc = write_dev(f, h->gdiag4, nv * 8, buf);
     if (rc == IF_OK) rc = write_dev(f, h->perm, nv * 4, buf);
     if (rc == IF_OK) rc = write_dev(f, h->iperm, nv * 4, buf);
     if (rc == IF_OK) rc = write_dev(f, h->halo_n, nt * 4, buf);
@@ -780,10 +845,33 @@ extern "C" int if_load(const char* path, if_handle* out) {
     FILE* f = fopen(path, "rb");
     if (!f) return IF_EIO;
     FileHeader hd;
-    if (fread(&hd, sizeof(hd), 1, f) != 1 || memcmp(hd.magic, "IFMESH01", 8) != 0 || hd.tile_rows != TILE_ROWS ||
+    if (fread(&hd, sizeof(hd), 1, f) != 1 || memcmp(hd.magic, "IFMESH02", 8) != 0 || hd.tile_rows != TILE_ROWS ||
         hd.halo_cap != HALO_CAP || hd.n_vert < 3 || hd.sell_slots < 0 || hd.n_tiles != (hd.n_vert + TILE_ROWS - 1) / TILE_ROWS) {
         fclose(f);
         return IF_EIO;
+    }
+    {
+        // the header is not trusted: sizes must fit each other, the library's allowed values and the file's length
+        ifl::Options chk;
+        bool ok = hd.pad_ == (int32_t)sizeof(ifl::Options) && (hd.sell_c == 32 || hd.sell_c == 64 || hd.sell_c == 128) &&
+                  TILE_ROWS % hd.sell_c == 0 && hd.n_vert <= 0x7fffffffLL &&
+                  hd.n_chunks == (hd.n_vert + hd.sell_c - 1) / hd.sell_c && hd.nnz >= hd.n_vert &&
+                  hd.sell_slots >= hd.nnz - hd.n_vert && hd.sell_slots % 2 == 0 && hd.opt.sell_c == hd.sell_c;
+        if (ok) {
+            if_options raw{};
+            raw.gamma = hd.opt.gamma; raw.tol = hd.opt.tol; raw.max_iter = hd.opt.max_iter;
+            raw.check_every = hd.opt.check_every; raw.batch = hd.opt.batch; raw.sell_c = hd.opt.sell_c;
+            raw.sell_sigma = hd.opt.sell_sigma; raw.sfc_kind = hd.opt.sfc_kind; raw.flags = hd.opt.flags;
+            raw.solver = hd.opt.solver; raw.mg_min_ell = hd.opt.mg_min_ell;
+            ok = ifl::resolve_options(&raw, nullptr, &chk) == IF_OK;
+        }
+        if (ok) {
+            const int64_t nv = hd.n_vert, ns = hd.sell_slots, nt = hd.n_tiles;
+            const int64_t expect = (int64_t)sizeof(hd) + (hd.n_chunks + 1) * 8 + ns * 16 + nv * (6 * 8 + 2 * 4) + nt * 4 +
+                                   nt * HALO_CAP * 4 + (nt + 1) * 64;
+            ok = fseek(f, 0, SEEK_END) == 0 && (int64_t)ftell(f) == expect && fseek(f, (long)sizeof(hd), SEEK_SET) == 0;
+        }
+        if (!ok) { fclose(f); return IF_EIO; }
     }
     if_mesh_s* h = new (std::nothrow) if_mesh_s();
     if (!h) { fclose(f); return IF_ENOMEM; }
@@ -799,6 +887,11 @@ extern "C" int if_load(const char* path, if_handle* out) {
     const size_t nv = (size_t)h->n_vert, ns = (size_t)h->sell_slots, nt = (size_t)h->n_tiles;
     int rc;
     if ((rc = read_dev(f, (void**)&h->chunk_ptr, (size_t)(h->n_chunks + 1) * 8, (size_t)(h->n_chunks + 1) * 8, buf))) return fail(rc);
+    {
+        int64_t last = -1;
+        memcpy(&last, buf.data() + (size_t)h->n_chunks * 8, 8);
+        if (last != h->sell_slots) return fail(IF_EIO);
+    }
     if ((rc = read_dev(f, (void**)&h->sell_col, ns * 4, ns * 4 + 16, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->sell_val, ns * 8, ns * 8 + 16, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->sell_lcol, ns * 4, ns * 4 + 16, buf))) return fail(rc);
@@ -806,6 +899,8 @@ extern "C" int if_load(const char* path, if_handle* out) {
     if ((rc = read_dev(f, (void**)&h->inv_area, nv * 8, nv * 8 + 16, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->sdiag, nv * 8, nv * 8 + 16, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->gdiag, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->gdiag3, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+    if ((rc = read_dev(f, (void**)&h->gdiag4, nv * 8, nv * 8 + 16, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->perm, nv * 4, nv * 4, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->iperm, nv * 4, nv * 4, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->halo_n, nt * 4, nt * 4, buf))) return fail(rc);

@@ -18,8 +18,8 @@ constexpr int MAX_BLOCKS_PER_SM = 8;
 struct Workspace {
     Ctrl* ctrl;
     double* partials;
-    double *x, *z, *p0, *p1, *q, *t;
-    double *energy, *relres, *ells, *k_mid, *E;
+    double *x, *z, *p0, *p1, *q, *t, *t2;
+    double *energy, *relres, *ells, *k_mid, *E, *epair;
     int32_t *iters, *status;
     void* mg_extra;   // buffers of the multigrid path (mg_solve.cuh), NULL if the handle has no hierarchy
     size_t bytes;
@@ -42,12 +42,14 @@ Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* bas
     w.p0 = (double*)take(vec);
     w.p1 = (double*)take(vec);
     w.q = (double*)take(vec);
-    w.t = order_n == 2 ? (double*)take(vec) : nullptr;
+    w.t = order_n >= 2 ? (double*)take(vec) : nullptr;
+    w.t2 = order_n >= 3 ? (double*)take(vec) : nullptr;
     w.energy = (double*)take(MAX_RHS * sizeof(double));
     w.relres = (double*)take(MAX_RHS * sizeof(double));
     w.ells = (double*)take(MAX_RHS * sizeof(double));
     w.k_mid = (double*)take(MAX_RHS * sizeof(double));
     w.E = (double*)take(MAX_RHS * sizeof(double));
+    w.epair = (double*)take(MAX_RHS * sizeof(double));
     w.iters = (int32_t*)take(MAX_RHS * sizeof(int32_t));
     w.status = (int32_t*)take(MAX_RHS * sizeof(int32_t));
     w.mg_extra = nullptr;
@@ -150,6 +152,19 @@ struct IterTimer {
 namespace ifl {
 namespace {
 
+// `count` more factors t <- M^-1 S t of the higher-order operators, alternating between w.t and w.t2; *t = the result
+template <int K>
+int more_factors(const Run& r, int count, double** t) {
+    int rc;
+    for (int k = 0; k < count; ++k) {
+        double* dst = *t == r.w.t ? r.w.t2 : r.w.t;
+        SpmmArgs f{*t, nullptr, nullptr, dst, nullptr, 1, 0};
+        if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, f))) return rc;
+        *t = dst;
+    }
+    return IF_OK;
+}
+
 // One CG iteration: kernel A (two launches for n = 2) and kernel B.  The direction buffers are picked on the device
 // from ctrl->cur_p, so every iteration is the same launch sequence and a graph may resume at any iteration.
 template <int K>
@@ -160,9 +175,13 @@ int enqueue_iteration(const Run& r, IterTimer* tm = nullptr) {
         SpmmArgs a{r.w.z, r.w.p0, r.w.x, r.w.q, r.w.p1, 0, 1};
         if ((rc = launch_spmm<K, MODE_CG1>(r, r.g.cga, a))) return rc;
     } else {
+        // S (M^-1 S)^(n-1) p' one factor at a time: t = M^-1 S p', n - 2 more factors t <- M^-1 S t
+        // between the two buffers, q = M p' + c S t
         SpmmArgs a{r.w.z, r.w.p0, r.w.x, r.w.t, r.w.p1, 0, 1};
         if ((rc = launch_spmm<K, MODE_CG2A>(r, r.g.cga, a))) return rc;
-        SpmmArgs b{r.w.t, r.w.p0, nullptr, r.w.q, r.w.p1, 0, 1};
+        double* t = r.w.t;
+        if ((rc = more_factors<K>(r, r.order_n - 2, &t))) return rc;
+        SpmmArgs b{t, r.w.p0, nullptr, r.w.q, r.w.p1, 0, 1};
         if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
     }
     if (tm && (rc = tm->mark(r.st, 0))) return rc;
@@ -210,7 +229,9 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
     } else {
         SpmmArgs a{r.w.x, nullptr, nullptr, r.w.t, nullptr, 1, 0};
         if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, a))) return rc;
-        SpmmArgs b{r.w.t, nullptr, nullptr, r.w.q, nullptr, 0, 0};
+        double* t = r.w.t;
+        if ((rc = more_factors<K>(r, r.order_n - 2, &t))) return rc;
+        SpmmArgs b{t, nullptr, nullptr, r.w.q, nullptr, 0, 0};
         if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, b))) return rc;
     }
     // multigrid phase: r0 into the residual buffer in use (w.z or its twin), z cleared, the column marked `starting`
@@ -280,10 +301,12 @@ int apply_all(Run& r, const double* d_fields, const std::vector<Rhs>& rhs, int n
         k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, sp, (1u << K) - 1u, d_fields, r.w.x);
         IF_LAUNCH_CHECK();
         const double* v = r.w.x;
-        if (r.order_n == 2) {
+        if (r.order_n >= 2) {
             SpmmArgs a{r.w.x, nullptr, nullptr, r.w.t, nullptr, 1, 0};
             if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, a))) return rc;
-            v = r.w.t;
+            double* t = r.w.t;
+            if ((rc = more_factors<K>(r, r.order_n - 2, &t))) return rc;
+            v = t;
         }
         SpmmArgs b{v, r.w.x, nullptr, r.w.q, nullptr, 0, 0};
         if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
@@ -482,8 +505,10 @@ int compact_columns(Run& r, QueueState& q) {
     double* t2 = w.z + vn;
     k_compact_ctrl<<<1, KMAX, 0, r.st>>>(w.ctrl, map, KN);
     IF_LAUNCH_CHECK();
+    double* t3 = w.p0;   // (the wide p0 is dead once repacked: room for the second factor buffer of n >= 3)
     w.x = x2; w.z = z2; w.p0 = p0_2; w.p1 = p1_2; w.q = q2;
-    if (r.order_n == 2) w.t = t2;
+    if (r.order_n >= 2) w.t = t2;
+    if (r.order_n >= 3) w.t2 = t3;
     q = nq;
     return IF_OK;
 }
@@ -530,10 +555,11 @@ int pick_k(int batch, size_t R) {
 int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
             double* d_out, double* energy, double* k_mid, double* E, void* d_ws, size_t ws_bytes, void* stream,
             const if_options* opt_in, if_stats* stats) {
-    if (!h || !d_fields || !ells || n_fields < 1 || n_ells < 1 || (order_n != 1 && order_n != 2) || !d_ws)
+    if (!h || !d_fields || !ells || n_fields < 1 || n_ells < 1 || order_n < 1 || order_n > 4 || !d_ws)
         return IF_EINVAL;
     if (job != JOB_SPECTRUM && !d_out) return IF_EINVAL;
     if (job == JOB_SPECTRUM && n_ells < 2) return IF_EINVAL;
+    if (job == JOB_SPECTRUM && opt_in && (opt_in->flags & IF_FLAG_PAIRS) && n_fields % 2 != 0) return IF_EINVAL;
     const int64_t R = (int64_t)n_fields * n_ells;
     if (R > MAX_RHS) return IF_EINVAL;
     for (int j = 0; j < n_ells; ++j) {
@@ -546,6 +572,8 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (rc != IF_OK) return rc;
     r.order_n = order_n;
     r.st = static_cast<cudaStream_t>(stream);
+    const bool pairs = job == JOB_SPECTRUM && (r.opt.flags & IF_FLAG_PAIRS);
+    const int n_out_fields = pairs ? n_fields / 2 : n_fields;
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return IF_ECUDA; }
     if (dev != h->device) IF_CUDA_TRY(cudaSetDevice(h->device));
@@ -553,7 +581,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (ws_bytes < r.w.bytes) return IF_EWORKSPACE;
     int log2c = 0;
     while ((1 << log2c) < h->sell_c) ++log2c;
-    r.m = MeshView{h->chunk_ptr, h->sell_col, h->sell_val, h->area, h->inv_area, h->sdiag, h->gdiag, h->perm,
+    r.m = MeshView{h->chunk_ptr, h->sell_col, h->sell_val, h->area, h->inv_area, h->sdiag, h->gdiag, h->gdiag3, h->gdiag4, h->perm,
                    h->sell_lcol, h->halo_rows, h->tile_desc, h->n_vert, h->n_chunks, log2c};
 
     PollState poll;
@@ -583,7 +611,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     KernelTimes ktimes, mgtimes;
     int64_t batch_iters = 0, mg_batch_iters = 0;
     // large scales by multigrid-preconditioned CG (option solver = 1): a stream of right-hand sides through 16 columns
-    if (job != JOB_APPLY && r.opt.solver == 1 && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
+    if (job != JOB_APPLY && r.opt.solver == 1 && order_n <= 2 && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
         const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)) *
                                h->mean_edge;
         size_t n_big = 0;
@@ -623,8 +651,15 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
     if (job == JOB_SPECTRUM) {
         IF_CUDA_TRY(cudaMemcpyAsync(r.w.ells, ells, (size_t)n_ells * sizeof(double), cudaMemcpyHostToDevice, r.st));
-        const int nb = n_fields * (n_ells - 1);
-        k_spectrum<<<(nb + 127) / 128, 128, 0, r.st>>>(r.w.energy, r.w.ells, n_fields, n_ells, r.w.k_mid, r.w.E);
+        const double* e_src = r.w.energy;
+        if (pairs) {
+            const int np = (n_fields / 2) * n_ells;
+            k_pair_sum<<<(np + 127) / 128, 128, 0, r.st>>>(r.w.energy, n_fields / 2, n_ells, r.w.epair);
+            IF_LAUNCH_CHECK();
+            e_src = r.w.epair;
+        }
+        const int nb = n_out_fields * (n_ells - 1);
+        k_spectrum<<<(nb + 127) / 128, 128, 0, r.st>>>(e_src, r.w.ells, n_out_fields, n_ells, r.w.k_mid, r.w.E);
         IF_LAUNCH_CHECK();
     }
     IF_CUDA_TRY(cudaEventRecord(t1, r.st));
@@ -638,9 +673,9 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
         IF_CUDA_TRY(cudaMemcpyAsync(h_relres.data(), r.w.relres, (size_t)R * 8, cudaMemcpyDeviceToHost, r.st));
     }
     if (job == JOB_SPECTRUM) {
-        if (energy) IF_CUDA_TRY(cudaMemcpyAsync(energy, r.w.energy, (size_t)R * 8, cudaMemcpyDeviceToHost, r.st));
+        if (energy) IF_CUDA_TRY(cudaMemcpyAsync(energy, pairs ? r.w.epair : r.w.energy, (size_t)n_out_fields * n_ells * 8, cudaMemcpyDeviceToHost, r.st));
         if (k_mid) IF_CUDA_TRY(cudaMemcpyAsync(k_mid, r.w.k_mid, (size_t)(n_ells - 1) * 8, cudaMemcpyDeviceToHost, r.st));
-        if (E) IF_CUDA_TRY(cudaMemcpyAsync(E, r.w.E, (size_t)n_fields * (n_ells - 1) * 8, cudaMemcpyDeviceToHost, r.st));
+        if (E) IF_CUDA_TRY(cudaMemcpyAsync(E, r.w.E, (size_t)n_out_fields * (n_ells - 1) * 8, cudaMemcpyDeviceToHost, r.st));
     }
     IF_CUDA_TRY(cudaStreamSynchronize(r.st));
     int result = IF_OK;
@@ -674,7 +709,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
 using namespace ifl;
 
 extern "C" int if_workspace_bytes(if_handle h, int order_n, int batch, size_t* bytes) {
-    if (!h || !bytes || (order_n != 1 && order_n != 2)) return IF_EINVAL;
+    if (!h || !bytes || order_n < 1 || order_n > 4) return IF_EINVAL;
     if (batch == 0) batch = h->opt.batch;
     if (batch != 4 && batch != 8 && batch != 16) return IF_EINVAL;
     *bytes = layout_workspace(h, order_n, batch, nullptr).bytes;
@@ -698,7 +733,7 @@ extern "C" int if_spectrum(if_handle h, const double* d_fields, int n_fields, co
 extern "C" int if_spectrum_host(if_handle h, const double* h_fields, int n_fields, const double* ells, int n_ells,
                                 int order_n, double* energy, double* k_mid, double* E, void* d_workspace,
                                 size_t ws_bytes, void* cuda_stream, const if_options* opt, if_stats* stats) {
-    if (!h || !h_fields || n_fields < 1 || !d_workspace || (order_n != 1 && order_n != 2)) return IF_EINVAL;
+    if (!h || !h_fields || n_fields < 1 || !d_workspace || order_n < 1 || order_n > 4) return IF_EINVAL;
     Options o;
     int rc = resolve_options(opt, &h->opt, &o);
     if (rc != IF_OK) return rc;
