@@ -309,20 +309,28 @@ __device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_r
 #endif
 constexpr int SPMM_BLOCK = IF_SPMM_BLOCK;
 constexpr int SPMM_STAGES = IF_SPMM_STAGES;
-// Threads per CTA, CTAs per SM and pipeline stages of k_spmm.  The 16-column layout fills an SM with one 512-thread
+// Threads per CTA, CTAs per SM and pipeline stages of k_spmm.  The 16-column CG kernels fill an SM with one 512-thread
 // CTA and three stages (186 KB).  The narrower layouts of the compacted tail have smaller stages and are bound by
 // per-tile fixed costs, not by HBM: two 256-thread CTAs per SM overlap each other's stalls (K = 8 with two stages to
-// fit shared memory).
-template <int K> struct SpmmCfg {
-    static constexpr int NT = (K == 16) ? SPMM_BLOCK : 256;
-    static constexpr int MINB = (K == 16) ? IF_SPMM_MINB : 2;
-    static constexpr int STAGES = (K == 8) ? 2 : SPMM_STAGES;
+// fit shared memory).  The multigrid sweeps (AX, MGR0) move fewer bytes per tile than kernel A and were bound the
+// same way as one CTA (0.57 of the copy bandwidth): their second vector -- needed for the tile's own rows only,
+// never gathered -- goes through registers instead of a shared-memory region (REGB), the stage shrinks to 46 KB, and
+// they run as two 256-thread CTAs per SM with two stages each (0.909 -> 0.849 ms per sweep on config 4).  MGR, which
+// also reads q and stores r', lost by the same change (1.11 -> 1.41 ms: 128 registers with spills) and stays as it was.
+template <int K, int MODE> struct SpmmCfg {
+    static constexpr bool REGB = (MODE == MODE_AX || MODE == MODE_MGR0);
+    static constexpr bool WIDE1 = (K == 16) && !REGB;              // one 512-thread CTA per SM
+    static constexpr int NT = WIDE1 ? SPMM_BLOCK : 256;
+    static constexpr int MINB = WIDE1 ? IF_SPMM_MINB : 2;
+    static constexpr int STAGES = (K == 8 || (K == 16 && REGB)) ? 2 : SPMM_STAGES;
 };
 
 template <int K, int MODE> struct TileSmem {
     static constexpr int T = TILE_ROWS;
-    static constexpr int NVEC = (MODE == MODE_PLAIN) ? 1 : 2;   // tile-sized vector regions of a stage
-    static constexpr int NLOAD = (MODE == MODE_PLAIN || MODE == MODE_MGR0) ? 1 : 2;   // vectors that arrive by bulk copy
+    // tile-sized vector regions of a stage: the gathered vector (+ halo), and the second vector unless it goes
+    // through registers
+    static constexpr int NVEC = (MODE == MODE_PLAIN || SpmmCfg<K, MODE>::REGB) ? 1 : 2;   // (MGR0 as non-REGB would keep 2)
+    static constexpr int NLOAD = (MODE == MODE_PLAIN || MODE == MODE_MGR0 || SpmmCfg<K, MODE>::REGB) ? 1 : 2;   // vectors that arrive by bulk copy
     static constexpr size_t vec_bytes = (size_t)T * K * sizeof(double);
     static constexpr size_t off_b = (size_t)(T + HALO_CAP) * K * sizeof(double);
     static constexpr size_t off_val = off_b + (NVEC - 1) * vec_bytes;
@@ -330,9 +338,9 @@ template <int K, int MODE> struct TileSmem {
     static constexpr size_t off_dg = off_col + (size_t)T * WCAP * sizeof(int32_t);   // S_vv of the tile's rows
     static constexpr size_t off_ar = off_dg + (size_t)T * sizeof(double);            // A_v or 1/A_v
     static constexpr size_t stage_bytes = off_ar + (size_t)T * sizeof(double);
-    static constexpr size_t off_desc = SpmmCfg<K>::STAGES * stage_bytes;
+    static constexpr size_t off_desc = SpmmCfg<K, MODE>::STAGES * stage_bytes;
     static constexpr size_t off_bar = off_desc + 4 * 16 * sizeof(int32_t);
-    static constexpr size_t bytes = off_bar + 8 * SpmmCfg<K>::STAGES + 8;
+    static constexpr size_t bytes = off_bar + 8 * SpmmCfg<K, MODE>::STAGES + 8;
 };
 
 // What one thread needs to issue the bulk copies of a tile (kept in registers by the issuing thread).
@@ -352,12 +360,13 @@ __device__ __forceinline__ TileIssue load_issue(const int32_t* __restrict__ desc
 //   descriptors and halo row ids are fetched two tiles ahead.
 // About 130 KB of loads per SM are outstanding at all times, which is what the loaded HBM latency of B200 needs.
 template <int K, int MODE>
-__global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
+__global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
                                                         double* __restrict__ partials, SpmmArgs a_in) {
     using SM = TileSmem<K, MODE>;
     constexpr int T = SM::T;
-    constexpr int NT = SpmmCfg<K>::NT;
-    constexpr int NS = SpmmCfg<K>::STAGES;               // pipeline stages
+    constexpr int NT = SpmmCfg<K, MODE>::NT;
+    constexpr int NS = SpmmCfg<K, MODE>::STAGES;         // pipeline stages
+    constexpr bool REGB = SpmmCfg<K, MODE>::REGB;        // second vector through registers (bq / bcur below)
     constexpr int LA = NS - 1;                           // tiles the bulk copies run ahead of the gather
     constexpr int TPR = K / 2;
     constexpr int ROWS = NT / TPR;
@@ -498,13 +507,28 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             }
         }
     };
-    // MGR: r' = r - alpha q over the q tile, e = omega r'/d over the r tile
-    auto elementwise_mgr = [&](unsigned char* st, int64_t tile) {
+    // second vector of the REGB modes, own rows only, through registers: element e = tid + i NT of the tile is row
+    // rg + i ROWS, column pair l -- the rows this thread handles in the gather loop
+    constexpr int BPT = REGB ? XPT : 1;
+    auto load_b = [&](int64_t tile, double2 (&bv)[BPT]) {
+        if (!REGB || tile >= ntiles || a.in1 == nullptr) return;
+        const int64_t row0 = tile * T;
+        const int nrows = (int)min((int64_t)T, m.nv - row0);
+#pragma unroll
+        for (int i = 0; i < BPT; ++i) {
+            const int e = tid + i * NT;
+            if (e < nrows * TPR) bv[i] = ld2(a.in1, row0 * K + 2 * (int64_t)e);
+        }
+    };
+    // MGR: r' = r - alpha q (q in registers, r' stored from registers and kept for the tile's epilogue),
+    // e = omega r'/d over the r tile
+    auto elementwise_mgr = [&](unsigned char* st, int64_t tile, double2 (&bv)[BPT]) {
         double2* sa = reinterpret_cast<double2*>(st);
-        double2* sb = reinterpret_cast<double2*>(st + SM::off_b);
+        double2* sb = reinterpret_cast<double2*>(st + SM::off_b);      // (not REGB: q arrives here, r' leaves from here)
         const double* sdg = reinterpret_cast<const double*>(st + SM::off_dg);
         const double* sar = reinterpret_cast<const double*>(st + SM::off_ar);
-        const int nrows = (int)min((int64_t)T, m.nv - tile * T);
+        const int64_t row0 = tile * T;
+        const int nrows = (int)min((int64_t)T, m.nv - row0);
 #pragma unroll
         for (int i = 0; i < XPT; ++i) {
             const int e = tid + i * NT;
@@ -514,11 +538,12 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 const double sd = sdg[rr], av = sar[rr];
                 double2 rn = rv;
                 if (MGQ) {
-                    const double2 qv = sb[e];
+                    const double2 qv = REGB ? bv[REGB ? i : 0] : sb[e];
                     rn.x = fma(-alpha.x, qv.x, rv.x);
                     rn.y = fma(-alpha.y, qv.y, rv.y);
+                    if (REGB) st2(a.x, row0 * K + 2 * (int64_t)e, rn);
                 }
-                sb[e] = rn;
+                if (REGB) bv[REGB ? i : 0] = rn; else sb[e] = rn;
                 sa[e] = make_double2(a.omega * rn.x * rcp_pos(fma(cc.x, sd, av)), a.omega * rn.y * rcp_pos(fma(cc.y, sd, av)));
             }
         }
@@ -545,11 +570,13 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
     }
     int hid_n[HPT];
     double2 h0[HPT], h1[HPT], xv[XPT];
+    double2 bq[BPT], bcur[BPT];   // REGB: second vector of the next tile in flight / of the current tile
     int dnext = 0;
     if (tile0 < ntiles) {
         load_hidx(tile0, hid_n);
         if (is_staged(sdesc)) load_halo(hid_n, sdesc[3], h0, h1);
         if (CG_A) load_x(tile0, xv);
+        if (REGB && !(MODE == MODE_MGR0)) load_b(tile0, bq);
         if (is_staged(sdesc)) halo_to_smem(smem, sdesc[3], h0, h1);
         load_hidx(tile0 + G, hid_n);
         if (tile0 + G < ntiles && is_staged(sdesc + 16)) load_halo(hid_n, sdesc[16 + 3], h0, h1);
@@ -562,8 +589,13 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             fence_proxy_async();
         }
         if (MGR) {
-            elementwise_mgr(smem, tile0);
+            elementwise_mgr(smem, tile0, bq);
             fence_proxy_async();
+        }
+        if (REGB) {
+#pragma unroll
+            for (int i = 0; i < BPT; ++i) bcur[i] = bq[i];
+            if (!(MODE == MODE_MGR0)) load_b(tile0 + G, bq);
         }
     }
     double2 acc[MODE == MODE_AX ? 2 : 1] = {};
@@ -592,7 +624,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             if (CG_A || MGR) {
                 // (MGR with out1 == nullptr: e is not stored, the prolongation kernel forms it again from r')
                 if (!MGR || a.out1) bulk_store(a.out1 + row0 * K, sa, (uint32_t)nrows * K * sizeof(double));
-                if (MGQ) bulk_store(a.x + row0 * K, sb, (uint32_t)nrows * K * sizeof(double));
+                if (MGQ && !REGB) bulk_store(a.x + row0 * K, sb, (uint32_t)nrows * K * sizeof(double));
                 bulk_commit();
             }
             if (t2 + G < ntiles) tq = load_issue(m.tile_desc, t2 + G);
@@ -602,7 +634,11 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
             dnext = tile + 4 * G < ntiles ? m.tile_desc[(tile + 4 * G) * 16 + tid] : 0;
         }
 
-        for (int r = rg; r < nrows; r += ROWS) {
+        constexpr int RPT = T / ROWS;                     // rows of a tile per thread (= BPT in the REGB modes)
+#pragma unroll(REGB ? RPT : 1)
+        for (int i = 0; i < RPT; ++i) {
+            const int r = rg + i * ROWS;
+            if (r >= nrows) break;
             const int64_t row = row0 + r;
             const int chl = r >> m.log2c;
             const int cpr = scp[chl];
@@ -693,7 +729,7 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 const double av = sar[r];
                 double2 o = {fma(cc.x, s.x, av * own.x), fma(cc.y, s.y, av * own.y)};   // A v
                 if (sub >= 1) {
-                    const double2 rv = sb[r * TPR + l];
+                    const double2 rv = REGB ? bcur[REGB ? i : 0] : sb[r * TPR + l];
                     o.x = rv.x - o.x; o.y = rv.y - o.y;                                  // r - A v
                     if (MGR && a.omega2 != 0.0) {      // second sweep: e2 = e1 + omega2 (r' - K e1)/d
                         o.x = fma(a.omega2 * o.x, rcp_pos(fma(cc.x, sd, av)), own.x);
@@ -743,8 +779,13 @@ __global__ void __launch_bounds__(SpmmCfg<K>::NT, SpmmCfg<K>::MINB) k_spmm(MeshV
                 fence_proxy_async();
             }
             if (MGR) {
-                elementwise_mgr(st1, tile + G);
+                elementwise_mgr(st1, tile + G, bq);
                 fence_proxy_async();
+            }
+            if (REGB) {
+#pragma unroll
+                for (int i = 0; i < BPT; ++i) bcur[i] = bq[i];
+                if (!(MODE == MODE_MGR0)) load_b(tile + 2 * G, bq);
             }
         }
     }

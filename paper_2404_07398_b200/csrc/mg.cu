@@ -29,12 +29,16 @@ namespace {
 constexpr int MG_POWER_ITERS = 24;     // power iteration for rho(D_S^-1 S)
 constexpr double MG_RHO_SAFETY = 1.05;  // the iteration approaches rho from below
 
+// Scratch and result buffers of the build come from the device's stream-ordered pool (cudaMallocAsync on the build's
+// stream): the build makes some forty allocations per level, and with cudaMalloc / cudaFree their fixed cost (a
+// millisecond each, with a device synchronisation) was most of the build time on the small levels.  mg_build keeps
+// the pool from returning memory to the driver while it runs and trims it at the end.
 struct DBuf {
     void* p = nullptr;
-    ~DBuf() { if (p) cudaFree(p); }
+    ~DBuf() { if (p) cudaFreeAsync(p, 0); }
     cudaError_t alloc(size_t bytes) {
-        if (p) { cudaFree(p); p = nullptr; }
-        return cudaMalloc(&p, bytes ? bytes : 1);
+        if (p) { cudaFreeAsync(p, 0); p = nullptr; }
+        return cudaMallocAsync(&p, bytes ? bytes : 1, 0);
     }
     template <class T> T* as() const { return static_cast<T*>(p); }
     void* release() { void* q = p; p = nullptr; return q; }
@@ -326,78 +330,158 @@ __global__ void k_mg_strong(const int64_t* __restrict__ rowptr, const int32_t* _
     }
 }
 
-// Greedy aggregation over the graph of the level's matrix, serial in row order (host).  agg[i] = aggregate of row
-// i, numbered in the order of their roots, so the coarse numbering follows the fine one along the curve.
+// Aggregation over the graph of the level's matrix, on the device.  Roots = a maximal set of rows that are pairwise
+// more than two strong connections apart (a distance-2 maximal independent set): every root takes its strong
+// neighbours, and what is left -- rows two connections away from the nearest root -- joins the aggregate of its first
+// aggregated neighbour.  That is what a serial greedy sweep builds too (a row whose neighbours are all free becomes
+// a root and takes them; round 1 ran that sweep on the host, 0.2-0.4 s per level for 7.3 M rows); here the roots are
+// found in parallel rounds with hashed priorities (Luby's scheme over two-ring maxima: an undecided row whose key is
+// the largest within distance two becomes a root, a row that sees a root within distance two is out), a dozen
+// rounds of two passes over the graph.  Aggregates are numbered in the order of their roots, so the coarse
+// numbering follows the fine one along the curve.
 // The graph is that of the strong connections (MG_THETA): weak ones -- across a sliver, or the small entries the
 // Galerkin products accumulate on the coarse levels -- do not pull a row into an aggregate.  Should the filtered
 // graph coarsen by less than MG_MIN_COARSENING (the prolongator is smoothed with the whole matrix, so small
 // aggregates mean fill-in on the next level), the level falls back to the whole graph.
+// key of a row: state (2 = root, 1 = undecided, 0 = out) << 61 | 30 hashed bits << 31 | row id
+__device__ __forceinline__ u64 agg_key(int state, int64_t i) {
+    if (state == 0) return 0ull;
+    u64 z = (u64)i * 0x9E3779B97F4A7C15ull + 0x7F4A7C159E3779B9ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    return ((u64)state << 61) | ((z & 0x3fffffffull) << 31) | (u64)i;
+}
+__global__ void k_agg_init(int64_t n, u64* __restrict__ key) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) key[i] = agg_key(1, i);
+}
+// out[i] = max of in over the row itself and its strong neighbours
+__global__ void k_agg_max(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                          const uint8_t* __restrict__ keep, int64_t n, const u64* __restrict__ in, u64* __restrict__ out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u64 m = in[i];
+    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k)
+        if (keep[k]) { const u64 v = in[col[k]]; m = v > m ? v : m; }
+    out[i] = m;
+}
+// t2 = two-ring maximum of the keys: decide the undecided rows
+__global__ void k_agg_decide(int64_t n, const u64* __restrict__ t2, u64* __restrict__ key, int* __restrict__ undecided) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u64 k = key[i];
+    if ((k >> 61) != 1ull) return;
+    const u64 m = t2[i];
+    if (m == k) key[i] = agg_key(2, i);
+    else if ((m >> 61) == 2ull) key[i] = 0ull;
+    else atomicAdd(undecided, 1);
+}
+__global__ void k_agg_root_flag(int64_t n, const u64* __restrict__ key, int64_t* __restrict__ flag) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i <= n) flag[i] = (i < n && (key[i] >> 61) == 2ull) ? 1 : 0;
+}
+// pass 1: a root and its strong neighbours (a row has at most one root among them)
+__global__ void k_agg_assign1(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                              const uint8_t* __restrict__ keep, int64_t n, const u64* __restrict__ key,
+                              const int64_t* __restrict__ root_id, int32_t* __restrict__ agg) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int32_t a = -1;
+    if ((key[i] >> 61) == 2ull) a = (int32_t)root_id[i];
+    else
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k)
+            if (keep[k] && (key[col[k]] >> 61) == 2ull) { a = (int32_t)root_id[col[k]]; break; }
+    agg[i] = a;
+}
+// pass 2: a leftover joins the aggregate (as of pass 1) of its first aggregated neighbour; leftover[i] = 1 if none
+__global__ void k_agg_assign2(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                              const uint8_t* __restrict__ keep, int64_t n, const int32_t* __restrict__ agg1,
+                              int32_t* __restrict__ agg, int64_t* __restrict__ leftover) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    if (i == n) { leftover[i] = 0; return; }
+    int32_t a = agg1[i];
+    if (a < 0)
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k)
+            if (keep[k] && agg1[col[k]] >= 0) { a = agg1[col[k]]; break; }
+    agg[i] = a;
+    leftover[i] = a < 0 ? 1 : 0;
+}
+// pass 3: what is still free becomes its own aggregate, numbered after the others
+__global__ void k_agg_assign3(int64_t n, const int64_t* __restrict__ left_id, int64_t n_roots, int32_t* __restrict__ agg) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && agg[i] < 0) agg[i] = (int32_t)(n_roots + left_id[i]);
+}
+__global__ void k_fill_u8(int64_t n, uint8_t v, uint8_t* __restrict__ p) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
+int exclusive_scan(int64_t* d_in, int64_t* d_out, int64_t n, int64_t* total, cudaStream_t st);
+
+int aggregate_graph(const MgLevel& f, const uint8_t* keep, DBuf& d_agg, int64_t* n_agg, cudaStream_t st) {
+    const int64_t n = f.n;
+    DBuf key, t1, t2, cnt, flag, ids, agg1, left, left_id;
+    IF_CUDA_TRY(key.alloc((size_t)n * 8));
+    IF_CUDA_TRY(t1.alloc((size_t)n * 8));
+    IF_CUDA_TRY(t2.alloc((size_t)n * 8));
+    IF_CUDA_TRY(cnt.alloc(sizeof(int)));
+    k_agg_init<<<gridf(n), 256, 0, st>>>(n, key.as<u64>());
+    IF_LAUNCH_CHECK();
+    for (int round = 0; round < 200; ++round) {
+        IF_CUDA_TRY(cudaMemsetAsync(cnt.p, 0, sizeof(int), st));
+        k_agg_max<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, keep, n, key.as<u64>(), t1.as<u64>());
+        IF_LAUNCH_CHECK();
+        k_agg_max<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, keep, n, t1.as<u64>(), t2.as<u64>());
+        IF_LAUNCH_CHECK();
+        k_agg_decide<<<gridf(n), 256, 0, st>>>(n, t2.as<u64>(), key.as<u64>(), cnt.as<int>());
+        IF_LAUNCH_CHECK();
+        int undecided = 0;
+        IF_CUDA_TRY(cudaMemcpyAsync(&undecided, cnt.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        if (undecided == 0) break;
+    }
+    IF_CUDA_TRY(flag.alloc((size_t)(n + 1) * 8));
+    IF_CUDA_TRY(ids.alloc((size_t)(n + 1) * 8));
+    k_agg_root_flag<<<gridf(n + 1), 256, 0, st>>>(n, key.as<u64>(), flag.as<int64_t>());
+    IF_LAUNCH_CHECK();
+    int64_t n_roots = 0;
+    int rc = exclusive_scan(flag.as<int64_t>(), ids.as<int64_t>(), n + 1, &n_roots, st);
+    if (rc) return rc;
+    IF_CUDA_TRY(agg1.alloc((size_t)n * 4));
+    IF_CUDA_TRY(d_agg.alloc((size_t)n * 4));
+    IF_CUDA_TRY(left.alloc((size_t)(n + 1) * 8));
+    IF_CUDA_TRY(left_id.alloc((size_t)(n + 1) * 8));
+    k_agg_assign1<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, keep, n, key.as<u64>(), ids.as<int64_t>(), agg1.as<int32_t>());
+    IF_LAUNCH_CHECK();
+    k_agg_assign2<<<gridf(n + 1), 256, 0, st>>>(f.rowptr, f.col, keep, n, agg1.as<int32_t>(), d_agg.as<int32_t>(),
+                                                left.as<int64_t>());
+    IF_LAUNCH_CHECK();
+    int64_t n_left = 0;
+    if ((rc = exclusive_scan(left.as<int64_t>(), left_id.as<int64_t>(), n + 1, &n_left, st))) return rc;
+    if (n_left > 0) {
+        k_agg_assign3<<<gridf(n), 256, 0, st>>>(n, left_id.as<int64_t>(), n_roots, d_agg.as<int32_t>());
+        IF_LAUNCH_CHECK();
+    }
+    *n_agg = n_roots + n_left;
+    return IF_OK;
+}
+
 int aggregate_rows(const MgLevel& f, DBuf& d_agg, int64_t* n_agg, cudaStream_t st) {
     const int64_t n = f.n;
-    std::vector<int64_t> rp, rps;
-    std::vector<int32_t> cj, cjs, agg;
-    std::vector<uint8_t> keep;
-    try {
-        rp.resize((size_t)n + 1);
-        cj.resize((size_t)f.nnz);
-        if (MG_THETA > 0.0) { keep.resize((size_t)f.nnz); rps.resize((size_t)n + 1); cjs.reserve((size_t)f.nnz); }
-    } catch (const std::bad_alloc&) { return IF_ENOMEM; }
-    IF_CUDA_TRY(cudaMemcpyAsync(rp.data(), f.rowptr, (size_t)(n + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-    IF_CUDA_TRY(cudaMemcpyAsync(cj.data(), f.col, (size_t)f.nnz * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    DBuf d_keep;
+    IF_CUDA_TRY(d_keep.alloc((size_t)f.nnz));
+    int rc;
     if (MG_THETA > 0.0) {
-        DBuf d_keep;
-        IF_CUDA_TRY(d_keep.alloc((size_t)f.nnz));
         k_mg_strong<<<gridf(n), 256, 0, st>>>(f.rowptr, f.col, f.sm, f.diag, MG_THETA * MG_THETA, n, d_keep.as<uint8_t>());
         IF_LAUNCH_CHECK();
-        IF_CUDA_TRY(cudaMemcpyAsync(keep.data(), d_keep.p, (size_t)f.nnz, cudaMemcpyDeviceToHost, st));
-        IF_CUDA_TRY(cudaStreamSynchronize(st));
-        for (int64_t i = 0; i < n; ++i) {
-            rps[(size_t)i] = (int64_t)cjs.size();
-            for (int64_t k = rp[i]; k < rp[i + 1]; ++k)
-                if (keep[(size_t)k]) cjs.push_back(cj[(size_t)k]);
-        }
-        rps[(size_t)n] = (int64_t)cjs.size();
+        if ((rc = aggregate_graph(f, d_keep.as<uint8_t>(), d_agg, n_agg, st))) return rc;
+        if ((double)*n_agg * MG_MIN_COARSENING <= (double)n) return IF_OK;
     }
-    IF_CUDA_TRY(cudaStreamSynchronize(st));
-    auto greedy = [&](const std::vector<int64_t>& rp, const std::vector<int32_t>& cj) -> int32_t {
-        agg.assign((size_t)n, -1);
-        int32_t na = 0;
-        // pass 1: roots
-        for (int64_t i = 0; i < n; ++i) {
-            if (agg[i] >= 0) continue;
-            bool all_free = true;
-            for (int64_t k = rp[i]; k < rp[i + 1] && all_free; ++k) all_free = agg[cj[k]] < 0;
-            if (!all_free) continue;
-            for (int64_t k = rp[i]; k < rp[i + 1]; ++k) agg[cj[k]] = na;
-            agg[i] = na++;
-        }
-        // pass 2: a leftover joins the aggregate (as of pass 1) of its first aggregated neighbour; joined rows are
-        // marked -2 - a until the end of the pass so that leftovers do not chain onto each other
-        for (int64_t i = 0; i < n; ++i) {
-            if (agg[i] != -1) continue;
-            for (int64_t k = rp[i]; k < rp[i + 1]; ++k)
-                if (agg[cj[k]] >= 0) { agg[i] = -2 - agg[cj[k]]; break; }
-        }
-        // pass 3: what is still free (possible only in a component without a root) becomes its own aggregate
-        for (int64_t i = 0; i < n; ++i) {
-            if (agg[i] <= -2) agg[i] = -2 - agg[i];
-            else if (agg[i] == -1) agg[i] = na++;
-        }
-        return na;
-    };
-    int32_t na = -1;
-    try {
-        if (MG_THETA > 0.0) {
-            na = greedy(rps, cjs);
-            if ((double)na * MG_MIN_COARSENING > (double)n) na = -1;
-        }
-        if (na < 0) na = greedy(rp, cj);
-    } catch (const std::bad_alloc&) { return IF_ENOMEM; }
-    IF_CUDA_TRY(d_agg.alloc((size_t)n * sizeof(int32_t)));
-    IF_CUDA_TRY(cudaMemcpyAsync(d_agg.p, agg.data(), (size_t)n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-    IF_CUDA_TRY(cudaStreamSynchronize(st));
-    *n_agg = na;
-    return IF_OK;
+    k_fill_u8<<<gridf(f.nnz), 256, 0, st>>>(f.nnz, 1, d_keep.as<uint8_t>());
+    IF_LAUNCH_CHECK();
+    return aggregate_graph(f, d_keep.as<uint8_t>(), d_agg, n_agg, st);
 }
 
 // transfer operators and the Galerkin pair of level `f` -> fills f.p_*, f.r_* and the matrix of level c
@@ -406,7 +490,18 @@ int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
     int rc;
     DBuf agg;
     int64_t nc = 0;
+    const bool verbose = getenv("IF_VERBOSE") != nullptr;
+    auto t_prev = std::chrono::steady_clock::now();
+    auto lap = [&](const char* what) {
+        if (!verbose) return;
+        cudaStreamSynchronize(st);
+        const auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "[implicit_filter]   %lld rows: %s %.1f ms\n", (long long)n, what,
+                1e3 * std::chrono::duration<double>(t - t_prev).count());
+        t_prev = t;
+    };
     if ((rc = aggregate_rows(f, agg, &nc, st))) return rc;
+    lap("aggregates");
     const double omega_p = 4.0 / (3.0 * f.rho);
     // ---- P
     {
@@ -427,6 +522,7 @@ int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
         f.n_coarse = nc; f.p_nnz = pn;
         f.p_rowptr = (int64_t*)prow.release(); f.p_col = (int32_t*)pcol.release(); f.p_val = (double*)pval.release();
     }
+    lap("P");
     // ---- R = P^T
     {
         DBuf keys, vals, k1, v1, tmp;
@@ -447,6 +543,7 @@ int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
         IF_CUDA_TRY(cudaStreamSynchronize(st));
         f.r_rowptr = (int64_t*)rrow.release(); f.r_col = (int32_t*)rcol.release(); f.r_val = (double*)v1.release();
     }
+    lap("R");
     // ---- T = G P
     DBuf trow, tcol, tsm;
     int64_t tn = 0;
@@ -470,6 +567,7 @@ int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
         IF_CUDA_TRY(cudaMemcpyAsync(tsm.p, uv.p, (size_t)tn * sizeof(double2), cudaMemcpyDeviceToDevice, st));
         IF_CUDA_TRY(cudaStreamSynchronize(st));
     }
+    lap("T = G P");
     // ---- G_c = P^T T
     {
         DBuf cnt, off;
@@ -500,6 +598,7 @@ int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
         c.rowptr = (int64_t*)crow.release(); c.col = (int32_t*)ccol.release();
         c.sm = (double2*)csm.release(); c.diag = (double2*)cdiag.release();
     }
+    lap("P^T T");
     return IF_OK;
 }
 
@@ -516,9 +615,26 @@ void mg_free(if_mesh_s* h) {
     h->mg_levels = 0;
 }
 
+struct PoolHold {     // keep freed blocks in the pool for the duration of the build
+    cudaMemPool_t pool = nullptr;
+    PoolHold(int device) {
+        if (cudaDeviceGetDefaultMemPool(&pool, device) != cudaSuccess) { pool = nullptr; cudaGetLastError(); return; }
+        uint64_t keep = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    ~PoolHold() {
+        if (!pool) return;
+        uint64_t keep = 0;
+        cudaStreamSynchronize(0);
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        cudaMemPoolTrimTo(pool, 0);
+    }
+};
+
 int mg_build(if_mesh_s* h) {
     const auto t_start = std::chrono::steady_clock::now();
     cudaStream_t st = 0;
+    PoolHold hold(h->device);
     const int64_t nv = h->n_vert;
     int log2c = 0;
     while ((1 << log2c) < h->sell_c) ++log2c;

@@ -305,10 +305,10 @@ int mg_setup(Run& r) {
     const if_mesh_s* h = r.h;
     const int64_t tiles = (h->n_vert + TILE_ROWS - 1) / TILE_ROWS;
     int rc;
-    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK>::NT))) return rc;
-    if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;
     if (r.order_n == 2 &&
-        (rc = resident_grid(k_spmm<MGK, MODE_MGR0>, TileSmem<MGK, MODE_MGR0>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<MGK>::NT))) return rc;
+        (rc = resident_grid(k_spmm<MGK, MODE_MGR0>, TileSmem<MGK, MODE_MGR0>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<MGK, MODE_MGR0>::NT))) return rc;
     return IF_OK;
 }
 

@@ -101,13 +101,13 @@ int setup_grids(Run& r) {
     const int64_t tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
     const int64_t passes = (nv + BLOCK / (K / 2) - 1) / (BLOCK / (K / 2));
     int rc;
-    if ((rc = resident_grid(k_spmm<K, MODE_PLAIN>, TileSmem<K, MODE_PLAIN>::bytes, n_sm, tiles, &r.g.plain, SpmmCfg<K>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_PLAIN>, TileSmem<K, MODE_PLAIN>::bytes, n_sm, tiles, &r.g.plain, SpmmCfg<K, MODE_PLAIN>::NT))) return rc;
     if (r.order_n == 1) {
-        if ((rc = resident_grid(k_spmm<K, MODE_CG1>, TileSmem<K, MODE_CG1>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K>::NT))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_CG1>, TileSmem<K, MODE_CG1>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K, MODE_CG1>::NT))) return rc;
     } else {
-        if ((rc = resident_grid(k_spmm<K, MODE_CG2A>, TileSmem<K, MODE_CG2A>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K>::NT))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_CG2A>, TileSmem<K, MODE_CG2A>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K, MODE_CG2A>::NT))) return rc;
     }
-    if ((rc = resident_grid(k_spmm<K, MODE_CG2B>, TileSmem<K, MODE_CG2B>::bytes, n_sm, tiles, &r.g.cgb, SpmmCfg<K>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_CG2B>, TileSmem<K, MODE_CG2B>::bytes, n_sm, tiles, &r.g.cgb, SpmmCfg<K, MODE_CG2B>::NT))) return rc;
     if ((rc = resident_grid(k_update<K>, 0, n_sm, passes, &r.g.update))) return rc;
     r.g.stream = (int)std::max<int64_t>(1, std::min<int64_t>(passes, (int64_t)n_sm * 4));
     return IF_OK;
@@ -115,7 +115,7 @@ int setup_grids(Run& r) {
 
 template <int K, int MODE>
 int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
-    k_spmm<K, MODE><<<grid, SpmmCfg<K>::NT, TileSmem<K, MODE>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
+    k_spmm<K, MODE><<<grid, SpmmCfg<K, MODE>::NT, TileSmem<K, MODE>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
     IF_LAUNCH_CHECK();
     return IF_OK;
 }
