@@ -178,9 +178,10 @@ int if_mesh_export_csr(if_handle h, int64_t* rowptr, int32_t* col, double* val, 
 int if_mesh_export_perm(if_handle h, int32_t* perm);
 
 /* The prepared mesh is independent of the scales and can be kept on disk and reused.
- * if_save writes every device array of the handle to `path` (HOST string); if_load rebuilds a handle on the current
- * CUDA device from such a file (same library build: the row-tile constants are checked).  The optional CSR copy of
- * IF_FLAG_KEEP_CSR is not saved.  IF_EIO on any file problem. */
+ * if_save writes every device array of the handle -- the multigrid hierarchy of IF_FLAG_MULTIGRID included -- to `path`
+ * (HOST string); if_load rebuilds a handle on the current CUDA device from such a file (same library build: the
+ * row-tile constants and the size of every array are checked against the header and the file's length).  The optional
+ * CSR copy of IF_FLAG_KEEP_CSR is not saved.  IF_EIO on any file problem. */
 int if_save(if_handle h, const char* path);
 int if_load(const char* path, if_handle* out);
 

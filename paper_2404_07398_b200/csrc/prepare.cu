@@ -786,6 +786,11 @@ struct FileHeader {
     ifl::Options opt;
 };
 
+struct LevelHeader {          // one multigrid level in the file
+    int64_t n, nnz, n_coarse, p_nnz;
+    double rho, rho_m, omega;
+};
+
 int write_dev(FILE* f, const void* d, size_t bytes, std::vector<char>& buf) {
     buf.resize(bytes);
     if (bytes) IF_CUDA_TRY(cudaMemcpy(buf.data(), d, bytes, cudaMemcpyDeviceToHost));
@@ -834,6 +839,29 @@ extern "C" int if_save(if_handle h, const char* path) {
     if (rc == IF_OK) rc = write_dev(f, h->halo_n, nt * 4, buf);
     if (rc == IF_OK) rc = write_dev(f, h->halo_rows, nt * HALO_CAP * 4, buf);
     if (rc == IF_OK) rc = write_dev(f, h->tile_desc, (nt + 1) * 64, buf);
+    // the multigrid hierarchy (IF_FLAG_MULTIGRID): level count, then per level its header, the (S, M) pair and the
+    // transfer operators to the next level
+    if (rc == IF_OK && (h->opt.flags & IF_FLAG_MULTIGRID)) {
+        const int64_t L = h->mg_levels;
+        rc = fwrite(&L, sizeof(L), 1, f) == 1 ? IF_OK : IF_EIO;
+        for (int l = 0; l < h->mg_levels && rc == IF_OK; ++l) {
+            const ifl::MgLevel& g = h->mg[l];
+            LevelHeader lh{g.n, g.nnz, g.n_coarse, g.p_nnz, g.rho, g.rho_m, g.omega};
+            rc = fwrite(&lh, sizeof(lh), 1, f) == 1 ? IF_OK : IF_EIO;
+            if (rc == IF_OK) rc = write_dev(f, g.rowptr, (size_t)(g.n + 1) * 8, buf);
+            if (rc == IF_OK) rc = write_dev(f, g.col, (size_t)g.nnz * 4, buf);
+            if (rc == IF_OK) rc = write_dev(f, g.sm, (size_t)g.nnz * 16, buf);
+            if (rc == IF_OK) rc = write_dev(f, g.diag, (size_t)g.n * 16, buf);
+            if (l + 1 < h->mg_levels) {
+                if (rc == IF_OK) rc = write_dev(f, g.p_rowptr, (size_t)(g.n + 1) * 8, buf);
+                if (rc == IF_OK) rc = write_dev(f, g.p_col, (size_t)g.p_nnz * 4, buf);
+                if (rc == IF_OK) rc = write_dev(f, g.p_val, (size_t)g.p_nnz * 8, buf);
+                if (rc == IF_OK) rc = write_dev(f, g.r_rowptr, (size_t)(g.n_coarse + 1) * 8, buf);
+                if (rc == IF_OK) rc = write_dev(f, g.r_col, (size_t)g.p_nnz * 4, buf);
+                if (rc == IF_OK) rc = write_dev(f, g.r_val, (size_t)g.p_nnz * 8, buf);
+            }
+        }
+    }
     if (fclose(f) != 0 && rc == IF_OK) rc = IF_EIO;
     return rc;
 }
@@ -869,7 +897,9 @@ extern "C" int if_load(const char* path, if_handle* out) {
             const int64_t nv = hd.n_vert, ns = hd.sell_slots, nt = hd.n_tiles;
             const int64_t expect = (int64_t)sizeof(hd) + (hd.n_chunks + 1) * 8 + ns * 16 + nv * (6 * 8 + 2 * 4) + nt * 4 +
                                    nt * HALO_CAP * 4 + (nt + 1) * 64;
-            ok = fseek(f, 0, SEEK_END) == 0 && (int64_t)ftell(f) == expect && fseek(f, (long)sizeof(hd), SEEK_SET) == 0;
+            const bool with_mg = (hd.opt.flags & IF_FLAG_MULTIGRID) != 0;      // the hierarchy follows the mesh arrays
+            ok = fseek(f, 0, SEEK_END) == 0 && (with_mg ? (int64_t)ftell(f) > expect : (int64_t)ftell(f) == expect) &&
+                 fseek(f, (long)sizeof(hd), SEEK_SET) == 0;
         }
         if (!ok) { fclose(f); return IF_EIO; }
     }
@@ -906,6 +936,32 @@ extern "C" int if_load(const char* path, if_handle* out) {
     if ((rc = read_dev(f, (void**)&h->halo_n, nt * 4, nt * 4, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->halo_rows, nt * HALO_CAP * 4, nt * HALO_CAP * 4, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->tile_desc, (nt + 1) * 64, (nt + 1) * 64, buf))) return fail(rc);
+    if (h->opt.flags & IF_FLAG_MULTIGRID) {
+        int64_t L = 0;
+        if (fread(&L, sizeof(L), 1, f) != 1 || L < 0 || L > ifl::MG_MAX_LEVELS) return fail(IF_EIO);
+        for (int l = 0; l < (int)L; ++l) {
+            ifl::MgLevel& g = h->mg[l];
+            LevelHeader lh;
+            if (fread(&lh, sizeof(lh), 1, f) != 1 || lh.n < 1 || lh.nnz < lh.n || lh.p_nnz < 0 || lh.n_coarse < 0 ||
+                (l == 0 && lh.n != h->n_vert) || (l > 0 && lh.n != h->mg[l - 1].n_coarse) || !(lh.omega > 0.0))
+                return fail(IF_EIO);
+            g.n = lh.n; g.nnz = lh.nnz; g.n_coarse = lh.n_coarse; g.p_nnz = lh.p_nnz;
+            g.rho = lh.rho; g.rho_m = lh.rho_m; g.omega = lh.omega;
+            h->mg_levels = l + 1;      // (if_destroy frees what has been read so far)
+            if ((rc = read_dev(f, (void**)&g.rowptr, (size_t)(g.n + 1) * 8, (size_t)(g.n + 1) * 8, buf))) return fail(rc);
+            if ((rc = read_dev(f, (void**)&g.col, (size_t)g.nnz * 4, (size_t)g.nnz * 4, buf))) return fail(rc);
+            if ((rc = read_dev(f, (void**)&g.sm, (size_t)g.nnz * 16, (size_t)g.nnz * 16, buf))) return fail(rc);
+            if ((rc = read_dev(f, (void**)&g.diag, (size_t)g.n * 16, (size_t)g.n * 16, buf))) return fail(rc);
+            if (l + 1 < (int)L) {
+                if ((rc = read_dev(f, (void**)&g.p_rowptr, (size_t)(g.n + 1) * 8, (size_t)(g.n + 1) * 8, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.p_col, (size_t)g.p_nnz * 4, (size_t)g.p_nnz * 4, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.p_val, (size_t)g.p_nnz * 8, (size_t)g.p_nnz * 8, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.r_rowptr, (size_t)(g.n_coarse + 1) * 8, (size_t)(g.n_coarse + 1) * 8, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.r_col, (size_t)g.p_nnz * 4, (size_t)g.p_nnz * 4, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.r_val, (size_t)g.p_nnz * 8, (size_t)g.p_nnz * 8, buf))) return fail(rc);
+            }
+        }
+    }
     char extra;
     if (fread(&extra, 1, 1, f) != 0) return fail(IF_EIO);   // trailing bytes: not a file of ours
     fclose(f);
@@ -914,10 +970,6 @@ extern "C" int if_load(const char* path, if_handle* out) {
         cudaGetLastError();
         if_destroy(h);
         return IF_ENOMEM;
-    }
-    if (h->opt.flags & IF_FLAG_MULTIGRID) {   // the hierarchy is not stored: rebuild it
-        int rc = mg_build(h);
-        if (rc != IF_OK) { if_destroy(h); return rc; }
     }
     *out = h;
     return IF_OK;

@@ -443,8 +443,9 @@ def test_multigrid_small_scales_through_the_hierarchy(ifl, oracle_mod):
 
 
 def test_multigrid_hierarchy_survives_save_and_load(ifl, tmp_path):
-    """if_save / if_load of a handle prepared with IF_FLAG_MULTIGRID: the loaded handle solves with solver = 1 and
-    gives the same iteration counts and bits (the hierarchy is rebuilt deterministically on load)."""
+    """if_save / if_load of a handle prepared with IF_FLAG_MULTIGRID: the hierarchy is stored with the mesh, the loaded
+    handle solves with solver = 1 (n = 1 and n = 2) and gives the same iteration counts and bits; a truncated or padded
+    file is refused."""
     w = make_config(4, level=5, n_ells=7)
     h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
     a, sa = ifl.if_filter(h, w.fields, w.ells, 1, solver=1, mg_min_ell=2.0)
@@ -454,7 +455,24 @@ def test_multigrid_hierarchy_survives_save_and_load(ifl, tmp_path):
     b, sb = ifl.if_filter(h2, w.fields, w.ells, 1, solver=1, mg_min_ell=2.0)
     assert np.array_equal(sa["iters"], sb["iters"]) and sa["iters"].max() < 60
     assert bool((a == b).all())
+    i1, i2 = ifl.if_mesh_multigrid_info(h), ifl.if_mesh_multigrid_info(h2)
+    assert i1["rows"] == i2["rows"] and i1["nnz"] == i2["nnz"] and i2["levels"] >= 3 and i2["build_seconds"] == 0.0
+    c, sc = ifl.if_filter(h, w.fields, w.ells[:4], 2, solver=1)
+    d, sd = ifl.if_filter(h2, w.fields, w.ells[:4], 2, solver=1)
+    assert sc["mg_batch_iters"] > 0 and np.array_equal(sc["iters"], sd["iters"]) and bool((c == d).all())
     h.close(); h2.close()
+    import os
+    size = os.path.getsize(path)
+    with open(path, "r+b") as fh:
+        fh.truncate(size - 64)
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_load(path)
+    assert e.value.code == -8
+    with open(path, "ab") as fh:
+        fh.write(b"\0" * 128)
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_load(path)
+    assert e.value.code == -8
 
 
 # ------------------------------------------------------------------------------------------ n = 2 at the top of its range
