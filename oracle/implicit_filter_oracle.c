@@ -44,6 +44,9 @@ typedef struct {
     double *area;     /* [nv] A_v */
     double *gdiag;    /* [nv] diag(S M^-1 S)_v = sum_j S_vj^2 / A_j */
     double *sdiag;    /* [nv] S_vv */
+    /* vector filter (orc_build_vector), on the sparsity pattern of S: */
+    double *dval;     /* [nnz] D~_vv'/l^2 = int (grad N_v . grad N_v' + (R_e^-2 + m^2) N_v N_v') dS            */
+    double *tval;     /* [nnz] T_vv'/l^2  = int m (-N_v' dx N_v + N_v dx N_v') dS   (antisymmetric, zero diagonal) */
 } orc_mesh;
 
 static void edge_vec(const double *coords, int dim, const double *period, int64_t from, int64_t to,
@@ -60,6 +63,7 @@ static void edge_vec(const double *coords, int dim, const double *period, int64_
 void orc_free(orc_mesh *m) {
     if (!m) return;
     free(m->rowptr); free(m->col); free(m->val); free(m->area); free(m->gdiag); free(m->sdiag);
+    free(m->dval); free(m->tval);
     free(m);
 }
 
@@ -405,4 +409,167 @@ int orc_threads(void) {
 #else
     return 1;
 #endif
+}
+
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * Vector filter with metric terms (section 2.1.2): the coarse-grained velocity (u, v) = (zonal,
+ * meridional) at the vertices of a mesh on the sphere solves the 2V x 2V system
+ *     S_2 = M_2 + gamma l^2 D_2            (n = 1),      S_2 = M_2 + gamma l^4 D_2 M_2^-1 D_2     (n = 2),
+ *     D_2 = [ D~  T ; -T  D~ ],  M_2 = diag(M, M),  M = diag(A_v)  (lumped, as in the scalar case and as PAPER.md:89
+ *     writes for the biharmonic form),
+ *     D~_vv' = int (grad N_v . grad N_v' + (R_e^-2 + m^2) N_v N_v') dS,
+ *     T_vv'  = int m (-N_v' dx N_v + N_v dx N_v') dS,      m = tan(theta) / R_e "taken constant on triangles".
+ * Readings: the triangles are the flat 3-D triangles of the mesh; theta and the zonal unit
+ * vector are those of the triangle's centroid; dx N = grad N . e_east; int N_v N_v' = area (1 + delta_vv') / 12 and
+ * int N_v = area / 3 (exact P1 integrals).  T is antisymmetric, so D_2 is symmetric; it is the weak form of the
+ * vector Laplacian, positive semidefinite.  A planar mesh (dim = 2) has no metric terms: m = 0 and 1/R_e = 0.
+ * Returns 0, or 4 out of memory. */
+static int64_t find_col(const orc_mesh *m, int64_t row, int64_t c) {
+    for (int64_t i = m->rowptr[row]; i < m->rowptr[row + 1]; ++i)
+        if (m->col[i] == c) return i;
+    return -1;
+}
+
+int orc_build_vector(orc_mesh *m, const double *coords, int dim, const int32_t *tri, int64_t nt, double radius) {
+    free(m->dval); free(m->tval);
+    m->dval = (double *)calloc((size_t)m->nnz, sizeof(double));
+    m->tval = (double *)calloc((size_t)m->nnz, sizeof(double));
+    if (!m->dval || !m->tval) return 4;
+    const double inv_r = (dim == 3 && radius > 0.0) ? 1.0 / radius : 0.0;
+    for (int64_t t = 0; t < nt; ++t) {
+        int64_t v[3] = {tri[3 * t], tri[3 * t + 1], tri[3 * t + 2]};
+        double x[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+        for (int c = 0; c < 3; ++c)
+            for (int d = 0; d < dim; ++d) x[c][d] = coords[v[c] * dim + d];
+        /* unit normal, area, P1 gradients in the triangle's plane: grad N_a = n x (x_c - x_b) / (2 area) */
+        double e1[3], e2[3], nrm[3];
+        for (int d = 0; d < 3; ++d) { e1[d] = x[1][d] - x[0][d]; e2[d] = x[2][d] - x[0][d]; }
+        nrm[0] = e1[1] * e2[2] - e1[2] * e2[1];
+        nrm[1] = e1[2] * e2[0] - e1[0] * e2[2];
+        nrm[2] = e1[0] * e2[1] - e1[1] * e2[0];
+        double cr = sqrt(nrm[0] * nrm[0] + nrm[1] * nrm[1] + nrm[2] * nrm[2]);
+        double area = 0.5 * cr;
+        for (int d = 0; d < 3; ++d) nrm[d] /= cr;
+        double g[3][3];
+        for (int a = 0; a < 3; ++a) {
+            int b = (a + 1) % 3, c = (a + 2) % 3;
+            double ed[3] = {x[c][0] - x[b][0], x[c][1] - x[b][1], x[c][2] - x[b][2]};
+            g[a][0] = (nrm[1] * ed[2] - nrm[2] * ed[1]) / cr;
+            g[a][1] = (nrm[2] * ed[0] - nrm[0] * ed[2]) / cr;
+            g[a][2] = (nrm[0] * ed[1] - nrm[1] * ed[0]) / cr;
+        }
+        /* metric factor and zonal direction at the centroid */
+        double mt = 0.0, east[3] = {1.0, 0.0, 0.0};
+        if (dim == 3 && inv_r > 0.0) {
+            double cx = (x[0][0] + x[1][0] + x[2][0]) / 3.0, cy = (x[0][1] + x[1][1] + x[2][1]) / 3.0;
+            double cz = (x[0][2] + x[1][2] + x[2][2]) / 3.0;
+            double rho = sqrt(cx * cx + cy * cy);
+            mt = (cz / rho) * inv_r;                       /* tan(theta) / R_e */
+            east[0] = -cy / rho; east[1] = cx / rho; east[2] = 0.0;
+        }
+        double gx[3];
+        for (int a = 0; a < 3; ++a) gx[a] = g[a][0] * east[0] + g[a][1] * east[1] + g[a][2] * east[2];
+        const double mass_c = inv_r * inv_r + mt * mt;
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                int64_t i = find_col(m, v[a], v[b]);
+                double gg = g[a][0] * g[b][0] + g[a][1] * g[b][1] + g[a][2] * g[b][2];
+                m->dval[i] += area * gg + mass_c * area * (a == b ? 2.0 : 1.0) / 12.0;
+                m->tval[i] += mt * (area / 3.0) * (gx[b] - gx[a]);     /* row v = v[a], column v' = v[b] */
+            }
+    }
+    return 0;
+}
+
+void orc_get_vector_csr(const orc_mesh *m, double *dval, double *tval) {
+    memcpy(dval, m->dval, (size_t)m->nnz * sizeof(double));
+    memcpy(tval, m->tval, (size_t)m->nnz * sizeof(double));
+}
+
+/* (yu, yv) = D_2 (pu, pv) / l^2 */
+static void apply_D2(const orc_mesh *m, const double *pu, const double *pv, double *yu, double *yv) {
+#pragma omp parallel for schedule(static)
+    for (int64_t v = 0; v < m->nv; ++v) {
+        double su = 0.0, sv = 0.0;
+        for (int64_t i = m->rowptr[v]; i < m->rowptr[v + 1]; ++i) {
+            int64_t j = m->col[i];
+            su += m->dval[i] * pu[j] + m->tval[i] * pv[j];
+            sv += m->dval[i] * pv[j] - m->tval[i] * pu[j];
+        }
+        yu[v] = su; yv[v] = sv;
+    }
+}
+
+/* (outu, outv) = S_2 (pu, pv);  tmp: scratch [4 nv] for n = 2 */
+void orc_apply_vector(const orc_mesh *m, double ell, int n, double gamma, const double *pu, const double *pv,
+                      double *outu, double *outv, double *tmp) {
+    const double c = gamma * pow(ell, 2.0 * n);
+    const int64_t nv = m->nv;
+    if (n == 1) {
+        apply_D2(m, pu, pv, outu, outv);
+    } else {
+        double *tu = tmp, *tv = tmp + nv;
+        apply_D2(m, pu, pv, tu, tv);
+        for (int64_t v = 0; v < nv; ++v) { tu[v] /= m->area[v]; tv[v] /= m->area[v]; }
+        apply_D2(m, tu, tv, outu, outv);
+    }
+    for (int64_t v = 0; v < nv; ++v) {
+        outu[v] = m->area[v] * pu[v] + c * outu[v];
+        outv[v] = m->area[v] * pv[v] + c * outv[v];
+    }
+}
+
+/* Jacobi-preconditioned CG on S_2 (x_u, x_v) = M_2 (u, v) from x0 = (u, v), one residual norm over both
+ * components: ||r||_2 <= tol ||M_2 (u, v)||_2.  Same outputs and return codes as orc_solve. */
+int orc_solve_vector(const orc_mesh *m, const double *u, const double *v, double ell, int n, double gamma, double tol,
+                     int64_t max_iter, double *xu, double *xv, int64_t *iters, double *rec_res, double *true_res) {
+    const int64_t nv = m->nv, N = 2 * m->nv;
+    const double c = gamma * pow(ell, 2.0 * n);
+    double *b = (double *)malloc((size_t)N * sizeof(double)), *r = (double *)malloc((size_t)N * sizeof(double));
+    double *z = (double *)malloc((size_t)N * sizeof(double)), *p = (double *)malloc((size_t)N * sizeof(double));
+    double *q = (double *)malloc((size_t)N * sizeof(double)), *d = (double *)malloc((size_t)N * sizeof(double));
+    double *x = (double *)malloc((size_t)N * sizeof(double)), *tmp = (double *)malloc((size_t)N * sizeof(double));
+    int status = 1;
+    if (!b || !r || !z || !p || !q || !d || !x || !tmp) { status = 4; goto done; }
+    for (int64_t i = 0; i < nv; ++i) {
+        /* diag(S_2): n = 1: A_v + c D~_vv;  n = 2: A_v + c sum_j (D~_vj^2 + T_vj^2) / A_j  (D_2 symmetric, T_vv = 0) */
+        double dg = 0.0;
+        for (int64_t k = m->rowptr[i]; k < m->rowptr[i + 1]; ++k) {
+            if (n == 1) { if (m->col[k] == i) dg = m->dval[k]; }
+            else dg += (m->dval[k] * m->dval[k] + m->tval[k] * m->tval[k]) / m->area[m->col[k]];
+        }
+        d[i] = d[nv + i] = m->area[i] + c * dg;
+        b[i] = m->area[i] * u[i]; b[nv + i] = m->area[i] * v[i];
+        x[i] = u[i]; x[nv + i] = v[i];
+    }
+    orc_apply_vector(m, ell, n, gamma, x, x + nv, q, q + nv, tmp);
+    for (int64_t i = 0; i < N; ++i) { r[i] = b[i] - q[i]; z[i] = r[i] / d[i]; p[i] = z[i]; }
+    double bb = dot(N, b, b), rho = dot(N, r, z), rr = dot(N, r, r);
+    int64_t it = 0;
+    if (rr <= tol * tol * bb) status = 0;
+    while (status == 1 && it < max_iter) {
+        orc_apply_vector(m, ell, n, gamma, p, p + nv, q, q + nv, tmp);
+        double pq = dot(N, p, q);
+        if (!(pq > 0.0) || !isfinite(pq)) { status = 2; break; }
+        double alpha = rho / pq;
+        for (int64_t i = 0; i < N; ++i) { x[i] += alpha * p[i]; r[i] -= alpha * q[i]; z[i] = r[i] / d[i]; }
+        double rho_new = dot(N, r, z);
+        rr = dot(N, r, r);
+        ++it;
+        if (rr <= tol * tol * bb) { status = 0; break; }
+        double beta = rho_new / rho;
+        rho = rho_new;
+        for (int64_t i = 0; i < N; ++i) p[i] = z[i] + beta * p[i];
+    }
+    *iters = it;
+    *rec_res = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+    orc_apply_vector(m, ell, n, gamma, x, x + nv, q, q + nv, tmp);
+    for (int64_t i = 0; i < N; ++i) q[i] = b[i] - q[i];
+    *true_res = bb > 0.0 ? sqrt(dot(N, q, q) / bb) : 0.0;
+    memcpy(xu, x, (size_t)nv * sizeof(double));
+    memcpy(xv, x + nv, (size_t)nv * sizeof(double));
+done:
+    free(b); free(r); free(z); free(p); free(q); free(d); free(x); free(tmp);
+    return status;
 }

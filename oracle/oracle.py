@@ -57,6 +57,13 @@ def _load():
         L.orc_dense_solve.restype = i32
         L.orc_dense_solve.argtypes = [vp, vp, dbl, i32, dbl, vp]
         L.orc_threads.restype = i32
+        L.orc_build_vector.restype = i32
+        L.orc_build_vector.argtypes = [vp, vp, i32, vp, i64, dbl]
+        L.orc_get_vector_csr.argtypes = [vp, vp, vp]
+        L.orc_apply_vector.argtypes = [vp, dbl, i32, dbl, vp, vp, vp, vp, vp]
+        L.orc_solve_vector.restype = i32
+        L.orc_solve_vector.argtypes = [vp, vp, vp, dbl, i32, dbl, dbl, i64, vp, vp, C.POINTER(i64), C.POINTER(dbl),
+                                       C.POINTER(dbl)]
         _lib = L
     return _lib
 
@@ -86,6 +93,8 @@ class OracleMesh:
             raise ValueError("oracle: " + self._ERR.get(err.value, f"error {err.value}"))
         self.nv = int(L.orc_nv(self._h))
         self.nnz = int(L.orc_nnz(self._h))
+        self._coords, self._tri = coords, tri          # kept for build_vector
+        self._vector = False
 
     def __del__(self):
         if getattr(self, "_h", None) and _lib is not None:
@@ -139,6 +148,50 @@ class OracleMesh:
         if st != 0:
             raise RuntimeError(f"oracle dense solve failed ({st})")
         return x
+
+    # ---- vector filter with metric terms
+    def build_vector(self, radius: float = 0.0):
+        """Assemble D~ and T (metric terms) on the pattern of S.  radius 0 => mean |x_v| (3-D meshes)."""
+        if self._coords.shape[1] == 3 and radius == 0.0:
+            radius = float(np.linalg.norm(self._coords, axis=1).mean())
+        st = _load().orc_build_vector(self._h, _p(self._coords), self._coords.shape[1], _p(self._tri),
+                                      self._tri.shape[0], float(radius))
+        if st != 0:
+            raise MemoryError("oracle: out of memory")
+        self._vector = True
+        self.radius = radius
+
+    def vector_csr(self):
+        """(D~/l^2, T/l^2) values on the CSR pattern of csr()."""
+        assert self._vector
+        d = np.empty(self.nnz, dtype=np.float64)
+        t = np.empty(self.nnz, dtype=np.float64)
+        _load().orc_get_vector_csr(self._h, _p(d), _p(t))
+        return d, t
+
+    def apply_vector(self, pu, pv, ell: float, n: int, gamma: float = GAMMA):
+        assert self._vector
+        pu = np.ascontiguousarray(pu, dtype=np.float64)
+        pv = np.ascontiguousarray(pv, dtype=np.float64)
+        ou, ov = np.empty(self.nv), np.empty(self.nv)
+        tmp = np.empty(4 * self.nv)
+        _load().orc_apply_vector(self._h, float(ell), int(n), float(gamma), _p(pu), _p(pv), _p(ou), _p(ov), _p(tmp))
+        return ou, ov
+
+    def solve_vector(self, u, v, ell: float, n: int, gamma: float = GAMMA, tol: float = TOL, max_iter: int = 2_000_000):
+        """Coarse-grained velocity (ubar, vbar) and an info dict."""
+        assert self._vector
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        xu, xv = np.empty(self.nv), np.empty(self.nv)
+        it = C.c_int64(0)
+        rec = C.c_double(0.0)
+        tru = C.c_double(0.0)
+        st = _load().orc_solve_vector(self._h, _p(u), _p(v), float(ell), int(n), float(gamma), float(tol), int(max_iter),
+                                      _p(xu), _p(xv), C.byref(it), C.byref(rec), C.byref(tru))
+        if st == 4:
+            raise MemoryError("oracle: out of memory")
+        return xu, xv, {"status": int(st), "iters": int(it.value), "rec_res": rec.value, "true_res": tru.value}
 
     def energy(self, x: np.ndarray) -> float:
         x = np.ascontiguousarray(x, dtype=np.float64)

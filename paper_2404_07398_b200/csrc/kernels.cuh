@@ -154,6 +154,9 @@ __device__ __forceinline__ void bulk_store(void* dst_gmem, const void* src_smem,
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)),
                  "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
@@ -429,6 +432,7 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
         mbar_expect_tx(bar, vbytes * SM::NLOAD + 2u * dbytes + (staged ? (uint32_t)ti.slots * 12u : 0u));
         bulk_load(st, a.in0 + row0 * K, vbytes, bar);
         if (SM::NLOAD >= 2) bulk_load(st + SM::off_b, a.in1 + row0 * K, vbytes, bar);
+        if (REGB && MODE == MODE_AX && a.in1) bulk_prefetch_l2(a.in1 + row0 * K, vbytes);
         bulk_load(st + SM::off_dg, m.sdiag + row0, dbytes, bar);
         bulk_load(st + SM::off_ar, rowfac + row0, dbytes, bar);
         if (staged) {
@@ -507,28 +511,14 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
             }
         }
     };
-    // second vector of the REGB modes, own rows only, through registers: element e = tid + i NT of the tile is row
-    // rg + i ROWS, column pair l -- the rows this thread handles in the gather loop
-    constexpr int BPT = REGB ? XPT : 1;
-    auto load_b = [&](int64_t tile, double2 (&bv)[BPT]) {
-        if (!REGB || tile >= ntiles || a.in1 == nullptr) return;
-        const int64_t row0 = tile * T;
-        const int nrows = (int)min((int64_t)T, m.nv - row0);
-#pragma unroll
-        for (int i = 0; i < BPT; ++i) {
-            const int e = tid + i * NT;
-            if (e < nrows * TPR) bv[i] = ld2(a.in1, row0 * K + 2 * (int64_t)e);
-        }
-    };
-    // MGR: r' = r - alpha q (q in registers, r' stored from registers and kept for the tile's epilogue),
-    // e = omega r'/d over the r tile
-    auto elementwise_mgr = [&](unsigned char* st, int64_t tile, double2 (&bv)[BPT]) {
+    // MGR: r' = r - alpha q over the q tile, e = omega r'/d over the r tile.  (REGB, i.e. MGR0: there is no q and no
+    // second region; the epilogue reads its own rows of w = r' again from global memory, an L2 hit)
+    auto elementwise_mgr = [&](unsigned char* st, int64_t tile) {
         double2* sa = reinterpret_cast<double2*>(st);
-        double2* sb = reinterpret_cast<double2*>(st + SM::off_b);      // (not REGB: q arrives here, r' leaves from here)
+        double2* sb = reinterpret_cast<double2*>(st + SM::off_b);
         const double* sdg = reinterpret_cast<const double*>(st + SM::off_dg);
         const double* sar = reinterpret_cast<const double*>(st + SM::off_ar);
-        const int64_t row0 = tile * T;
-        const int nrows = (int)min((int64_t)T, m.nv - row0);
+        const int nrows = (int)min((int64_t)T, m.nv - tile * T);
 #pragma unroll
         for (int i = 0; i < XPT; ++i) {
             const int e = tid + i * NT;
@@ -538,12 +528,11 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
                 const double sd = sdg[rr], av = sar[rr];
                 double2 rn = rv;
                 if (MGQ) {
-                    const double2 qv = REGB ? bv[REGB ? i : 0] : sb[e];
+                    const double2 qv = sb[e];
                     rn.x = fma(-alpha.x, qv.x, rv.x);
                     rn.y = fma(-alpha.y, qv.y, rv.y);
-                    if (REGB) st2(a.x, row0 * K + 2 * (int64_t)e, rn);
                 }
-                if (REGB) bv[REGB ? i : 0] = rn; else sb[e] = rn;
+                if (!REGB) sb[e] = rn;
                 sa[e] = make_double2(a.omega * rn.x * rcp_pos(fma(cc.x, sd, av)), a.omega * rn.y * rcp_pos(fma(cc.y, sd, av)));
             }
         }
@@ -570,13 +559,11 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
     }
     int hid_n[HPT];
     double2 h0[HPT], h1[HPT], xv[XPT];
-    double2 bq[BPT], bcur[BPT];   // REGB: second vector of the next tile in flight / of the current tile
     int dnext = 0;
     if (tile0 < ntiles) {
         load_hidx(tile0, hid_n);
         if (is_staged(sdesc)) load_halo(hid_n, sdesc[3], h0, h1);
         if (CG_A) load_x(tile0, xv);
-        if (REGB && !(MODE == MODE_MGR0)) load_b(tile0, bq);
         if (is_staged(sdesc)) halo_to_smem(smem, sdesc[3], h0, h1);
         load_hidx(tile0 + G, hid_n);
         if (tile0 + G < ntiles && is_staged(sdesc + 16)) load_halo(hid_n, sdesc[16 + 3], h0, h1);
@@ -589,13 +576,8 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
             fence_proxy_async();
         }
         if (MGR) {
-            elementwise_mgr(smem, tile0, bq);
+            elementwise_mgr(smem, tile0);
             fence_proxy_async();
-        }
-        if (REGB) {
-#pragma unroll
-            for (int i = 0; i < BPT; ++i) bcur[i] = bq[i];
-            if (!(MODE == MODE_MGR0)) load_b(tile0 + G, bq);
         }
     }
     double2 acc[MODE == MODE_AX ? 2 : 1] = {};
@@ -634,12 +616,15 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
             dnext = tile + 4 * G < ntiles ? m.tile_desc[(tile + 4 * G) * 16 + tid] : 0;
         }
 
-        constexpr int RPT = T / ROWS;                     // rows of a tile per thread (= BPT in the REGB modes)
-#pragma unroll(REGB ? RPT : 1)
-        for (int i = 0; i < RPT; ++i) {
-            const int r = rg + i * ROWS;
-            if (r >= nrows) break;
+        for (int r = rg; r < nrows; r += ROWS) {
             const int64_t row = row0 + r;
+            // REGB: the row's own entry of the second vector straight from global memory, asked for before the gather
+            // (thread 0 prefetched the tile into L2 when it issued the tile's bulk copies)
+            double2 rv_g = {0.0, 0.0};
+            if (REGB) {
+                const double* __restrict__ src = (MODE == MODE_MGR0) ? a.in0 : a.in1;
+                if (src) rv_g = ld2(src, row * K + 2 * l);
+            }
             const int chl = r >> m.log2c;
             const int cpr = scp[chl];
             const int w = (scp[chl + 1] - cpr) >> m.log2c;
@@ -729,7 +714,7 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
                 const double av = sar[r];
                 double2 o = {fma(cc.x, s.x, av * own.x), fma(cc.y, s.y, av * own.y)};   // A v
                 if (sub >= 1) {
-                    const double2 rv = REGB ? bcur[REGB ? i : 0] : sb[r * TPR + l];
+                    const double2 rv = REGB ? rv_g : sb[r * TPR + l];
                     o.x = rv.x - o.x; o.y = rv.y - o.y;                                  // r - A v
                     if (MGR && a.omega2 != 0.0) {      // second sweep: e2 = e1 + omega2 (r' - K e1)/d
                         o.x = fma(a.omega2 * o.x, rcp_pos(fma(cc.x, sd, av)), own.x);
@@ -779,13 +764,8 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
                 fence_proxy_async();
             }
             if (MGR) {
-                elementwise_mgr(st1, tile + G, bq);
+                elementwise_mgr(st1, tile + G);
                 fence_proxy_async();
-            }
-            if (REGB) {
-#pragma unroll
-                for (int i = 0; i < BPT; ++i) bcur[i] = bq[i];
-                if (!(MODE == MODE_MGR0)) load_b(tile + 2 * G, bq);
             }
         }
     }
