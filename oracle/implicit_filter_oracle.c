@@ -431,7 +431,8 @@ static int64_t find_col(const orc_mesh *m, int64_t row, int64_t c) {
     return -1;
 }
 
-int orc_build_vector(orc_mesh *m, const double *coords, int dim, const int32_t *tri, int64_t nt, double radius) {
+int orc_build_vector(orc_mesh *m, const double *coords, int dim, const int32_t *tri, int64_t nt, const double *period,
+                     double radius) {
     free(m->dval); free(m->tval);
     m->dval = (double *)calloc((size_t)m->nnz, sizeof(double));
     m->tval = (double *)calloc((size_t)m->nnz, sizeof(double));
@@ -440,8 +441,12 @@ int orc_build_vector(orc_mesh *m, const double *coords, int dim, const int32_t *
     for (int64_t t = 0; t < nt; ++t) {
         int64_t v[3] = {tri[3 * t], tri[3 * t + 1], tri[3 * t + 2]};
         double x[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
-        for (int c = 0; c < 3; ++c)
-            for (int d = 0; d < dim; ++d) x[c][d] = coords[v[c] * dim + d];
+        for (int d = 0; d < dim; ++d) x[0][d] = coords[v[0] * dim + d];
+        for (int c = 1; c < 3; ++c) {                      /* minimum image on periodic axes, as in orc_build */
+            double e[3];
+            edge_vec(coords, dim, period, v[0], v[c], e);
+            for (int d = 0; d < dim; ++d) x[c][d] = x[0][d] + e[d];
+        }
         /* unit normal, area, P1 gradients in the triangle's plane: grad N_a = n x (x_c - x_b) / (2 area) */
         double e1[3], e2[3], nrm[3];
         for (int d = 0; d < 3; ++d) { e1[d] = x[1][d] - x[0][d]; e2[d] = x[2][d] - x[0][d]; }

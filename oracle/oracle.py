@@ -58,7 +58,7 @@ def _load():
         L.orc_dense_solve.argtypes = [vp, vp, dbl, i32, dbl, vp]
         L.orc_threads.restype = i32
         L.orc_build_vector.restype = i32
-        L.orc_build_vector.argtypes = [vp, vp, i32, vp, i64, dbl]
+        L.orc_build_vector.argtypes = [vp, vp, i32, vp, i64, vp, dbl]
         L.orc_get_vector_csr.argtypes = [vp, vp, vp]
         L.orc_apply_vector.argtypes = [vp, dbl, i32, dbl, vp, vp, vp, vp, vp]
         L.orc_solve_vector.restype = i32
@@ -93,7 +93,7 @@ class OracleMesh:
             raise ValueError("oracle: " + self._ERR.get(err.value, f"error {err.value}"))
         self.nv = int(L.orc_nv(self._h))
         self.nnz = int(L.orc_nnz(self._h))
-        self._coords, self._tri = coords, tri          # kept for build_vector
+        self._coords, self._tri, self._period = coords, tri, per          # kept for build_vector
         self._vector = False
 
     def __del__(self):
@@ -155,7 +155,8 @@ class OracleMesh:
         if self._coords.shape[1] == 3 and radius == 0.0:
             radius = float(np.linalg.norm(self._coords, axis=1).mean())
         st = _load().orc_build_vector(self._h, _p(self._coords), self._coords.shape[1], _p(self._tri),
-                                      self._tri.shape[0], float(radius))
+                                      self._tri.shape[0], None if self._period is None else _p(self._period),
+                                      float(radius))
         if st != 0:
             raise MemoryError("oracle: out of memory")
         self._vector = True

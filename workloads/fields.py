@@ -84,3 +84,33 @@ def log_spaced(lo: float, hi: float, count: int) -> np.ndarray:
         return np.array([lo], dtype=np.float64)
     j = np.arange(count, dtype=np.float64)
     return lo * (hi / lo) ** (j / (count - 1))
+
+
+def sphere_frames(coords: np.ndarray):
+    """Unit zonal (east) and meridional (north) vectors at points of a sphere centred at the origin."""
+    x = coords / np.linalg.norm(coords, axis=1, keepdims=True)
+    rho = np.sqrt(x[:, 0] ** 2 + x[:, 1] ** 2)
+    east = np.stack([-x[:, 1] / rho, x[:, 0] / rho, np.zeros_like(rho)], 1)
+    north = np.cross(x, east)
+    return east, north
+
+
+def sphere_velocity_field(coords: np.ndarray, kmax: int, n_waves: int, rng: np.random.Generator):
+    """Seeded tangent velocity field on the sphere in zonal / meridional components (u, v): the tangential part of
+    U(x) = sum_j |kappa_j|^-1.5 cos(kappa_j.x + theta_j) b_j with random unit vectors b_j, plus a rigid rotation about
+    a random axis (amplitude 1).  Stand-in for the FESOM2 surface velocities of PAPER.md:133."""
+    k = rng.integers(-kmax, kmax + 1, size=(4 * n_waves + 16, 3))
+    n2 = (k * k).sum(1)
+    k = k[(n2 >= 1) & (n2 <= kmax * kmax)][:n_waves].astype(np.float64)
+    theta = rng.uniform(0.0, 2.0 * np.pi, size=k.shape[0])
+    b = rng.normal(size=(k.shape[0], 3))
+    b /= np.linalg.norm(b, axis=1, keepdims=True)
+    amp = np.sqrt((k * k).sum(1)) ** -1.5
+    axis = rng.normal(size=3)
+    axis /= np.linalg.norm(axis)
+    U = np.cross(axis[None, :], coords)
+    step = 1 << 15
+    for s in range(0, coords.shape[0], step):
+        U[s:s + step] += (np.cos(coords[s:s + step] @ k.T + theta) * amp) @ b
+    east, north = sphere_frames(coords)
+    return np.einsum("ij,ij->i", U, east), np.einsum("ij,ij->i", U, north)

@@ -237,3 +237,20 @@ def delaunay_mesh(n: int, rng: np.random.Generator, hubs: int = 3, hub_valence: 
     tri = Delaunay(pts).simplices.astype(np.int32)
     return Mesh(coords=np.ascontiguousarray(pts), tri=np.ascontiguousarray(tri), period=None, h=1.0,
                 name=f"delaunay{n}")
+
+
+def sphere_band(mesh: Mesh, max_lat_deg: float) -> Mesh:
+    """Keep the part of a sphere mesh with |latitude| <= max_lat_deg: every triangle touching a removed vertex is
+    dropped, ids are compacted.  Model meshes keep their grid poles out of the ocean (a rotated grid with
+    the pole over land); the lon/lat components of a velocity, which the vector filter of PAPER.md:87-91 works
+    with, are singular at the poles (metric factor m = tan(latitude) / R_e)."""
+    x = mesh.coords
+    lat = np.degrees(np.arcsin(x[:, 2] / np.linalg.norm(x, axis=1)))
+    keep_v = np.abs(lat) <= max_lat_deg
+    tri = mesh.tri
+    tri = tri[keep_v[tri[:, 0]] & keep_v[tri[:, 1]] & keep_v[tri[:, 2]]]
+    used = np.zeros(x.shape[0], dtype=bool)
+    used[tri.ravel()] = True
+    new_id = np.cumsum(used, dtype=np.int64) - 1
+    return Mesh(coords=np.ascontiguousarray(x[used]), tri=np.ascontiguousarray(new_id[tri].astype(np.int32)),
+                period=None, h=mesh.h, name=mesh.name + f"b{max_lat_deg:g}")
