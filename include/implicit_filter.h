@@ -64,6 +64,18 @@ enum {
                               (about 3 x the memory of the prepared mesh, a second or two of device time)          */
     IF_FLAG_HIGHPASS = 2, /* if_filter (per call): write the high-pass field phi - phibar_l (PAPER.md:143-147,
                              Fig. 3) instead of phibar_l                                                    */
+    IF_FLAG_VECTOR = 16,  /* if_prepare: also assemble the metric terms of the vector Laplacian.
+                             if_filter / if_spectrum / if_apply (per call, order_n 1|2, n_fields even): the fields are
+                             velocities in pairs (u_0, v_0, u_1, v_1, ...) = (zonal, meridional) components at the
+                             vertices, and every pair is filtered as ONE coupled 2V x 2V system
+                                 S_2 = M_2 + gamma l^2 D_2   |   M_2 + gamma l^4 D_2 M_2^-1 D_2,   D_2 = [D~ T; -T D~],
+                                 D~_vv' = int (grad N_v . grad N_v' + (R_e^-2 + m^2) N_v N_v') dS,
+                                 T_vv'  = int m (-N_v' dx N_v + N_v dx N_v') dS,   m = tan(latitude) / R_e per triangle
+                             (dim = 3: the mesh lies on a sphere about the origin, latitude from the z axis; dim = 2: no
+                             metric terms, two scalar filters).  T is antisymmetric, D_2 symmetric positive semidefinite:
+                             Jacobi-preconditioned CG with one residual norm over both components.  if_stats reports a
+                             pair's iterations and status under both of its fields.  Combine with IF_FLAG_PAIRS for
+                             the kinetic-energy spectrum                                                        */
     IF_FLAG_PAIRS = 8     /* if_spectrum (per call): the fields are velocity components in pairs (u_0, v_0, u_1, v_1, ...)
                              and the spectra of a pair are added (kinetic energy 1/2 <u^2 + v^2>, the quantity of
                              PAPER.md:149-157): n_fields even; energy is [n_fields/2][n_ells], E [n_fields/2][n_ells-1];
@@ -89,6 +101,7 @@ typedef struct {
                         prepared with IF_FLAG_MULTIGRID, else ignored); the rest by Jacobi-PCG.  Same systems, same
                         start vector, same stop test, same answers within the tolerance (PAPER.md:207 names the
                         convergence of plain CG at large scales, above all for n = 2, as the open problem)           */
+    double radius;     /* if_prepare with IF_FLAG_VECTOR: R_e of the metric terms; 0 => the mean |x_v| of a dim = 3 mesh    */
     double mg_min_ell; /* 0 => 4 for n = 1, 0.5 for n = 2 (in mean edge lengths; below that Jacobi-PCG is cheaper)     */
 } if_options;
 

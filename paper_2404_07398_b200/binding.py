@@ -21,6 +21,7 @@ IF_FLAG_KEEP_CSR = 1
 IF_FLAG_HIGHPASS = 2
 IF_FLAG_MULTIGRID = 4
 IF_FLAG_PAIRS = 8
+IF_FLAG_VECTOR = 16
 
 EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_spectrum_host", "if_apply", "if_mesh_info", "if_mesh_tile_info",
            "if_mesh_multigrid_info",
@@ -30,7 +31,7 @@ EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_s
 class if_options(C.Structure):
     _fields_ = [("gamma", C.c_double), ("tol", C.c_double), ("max_iter", C.c_int), ("check_every", C.c_int),
                 ("batch", C.c_int), ("sell_c", C.c_int), ("sell_sigma", C.c_int), ("sfc_kind", C.c_int),
-                ("flags", C.c_int), ("solver", C.c_int), ("mg_min_ell", C.c_double)]
+                ("flags", C.c_int), ("solver", C.c_int), ("radius", C.c_double), ("mg_min_ell", C.c_double)]
 
 
 class if_stats(C.Structure):

@@ -53,6 +53,7 @@ struct Options {
     int sfc_kind = 0;
     int flags = 0;
     int solver = 0;
+    double radius = 0.0;        // R_e of the vector filter's metric terms; 0: mean |x_v| (dim = 3)
     double mg_min_ell = 0.0;    // 0: the default of the order (mg_solve.cuh: 4 mean edges for n = 1, 0.5 for n = 2)
 };
 
@@ -145,6 +146,12 @@ struct if_mesh_s {
     double* gdiag = nullptr;        // [n_vert] sum_j S_vj^2/A_j = diag(S M^-1 S)
     double* gdiag3 = nullptr;       // [n_vert] diag(S (M^-1 S)^2)   (filter order 3)
     double* gdiag4 = nullptr;       // [n_vert] diag(S (M^-1 S)^3)   (filter order 4)
+    // vector filter with metric terms (IF_FLAG_VECTOR), same SELL slots as sell_val:
+    double* sell_dval = nullptr;    // [sell_slots] D~_vv' / l^2 (off-diagonal)
+    double* sell_tval = nullptr;    // [sell_slots] T_vv' / l^2
+    double* ddiag = nullptr;        // [n_vert] D~_vv / l^2
+    double* gdiag_vec = nullptr;    // [n_vert] diag(D_2 M_2^-1 D_2) = sum_j (D~_vj^2 + T_vj^2) / A_j
+    double radius = 0.0;            // R_e used for the metric terms (0: planar mesh, none)
     int32_t* perm = nullptr;        // [n_vert] internal -> caller
     int32_t* iperm = nullptr;       // [n_vert] caller -> internal
     // optional unpermuted CSR (IF_FLAG_KEEP_CSR), caller numbering

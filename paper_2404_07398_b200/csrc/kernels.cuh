@@ -34,6 +34,7 @@ struct MeshView {
     const int64_t* __restrict__ chunk_ptr;
     const int32_t* __restrict__ col;
     const double* __restrict__ val;
+    const double* __restrict__ tval;        // vector filter: T entries beside val = D~ entries (null for scalar fields)
     const double* __restrict__ area;
     const double* __restrict__ inv_area;
     const double* __restrict__ sdiag;
@@ -71,7 +72,8 @@ struct Ctrl {
     int starting[KMAX];   // multigrid path: the column was (re)started; its first iteration only applies the
                           // preconditioner (alpha = 0, then rho = r.z, beta = 0), see k_init
     int cur_r;            // multigrid path: which residual buffer holds r (flipped with cur_p)
-    int pad1_;
+    int pair_mode;        // vector filter: columns (2i, 2i+1) are the (u, v) of ONE system: its dot products are the
+                          // sums over both columns, so both share alpha, beta and the stop decision
     int all_done;
     int cur_p;            // which direction buffer holds the current direction (flipped at the end of every iteration)
     int max_iter;
@@ -271,15 +273,18 @@ struct SpmmArgs {
 
 // One row of the staged SpMM: all column ids and values of the row first, then all W gathers from the shared
 // tile, then the multiply-adds on two accumulators -- one shared-memory latency per phase instead of one per entry.
-template <int W, int TPR>
+// VEC (vector filter): the thread's two columns are the (u, v) of one system and every entry carries the
+// pair (D~_ij, T_ij):  s_u += D~ p_u + T p_v ;  s_v += D~ p_v - T p_u.
+template <int W, int TPR, bool VEC>
 __device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_row, const double* __restrict__ sval_row,
-                                              const double2* __restrict__ sa, int l) {
+                                              const double* __restrict__ stval_row, const double2* __restrict__ sa, int l) {
     int2 cj[W / 2];
-    double2 vj[W / 2];
+    double2 vj[W / 2], tj[VEC ? W / 2 : 1];
 #pragma unroll
     for (int k = 0; k < W / 2; ++k) {
         cj[k] = reinterpret_cast<const int2*>(scol_row)[k];
         vj[k] = reinterpret_cast<const double2*>(sval_row)[k];
+        if (VEC) tj[VEC ? k : 0] = reinterpret_cast<const double2*>(stval_row)[k];
     }
     double2 g[W];
 #pragma unroll
@@ -292,6 +297,11 @@ __device__ __forceinline__ double2 gather_row(const int32_t* __restrict__ scol_r
     for (int k = 0; k < W / 2; ++k) {
         s0.x = fma(vj[k].x, g[2 * k].x, s0.x);     s0.y = fma(vj[k].x, g[2 * k].y, s0.y);
         s1.x = fma(vj[k].y, g[2 * k + 1].x, s1.x); s1.y = fma(vj[k].y, g[2 * k + 1].y, s1.y);
+        if (VEC) {
+            const double2 t = tj[VEC ? k : 0];
+            s0.x = fma(t.x, g[2 * k].y, s0.x);      s0.y = fma(-t.x, g[2 * k].x, s0.y);
+            s1.x = fma(t.y, g[2 * k + 1].y, s1.x);  s1.y = fma(-t.y, g[2 * k + 1].x, s1.y);
+        }
     }
     s0.x += s1.x;
     s0.y += s1.y;
@@ -328,7 +338,7 @@ template <int K, int MODE> struct SpmmCfg {
     static constexpr int STAGES = (K == 8 || (K == 16 && REGB)) ? 2 : SPMM_STAGES;
 };
 
-template <int K, int MODE> struct TileSmem {
+template <int K, int MODE, bool VEC = false> struct TileSmem {
     static constexpr int T = TILE_ROWS;
     // tile-sized vector regions of a stage: the gathered vector (+ halo), and the second vector unless it goes
     // through registers
@@ -337,7 +347,8 @@ template <int K, int MODE> struct TileSmem {
     static constexpr size_t vec_bytes = (size_t)T * K * sizeof(double);
     static constexpr size_t off_b = (size_t)(T + HALO_CAP) * K * sizeof(double);
     static constexpr size_t off_val = off_b + (NVEC - 1) * vec_bytes;
-    static constexpr size_t off_col = off_val + (size_t)T * WCAP * sizeof(double);
+    static constexpr size_t off_tval = off_val + (size_t)T * WCAP * sizeof(double);   // vector filter: T entries
+    static constexpr size_t off_col = off_tval + (VEC ? (size_t)T * WCAP * sizeof(double) : 0);
     static constexpr size_t off_dg = off_col + (size_t)T * WCAP * sizeof(int32_t);   // S_vv of the tile's rows
     static constexpr size_t off_ar = off_dg + (size_t)T * sizeof(double);            // A_v or 1/A_v
     static constexpr size_t stage_bytes = off_ar + (size_t)T * sizeof(double);
@@ -362,10 +373,10 @@ __device__ __forceinline__ TileIssue load_issue(const int32_t* __restrict__ desc
 //   x and the halo rows of tile i+1 are in flight into registers,
 //   descriptors and halo row ids are fetched two tiles ahead.
 // About 130 KB of loads per SM are outstanding at all times, which is what the loaded HBM latency of B200 needs.
-template <int K, int MODE>
+template <int K, int MODE, bool VEC = false>
 __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) k_spmm(MeshView m, Ctrl* __restrict__ ctrl,
                                                         double* __restrict__ partials, SpmmArgs a_in) {
-    using SM = TileSmem<K, MODE>;
+    using SM = TileSmem<K, MODE, VEC>;
     constexpr int T = SM::T;
     constexpr int NT = SpmmCfg<K, MODE>::NT;
     constexpr int NS = SpmmCfg<K, MODE>::STAGES;         // pipeline stages
@@ -429,7 +440,7 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
         const uint32_t dbytes = ((uint32_t)nrows * 8u + 15u) & ~15u;   // the arrays are padded by 16 bytes
         const bool staged = ti.nh >= 0 && ti.slots <= T * WCAP;
         uint64_t* bar = &bars[stage];
-        mbar_expect_tx(bar, vbytes * SM::NLOAD + 2u * dbytes + (staged ? (uint32_t)ti.slots * 12u : 0u));
+        mbar_expect_tx(bar, vbytes * SM::NLOAD + 2u * dbytes + (staged ? (uint32_t)ti.slots * (VEC ? 20u : 12u) : 0u));
         bulk_load(st, a.in0 + row0 * K, vbytes, bar);
         if (SM::NLOAD >= 2) bulk_load(st + SM::off_b, a.in1 + row0 * K, vbytes, bar);
         if (REGB && MODE == MODE_AX && a.in1) bulk_prefetch_l2(a.in1 + row0 * K, vbytes);
@@ -437,6 +448,7 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
         bulk_load(st + SM::off_ar, rowfac + row0, dbytes, bar);
         if (staged) {
             bulk_load(st + SM::off_val, m.val + ti.cp_first, (uint32_t)ti.slots * 8u, bar);
+            if (VEC) bulk_load(st + SM::off_tval, m.tval + ti.cp_first, (uint32_t)ti.slots * 8u, bar);
             bulk_load(st + SM::off_col, m.lcol + ti.cp_first, (uint32_t)ti.slots * 4u, bar);
         }
     };
@@ -589,6 +601,7 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
         const double2* sa = reinterpret_cast<const double2*>(st);          // gathered vector: tile + halo
         const double2* sb = reinterpret_cast<const double2*>(st + SM::off_b);   // own p' (CG2B)
         const double* sval = reinterpret_cast<const double*>(st + SM::off_val);
+        const double* stval = reinterpret_cast<const double*>(st + SM::off_tval);
         const int32_t* scol = reinterpret_cast<const int32_t*>(st + SM::off_col);
         const double* sdg = reinterpret_cast<const double*>(st + SM::off_dg);
         const double* sar = reinterpret_cast<const double*>(st + SM::off_ar);
@@ -635,10 +648,10 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
                 // every neighbour (tile or halo) is in shared memory under its tile-local index
                 // the width is the same for all rows of a SELL slice, hence warp-uniform: fully unrolled rows
                 switch (w) {
-                    case 2: s = gather_row<2, TPR>(scol + o, sval + o, sa, l); break;
-                    case 4: s = gather_row<4, TPR>(scol + o, sval + o, sa, l); break;
-                    case 6: s = gather_row<6, TPR>(scol + o, sval + o, sa, l); break;
-                    case 8: s = gather_row<8, TPR>(scol + o, sval + o, sa, l); break;
+                    case 2: s = gather_row<2, TPR, VEC>(scol + o, sval + o, stval + o, sa, l); break;
+                    case 4: s = gather_row<4, TPR, VEC>(scol + o, sval + o, stval + o, sa, l); break;
+                    case 6: s = gather_row<6, TPR, VEC>(scol + o, sval + o, stval + o, sa, l); break;
+                    case 8: s = gather_row<8, TPR, VEC>(scol + o, sval + o, stval + o, sa, l); break;
                     default:
                         // a slice wider than 8 (a vertex of valence 9 or more in its 32 rows): the tile's slots still
                         // fit the shared slice (is_staged checks the total), so the same gather as a plain loop
@@ -648,6 +661,11 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
                             const double2 g0 = sa[cj.x * TPR + l], g1 = sa[cj.y * TPR + l];
                             s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
                             s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
+                            if (VEC) {
+                                const double2 tj = *reinterpret_cast<const double2*>(stval + o + k);
+                                s.x = fma(tj.x, g0.y, s.x); s.y = fma(-tj.x, g0.x, s.y);
+                                s.x = fma(tj.y, g1.y, s.x); s.y = fma(-tj.y, g1.x, s.y);
+                            }
                         }
                         break;
                 }
@@ -696,6 +714,11 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
                     }
                     s.x = fma(vj.x, g0.x, s.x); s.y = fma(vj.x, g0.y, s.y);
                     s.x = fma(vj.y, g1.x, s.x); s.y = fma(vj.y, g1.y, s.y);
+                    if (VEC) {
+                        const double2 tj = ld2(m.tval, cp_first + o + k);
+                        s.x = fma(tj.x, g0.y, s.x); s.y = fma(-tj.x, g0.x, s.y);
+                        s.x = fma(tj.y, g1.y, s.x); s.y = fma(-tj.y, g1.x, s.y);
+                    }
                 }
             }
             const double sd = sdg[r];
@@ -775,7 +798,7 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
         const double2 acc1[1] = {acc[0]};
         if (grid_reduce<K, 1, NT>(acc1, partials, &ctrl->ticket[0], tot)) {
             if (tid < K) {
-                const double pq = tot[tid];
+                const double pq = ctrl->pair_mode ? tot[tid & ~1] + tot[tid | 1] : tot[tid];
                 double al = 0.0;
                 if (!ctrl->done[tid] && !ctrl->starting[tid]) {   // (a starting column has no direction yet)
                     if (pq > 0.0 && isfinite(pq)) al = ctrl->rho[tid] / pq;
@@ -856,7 +879,10 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
     __shared__ double tot[3 * KMAX];
     if (grid_reduce<K, 3>(acc, partials, &ctrl->ticket[1], tot)) {
         if (tid < K && ((mask >> tid) & 1u)) {
-            const double rho = tot[tid], rr = tot[KMAX + tid], bb = tot[2 * KMAX + tid];
+            const int ta = ctrl->pair_mode ? (tid & ~1) : tid, tb = ctrl->pair_mode ? (tid | 1) : tid;
+            const double w2 = ctrl->pair_mode ? 1.0 : 0.5;      // (ta == tb without pairs: the value itself)
+            const double rho = w2 * (tot[ta] + tot[tb]), rr = w2 * (tot[KMAX + ta] + tot[KMAX + tb]),
+                         bb = w2 * (tot[2 * KMAX + ta] + tot[2 * KMAX + tb]);
             ctrl->c[tid] = sp.c[tid]; ctrl->c1[tid] = sp.c1[tid]; ctrl->field[tid] = sp.field[tid]; ctrl->rhs[tid] = sp.rhs[tid];
             ctrl->starting[tid] = mg;
             ctrl->rho[tid] = rho; ctrl->rr[tid] = rr; ctrl->bb[tid] = bb;
@@ -928,7 +954,9 @@ __global__ void __launch_bounds__(BLOCK, 2) k_update(MeshView m, Ctrl* __restric
         __syncthreads();
         if (tid < K) {
             if (!ctrl->done[tid]) {
-                const double rho_new = tot[tid], rr = tot[KMAX + tid];
+                const bool pr = ctrl->pair_mode != 0;
+                const double rho_new = pr ? tot[tid & ~1] + tot[tid | 1] : tot[tid];
+                const double rr = pr ? tot[KMAX + (tid & ~1)] + tot[KMAX + (tid | 1)] : tot[KMAX + tid];
                 const int it = ctrl->iters[tid] + 1;
                 ctrl->iters[tid] = it;
                 ctrl->rr[tid] = rr;

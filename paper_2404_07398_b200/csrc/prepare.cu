@@ -94,6 +94,93 @@ __global__ void k_tri_emit(const double* __restrict__ coords, int dim, int64_t n
     }
 }
 
+// Vector filter: per triangle the 9 contributions to D~ = int (grad N_v . grad N_v' + (R_e^-2 + m^2) N_v N_v')
+// and to T = int m (-N_v' dx N_v + N_v dx N_v'), with the same 9 keys (row, col) as the stiffness assembly, so that after
+// sort + sum by key the entries line up one to one with the CSR of S.  The triangle is the flat 3-D triangle; latitude
+// and zonal direction are those of its centroid, m = tan(latitude) / R_e constant on it; P1 gradients
+// grad N_a = n x (x_c - x_b) / (2 area); int N_a N_b = area (1 + delta_ab) / 12, int N_a = area / 3.
+struct Add2v {
+    __device__ __forceinline__ double2 operator()(const double2& a, const double2& b) const {
+        return make_double2(a.x + b.x, a.y + b.y);
+    }
+};
+__global__ void k_tri_emit_vec(const double* __restrict__ coords, int dim, const int32_t* __restrict__ tri, int64_t nt,
+                               Period per, double inv_r, unsigned long long* __restrict__ keys, double2* __restrict__ vals) {
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nt) return;
+    const int64_t v[3] = {tri[3 * t], tri[3 * t + 1], tri[3 * t + 2]};
+    double x[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    for (int d = 0; d < dim; ++d) x[0][d] = coords[v[0] * dim + d];
+    for (int c = 1; c < 3; ++c) {
+        double e[3];
+        edge_vec(coords, dim, per, v[0], v[c], e);
+        for (int d = 0; d < 3; ++d) x[c][d] = x[0][d] + e[d];
+    }
+    double e1[3], e2[3], nrm[3];
+    for (int d = 0; d < 3; ++d) { e1[d] = x[1][d] - x[0][d]; e2[d] = x[2][d] - x[0][d]; }
+    nrm[0] = e1[1] * e2[2] - e1[2] * e2[1];
+    nrm[1] = e1[2] * e2[0] - e1[0] * e2[2];
+    nrm[2] = e1[0] * e2[1] - e1[1] * e2[0];
+    const double cr = sqrt(nrm[0] * nrm[0] + nrm[1] * nrm[1] + nrm[2] * nrm[2]);
+    const double area = 0.5 * cr;
+    for (int d = 0; d < 3; ++d) nrm[d] /= cr;
+    double g[3][3];
+    for (int a = 0; a < 3; ++a) {
+        const int b = (a + 1) % 3, c = (a + 2) % 3;
+        const double ed[3] = {x[c][0] - x[b][0], x[c][1] - x[b][1], x[c][2] - x[b][2]};
+        g[a][0] = (nrm[1] * ed[2] - nrm[2] * ed[1]) / cr;
+        g[a][1] = (nrm[2] * ed[0] - nrm[0] * ed[2]) / cr;
+        g[a][2] = (nrm[0] * ed[1] - nrm[1] * ed[0]) / cr;
+    }
+    double mt = 0.0, east[3] = {1.0, 0.0, 0.0};
+    if (dim == 3 && inv_r > 0.0) {
+        const double cx = (x[0][0] + x[1][0] + x[2][0]) / 3.0, cy = (x[0][1] + x[1][1] + x[2][1]) / 3.0;
+        const double cz = (x[0][2] + x[1][2] + x[2][2]) / 3.0;
+        const double rho = sqrt(cx * cx + cy * cy);
+        mt = (cz / rho) * inv_r;
+        east[0] = -cy / rho; east[1] = cx / rho; east[2] = 0.0;
+    }
+    double gx[3];
+    for (int a = 0; a < 3; ++a) gx[a] = g[a][0] * east[0] + g[a][1] * east[1] + g[a][2] * east[2];
+    const double mass_c = inv_r * inv_r + mt * mt;
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+            const double gg = g[a][0] * g[b][0] + g[a][1] * g[b][1] + g[a][2] * g[b][2];
+            keys[9 * t + 3 * a + b] = ((unsigned long long)v[a] << 32) | (unsigned long long)v[b];
+            vals[9 * t + 3 * a + b] = make_double2(area * gg + mass_c * area * (a == b ? 2.0 : 1.0) / 12.0,
+                                                   mt * (area / 3.0) * (gx[b] - gx[a]));
+        }
+}
+
+// the (D~, T) pairs of the CSR (caller numbering) into the SELL slots of the internal order, exactly as k_sell_fill
+// placed the entries of S; per row D~_vv and diag(D_2 M_2^-1 D_2)_v = sum_j (D~_vj^2 + T_vj^2) / A_j
+__global__ void k_sell_fill_vec(const int32_t* __restrict__ perm, const int64_t* __restrict__ rowptr,
+                                const int32_t* __restrict__ col, const double2* __restrict__ dt,
+                                const double* __restrict__ area_u, int64_t nv, int64_t n_chunks, int C,
+                                const int64_t* __restrict__ chunk_ptr, double* __restrict__ sell_dval,
+                                double* __restrict__ sell_tval, double* __restrict__ ddiag, double* __restrict__ gdiag_vec) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_chunks * C) return;
+    const int64_t c = r / C;
+    const int64_t w = (chunk_ptr[c + 1] - chunk_ptr[c]) / C;
+    const int64_t o = chunk_ptr[c] + (r - c * C) * w;
+    int64_t k = 0;
+    if (r < nv) {
+        const int64_t u = perm[r];
+        double gv = 0.0;
+        for (int64_t i = rowptr[u]; i < rowptr[u + 1]; ++i) {
+            const double2 e = dt[i];
+            gv += (e.x * e.x + e.y * e.y) / area_u[col[i]];
+            if (col[i] == u) { ddiag[r] = e.x; continue; }
+            sell_dval[o + k] = e.x;
+            sell_tval[o + k] = e.y;
+            ++k;
+        }
+        gdiag_vec[r] = gv;
+    }
+    for (; k < w; ++k) { sell_dval[o + k] = 0.0; sell_tval[o + k] = 0.0; }
+}
+
 // rowptr[r] = first unique entry whose row >= r.
 __global__ void k_rowptr(const unsigned long long* __restrict__ ukeys, int64_t nnz, int64_t nv,
                          int64_t* __restrict__ rowptr) {
@@ -407,16 +494,23 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
         if (in->batch != 0) o.batch = in->batch;
         if (in->solver != 0) o.solver = in->solver;
         if (in->mg_min_ell != 0.0) o.mg_min_ell = in->mg_min_ell;
+        if (!base && in->radius != 0.0) o.radius = in->radius;
         if (!base) {   // mesh-layout options are fixed at if_prepare
             if (in->sell_c != 0) o.sell_c = in->sell_c;
             if (in->sell_sigma != 0) o.sell_sigma = in->sell_sigma;
             o.sfc_kind = in->sfc_kind;
             o.flags = in->flags;
         } else {   // per-call flags
-            o.flags = (o.flags & ~(IF_FLAG_HIGHPASS | IF_FLAG_PAIRS)) | (in->flags & (IF_FLAG_HIGHPASS | IF_FLAG_PAIRS));
+            // per-call flags; IF_FLAG_VECTOR per call = "these fields are (u, v) pairs", valid on a handle that has the
+            // metric terms (checked in run_job)
+            const int per_call = IF_FLAG_HIGHPASS | IF_FLAG_PAIRS | IF_FLAG_VECTOR;
+            const bool has_metric = (o.flags & IF_FLAG_VECTOR) != 0;
+            o.flags = (o.flags & ~per_call) | (in->flags & per_call);
+            if ((o.flags & IF_FLAG_VECTOR) && !has_metric) return IF_EINVAL;
         }
     }
     if (!(o.gamma > 0.0) || !std::isfinite(o.gamma) || !(o.tol > 0.0) || !std::isfinite(o.tol)) return IF_EINVAL;
+    if (!(o.radius >= 0.0) || !std::isfinite(o.radius)) return IF_EINVAL;
     if (o.max_iter < 1 || o.check_every < 1) return IF_EINVAL;
     if (o.batch != 4 && o.batch != 8 && o.batch != 16) return IF_EINVAL;
     if ((o.sell_c != 32 && o.sell_c != 64 && o.sell_c != 128) || TILE_ROWS % o.sell_c != 0) return IF_EINVAL;   // must divide the SpMM row tile
@@ -438,7 +532,8 @@ extern "C" void if_destroy(if_handle h) {
     cudaGetDevice(&prev);
     cudaSetDevice(h->device);
     cudaFree(h->chunk_ptr); cudaFree(h->sell_col); cudaFree(h->sell_val); cudaFree(h->area);
-    cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->gdiag3); cudaFree(h->gdiag4); cudaFree(h->perm); cudaFree(h->iperm);
+    cudaFree(h->inv_area); cudaFree(h->sdiag); cudaFree(h->gdiag); cudaFree(h->gdiag3); cudaFree(h->gdiag4);
+    cudaFree(h->sell_dval); cudaFree(h->sell_tval); cudaFree(h->ddiag); cudaFree(h->gdiag_vec); cudaFree(h->perm); cudaFree(h->iperm);
     cudaFree(h->sell_lcol); cudaFree(h->halo_n); cudaFree(h->tile_desc); cudaFree(h->halo_rows);
     ifl::mg_free(h);
     cudaFree(h->csr_rowptr); cudaFree(h->csr_col); cudaFree(h->csr_val); cudaFree(h->csr_area);
@@ -656,6 +751,71 @@ static int prepare_impl(const double* coords, int dim, int64_t nv, const int32_t
     IF_LAUNCH_CHECK();
     IF_CUDA_TRY(cudaStreamSynchronize(st));
 
+    // ---- vector filter: metric terms (D~, T) on the slots of S
+    if (opt.flags & IF_FLAG_VECTOR) {
+        double radius = 0.0;
+        if (dim == 3) {
+            radius = opt.radius;
+            if (radius == 0.0) {           // mean |x_v| (host pass, like the bounding box)
+                double sum = 0.0;
+                for (int64_t v = 0; v < nv; ++v)
+                    sum += std::sqrt(coords[3 * v] * coords[3 * v] + coords[3 * v + 1] * coords[3 * v + 1] +
+                                     coords[3 * v + 2] * coords[3 * v + 2]);
+                radius = sum / (double)nv;
+            }
+            if (!(radius > 0.0)) return IF_EINVAL;
+        }
+        h->radius = radius;
+        DevBuf ek, ev, ek1, ev1, uk, uv, d_n;
+        IF_CUDA_TRY(ek.alloc((size_t)n_emit * 8));
+        IF_CUDA_TRY(ev.alloc((size_t)n_emit * 16));
+        IF_CUDA_TRY(ek1.alloc((size_t)n_emit * 8));
+        IF_CUDA_TRY(ev1.alloc((size_t)n_emit * 16));
+        k_tri_emit_vec<<<grid_for(nt), 256, 0, st>>>(d_coords.as<double>(), dim, d_tri.as<int32_t>(), nt, per,
+                                                    radius > 0.0 ? 1.0 / radius : 0.0, ek.as<unsigned long long>(),
+                                                    ev.as<double2>());
+        IF_LAUNCH_CHECK();
+        tb = 0;
+        IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tb, ek.as<unsigned long long>(), ek1.as<unsigned long long>(),
+                                                    ev.as<double2>(), ev1.as<double2>(), n_emit, 0, key_bits, st));
+        IF_CUDA_TRY(tmp.alloc(tb));
+        IF_CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tb, ek.as<unsigned long long>(), ek1.as<unsigned long long>(),
+                                                    ev.as<double2>(), ev1.as<double2>(), n_emit, 0, key_bits, st));
+        ++g_launches;
+        ek.alloc(0); ev.alloc(0);
+        IF_CUDA_TRY(uk.alloc((size_t)n_emit * 8));
+        IF_CUDA_TRY(uv.alloc((size_t)n_emit * 16));
+        IF_CUDA_TRY(d_n.alloc(sizeof(int64_t)));
+        tb = 0;
+        IF_CUDA_TRY(cub::DeviceReduce::ReduceByKey(nullptr, tb, ek1.as<unsigned long long>(), uk.as<unsigned long long>(),
+                                                   ev1.as<double2>(), uv.as<double2>(), d_n.as<int64_t>(), Add2v(), n_emit, st));
+        IF_CUDA_TRY(tmp.alloc(tb));
+        IF_CUDA_TRY(cub::DeviceReduce::ReduceByKey(tmp.p, tb, ek1.as<unsigned long long>(), uk.as<unsigned long long>(),
+                                                   ev1.as<double2>(), uv.as<double2>(), d_n.as<int64_t>(), Add2v(), n_emit, st));
+        ++g_launches;
+        int64_t n_u = 0;
+        IF_CUDA_TRY(cudaMemcpyAsync(&n_u, d_n.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        if (n_u != nnz) return IF_ECUDA;      // cannot happen: the keys are those of the stiffness assembly
+        DevBuf dval, tval, ddiag, gvec;
+        IF_CUDA_TRY(dval.alloc((size_t)sell_slots * 8 + 16));
+        IF_CUDA_TRY(tval.alloc((size_t)sell_slots * 8 + 16));
+        IF_CUDA_TRY(ddiag.alloc((size_t)nv * 8 + 16));
+        IF_CUDA_TRY(cudaMemsetAsync(ddiag.p, 0, (size_t)nv * 8 + 16, st));
+        IF_CUDA_TRY(gvec.alloc((size_t)nv * 8 + 16));
+        IF_CUDA_TRY(cudaMemsetAsync(gvec.p, 0, (size_t)nv * 8 + 16, st));
+        k_sell_fill_vec<<<grid_for(n_chunks * C), 256, 0, st>>>(perm.as<int32_t>(), rowptr.as<int64_t>(), ccol.as<int32_t>(),
+                                                               uv.as<double2>(), area_u.as<double>(), nv, n_chunks, C,
+                                                               chunk_ptr.as<int64_t>(), dval.as<double>(), tval.as<double>(),
+                                                               ddiag.as<double>(), gvec.as<double>());
+        IF_LAUNCH_CHECK();
+        IF_CUDA_TRY(cudaStreamSynchronize(st));
+        h->sell_dval = (double*)dval.release();
+        h->sell_tval = (double*)tval.release();
+        h->ddiag = (double*)ddiag.release();
+        h->gdiag_vec = (double*)gvec.release();
+    }
+
     // ---- row tiles of the SpMM kernel: halo lists and tile-local column ids
     const int64_t n_tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
     h->n_tiles = n_tiles;
@@ -820,6 +980,7 @@ extern "C" int if_save(if_handle h, const char* path) {
     hd.n_tiles = h->n_tiles; hd.halo_total = h->halo_total; hd.halo_max = h->halo_max;
     hd.unstaged_tiles = h->unstaged_tiles; hd.total_area = h->total_area; hd.mean_edge = h->mean_edge;
     hd.opt = h->opt;
+    hd.opt.radius = h->radius;     // the radius actually used
     hd.opt.flags &= ~(IF_FLAG_KEEP_CSR | IF_FLAG_HIGHPASS | IF_FLAG_PAIRS);
     std::vector<char> buf;
     const size_t nv = (size_t)h->n_vert, ns = (size_t)h->sell_slots, nt = (size_t)h->n_tiles;
@@ -834,6 +995,12 @@ extern "C" int if_save(if_handle h, const char* path) {
     if (rc == IF_OK) rc = write_dev(f, h->gdiag, nv * 8, buf);
     if (rc == IF_OK) rc = write_dev(f, h->gdiag3, nv * 8, buf);
     if (rc == IF_OK) rc = write_dev(f, h->gdiag4, nv * 8, buf);
+    if (h->opt.flags & IF_FLAG_VECTOR) {      // metric terms of the vector filter
+        if (rc == IF_OK) rc = write_dev(f, h->sell_dval, ns * 8, buf);
+        if (rc == IF_OK) rc = write_dev(f, h->sell_tval, ns * 8, buf);
+        if (rc == IF_OK) rc = write_dev(f, h->ddiag, nv * 8, buf);
+        if (rc == IF_OK) rc = write_dev(f, h->gdiag_vec, nv * 8, buf);
+    }
     if (rc == IF_OK) rc = write_dev(f, h->perm, nv * 4, buf);
     if (rc == IF_OK) rc = write_dev(f, h->iperm, nv * 4, buf);
     if (rc == IF_OK) rc = write_dev(f, h->halo_n, nt * 4, buf);
@@ -890,13 +1057,14 @@ extern "C" int if_load(const char* path, if_handle* out) {
             raw.gamma = hd.opt.gamma; raw.tol = hd.opt.tol; raw.max_iter = hd.opt.max_iter;
             raw.check_every = hd.opt.check_every; raw.batch = hd.opt.batch; raw.sell_c = hd.opt.sell_c;
             raw.sell_sigma = hd.opt.sell_sigma; raw.sfc_kind = hd.opt.sfc_kind; raw.flags = hd.opt.flags;
-            raw.solver = hd.opt.solver; raw.mg_min_ell = hd.opt.mg_min_ell;
+            raw.solver = hd.opt.solver; raw.mg_min_ell = hd.opt.mg_min_ell; raw.radius = hd.opt.radius;
             ok = ifl::resolve_options(&raw, nullptr, &chk) == IF_OK;
         }
         if (ok) {
             const int64_t nv = hd.n_vert, ns = hd.sell_slots, nt = hd.n_tiles;
             const int64_t expect = (int64_t)sizeof(hd) + (hd.n_chunks + 1) * 8 + ns * 16 + nv * (6 * 8 + 2 * 4) + nt * 4 +
-                                   nt * HALO_CAP * 4 + (nt + 1) * 64;
+                                   nt * HALO_CAP * 4 + (nt + 1) * 64 +
+                                   ((hd.opt.flags & IF_FLAG_VECTOR) ? ns * 16 + nv * 16 : 0);
             const bool with_mg = (hd.opt.flags & IF_FLAG_MULTIGRID) != 0;      // the hierarchy follows the mesh arrays
             ok = fseek(f, 0, SEEK_END) == 0 && (with_mg ? (int64_t)ftell(f) > expect : (int64_t)ftell(f) == expect) &&
                  fseek(f, (long)sizeof(hd), SEEK_SET) == 0;
@@ -931,6 +1099,13 @@ extern "C" int if_load(const char* path, if_handle* out) {
     if ((rc = read_dev(f, (void**)&h->gdiag, nv * 8, nv * 8 + 16, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->gdiag3, nv * 8, nv * 8 + 16, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->gdiag4, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+    if (h->opt.flags & IF_FLAG_VECTOR) {
+        if ((rc = read_dev(f, (void**)&h->sell_dval, ns * 8, ns * 8 + 16, buf))) return fail(rc);
+        if ((rc = read_dev(f, (void**)&h->sell_tval, ns * 8, ns * 8 + 16, buf))) return fail(rc);
+        if ((rc = read_dev(f, (void**)&h->ddiag, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+        if ((rc = read_dev(f, (void**)&h->gdiag_vec, nv * 8, nv * 8 + 16, buf))) return fail(rc);
+        h->radius = hd.opt.radius;
+    }
     if ((rc = read_dev(f, (void**)&h->perm, nv * 4, nv * 4, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->iperm, nv * 4, nv * 4, buf))) return fail(rc);
     if ((rc = read_dev(f, (void**)&h->halo_n, nt * 4, nt * 4, buf))) return fail(rc);

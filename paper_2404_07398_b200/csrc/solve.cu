@@ -74,6 +74,7 @@ struct Run {
     int order_n;
     Options opt;
     Grids g;
+    bool vec = false;  // vector filter: columns (2i, 2i+1) are the (u, v) of one coupled system (IF_FLAG_VECTOR)
     bool mg = false;   // this phase runs multigrid-preconditioned CG (mg_solve.cuh) instead of Jacobi-PCG
     MgGrids mgg;
     int mg_nu[3] = {1, 1, 2};   // Jacobi sweeps per side of the V cycle on the mesh, on level 1, below (mg_solve.cuh)
@@ -94,27 +95,37 @@ int resident_grid(Kern kern, size_t smem, int n_sm, int64_t work_items, int* gri
     return IF_OK;
 }
 
-template <int K>
-int setup_grids(Run& r) {
+template <int K, bool VEC>
+int setup_grids_v(Run& r) {
     const int64_t nv = r.h->n_vert;
     const int n_sm = r.h->n_sm;
     const int64_t tiles = (nv + TILE_ROWS - 1) / TILE_ROWS;
     const int64_t passes = (nv + BLOCK / (K / 2) - 1) / (BLOCK / (K / 2));
     int rc;
-    if ((rc = resident_grid(k_spmm<K, MODE_PLAIN>, TileSmem<K, MODE_PLAIN>::bytes, n_sm, tiles, &r.g.plain, SpmmCfg<K, MODE_PLAIN>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_PLAIN, VEC>, TileSmem<K, MODE_PLAIN, VEC>::bytes, n_sm, tiles, &r.g.plain, SpmmCfg<K, MODE_PLAIN>::NT))) return rc;
     if (r.order_n == 1) {
-        if ((rc = resident_grid(k_spmm<K, MODE_CG1>, TileSmem<K, MODE_CG1>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K, MODE_CG1>::NT))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_CG1, VEC>, TileSmem<K, MODE_CG1, VEC>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K, MODE_CG1>::NT))) return rc;
     } else {
-        if ((rc = resident_grid(k_spmm<K, MODE_CG2A>, TileSmem<K, MODE_CG2A>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K, MODE_CG2A>::NT))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_CG2A, VEC>, TileSmem<K, MODE_CG2A, VEC>::bytes, n_sm, tiles, &r.g.cga, SpmmCfg<K, MODE_CG2A>::NT))) return rc;
     }
-    if ((rc = resident_grid(k_spmm<K, MODE_CG2B>, TileSmem<K, MODE_CG2B>::bytes, n_sm, tiles, &r.g.cgb, SpmmCfg<K, MODE_CG2B>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_CG2B, VEC>, TileSmem<K, MODE_CG2B, VEC>::bytes, n_sm, tiles, &r.g.cgb, SpmmCfg<K, MODE_CG2B>::NT))) return rc;
     if ((rc = resident_grid(k_update<K>, 0, n_sm, passes, &r.g.update))) return rc;
     r.g.stream = (int)std::max<int64_t>(1, std::min<int64_t>(passes, (int64_t)n_sm * 4));
     return IF_OK;
 }
+template <int K>
+int setup_grids(Run& r) { return r.vec ? setup_grids_v<K, true>(r) : setup_grids_v<K, false>(r); }
 
 template <int K, int MODE>
 int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
+    constexpr bool CG_MODE = MODE == MODE_PLAIN || MODE == MODE_CG1 || MODE == MODE_CG2A || MODE == MODE_CG2B;
+    if constexpr (CG_MODE) {
+        if (r.vec) {
+            k_spmm<K, MODE, true><<<grid, SpmmCfg<K, MODE>::NT, TileSmem<K, MODE, true>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
+            IF_LAUNCH_CHECK();
+            return IF_OK;
+        }
+    }
     k_spmm<K, MODE><<<grid, SpmmCfg<K, MODE>::NT, TileSmem<K, MODE>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
     IF_LAUNCH_CHECK();
     return IF_OK;
@@ -274,6 +285,7 @@ Ctrl fresh_ctrl(const Run& r) {
     hc.all_done = 1;
     hc.max_iter = r.opt.max_iter;
     hc.tol2 = r.opt.tol * r.opt.tol;
+    hc.pair_mode = r.vec ? 1 : 0;
     return hc;
 }
 
@@ -283,17 +295,20 @@ int apply_all(Run& r, const double* d_fields, const std::vector<Rhs>& rhs, int n
     const if_mesh_s* h = r.h;
     int rc;
     if ((rc = setup_grids<K>(r))) return rc;
-    for (size_t first = 0; first < rhs.size(); first += K) {
-        const size_t count = std::min<size_t>(K, rhs.size() - first);
+    const size_t step = r.vec ? 2 : 1;          // columns per right-hand side (vector filter: the (u, v) pair)
+    const size_t per_batch = K / step;
+    for (size_t first = 0; first < rhs.size(); first += per_batch) {
+        const size_t count = std::min<size_t>(per_batch, rhs.size() - first) * step;     // columns in use
         Ctrl hc = fresh_ctrl(r);
         StartParams sp;
         memset(&sp, 0, sizeof(sp));
         for (int c = 0; c < KMAX; ++c) sp.field[c] = -1;
         for (size_t i = 0; i < count; ++i) {
-            const Rhs& q = rhs[first + i];
+            const Rhs& q = rhs[first + i / step];
+            const int f = r.vec ? 2 * q.f + (int)(i % step) : q.f;
             hc.c[i] = sp.c[i] = r.opt.gamma * std::pow(q.ell, 2.0 * r.order_n);
-            hc.field[i] = sp.field[i] = q.f;
-            hc.rhs[i] = sp.rhs[i] = q.f * n_ells + q.j;
+            hc.field[i] = sp.field[i] = f;
+            hc.rhs[i] = sp.rhs[i] = f * n_ells + q.j;
         }
         hc.all_done = 0;
         IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
@@ -341,21 +356,28 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
         memset(sp, 0, sizeof(*sp));
         for (int c = 0; c < KMAX; ++c) sp->field[c] = -1;
         *started = 0;
-        for (int c = 0; c < K; ++c) {
-            if (!((mask >> c) & 1u)) continue;
-            if (q.next < R) {
-                const Rhs& s = rhs[q.next];
-                sp->c[c] = r.opt.gamma * std::pow(s.ell, 2.0 * r.order_n);
-                sp->c1[c] = r.order_n == 1 ? sp->c[c] : std::sqrt(sp->c[c]);   // K = M + sqrt(c) S (mg_solve.cuh)
-                sp->field[c] = s.f;
-                sp->rhs[c] = s.f * n_ells + s.j;
-                q.col_rhs[c] = (int)q.next++;
-                ++q.active;
-            } else {
-                q.col_rhs[c] = -1;
+        // vector filter: a right-hand side is a (u, v) pair (field index = pair index) and takes the columns (c, c + 1)
+        const int step = r.vec ? 2 : 1;
+        for (int c0 = 0; c0 < K; c0 += step) {
+            if (!((mask >> c0) & 1u)) continue;
+            const bool have = q.next < R;
+            for (int c = c0; c < c0 + step; ++c) {
+                if (have) {
+                    const Rhs& s = rhs[q.next];
+                    const int f = r.vec ? 2 * s.f + (c - c0) : s.f;
+                    sp->c[c] = r.opt.gamma * std::pow(s.ell, 2.0 * r.order_n);
+                    sp->c1[c] = r.order_n == 1 ? sp->c[c] : std::sqrt(sp->c[c]);   // K = M + sqrt(c) S (mg_solve.cuh)
+                    sp->field[c] = f;
+                    sp->rhs[c] = f * n_ells + s.j;
+                    q.col_rhs[c] = (int)q.next;
+                    ++q.active;
+                } else {
+                    q.col_rhs[c] = -1;
+                }
+                *started |= 1u << c;
+                q.host_epoch[c] += 1;
             }
-            *started |= 1u << c;
-            q.host_epoch[c] += 1;
+            if (have) ++q.next;
         }
     };
     StartParams sp;
@@ -572,6 +594,8 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (rc != IF_OK) return rc;
     r.order_n = order_n;
     r.st = static_cast<cudaStream_t>(stream);
+    r.vec = opt_in && (opt_in->flags & IF_FLAG_VECTOR);      // per call only: the handle's own flag just says "assembled"
+    if (r.vec && (n_fields % 2 != 0 || order_n > 2 || !h->sell_dval)) return IF_EINVAL;
     const bool pairs = job == JOB_SPECTRUM && (r.opt.flags & IF_FLAG_PAIRS);
     const int n_out_fields = pairs ? n_fields / 2 : n_fields;
     int dev = -1;
@@ -581,7 +605,9 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (ws_bytes < r.w.bytes) return IF_EWORKSPACE;
     int log2c = 0;
     while ((1 << log2c) < h->sell_c) ++log2c;
-    r.m = MeshView{h->chunk_ptr, h->sell_col, h->sell_val, h->area, h->inv_area, h->sdiag, h->gdiag, h->gdiag3, h->gdiag4, h->perm,
+    // vector filter: D~ takes the place of S (entries, diagonal, Jacobi diagonal of n = 2), T rides beside it
+    r.m = MeshView{h->chunk_ptr, h->sell_col, r.vec ? h->sell_dval : h->sell_val, r.vec ? h->sell_tval : nullptr, h->area,
+                   h->inv_area, r.vec ? h->ddiag : h->sdiag, r.vec ? h->gdiag_vec : h->gdiag, h->gdiag3, h->gdiag4, h->perm,
                    h->sell_lcol, h->halo_rows, h->tile_desc, h->n_vert, h->n_chunks, log2c};
 
     PollState poll;
@@ -603,7 +629,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     // queue of right-hand sides: largest scale (most iterations) first, so that the short solves fill the tail
     std::vector<Rhs> rhs;
     rhs.reserve((size_t)R);
-    for (int f = 0; f < n_fields; ++f)
+    for (int f = 0; f < (r.vec ? n_fields / 2 : n_fields); ++f)      // (vector filter: f counts (u, v) pairs)
         for (int j = 0; j < n_ells; ++j) rhs.push_back(Rhs{ells[j], f, j});
     if (job != JOB_APPLY)
         std::stable_sort(rhs.begin(), rhs.end(), [](const Rhs& a, const Rhs& b) { return a.ell > b.ell; });
@@ -611,7 +637,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     KernelTimes ktimes, mgtimes;
     int64_t batch_iters = 0, mg_batch_iters = 0;
     // large scales by multigrid-preconditioned CG (option solver = 1): a stream of right-hand sides through 16 columns
-    if (job != JOB_APPLY && r.opt.solver == 1 && order_n <= 2 && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
+    if (job != JOB_APPLY && r.opt.solver == 1 && order_n <= 2 && !r.vec && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
         const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)) *
                                h->mean_edge;
         size_t n_big = 0;
@@ -636,7 +662,7 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
             batch_iters += mg_batch_iters;
         }
     }
-    const int K = pick_k(r.opt.batch, rhs.size());
+    const int K = pick_k(r.opt.batch, rhs.size() * (r.vec ? 2 : 1));
     if (job == JOB_APPLY) {
         rc = K == 4 ? apply_all<4>(r, d_fields, rhs, n_ells, d_out)
            : K == 8 ? apply_all<8>(r, d_fields, rhs, n_ells, d_out)

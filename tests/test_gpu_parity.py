@@ -805,3 +805,101 @@ def test_velocity_pairs_spectrum(ifl, oracle_mod):
         ifl.if_spectrum(h, w.fields[:3], w.ells, 1, flags=ifl.IF_FLAG_PAIRS)
     assert e.value.code == -1
     h.close()
+
+
+# ------------------------------------------------------------------------------------------ vector filter with metric terms
+def vector_workload(level, n_pairs, seed=21):
+    from workloads import icosphere, jitter_sphere, sphere_band, sphere_velocity_field
+    mesh = sphere_band(jitter_sphere(icosphere(level), 0.2, np.random.default_rng(seed)), 70.0)
+    rng = np.random.default_rng(seed + 1)
+    fields = np.empty((2 * n_pairs, mesh.n_vert))
+    for p in range(n_pairs):
+        fields[2 * p], fields[2 * p + 1] = sphere_velocity_field(mesh.coords, 3 * 2 ** (level - 3), 24, rng)
+    return mesh, fields
+
+
+@pytest.mark.parametrize("order_n", [1, 2])
+def test_vector_filter_matches_oracle(ifl, oracle_mod, order_n):
+    """IF_FLAG_VECTOR: (u, v) pairs filtered as coupled 2V x 2V systems with the metric terms D~, T.
+    Operator to 1e-12, coarse-grained velocities against the oracle's joint PCG with the tolerance derived from both
+    true residuals (S_2 >= M_2: D_2 is positive semidefinite), kinetic-energy spectra (IF_FLAG_PAIRS) to 1e-6; three
+    column widths, more pairs than columns (refill in pairs), and the scalar path of the same handle unchanged."""
+    mesh, fields = vector_workload(5, 3)
+    top = 20.0 if order_n == 1 else 8.0
+    from workloads import log_spaced
+    ells = mesh.h * log_spaced(1.0, top, 5)
+    om = oracle_mod.OracleMesh(mesh.coords, mesh.tri, None)
+    om.build_vector(1.0)
+    area = om.area()
+    VEC = ifl.IF_FLAG_VECTOR
+    h = ifl.if_prepare(mesh.coords, mesh.tri, None, flags=VEC, radius=1.0)
+    ap = ifl.if_apply(h, fields, ells, order_n, flags=VEC).cpu().numpy()
+    ref = {}
+    for p in range(3):
+        for j, ell in enumerate(ells):
+            ou, ov = om.apply_vector(fields[2 * p], fields[2 * p + 1], float(ell), order_n)
+            assert rel(ap[2 * p, j], ou) <= 1e-12 and rel(ap[2 * p + 1, j], ov) <= 1e-12, (p, j)
+            ref[p, j] = om.solve_vector(fields[2 * p], fields[2 * p + 1], float(ell), order_n)
+            assert ref[p, j][2]["status"] == 0
+    import torch
+    for batch in (16, 8, 4):
+        out, st = ifl.if_filter(h, fields, ells, order_n, flags=VEC, batch=batch)
+        assert st["code"] == 0
+        for p in range(3):
+            bnorm = np.linalg.norm(np.concatenate([area * fields[2 * p], area * fields[2 * p + 1]]))
+            for j, ell in enumerate(ells):
+                xu, xv, info = ref[p, j]
+                x = out[2 * p:2 * p + 2, j]
+                ax = ifl.if_apply(h, x, np.array([ell]), order_n, flags=VEC)[:, 0].cpu().numpy()
+                res_gpu = np.linalg.norm(np.concatenate([area * fields[2 * p] - ax[0], area * fields[2 * p + 1] - ax[1]])) / bnorm
+                xr = np.concatenate([xu, xv])
+                tol = max(TOL_FIELD, (res_gpu + info["true_res"]) * bnorm / area.min() / np.linalg.norm(xr))
+                err = rel(np.concatenate([x[0].cpu().numpy(), x[1].cpu().numpy()]), xr)
+                assert err <= tol, (batch, p, j, err, tol)
+                assert st["iters"][2 * p, j] == st["iters"][2 * p + 1, j] and st["status"][2 * p, j] == 0
+                assert 0.7 * info["iters"] <= st["iters"][2 * p, j] <= info["iters"] + 3
+    sp = ifl.if_spectrum(h, fields, ells, order_n, flags=VEC | ifl.IF_FLAG_PAIRS)
+    assert sp["energy"].shape == (3, 5)
+    for p in range(3):
+        ke = np.array([om.energy(ref[p, j][0]) + om.energy(ref[p, j][1]) for j in range(5)])
+        k_mid, E = oracle_mod.spectrum(ells, ke)
+        assert np.all(np.abs(sp["energy"][p] - ke) <= TOL_BIN * ke) and np.all(np.abs(sp["E"][p] - E) <= TOL_BIN * np.abs(E))
+    # without the per-call flag the same handle filters scalars, and the coupling is not a small effect
+    sc, _ = ifl.if_filter(h, fields[:2], ells[-1:], order_n)
+    su, _ = om.solve(fields[0], float(ells[-1]), order_n)
+    assert rel(sc[0, 0].cpu().numpy(), su) <= TOL_FIELD and rel(su, ref[0, 4][0]) > 1e-3
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_filter(h, fields[:3], ells, order_n, flags=VEC)               # odd number of fields
+    assert e.value.code == -1
+    h0 = ifl.if_prepare(mesh.coords, mesh.tri, None)
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_filter(h0, fields[:2], ells, order_n, flags=VEC)              # handle without metric terms
+    assert e.value.code == -1
+    h.close(); h0.close()
+
+
+def test_vector_filter_planar_mesh_and_save_load(ifl, oracle_mod, tmp_path):
+    """A planar mesh has no metric terms: the vector filter returns the two scalar filters.  The metric arrays go
+    through if_save / if_load."""
+    m = grid_mesh(40, periodic=True, jitter=0.2, random_diagonals=True, rng=np.random.default_rng(31))
+    fields = np.random.default_rng(32).standard_normal((2, m.n_vert))
+    ells = np.array([0.8, 2.5, 6.0])
+    h = ifl.if_prepare(m.coords, m.tri, m.period, flags=ifl.IF_FLAG_VECTOR)
+    a, sa = ifl.if_filter(h, fields, ells, 1, flags=ifl.IF_FLAG_VECTOR)
+    b, sb = ifl.if_filter(h, fields, ells, 1)
+    assert sa["code"] == 0 and float((a - b).abs().max()) <= 1e-9 * float(b.abs().max())
+    h.close()
+    mesh, vf = vector_workload(4, 1)
+    h = ifl.if_prepare(mesh.coords, mesh.tri, None, flags=ifl.IF_FLAG_VECTOR)     # radius 0 => mean |x_v| = 1
+    c, sc = ifl.if_filter(h, vf, mesh.h * ells, 2, flags=ifl.IF_FLAG_VECTOR)
+    path = str(tmp_path / "vec.ifm")
+    ifl.if_save(h, path)
+    h.close()
+    g = ifl.if_load(path)
+    d, sd = ifl.if_filter(g, vf, mesh.h * ells, 2, flags=ifl.IF_FLAG_VECTOR)
+    assert sc["code"] == 0 and np.array_equal(sc["iters"], sd["iters"]) and bool((c == d).all())
+    om = oracle_mod.OracleMesh(mesh.coords, mesh.tri, None)
+    om.build_vector()
+    xu, xv, info = om.solve_vector(vf[0], vf[1], float(mesh.h * ells[1]), 2)
+    assert rel(c[0, 1].cpu().numpy(), xu) <= TOL_FIELD and rel(c[1, 1].cpu().numpy(), xv) <= TOL_FIELD
+    g.close()
