@@ -191,7 +191,7 @@ def test_degenerate_inputs(ifl, oracle_mod):
         ifl.if_filter(h, w.fields, [1.0, -1.0], 1)
     assert e.value.code == -1
     with pytest.raises(ifl.ImplicitFilterError) as e:
-        ifl.if_filter(h, w.fields, [1.0], 3)
+        ifl.if_filter(h, w.fields, [1.0], 5)                     # orders 1 ... 4 exist
     assert e.value.code == -1
     with pytest.raises(ifl.ImplicitFilterError) as e:
         ifl.if_spectrum(h, w.fields, [2.0, 1.0], 1)
@@ -659,8 +659,9 @@ def test_refill_while_other_columns_have_a_pending_step(ifl, oracle_mod, check_e
                     # amplifies their rounding to 6e-7 with or without refill -- a misapplied last step is >= 1e-5
                     assert rel(out[f, j], x) <= (1e-12 if order_n == 1 else 5e-6), (order_n, f, j, rel(out[f, j], x))
                 else:
-                    assert abs(info["iters"] - st["iters"][f, j]) <= 1 and rel(out[f, j], x) <= 1e-3
-        assert same >= 24
+                    # (n = 2: a few hundred iterations on white noise move the stop of two implementations by a few)
+                    assert abs(info["iters"] - st["iters"][f, j]) <= (1 if order_n == 1 else 4) and rel(out[f, j], x) <= 1e-3
+        assert same >= (24 if order_n == 1 else 14)
     h.close()
 
 
