@@ -55,7 +55,8 @@ enum {
     IF_ENOMEM = -5,       /* host or device allocation failed                                              */
     IF_ECUDA = -6,        /* CUDA runtime error, or no device                                              */
     IF_EWORKSPACE = -7,   /* workspace smaller than if_workspace_bytes says                                */
-    IF_EIO = -8           /* if_save / if_load: file cannot be written / read, or is not a prepared mesh   */
+    IF_EIO = -8,          /* if_save / if_load: file cannot be written / read, or is not a prepared mesh   */
+    IF_ELIMIT = -9        /* if_energy_noalloc: more fields than its static scratch array serves per call  */
 };
 
 enum {
@@ -160,6 +161,16 @@ int if_spectrum(if_handle h, const double* d_fields, int n_fields, const double*
 int if_spectrum_host(if_handle h, const double* h_fields, int n_fields, const double* ells, int n_ells, int order_n,
                      double* energy, double* k_mid, double* E, void* d_workspace, size_t ws_bytes,
                      void* cuda_stream, const if_options* opt, if_stats* stats);
+
+/* The energy reduction alone, for callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses
+ * that forbid it):  d_energy[f] = 1/2 sum_v A_v x_fv^2 / sum_v A_v  (what if_spectrum reports per filtered
+ * field) for d_fields DEVICE [n_fields][n_vert] in the caller's numbering, e.g. the output of if_filter; d_energy DEVICE
+ * [n_fields].  Takes no workspace and allocates nothing: the scratch of its grid reduction is a static device array of
+ * 258 KiB inside the library (held by every GPU that loads the library until exit), which serves at most 32 fields per
+ * call -- more returns IF_ELIMIT.  One memset of 256 bytes and one kernel are enqueued on `cuda_stream`; no
+ * synchronisation.  The handle's device must be current (else IF_EINVAL).  All calls share the array: calls that
+ * overlap on the GPU (other streams or threads) race -- serialise them.  The result is deterministic. */
+int if_energy_noalloc(if_handle h, const double* d_fields, int n_fields, double* d_energy, void* cuda_stream);
 
 /* Operator only: d_out[f][j] = (M + gamma l_j^(2n) S (M^-1 S)^(n-1)) d_fields[f].  Same layouts as if_filter. */
 int if_apply(if_handle h, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,

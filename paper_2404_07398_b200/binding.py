@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libimplicit_filter.so")
 
 IF_OK, IF_WNOTCONVERGED = 0, 1
-IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKSPACE, IF_EIO = -1, -2, -3, -4, -5, -6, -7, -8
+IF_EINVAL, IF_EINDEX, IF_EDEGENERATE, IF_EORPHAN, IF_ENOMEM, IF_ECUDA, IF_EWORKSPACE, IF_EIO, IF_ELIMIT = -1, -2, -3, -4, -5, -6, -7, -8, -9
 IF_FLAG_KEEP_CSR = 1
 IF_FLAG_HIGHPASS = 2
 IF_FLAG_MULTIGRID = 4
@@ -24,7 +24,7 @@ IF_FLAG_PAIRS = 8
 IF_FLAG_VECTOR = 16
 
 EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_spectrum_host", "if_apply", "if_mesh_info", "if_mesh_tile_info",
-           "if_mesh_multigrid_info",
+           "if_mesh_multigrid_info", "if_energy_noalloc",
            "if_mesh_export_csr", "if_mesh_export_perm", "if_save", "if_load", "if_destroy", "if_strerror", "if_launch_count")
 
 
@@ -73,6 +73,8 @@ def load_library():
                               C.POINTER(if_stats)]
     L.if_spectrum_host.restype = i32
     L.if_spectrum_host.argtypes = L.if_spectrum.argtypes
+    L.if_energy_noalloc.restype = i32
+    L.if_energy_noalloc.argtypes = [vp, vp, i32, vp, vp]
     L.if_apply.restype = i32
     L.if_apply.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, C.c_size_t, vp, C.POINTER(if_options)]
     L.if_mesh_info.restype = i32
@@ -313,6 +315,24 @@ def if_spectrum_host(h: Handle, fields, ells: Sequence[float], order_n: int, wor
         _np_ptr(E), C.c_void_p(workspace.data_ptr()), workspace.numel(), s, None if opt is None else C.byref(opt),
         C.byref(st.c)), stream)
     return {"energy": energy, "k_mid": k_mid, "E": E, "stats": st.as_dict(rc)}
+
+
+def if_energy_noalloc(h: Handle, fields, out=None, stream=None):
+    """e_f = 1/2 sum_v A_v x_fv^2 / sum_v A_v for DEVICE fields [F][V] (torch.float64, caller's vertex order) into the
+    DEVICE tensor `out` [F]: the entry point that allocates nothing (at most 32 fields per call; enqueued on the
+    current torch stream, or `stream`, without synchronisation).  Pass `out` to keep the call itself allocation-free."""
+    import torch
+    if not isinstance(fields, torch.Tensor) or fields.device != h.device or fields.dtype != torch.float64 or \
+            not fields.is_contiguous() or fields.dim() != 2 or fields.shape[1] != h.n_vert:
+        raise ValueError(f"fields must be a contiguous float64 tensor [F][{h.n_vert}] on {h.device}")
+    if out is None:
+        out = torch.empty(fields.shape[0], dtype=torch.float64, device=h.device)
+    st = torch.cuda.current_stream(h.device) if stream is None else stream
+    rc = load_library().if_energy_noalloc(h._ptr, C.c_void_p(fields.data_ptr()), int(fields.shape[0]),
+                                          C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream))
+    if rc != IF_OK:
+        raise ImplicitFilterError(rc, "if_energy_noalloc")
+    return out
 
 
 def if_apply(h: Handle, fields, ells: Sequence[float], order_n: int, out=None, workspace=None, stream=None,

@@ -12,7 +12,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
-SRC = [os.path.join(HERE, "csrc", f) for f in ("prepare.cu", "solve.cu", "mg.cu")]
+SRC = [os.path.join(HERE, "csrc", f) for f in ("prepare.cu", "solve.cu", "mg.cu", "noalloc.cu")]
 DEPS = ([os.path.join(HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(HERE, "csrc")))]
         + [os.path.join(ROOT, "include", "implicit_filter.h")])
 LIB = os.path.join(HERE, "libimplicit_filter.so")

@@ -62,6 +62,7 @@ int resolve_options(const if_options* in, const Options* base, Options* out);
 struct if_mesh_s;
 namespace ifl {
 int mg_build(if_mesh_s* h);    // mg.cu: builds h->mg from the SELL matrix and the areas
+int na_setup(if_mesh_s* h);    // noalloc.cu: looks up the device address of its static scratch array (once per handle)
 void mg_free(if_mesh_s* h);
 
 // ---- multigrid hierarchy (optional, IF_FLAG_MULTIGRID): smoothed aggregation on the internal row order.
@@ -163,6 +164,7 @@ struct if_mesh_s {
     ifl::MgLevel mg[ifl::MG_MAX_LEVELS];
     int mg_levels = 0;              // 0: no hierarchy
     double mg_build_seconds = 0.0;  // wall clock of mg_build
+    void* na_scratch = nullptr;     // device address of the static scratch array of if_energy_noalloc (noalloc.cu)
     // pinned host staging for per-call control data and read-back
     void* h_pinned = nullptr;
     size_t h_pinned_bytes = 0;

@@ -890,6 +890,7 @@ extern "C" int if_prepare(const double* coords, int dim, int64_t n_vert, const i
     if_mesh_s* h = new (std::nothrow) if_mesh_s();
     if (!h) return IF_ENOMEM;
     rc = prepare_impl(coords, dim, n_vert, tri, n_tri, period, o, h);
+    if (rc == IF_OK) rc = ifl::na_setup(h);
     if (rc != IF_OK) {
         if_destroy(h);
         return rc;
@@ -1146,6 +1147,7 @@ extern "C" int if_load(const char* path, if_handle* out) {
         if_destroy(h);
         return IF_ENOMEM;
     }
+    if (ifl::na_setup(h) != IF_OK) { if_destroy(h); return IF_ECUDA; }
     *out = h;
     return IF_OK;
 }
@@ -1161,6 +1163,7 @@ extern "C" const char* if_strerror(int code) {
         case IF_ENOMEM: return "out of memory";
         case IF_ECUDA: return "CUDA error or no device";
         case IF_EWORKSPACE: return "workspace too small";
+        case IF_ELIMIT: return "more fields than the static scratch array of if_energy_noalloc serves per call (32)";
         case IF_EIO: return "file cannot be written or read, or is not a prepared mesh of this library build";
         default: return "unknown error";
     }
