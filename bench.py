@@ -55,7 +55,7 @@ def parse_args():
     ap.add_argument("--cpu-sample-iters", type=int, default=60)
     ap.add_argument("--solver", default="jacobi", choices=["jacobi", "multigrid"],
                     help="preconditioner of the timed headline run (the metric is quoted on jacobi)")
-    ap.add_argument("--mg-min-ell", type=float, default=0.0, help="0 = library default (4 mean edge lengths)")
+    ap.add_argument("--mg-min-ell", type=float, default=0.0, help="0 = library default (0.5 mean edge lengths)")
     ap.add_argument("--no-multigrid", action="store_true", help="skip the extra multigrid-preconditioned leg")
     ap.add_argument("--budget-seconds", type=float, default=150.0,
                     help="a timed leg stops adding steps once it has run this long (at least one step; the line "
@@ -445,7 +445,7 @@ def run_ours(args):
               "rhs_iterations_per_step": sum(r["stats"]["rhs_iters"] for r in res_m) / n_m,
               "batch_iterations_per_step": sum(r["stats"]["batch_iters"] for r in res_m) / n_m,
               "multigrid_batch_iterations_per_step": sum(r["stats"]["mg_batch_iters"] for r in res_m) / n_m,
-              "mg_min_ell_in_mean_edges": args.mg_min_ell or (4.0 if w.order_n == 1 else 0.5),
+              "mg_min_ell_in_mean_edges": args.mg_min_ell or 0.5,
               "gpu_launches": int(launches_m),
               "solver_codes": sorted({r["stats"]["code"] for r in res_m}),
               "max_rel_energy_diff_vs_jacobi": float(np.max(np.abs(e_m - e_j) / np.abs(e_j))),

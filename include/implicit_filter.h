@@ -103,7 +103,7 @@ typedef struct {
                         start vector, same stop test, same answers within the tolerance (PAPER.md:207 names the
                         convergence of plain CG at large scales, above all for n = 2, as the open problem)           */
     double radius;     /* if_prepare with IF_FLAG_VECTOR: R_e of the metric terms; 0 => the mean |x_v| of a dim = 3 mesh    */
-    double mg_min_ell; /* 0 => 4 for n = 1, 0.5 for n = 2 (in mean edge lengths; below that Jacobi-PCG is cheaper)     */
+    double mg_min_ell; /* 0 => 0.5 (in mean edge lengths; right-hand sides below that stay on the Jacobi path)         */
 } if_options;
 
 typedef struct {

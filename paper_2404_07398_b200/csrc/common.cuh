@@ -54,7 +54,7 @@ struct Options {
     int flags = 0;
     int solver = 0;
     double radius = 0.0;        // R_e of the vector filter's metric terms; 0: mean |x_v| (dim = 3)
-    double mg_min_ell = 0.0;    // 0: the default of the order (mg_solve.cuh: 4 mean edges for n = 1, 0.5 for n = 2)
+    double mg_min_ell = 0.0;    // 0: the default of the order (mg_solve.cuh: 0.5 mean edges)
 };
 
 int resolve_options(const if_options* in, const Options* base, Options* out);

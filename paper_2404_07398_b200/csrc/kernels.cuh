@@ -69,8 +69,8 @@ struct Ctrl {
     int status[KMAX];
     int iters[KMAX];
     double c1[KMAX];      // multigrid path: coefficient of the cycle's operator K = M + c1 S (n = 1: c; n = 2: sqrt(c))
-    int starting[KMAX];   // multigrid path: the column was (re)started; its first iteration only applies the
-                          // preconditioner (alpha = 0, then rho = r.z, beta = 0), see k_init
+    int starting[KMAX];   // multigrid path: the column was (re)started (k_mg_start): its first iteration has alpha = 1
+                          // (forms r0), then rho = r0.z0, beta = 0, nothing counted
     int cur_r;            // multigrid path: which residual buffer holds r (flipped with cur_p)
     int pair_mode;        // vector filter: columns (2i, 2i+1) are the (u, v) of ONE system: its dot products are the
                           // sums over both columns, so both share alpha, beta and the stop decision
@@ -214,7 +214,7 @@ __device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __
 
 // CG bookkeeping after z = B r (run by the last block of a grid reduction; tot = rho' per column, then ||r||^2):
 // beta = rho'/rho, stop test, iteration count -- the same rules as the tail of k_update.  A column that was
-// (re)started (Ctrl::starting) has only had its preconditioner applied: rho = rho', beta = 0, nothing counted.
+// (re)started (Ctrl::starting, k_mg_start) has just had r0 and z0 = B r0 formed: rho = rho', beta = 0, nothing counted.
 template <int K>
 __device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const double* tot) {
     __shared__ int any_active;
@@ -800,8 +800,9 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
             if (tid < K) {
                 const double pq = ctrl->pair_mode ? tot[tid & ~1] + tot[tid | 1] : tot[tid];
                 double al = 0.0;
-                if (!ctrl->done[tid] && !ctrl->starting[tid]) {   // (a starting column has no direction yet)
-                    if (pq > 0.0 && isfinite(pq)) al = ctrl->rho[tid] / pq;
+                if (!ctrl->done[tid]) {
+                    if (ctrl->starting[tid]) al = 1.0;     // p' = phi, q = A phi: the next kernel forms r0 = M phi - A phi
+                    else if (pq > 0.0 && isfinite(pq)) al = ctrl->rho[tid] / pq;
                     else { ctrl->done[tid] = 1; ctrl->status[tid] = 2; }
                 }
                 ctrl->alpha[tid] = al;
@@ -836,11 +837,8 @@ template <int K>
 __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
                                                 StartParams sp, unsigned mask, const double* __restrict__ x,
                                                 const double* __restrict__ y, double* __restrict__ z_,
-                                                double* __restrict__ p0, double* __restrict__ p1, int order_n,
-                                                double* __restrict__ r_alt, double* __restrict__ z_clear, int mg) {
-    // multigrid path (mg): the iteration is carried in r, double-buffered: r0 goes to the buffer ctrl->cur_r names,
-    // and the column is marked `starting` (its first iteration applies the preconditioner only)
-    double* __restrict__ z = (mg && ctrl->cur_r) ? r_alt : z_;
+                                                double* __restrict__ p0, double* __restrict__ p1, int order_n) {
+    double* __restrict__ z = z_;
     constexpr int TPR = K / 2;
     constexpr int ROWS = BLOCK / TPR;
     const int tid = threadIdx.x, l = tid % TPR;
@@ -858,22 +856,16 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
             const double2 r = {-cc.x * yv.x, -cc.y * yv.y};
             const double2 b = {av * xv.x, av * xv.y};
             if (on0) {
-                zv.x = mg ? r.x : r.x / d.x; pa.x = 0.0; pb.x = 0.0;
+                zv.x = r.x / d.x; pa.x = 0.0; pb.x = 0.0;
                 acc[0].x = fma(r.x, zv.x, acc[0].x); acc[1].x = fma(r.x, r.x, acc[1].x); acc[2].x = fma(b.x, b.x, acc[2].x);
             }
             if (on1) {
-                zv.y = mg ? r.y : r.y / d.y; pa.y = 0.0; pb.y = 0.0;
+                zv.y = r.y / d.y; pa.y = 0.0; pb.y = 0.0;
                 acc[0].y = fma(r.y, zv.y, acc[0].y); acc[1].y = fma(r.y, r.y, acc[1].y); acc[2].y = fma(b.y, b.y, acc[2].y);
             }
             st2(z, ri, zv);
             st2(p0, ri, pa);
             st2(p1, ri, pb);
-            if (z_clear) {   // (multigrid path) the preconditioned residual of a starting column: finite before its first use
-                double2 zc = ld2(z_clear, ri);
-                if (on0) zc.x = 0.0;
-                if (on1) zc.y = 0.0;
-                st2(z_clear, ri, zc);
-            }
         }
     }
     __shared__ double tot[3 * KMAX];
@@ -884,7 +876,7 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
             const double rho = w2 * (tot[ta] + tot[tb]), rr = w2 * (tot[KMAX + ta] + tot[KMAX + tb]),
                          bb = w2 * (tot[2 * KMAX + ta] + tot[2 * KMAX + tb]);
             ctrl->c[tid] = sp.c[tid]; ctrl->c1[tid] = sp.c1[tid]; ctrl->field[tid] = sp.field[tid]; ctrl->rhs[tid] = sp.rhs[tid];
-            ctrl->starting[tid] = mg;
+            ctrl->starting[tid] = 0;
             ctrl->rho[tid] = rho; ctrl->rr[tid] = rr; ctrl->bb[tid] = bb;
             ctrl->alpha[tid] = 0.0; ctrl->beta[tid] = 0.0; ctrl->iters[tid] = 0;
             int st = 0;
@@ -893,6 +885,68 @@ __global__ void __launch_bounds__(BLOCK) k_init(MeshView m, Ctrl* __restrict__ c
             ctrl->status[tid] = st;
             ctrl->epoch[tid] = ctrl->epoch[tid] + 1;
             ctrl->done[tid] = dn;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int any = 0;
+            for (int c = 0; c < K; ++c) any |= !ctrl->done[c];
+            ctrl->all_done = !any;
+        }
+    }
+}
+
+// Start of multigrid-preconditioned CG for the columns in `mask` (mg_solve.cuh), from x0 = phi without a
+// pass of its own over the matrix: the column joins the stream with
+//     x = 0 ,  z = phi ,  p = 0 ,  r = M phi ,  beta = 0 ,  starting = 1,
+// and its first iteration -- the same launch sequence as every other -- does the rest: kernel A forms p' = z = phi and
+// q = A phi and sets alpha = 1 for a starting column, the fused residual kernel forms r0 = r - alpha q = M phi - A phi,
+// the cycle gives z0 = B r0, the bookkeeping sets rho = r0.z0, beta = 0 and counts nothing; the next kernel A applies
+// the pending x += alpha p' = phi.  (Jacobi path: k_init, with r0 = -c S (M^-1 S)^(n-1) phi from a plain SpMM.)
+// fields are gathered through the permutation; r goes to the residual buffer in use (Ctrl::cur_r).
+template <int K>
+__global__ void __launch_bounds__(BLOCK) k_mg_start(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+                                                    StartParams sp, unsigned mask, const double* __restrict__ fields,
+                                                    double* __restrict__ x, double* __restrict__ z,
+                                                    double* __restrict__ r0, double* __restrict__ r1,
+                                                    double* __restrict__ p0, double* __restrict__ p1) {
+    constexpr int TPR = K / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    const int tid = threadIdx.x, l = tid % TPR;
+    const bool on0 = (mask >> (2 * l)) & 1u, on1 = (mask >> (2 * l + 1)) & 1u;
+    const int f0 = sp.field[2 * l], f1 = sp.field[2 * l + 1];
+    double* __restrict__ r = ctrl->cur_r ? r1 : r0;
+    double2 acc[1] = {{0.0, 0.0}};
+    if (on0 || on1) {
+        for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < m.nv; row += (int64_t)gridDim.x * ROWS) {
+            const int64_t ri = row * K + 2 * l;
+            const double av = m.area[row];
+            const int64_t u = m.perm[row];
+            double2 xv = ld2(x, ri), zv = ld2(z, ri), rv = ld2(r, ri), pa = ld2(p0, ri), pb = ld2(p1, ri);
+            if (on0) {
+                const double phi = f0 >= 0 ? fields[(int64_t)f0 * m.nv + u] : 0.0;
+                xv.x = 0.0; zv.x = phi; rv.x = av * phi; pa.x = 0.0; pb.x = 0.0;
+                acc[0].x = fma(rv.x, rv.x, acc[0].x);
+            }
+            if (on1) {
+                const double phi = f1 >= 0 ? fields[(int64_t)f1 * m.nv + u] : 0.0;
+                xv.y = 0.0; zv.y = phi; rv.y = av * phi; pa.y = 0.0; pb.y = 0.0;
+                acc[0].y = fma(rv.y, rv.y, acc[0].y);
+            }
+            st2(x, ri, xv); st2(z, ri, zv); st2(r, ri, rv); st2(p0, ri, pa); st2(p1, ri, pb);
+        }
+    }
+    __shared__ double tot[KMAX];
+    if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[1], tot)) {
+        if (tid < K && ((mask >> tid) & 1u)) {
+            const int ta = ctrl->pair_mode ? (tid & ~1) : tid, tb = ctrl->pair_mode ? (tid | 1) : tid;
+            const double bb = (ctrl->pair_mode ? 1.0 : 0.5) * (tot[ta] + tot[tb]);
+            ctrl->c[tid] = sp.c[tid]; ctrl->c1[tid] = sp.c1[tid]; ctrl->field[tid] = sp.field[tid]; ctrl->rhs[tid] = sp.rhs[tid];
+            ctrl->rho[tid] = 0.0; ctrl->rr[tid] = bb; ctrl->bb[tid] = bb;
+            ctrl->alpha[tid] = 0.0; ctrl->beta[tid] = 0.0; ctrl->iters[tid] = 0;
+            ctrl->status[tid] = isfinite(bb) ? 0 : 2;
+            ctrl->epoch[tid] = ctrl->epoch[tid] + 1;
+            ctrl->done[tid] = (sp.field[tid] < 0 || !isfinite(bb)) ? 1 : 0;
+            ctrl->starting[tid] = ctrl->done[tid] ? 0 : 1;
         }
         __syncthreads();
         if (tid == 0) {

@@ -17,9 +17,10 @@
 //       k_spmm<16, AX> sub 3 z = last sweep ; rho' = r'.z ; ||r'||^2 ; beta ; stop test      (CG bookkeeping)
 //   n = 2: the last sweep of the first cycle is sub 5 (y = V r', w = M y, rho' = y.w, bookkeeping), then a second
 //   cycle on w (k_spmm<16, MGR0>, transfers, coarse levels, sub 2) gives z = V w.
-// A (re)started column (Ctrl::starting, set by k_init) joins at an iteration boundary: its first iteration has alpha = 0
-// and ends with rho = r0.z0, beta = 0 -- the start of PCG -- so columns are refilled from the queue as in the Jacobi
-// path and the host never waits inside the loop.
+// A (re)started column (Ctrl::starting, set by k_mg_start) joins at an iteration boundary with x = 0, z = phi, r = M phi:
+// its first iteration has alpha = 1, which makes kernel A and the fused residual kernel form r0 = M phi - A phi on the
+// way (no pass of its own over the matrix), and ends with rho = r0.z0, beta = 0 -- the start of PCG from x0 = phi -- so
+// columns are refilled from the queue as in the Jacobi path and the host never waits inside the loop.
 // The stop test is the same as in the Jacobi path: recursive ||r||_2 <= tol ||M phi||_2.
 #pragma once
 
@@ -29,7 +30,7 @@ namespace {
 constexpr int MGK = 16;               // columns of the multigrid path
 constexpr int MG_REFILL_MIN = 1;      // stopped columns are restarted as soon as this many are free (solve.cu)
 // right-hand sides below this many mean edge lengths stay on the Jacobi path (option mg_min_ell = 0)
-constexpr double MG_MIN_ELL_N1 = 4.0;
+constexpr double MG_MIN_ELL_N1 = 0.5;
 constexpr double MG_MIN_ELL_N2 = 0.5;
 // n = 2: sweeps per side of the cycle on the mesh and on level 1 (Chebyshev-root dampings, mg_omegas)
 constexpr int MG_NU0_N2 = 4;

@@ -232,6 +232,16 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
     const if_mesh_s* h = r.h;
     const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
     int rc;
+    if (r.mg) {   // multigrid path: the column joins the stream, its first iteration forms r0 (k_mg_start)
+        if constexpr (K == KMAX) {
+            const MgBuffers b = mg_layout(h, r.w, r.order_n);
+            k_mg_start<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, d_fields, b.x, b.zb, b.r[0],
+                                                          b.r[1], b.p[0], b.p[1]);
+            IF_LAUNCH_CHECK();
+            return IF_OK;
+        }
+        return IF_EINVAL;
+    }
     k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, sp, mask, d_fields, r.w.x);
     IF_LAUNCH_CHECK();
     if (r.order_n == 1) {
@@ -245,16 +255,8 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
         SpmmArgs b{t, nullptr, nullptr, r.w.q, nullptr, 0, 0};
         if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, b))) return rc;
     }
-    // multigrid phase: r0 into the residual buffer in use (w.z or its twin), z cleared, the column marked `starting`
-    double* r_alt = nullptr;
-    double* z_clear = nullptr;
-    if (r.mg) {
-        const MgBuffers b = mg_layout(h, r.w, r.order_n);
-        r_alt = b.r[1];
-        z_clear = b.zb;
-    }
     k_init<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, r.w.x, r.w.q, r.w.z, r.w.p0,
-                                              r.w.p1, r.order_n, r_alt, z_clear, r.mg ? 1 : 0);
+                                              r.w.p1, r.order_n);
     IF_LAUNCH_CHECK();
     return IF_OK;
 }
