@@ -23,10 +23,11 @@
  *     passes (inputs, outputs, workspace); the handle owns the device arrays it built and if_destroy frees
  *     them.  The library keeps no caller pointer past return and never frees or resizes caller memory.
  *   - Inputs and outputs use the CALLER's vertex numbering; the internal reordering is invisible.
- *   - Work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).  Calls that
- *     return host outputs (if_spectrum, or any call given a non-NULL if_stats) synchronise that stream
- *     before returning; if_filter/if_apply with stats == NULL return after the last poll of the
- *     convergence flag (the output is complete in stream order).
+ *   - Work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).  The solving calls
+ *     (if_filter, if_spectrum, if_spectrum_host, if_apply) are synchronous: they poll the convergence flags while the
+ *     iteration runs and wait for the stream before returning, on success and on every error path; outputs are
+ *     complete on return.  if_energy_noalloc only enqueues.  The handle's device is made current for the duration of
+ *     a solving call and the caller's current device is restored before it returns.
  *   - Return value: 0 on success; negative IF_E* on error (outputs untouched, nothing thrown);
  *     positive IF_WNOTCONVERGED when some right-hand side hit max_iter or broke down -- an expected outcome
  *     for n = 2 at large l; outputs then hold the last iterate and if_stats says which.

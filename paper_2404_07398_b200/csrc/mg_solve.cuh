@@ -28,6 +28,7 @@ namespace ifl {
 namespace {
 
 constexpr int MGK = 16;               // columns of the multigrid path
+constexpr size_t MG_FACTOR_SMEM = 2 * (size_t)MG_COARSEST * (MG_COARSEST + 1) * sizeof(double);   // k_mg_coarse_factor
 constexpr int MG_REFILL_MIN = 1;      // stopped columns are restarted as soon as this many are free (solve.cu)
 // right-hand sides below this many mean edge lengths stay on the Jacobi path (option mg_min_ell = 0)
 constexpr double MG_MIN_ELL_N1 = 0.5;
@@ -222,17 +223,22 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_prolong0(const int64_t
     }
 }
 
-// coarsest level: dense Cholesky of A = M + c S per column (one block per column), then the two triangular solves
-__global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ r, double* __restrict__ e) {
-    __shared__ double a[MG_COARSEST][MG_COARSEST + 1];
-    __shared__ double v[MG_COARSEST];
+// Coarsest level (n <= MG_COARSEST unknowns).  K = M + c1 S depends on the column only through c1, which changes when
+// the column is (re)started -- not from cycle to cycle -- so its inverse is formed once per column start
+// (k_mg_coarse_factor: dense Cholesky K = L L^T in shared memory, L^-1 by forward substitution on the unit vectors,
+// K^-1 = L^-T L^-1, symmetric by construction; one block per column) and a cycle only multiplies by it.  Round 1
+// factorised in every cycle: 118 us of the 385 us the levels >= 2 took per cycle on config 4.
+// inv: [MGK][MG_COARSEST][MG_COARSEST] in the workspace.
+__global__ void __launch_bounds__(64) k_mg_coarse_factor(MgMat g, const Ctrl* __restrict__ ctrl, unsigned mask,
+                                                         double* __restrict__ inv) {
+    extern __shared__ double coarse_sm[];            // two [MG_COARSEST][MG_COARSEST + 1] arrays (65 KB: opt-in)
+    double (*a)[MG_COARSEST + 1] = reinterpret_cast<double (*)[MG_COARSEST + 1]>(coarse_sm);
+    double (*li)[MG_COARSEST + 1] = reinterpret_cast<double (*)[MG_COARSEST + 1]>(coarse_sm + MG_COARSEST * (MG_COARSEST + 1));
     const int c = blockIdx.x, t = threadIdx.x, n = (int)g.n;
-    if (ctrl->all_done) return;
+    if (!((mask >> c) & 1u)) return;
     const double cc = ctrl->c1[c];
-    for (int i = t; i < n; i += 64) {
-        for (int j = 0; j < n; ++j) a[i][j] = 0.0;
-        v[i] = r[(int64_t)i * MGK + c];
-    }
+    for (int i = t; i < n; i += 64)
+        for (int j = 0; j < n; ++j) { a[i][j] = 0.0; li[i][j] = 0.0; }
     __syncthreads();
     for (int i = t; i < n; i += 64)
         for (int64_t k = g.rowptr[i]; k < g.rowptr[i + 1]; ++k) a[i][g.col[k]] += fma(cc, g.sm[k].x, g.sm[k].y);
@@ -246,26 +252,45 @@ __global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, const Ctrl* __restric
             for (int j = k + 1; j <= i; ++j) a[i][j] -= a[i][k] * a[j][k];
         __syncthreads();
     }
-    if (t == 0) {                                 // L y = v ; L^T x = y  (n <= 64: one thread is enough)
-        for (int i = 0; i < n; ++i) {
-            double s = v[i];
-            for (int j = 0; j < i; ++j) s -= a[i][j] * v[j];
-            v[i] = s / a[i][i];
+    // column j of L^-1 (thread j): L y = e_j by forward substitution; y_i = 0 for i < j
+    for (int j = t; j < n; j += 64)
+        for (int i = j; i < n; ++i) {
+            double s = i == j ? 1.0 : 0.0;
+            for (int k = j; k < i; ++k) s -= a[i][k] * li[k][j];
+            li[i][j] = s / a[i][i];
         }
-        for (int i = n - 1; i >= 0; --i) {
-            double s = v[i];
-            for (int j = i + 1; j < n; ++j) s -= a[j][i] * v[j];
-            v[i] = s / a[i][i];
-        }
-    }
     __syncthreads();
-    for (int i = t; i < n; i += 64) e[(int64_t)i * MGK + c] = v[i];
+    // K^-1 = L^-T L^-1: entry (i, j) = sum_k li[k][i] li[k][j], k >= max(i, j); thread i fills row i
+    double* out = inv + (size_t)c * MG_COARSEST * MG_COARSEST;
+    for (int i = t; i < n; i += 64)
+        for (int j = 0; j < n; ++j) {
+            double s = 0.0;
+            for (int k = (i > j ? i : j); k < n; ++k) s = fma(li[k][i], li[k][j], s);
+            out[i * MG_COARSEST + j] = s;
+        }
+}
+
+// e = K^-1 r on the coarsest level, one block per column
+__global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ inv,
+                                                  const double* __restrict__ r, double* __restrict__ e) {
+    __shared__ double v[MG_COARSEST];
+    const int c = blockIdx.x, t = threadIdx.x, n = (int)g.n;
+    if (ctrl->all_done) return;
+    for (int i = t; i < n; i += 64) v[i] = r[(int64_t)i * MGK + c];
+    __syncthreads();
+    const double* a = inv + (size_t)c * MG_COARSEST * MG_COARSEST;
+    for (int i = t; i < n; i += 64) {
+        double s = 0.0;
+        for (int j = 0; j < n; ++j) s = fma(a[i * MG_COARSEST + j], v[j], s);
+        e[(int64_t)i * MGK + c] = s;
+    }
 }
 
 // ------------------------------------------------------------------------------------------- host side
 struct MgBuffers {
     double *x, *r[2], *p[2], *q, *za, *zb, *t;  // level 0, [n][16]; r is double-buffered (k_spmm<16, MGR>)
     double* lev[MG_MAX_LEVELS][4];              // levels >= 1: R, E, T, E2
+    double* coarse_inv;                         // [MGK][MG_COARSEST][MG_COARSEST]: K^-1 of the coarsest level per column
 };
 
 // level-0 vectors beyond the Jacobi workspace: za (e), zb (z), the second r; for n = 1 also t (the n = 2 workspace has one)
@@ -273,6 +298,7 @@ inline size_t mg_extra_bytes(const if_mesh_s* h, int order_n) {
     if (h->mg_levels < 2) return 0;
     size_t b = (order_n == 1 ? 4 : 3) * align_up((size_t)h->n_vert * MGK * sizeof(double));
     for (int l = 1; l < h->mg_levels; ++l) b += 4 * align_up((size_t)h->mg[l].n * MGK * sizeof(double));
+    b += align_up((size_t)MGK * MG_COARSEST * MG_COARSEST * sizeof(double));
     return b;
 }
 
@@ -288,6 +314,7 @@ inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, int order_n) 
     m.t = order_n == 1 ? (double*)take((size_t)h->n_vert * MGK * sizeof(double)) : w.t;
     for (int l = 1; l < h->mg_levels; ++l)
         for (int k = 0; k < 4; ++k) m.lev[l][k] = (double*)take((size_t)h->mg[l].n * MGK * sizeof(double));
+    m.coarse_inv = (double*)take((size_t)MGK * MG_COARSEST * MG_COARSEST * sizeof(double));
     return m;
 }
 
@@ -304,6 +331,7 @@ enum { MGT_A = 0, MGT_MGR = 1, MGT_RESTRICT0 = 2, MGT_LEVEL1 = 3, MGT_COARSE = 4
 
 int mg_setup(Run& r) {
     const if_mesh_s* h = r.h;
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_coarse_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MG_FACTOR_SMEM));
     const int64_t tiles = (h->n_vert + TILE_ROWS - 1) / TILE_ROWS;
     int rc;
     if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
@@ -338,7 +366,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
     const bool last = l == h->mg_levels - 1;
     int rc;
     if (last && g.n <= MG_COARSEST) {
-        k_mg_coarse<<<MGK, 64, 0, r.st>>>(gm, ctrl, R, E);
+        k_mg_coarse<<<MGK, 64, 0, r.st>>>(gm, ctrl, b.coarse_inv, R, E);
         IF_LAUNCH_CHECK();
         if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
         *result = E;

@@ -238,6 +238,11 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
             k_mg_start<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, d_fields, b.x, b.zb, b.r[0],
                                                           b.r[1], b.p[0], b.p[1]);
             IF_LAUNCH_CHECK();
+            const MgLevel& gl = h->mg[h->mg_levels - 1];      // K^-1 of the coarsest level for the new columns' c1
+            if (gl.n <= MG_COARSEST) {
+                k_mg_coarse_factor<<<MGK, 64, MG_FACTOR_SMEM, r.st>>>(mg_mat(gl), r.w.ctrl, mask, b.coarse_inv);
+                IF_LAUNCH_CHECK();
+            }
             return IF_OK;
         }
         return IF_EINVAL;
@@ -576,9 +581,27 @@ int pick_k(int batch, size_t R) {
     return K;
 }
 
+int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
+                      double* d_out, double* energy, double* k_mid, double* E, void* d_ws, size_t ws_bytes, void* stream,
+                      const if_options* opt_in, if_stats* stats);
+
+// The handle's device is made current for the call and the caller's device restored afterwards, whatever the outcome.
 int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
             double* d_out, double* energy, double* k_mid, double* E, void* d_ws, size_t ws_bytes, void* stream,
             const if_options* opt_in, if_stats* stats) {
+    if (!h) return IF_EINVAL;
+    int prev = -1;
+    if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return IF_ECUDA; }
+    if (prev != h->device) IF_CUDA_TRY(cudaSetDevice(h->device));
+    const int rc = run_job_on_device(h, job, d_fields, n_fields, ells, n_ells, order_n, d_out, energy, k_mid, E, d_ws, ws_bytes,
+                                     stream, opt_in, stats);
+    if (prev != h->device) cudaSetDevice(prev);
+    return rc;
+}
+
+int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields, const double* ells, int n_ells, int order_n,
+                      double* d_out, double* energy, double* k_mid, double* E, void* d_ws, size_t ws_bytes, void* stream,
+                      const if_options* opt_in, if_stats* stats) {
     if (!h || !d_fields || !ells || n_fields < 1 || n_ells < 1 || order_n < 1 || order_n > 4 || !d_ws)
         return IF_EINVAL;
     if (job != JOB_SPECTRUM && !d_out) return IF_EINVAL;
@@ -600,9 +623,6 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
     if (r.vec && (n_fields % 2 != 0 || order_n > 2 || !h->sell_dval)) return IF_EINVAL;
     const bool pairs = job == JOB_SPECTRUM && (r.opt.flags & IF_FLAG_PAIRS);
     const int n_out_fields = pairs ? n_fields / 2 : n_fields;
-    int dev = -1;
-    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return IF_ECUDA; }
-    if (dev != h->device) IF_CUDA_TRY(cudaSetDevice(h->device));
     r.w = layout_workspace(h, order_n, r.opt.batch, d_ws);
     if (ws_bytes < r.w.bytes) return IF_EWORKSPACE;
     int log2c = 0;
@@ -622,10 +642,16 @@ int run_job(if_handle h, Job job, const double* d_fields, int n_fields, const do
         poll.own_pinned = true;
     }
     for (auto& e : poll.ev) IF_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-    cudaEvent_t t0 = nullptr, t1 = nullptr;
-    IF_CUDA_TRY(cudaEventCreate(&t0));
-    IF_CUDA_TRY(cudaEventCreate(&t1));
-    struct EvGuard { cudaEvent_t a, b; ~EvGuard() { cudaEventDestroy(a); cudaEventDestroy(b); } } evg{t0, t1};
+    struct EvGuard {
+        cudaEvent_t a = nullptr, b = nullptr;
+        ~EvGuard() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+    } evg;
+    IF_CUDA_TRY(cudaEventCreate(&evg.a));
+    IF_CUDA_TRY(cudaEventCreate(&evg.b));
+    const cudaEvent_t t0 = evg.a, t1 = evg.b;
+    // every way out of this function -- error returns included -- waits for what it has enqueued before the pinned
+    // snapshot buffer, the events and this stack frame go away (declared last: runs first)
+    struct SyncGuard { cudaStream_t s; ~SyncGuard() { cudaStreamSynchronize(s); } } sync_guard{r.st};
     IF_CUDA_TRY(cudaEventRecord(t0, r.st));
 
     // queue of right-hand sides: largest scale (most iterations) first, so that the short solves fill the tail
