@@ -328,10 +328,15 @@ constexpr int SPMM_STAGES = IF_SPMM_STAGES;
 // fit shared memory).  The multigrid sweeps (AX, MGR0) move fewer bytes per tile than kernel A and were bound the
 // same way as one CTA (0.57 of the copy bandwidth): their second vector -- needed for the tile's own rows only,
 // never gathered -- goes through registers instead of a shared-memory region (REGB), the stage shrinks to 46 KB, and
-// they run as two 256-thread CTAs per SM with two stages each (0.909 -> 0.849 ms per sweep on config 4).  MGR, which
-// also reads q and stores r', lost by the same change (1.11 -> 1.41 ms: 128 registers with spills) and stays as it was.
+// they run as two 256-thread CTAs per SM with two stages each (0.909 -> 0.776 ms per sweep on config 4).  MGR, which
+// also reads q and stores r', lost by the same change in both forms tried (below) and stays as it was.
+// MGR the same way (q by direct loads, r' stored from registers and read back by its thread): measured on config 4,
+// 1.075 -> 1.235 ms (128 registers with spills at 256 threads x 2 CTAs) -- off.
+#ifndef IF_MGR_REGB
+#define IF_MGR_REGB 0
+#endif
 template <int K, int MODE> struct SpmmCfg {
-    static constexpr bool REGB = (MODE == MODE_AX || MODE == MODE_MGR0);
+    static constexpr bool REGB = (MODE == MODE_AX || MODE == MODE_MGR0 || (MODE == MODE_MGR && IF_MGR_REGB));
     static constexpr bool WIDE1 = (K == 16) && !REGB;              // one 512-thread CTA per SM
     static constexpr int NT = WIDE1 ? SPMM_BLOCK : 256;
     static constexpr int MINB = WIDE1 ? IF_SPMM_MINB : 2;
@@ -443,7 +448,7 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
         mbar_expect_tx(bar, vbytes * SM::NLOAD + 2u * dbytes + (staged ? (uint32_t)ti.slots * (VEC ? 20u : 12u) : 0u));
         bulk_load(st, a.in0 + row0 * K, vbytes, bar);
         if (SM::NLOAD >= 2) bulk_load(st + SM::off_b, a.in1 + row0 * K, vbytes, bar);
-        if (REGB && MODE == MODE_AX && a.in1) bulk_prefetch_l2(a.in1 + row0 * K, vbytes);
+        if (REGB && (MODE == MODE_AX || MODE == MODE_MGR) && a.in1) bulk_prefetch_l2(a.in1 + row0 * K, vbytes);
         bulk_load(st + SM::off_dg, m.sdiag + row0, dbytes, bar);
         bulk_load(st + SM::off_ar, rowfac + row0, dbytes, bar);
         if (staged) {
@@ -530,7 +535,16 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
         double2* sb = reinterpret_cast<double2*>(st + SM::off_b);
         const double* sdg = reinterpret_cast<const double*>(st + SM::off_dg);
         const double* sar = reinterpret_cast<const double*>(st + SM::off_ar);
-        const int nrows = (int)min((int64_t)T, m.nv - tile * T);
+        const int64_t row0 = tile * T;
+        const int nrows = (int)min((int64_t)T, m.nv - row0);
+        double2 qg[XPT];
+        if (MGQ && REGB) {      // q of the tile's own rows straight from global memory (L2: prefetched with the tile)
+#pragma unroll
+            for (int i = 0; i < XPT; ++i) {
+                const int e = tid + i * NT;
+                if (e < nrows * TPR) qg[i] = ld2(a.in1, row0 * K + 2 * (int64_t)e);
+            }
+        }
 #pragma unroll
         for (int i = 0; i < XPT; ++i) {
             const int e = tid + i * NT;
@@ -540,9 +554,11 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
                 const double sd = sdg[rr], av = sar[rr];
                 double2 rn = rv;
                 if (MGQ) {
-                    const double2 qv = sb[e];
+                    const double2 qv = REGB ? qg[i] : sb[e];
                     rn.x = fma(-alpha.x, qv.x, rv.x);
                     rn.y = fma(-alpha.y, qv.y, rv.y);
+                    // (REGB: r' goes out from registers; the same thread reads it back in the tile's epilogue)
+                    if (REGB) st2(a.x, row0 * K + 2 * (int64_t)e, rn);
                 }
                 if (!REGB) sb[e] = rn;
                 sa[e] = make_double2(a.omega * rn.x * rcp_pos(fma(cc.x, sd, av)), a.omega * rn.y * rcp_pos(fma(cc.y, sd, av)));
@@ -635,8 +651,12 @@ __global__ void __launch_bounds__(SpmmCfg<K, MODE>::NT, SpmmCfg<K, MODE>::MINB) 
             // (thread 0 prefetched the tile into L2 when it issued the tile's bulk copies)
             double2 rv_g = {0.0, 0.0};
             if (REGB) {
-                const double* __restrict__ src = (MODE == MODE_MGR0) ? a.in0 : a.in1;
-                if (src) rv_g = ld2(src, row * K + 2 * l);
+                if (MODE == MODE_MGR) {     // r', written by this very thread when it prepared the tile: a coherent (L2) load
+                    rv_g = __ldcg(reinterpret_cast<const double2*>(a.x + row * K + 2 * l));
+                } else {
+                    const double* __restrict__ src = (MODE == MODE_MGR0) ? a.in0 : a.in1;
+                    if (src) rv_g = ld2(src, row * K + 2 * l);
+                }
             }
             const int chl = r >> m.log2c;
             const int cpr = scp[chl];
