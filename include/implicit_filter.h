@@ -78,6 +78,10 @@ enum {
                              Jacobi-preconditioned CG with one residual norm over both components.  if_stats reports a
                              pair's iterations and status under both of its fields.  Combine with IF_FLAG_PAIRS for
                              the kinetic-energy spectrum                                                        */
+    IF_FLAG_TRUE_RESIDUAL = 32, /* if_filter (per call, with a non-NULL if_stats.true_res; not with IF_FLAG_HIGHPASS): after the
+                             solves, apply the operator to every returned field and report the TRUE relative residual
+                             ||M phi - A_l x||_2 / ||M phi||_2 next to the recursive one (it floors near u * condition
+                             number; one SpMM per right-hand side, outside if_stats.seconds)                       */
     IF_FLAG_PAIRS = 8     /* if_spectrum (per call): the fields are velocity components in pairs (u_0, v_0, u_1, v_1, ...)
                              and the spectra of a pair are added (kinetic energy 1/2 <u^2 + v^2>, the quantity of
                              PAPER.md:149-157): n_fields even; energy is [n_fields/2][n_ells], E [n_fields/2][n_ells-1];
@@ -127,6 +131,8 @@ typedef struct {
                               for n = 2 groups 1-6 hold the sum over both cycles; [7] unused                         */
     int64_t mg_samples;     /* out: samples behind mg_kernel_seconds                                          */
     int64_t mg_batch_iters; /* out: 16-column iterations of the multigrid-preconditioned path (part of batch_iters) */
+    double* true_res;   /* HOST [n_fields*n_ells] or NULL: filled by if_filter with IF_FLAG_TRUE_RESIDUAL (the vector
+                           filter reports a pair's joint residual under both of its fields)                          */
 } if_stats;
 
 /* Preparation phase.  All pointers HOST.

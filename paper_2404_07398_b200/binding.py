@@ -22,6 +22,7 @@ IF_FLAG_HIGHPASS = 2
 IF_FLAG_MULTIGRID = 4
 IF_FLAG_PAIRS = 8
 IF_FLAG_VECTOR = 16
+IF_FLAG_TRUE_RESIDUAL = 32
 
 EXPORTS = ("if_prepare", "if_workspace_bytes", "if_filter", "if_spectrum", "if_spectrum_host", "if_apply", "if_mesh_info", "if_mesh_tile_info",
            "if_mesh_multigrid_info", "if_energy_noalloc",
@@ -39,7 +40,7 @@ class if_stats(C.Structure):
                 ("status", C.POINTER(C.c_int32)), ("seconds", C.c_double), ("batch_iters", C.c_int64),
                 ("rhs_iters", C.c_int64), ("spmm_seconds", C.c_double), ("update_seconds", C.c_double),
                 ("kernel_samples", C.c_int64), ("mg_kernel_seconds", C.c_double * 8), ("mg_samples", C.c_int64),
-                ("mg_batch_iters", C.c_int64)]
+                ("mg_batch_iters", C.c_int64), ("true_res", C.POINTER(C.c_double))]
 
 
 class ImplicitFilterError(RuntimeError):
@@ -223,10 +224,13 @@ class _Stats:
                           self.rel_res.ctypes.data_as(C.POINTER(C.c_double)),
                           self.status.ctypes.data_as(C.POINTER(C.c_int32)), 0.0, 0, 0, 0.0, 0.0, 0)
         self.c.mg_samples = 0
+        self.true_res = np.full(n_rhs, np.nan, dtype=np.float64)      # filled with IF_FLAG_TRUE_RESIDUAL
+        self.c.true_res = self.true_res.ctypes.data_as(C.POINTER(C.c_double))
 
     def as_dict(self, rc: int):
         return {"iters": self.iters.reshape(self.shape), "rel_res": self.rel_res.reshape(self.shape),
-                "status": self.status.reshape(self.shape), "seconds": float(self.c.seconds),
+                "status": self.status.reshape(self.shape), "true_res": self.true_res.reshape(self.shape),
+                "seconds": float(self.c.seconds),
                 "batch_iters": int(self.c.batch_iters), "rhs_iters": int(self.c.rhs_iters), "spmm_seconds": float(self.c.spmm_seconds),
                 "update_seconds": float(self.c.update_seconds), "kernel_samples": int(self.c.kernel_samples),
                 "mg_kernel_seconds": [float(v) for v in self.c.mg_kernel_seconds], "mg_samples": int(self.c.mg_samples),

@@ -1121,6 +1121,40 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(MeshView m, const Ctrl* __res
     }
 }
 
+// True residual of returned solutions (IF_FLAG_TRUE_RESIDUAL): q = A_c x_c is given for the K columns (x = the filtered
+// fields as the caller received them); per column ||M phi - q||_2 / ||M phi||_2 with phi gathered from the caller's
+// fields through the permutation (sp.field = field of the column, sp.rhs = where the result goes; pairs of the vector
+// filter share one norm over both components).
+template <int K>
+__global__ void __launch_bounds__(BLOCK) k_true_res(MeshView m, Ctrl* __restrict__ ctrl, double* __restrict__ partials,
+                                                    StartParams sp, const double* __restrict__ fields,
+                                                    const double* __restrict__ q, double* __restrict__ out) {
+    constexpr int TPR = K / 2;
+    constexpr int ROWS = BLOCK / TPR;
+    const int tid = threadIdx.x, l = tid % TPR;
+    const int f0 = sp.field[2 * l], f1 = sp.field[2 * l + 1];
+    double2 acc[2] = {{0.0, 0.0}, {0.0, 0.0}};
+    for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < m.nv; row += (int64_t)gridDim.x * ROWS) {
+        const double av = m.area[row];
+        const int64_t u = m.perm[row];
+        const double2 qv = ld2(q, row * K + 2 * l);
+        const double b0 = f0 >= 0 ? av * fields[(int64_t)f0 * m.nv + u] : 0.0;
+        const double b1 = f1 >= 0 ? av * fields[(int64_t)f1 * m.nv + u] : 0.0;
+        const double d0 = f0 >= 0 ? b0 - qv.x : 0.0, d1 = f1 >= 0 ? b1 - qv.y : 0.0;
+        acc[0].x = fma(d0, d0, acc[0].x); acc[0].y = fma(d1, d1, acc[0].y);
+        acc[1].x = fma(b0, b0, acc[1].x); acc[1].y = fma(b1, b1, acc[1].y);
+    }
+    __shared__ double tot[2 * KMAX];
+    if (grid_reduce<K, 2>(acc, partials, &ctrl->ticket[1], tot)) {
+        if (tid < K && sp.field[tid] >= 0) {
+            const int ta = ctrl->pair_mode ? (tid & ~1) : tid, tb = ctrl->pair_mode ? (tid | 1) : tid;
+            const double w2 = ctrl->pair_mode ? 1.0 : 0.5;
+            const double rr = w2 * (tot[ta] + tot[tb]), bb = w2 * (tot[KMAX + ta] + tot[KMAX + tb]);
+            out[sp.rhs[tid]] = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+        }
+    }
+}
+
 // per-right-hand-side results of the columns in `mask`
 __global__ void k_stats(const Ctrl* __restrict__ ctrl, int K, unsigned mask, int32_t* __restrict__ iters,
                         int32_t* __restrict__ status, double* __restrict__ relres) {

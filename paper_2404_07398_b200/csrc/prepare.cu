@@ -503,7 +503,7 @@ int resolve_options(const if_options* in, const Options* base, Options* out) {
         } else {   // per-call flags
             // per-call flags; IF_FLAG_VECTOR per call = "these fields are (u, v) pairs", valid on a handle that has the
             // metric terms (checked in run_job)
-            const int per_call = IF_FLAG_HIGHPASS | IF_FLAG_PAIRS | IF_FLAG_VECTOR;
+            const int per_call = IF_FLAG_HIGHPASS | IF_FLAG_PAIRS | IF_FLAG_VECTOR | IF_FLAG_TRUE_RESIDUAL;
             const bool has_metric = (o.flags & IF_FLAG_VECTOR) != 0;
             o.flags = (o.flags & ~per_call) | (in->flags & per_call);
             if ((o.flags & IF_FLAG_VECTOR) && !has_metric) return IF_EINVAL;
@@ -982,7 +982,7 @@ extern "C" int if_save(if_handle h, const char* path) {
     hd.unstaged_tiles = h->unstaged_tiles; hd.total_area = h->total_area; hd.mean_edge = h->mean_edge;
     hd.opt = h->opt;
     hd.opt.radius = h->radius;     // the radius actually used
-    hd.opt.flags &= ~(IF_FLAG_KEEP_CSR | IF_FLAG_HIGHPASS | IF_FLAG_PAIRS);
+    hd.opt.flags &= ~(IF_FLAG_KEEP_CSR | IF_FLAG_HIGHPASS | IF_FLAG_PAIRS | IF_FLAG_TRUE_RESIDUAL);
     std::vector<char> buf;
     const size_t nv = (size_t)h->n_vert, ns = (size_t)h->sell_slots, nt = (size_t)h->n_tiles;
     int rc = fwrite(&hd, sizeof(hd), 1, f) == 1 ? IF_OK : IF_EIO;

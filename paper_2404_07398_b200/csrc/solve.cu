@@ -296,44 +296,84 @@ Ctrl fresh_ctrl(const Run& r) {
     return hc;
 }
 
+// q = A_c x_c for up to K columns: column i takes its values from src[field_i] (caller's numbering) and its scale from
+// sp.c[i]; the control block is reset (no solve may be in flight).  Result in r.w.q, internal order.
+template <int K>
+int apply_columns(Run& r, const StartParams& sp, const double* d_src) {
+    const if_mesh_s* h = r.h;
+    int rc;
+    Ctrl hc = fresh_ctrl(r);
+    for (int c = 0; c < KMAX; ++c) { hc.c[c] = sp.c[c]; hc.field[c] = sp.field[c]; hc.rhs[c] = sp.rhs[c]; }
+    hc.all_done = 0;
+    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
+    IF_CUDA_TRY(cudaStreamSynchronize(r.st));      // hc lives on this stack frame
+    const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
+    k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, sp, (1u << K) - 1u, d_src, r.w.x);
+    IF_LAUNCH_CHECK();
+    const double* v = r.w.x;
+    if (r.order_n >= 2) {
+        SpmmArgs a{r.w.x, nullptr, nullptr, r.w.t, nullptr, 1, 0};
+        if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, a))) return rc;
+        double* t = r.w.t;
+        if ((rc = more_factors<K>(r, r.order_n - 2, &t))) return rc;
+        v = t;
+    }
+    SpmmArgs b{v, r.w.x, nullptr, r.w.q, nullptr, 0, 0};
+    return launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b);
+}
+
+// Batches of right-hand sides for apply_columns: rhs[first ...] into columns (pairs of columns for the vector filter);
+// src_by_rhs: the source field of a column is the right-hand side's own slot f * n_ells + j (the filtered fields in
+// d_out) instead of field f.  Returns the number of columns in use.
+template <int K>
+size_t fill_columns(const Run& r, const std::vector<Rhs>& rhs, size_t first, int n_ells, bool src_by_rhs, StartParams* sp,
+                    StartParams* orig) {
+    const size_t step = r.vec ? 2 : 1, per_batch = K / step;
+    const size_t count = std::min<size_t>(per_batch, rhs.size() - first) * step;
+    memset(sp, 0, sizeof(*sp));
+    for (int c = 0; c < KMAX; ++c) sp->field[c] = -1;
+    if (orig) *orig = *sp;
+    for (size_t i = 0; i < count; ++i) {
+        const Rhs& q = rhs[first + i / step];
+        const int f = r.vec ? 2 * q.f + (int)(i % step) : q.f;
+        sp->c[i] = r.opt.gamma * std::pow(q.ell, 2.0 * r.order_n);
+        sp->rhs[i] = f * n_ells + q.j;
+        sp->field[i] = src_by_rhs ? sp->rhs[i] : f;
+        if (orig) { orig->c[i] = sp->c[i]; orig->rhs[i] = sp->rhs[i]; orig->field[i] = f; }
+    }
+    return count;
+}
+
 // if_apply: out = A_c phi for every right-hand side, K at a time (no iteration).
 template <int K>
 int apply_all(Run& r, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out) {
     const if_mesh_s* h = r.h;
     int rc;
     if ((rc = setup_grids<K>(r))) return rc;
-    const size_t step = r.vec ? 2 : 1;          // columns per right-hand side (vector filter: the (u, v) pair)
-    const size_t per_batch = K / step;
+    const size_t per_batch = K / (r.vec ? 2 : 1);
     for (size_t first = 0; first < rhs.size(); first += per_batch) {
-        const size_t count = std::min<size_t>(per_batch, rhs.size() - first) * step;     // columns in use
-        Ctrl hc = fresh_ctrl(r);
         StartParams sp;
-        memset(&sp, 0, sizeof(sp));
-        for (int c = 0; c < KMAX; ++c) sp.field[c] = -1;
-        for (size_t i = 0; i < count; ++i) {
-            const Rhs& q = rhs[first + i / step];
-            const int f = r.vec ? 2 * q.f + (int)(i % step) : q.f;
-            hc.c[i] = sp.c[i] = r.opt.gamma * std::pow(q.ell, 2.0 * r.order_n);
-            hc.field[i] = sp.field[i] = f;
-            hc.rhs[i] = sp.rhs[i] = f * n_ells + q.j;
-        }
-        hc.all_done = 0;
-        IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
-        const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
-        k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, sp, (1u << K) - 1u, d_fields, r.w.x);
-        IF_LAUNCH_CHECK();
-        const double* v = r.w.x;
-        if (r.order_n >= 2) {
-            SpmmArgs a{r.w.x, nullptr, nullptr, r.w.t, nullptr, 1, 0};
-            if ((rc = launch_spmm<K, MODE_PLAIN>(r, r.g.plain, a))) return rc;
-            double* t = r.w.t;
-            if ((rc = more_factors<K>(r, r.order_n - 2, &t))) return rc;
-            v = t;
-        }
-        SpmmArgs b{v, r.w.x, nullptr, r.w.q, nullptr, 0, 0};
-        if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, b))) return rc;
+        fill_columns<K>(r, rhs, first, n_ells, false, &sp, nullptr);
+        if ((rc = apply_columns<K>(r, sp, d_fields))) return rc;
         const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
         k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, (1u << K) - 1u, r.w.q, r.w.p0, r.w.p1, 0, d_out, nullptr, 0);
+        IF_LAUNCH_CHECK();
+    }
+    return IF_OK;
+}
+
+// IF_FLAG_TRUE_RESIDUAL after if_filter: ||M phi - A x|| / ||M phi|| of every returned field, into d_true[rhs]
+template <int K>
+int true_residuals(Run& r, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, const double* d_out,
+                   double* d_true) {
+    int rc;
+    if ((rc = setup_grids<K>(r))) return rc;
+    const size_t per_batch = K / (r.vec ? 2 : 1);
+    for (size_t first = 0; first < rhs.size(); first += per_batch) {
+        StartParams sp, orig;
+        fill_columns<K>(r, rhs, first, n_ells, true, &sp, &orig);
+        if ((rc = apply_columns<K>(r, sp, d_out))) return rc;
+        k_true_res<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, orig, d_fields, r.w.q, d_true);
         IF_LAUNCH_CHECK();
     }
     return IF_OK;
@@ -718,6 +758,26 @@ int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields
     }
     IF_CUDA_TRY(cudaEventRecord(t1, r.st));
 
+    // IF_FLAG_TRUE_RESIDUAL (if_filter, low-pass output): one operator application per returned field, after the
+    // timed part.  The workspace is laid out afresh (column compaction may have re-used buffers for narrower layouts).
+    const bool want_true = job == JOB_FILTER && stats && stats->true_res && (r.opt.flags & IF_FLAG_TRUE_RESIDUAL) &&
+                           !(r.opt.flags & IF_FLAG_HIGHPASS);
+    std::vector<double> h_true;
+    if (want_true) {
+        r.w = layout_workspace(h, order_n, r.opt.batch, d_ws);
+        r.mg = false;
+        std::vector<Rhs> all;
+        for (int f = 0; f < (r.vec ? n_fields / 2 : n_fields); ++f)
+            for (int j = 0; j < n_ells; ++j) all.push_back(Rhs{ells[j], f, j});
+        const int KB = r.opt.batch;
+        rc = KB == 4 ? true_residuals<4>(r, d_fields, all, n_ells, d_out, r.w.E)
+           : KB == 8 ? true_residuals<8>(r, d_fields, all, n_ells, d_out, r.w.E)
+                     : true_residuals<16>(r, d_fields, all, n_ells, d_out, r.w.E);
+        if (rc != IF_OK) return rc;
+        h_true.resize((size_t)R);
+        IF_CUDA_TRY(cudaMemcpyAsync(h_true.data(), r.w.E, (size_t)R * 8, cudaMemcpyDeviceToHost, r.st));
+    }
+
     // results back to the host (small), then one synchronisation
     std::vector<int32_t> h_status((size_t)R, 0), h_iters((size_t)R, 0);
     std::vector<double> h_relres((size_t)R, 0.0);
@@ -752,6 +812,7 @@ int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields
             if (stats->iters) stats->iters[i] = h_iters[(size_t)i];
             if (stats->status) stats->status[i] = h_status[(size_t)i];
             if (stats->rel_res) stats->rel_res[i] = h_relres[(size_t)i];
+            if (want_true) stats->true_res[i] = h_true[(size_t)i];
         }
     }
     return result;

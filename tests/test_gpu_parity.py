@@ -904,3 +904,30 @@ def test_vector_filter_planar_mesh_and_save_load(ifl, oracle_mod, tmp_path):
     xu, xv, info = om.solve_vector(vf[0], vf[1], float(mesh.h * ells[1]), 2)
     assert rel(c[0, 1].cpu().numpy(), xu) <= TOL_FIELD and rel(c[1, 1].cpu().numpy(), xv) <= TOL_FIELD
     g.close()
+
+
+def test_true_residual_in_stats(ifl, oracle_mod):
+    """IF_FLAG_TRUE_RESIDUAL: if_filter also reports ||M phi - A_l x|| / ||M phi|| of the fields it returns (SURVEY.md
+    section 5 metrics).  Checked against the same quantity formed from if_apply in the test and against the oracle's
+    recorded true residual (same floor u * kappa, within a factor); n = 1, 2, both solvers, narrow batches, the vector
+    filter."""
+    w = make_config(5, level=5, n_fields=3, n_ells=5, ell_max=32.0)
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    area = om.area()
+    TR = ifl.IF_FLAG_TRUE_RESIDUAL
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID | ifl.IF_FLAG_VECTOR)
+    for order_n, kw in ((1, {}), (2, {}), (2, dict(solver=1)), (1, dict(batch=4))):
+        out, st = ifl.if_filter(h, w.fields, w.ells, order_n, flags=TR, **kw)
+        assert st["code"] == 0 and np.all(np.isfinite(st["true_res"]))
+        for f in range(3):
+            for j, ell in enumerate(w.ells):
+                mine = true_residual(ifl, h, out[f, j], w.fields[f], area, float(ell), order_n)
+                assert abs(st["true_res"][f, j] - mine) <= 1e-6 * mine + 1e-16, (order_n, kw, f, j)
+                assert st["true_res"][f, j] >= 0.3 * st["rel_res"][f, j] - 1e-15
+        _, info = om.solve(w.fields[0], float(w.ells[-1]), order_n)
+        assert st["true_res"][0, -1] <= 20.0 * max(info["true_res"], 1e-12)
+    _, st = ifl.if_filter(h, w.fields, w.ells, 1)
+    assert np.all(np.isnan(st["true_res"]))                      # off by default
+    out, st = ifl.if_filter(h, w.fields[:2], w.ells[:3], 1, flags=TR | ifl.IF_FLAG_VECTOR)
+    assert st["code"] == 0 and np.array_equal(st["true_res"][0], st["true_res"][1]) and np.all(st["true_res"] <= 1e-11)
+    h.close()
