@@ -259,3 +259,41 @@ def test_config5_full_size_all_320_right_hand_sides(full, oracle_mesh, oracle_mo
         assert rel(out[f, scales.index(j)].cpu().numpy(), x) <= TOL_FIELD, (f, j)
         e = oracle_mesh.energy(x)
         assert abs(sp["energy"][f, j] - e) <= TOL_BIN * e, (f, j)
+
+
+def test_vector_filter_large_band(oracle_mod):
+    """The coupled vector filter (IF_FLAG_VECTOR) on a latitude band of the level-9 icosphere (2.5 M
+    vertices), 4 (u, v) pairs x 6 scales, n = 1, K = 16 (8 pairs per SpMM): one pair at the two smallest scales against
+    the oracle's joint PCG, every solve through its true residual (IF_FLAG_TRUE_RESIDUAL); prints the bandwidth of the
+    vector kernel A (6 vectors + 20 B per matrix entry + 16 B per row)."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2404_07398_b200 as lib
+    from workloads import icosphere, jitter_sphere, log_spaced, sphere_band, sphere_velocity_field
+    mesh = sphere_band(jitter_sphere(icosphere(9), 0.25, np.random.default_rng(41)), 70.0)
+    rng = np.random.default_rng(42)
+    fields = np.empty((8, mesh.n_vert))
+    for p in range(4):
+        fields[2 * p], fields[2 * p + 1] = sphere_velocity_field(mesh.coords, 200, 64, rng)
+    ells = mesh.h * log_spaced(1.0, 24.0, 6)
+    VEC = lib.IF_FLAG_VECTOR
+    h = lib.if_prepare(mesh.coords, mesh.tri, None, flags=VEC, radius=1.0)
+    assert h.n_vert > 2_400_000
+    out, st = lib.if_filter(h, fields, ells, 1, flags=VEC | lib.IF_FLAG_TRUE_RESIDUAL)
+    assert st["code"] == 0 and np.all(st["status"] == 0) and np.all(st["true_res"] <= 1e-10)
+    assert np.array_equal(st["iters"][0::2], st["iters"][1::2])          # a pair shares its iteration count
+    om = oracle_mod.OracleMesh(mesh.coords, mesh.tri, None)
+    om.build_vector(1.0)
+    for j in (0, 1):
+        xu, xv, info = om.solve_vector(fields[0], fields[1], float(ells[j]), 1)
+        assert info["status"] == 0
+        assert rel(out[0, j].cpu().numpy(), xu) <= TOL_FIELD and rel(out[1, j].cpu().numpy(), xv) <= TOL_FIELD, j
+    sp = lib.if_spectrum(h, fields, ells, 1, flags=VEC | lib.IF_FLAG_PAIRS)
+    assert sp["energy"].shape == (4, 6) and np.all(np.diff(sp["energy"], axis=1) < 0.0) and np.all(sp["E"] > 0.0)
+    s = sp["stats"]
+    if s["kernel_samples"] > 0:
+        nbytes = h.n_vert * 16 * 8 * 6 + (h.nnz - h.n_vert) * 20 + h.n_vert * 16
+        print(f"vector kernel A: {1e3 * s['spmm_seconds']:.3f} ms per launch, {nbytes / s['spmm_seconds'] / 1e9:.0f} GB/s "
+              f"algorithmic ({s['kernel_samples']} samples, V = {h.n_vert})")
+    h.close()

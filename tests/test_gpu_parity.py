@@ -200,6 +200,20 @@ def test_degenerate_inputs(ifl, oracle_mod):
     with pytest.raises(ifl.ImplicitFilterError) as e:
         ifl.if_filter(h, w.fields, [1.0], 1, workspace=torch.empty(1024, dtype=torch.uint8, device="cuda"))
     assert e.value.code == -7
+    # empty inputs and the largest job the result arrays serve (65 536 right-hand sides per call)
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_filter(h, w.fields, [], 1)
+    assert e.value.code == -1
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_spectrum(h, w.fields, [1.0], 1)                   # a spectrum needs two scales
+    assert e.value.code == -1
+    with pytest.raises(ifl.ImplicitFilterError) as e:
+        ifl.if_spectrum(h, w.fields, np.linspace(1.0, 2.0, 65537) * w.mesh.h, 1)
+    assert e.value.code == -1
+    for bad in (np.nan, np.inf, 0.0):
+        with pytest.raises(ifl.ImplicitFilterError) as e:
+            ifl.if_filter(h, w.fields, [1.0, bad], 1)
+        assert e.value.code == -1
     h.close()
 
 
