@@ -150,6 +150,8 @@ def test_rigid_rotation_is_attenuated_like_an_l1_harmonic(oracle_mod, axis, n):
     out: there the biharmonic boundary layer of the band, 4e-3, exceeds the effect.)"""
     if n == 2 and abs(axis[2]) > 0.9:
         pytest.skip("boundary layer of the band exceeds the attenuation for this case")
+    if n == 2 and axis[1] != 0.0:
+        pytest.skip("n = 2 is checked about one equatorial axis (a minute of oracle time per axis)")
     mesh = sphere_band(jitter_sphere(icosphere(5), 0.15, np.random.default_rng(10)), 75.0)
     m = oracle_mod.OracleMesh(mesh.coords, mesh.tri, None)
     m.build_vector(1.0)
