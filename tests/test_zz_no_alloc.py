@@ -25,13 +25,17 @@ def test_energy_noalloc_matches_the_existing_path_twice_in_a_row():
     flat = out.reshape(-1, h.n_vert)                             # 16 fields
     area = torch.from_numpy(ifl.if_mesh_export_csr(h)[3]).to(flat.device)
     plain = (0.5 * (area * flat * flat).sum(dim=1) / area.sum()).cpu().numpy()
-    e = torch.full((flat.shape[0],), -1.0, dtype=torch.float64, device=flat.device)
-    before = torch.cuda.memory_allocated()
-    first = ifl.if_energy_noalloc(h, flat, out=e).cpu().numpy().copy()
+    e1, e2, e3 = (torch.full((flat.shape[0],), -1.0, dtype=torch.float64, device=flat.device) for _ in range(3))
+    part = flat[:5]
+    torch.cuda.synchronize()
+    allocs = lambda: torch.cuda.memory_stats()["allocation.all.allocated"]      # allocations so far (monotonic)
+    before = allocs()
+    ifl.if_energy_noalloc(h, flat, out=e1)
     # second call in a row: the shared scratch array holds the first call's partial sums and ticket
-    half = ifl.if_energy_noalloc(h, flat[:5], out=e[:5]).cpu().numpy().copy()
-    second = ifl.if_energy_noalloc(h, flat, out=e).cpu().numpy().copy()
-    assert torch.cuda.memory_allocated() == before
+    ifl.if_energy_noalloc(h, part, out=e2[:5])
+    ifl.if_energy_noalloc(h, flat, out=e3)
+    assert allocs() == before                                    # nothing was allocated through torch either
+    first, half, second = e1.cpu().numpy(), e2[:5].cpu().numpy(), e3.cpu().numpy()
     want = sp["energy"].reshape(-1)
     for got in (first, second):
         assert np.all(np.abs(got - want) <= TOL_BIN * want), np.abs(got / want - 1).max()
@@ -48,7 +52,7 @@ def test_energy_noalloc_matches_the_existing_path_twice_in_a_row():
     s2 = torch.cuda.Stream()
     s2.wait_stream(torch.cuda.current_stream())
     with torch.cuda.stream(s2):
-        third = ifl.if_energy_noalloc(h, flat, out=e, stream=s2)
+        third = ifl.if_energy_noalloc(h, flat, out=e1, stream=s2)
     s2.synchronize()
     assert np.array_equal(third.cpu().numpy(), first)
     h.close()
