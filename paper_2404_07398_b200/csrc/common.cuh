@@ -62,6 +62,7 @@ int resolve_options(const if_options* in, const Options* base, Options* out);
 struct if_mesh_s;
 namespace ifl {
 int mg_build(if_mesh_s* h);    // mg.cu: builds h->mg from the SELL matrix and the areas
+int mg_tile_caps(if_mesh_s* h);   // mg.cu: fills MgLevel::cap_* (after mg_build or if_load)
 int na_setup(if_mesh_s* h);    // noalloc.cu: looks up the device address of its static scratch array (once per handle)
 void mg_free(if_mesh_s* h);
 
@@ -69,6 +70,7 @@ void mg_free(if_mesh_s* h);
 // Level 0 is the mesh itself; level l+1 has one unknown per graph aggregate of level l (mg.cu).  Every level stores
 // the pair (S_l, M_l) on one sparsity pattern, so that A_l = M_l + c S_l is applied matrix-free for any scale.
 constexpr int MG_MAX_LEVELS = 12;
+constexpr int MG_TILE = 64;        // rows per tile of the row-block kernels (k_mg_rows, mg_solve.cuh)
 constexpr int MG_COARSEST = 64;    // the hierarchy stops at a level with at most this many unknowns (dense solve)
 // Cycle and aggregation parameters (macros: the tuning runs of DESIGN.md section 9b rebuild with -DIF_MG_...).
 #ifndef IF_MG_THETA
@@ -103,6 +105,9 @@ struct MgLevel {
     double2* diag = nullptr;     // [n]    (S_ii, M_ii)
     // transfer to level l+1 (absent on the coarsest level): P [n x n_coarse] by rows, R = P^T by rows
     int64_t n_coarse = 0, p_nnz = 0;
+    // most entries in a block of MG_TILE consecutive rows of the level's matrix, of P and of R (mg_tile_caps): what a
+    // stage of the row-block kernels of the cycle must hold
+    int cap_a = 0, cap_p = 0, cap_r = 0;
     int64_t* p_rowptr = nullptr;
     int32_t* p_col = nullptr;
     double* p_val = nullptr;

@@ -38,7 +38,7 @@ struct DBuf {
     ~DBuf() { if (p) cudaFreeAsync(p, 0); }
     cudaError_t alloc(size_t bytes) {
         if (p) { cudaFreeAsync(p, 0); p = nullptr; }
-        return cudaMallocAsync(&p, bytes ? bytes : 1, 0);
+        return cudaMallocAsync(&p, bytes + 16, 0);      // +16: the row-block kernels bulk-copy 16-byte multiples
     }
     template <class T> T* as() const { return static_cast<T*>(p); }
     void* release() { void* q = p; p = nullptr; return q; }
@@ -604,6 +604,39 @@ int build_next_level(MgLevel& f, MgLevel& c, cudaStream_t st) {
 
 }  // namespace
 
+namespace {
+__global__ void k_mg_tile_cap(const int64_t* __restrict__ rowptr, int64_t n, int* __restrict__ cap) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t r0 = t * MG_TILE;
+    if (r0 >= n) return;
+    const int64_t r1 = r0 + MG_TILE < n ? r0 + MG_TILE : n;
+    atomicMax(cap, (int)(rowptr[r1] - rowptr[r0]));
+}
+}  // namespace
+
+int mg_tile_caps(if_mesh_s* h) {
+    if (h->mg_levels < 1) return IF_OK;
+    int* d = nullptr;
+    IF_CUDA_TRY(cudaMalloc((void**)&d, 3 * MG_MAX_LEVELS * sizeof(int)));
+    IF_CUDA_TRY(cudaMemset(d, 0, 3 * MG_MAX_LEVELS * sizeof(int)));
+    for (int l = 0; l < h->mg_levels; ++l) {
+        const MgLevel& g = h->mg[l];
+        const unsigned ga = (unsigned)(((g.n + MG_TILE - 1) / MG_TILE + 255) / 256);
+        k_mg_tile_cap<<<ga, 256>>>(g.rowptr, g.n, d + 3 * l);
+        if (l + 1 < h->mg_levels && g.p_rowptr) {
+            k_mg_tile_cap<<<ga, 256>>>(g.p_rowptr, g.n, d + 3 * l + 1);
+            const unsigned gr = (unsigned)(((g.n_coarse + MG_TILE - 1) / MG_TILE + 255) / 256);
+            k_mg_tile_cap<<<gr, 256>>>(g.r_rowptr, g.n_coarse, d + 3 * l + 2);
+        }
+    }
+    int host[3 * MG_MAX_LEVELS];
+    cudaError_t e = cudaMemcpy(host, d, sizeof(host), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    IF_CUDA_TRY(e);
+    for (int l = 0; l < h->mg_levels; ++l) { h->mg[l].cap_a = host[3 * l]; h->mg[l].cap_p = host[3 * l + 1]; h->mg[l].cap_r = host[3 * l + 2]; }
+    return IF_OK;
+}
+
 void mg_free(if_mesh_s* h) {
     for (int l = 0; l < MG_MAX_LEVELS; ++l) {
         MgLevel& g = h->mg[l];
@@ -676,6 +709,7 @@ int mg_build(if_mesh_s* h) {
     }
     h->mg_levels = L;
     IF_CUDA_TRY(cudaStreamSynchronize(st));
+    { int rc = mg_tile_caps(h); if (rc != IF_OK) { mg_free(h); return rc; } }
     h->mg_build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
     if (getenv("IF_VERBOSE"))
         for (int l = 0; l < L; ++l)

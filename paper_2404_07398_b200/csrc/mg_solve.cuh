@@ -223,6 +223,168 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_prolong0(const int64_t
     }
 }
 
+// ---- row-block kernels of the cycle (round 2).  The CSR kernels above walk a dependent chain per row -- row pointer ->
+// entries -> gathered rows of x, three trips to memory, the first two to lines nobody has touched -- and are bound by
+// exactly that chain: 9 latencies per group of four rows on level 1 (12.5 entries per row in batches of four) give
+// 0.20 ms for its 815 k rows on config 4 (measured 0.216), 3 latencies give 0.64 ms for the prolongation onto the mesh
+// (measured 0.64).  Here a persistent CTA walks tiles of MG_TILE consecutive rows through a ring of shared-memory
+// stages: one thread issues bulk async copies (TMA, mbarrier complete_tx) of the tile's row pointers, its contiguous
+// range of entries (columns, values) and its own rows of the per-row operands two tiles ahead, and the only trip to
+// memory left in a row's chain is the gather itself, eight entries in flight per thread.  Same sums in the same order
+// as the CSR kernels (entry by entry), so the results are bit-identical.
+// (First form tried: a persistent CTA with a ring of stages that also held the own-row vectors -- 16 warps per SM and
+// a block barrier per 64 rows: restriction 0.34 -> 0.93 ms, level 1 0.62 -> 1.06 ms.  Rejected.)
+enum RowsKind { ROWS_RES = 0, ROWS_SWEEP = 1, ROWS_SET = 2, ROWS_ACC = 3, ROWS_PROLONG0 = 4 };
+//   ROWS_RES      y = r - K x                      K = M + c1 S, (S, M) pairs per entry
+//   ROWS_SWEEP    y = x + omega (r - K x) / d
+//   ROWS_SET      y = B x                          scalar entries (restriction)
+//   ROWS_ACC      y += B x                         (prolongation)
+//   ROWS_PROLONG0 y = omega r / d + B x            (prolongation onto the mesh fused with the first sweep, as k_mg_prolong0)
+struct RowsArgs {
+    const int64_t* rowptr;
+    const int32_t* col;
+    const void* val;          // double2 (S, M) for RES / SWEEP, double for the others
+    const double2* diag;      // SWEEP, PROLONG0: (S_ii, M_ii)
+    int64_t n;                // rows
+    const double* x;          // the gathered vector
+    const double* own0;       // RES, SWEEP, PROLONG0: r ;  ACC: y (read)
+    const double* own1;       // SWEEP: x (own rows) ;  PROLONG0 with r_select: the second residual buffer
+    double* y;
+    double omega;
+    int r_select;             // PROLONG0: r = (own0, own1)[cur_r ^ 1] (see SpmmArgs::r_select)
+    int cap;                  // entries a stage holds (MgLevel::cap_*)
+    int stages;
+};
+
+constexpr int ROWS_PER_CTA = 2 * MG_TILE;      // rows of one CTA (MgLevel::cap_* bounds the entries of MG_TILE rows)
+
+struct RowsLayout { uint32_t col, val, bytes; };      // offsets inside the CTA's shared memory
+template <int KIND>
+__host__ __device__ inline RowsLayout rows_layout(int cap) {
+    constexpr bool PAIR = KIND <= ROWS_SWEEP;
+    const uint32_t ce = (uint32_t)cap * (ROWS_PER_CTA / MG_TILE);      // entries of the CTA's rows, at most
+    RowsLayout L;
+    L.col = (uint32_t)((ROWS_PER_CTA + 2) * 8);
+    L.val = L.col + (((ce + 4u) * 4u + 15u) & ~15u);
+    L.bytes = L.val + (PAIR ? ce * 16u : (((ce + 2u) * 8u + 15u) & ~15u)) + 16u;     // + the mbarrier
+    return L;
+}
+
+// One CTA = ROWS_PER_CTA consecutive rows: thread 0 asks for the two row pointers that bound the CTA's entries and
+// issues three bulk copies (row pointers, columns, values); meanwhile every thread loads the own-row operands of its
+// rows; after the mbarrier the rows are walked with the gathers as the only trips to memory.  Several CTAs are
+// resident per SM, so one CTA's copy phase hides behind the others' gathers (no block barrier inside the loop).
+#ifndef IF_ROWS_UB_PAIR
+#define IF_ROWS_UB_PAIR 8
+#endif
+#ifndef IF_ROWS_MINB_PAIR
+#define IF_ROWS_MINB_PAIR 2
+#endif
+template <int KIND>
+__global__ void __launch_bounds__(BLOCK, KIND <= 1 ? IF_ROWS_MINB_PAIR : 4) k_mg_rows(RowsArgs a, const Ctrl* __restrict__ ctrl) {
+    constexpr bool PAIR = KIND <= ROWS_SWEEP;
+    // gathers a thread has in flight: rows of the level matrices have a dozen entries and more, prolongator rows 2-5
+    constexpr int ROWS_UB = (KIND == ROWS_ACC || KIND == ROWS_PROLONG0) ? 4 : (KIND <= ROWS_SWEEP ? IF_ROWS_UB_PAIR : 8);
+    constexpr bool OWN0 = KIND != ROWS_SET, OWN1 = KIND == ROWS_SWEEP, DIAG = KIND == ROWS_SWEEP || KIND == ROWS_PROLONG0;
+    constexpr int RPT = ROWS_PER_CTA / (BLOCK / 8);      // rows per thread group
+    if (ctrl->all_done) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const RowsLayout L = rows_layout<KIND>(a.cap);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bytes - 16);
+    const int tid = threadIdx.x, l = tid % 8, g = tid / 8;
+    const int64_t r0 = (int64_t)blockIdx.x * ROWS_PER_CTA;
+    const int nr = (int)min((int64_t)ROWS_PER_CTA, a.n - r0);
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        fence_proxy_async();
+        const int64_t k0 = a.rowptr[r0], k1 = a.rowptr[r0 + nr];
+        const uint32_t rp_bytes = ((uint32_t)(nr + 1) * 8u + 15u) & ~15u;
+        const int64_t kA = k0 & ~3LL;
+        const uint32_t col_bytes = ((uint32_t)(k1 - kA) * 4u + 15u) & ~15u;
+        const int64_t kB = PAIR ? k0 : (k0 & ~1LL);
+        const uint32_t val_bytes = PAIR ? (uint32_t)(k1 - k0) * 16u : (((uint32_t)(k1 - kB) * 8u + 15u) & ~15u);
+        mbar_expect_tx(bar, rp_bytes + col_bytes + val_bytes);
+        bulk_load(smem, a.rowptr + r0, rp_bytes, bar);
+        bulk_load(smem + L.col, a.col + kA, col_bytes, bar);
+        if (PAIR) bulk_load(smem + L.val, static_cast<const double2*>(a.val) + k0, val_bytes, bar);
+        else bulk_load(smem + L.val, static_cast<const double*>(a.val) + kB, val_bytes, bar);
+    }
+    double2 cc = {0.0, 0.0};
+    if (PAIR || KIND == ROWS_PROLONG0) cc = ld2(ctrl->c1, 2 * l);
+    const double* own0 = a.own0;
+    if (KIND == ROWS_PROLONG0 && a.r_select) own0 = ctrl->cur_r ? a.own0 : a.own1;
+    // own-row operands: those of the thread's first row are in flight while the bulk copies land, those of row i + 1
+    // while row i is gathered
+    double2 o0n = {0.0, 0.0}, o1n = {0.0, 0.0}, dgn = {0.0, 0.0};
+    auto load_own = [&](int r) {
+        if (r < nr) {
+            const int64_t ri = (r0 + r) * MGK + 2 * l;
+            if (OWN0) o0n = ld2(own0, ri);
+            if (OWN1) o1n = ld2(a.own1, ri);
+            if (DIAG) dgn = a.diag[r0 + r];
+        }
+    };
+    load_own(g);
+    __syncthreads();            // the mbarrier is initialised
+    mbar_wait(bar, 0u);
+    const int64_t* srp = reinterpret_cast<const int64_t*>(smem);
+    const int32_t* scol = reinterpret_cast<const int32_t*>(smem + L.col);
+    const double2* sval2 = reinterpret_cast<const double2*>(smem + L.val);
+    const double* sval1 = reinterpret_cast<const double*>(smem + L.val);
+    const int64_t k0 = srp[0];
+    const int64_t kA = k0 & ~3LL, kB = PAIR ? k0 : (k0 & ~1LL);
+#pragma unroll
+    for (int i = 0; i < RPT; ++i) {
+        const int r = g + i * (BLOCK / 8);
+        if (r >= nr) break;
+        const double2 o0c = o0n, o1c = o1n, dgc = dgn;
+        load_own(r + BLOCK / 8);
+        const int64_t kb = srp[r], ke = srp[r + 1];
+        double2 s = {0.0, 0.0};
+        for (int64_t k = kb; k < ke; k += ROWS_UB) {
+            int32_t cj[ROWS_UB];
+            double2 v[ROWS_UB];
+#pragma unroll
+            for (int j = 0; j < ROWS_UB; ++j) cj[j] = scol[(k + j < ke ? k + j : k) - kA];
+#pragma unroll
+            for (int j = 0; j < ROWS_UB; ++j) v[j] = ld2(a.x, (int64_t)cj[j] * MGK + 2 * l);
+#pragma unroll
+            for (int j = 0; j < ROWS_UB; ++j)
+                if (k + j < ke) {
+                    if (PAIR) {
+                        const double2 w = sval2[k + j - k0];
+                        s.x = fma(fma(cc.x, w.x, w.y), v[j].x, s.x);
+                        s.y = fma(fma(cc.y, w.x, w.y), v[j].y, s.y);
+                    } else {
+                        const double w = sval1[k + j - kB];
+                        s.x = fma(w, v[j].x, s.x);
+                        s.y = fma(w, v[j].y, s.y);
+                    }
+                }
+        }
+        const int64_t ri = (r0 + r) * MGK + 2 * l;
+        if (KIND == ROWS_SET) {
+            st2(a.y, ri, s);
+        } else if (KIND == ROWS_ACC) {
+            st2(a.y, ri, make_double2(s.x + o0c.x, s.y + o0c.y));
+        } else if (KIND == ROWS_PROLONG0) {
+            const double2 rv = o0c, d = dgc;
+            s.x += a.omega * rv.x * rcp_pos(fma(cc.x, d.x, d.y));       // the arithmetic of k_mg_prolong0
+            s.y += a.omega * rv.y * rcp_pos(fma(cc.y, d.x, d.y));
+            st2(a.y, ri, s);
+        } else {
+            const double2 rv = o0c;
+            double2 t = {rv.x - s.x, rv.y - s.y};
+            if (KIND == ROWS_SWEEP) {
+                const double2 d = dgc, xv = o1c;
+                t.x = fma(a.omega * t.x, 1.0 / fma(cc.x, d.x, d.y), xv.x);   // the arithmetic of k_mg_apply<2, *>
+                t.y = fma(a.omega * t.y, 1.0 / fma(cc.y, d.x, d.y), xv.y);
+            }
+            st2(a.y, ri, t);
+        }
+    }
+}
+
 // Coarsest level (n <= MG_COARSEST unknowns).  K = M + c1 S depends on the column only through c1, which changes when
 // the column is (re)started -- not from cycle to cycle -- so its inverse is formed once per column start
 // (k_mg_coarse_factor: dense Cholesky K = L L^T in shared memory, L^-1 by forward substitution on the unit vectors,
@@ -329,8 +491,35 @@ inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
 // groups of the per-kernel timing (if_stats.mg_kernel_seconds)
 enum { MGT_A = 0, MGT_MGR = 1, MGT_RESTRICT0 = 2, MGT_LEVEL1 = 3, MGT_COARSE = 4, MGT_PROLONG0 = 5, MGT_LAST = 6 };
 
+#ifndef IF_MG_ROWS
+#define IF_MG_ROWS 1                 // 0: the CSR kernels everywhere (A/B measurements)
+#endif
+constexpr size_t ROWS_SMEM_MAX = 200 * 1024;      // dynamic shared memory a k_mg_rows CTA may ask for
+constexpr size_t ROWS_SMEM_SM = 220 * 1024;       // what the CTAs of one SM share
+
+// Launch k_mg_rows<KIND> if the entries of a CTA's rows fit its shared memory; *done = false means "use the CSR kernel".
+template <int KIND>
+int launch_rows(const Run& r, RowsArgs a, int cap, bool* done) {
+    *done = false;
+    if (!IF_MG_ROWS || cap <= 0 || a.n < 4 * ROWS_PER_CTA) return IF_OK;
+    const RowsLayout L = rows_layout<KIND>(cap);
+    if (L.bytes > ROWS_SMEM_MAX / 3) return IF_OK;          // fewer than three CTAs per SM: the copy phases would show
+    a.cap = cap;
+    a.stages = 1;
+    const unsigned grid = (unsigned)((a.n + ROWS_PER_CTA - 1) / ROWS_PER_CTA);
+    k_mg_rows<KIND><<<grid, BLOCK, L.bytes, r.st>>>(a, r.w.ctrl);
+    IF_LAUNCH_CHECK();
+    *done = true;
+    return IF_OK;
+}
+
 int mg_setup(Run& r) {
     const if_mesh_s* h = r.h;
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_RES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_SET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_PROLONG0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
     IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_coarse_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MG_FACTOR_SMEM));
     const int64_t tiles = (h->n_vert + TILE_ROWS - 1) / TILE_ROWS;
     int rc;
@@ -338,6 +527,38 @@ int mg_setup(Run& r) {
     if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;
     if (r.order_n == 2 &&
         (rc = resident_grid(k_spmm<MGK, MODE_MGR0>, TileSmem<MGK, MODE_MGR0>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<MGK, MODE_MGR0>::NT))) return rc;
+    return IF_OK;
+}
+
+// y = R x (restriction of level l, rows = the coarse level) and y += P x (prolongation, rows = level l)
+int mg_restrict(const Run& r, const MgLevel& g, const double* x, double* y) {
+    const if_mesh_s* h = r.h;
+    const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse;
+    bool done = false;
+    int rc;
+    if (!wide_r) {
+        RowsArgs a{g.r_rowptr, g.r_col, g.r_val, nullptr, g.n_coarse, x, nullptr, nullptr, y, 0.0, 0, 0, 0};
+        if ((rc = launch_rows<ROWS_SET>(r, a, g.cap_r, &done))) return rc;
+        if (done) return IF_OK;
+    }
+    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, r.w.ctrl, x, y);
+    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, r.w.ctrl, x, y);
+    IF_LAUNCH_CHECK();
+    return IF_OK;
+}
+int mg_prolong_add(const Run& r, const MgLevel& g, const double* x, double* y) {
+    const if_mesh_s* h = r.h;
+    const bool wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
+    bool done = false;
+    int rc;
+    if (!wide_p) {
+        RowsArgs a{g.p_rowptr, g.p_col, g.p_val, nullptr, g.n, x, y, nullptr, y, 0.0, 0, 0, 0};
+        if ((rc = launch_rows<ROWS_ACC>(r, a, g.cap_p, &done))) return rc;
+        if (done) return IF_OK;
+    }
+    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, r.w.ctrl, x, y);
+    else k_mg_csr<1, 1><<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, r.w.ctrl, x, y);
+    IF_LAUNCH_CHECK();
     return IF_OK;
 }
 
@@ -379,6 +600,14 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
     // sub 1: out = R - K v ;  sub 2: out = v + omega (R - K v) / d
     auto apply = [&](int sub, double omega, const double* v, double* out) -> int {
         gm.omega = omega;
+        if (!wide) {       // the row-block kernel, if a stage for this level's tiles fits
+            bool done = false;
+            int rcc;
+            RowsArgs a{g.rowptr, g.col, g.sm, g.diag, g.n, v, R, v, out, omega, 0, 0, 0};
+            if (sub == 1) rcc = launch_rows<ROWS_RES>(r, a, g.cap_a, &done);
+            else rcc = launch_rows<ROWS_SWEEP>(r, a, g.cap_a, &done);
+            if (rcc != IF_OK || done) return rcc;
+        }
         if (sub == 1) {
             if (wide) k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
             else k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
@@ -411,17 +640,12 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
     }
     if ((rc = apply(1, 0.0, cur, spare[1]))) return rc;                // residual of the level
     double* const* nb = b.lev[l + 1];
-    const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse, wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
-    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, spare[1], nb[0]);
-    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, spare[1], nb[0]);
-    IF_LAUNCH_CHECK();
+    if ((rc = mg_restrict(r, g, spare[1], nb[0]))) return rc;
     if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
     double* ec = nullptr;
     if ((rc = mg_vcycle(r, b, l + 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
     if (l == 1 && tm && (rc = tm->mark(r.st, MGT_COARSE))) return rc;
-    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
-    else k_mg_csr<1, 1><<<grid1, BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
-    IF_LAUNCH_CHECK();
+    if ((rc = mg_prolong_add(r, g, ec, cur))) return rc;
     for (int k = 0; k < nu; ++k) {
         if ((rc = apply(2, om[nu - 1 - k], cur, spare[k & 1]))) return rc;
         std::swap(cur, spare[k & 1]);
@@ -462,18 +686,21 @@ int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const do
         if (tm && (rc = tm->mark(r.st, MGT_LAST))) return rc;
     }
     double* const* nb = b.lev[1];
-    const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse, wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
-    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, b.t, nb[0]);
-    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, ctrl, b.t, nb[0]);
-    IF_LAUNCH_CHECK();
+    if ((rc = mg_restrict(r, g, b.t, nb[0]))) return rc;
     if (tm && (rc = tm->mark(r.st, MGT_RESTRICT0))) return rc;
     double* ec = nullptr;
     if ((rc = mg_vcycle(r, b, 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
-    if (nu == 1 && mg_fused_prolongation(g))      // e = omega R/d formed again here: it has not been stored
-        k_mg_prolong0<<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, mg_mat(g), ctrl, ec, R0, R1, r_select, cur);
-    else if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
-    else k_mg_csr<1, 1><<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, ctrl, ec, cur);
-    IF_LAUNCH_CHECK();
+    if (nu == 1 && mg_fused_prolongation(g)) {    // e = omega R/d formed again here: it has not been stored
+        bool done = false;
+        RowsArgs a{g.p_rowptr, g.p_col, g.p_val, g.diag, g.n, ec, R0, R1, cur, g.omega, r_select, 0, 0};
+        if ((rc = launch_rows<ROWS_PROLONG0>(r, a, g.cap_p, &done))) return rc;
+        if (!done) {
+            k_mg_prolong0<<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, mg_mat(g), ctrl, ec, R0, R1, r_select, cur);
+            IF_LAUNCH_CHECK();
+        }
+    } else if ((rc = mg_prolong_add(r, g, ec, cur))) {
+        return rc;
+    }
     if (tm && (rc = tm->mark(r.st, MGT_PROLONG0))) return rc;
     // sweeps after the correction, dampings in reverse order (the cycle is symmetric); scratch: za, zb, t minus `out`
     for (int k = 0; k < nu - 1; ++k) {

@@ -1124,17 +1124,18 @@ extern "C" int if_load(const char* path, if_handle* out) {
             g.n = lh.n; g.nnz = lh.nnz; g.n_coarse = lh.n_coarse; g.p_nnz = lh.p_nnz;
             g.rho = lh.rho; g.rho_m = lh.rho_m; g.omega = lh.omega;
             h->mg_levels = l + 1;      // (if_destroy frees what has been read so far)
-            if ((rc = read_dev(f, (void**)&g.rowptr, (size_t)(g.n + 1) * 8, (size_t)(g.n + 1) * 8, buf))) return fail(rc);
-            if ((rc = read_dev(f, (void**)&g.col, (size_t)g.nnz * 4, (size_t)g.nnz * 4, buf))) return fail(rc);
-            if ((rc = read_dev(f, (void**)&g.sm, (size_t)g.nnz * 16, (size_t)g.nnz * 16, buf))) return fail(rc);
-            if ((rc = read_dev(f, (void**)&g.diag, (size_t)g.n * 16, (size_t)g.n * 16, buf))) return fail(rc);
+            // (+16: the row-block kernels of the cycle bulk-copy 16-byte multiples)
+            if ((rc = read_dev(f, (void**)&g.rowptr, (size_t)(g.n + 1) * 8, (size_t)(g.n + 1) * 8 + 16, buf))) return fail(rc);
+            if ((rc = read_dev(f, (void**)&g.col, (size_t)g.nnz * 4, (size_t)g.nnz * 4 + 16, buf))) return fail(rc);
+            if ((rc = read_dev(f, (void**)&g.sm, (size_t)g.nnz * 16, (size_t)g.nnz * 16 + 16, buf))) return fail(rc);
+            if ((rc = read_dev(f, (void**)&g.diag, (size_t)g.n * 16, (size_t)g.n * 16 + 16, buf))) return fail(rc);
             if (l + 1 < (int)L) {
-                if ((rc = read_dev(f, (void**)&g.p_rowptr, (size_t)(g.n + 1) * 8, (size_t)(g.n + 1) * 8, buf))) return fail(rc);
-                if ((rc = read_dev(f, (void**)&g.p_col, (size_t)g.p_nnz * 4, (size_t)g.p_nnz * 4, buf))) return fail(rc);
-                if ((rc = read_dev(f, (void**)&g.p_val, (size_t)g.p_nnz * 8, (size_t)g.p_nnz * 8, buf))) return fail(rc);
-                if ((rc = read_dev(f, (void**)&g.r_rowptr, (size_t)(g.n_coarse + 1) * 8, (size_t)(g.n_coarse + 1) * 8, buf))) return fail(rc);
-                if ((rc = read_dev(f, (void**)&g.r_col, (size_t)g.p_nnz * 4, (size_t)g.p_nnz * 4, buf))) return fail(rc);
-                if ((rc = read_dev(f, (void**)&g.r_val, (size_t)g.p_nnz * 8, (size_t)g.p_nnz * 8, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.p_rowptr, (size_t)(g.n + 1) * 8, (size_t)(g.n + 1) * 8 + 16, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.p_col, (size_t)g.p_nnz * 4, (size_t)g.p_nnz * 4 + 16, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.p_val, (size_t)g.p_nnz * 8, (size_t)g.p_nnz * 8 + 16, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.r_rowptr, (size_t)(g.n_coarse + 1) * 8, (size_t)(g.n_coarse + 1) * 8 + 16, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.r_col, (size_t)g.p_nnz * 4, (size_t)g.p_nnz * 4 + 16, buf))) return fail(rc);
+                if ((rc = read_dev(f, (void**)&g.r_val, (size_t)g.p_nnz * 8, (size_t)g.p_nnz * 8 + 16, buf))) return fail(rc);
             }
         }
     }
@@ -1147,7 +1148,7 @@ extern "C" int if_load(const char* path, if_handle* out) {
         if_destroy(h);
         return IF_ENOMEM;
     }
-    if (ifl::na_setup(h) != IF_OK) { if_destroy(h); return IF_ECUDA; }
+    if (ifl::na_setup(h) != IF_OK || ifl::mg_tile_caps(h) != IF_OK) { if_destroy(h); return IF_ECUDA; }
     *out = h;
     return IF_OK;
 }
