@@ -6,6 +6,8 @@ returns the wave parameters so a test can evaluate closed forms for them.
 """
 from __future__ import annotations
 
+import os
+from concurrent.futures import ThreadPoolExecutor
 from dataclasses import dataclass
 
 import numpy as np
@@ -19,27 +21,54 @@ class Waves:
     scale: float         # phase = scale * (k . x) + theta
 
 
+def _cos_phases(x, kt, theta):
+    """cos(x . k_j + theta_j) for a chunk of points x [m][dim] and wavevectors kt [dim][J]: elementwise operations only."""
+    ph = np.multiply.outer(x[:, 0], kt[0])
+    for d in range(1, x.shape[1]):
+        ph += np.multiply.outer(x[:, d], kt[d])
+    ph += theta
+    np.cos(ph, out=ph)
+    return ph
+
+
+def _eval_chunk(coords, kt, theta, amp, out, s, e):
+    c = _cos_phases(coords[s:e], kt, theta)
+    c *= amp
+    out[s:e] = c.sum(axis=1)
+
+
+_EVAL_STEP = 2048        # vertices per chunk: fixed, so that the arithmetic does not depend on the number of threads
+
+
 def _eval_waves(coords: np.ndarray, w: Waves) -> np.ndarray:
-    """phi(x) = sum_j amp_j cos(scale * k_j.x + theta_j), chunked over vertices."""
+    """phi(x) = sum_j amp_j cos(scale * k_j.x + theta_j).
+
+    Bit-reproducible from run to run: every value is a fixed sequence of elementwise numpy operations (products and sums
+    of the phase in coordinate order, cos, the weighted sum over the waves in numpy's fixed pairwise order) on chunks of
+    a fixed size; threads only share out the chunks.  No BLAS and no multithreaded library kernel is involved: an
+    earlier form (torch CPU matmul / cos_) gave fields that differed by 1e-10 in a few percent of processes on a
+    16-thread host, which showed as changed iteration counts on the finite-termination case of config 1."""
+    coords = np.ascontiguousarray(coords, dtype=np.float64)
     out = np.empty(coords.shape[0], dtype=np.float64)
     kt = np.ascontiguousarray(w.k.T.astype(np.float64)) * w.scale
+    theta = np.ascontiguousarray(w.theta, dtype=np.float64)
+    amp = np.ascontiguousarray(w.amp, dtype=np.float64)
+    starts = range(0, coords.shape[0], _EVAL_STEP)
     try:
-        import torch
-        ktt = torch.from_numpy(kt)
-        th = torch.from_numpy(w.theta)
-        am = torch.from_numpy(w.amp)
-        xs = torch.from_numpy(np.ascontiguousarray(coords))
-        o = torch.from_numpy(out)
-        step = 1 << 16
-        for s in range(0, coords.shape[0], step):
-            ph = xs[s:s + step] @ ktt
-            ph += th
-            torch.cos_(ph)
-            o[s:s + step] = ph @ am
-    except ImportError:  # pragma: no cover - numpy path gives the same numbers to rounding
-        step = 1 << 15
-        for s in range(0, coords.shape[0], step):
-            out[s:s + step] = np.cos(coords[s:s + step] @ kt + w.theta) @ w.amp
+        n_threads = len(os.sched_getaffinity(0))
+    except AttributeError:  # pragma: no cover
+        n_threads = os.cpu_count() or 1
+    n_threads = max(1, min(n_threads, 32, len(starts)))
+
+    def run(s):
+        _eval_chunk(coords, kt, theta, amp, out, s, min(s + _EVAL_STEP, coords.shape[0]))
+
+    if n_threads == 1:
+        for s in starts:
+            run(s)
+    else:
+        with ThreadPoolExecutor(n_threads) as pool:
+            list(pool.map(run, starts))
     return out
 
 
@@ -109,8 +138,11 @@ def sphere_velocity_field(coords: np.ndarray, kmax: int, n_waves: int, rng: np.r
     axis = rng.normal(size=3)
     axis /= np.linalg.norm(axis)
     U = np.cross(axis[None, :], coords)
-    step = 1 << 15
-    for s in range(0, coords.shape[0], step):
-        U[s:s + step] += (np.cos(coords[s:s + step] @ k.T + theta) * amp) @ b
+    kt = np.ascontiguousarray(k.T)
+    for s in range(0, coords.shape[0], _EVAL_STEP):        # same fixed-order elementwise evaluation as _eval_waves
+        c = _cos_phases(coords[s:s + _EVAL_STEP], kt, theta)
+        c *= amp
+        for d in range(3):
+            U[s:s + _EVAL_STEP, d] += (c * b[:, d]).sum(axis=1)
     east, north = sphere_frames(coords)
     return np.einsum("ij,ij->i", U, east), np.einsum("ij,ij->i", U, north)
