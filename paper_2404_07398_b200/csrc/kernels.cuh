@@ -212,6 +212,102 @@ __device__ __forceinline__ bool grid_reduce(const double2 (&acc)[NV], double* __
     return true;
 }
 
+// Fixed-order grid reduction for the kernels in which a thread owns ROWS and carries one accumulator per column (the
+// start and the end of a column: few columns of the K are touched, so threads are spread over rows, not over column
+// pairs).  Per column in `mask`: xor tree inside a warp, the warps in order, partials[block][K], a ticket, and the last
+// block adds the blocks' partial sums as grid_reduce does.  Returns true in the last block with the totals in tot[c].
+template <int K, int NT = BLOCK>
+__device__ __forceinline__ bool grid_reduce_cols(const double (&acc)[K], unsigned mask, double* __restrict__ partials,
+                                                 unsigned int* ticket, double* tot /* shared [KMAX] */) {
+    __shared__ double wsum[NT / 32][K];
+    __shared__ double redd[NT];
+    __shared__ bool is_last;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int c = 0; c < K; ++c) {
+        if (!((mask >> c) & 1u)) continue;
+        double s = acc[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) wsum[warp][c] = s;
+    }
+    __syncthreads();
+    if (tid < K) {
+        double s = 0.0;
+        if ((mask >> tid) & 1u)
+            for (int w = 0; w < NT / 32; ++w) s += wsum[w][tid];
+        partials[(size_t)blockIdx.x * K + tid] = s;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        unsigned int t = atomicAdd(ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    __threadfence();
+    constexpr int LANES = NT / K;                  // threads per column
+    const int c = tid % K, ln = tid / K;
+    double s = 0.0;
+    for (unsigned b = ln; b < gridDim.x; b += LANES) s += __ldcg(&partials[(size_t)b * K + c]);
+    redd[tid] = s;
+    __syncthreads();
+    if (tid < K) {
+        double t = 0.0;
+        for (int i = 0; i < LANES; ++i) t += redd[i * K + tid];
+        tot[tid] = t;
+    }
+    __syncthreads();
+    if (tid == 0) *ticket = 0u;
+    return true;
+}
+
+// Fixed-order grid reduction for k_mg_start: thread tid keeps column pair `pair` (slot tid % PP of the compacted pair
+// list, PP a power of two, slots >= P idle).  Per slot the threads are added in thread order, partials[block][K], a
+// ticket, and the last block adds the blocks' partial sums as grid_reduce does (columns of idle pairs come out as 0).
+template <int K, int NT = BLOCK>
+__device__ __forceinline__ bool grid_reduce_pairs(double2 acc, int PP, int P, int pair, double* __restrict__ partials,
+                                                  unsigned int* ticket, double* tot /* shared [KMAX] */) {
+    __shared__ double2 red[NT];
+    __shared__ bool is_last;
+    const int tid = threadIdx.x;
+    red[tid] = acc;
+    if (tid < K) partials[(size_t)blockIdx.x * K + tid] = 0.0;
+    __syncthreads();
+    if (tid < P) {
+        double2 s = red[tid];
+        for (int i = tid + PP; i < NT; i += PP) { s.x += red[i].x; s.y += red[i].y; }
+        partials[(size_t)blockIdx.x * K + 2 * pair] = s.x;
+        partials[(size_t)blockIdx.x * K + 2 * pair + 1] = s.y;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        unsigned int t = atomicAdd(ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    __threadfence();
+    double* redd = reinterpret_cast<double*>(red);
+    constexpr int LANES = NT / K;                  // threads per column
+    const int c = tid % K, ln = tid / K;
+    double s = 0.0;
+    for (unsigned b = ln; b < gridDim.x; b += LANES) s += __ldcg(&partials[(size_t)b * K + c]);
+    __syncthreads();
+    redd[tid] = s;
+    __syncthreads();
+    if (tid < K) {
+        double t = 0.0;
+        for (int i = 0; i < LANES; ++i) t += redd[i * K + tid];
+        tot[tid] = t;
+    }
+    __syncthreads();
+    if (tid == 0) *ticket = 0u;
+    return true;
+}
+
 // CG bookkeeping after z = B r (run by the last block of a grid reduction; tot = rho' per column, then ||r||^2):
 // beta = rho'/rho, stop test, iteration count -- the same rules as the tail of k_update.  A column that was
 // (re)started (Ctrl::starting, k_mg_start) has just had r0 and z0 = B r0 formed: rho = rho', beta = 0, nothing counted.
@@ -929,34 +1025,72 @@ __global__ void __launch_bounds__(BLOCK) k_mg_start(MeshView m, Ctrl* __restrict
                                                     double* __restrict__ x, double* __restrict__ z,
                                                     double* __restrict__ r0, double* __restrict__ r1,
                                                     double* __restrict__ p0, double* __restrict__ p1) {
+    // Mostly one to four of the K columns start at a time.  Measured on B200 (7.3 M rows, four vectors): 8-byte stores
+    // that miss in L2 are not merged -- each becomes its own 32-byte read-modify-write in DRAM (0.72 ms for one
+    // column, 4.7 ms for sixteen) -- while 16-byte updates of lines loaded first cost about 1.1 ms for any mask when only
+    // the lanes of the masked pairs work.  So: 16-byte read-modify-write with the masked column PAIRS compacted, P of
+    // them padded to a power of two PP: a thread keeps one pair and walks rows, every thread works; pairs with both
+    // columns starting are stored without a load; of the two direction buffers only p[cur_p] -- the one kernel A reads
+    // as the old direction -- is cleared (kernel A writes the other one in full).
     constexpr int TPR = K / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    const int tid = threadIdx.x, l = tid % TPR;
-    const bool on0 = (mask >> (2 * l)) & 1u, on1 = (mask >> (2 * l + 1)) & 1u;
+    constexpr int U = 2;
+    __shared__ int s_pair[TPR];
+    __shared__ int s_np;
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        int n = 0;
+        for (int l = 0; l < TPR; ++l)
+            if ((mask >> (2 * l)) & 3u) s_pair[n++] = l;
+        s_np = n;
+    }
+    __syncthreads();
+    const int P = s_np;
+    const int PP = P <= 1 ? 1 : P <= 2 ? 2 : P <= 4 ? 4 : P <= 8 ? 8 : TPR;
+    const int j = tid & (PP - 1);
+    const bool active = j < P;
+    const int l = active ? s_pair[j] : 0;
+    const bool on0 = active && ((mask >> (2 * l)) & 1u), on1 = active && ((mask >> (2 * l + 1)) & 1u);
     const int f0 = sp.field[2 * l], f1 = sp.field[2 * l + 1];
     double* __restrict__ r = ctrl->cur_r ? r1 : r0;
-    double2 acc[1] = {{0.0, 0.0}};
-    if (on0 || on1) {
-        for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < m.nv; row += (int64_t)gridDim.x * ROWS) {
-            const int64_t ri = row * K + 2 * l;
-            const double av = m.area[row];
-            const int64_t u = m.perm[row];
-            double2 xv = ld2(x, ri), zv = ld2(z, ri), rv = ld2(r, ri), pa = ld2(p0, ri), pb = ld2(p1, ri);
-            if (on0) {
-                const double phi = f0 >= 0 ? fields[(int64_t)f0 * m.nv + u] : 0.0;
-                xv.x = 0.0; zv.x = phi; rv.x = av * phi; pa.x = 0.0; pb.x = 0.0;
-                acc[0].x = fma(rv.x, rv.x, acc[0].x);
+    double* __restrict__ p = ctrl->cur_p ? p1 : p0;
+    double2 acc = {0.0, 0.0};
+    if (active) {
+        const int rows_blk = BLOCK / PP;
+        const int64_t stride = (int64_t)gridDim.x * rows_blk;
+        const bool both = on0 && on1;
+        for (int64_t base = (int64_t)blockIdx.x * rows_blk + tid / PP; base < m.nv; base += U * stride) {
+            double2 xv[U], zv[U], rv[U], pv[U];
+            double av[U], ph0[U], ph1[U];
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const int64_t row = base + i * stride;
+                if (row >= m.nv) continue;
+                const int64_t ri = row * K + 2 * l;
+                if (!both) { xv[i] = ld2(x, ri); zv[i] = ld2(z, ri); rv[i] = ld2(r, ri); pv[i] = ld2(p, ri); }
+                av[i] = m.area[row];
+                const int64_t u = m.perm[row];
+                ph0[i] = (on0 && f0 >= 0) ? fields[(int64_t)f0 * m.nv + u] : 0.0;
+                ph1[i] = (on1 && f1 >= 0) ? fields[(int64_t)f1 * m.nv + u] : 0.0;
             }
-            if (on1) {
-                const double phi = f1 >= 0 ? fields[(int64_t)f1 * m.nv + u] : 0.0;
-                xv.y = 0.0; zv.y = phi; rv.y = av * phi; pa.y = 0.0; pb.y = 0.0;
-                acc[0].y = fma(rv.y, rv.y, acc[0].y);
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const int64_t row = base + i * stride;
+                if (row >= m.nv) continue;
+                const int64_t ri = row * K + 2 * l;
+                if (on0) {
+                    xv[i].x = 0.0; zv[i].x = ph0[i]; rv[i].x = av[i] * ph0[i]; pv[i].x = 0.0;
+                    acc.x = fma(rv[i].x, rv[i].x, acc.x);
+                }
+                if (on1) {
+                    xv[i].y = 0.0; zv[i].y = ph1[i]; rv[i].y = av[i] * ph1[i]; pv[i].y = 0.0;
+                    acc.y = fma(rv[i].y, rv[i].y, acc.y);
+                }
+                st2(x, ri, xv[i]); st2(z, ri, zv[i]); st2(r, ri, rv[i]); st2(p, ri, pv[i]);
             }
-            st2(x, ri, xv); st2(z, ri, zv); st2(r, ri, rv); st2(p0, ri, pa); st2(p1, ri, pb);
         }
     }
     __shared__ double tot[KMAX];
-    if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[1], tot)) {
+    if (grid_reduce_pairs<K>(acc, PP, P, l, partials, &ctrl->ticket[1], tot)) {
         if (tid < K && ((mask >> tid) & 1u)) {
             const int ta = ctrl->pair_mode ? (tid & ~1) : tid, tb = ctrl->pair_mode ? (tid | 1) : tid;
             const double bb = (ctrl->pair_mode ? 1.0 : 0.5) * (tot[ta] + tot[tb]);
@@ -1061,24 +1195,41 @@ __global__ void __launch_bounds__(BLOCK) k_energy(MeshView m, Ctrl* __restrict__
                                                   unsigned mask, const double* __restrict__ x,
                                                   const double* __restrict__ pa, const double* __restrict__ pb,
                                                   double total_area, double* __restrict__ energy) {
-    constexpr int TPR = K / 2;
-    constexpr int ROWS = BLOCK / TPR;
-    const int tid = threadIdx.x, l = tid % TPR;
+    // as k_mg_start: a thread owns rows and loops over the columns in `mask`
+    constexpr int U = 2;
+    const int tid = threadIdx.x;
     const double* __restrict__ p = ctrl->cur_p ? pb : pa;
-    const double2 alpha = ld2(ctrl->alpha, 2 * l);
-    double2 acc[1] = {{0.0, 0.0}};
-    if ((mask >> (2 * l)) & 3u) {
-        for (int64_t row = (int64_t)blockIdx.x * ROWS + tid / TPR; row < m.nv; row += (int64_t)gridDim.x * ROWS) {
-            const int64_t ri = row * K + 2 * l;
-            const double av = m.area[row];
-            const double2 xv = ld2(x, ri), pv = ld2(p, ri);
-            const double2 xf = {fma(alpha.x, pv.x, xv.x), fma(alpha.y, pv.y, xv.y)};
-            acc[0].x = fma(av * xf.x, xf.x, acc[0].x);
-            acc[0].y = fma(av * xf.y, xf.y, acc[0].y);
+    __shared__ double s_alpha[KMAX];
+    if (tid < KMAX) s_alpha[tid] = ctrl->alpha[tid];
+    __syncthreads();
+    double acc[K];
+#pragma unroll
+    for (int c = 0; c < K; ++c) acc[c] = 0.0;
+    const int64_t stride = (int64_t)gridDim.x * BLOCK;
+    for (int64_t base = (int64_t)blockIdx.x * BLOCK + tid; base < m.nv; base += U * stride) {
+        double av[U];
+#pragma unroll
+        for (int i = 0; i < U; ++i) av[i] = base + i * stride < m.nv ? m.area[base + i * stride] : 0.0;
+#pragma unroll
+        for (int c = 0; c < K; ++c) {
+            if (!((mask >> c) & 1u)) continue;
+            double xv[U], pv[U];
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const int64_t row = base + i * stride;
+                const bool ok = row < m.nv;
+                xv[i] = ok ? x[row * K + c] : 0.0;
+                pv[i] = ok ? p[row * K + c] : 0.0;
+            }
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const double xf = fma(s_alpha[c], pv[i], xv[i]);
+                acc[c] = fma(av[i] * xf, xf, acc[c]);
+            }
         }
     }
     __shared__ double tot[KMAX];
-    if (grid_reduce<K, 1>(acc, partials, &ctrl->ticket[3], tot)) {
+    if (grid_reduce_cols<K>(acc, mask, partials, &ctrl->ticket[3], tot)) {
         if (tid < K && ((mask >> tid) & 1u) && ctrl->field[tid] >= 0)
             energy[ctrl->rhs[tid]] = 0.5 * tot[tid] / total_area;
     }
