@@ -106,7 +106,10 @@ typedef struct {
                         iteration for n = 1, the product V M V of two cycles for n = 2 (needs batch = 16 and a handle
                         prepared with IF_FLAG_MULTIGRID, else ignored); the rest by Jacobi-PCG.  Same systems, same
                         start vector, same stop test, same answers within the tolerance (PAPER.md:207 names the
-                        convergence of plain CG at large scales, above all for n = 2, as the open problem)           */
+                        convergence of plain CG at large scales, above all for n = 2, as the open problem).  On
+                        meshes of 400 000 vertices or more (n = 2: 100 000) the stream ends and starts its columns on
+                        the device, inside each iteration's CUDA graph; the host only launches graphs and reads a
+                        16-byte snapshot one launch behind (environment IF_MG_HOST_REFILL = 0 / 1 forces either way) */
     double radius;     /* if_prepare with IF_FLAG_VECTOR: R_e of the metric terms; 0 => the mean |x_v| of a dim = 3 mesh    */
     double mg_min_ell; /* 0 => 0.5 (in mean edge lengths; right-hand sides below that stay on the Jacobi path)         */
 } if_options;

@@ -55,6 +55,20 @@ __device__ __forceinline__ const double* jacobi_diag(const MeshView& m, int orde
     return order_n == 1 ? m.sdiag : order_n == 2 ? m.gdiag : order_n == 3 ? m.gdiag3 : m.gdiag4;
 }
 
+// per-column parameters of a (re)start, passed by value to k_init
+struct StartParams {
+    double c[KMAX];
+    double c1[KMAX];      // multigrid path (see Ctrl::c1)
+    int field[KMAX];
+    int rhs[KMAX];
+};
+
+// one right-hand side of the device-side queue (multigrid stream with the column turnover on the device)
+struct QEntry {
+    double c, c1;
+    int field, rhs;
+};
+
 struct Ctrl {
     double c[KMAX];       // gamma l^(2n)
     double alpha[KMAX];
@@ -81,6 +95,13 @@ struct Ctrl {
     double tol2;
     long long total_iters;   // fused iterations executed while some column was active
     unsigned int ticket[4];
+    // column turnover on the device (multigrid stream, k_turn_plan): the queue position, which columns hold a
+    // right-hand side, what this iteration's turnover finalises and starts, and what the host reads back
+    int q_next, q_total;
+    int occupied[KMAX];
+    unsigned int turn_fin, turn_start;
+    StartParams turn_sp;
+    int snap[4];          // {columns holding a right-hand side, of those still running, q_next, 0} after the turnover
 };
 
 // what the host reads back every check_every iterations
@@ -89,13 +110,9 @@ struct Snapshot {
     int epoch[KMAX];
 };
 
-// per-column parameters of a (re)start, passed by value to k_init
-struct StartParams {
-    double c[KMAX];
-    double c1[KMAX];      // multigrid path (see Ctrl::c1)
-    int field[KMAX];
-    int rhs[KMAX];
-};
+// mask arguments of the start / end-of-column kernels: these values mean "what k_turn_plan left in the control block"
+constexpr unsigned MASK_TURN_FIN = 0x80000000u;     // ctrl->turn_fin
+constexpr unsigned MASK_TURN_START = 0x40000000u;   // ctrl->turn_start, parameters from ctrl->turn_sp
 
 enum Mode { MODE_PLAIN = 0, MODE_CG1 = 1, MODE_CG2A = 2, MODE_CG2B = 3, MODE_AX = 4, MODE_MGR = 5, MODE_MGR0 = 6 };
 // MODE_AX (multigrid path, level 0): v = in0 (gathered), r = in1 (own rows), K = M + c1 S per column (Ctrl::c1), and with
@@ -1037,6 +1054,9 @@ __global__ void __launch_bounds__(BLOCK) k_mg_start(MeshView m, Ctrl* __restrict
     __shared__ int s_pair[TPR];
     __shared__ int s_np;
     const int tid = threadIdx.x;
+    const bool dev = mask == MASK_TURN_START;      // turnover on the device: mask and parameters from k_turn_plan
+    if (dev) mask = ctrl->turn_start;
+    if (mask == 0u) return;
     if (tid == 0) {
         int n = 0;
         for (int l = 0; l < TPR; ++l)
@@ -1050,7 +1070,8 @@ __global__ void __launch_bounds__(BLOCK) k_mg_start(MeshView m, Ctrl* __restrict
     const bool active = j < P;
     const int l = active ? s_pair[j] : 0;
     const bool on0 = active && ((mask >> (2 * l)) & 1u), on1 = active && ((mask >> (2 * l + 1)) & 1u);
-    const int f0 = sp.field[2 * l], f1 = sp.field[2 * l + 1];
+    const int f0 = dev ? ctrl->turn_sp.field[2 * l] : sp.field[2 * l];
+    const int f1 = dev ? ctrl->turn_sp.field[2 * l + 1] : sp.field[2 * l + 1];
     double* __restrict__ r = ctrl->cur_r ? r1 : r0;
     double* __restrict__ p = ctrl->cur_p ? p1 : p0;
     double2 acc = {0.0, 0.0};
@@ -1094,12 +1115,16 @@ __global__ void __launch_bounds__(BLOCK) k_mg_start(MeshView m, Ctrl* __restrict
         if (tid < K && ((mask >> tid) & 1u)) {
             const int ta = ctrl->pair_mode ? (tid & ~1) : tid, tb = ctrl->pair_mode ? (tid | 1) : tid;
             const double bb = (ctrl->pair_mode ? 1.0 : 0.5) * (tot[ta] + tot[tb]);
-            ctrl->c[tid] = sp.c[tid]; ctrl->c1[tid] = sp.c1[tid]; ctrl->field[tid] = sp.field[tid]; ctrl->rhs[tid] = sp.rhs[tid];
+            const int fld = dev ? ctrl->turn_sp.field[tid] : sp.field[tid];
+            ctrl->c[tid] = dev ? ctrl->turn_sp.c[tid] : sp.c[tid];
+            ctrl->c1[tid] = dev ? ctrl->turn_sp.c1[tid] : sp.c1[tid];
+            ctrl->field[tid] = fld;
+            ctrl->rhs[tid] = dev ? ctrl->turn_sp.rhs[tid] : sp.rhs[tid];
             ctrl->rho[tid] = 0.0; ctrl->rr[tid] = bb; ctrl->bb[tid] = bb;
             ctrl->alpha[tid] = 0.0; ctrl->beta[tid] = 0.0; ctrl->iters[tid] = 0;
             ctrl->status[tid] = isfinite(bb) ? 0 : 2;
             ctrl->epoch[tid] = ctrl->epoch[tid] + 1;
-            ctrl->done[tid] = (sp.field[tid] < 0 || !isfinite(bb)) ? 1 : 0;
+            ctrl->done[tid] = (fld < 0 || !isfinite(bb)) ? 1 : 0;
             ctrl->starting[tid] = ctrl->done[tid] ? 0 : 1;
         }
         __syncthreads();
@@ -1198,6 +1223,8 @@ __global__ void __launch_bounds__(BLOCK) k_energy(MeshView m, Ctrl* __restrict__
     // as k_mg_start: a thread owns rows and loops over the columns in `mask`
     constexpr int U = 2;
     const int tid = threadIdx.x;
+    if (mask == MASK_TURN_FIN) mask = ctrl->turn_fin;
+    if (mask == 0u) return;
     const double* __restrict__ p = ctrl->cur_p ? pb : pa;
     __shared__ double s_alpha[KMAX];
     if (tid < KMAX) s_alpha[tid] = ctrl->alpha[tid];
@@ -1245,6 +1272,8 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(MeshView m, const Ctrl* __res
     __shared__ double tile[K][33];
     __shared__ int32_t dst[32];
     const int tid = threadIdx.x;
+    if (mask == MASK_TURN_FIN) mask = ctrl->turn_fin;
+    if (mask == 0u) return;
     const double* __restrict__ p = ctrl->cur_p ? pb : pa;
     // BLOCK threads move 32 rows x K columns per step
     for (int64_t base = (int64_t)blockIdx.x * 32; base < m.nv; base += (int64_t)gridDim.x * 32) {
@@ -1315,6 +1344,53 @@ __global__ void k_stats(const Ctrl* __restrict__ ctrl, int K, unsigned mask, int
         iters[r] = ctrl->iters[c];
         status[r] = ctrl->status[c];
         relres[r] = ctrl->bb[c] > 0.0 ? sqrt(ctrl->rr[c] / ctrl->bb[c]) : 0.0;
+    }
+}
+
+// Column turnover on the device (multigrid stream; one thread, at the end of every iteration's graph): the columns that
+// hold a right-hand side and have stopped are to be finalised (turn_fin); every free column takes the next entry of
+// the queue (turn_start, turn_sp).  The kernels that follow in the same graph -- k_energy or k_scatter,
+// k_mg_start, k_mg_coarse_factor -- read these masks and return at once when they are empty, so a stopped column is
+// running its next right-hand side in the very next iteration and the host only watches `snap`.
+// `first` (before the first iteration): every column is started -- those the queue has nothing for as empty columns
+// (zeroed, stopped at once), so that no kernel ever reads what the workspace held before.
+__global__ void k_turn_plan(Ctrl* __restrict__ ctrl, const QEntry* __restrict__ queue, int K, int first,
+                            int32_t* __restrict__ iters, int32_t* __restrict__ status, double* __restrict__ relres) {
+    // one warp, lane c = column c: masks by ballot, the queue position of a free column = its rank among the free ones
+    const unsigned full = 0xffffffffu;
+    const int c = threadIdx.x;
+    const bool in = c < K;
+    const int occ0 = in ? ctrl->occupied[c] : 0;
+    const int dn = in ? ctrl->done[c] : 1;
+    const int next = ctrl->q_next, total = ctrl->q_total;
+    const bool fin_c = occ0 && dn;
+    if (fin_c) {                                 // the per-right-hand-side results (k_stats of the host-driven refill)
+        const int r = ctrl->rhs[c];
+        iters[r] = ctrl->iters[c];
+        status[r] = ctrl->status[c];
+        relres[r] = ctrl->bb[c] > 0.0 ? sqrt(ctrl->rr[c] / ctrl->bb[c]) : 0.0;
+    }
+    const bool free_c = in && (!occ0 || fin_c);
+    const unsigned fin = __ballot_sync(full, fin_c);
+    const unsigned freem = __ballot_sync(full, free_c);
+    const int rank = __popc(freem & ((1u << c) - 1u));
+    const bool take = free_c && next + rank < total;
+    const bool occ = (occ0 && !fin_c) || take;
+    if (in) {
+        QEntry e = {0.0, 0.0, -1, 0};
+        if (take) e = queue[next + rank];
+        ctrl->turn_sp.c[c] = e.c; ctrl->turn_sp.c1[c] = e.c1; ctrl->turn_sp.field[c] = e.field; ctrl->turn_sp.rhs[c] = e.rhs;
+        ctrl->occupied[c] = occ ? 1 : 0;
+    }
+    const unsigned start = __ballot_sync(full, take || (first && free_c));
+    const unsigned occm = __ballot_sync(full, occ);
+    const unsigned runm = __ballot_sync(full, occ && (take || !dn));
+    const unsigned takem = __ballot_sync(full, take);
+    if (c == 0) {
+        ctrl->q_next = next + __popc(takem);
+        ctrl->turn_fin = fin;
+        ctrl->turn_start = start;
+        ctrl->snap[0] = __popc(occm); ctrl->snap[1] = __popc(runm); ctrl->snap[2] = next + __popc(takem); ctrl->snap[3] = 0;
     }
 }
 

@@ -397,6 +397,7 @@ __global__ void __launch_bounds__(64) k_mg_coarse_factor(MgMat g, const Ctrl* __
     double (*a)[MG_COARSEST + 1] = reinterpret_cast<double (*)[MG_COARSEST + 1]>(coarse_sm);
     double (*li)[MG_COARSEST + 1] = reinterpret_cast<double (*)[MG_COARSEST + 1]>(coarse_sm + MG_COARSEST * (MG_COARSEST + 1));
     const int c = blockIdx.x, t = threadIdx.x, n = (int)g.n;
+    if (mask == MASK_TURN_START) mask = ctrl->turn_start;
     if (!((mask >> c) & 1u)) return;
     const double cc = ctrl->c1[c];
     for (int i = t; i < n; i += 64)

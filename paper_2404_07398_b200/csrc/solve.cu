@@ -13,6 +13,7 @@ namespace ifl {
 namespace {
 
 constexpr int MAX_RHS = 65536;
+constexpr int64_t MG_DEVICE_TURNOVER_ROWS = 400000;   // see solve_all
 constexpr int MAX_BLOCKS_PER_SM = 8;
 
 struct Workspace {
@@ -21,6 +22,7 @@ struct Workspace {
     double *x, *z, *p0, *p1, *q, *t, *t2;
     double *energy, *relres, *ells, *k_mid, *E, *epair;
     int32_t *iters, *status;
+    QEntry* queue;    // right-hand sides of the multigrid stream, read by the turnover on the device (k_turn_plan)
     void* mg_extra;   // buffers of the multigrid path (mg_solve.cuh), NULL if the handle has no hierarchy
     size_t bytes;
 };
@@ -53,7 +55,11 @@ Workspace layout_workspace(const if_mesh_s* h, int order_n, int batch, void* bas
     w.iters = (int32_t*)take(MAX_RHS * sizeof(int32_t));
     w.status = (int32_t*)take(MAX_RHS * sizeof(int32_t));
     w.mg_extra = nullptr;
-    if (batch == KMAX && h->mg_levels > 1) w.mg_extra = take(mg_extra_bytes(h, order_n));
+    w.queue = nullptr;
+    if (batch == KMAX && h->mg_levels > 1) {
+        w.queue = (QEntry*)take(MAX_RHS * sizeof(QEntry));
+        w.mg_extra = take(mg_extra_bytes(h, order_n));
+    }
     w.bytes = off;
     return w;
 }
@@ -602,11 +608,148 @@ int solve_from(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& 
     return IF_ECUDA;
 }
 
+// End and start of columns inside the stream (multigrid path): what k_turn_plan decided is carried out by the same
+// kernels the host-driven refill uses, with their masks read from the control block.
+int mg_enqueue_turnover(const Run& r, Job job, double* d_out, const double* d_fields, bool first = false) {
+    const if_mesh_s* h = r.h;
+    const MgBuffers b = mg_layout(h, r.w, r.order_n);
+    k_turn_plan<<<1, 32, 0, r.st>>>(r.w.ctrl, r.w.queue, MGK, first ? 1 : 0, r.w.iters, r.w.status, r.w.relres);
+    IF_LAUNCH_CHECK();
+    if (job == JOB_SPECTRUM) {
+        k_energy<MGK><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1,
+                                                      h->total_area, r.w.energy);
+    } else {
+        const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
+        k_scatter<MGK><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1, 1, d_out, d_fields,
+                                                  (r.opt.flags & IF_FLAG_HIGHPASS) ? 1 : 0);
+    }
+    IF_LAUNCH_CHECK();
+    StartParams none;
+    memset(&none, 0, sizeof(none));
+    k_mg_start<MGK><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, none, MASK_TURN_START, d_fields, b.x, b.zb,
+                                                    b.r[0], b.r[1], b.p[0], b.p[1]);
+    IF_LAUNCH_CHECK();
+    const MgLevel& gl = h->mg[h->mg_levels - 1];
+    if (gl.n <= MG_COARSEST) {
+        k_mg_coarse_factor<<<MGK, 64, MG_FACTOR_SMEM, r.st>>>(mg_mat(gl), r.w.ctrl, MASK_TURN_START, b.coarse_inv);
+        IF_LAUNCH_CHECK();
+    }
+    return IF_OK;
+}
+
+// The multigrid stream with the column turnover on the device: the queue of right-hand sides lives in the workspace,
+// one CUDA graph = one iteration + the turnover, and the host only launches graphs and reads, one launch behind, how
+// many columns still hold a right-hand side.  A stopped column runs its next right-hand side in the very next iteration
+// (the host-driven refill of solve_phase, which sees a stop one launch late, loses an iteration per right-hand side).
+int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
+                        PollState& poll, KernelTimes* times) {
+    int rc;
+    if ((rc = setup_grids<MGK>(r))) return rc;
+    if ((rc = mg_setup(r))) return rc;
+    const size_t R = rhs.size();
+    if (R == 0 || R > (size_t)MAX_RHS || !r.w.queue) return IF_EINVAL;
+    std::vector<QEntry> hq(R);
+    for (size_t i = 0; i < R; ++i) {
+        const Rhs& s = rhs[i];
+        hq[i].c = r.opt.gamma * std::pow(s.ell, 2.0 * r.order_n);
+        hq[i].c1 = r.order_n == 1 ? hq[i].c : std::sqrt(hq[i].c);   // K = M + sqrt(c) S (mg_solve.cuh)
+        hq[i].field = s.f;
+        hq[i].rhs = s.f * n_ells + s.j;
+    }
+    Ctrl hc = fresh_ctrl(r);
+    hc.q_next = 0;
+    hc.q_total = (int)R;
+    // (pageable sources: both copies are staged by the runtime before the call returns)
+    IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
+    IF_CUDA_TRY(cudaMemcpyAsync(r.w.queue, hq.data(), R * sizeof(QEntry), cudaMemcpyHostToDevice, r.st));
+    if ((rc = mg_enqueue_turnover(r, job, d_out, d_fields, true))) return rc;      // the first MGK right-hand sides
+
+    long long launches_per_graph = 0;
+    GraphSet gs;
+    if (r.st != nullptr && r.st != cudaStreamLegacy) {
+        for (int gi = 0; gi < 2; ++gi) {
+            if (gs.tev[gi].create() != IF_OK) return IF_ECUDA;
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(r.st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+                cudaGetLastError();   // stream cannot be captured: direct launches below
+                break;
+            }
+            const long long before = g_launches.load();
+            int rcc = mg_enqueue_iteration(r, &gs.tev[gi]);
+            if (rcc == IF_OK) rcc = mg_enqueue_turnover(r, job, d_out, d_fields);
+            launches_per_graph = g_launches.load() - before;
+            g_launches -= launches_per_graph;   // captured, not launched
+            cudaError_t e = cudaStreamEndCapture(r.st, &graph);
+            if (rcc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
+            e = cudaGraphInstantiate(&gs.exec[gi], graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { gs.exec[gi] = nullptr; cudaGetLastError(); return IF_ECUDA; }
+        }
+    }
+    const bool use_graph = gs.exec[0] && gs.exec[1];
+    const int64_t max_loops = ((int64_t)(R + MGK - 1) / MGK + 1) * ((int64_t)r.opt.max_iter + 3) + 8;
+    int* snap = reinterpret_cast<int*>(poll.snap);      // four slots of four ints in the pinned snapshot buffer
+    bool finished = false;
+    int running_before = 0;
+    for (int64_t it = 0; it < max_loops && !finished; ++it) {
+        if (use_graph) {
+            IF_CUDA_TRY(cudaGraphLaunch(gs.exec[it & 1], r.st));
+            g_launches += launches_per_graph;
+        } else {
+            if ((rc = mg_enqueue_iteration(r, nullptr))) return rc;
+            if ((rc = mg_enqueue_turnover(r, job, d_out, d_fields))) return rc;
+        }
+        const int slot = (int)(it & 3);
+        IF_CUDA_TRY(cudaMemcpyAsync(snap + 4 * slot, reinterpret_cast<const char*>(r.w.ctrl) + offsetof(Ctrl, snap),
+                                    4 * sizeof(int), cudaMemcpyDeviceToHost, r.st));
+        IF_CUDA_TRY(cudaEventRecord(poll.ev[slot], r.st));
+        if (it == 0) continue;
+        const int prev = (int)((it - 1) & 3);
+        IF_CUDA_TRY(cudaEventSynchronize(poll.ev[prev]));
+        const int occupied = snap[4 * prev], running = snap[4 * prev + 1];
+        const bool worked = it == 1 || running_before > 0;     // columns were running when launch it-1 began
+        running_before = running;
+        if (times && use_graph && worked && running > 0) {
+            // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
+            const IterTimer& te = gs.tev[(it - 1) & 1];
+            double ms[TIMER_GROUPS] = {};
+            bool ok = te.n > 1;
+            for (int i = 1; i < te.n && ok; ++i) {
+                float dt = 0.f;
+                ok = cudaEventElapsedTime(&dt, te.ev[i - 1], te.ev[i]) == cudaSuccess;
+                if (ok && te.gid[i] >= 0 && te.gid[i] < TIMER_GROUPS) ms[te.gid[i]] += dt;
+            }
+            if (ok) {
+                for (int g = 0; g < TIMER_GROUPS; ++g) times->ms[g] += ms[g];
+                times->samples += 1;
+            } else {
+                cudaGetLastError();
+            }
+        }
+        if (occupied == 0) finished = true;      // every right-hand side has been started, stopped and finalised
+    }
+    if (!finished) return IF_ECUDA;   // cannot happen: every column stops at max_iter
+    return IF_OK;
+}
+
 template <int K>
 int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
               PollState& poll, KernelTimes* times, int64_t* batch_iters) {
     QueueState q;
-    int rc = solve_from<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, q, true);
+    int rc = IF_OK;
+    bool on_device = false;
+    if constexpr (K == MGK) {
+        // multigrid stream: column turnover on the device where an iteration is long enough to pay for the four extra
+        // graph nodes (about 12 us per iteration against one idle column-iteration per right-hand side: break-even
+        // near 0.5 ms per iteration = 400 k rows for n = 1, a quarter of that for n = 2; measured on configs 2 and 4),
+        // else the host-driven refill of solve_phase.  IF_MG_HOST_REFILL = 1 / 0 forces one or the other (tests).
+        const char* env = getenv("IF_MG_HOST_REFILL");
+        const bool big = r.h->n_vert * (r.order_n == 1 ? 1 : 4) >= MG_DEVICE_TURNOVER_ROWS;
+        const bool host_refill = env != nullptr ? atoi(env) != 0 : !big;
+        on_device = r.mg && !r.vec && !host_refill;
+        if (on_device) rc = mg_stream_on_device(r, job, d_fields, rhs, n_ells, d_out, poll, times);
+    }
+    if (!on_device) rc = solve_from<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, q, true);
     if (rc != IF_OK) return rc;
     long long total = 0;
     IF_CUDA_TRY(cudaMemcpyAsync(&total, &r.w.ctrl->total_iters, sizeof(long long), cudaMemcpyDeviceToHost, r.st));

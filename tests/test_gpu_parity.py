@@ -715,11 +715,14 @@ def test_biharmonic_multigrid_product_preconditioner_matches_oracle(ifl, oracle_
     h.close()
 
 
+@pytest.mark.parametrize("turnover", ["host", "device"])
 @pytest.mark.parametrize("order_n", [1, 2])
-def test_multigrid_stream_refills_columns_and_is_deterministic(ifl, oracle_mod, order_n):
+def test_multigrid_stream_refills_columns_and_is_deterministic(ifl, oracle_mod, order_n, turnover, monkeypatch):
     """More right-hand sides than columns (3 fields x 11 scales = 33 through 16 columns), very unequal scales: stopped
     columns are restarted from the queue at iteration boundaries next to running ones.  The preconditioner is a fixed
-    operator per column, so two runs give the same iteration counts and the same bits; answers are the oracle's."""
+    operator per column, so two runs give the same iteration counts and the same bits; answers are the oracle's.
+    Both ways of ending and starting columns: by the host one launch behind, and on the device inside the graph."""
+    monkeypatch.setenv("IF_MG_HOST_REFILL", "1" if turnover == "host" else "0")
     w = make_config(5 if order_n == 2 else 4, level=5, n_fields=3, n_ells=11, ell_max=32.0)
     om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
     area = om.area()
@@ -741,6 +744,57 @@ def test_multigrid_stream_refills_columns_and_is_deterministic(ifl, oracle_mod, 
     assert float((c - a).abs().max()) <= 1e-8 * float(a.abs().max())
     d, sd = ifl.if_filter(h, w.fields[:1], w.ells[-1:], order_n, solver=1, max_iter=3)
     assert sd["code"] == 1 and sd["status"][0, 0] == 1 and sd["iters"][0, 0] == 3 and bool(d.isfinite().all())
+    h.close()
+
+
+@pytest.mark.parametrize("order_n", [1, 2])
+def test_multigrid_turnover_on_device_matches_host_refill(ifl, oracle_mod, order_n, monkeypatch):
+    """The multigrid stream ends and starts its columns on the device (k_turn_plan inside every iteration's graph;
+    the host only watches).  Against the host-driven refill of the Jacobi path's loop (IF_MG_HOST_REFILL=1), which
+    sees a stop one launch late: the same per-right-hand-side arithmetic, so the same iteration counts and fields to
+    rounding, in fewer fused iterations; for fewer right-hand sides than columns, exactly 16, and many more; filter,
+    high-pass and spectrum jobs; answers are the oracle's."""
+    w = make_config(5 if order_n == 2 else 4, level=5, n_fields=5, n_ells=9, ell_max=24.0)
+    om = oracle_mod.OracleMesh(w.mesh.coords, w.mesh.tri, None)
+    area = om.area()
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    for nf, ne in ((1, 3), (2, 8), (5, 9)):                      # 3, 16 and 45 right-hand sides
+        fields, ells = w.fields[:nf], w.ells[:ne]
+        monkeypatch.setenv("IF_MG_HOST_REFILL", "0")             # (unset: by mesh size, the host on a mesh this small)
+        dev, sd = ifl.if_filter(h, fields, ells, order_n, solver=1, mg_min_ell=0.5)
+        spd = ifl.if_spectrum(h, fields, ells, order_n, solver=1, mg_min_ell=0.5)
+        monkeypatch.setenv("IF_MG_HOST_REFILL", "1")
+        host, sh = ifl.if_filter(h, fields, ells, order_n, solver=1, mg_min_ell=0.5)
+        sph = ifl.if_spectrum(h, fields, ells, order_n, solver=1, mg_min_ell=0.5)
+        monkeypatch.delenv("IF_MG_HOST_REFILL")
+        assert sd["code"] == 0 and sh["code"] == 0 and spd["stats"]["code"] == 0
+        assert sd["mg_batch_iters"] == sd["batch_iters"] > 0
+        assert np.array_equal(sd["status"], sh["status"])
+        assert np.abs(sd["iters"].astype(np.int64) - sh["iters"]).max() <= 1, (sd["iters"], sh["iters"])
+        assert sd["mg_batch_iters"] <= sh["mg_batch_iters"], (nf, ne, sd["mg_batch_iters"], sh["mg_batch_iters"])
+        if nf * ne > 16:
+            assert sd["mg_batch_iters"] < sh["mg_batch_iters"]           # the refills no longer idle an iteration
+        scale = float(host.abs().max())
+        assert float((dev - host).abs().max()) <= 1e-9 * scale
+        assert np.all(np.abs(spd["energy"] - sph["energy"]) <= 1e-9 * sph["energy"])
+        d = dev.cpu().numpy()
+        en = 0.5 * (area * d * d).sum(axis=-1) / area.sum()             # the plain definition on the returned fields
+        assert np.all(np.abs(spd["energy"] - en) <= 1e-9 * en)
+    # the oracle, on a sample of the largest case
+    for f, j in ((0, 0), (2, 4), (4, 8), (3, 6)):
+        x, info = om.solve(w.fields[f], float(w.ells[j]), order_n)
+        res_gpu = true_residual(ifl, h, dev[f, j], w.fields[f], area, float(w.ells[j]), order_n)
+        tol = parity_tolerance(area, w.fields[f], x, res_gpu, info["true_res"])
+        assert info["status"] == 0 and rel(dev[f, j].cpu().numpy(), x) <= tol, (f, j)
+    # high-pass output and the iteration cap through the device turnover
+    monkeypatch.setenv("IF_MG_HOST_REFILL", "0")
+    hp, shp = ifl.if_filter(h, w.fields[:3], w.ells, order_n, solver=1, mg_min_ell=0.5, flags=ifl.IF_FLAG_HIGHPASS)
+    import torch
+    phi = torch.from_numpy(w.fields[:3]).to(hp.device)[:, None, :]
+    assert float((hp - (phi - dev[:3])).abs().max()) <= 1e-9 * scale
+    cap, sc = ifl.if_filter(h, w.fields, w.ells, order_n, solver=1, mg_min_ell=0.5, max_iter=4)
+    assert sc["code"] == 1 and int(sc["iters"].max()) == 4 and bool(cap.isfinite().all())
+    assert np.all(((sc["status"] == 0) & (sc["iters"] <= 4)) | ((sc["status"] == 1) & (sc["iters"] == 4)))
     h.close()
 
 
