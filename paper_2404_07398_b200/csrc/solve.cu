@@ -218,7 +218,52 @@ struct GraphSet {
     }
 };
 
+// What `enqueue(timer)` launches on `st`, captured twice into two graph instances (launched alternately, so that the
+// timing events of one can be read while the other runs).  A stream that cannot be captured (the legacy default
+// stream) leaves gs empty: the caller launches directly.  *launches_per_graph = kernels in one instance.
+template <class F>
+int capture_graphs(cudaStream_t st, GraphSet& gs, long long* launches_per_graph, F&& enqueue) {
+    *launches_per_graph = 0;
+    if (st == nullptr || st == cudaStreamLegacy) return IF_OK;
+    for (int gi = 0; gi < 2; ++gi) {
+        if (gs.tev[gi].create() != IF_OK) return IF_ECUDA;
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+            cudaGetLastError();   // stream cannot be captured: direct launches
+            if (gs.exec[0]) { cudaGraphExecDestroy(gs.exec[0]); gs.exec[0] = nullptr; }
+            return IF_OK;
+        }
+        const long long before = g_launches.load();
+        const int rcc = enqueue(&gs.tev[gi]);
+        *launches_per_graph = g_launches.load() - before;
+        g_launches -= *launches_per_graph;   // captured, not launched
+        cudaError_t e = cudaStreamEndCapture(st, &graph);
+        if (rcc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
+        e = cudaGraphInstantiate(&gs.exec[gi], graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) { gs.exec[gi] = nullptr; cudaGetLastError(); return IF_ECUDA; }
+    }
+    return IF_OK;
+}
+
 struct KernelTimes { double ms[TIMER_GROUPS] = {}; int64_t samples = 0; };   // per group, summed over samples
+
+// one timed iteration of a finished graph launch into the per-group sums (events recorded inside the graph)
+inline void add_timing_sample(KernelTimes& times, const IterTimer& te) {
+    double ms[TIMER_GROUPS] = {};
+    bool ok = te.n > 1;
+    for (int i = 1; i < te.n && ok; ++i) {
+        float dt = 0.f;
+        ok = cudaEventElapsedTime(&dt, te.ev[i - 1], te.ev[i]) == cudaSuccess;
+        if (ok && te.gid[i] >= 0 && te.gid[i] < TIMER_GROUPS) ms[te.gid[i]] += dt;
+    }
+    if (ok) {
+        for (int g = 0; g < TIMER_GROUPS; ++g) times.ms[g] += ms[g];
+        times.samples += 1;
+    } else {
+        cudaGetLastError();
+    }
+}
 
 struct PollState {
     Snapshot* snap = nullptr;          // pinned [4]
@@ -448,30 +493,16 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
     const int per_graph = r.mg ? 1 : r.opt.check_every;
     long long launches_per_graph = 0;
     GraphSet gs;
-    if (r.st != nullptr && r.st != cudaStreamLegacy) {
-        for (int gi = 0; gi < 2; ++gi) {
-            if (gs.tev[gi].create() != IF_OK) return IF_ECUDA;
-            cudaGraph_t graph = nullptr;
-            if (cudaStreamBeginCapture(r.st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
-                cudaGetLastError();   // stream cannot be captured: direct launches below
-                break;
-            }
-            int rcc = IF_OK;
-            const int timed_it = per_graph > 2 ? 2 : 0;
-            const long long before = g_launches.load();
-            for (int i = 0; i < per_graph && rcc == IF_OK; ++i) {
-                IterTimer* tm = i == timed_it ? &gs.tev[gi] : nullptr;
-                rcc = r.mg ? mg_enqueue_iteration(r, tm) : enqueue_iteration<K>(r, tm);
-            }
-            launches_per_graph = g_launches.load() - before;
-            g_launches -= launches_per_graph;   // captured, not launched
-            cudaError_t e = cudaStreamEndCapture(r.st, &graph);
-            if (rcc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
-            e = cudaGraphInstantiate(&gs.exec[gi], graph, 0);
-            cudaGraphDestroy(graph);
-            if (e != cudaSuccess) { gs.exec[gi] = nullptr; cudaGetLastError(); return IF_ECUDA; }
+    rc = capture_graphs(r.st, gs, &launches_per_graph, [&](IterTimer* timer) {
+        int rcc = IF_OK;
+        const int timed_it = per_graph > 2 ? 2 : 0;
+        for (int i = 0; i < per_graph && rcc == IF_OK; ++i) {
+            IterTimer* tm = i == timed_it ? timer : nullptr;
+            rcc = r.mg ? mg_enqueue_iteration(r, tm) : enqueue_iteration<K>(r, tm);
         }
-    }
+        return rcc;
+    });
+    if (rc != IF_OK) return rc;
     const bool use_graph = gs.exec[0] && gs.exec[1];
     const int64_t per_rhs = (r.opt.max_iter + per_graph - 1) / per_graph + 3;
     const int64_t max_loops = ((int64_t)(R + K - 1) / K + 1) * per_rhs + 8;
@@ -498,23 +529,8 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
             if (q.col_rhs[c] < 0 || s.epoch[c] != q.host_epoch[c]) continue;
             if (s.done[c]) fin |= 1u << c; else any_running = true;
         }
-        if (times && use_graph && any_running) {
-            // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
-            const IterTimer& te = gs.tev[(it - 1) & 1];
-            double ms[TIMER_GROUPS] = {};
-            bool ok = te.n > 1;
-            for (int i = 1; i < te.n && ok; ++i) {
-                float dt = 0.f;
-                ok = cudaEventElapsedTime(&dt, te.ev[i - 1], te.ev[i]) == cudaSuccess;
-                if (ok && te.gid[i] >= 0 && te.gid[i] < TIMER_GROUPS) ms[te.gid[i]] += dt;
-            }
-            if (ok) {
-                for (int g = 0; g < TIMER_GROUPS; ++g) times->ms[g] += ms[g];
-                times->samples += 1;
-            } else {
-                cudaGetLastError();
-            }
-        }
+        // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
+        if (times && use_graph && any_running) add_timing_sample(*times, gs.tev[(it - 1) & 1]);
         if (fin) {
             // these columns stopped before launch it-1 ended and stayed frozen through launch it
             if ((rc = finalize_columns<K>(r, job, fin, d_out, d_fields))) return rc;
@@ -666,26 +682,11 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
 
     long long launches_per_graph = 0;
     GraphSet gs;
-    if (r.st != nullptr && r.st != cudaStreamLegacy) {
-        for (int gi = 0; gi < 2; ++gi) {
-            if (gs.tev[gi].create() != IF_OK) return IF_ECUDA;
-            cudaGraph_t graph = nullptr;
-            if (cudaStreamBeginCapture(r.st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
-                cudaGetLastError();   // stream cannot be captured: direct launches below
-                break;
-            }
-            const long long before = g_launches.load();
-            int rcc = mg_enqueue_iteration(r, &gs.tev[gi]);
-            if (rcc == IF_OK) rcc = mg_enqueue_turnover(r, job, d_out, d_fields);
-            launches_per_graph = g_launches.load() - before;
-            g_launches -= launches_per_graph;   // captured, not launched
-            cudaError_t e = cudaStreamEndCapture(r.st, &graph);
-            if (rcc != IF_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return IF_ECUDA; }
-            e = cudaGraphInstantiate(&gs.exec[gi], graph, 0);
-            cudaGraphDestroy(graph);
-            if (e != cudaSuccess) { gs.exec[gi] = nullptr; cudaGetLastError(); return IF_ECUDA; }
-        }
-    }
+    rc = capture_graphs(r.st, gs, &launches_per_graph, [&](IterTimer* timer) {
+        const int rcc = mg_enqueue_iteration(r, timer);
+        return rcc != IF_OK ? rcc : mg_enqueue_turnover(r, job, d_out, d_fields);
+    });
+    if (rc != IF_OK) return rc;
     const bool use_graph = gs.exec[0] && gs.exec[1];
     const int64_t max_loops = ((int64_t)(R + MGK - 1) / MGK + 1) * ((int64_t)r.opt.max_iter + 3) + 8;
     int* snap = reinterpret_cast<int*>(poll.snap);      // four slots of four ints in the pinned snapshot buffer
@@ -709,23 +710,8 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
         const int occupied = snap[4 * prev], running = snap[4 * prev + 1];
         const bool worked = it == 1 || running_before > 0;     // columns were running when launch it-1 began
         running_before = running;
-        if (times && use_graph && worked && running > 0) {
-            // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
-            const IterTimer& te = gs.tev[(it - 1) & 1];
-            double ms[TIMER_GROUPS] = {};
-            bool ok = te.n > 1;
-            for (int i = 1; i < te.n && ok; ++i) {
-                float dt = 0.f;
-                ok = cudaEventElapsedTime(&dt, te.ev[i - 1], te.ev[i]) == cudaSuccess;
-                if (ok && te.gid[i] >= 0 && te.gid[i] < TIMER_GROUPS) ms[te.gid[i]] += dt;
-            }
-            if (ok) {
-                for (int g = 0; g < TIMER_GROUPS; ++g) times->ms[g] += ms[g];
-                times->samples += 1;
-            } else {
-                cudaGetLastError();
-            }
-        }
+        // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
+        if (times && use_graph && worked && running > 0) add_timing_sample(*times, gs.tev[(it - 1) & 1]);
         if (occupied == 0) finished = true;      // every right-hand side has been started, stopped and finalised
     }
     if (!finished) return IF_ECUDA;   // cannot happen: every column stops at max_iter
