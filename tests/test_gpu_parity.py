@@ -798,6 +798,31 @@ def test_multigrid_turnover_on_device_matches_host_refill(ifl, oracle_mod, order
     h.close()
 
 
+def test_legacy_default_stream_runs_without_graphs(ifl, monkeypatch):
+    """Stream 0 (the legacy default stream) cannot be captured: both stream loops then launch their kernels directly.
+    Same kernels in the same order, so the same bits as the graph path on a side stream -- Jacobi-PCG, the multigrid
+    stream with the host-driven refill and with the turnover on the device."""
+    import torch
+    w = make_config(4, level=5, n_fields=3, n_ells=7, ell_max=24.0)                # 21 right-hand sides
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    legacy = torch.cuda.default_stream()
+    assert legacy.cuda_stream == 0
+    for opts, env in ((dict(), None), (dict(solver=1, mg_min_ell=0.5), "1"), (dict(solver=1, mg_min_ell=0.5), "0")):
+        if env is None:
+            monkeypatch.delenv("IF_MG_HOST_REFILL", raising=False)
+        else:
+            monkeypatch.setenv("IF_MG_HOST_REFILL", env)
+        a, sa = ifl.if_filter(h, w.fields, w.ells, 1, **opts)                      # the binding's side stream: graphs
+        b, sb = ifl.if_filter(h, w.fields, w.ells, 1, stream=legacy, **opts)       # stream 0: direct launches
+        assert sa["code"] == 0 and sb["code"] == 0
+        assert np.array_equal(sa["iters"], sb["iters"]) and bool((a == b).all()), (opts, env)
+        assert sa["batch_iters"] == sb["batch_iters"]
+        spa = ifl.if_spectrum(h, w.fields, w.ells, 1, **opts)
+        spb = ifl.if_spectrum(h, w.fields, w.ells, 1, stream=legacy, **opts)
+        assert np.array_equal(spa["energy"], spb["energy"]) and np.array_equal(spa["E"], spb["E"])
+    h.close()
+
+
 # ------------------------------------------------------------------------------------------ higher orders, velocity pairs
 @pytest.mark.parametrize("order_n", [3, 4])
 def test_higher_order_filters_match_oracle(ifl, oracle_mod, order_n):
