@@ -98,6 +98,8 @@ struct Ctrl {
     // column turnover on the device (multigrid stream, k_turn_plan): the queue position, which columns hold a
     // right-hand side, what this iteration's turnover finalises and starts, and what the host reads back
     int q_next, q_total;
+    int rhs_stride;       // vector filter: output slot of the v component = that of u + rhs_stride (= n_ells)
+    int pad2_;
     int occupied[KMAX];
     unsigned int turn_fin, turn_start;
     StartParams turn_sp;
@@ -337,7 +339,10 @@ __device__ __forceinline__ void cg_bookkeeping(Ctrl* __restrict__ ctrl, const do
     if (tid < K) {
         if (!ctrl->done[tid]) {
             const bool start = ctrl->starting[tid] != 0;
-            const double rho_new = tot[tid], rr = tot[KMAX + tid];
+            // (vector filter: the two columns of a pair are one system -- its dot products are the sums over both)
+            const int ta = ctrl->pair_mode ? (tid & ~1) : tid, tb = ctrl->pair_mode ? (tid | 1) : tid;
+            const double w2 = ctrl->pair_mode ? 1.0 : 0.5;      // (ta == tb without pairs: the value itself)
+            const double rho_new = w2 * (tot[ta] + tot[tb]), rr = w2 * (tot[KMAX + ta] + tot[KMAX + tb]);
             const int it = start ? 0 : ctrl->iters[tid] + 1;
             ctrl->iters[tid] = it;
             ctrl->rr[tid] = rr;
@@ -1356,37 +1361,55 @@ __global__ void k_stats(const Ctrl* __restrict__ ctrl, int K, unsigned mask, int
 // (zeroed, stopped at once), so that no kernel ever reads what the workspace held before.
 __global__ void k_turn_plan(Ctrl* __restrict__ ctrl, const QEntry* __restrict__ queue, int K, int first,
                             int32_t* __restrict__ iters, int32_t* __restrict__ status, double* __restrict__ relres) {
-    // one warp, lane c = column c: masks by ballot, the queue position of a free column = its rank among the free ones
+    // one warp, lane s = slot s: a column, or with the vector filter (pair_mode) the column pair (2s, 2s+1) of one
+    // coupled system, whose queue entry names the u field and output slot; v follows at field + 1, slot + rhs_stride.
+    // Masks by ballot, the queue position of a free slot = its rank among the free ones.
     const unsigned full = 0xffffffffu;
-    const int c = threadIdx.x;
-    const bool in = c < K;
-    const int occ0 = in ? ctrl->occupied[c] : 0;
-    const int dn = in ? ctrl->done[c] : 1;
+    const int s = threadIdx.x;
+    const int step = ctrl->pair_mode ? 2 : 1;
+    const unsigned bits = step == 2 ? 3u : 1u;
+    const bool in = s < K / step;
+    const int c0 = in ? s * step : 0;
+    const int occ0 = in ? ctrl->occupied[c0] : 0;
+    const int dn = in ? ctrl->done[c0] : 1;            // (the columns of a pair share every decision)
     const int next = ctrl->q_next, total = ctrl->q_total;
-    const bool fin_c = occ0 && dn;
-    if (fin_c) {                                 // the per-right-hand-side results (k_stats of the host-driven refill)
-        const int r = ctrl->rhs[c];
-        iters[r] = ctrl->iters[c];
-        status[r] = ctrl->status[c];
-        relres[r] = ctrl->bb[c] > 0.0 ? sqrt(ctrl->rr[c] / ctrl->bb[c]) : 0.0;
+    const bool fin_s = occ0 && dn;
+    if (fin_s) {                                 // the per-right-hand-side results (k_stats of the host-driven refill)
+        for (int c = c0; c < c0 + step; ++c) {
+            const int r = ctrl->rhs[c];
+            iters[r] = ctrl->iters[c];
+            status[r] = ctrl->status[c];
+            relres[r] = ctrl->bb[c] > 0.0 ? sqrt(ctrl->rr[c] / ctrl->bb[c]) : 0.0;
+        }
     }
-    const bool free_c = in && (!occ0 || fin_c);
-    const unsigned fin = __ballot_sync(full, fin_c);
-    const unsigned freem = __ballot_sync(full, free_c);
-    const int rank = __popc(freem & ((1u << c) - 1u));
-    const bool take = free_c && next + rank < total;
-    const bool occ = (occ0 && !fin_c) || take;
+    const bool free_s = in && (!occ0 || fin_s);
+    const unsigned finm = __ballot_sync(full, fin_s);
+    const unsigned freem = __ballot_sync(full, free_s);
+    const int rank = __popc(freem & ((1u << s) - 1u));
+    const bool take = free_s && next + rank < total;
+    const bool occ = (occ0 && !fin_s) || take;
     if (in) {
         QEntry e = {0.0, 0.0, -1, 0};
         if (take) e = queue[next + rank];
-        ctrl->turn_sp.c[c] = e.c; ctrl->turn_sp.c1[c] = e.c1; ctrl->turn_sp.field[c] = e.field; ctrl->turn_sp.rhs[c] = e.rhs;
-        ctrl->occupied[c] = occ ? 1 : 0;
+        for (int i = 0; i < step; ++i) {
+            const int c = c0 + i;
+            ctrl->turn_sp.c[c] = e.c; ctrl->turn_sp.c1[c] = e.c1;
+            ctrl->turn_sp.field[c] = e.field < 0 ? -1 : e.field + i;
+            ctrl->turn_sp.rhs[c] = e.rhs + i * ctrl->rhs_stride;
+            ctrl->occupied[c] = occ ? 1 : 0;
+        }
     }
-    const unsigned start = __ballot_sync(full, take || (first && free_c));
+    const unsigned startm = __ballot_sync(full, take || (first && free_s));
     const unsigned occm = __ballot_sync(full, occ);
     const unsigned runm = __ballot_sync(full, occ && (take || !dn));
     const unsigned takem = __ballot_sync(full, take);
-    if (c == 0) {
+    if (s == 0) {
+        // slot masks -> column masks
+        unsigned fin = 0u, start = 0u;
+        for (int i = 0; i < K / step; ++i) {
+            if ((finm >> i) & 1u) fin |= bits << (i * step);
+            if ((startm >> i) & 1u) start |= bits << (i * step);
+        }
         ctrl->q_next = next + __popc(takem);
         ctrl->turn_fin = fin;
         ctrl->turn_start = start;

@@ -524,6 +524,11 @@ int mg_setup(Run& r) {
     IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_coarse_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MG_FACTOR_SMEM));
     const int64_t tiles = (h->n_vert + TILE_ROWS - 1) / TILE_ROWS;
     int rc;
+    if (r.vec) {      // vector filter (n = 1): the coupled operator in the level-0 kernels of the cycle
+        if ((rc = resident_grid(k_spmm<MGK, MODE_AX, true>, TileSmem<MGK, MODE_AX, true>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
+        if ((rc = resident_grid(k_spmm<MGK, MODE_MGR, true>, TileSmem<MGK, MODE_MGR, true>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;
+        return r.order_n == 1 ? IF_OK : IF_EINVAL;
+    }
     if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
     if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;
     if (r.order_n == 2 &&
@@ -691,7 +696,7 @@ int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const do
     if (tm && (rc = tm->mark(r.st, MGT_RESTRICT0))) return rc;
     double* ec = nullptr;
     if ((rc = mg_vcycle(r, b, 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
-    if (nu == 1 && mg_fused_prolongation(g)) {    // e = omega R/d formed again here: it has not been stored
+    if (nu == 1 && mg_fused_prolongation(g) && !r.vec) {    // e = omega R/d formed again here: it has not been stored
         bool done = false;
         RowsArgs a{g.p_rowptr, g.p_col, g.p_val, g.diag, g.n, ec, R0, R1, cur, g.omega, r_select, 0, 0};
         if ((rc = launch_rows<ROWS_PROLONG0>(r, a, g.cap_p, &done))) return rc;
@@ -725,7 +730,8 @@ int mg_enqueue_iteration(const Run& r, IterTimer* tm) {
     double om[MG_MAX_NU];
     mg_omegas(h->mg[0], nu, om);
     // what the fused first-sweep kernel leaves behind (see mg_cycle_level0)
-    double* e_store = (nu == 1 && !mg_fused_prolongation(h->mg[0])) ? b.za : nullptr;
+    // (vector filter: the first sweep divides by the diagonal of D~, which the prolongation kernel does not have: stored)
+    double* e_store = (nu == 1 && (r.vec || !mg_fused_prolongation(h->mg[0]))) ? b.za : nullptr;
     double* first_out = nu >= 2 ? b.za : b.t;
     const double omega2 = nu >= 2 ? om[1] : 0.0;
     int rc;

@@ -124,7 +124,10 @@ int setup_grids(Run& r) { return r.vec ? setup_grids_v<K, true>(r) : setup_grids
 
 template <int K, int MODE>
 int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
-    constexpr bool CG_MODE = MODE == MODE_PLAIN || MODE == MODE_CG1 || MODE == MODE_CG2A || MODE == MODE_CG2B;
+    // the vector filter's variants: every mode of the Jacobi path, and the level-0 kernels of the multigrid cycle for
+    // n = 1 (smoothing and residuals on the coupled operator, mg_solve.cuh)
+    constexpr bool CG_MODE = MODE == MODE_PLAIN || MODE == MODE_CG1 || MODE == MODE_CG2A || MODE == MODE_CG2B ||
+                             (K == KMAX && (MODE == MODE_AX || MODE == MODE_MGR));
     if constexpr (CG_MODE) {
         if (r.vec) {
             k_spmm<K, MODE, true><<<grid, SpmmCfg<K, MODE>::NT, TileSmem<K, MODE, true>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
@@ -669,12 +672,15 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
         const Rhs& s = rhs[i];
         hq[i].c = r.opt.gamma * std::pow(s.ell, 2.0 * r.order_n);
         hq[i].c1 = r.order_n == 1 ? hq[i].c : std::sqrt(hq[i].c);   // K = M + sqrt(c) S (mg_solve.cuh)
-        hq[i].field = s.f;
-        hq[i].rhs = s.f * n_ells + s.j;
+        // (vector filter: s.f counts (u, v) pairs; the entry names the u field and slot, k_turn_plan derives v's)
+        const int f = r.vec ? 2 * s.f : s.f;
+        hq[i].field = f;
+        hq[i].rhs = f * n_ells + s.j;
     }
     Ctrl hc = fresh_ctrl(r);
     hc.q_next = 0;
     hc.q_total = (int)R;
+    hc.rhs_stride = n_ells;
     // (pageable sources: both copies are staged by the runtime before the call returns)
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.queue, hq.data(), R * sizeof(QEntry), cudaMemcpyHostToDevice, r.st));
@@ -688,7 +694,8 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
     });
     if (rc != IF_OK) return rc;
     const bool use_graph = gs.exec[0] && gs.exec[1];
-    const int64_t max_loops = ((int64_t)(R + MGK - 1) / MGK + 1) * ((int64_t)r.opt.max_iter + 3) + 8;
+    const int64_t slots = r.vec ? MGK / 2 : MGK;
+    const int64_t max_loops = ((int64_t)(R + slots - 1) / slots + 1) * ((int64_t)r.opt.max_iter + 3) + 8;
     int* snap = reinterpret_cast<int*>(poll.snap);      // four slots of four ints in the pinned snapshot buffer
     bool finished = false;
     int running_before = 0;
@@ -732,7 +739,7 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
         const char* env = getenv("IF_MG_HOST_REFILL");
         const bool big = r.h->n_vert * (r.order_n == 1 ? 1 : 4) >= MG_DEVICE_TURNOVER_ROWS;
         const bool host_refill = env != nullptr ? atoi(env) != 0 : !big;
-        on_device = r.mg && !r.vec && !host_refill;
+        on_device = r.mg && !host_refill;
         if (on_device) rc = mg_stream_on_device(r, job, d_fields, rhs, n_ells, d_out, poll, times);
     }
     if (!on_device) rc = solve_from<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, q, true);
@@ -834,7 +841,9 @@ int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields
     KernelTimes ktimes, mgtimes;
     int64_t batch_iters = 0, mg_batch_iters = 0;
     // large scales by multigrid-preconditioned CG (option solver = 1): a stream of right-hand sides through 16 columns
-    if (job != JOB_APPLY && r.opt.solver == 1 && order_n <= 2 && !r.vec && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
+    // (vector filter: n = 1 only, through the scalar hierarchy with the coupled operator on the mesh)
+    if (job != JOB_APPLY && r.opt.solver == 1 && (r.vec ? order_n == 1 : order_n <= 2) && r.opt.batch == MGK && r.w.mg_extra &&
+        h->mean_edge > 0.0) {
         const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)) *
                                h->mean_edge;
         size_t n_big = 0;

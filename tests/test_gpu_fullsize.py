@@ -297,3 +297,45 @@ def test_vector_filter_large_band(oracle_mod):
         print(f"vector kernel A: {1e3 * s['spmm_seconds']:.3f} ms per launch, {nbytes / s['spmm_seconds'] / 1e9:.0f} GB/s "
               f"algorithmic ({s['kernel_samples']} samples, V = {h.n_vert})")
     h.close()
+
+
+def test_vector_filter_large_band_multigrid():
+    """The vector filter through the multigrid path (solver = 1: the scalar hierarchy preconditions the coupled system,
+    smoothing on the mesh with the metric terms) on the same band, 8 (u, v) pairs x 12 scales from 1 to 400 edge lengths
+    -- scales Jacobi-PCG needs thousands of iterations for: every solve through its true residual
+    (IF_FLAG_TRUE_RESIDUAL), the small scales against the Jacobi path, kinetic-energy spectra of both paths."""
+    import time
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2404_07398_b200 as lib
+    from workloads import icosphere, jitter_sphere, log_spaced, sphere_band, sphere_velocity_field
+    mesh = sphere_band(jitter_sphere(icosphere(9), 0.25, np.random.default_rng(41)), 70.0)
+    rng = np.random.default_rng(42)
+    fields = np.empty((16, mesh.n_vert))
+    for p in range(8):
+        fields[2 * p], fields[2 * p + 1] = sphere_velocity_field(mesh.coords, 200, 64, rng)
+    ells = mesh.h * log_spaced(1.0, 400.0, 12)
+    VEC = lib.IF_FLAG_VECTOR
+    h = lib.if_prepare(mesh.coords, mesh.tri, None, flags=VEC | lib.IF_FLAG_MULTIGRID, radius=1.0)
+    out, st = lib.if_filter(h, fields, ells, 1, flags=VEC | lib.IF_FLAG_TRUE_RESIDUAL, solver=1)
+    assert st["code"] == 0 and np.all(st["status"] == 0) and np.all(st["true_res"] <= 1e-10), st["true_res"].max()
+    assert st["mg_batch_iters"] == st["batch_iters"] > 0
+    assert np.array_equal(st["iters"][0::2], st["iters"][1::2])
+    jac, sj = lib.if_filter(h, fields[:4], ells[:5], 1, flags=VEC)                      # up to 9 edge lengths
+    assert sj["code"] == 0
+    assert float((out[:4, :5] - jac).abs().max()) <= 1e-8 * float(jac.abs().max())
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    sp = lib.if_spectrum(h, fields, ells, 1, flags=VEC | lib.IF_FLAG_PAIRS, solver=1)
+    t_mg = time.perf_counter() - t0
+    assert sp["energy"].shape == (8, 12) and np.all(np.diff(sp["energy"], axis=1) < 0.0) and np.all(sp["E"] > 0.0)
+    o = out.cpu().numpy()
+    area = lib.if_mesh_export_csr(lib.if_prepare(mesh.coords, mesh.tri, None, flags=lib.IF_FLAG_KEEP_CSR))[3]
+    ke = 0.5 * ((area * o[0::2] ** 2).sum(-1) + (area * o[1::2] ** 2).sum(-1)) / area.sum()
+    assert np.all(np.abs(sp["energy"] - ke) <= 1e-9 * ke)
+    s = sp["stats"]
+    print(f"vector filter, multigrid path: V = {h.n_vert}, 8 pairs x 12 scales (1 ... 400 h) in {t_mg:.3f} s, "
+          f"{int(s['iters'][0::2].sum())} pair-iterations ({int(s['iters'].min())}-{int(s['iters'].max())} per solve), "
+          f"{s['mg_batch_iters']} fused iterations; Jacobi-PCG at 9 h: {int(sj['iters'][:, -1].max())} iterations")
+    h.close()

@@ -972,6 +972,53 @@ def test_vector_filter_matches_oracle(ifl, oracle_mod, order_n):
     h.close(); h0.close()
 
 
+@pytest.mark.parametrize("turnover", ["host", "device"])
+def test_vector_filter_through_the_multigrid_path(ifl, oracle_mod, turnover, monkeypatch):
+    """solver = 1 with IF_FLAG_VECTOR (n = 1): PCG on the coupled 2V system preconditioned by the V cycle of the
+    scalar hierarchy -- smoothing and residuals on the mesh with the coupled operator (metric terms D~, T), coarse
+    correction per component.  Same systems, same start, same stop test: the oracle's joint PCG is the reference, with
+    the tolerance derived from both true residuals; both columns of a pair share the iteration count; more pairs
+    than columns (refill in pairs); far fewer iterations than Jacobi-PCG at the large scales; spectra of pairs."""
+    monkeypatch.setenv("IF_MG_HOST_REFILL", "1" if turnover == "host" else "0")     # pairs end and start together
+    mesh, fields = vector_workload(5, 10)                       # 10 (u, v) pairs = 20 fields
+    from workloads import log_spaced
+    ells = mesh.h * log_spaced(1.0, 48.0, 4)                    # 40 pair solves through 8 pair slots
+    om = oracle_mod.OracleMesh(mesh.coords, mesh.tri, None)
+    om.build_vector(1.0)
+    area = om.area()
+    VEC = ifl.IF_FLAG_VECTOR
+    h = ifl.if_prepare(mesh.coords, mesh.tri, None, flags=VEC | ifl.IF_FLAG_MULTIGRID, radius=1.0)
+    out, st = ifl.if_filter(h, fields, ells, 1, flags=VEC, solver=1, mg_min_ell=0.5)
+    jac, sj = ifl.if_filter(h, fields, ells, 1, flags=VEC)
+    assert st["code"] == 0 and sj["code"] == 0
+    assert st["mg_batch_iters"] == st["batch_iters"] > 0 and sj["mg_batch_iters"] == 0
+    assert np.array_equal(st["iters"][0::2], st["iters"][1::2])                 # a pair is one system
+    assert int(st["iters"][:, -1].max()) * 4 < int(sj["iters"][:, -1].min())     # the large scale: far fewer iterations
+    assert float((out - jac).abs().max()) <= 1e-8 * float(jac.abs().max())
+    for p in (0, 4, 9):
+        bnorm = np.linalg.norm(np.concatenate([area * fields[2 * p], area * fields[2 * p + 1]]))
+        for j, ell in enumerate(ells):
+            xu, xv, info = om.solve_vector(fields[2 * p], fields[2 * p + 1], float(ell), 1)
+            assert info["status"] == 0
+            x = out[2 * p:2 * p + 2, j]
+            ax = ifl.if_apply(h, x, np.array([ell]), 1, flags=VEC)[:, 0].cpu().numpy()
+            res_gpu = np.linalg.norm(np.concatenate([area * fields[2 * p] - ax[0], area * fields[2 * p + 1] - ax[1]])) / bnorm
+            xr = np.concatenate([xu, xv])
+            tol = max(TOL_FIELD, (res_gpu + info["true_res"]) * bnorm / area.min() / np.linalg.norm(xr))
+            err = rel(np.concatenate([x[0].cpu().numpy(), x[1].cpu().numpy()]), xr)
+            assert err <= tol and res_gpu <= 1e-10, (p, j, err, tol, res_gpu)
+    sp = ifl.if_spectrum(h, fields, ells, 1, flags=VEC | ifl.IF_FLAG_PAIRS, solver=1, mg_min_ell=0.5)
+    sq = ifl.if_spectrum(h, fields, ells, 1, flags=VEC | ifl.IF_FLAG_PAIRS)
+    assert sp["energy"].shape == (10, 4) and np.all(np.abs(sp["energy"] - sq["energy"]) <= 1e-9 * sq["energy"])
+    assert np.all(np.abs(sp["E"] - sq["E"]) <= TOL_BIN * np.abs(sq["E"]))
+    # two runs: the same bits (a fixed operator per column), and n = 2 pairs stay on the Jacobi path
+    again, _ = ifl.if_filter(h, fields, ells, 1, flags=VEC, solver=1, mg_min_ell=0.5)
+    assert bool((again == out).all())
+    b2, s2 = ifl.if_filter(h, fields[:2], ells[:2], 2, flags=VEC, solver=1)
+    assert s2["code"] == 0 and s2["mg_batch_iters"] == 0
+    h.close()
+
+
 def test_vector_filter_planar_mesh_and_save_load(ifl, oracle_mod, tmp_path):
     """A planar mesh has no metric terms: the vector filter returns the two scalar filters.  The metric arrays go
     through if_save / if_load."""
