@@ -105,8 +105,8 @@ typedef struct {
                         solved by multigrid-preconditioned CG: one V cycle of a smoothed-aggregation hierarchy per
                         iteration for n = 1, the product V M V of two cycles for n = 2 (needs batch = 16 and a handle
                         prepared with IF_FLAG_MULTIGRID, else ignored); the rest by Jacobi-PCG.  With IF_FLAG_VECTOR
-                        (n = 1 only; n = 2 pairs stay on Jacobi-PCG) the same hierarchy preconditions the coupled
-                        system: the coupled operator on the mesh, the scalar levels below per component.  Same systems, same
+                        the same hierarchy preconditions the coupled system: the coupled operator on the mesh,
+                        the scalar levels below per component.  Same systems, same
                         start vector, same stop test, same answers within the tolerance (PAPER.md:207 names the
                         convergence of plain CG at large scales, above all for n = 2, as the open problem).  On
                         meshes of 400 000 vertices or more (n = 2: 100 000) the stream ends and starts its columns on

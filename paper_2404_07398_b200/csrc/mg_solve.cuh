@@ -524,10 +524,12 @@ int mg_setup(Run& r) {
     IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_coarse_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MG_FACTOR_SMEM));
     const int64_t tiles = (h->n_vert + TILE_ROWS - 1) / TILE_ROWS;
     int rc;
-    if (r.vec) {      // vector filter (n = 1): the coupled operator in the level-0 kernels of the cycle
+    if (r.vec) {      // vector filter: the coupled operator in the level-0 kernels of the cycle
         if ((rc = resident_grid(k_spmm<MGK, MODE_AX, true>, TileSmem<MGK, MODE_AX, true>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
         if ((rc = resident_grid(k_spmm<MGK, MODE_MGR, true>, TileSmem<MGK, MODE_MGR, true>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;
-        return r.order_n == 1 ? IF_OK : IF_EINVAL;
+        if (r.order_n == 2 &&
+            (rc = resident_grid(k_spmm<MGK, MODE_MGR0, true>, TileSmem<MGK, MODE_MGR0, true>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<MGK, MODE_MGR0>::NT))) return rc;
+        return IF_OK;
     }
     if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
     if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;

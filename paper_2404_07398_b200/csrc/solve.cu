@@ -125,9 +125,9 @@ int setup_grids(Run& r) { return r.vec ? setup_grids_v<K, true>(r) : setup_grids
 template <int K, int MODE>
 int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
     // the vector filter's variants: every mode of the Jacobi path, and the level-0 kernels of the multigrid cycle for
-    // n = 1 (smoothing and residuals on the coupled operator, mg_solve.cuh)
+    // (smoothing and residuals on the coupled operator, mg_solve.cuh)
     constexpr bool CG_MODE = MODE == MODE_PLAIN || MODE == MODE_CG1 || MODE == MODE_CG2A || MODE == MODE_CG2B ||
-                             (K == KMAX && (MODE == MODE_AX || MODE == MODE_MGR));
+                             (K == KMAX && (MODE == MODE_AX || MODE == MODE_MGR || MODE == MODE_MGR0));
     if constexpr (CG_MODE) {
         if (r.vec) {
             k_spmm<K, MODE, true><<<grid, SpmmCfg<K, MODE>::NT, TileSmem<K, MODE, true>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
@@ -841,9 +841,8 @@ int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields
     KernelTimes ktimes, mgtimes;
     int64_t batch_iters = 0, mg_batch_iters = 0;
     // large scales by multigrid-preconditioned CG (option solver = 1): a stream of right-hand sides through 16 columns
-    // (vector filter: n = 1 only, through the scalar hierarchy with the coupled operator on the mesh)
-    if (job != JOB_APPLY && r.opt.solver == 1 && (r.vec ? order_n == 1 : order_n <= 2) && r.opt.batch == MGK && r.w.mg_extra &&
-        h->mean_edge > 0.0) {
+    // (vector filter: through the scalar hierarchy with the coupled operator on the mesh)
+    if (job != JOB_APPLY && r.opt.solver == 1 && order_n <= 2 && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
         const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)) *
                                h->mean_edge;
         size_t n_big = 0;

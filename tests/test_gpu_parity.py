@@ -1014,8 +1014,29 @@ def test_vector_filter_through_the_multigrid_path(ifl, oracle_mod, turnover, mon
     # two runs: the same bits (a fixed operator per column), and n = 2 pairs stay on the Jacobi path
     again, _ = ifl.if_filter(h, fields, ells, 1, flags=VEC, solver=1, mg_min_ell=0.5)
     assert bool((again == out).all())
-    b2, s2 = ifl.if_filter(h, fields[:2], ells[:2], 2, flags=VEC, solver=1)
-    assert s2["code"] == 0 and s2["mg_batch_iters"] == 0
+    # n = 2 pairs: the product preconditioner V M_2 V with the same coupled cycle (scales to 16 edge lengths)
+    ells2 = mesh.h * log_spaced(1.0, 16.0, 4)
+    b2, s2 = ifl.if_filter(h, fields[:6], ells2, 2, flags=VEC, solver=1, mg_min_ell=0.5)
+    j2, sj2 = ifl.if_filter(h, fields[:6], ells2, 2, flags=VEC)
+    assert s2["code"] == 0 and sj2["code"] == 0 and s2["mg_batch_iters"] == s2["batch_iters"] > 0
+    assert np.array_equal(s2["iters"][0::2], s2["iters"][1::2])
+    assert int(s2["iters"][:, -1].max()) * 10 < int(sj2["iters"][:, -1].min())
+    for p in range(3):
+        bnorm = np.linalg.norm(np.concatenate([area * fields[2 * p], area * fields[2 * p + 1]]))
+        for j, ell in enumerate(ells2):
+            res = []
+            for x in (b2[2 * p:2 * p + 2, j], j2[2 * p:2 * p + 2, j]):
+                ax = ifl.if_apply(h, x, np.array([ell]), 2, flags=VEC)[:, 0].cpu().numpy()
+                res.append(np.linalg.norm(np.concatenate([area * fields[2 * p] - ax[0], area * fields[2 * p + 1] - ax[1]])) / bnorm)
+            xa = np.concatenate([b2[2 * p, j].cpu().numpy(), b2[2 * p + 1, j].cpu().numpy()])
+            xb = np.concatenate([j2[2 * p, j].cpu().numpy(), j2[2 * p + 1, j].cpu().numpy()])
+            tol = max(TOL_FIELD, (res[0] + res[1]) * bnorm / area.min() / np.linalg.norm(xb))      # S_2 >= M_2
+            assert rel(xa, xb) <= tol, (p, j, rel(xa, xb), tol, res)
+            if p == 0 and j <= 1:        # and the oracle's joint PCG where it finishes in seconds
+                xu, xv, info = om.solve_vector(fields[0], fields[1], float(ell), 2)
+                xr = np.concatenate([xu, xv])
+                tol = max(TOL_FIELD, (res[0] + info["true_res"]) * bnorm / area.min() / np.linalg.norm(xr))
+                assert info["status"] == 0 and rel(xa, xr) <= tol, (j, rel(xa, xr), tol)
     h.close()
 
 
