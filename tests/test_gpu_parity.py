@@ -973,7 +973,7 @@ def test_vector_filter_matches_oracle(ifl, oracle_mod, order_n):
 
 
 @pytest.mark.parametrize("turnover", ["host", "device"])
-def test_vector_filter_through_the_multigrid_path(ifl, oracle_mod, turnover, monkeypatch):
+def test_vector_filter_through_the_multigrid_path(ifl, oracle_mod, turnover, monkeypatch, tmp_path):
     """solver = 1 with IF_FLAG_VECTOR (n = 1): PCG on the coupled 2V system preconditioned by the V cycle of the
     scalar hierarchy -- smoothing and residuals on the mesh with the coupled operator (metric terms D~, T), coarse
     correction per component.  Same systems, same start, same stop test: the oracle's joint PCG is the reference, with
@@ -1014,6 +1014,13 @@ def test_vector_filter_through_the_multigrid_path(ifl, oracle_mod, turnover, mon
     # two runs: the same bits (a fixed operator per column), and n = 2 pairs stay on the Jacobi path
     again, _ = ifl.if_filter(h, fields, ells, 1, flags=VEC, solver=1, mg_min_ell=0.5)
     assert bool((again == out).all())
+    # a handle with both the metric terms and the hierarchy through if_save / if_load: the same bits
+    path = str(tmp_path / "vec_mg.ifm")
+    ifl.if_save(h, path)
+    h2 = ifl.if_load(path)
+    loaded, sl = ifl.if_filter(h2, fields, ells, 1, flags=VEC, solver=1, mg_min_ell=0.5)
+    assert sl["code"] == 0 and sl["mg_batch_iters"] == st["mg_batch_iters"] and bool((loaded == out).all())
+    h2.close()
     # n = 2 pairs: the product preconditioner V M_2 V with the same coupled cycle (scales to 16 edge lengths)
     ells2 = mesh.h * log_spaced(1.0, 16.0, 4)
     b2, s2 = ifl.if_filter(h, fields[:6], ells2, 2, flags=VEC, solver=1, mg_min_ell=0.5)
