@@ -113,7 +113,10 @@ typedef struct {
                         the device, inside each iteration's CUDA graph; the host only launches graphs and reads a
                         16-byte snapshot one launch behind (environment IF_MG_HOST_REFILL = 0 / 1 forces either way) */
     double radius;     /* if_prepare with IF_FLAG_VECTOR: R_e of the metric terms; 0 => the mean |x_v| of a dim = 3 mesh    */
-    double mg_min_ell; /* 0 => 0.5 (in mean edge lengths; right-hand sides below that stay on the Jacobi path)         */
+    double mg_min_ell; /* in mean edge lengths; right-hand sides below that stay on the Jacobi path.  0 => 0.5 when
+                          the call has 12 or more columns (right-hand sides; a (u, v) pair counts two), else the scale
+                          from which the 16-column multigrid kernels beat Jacobi-PCG on 4 or 8 columns: 1.5 / 3 / 6
+                          for more than 8 / more than 4 / up to 4 columns with n = 1, 1.5 / 2.5 with n = 2            */
 } if_options;
 
 typedef struct {

@@ -843,8 +843,16 @@ int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields
     // large scales by multigrid-preconditioned CG (option solver = 1): a stream of right-hand sides through 16 columns
     // (vector filter: through the scalar hierarchy with the coupled operator on the mesh)
     if (job != JOB_APPLY && r.opt.solver == 1 && order_n <= 2 && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
-        const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)) *
-                               h->mean_edge;
+        // default split between the paths (option mg_min_ell = 0), in mean edge lengths: with 12 or more columns in
+        // use the stream takes every scale from 0.5 up; a call with fewer leaves most of the 16 columns of the
+        // multigrid kernels empty, and Jacobi-PCG on 4 or 8 columns is faster at the small scales (measured on config
+        // 4's mesh, one field: 1 / 4 / 8 right-hand sides break even near 6 / 6 / 3 edge lengths for n = 1; n = 2,
+        // whose Jacobi iterations grow with l^2, from about 2.5 / 1.5)
+        const size_t cols = rhs.size() * (r.vec ? 2 : 1);
+        const double dflt = cols >= 12 ? (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)
+                          : order_n == 1 ? (cols > 8 ? 1.5 : cols > 4 ? 3.0 : 6.0)
+                                         : (cols > 4 ? 1.5 : 2.5);
+        const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : dflt) * h->mean_edge;
         size_t n_big = 0;
         while (n_big < rhs.size() && rhs[n_big].ell >= min_ell) ++n_big;
         if (n_big > 0) {

@@ -798,6 +798,30 @@ def test_multigrid_turnover_on_device_matches_host_refill(ifl, oracle_mod, order
     h.close()
 
 
+def test_default_split_between_the_paths_depends_on_the_number_of_columns(ifl):
+    """mg_min_ell = 0 (default): with 12 or more right-hand sides every scale from 0.5 mean edges goes through the
+    multigrid stream; a call with fewer would leave most of its 16 columns empty, so its small scales stay on
+    Jacobi-PCG (narrower kernels) and only the scales beyond the measured break-even (6 / 3 / 1.5 edge lengths for up
+    to 4 / up to 8 / fewer than 12 columns, n = 1) use the hierarchy.  The answers do not depend on the split."""
+    w = make_config(4, level=5, n_fields=2, n_ells=8, ell_max=32.0)        # scales 1 ... 32 edge lengths
+    h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
+    ref, sr = ifl.if_filter(h, w.fields, w.ells, 1)                        # Jacobi-PCG
+    many, sm = ifl.if_filter(h, w.fields, w.ells, 1, solver=1)             # 16 right-hand sides: all through the stream
+    assert sm["code"] == 0 and sm["mg_batch_iters"] == sm["batch_iters"] > 0
+    few_small, s1 = ifl.if_filter(h, w.fields[:1], w.ells[:3], 1, solver=1)      # 3 right-hand sides below 6 edges
+    assert s1["code"] == 0 and s1["mg_batch_iters"] == 0
+    forced, s2 = ifl.if_filter(h, w.fields[:1], w.ells[:3], 1, solver=1, mg_min_ell=0.5)
+    assert s2["mg_batch_iters"] == s2["batch_iters"] > 0
+    few_large, s3 = ifl.if_filter(h, w.fields[:1], w.ells[5:], 1, solver=1)      # 3 right-hand sides beyond 6 edges
+    assert s3["mg_batch_iters"] == s3["batch_iters"] > 0
+    mixed, s4 = ifl.if_filter(h, w.fields[:1], w.ells, 1, solver=1)              # 8 right-hand sides: split at 3 edges
+    assert 0 < s4["mg_batch_iters"] < s4["batch_iters"]
+    scale = float(ref.abs().max())
+    for got, want in ((many, ref), (few_small, ref[:1, :3]), (forced, ref[:1, :3]), (few_large, ref[:1, 5:]), (mixed, ref[:1])):
+        assert float((got - want).abs().max()) <= 1e-9 * scale
+    h.close()
+
+
 def test_legacy_default_stream_runs_without_graphs(ifl, monkeypatch):
     """Stream 0 (the legacy default stream) cannot be captured: both stream loops then launch their kernels directly.
     Same kernels in the same order, so the same bits as the graph path on a side stream -- Jacobi-PCG, the multigrid
