@@ -114,9 +114,9 @@ typedef struct {
                         16-byte snapshot one launch behind (environment IF_MG_HOST_REFILL = 0 / 1 forces either way) */
     double radius;     /* if_prepare with IF_FLAG_VECTOR: R_e of the metric terms; 0 => the mean |x_v| of a dim = 3 mesh    */
     double mg_min_ell; /* in mean edge lengths; right-hand sides below that stay on the Jacobi path.  0 => 0.5 when
-                          the call has 12 or more columns (right-hand sides; a (u, v) pair counts two), else the scale
-                          from which the 16-column multigrid kernels beat Jacobi-PCG on 4 or 8 columns: 1.5 / 3 / 6
-                          for more than 8 / more than 4 / up to 4 columns with n = 1, 1.5 / 2.5 with n = 2            */
+                          the call has 12 or more columns (right-hand sides; a (u, v) pair counts two); a call with
+                          fewer runs 4- or 8-column kernels, which cost more per right-hand side, and Jacobi-PCG keeps
+                          its smallest scales: n = 1 up to 2.5 (up to 4 columns) or 1.5 edge lengths, n = 2 up to 1  */
 } if_options;
 
 typedef struct {

@@ -60,19 +60,20 @@ struct MgMat {                        // one level's (S, M) pair
 // short rows of the fine levels; SL = 4 (one row per warp, slices added with two shuffles) for the coarse levels
 // whose rows have hundreds of entries and would otherwise be walked serially.
 // MODE 0: y = A x ;  MODE 1: y = r - A x ;  MODE 2: y = x + omega (r - A x) / d        with A = M + c S per column
-template <int MODE, int SL>
+template <int MODE, int SL, int K = MGK>
 __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ x,
                                                     const double* __restrict__ r, double* __restrict__ y) {
-    constexpr int WPB = BLOCK / (8 * SL);
-    const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
+    constexpr int TPR = K / 2, RPW = 32 / TPR;         // lanes per row (one column pair each), rows per warp at SL = 1
+    constexpr int WPB = BLOCK / (TPR * SL);
+    const int l = threadIdx.x % TPR, sl = (threadIdx.x / TPR) % SL;
     if (ctrl->all_done) return;
     const double2 cc = ld2(ctrl->c1, 2 * l);
     // (rows are padded to whole warps by the loop bound: every lane of a warp takes part in the shuffles)
     // a block walks a contiguous range of rows, WPB at a time: neighbouring rows gather the same rows of x, which
     // the L1 then serves (a grid-stride assignment sends every gather to the L2)
     const int64_t per_block = ((g.n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;
-    const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, (g.n + 3) / 4 * 4);
-    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / (8 * SL); row < row_end; row += WPB) {
+    const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, (g.n + RPW - 1) / RPW * RPW);
+    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / (TPR * SL); row < row_end; row += WPB) {
         double2 s = {0.0, 0.0};
         const bool live = row < g.n;
         const int64_t k1 = live ? g.rowptr[row + 1] : 0;
@@ -87,7 +88,7 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, const C
                 w[j] = g.sm[kk];
             }
 #pragma unroll
-            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * MGK + 2 * l);
+            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * K + 2 * l);
 #pragma unroll
             for (int j = 0; j < MG_UB; ++j)
                 if (k + j * SL < k1) {
@@ -95,10 +96,10 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, const C
                     s.y = fma(fma(cc.y, w[j].x, w[j].y), v[j].y, s.y);
                 }
         }
-        if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 8);  s.y += __shfl_xor_sync(0xffffffffu, s.y, 8); }
-        if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 16); s.y += __shfl_xor_sync(0xffffffffu, s.y, 16); }
+        if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, TPR);  s.y += __shfl_xor_sync(0xffffffffu, s.y, TPR); }
+        if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 2 * TPR); s.y += __shfl_xor_sync(0xffffffffu, s.y, 2 * TPR); }
         if (sl != 0 || !live) continue;
-        const int64_t ri = row * MGK + 2 * l;
+        const int64_t ri = row * K + 2 * l;
         if (MODE == 0) {
             st2(y, ri, s);
         } else {
@@ -116,15 +117,16 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_apply(MgMat g, const C
 }
 
 // e = omega r / d  (Jacobi sweep from a zero initial guess)
+template <int K = MGK>
 __global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ r,
                                                       double* __restrict__ e) {
-    constexpr int TPR = MGK / 2;
+    constexpr int TPR = K / 2;
     constexpr int ROWS = BLOCK / TPR;
     const int l = threadIdx.x % TPR;
     if (ctrl->all_done) return;
     const double2 cc = ld2(ctrl->c1, 2 * l);
     for (int64_t row = (int64_t)blockIdx.x * ROWS + threadIdx.x / TPR; row < g.n; row += (int64_t)gridDim.x * ROWS) {
-        const int64_t ri = row * MGK + 2 * l;
+        const int64_t ri = row * K + 2 * l;
         const double2 d = g.diag[row];
         const double2 rv = ld2(r, ri);
         st2(e, ri, make_double2(g.omega * rv.x / fma(cc.x, d.x, d.y), g.omega * rv.y / fma(cc.y, d.x, d.y)));
@@ -132,17 +134,18 @@ __global__ void __launch_bounds__(BLOCK) k_mg_jacobi0(MgMat g, const Ctrl* __res
 }
 
 // y (+)= B x for a scalar CSR matrix (restriction R, prolongation P); thread mapping as above
-template <int ACC, int SL>
+template <int ACC, int SL, int K = MGK>
 __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                                                   const double* __restrict__ val, int64_t n,
                                                   const Ctrl* __restrict__ ctrl, const double* __restrict__ x,
                                                   double* __restrict__ y) {
-    constexpr int WPB = BLOCK / (8 * SL);
+    constexpr int TPR = K / 2, RPW = 32 / TPR;
+    constexpr int WPB = BLOCK / (TPR * SL);
     if (ctrl->all_done) return;
-    const int l = threadIdx.x % 8, sl = (threadIdx.x / 8) % SL;
+    const int l = threadIdx.x % TPR, sl = (threadIdx.x / TPR) % SL;
     const int64_t per_block = ((n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;   // contiguous rows per block
-    const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, (n + 3) / 4 * 4);
-    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / (8 * SL); row < row_end; row += WPB) {
+    const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, (n + RPW - 1) / RPW * RPW);
+    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / (TPR * SL); row < row_end; row += WPB) {
         double2 s = {0.0, 0.0};
         const bool live = row < n;
         const int64_t k1 = live ? rowptr[row + 1] : 0;
@@ -157,7 +160,7 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __r
                 w[j] = val[kk];
             }
 #pragma unroll
-            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * MGK + 2 * l);
+            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * K + 2 * l);
 #pragma unroll
             for (int j = 0; j < MG_UB; ++j)
                 if (k + j * SL < k1) {
@@ -165,10 +168,10 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __r
                     s.y = fma(w[j], v[j].y, s.y);
                 }
         }
-        if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 8);  s.y += __shfl_xor_sync(0xffffffffu, s.y, 8); }
-        if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 16); s.y += __shfl_xor_sync(0xffffffffu, s.y, 16); }
+        if (SL >= 2) { s.x += __shfl_xor_sync(0xffffffffu, s.x, TPR);  s.y += __shfl_xor_sync(0xffffffffu, s.y, TPR); }
+        if (SL >= 4) { s.x += __shfl_xor_sync(0xffffffffu, s.x, 2 * TPR); s.y += __shfl_xor_sync(0xffffffffu, s.y, 2 * TPR); }
         if (sl != 0 || !live) continue;
-        const int64_t ri = row * MGK + 2 * l;
+        const int64_t ri = row * K + 2 * l;
         if (ACC) { const double2 o = ld2(y, ri); s.x += o.x; s.y += o.y; }
         st2(y, ri, s);
     }
@@ -177,22 +180,24 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_csr(const int64_t* __r
 // Prolongation onto the mesh fused with the first sweep:  e = omega r / d + P e_c  (8 threads per row as above; the
 // prolongator has 2.6 entries per row).  k_spmm<16, MGR> then does not store its e = omega r'/d, and this kernel
 // reads r' where k_mg_csr<1, 1> would read e back: one pass over a [V][16] vector less per iteration.
+template <int K = MGK>
 __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_prolong0(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                                                        const double* __restrict__ val, MgMat g, const Ctrl* __restrict__ ctrl,
                                                        const double* __restrict__ x, const double* __restrict__ r0,
                                                        const double* __restrict__ r1, int r_select,
                                                        double* __restrict__ y) {
-    constexpr int WPB = BLOCK / 8;
+    constexpr int TPR = K / 2;
+    constexpr int WPB = BLOCK / TPR;
     // r_select: the residual k_spmm<16, MGR> has just written, r[cur_r ^ 1] of the double buffer (r0, r1); else r0
     const double* __restrict__ r = r_select ? (ctrl->cur_r ? r0 : r1) : r0;
-    const int l = threadIdx.x % 8;
+    const int l = threadIdx.x % TPR;
     if (ctrl->all_done) return;
     const double2 cc = ld2(ctrl->c1, 2 * l);
     const int64_t n = g.n;
     const int64_t per_block = ((n + gridDim.x - 1) / gridDim.x + WPB - 1) / WPB * WPB;   // contiguous rows per block
     const int64_t row_end = min((int64_t)(blockIdx.x + 1) * per_block, n);
-    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / 8; row < row_end; row += WPB) {
-        const int64_t ri = row * MGK + 2 * l;
+    for (int64_t row = (int64_t)blockIdx.x * per_block + threadIdx.x / TPR; row < row_end; row += WPB) {
+        const int64_t ri = row * K + 2 * l;
         const double2 rv = ld2(r, ri);
         const double2 d = g.diag[row];
         double2 s = {0.0, 0.0};
@@ -208,7 +213,7 @@ __global__ void __launch_bounds__(BLOCK, IF_MG_MINB) k_mg_prolong0(const int64_t
                 w[j] = val[kk];
             }
 #pragma unroll
-            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * MGK + 2 * l);
+            for (int j = 0; j < MG_UB; ++j) v[j] = ld2(x, (int64_t)cj[j] * K + 2 * l);
 #pragma unroll
             for (int j = 0; j < MG_UB; ++j)
                 if (k + j < k1) {
@@ -280,18 +285,19 @@ __host__ __device__ inline RowsLayout rows_layout(int cap) {
 #ifndef IF_ROWS_MINB_PAIR
 #define IF_ROWS_MINB_PAIR 2
 #endif
-template <int KIND>
+template <int KIND, int K = MGK>
 __global__ void __launch_bounds__(BLOCK, KIND <= 1 ? IF_ROWS_MINB_PAIR : 4) k_mg_rows(RowsArgs a, const Ctrl* __restrict__ ctrl) {
+    constexpr int TPR = K / 2;
     constexpr bool PAIR = KIND <= ROWS_SWEEP;
     // gathers a thread has in flight: rows of the level matrices have a dozen entries and more, prolongator rows 2-5
     constexpr int ROWS_UB = (KIND == ROWS_ACC || KIND == ROWS_PROLONG0) ? 4 : (KIND <= ROWS_SWEEP ? IF_ROWS_UB_PAIR : 8);
     constexpr bool OWN0 = KIND != ROWS_SET, OWN1 = KIND == ROWS_SWEEP, DIAG = KIND == ROWS_SWEEP || KIND == ROWS_PROLONG0;
-    constexpr int RPT = ROWS_PER_CTA / (BLOCK / 8);      // rows per thread group
+    constexpr int RPT = ROWS_PER_CTA / (BLOCK / TPR);      // rows per thread group
     if (ctrl->all_done) return;
     extern __shared__ __align__(128) unsigned char smem[];
     const RowsLayout L = rows_layout<KIND>(a.cap);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bytes - 16);
-    const int tid = threadIdx.x, l = tid % 8, g = tid / 8;
+    const int tid = threadIdx.x, l = tid % TPR, g = tid / TPR;
     const int64_t r0 = (int64_t)blockIdx.x * ROWS_PER_CTA;
     const int nr = (int)min((int64_t)ROWS_PER_CTA, a.n - r0);
     if (tid == 0) {
@@ -318,7 +324,7 @@ __global__ void __launch_bounds__(BLOCK, KIND <= 1 ? IF_ROWS_MINB_PAIR : 4) k_mg
     double2 o0n = {0.0, 0.0}, o1n = {0.0, 0.0}, dgn = {0.0, 0.0};
     auto load_own = [&](int r) {
         if (r < nr) {
-            const int64_t ri = (r0 + r) * MGK + 2 * l;
+            const int64_t ri = (r0 + r) * K + 2 * l;
             if (OWN0) o0n = ld2(own0, ri);
             if (OWN1) o1n = ld2(a.own1, ri);
             if (DIAG) dgn = a.diag[r0 + r];
@@ -335,10 +341,10 @@ __global__ void __launch_bounds__(BLOCK, KIND <= 1 ? IF_ROWS_MINB_PAIR : 4) k_mg
     const int64_t kA = k0 & ~3LL, kB = PAIR ? k0 : (k0 & ~1LL);
 #pragma unroll
     for (int i = 0; i < RPT; ++i) {
-        const int r = g + i * (BLOCK / 8);
+        const int r = g + i * (BLOCK / TPR);
         if (r >= nr) break;
         const double2 o0c = o0n, o1c = o1n, dgc = dgn;
-        load_own(r + BLOCK / 8);
+        load_own(r + BLOCK / TPR);
         const int64_t kb = srp[r], ke = srp[r + 1];
         double2 s = {0.0, 0.0};
         for (int64_t k = kb; k < ke; k += ROWS_UB) {
@@ -347,7 +353,7 @@ __global__ void __launch_bounds__(BLOCK, KIND <= 1 ? IF_ROWS_MINB_PAIR : 4) k_mg
 #pragma unroll
             for (int j = 0; j < ROWS_UB; ++j) cj[j] = scol[(k + j < ke ? k + j : k) - kA];
 #pragma unroll
-            for (int j = 0; j < ROWS_UB; ++j) v[j] = ld2(a.x, (int64_t)cj[j] * MGK + 2 * l);
+            for (int j = 0; j < ROWS_UB; ++j) v[j] = ld2(a.x, (int64_t)cj[j] * K + 2 * l);
 #pragma unroll
             for (int j = 0; j < ROWS_UB; ++j)
                 if (k + j < ke) {
@@ -362,7 +368,7 @@ __global__ void __launch_bounds__(BLOCK, KIND <= 1 ? IF_ROWS_MINB_PAIR : 4) k_mg
                     }
                 }
         }
-        const int64_t ri = (r0 + r) * MGK + 2 * l;
+        const int64_t ri = (r0 + r) * K + 2 * l;
         if (KIND == ROWS_SET) {
             st2(a.y, ri, s);
         } else if (KIND == ROWS_ACC) {
@@ -434,18 +440,19 @@ __global__ void __launch_bounds__(64) k_mg_coarse_factor(MgMat g, const Ctrl* __
 }
 
 // e = K^-1 r on the coarsest level, one block per column
+template <int K = MGK>
 __global__ void __launch_bounds__(64) k_mg_coarse(MgMat g, const Ctrl* __restrict__ ctrl, const double* __restrict__ inv,
                                                   const double* __restrict__ r, double* __restrict__ e) {
     __shared__ double v[MG_COARSEST];
     const int c = blockIdx.x, t = threadIdx.x, n = (int)g.n;
     if (ctrl->all_done) return;
-    for (int i = t; i < n; i += 64) v[i] = r[(int64_t)i * MGK + c];
+    for (int i = t; i < n; i += 64) v[i] = r[(int64_t)i * K + c];
     __syncthreads();
     const double* a = inv + (size_t)c * MG_COARSEST * MG_COARSEST;
     for (int i = t; i < n; i += 64) {
         double s = 0.0;
         for (int j = 0; j < n; ++j) s = fma(a[i * MG_COARSEST + j], v[j], s);
-        e[(int64_t)i * MGK + c] = s;
+        e[(int64_t)i * K + c] = s;
     }
 }
 
@@ -484,8 +491,8 @@ inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, int order_n) 
 // level 0: the prolongation kernel can form e = omega r'/d itself (short prolongator rows only)
 inline bool mg_fused_prolongation(const MgLevel& g) { return g.p_nnz < IF_MG_WIDE * g.n; }
 inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n, g.omega}; }
-inline int mg_grid(const if_mesh_s* h, int64_t n, int sl = 1) {
-    const int64_t rows = BLOCK / (8 * sl);
+inline int mg_grid(const if_mesh_s* h, int64_t n, int tpr, int sl = 1) {
+    const int64_t rows = BLOCK / (tpr * sl);
     return (int)std::max<int64_t>(1, std::min<int64_t>((n + rows - 1) / rows, (int64_t)h->n_sm * IF_MG_BPS));
 }
 
@@ -499,7 +506,7 @@ constexpr size_t ROWS_SMEM_MAX = 200 * 1024;      // dynamic shared memory a k_m
 constexpr size_t ROWS_SMEM_SM = 220 * 1024;       // what the CTAs of one SM share
 
 // Launch k_mg_rows<KIND> if the entries of a CTA's rows fit its shared memory; *done = false means "use the CSR kernel".
-template <int KIND>
+template <int KIND, int K>
 int launch_rows(const Run& r, RowsArgs a, int cap, bool* done) {
     *done = false;
     if (!IF_MG_ROWS || cap <= 0 || a.n < 4 * ROWS_PER_CTA) return IF_OK;
@@ -508,37 +515,39 @@ int launch_rows(const Run& r, RowsArgs a, int cap, bool* done) {
     a.cap = cap;
     a.stages = 1;
     const unsigned grid = (unsigned)((a.n + ROWS_PER_CTA - 1) / ROWS_PER_CTA);
-    k_mg_rows<KIND><<<grid, BLOCK, L.bytes, r.st>>>(a, r.w.ctrl);
+    k_mg_rows<KIND, K><<<grid, BLOCK, L.bytes, r.st>>>(a, r.w.ctrl);
     IF_LAUNCH_CHECK();
     *done = true;
     return IF_OK;
 }
 
+template <int K>
 int mg_setup(Run& r) {
     const if_mesh_s* h = r.h;
-    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_RES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
-    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
-    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_SET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
-    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
-    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_PROLONG0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_RES, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_SWEEP, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_SET, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_ACC, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
+    IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_rows<ROWS_PROLONG0, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROWS_SMEM_MAX));
     IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_coarse_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MG_FACTOR_SMEM));
     const int64_t tiles = (h->n_vert + TILE_ROWS - 1) / TILE_ROWS;
     int rc;
     if (r.vec) {      // vector filter: the coupled operator in the level-0 kernels of the cycle
-        if ((rc = resident_grid(k_spmm<MGK, MODE_AX, true>, TileSmem<MGK, MODE_AX, true>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
-        if ((rc = resident_grid(k_spmm<MGK, MODE_MGR, true>, TileSmem<MGK, MODE_MGR, true>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_AX, true>, TileSmem<K, MODE_AX, true>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<K, MODE_AX>::NT))) return rc;
+        if ((rc = resident_grid(k_spmm<K, MODE_MGR, true>, TileSmem<K, MODE_MGR, true>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<K, MODE_MGR>::NT))) return rc;
         if (r.order_n == 2 &&
-            (rc = resident_grid(k_spmm<MGK, MODE_MGR0, true>, TileSmem<MGK, MODE_MGR0, true>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<MGK, MODE_MGR0>::NT))) return rc;
+            (rc = resident_grid(k_spmm<K, MODE_MGR0, true>, TileSmem<K, MODE_MGR0, true>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<K, MODE_MGR0>::NT))) return rc;
         return IF_OK;
     }
-    if ((rc = resident_grid(k_spmm<MGK, MODE_AX>, TileSmem<MGK, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<MGK, MODE_AX>::NT))) return rc;
-    if ((rc = resident_grid(k_spmm<MGK, MODE_MGR>, TileSmem<MGK, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<MGK, MODE_MGR>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_AX>, TileSmem<K, MODE_AX>::bytes, h->n_sm, tiles, &r.mgg.ax, SpmmCfg<K, MODE_AX>::NT))) return rc;
+    if ((rc = resident_grid(k_spmm<K, MODE_MGR>, TileSmem<K, MODE_MGR>::bytes, h->n_sm, tiles, &r.mgg.mgr, SpmmCfg<K, MODE_MGR>::NT))) return rc;
     if (r.order_n == 2 &&
-        (rc = resident_grid(k_spmm<MGK, MODE_MGR0>, TileSmem<MGK, MODE_MGR0>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<MGK, MODE_MGR0>::NT))) return rc;
+        (rc = resident_grid(k_spmm<K, MODE_MGR0>, TileSmem<K, MODE_MGR0>::bytes, h->n_sm, tiles, &r.mgg.mgr0, SpmmCfg<K, MODE_MGR0>::NT))) return rc;
     return IF_OK;
 }
 
 // y = R x (restriction of level l, rows = the coarse level) and y += P x (prolongation, rows = level l)
+template <int K>
 int mg_restrict(const Run& r, const MgLevel& g, const double* x, double* y) {
     const if_mesh_s* h = r.h;
     const bool wide_r = g.p_nnz >= IF_MG_WIDE * g.n_coarse;
@@ -546,14 +555,15 @@ int mg_restrict(const Run& r, const MgLevel& g, const double* x, double* y) {
     int rc;
     if (!wide_r) {
         RowsArgs a{g.r_rowptr, g.r_col, g.r_val, nullptr, g.n_coarse, x, nullptr, nullptr, y, 0.0, 0, 0, 0};
-        if ((rc = launch_rows<ROWS_SET>(r, a, g.cap_r, &done))) return rc;
+        if ((rc = launch_rows<ROWS_SET, K>(r, a, g.cap_r, &done))) return rc;
         if (done) return IF_OK;
     }
-    if (wide_r) k_mg_csr<0, 4><<<mg_grid(h, g.n_coarse, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, r.w.ctrl, x, y);
-    else k_mg_csr<0, 1><<<mg_grid(h, g.n_coarse), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, r.w.ctrl, x, y);
+    if (wide_r) k_mg_csr<0, 4, K><<<mg_grid(h, g.n_coarse, K / 2, 4), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, r.w.ctrl, x, y);
+    else k_mg_csr<0, 1, K><<<mg_grid(h, g.n_coarse, K / 2), BLOCK, 0, r.st>>>(g.r_rowptr, g.r_col, g.r_val, g.n_coarse, r.w.ctrl, x, y);
     IF_LAUNCH_CHECK();
     return IF_OK;
 }
+template <int K>
 int mg_prolong_add(const Run& r, const MgLevel& g, const double* x, double* y) {
     const if_mesh_s* h = r.h;
     const bool wide_p = g.p_nnz >= IF_MG_WIDE * g.n;
@@ -561,11 +571,11 @@ int mg_prolong_add(const Run& r, const MgLevel& g, const double* x, double* y) {
     int rc;
     if (!wide_p) {
         RowsArgs a{g.p_rowptr, g.p_col, g.p_val, nullptr, g.n, x, y, nullptr, y, 0.0, 0, 0, 0};
-        if ((rc = launch_rows<ROWS_ACC>(r, a, g.cap_p, &done))) return rc;
+        if ((rc = launch_rows<ROWS_ACC, K>(r, a, g.cap_p, &done))) return rc;
         if (done) return IF_OK;
     }
-    if (wide_p) k_mg_csr<1, 4><<<mg_grid(h, g.n, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, r.w.ctrl, x, y);
-    else k_mg_csr<1, 1><<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, r.w.ctrl, x, y);
+    if (wide_p) k_mg_csr<1, 4, K><<<mg_grid(h, g.n, K / 2, 4), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, r.w.ctrl, x, y);
+    else k_mg_csr<1, 1, K><<<mg_grid(h, g.n, K / 2), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, g.n, r.w.ctrl, x, y);
     IF_LAUNCH_CHECK();
     return IF_OK;
 }
@@ -586,6 +596,7 @@ constexpr int MG_MAX_NU = 8;
 // Levels >= 1 of a V cycle: e = V_l r.  nu Jacobi sweeps (the first from a zero guess), coarse correction, nu sweeps;
 // nu = r.mg_nu[1] on level 1 and r.mg_nu[2] below.  R holds r and is not changed; E, T, E2 are work buffers of the
 // level; *result is the one that holds e.
+template <int K>
 int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, double* T, double* E2, double** result,
               IterTimer* tm) {
     const if_mesh_s* h = r.h;
@@ -595,7 +606,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
     const bool last = l == h->mg_levels - 1;
     int rc;
     if (last && g.n <= MG_COARSEST) {
-        k_mg_coarse<<<MGK, 64, 0, r.st>>>(gm, ctrl, b.coarse_inv, R, E);
+        k_mg_coarse<K><<<K, 64, 0, r.st>>>(gm, ctrl, b.coarse_inv, R, E);
         IF_LAUNCH_CHECK();
         if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
         *result = E;
@@ -603,8 +614,8 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
     }
     // rows with many entries (coarse levels, restriction) are split over four entry slices
     const bool wide = g.nnz >= IF_MG_WIDE * g.n;
-    const int grid1 = mg_grid(h, g.n);
-    const int grid = mg_grid(h, g.n, wide ? 4 : 1);
+    const int grid1 = mg_grid(h, g.n, K / 2);
+    const int grid = mg_grid(h, g.n, K / 2, wide ? 4 : 1);
     // sub 1: out = R - K v ;  sub 2: out = v + omega (R - K v) / d
     auto apply = [&](int sub, double omega, const double* v, double* out) -> int {
         gm.omega = omega;
@@ -612,16 +623,16 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
             bool done = false;
             int rcc;
             RowsArgs a{g.rowptr, g.col, g.sm, g.diag, g.n, v, R, v, out, omega, 0, 0, 0};
-            if (sub == 1) rcc = launch_rows<ROWS_RES>(r, a, g.cap_a, &done);
-            else rcc = launch_rows<ROWS_SWEEP>(r, a, g.cap_a, &done);
+            if (sub == 1) rcc = launch_rows<ROWS_RES, K>(r, a, g.cap_a, &done);
+            else rcc = launch_rows<ROWS_SWEEP, K>(r, a, g.cap_a, &done);
             if (rcc != IF_OK || done) return rcc;
         }
         if (sub == 1) {
-            if (wide) k_mg_apply<1, 4><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
-            else k_mg_apply<1, 1><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
+            if (wide) k_mg_apply<1, 4, K><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
+            else k_mg_apply<1, 1, K><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
         } else {
-            if (wide) k_mg_apply<2, 4><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
-            else k_mg_apply<2, 1><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
+            if (wide) k_mg_apply<2, 4, K><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
+            else k_mg_apply<2, 1, K><<<grid, BLOCK, 0, r.st>>>(gm, ctrl, v, R, out);
         }
         IF_LAUNCH_CHECK();
         return IF_OK;
@@ -635,7 +646,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
     double* cur = E;
     double* spare[2] = {E2, T};
     gm.omega = om[0];
-    k_mg_jacobi0<<<grid1, BLOCK, 0, r.st>>>(gm, ctrl, R, cur);
+    k_mg_jacobi0<K><<<grid1, BLOCK, 0, r.st>>>(gm, ctrl, R, cur);
     IF_LAUNCH_CHECK();
     for (int k = 1; k < nu; ++k) {
         if ((rc = apply(2, om[k], cur, spare[0]))) return rc;
@@ -648,12 +659,12 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
     }
     if ((rc = apply(1, 0.0, cur, spare[1]))) return rc;                // residual of the level
     double* const* nb = b.lev[l + 1];
-    if ((rc = mg_restrict(r, g, spare[1], nb[0]))) return rc;
+    if ((rc = mg_restrict<K>(r, g, spare[1], nb[0]))) return rc;
     if (l == 1 && tm && (rc = tm->mark(r.st, MGT_LEVEL1))) return rc;
     double* ec = nullptr;
-    if ((rc = mg_vcycle(r, b, l + 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
+    if ((rc = mg_vcycle<K>(r, b, l + 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
     if (l == 1 && tm && (rc = tm->mark(r.st, MGT_COARSE))) return rc;
-    if ((rc = mg_prolong_add(r, g, ec, cur))) return rc;
+    if ((rc = mg_prolong_add<K>(r, g, ec, cur))) return rc;
     for (int k = 0; k < nu; ++k) {
         if ((rc = apply(2, om[nu - 1 - k], cur, spare[k & 1]))) return rc;
         std::swap(cur, spare[k & 1]);
@@ -670,6 +681,7 @@ int mg_vcycle(const Run& r, const MgBuffers& b, int l, double* R, double* E, dou
 // Then restriction, coarse levels, prolongation, nu0 sweeps, the last one with sub-mode `final_sub` into `out`.
 // R is (R0, R1) picked on the device (r_select, see SpmmArgs) or R0.  Work buffers: b.za, b.zb, b.t (and out, which
 // is only written by the last sweep).
+template <int K>
 int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const double* R1, int r_select, double* out,
                     int final_sub, IterTimer* tm) {
     const if_mesh_s* h = r.h;
@@ -681,7 +693,7 @@ int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const do
     int rc;
     auto sweep = [&](int sub, double omega, const double* v, double* dst) -> int {
         SpmmArgs a{v, R0, const_cast<double*>(R1), dst, nullptr, sub, 0, omega, 0.0, r_select};
-        return launch_spmm<MGK, MODE_AX>(r, r.mgg.ax, a);
+        return launch_spmm<K, MODE_AX>(r, r.mgg.ax, a);
     };
     double* cur = b.za;
     if (nu >= 2) {
@@ -694,19 +706,19 @@ int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const do
         if (tm && (rc = tm->mark(r.st, MGT_LAST))) return rc;
     }
     double* const* nb = b.lev[1];
-    if ((rc = mg_restrict(r, g, b.t, nb[0]))) return rc;
+    if ((rc = mg_restrict<K>(r, g, b.t, nb[0]))) return rc;
     if (tm && (rc = tm->mark(r.st, MGT_RESTRICT0))) return rc;
     double* ec = nullptr;
-    if ((rc = mg_vcycle(r, b, 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
+    if ((rc = mg_vcycle<K>(r, b, 1, nb[0], nb[1], nb[2], nb[3], &ec, tm))) return rc;
     if (nu == 1 && mg_fused_prolongation(g) && !r.vec) {    // e = omega R/d formed again here: it has not been stored
         bool done = false;
         RowsArgs a{g.p_rowptr, g.p_col, g.p_val, g.diag, g.n, ec, R0, R1, cur, g.omega, r_select, 0, 0};
-        if ((rc = launch_rows<ROWS_PROLONG0>(r, a, g.cap_p, &done))) return rc;
+        if ((rc = launch_rows<ROWS_PROLONG0, K>(r, a, g.cap_p, &done))) return rc;
         if (!done) {
-            k_mg_prolong0<<<mg_grid(h, g.n), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, mg_mat(g), ctrl, ec, R0, R1, r_select, cur);
+            k_mg_prolong0<K><<<mg_grid(h, g.n, K / 2), BLOCK, 0, r.st>>>(g.p_rowptr, g.p_col, g.p_val, mg_mat(g), ctrl, ec, R0, R1, r_select, cur);
             IF_LAUNCH_CHECK();
         }
-    } else if ((rc = mg_prolong_add(r, g, ec, cur))) {
+    } else if ((rc = mg_prolong_add<K>(r, g, ec, cur))) {
         return rc;
     }
     if (tm && (rc = tm->mark(r.st, MGT_PROLONG0))) return rc;
@@ -725,6 +737,7 @@ int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const do
 
 // ONE iteration of multigrid-preconditioned CG for the 16 columns (see the head of this file); every pointer that
 // alternates between iterations is picked on the device, so the sequence is the same every time (CUDA graph).
+template <int K>
 int mg_enqueue_iteration(const Run& r, IterTimer* tm) {
     const if_mesh_s* h = r.h;
     const MgBuffers b = mg_layout(h, r.w, r.order_n);
@@ -740,28 +753,28 @@ int mg_enqueue_iteration(const Run& r, IterTimer* tm) {
     if (tm && (rc = tm->mark(r.st, -1))) return rc;
     if (r.order_n == 1) {
         SpmmArgs a{b.zb, b.p[0], b.x, b.q, b.p[1], 0, 1, 0.0, 0.0, 0};          // kernel A of the Jacobi path
-        if ((rc = launch_spmm<MGK, MODE_CG1>(r, r.g.cga, a))) return rc;
+        if ((rc = launch_spmm<K, MODE_CG1>(r, r.g.cga, a))) return rc;
     } else {
         SpmmArgs a{b.zb, b.p[0], b.x, b.t, b.p[1], 0, 1, 0.0, 0.0, 0};
-        if ((rc = launch_spmm<MGK, MODE_CG2A>(r, r.g.cga, a))) return rc;
+        if ((rc = launch_spmm<K, MODE_CG2A>(r, r.g.cga, a))) return rc;
         SpmmArgs c{b.t, b.p[0], nullptr, b.q, b.p[1], 0, 1, 0.0, 0.0, 0};
-        if ((rc = launch_spmm<MGK, MODE_CG2B>(r, r.g.cgb, c))) return rc;
+        if ((rc = launch_spmm<K, MODE_CG2B>(r, r.g.cgb, c))) return rc;
     }
     if (tm && (rc = tm->mark(r.st, MGT_A))) return rc;
     {
         SpmmArgs a{b.r[0], b.q, b.r[1], first_out, e_store, 0, 0, om[0], omega2, 1};
-        if ((rc = launch_spmm<MGK, MODE_MGR>(r, r.mgg.mgr, a))) return rc;
+        if ((rc = launch_spmm<K, MODE_MGR>(r, r.mgg.mgr, a))) return rc;
     }
     if (tm && (rc = tm->mark(r.st, MGT_MGR))) return rc;
-    if (r.order_n == 1) return mg_cycle_level0(r, b, b.r[0], b.r[1], 1, b.zb, 3, tm);
+    if (r.order_n == 1) return mg_cycle_level0<K>(r, b, b.r[0], b.r[1], 1, b.zb, 3, tm);
     // n = 2: y = V r', w = M y (into q, dead by now), bookkeeping with rho' = y.w; then z = V w
-    if ((rc = mg_cycle_level0(r, b, b.r[0], b.r[1], 1, b.q, 5, tm))) return rc;
+    if ((rc = mg_cycle_level0<K>(r, b, b.r[0], b.r[1], 1, b.q, 5, tm))) return rc;
     {
         SpmmArgs a{b.q, nullptr, nullptr, first_out, e_store, 0, 0, om[0], omega2, 0};
-        if ((rc = launch_spmm<MGK, MODE_MGR0>(r, r.mgg.mgr0, a))) return rc;
+        if ((rc = launch_spmm<K, MODE_MGR0>(r, r.mgg.mgr0, a))) return rc;
     }
     if (tm && (rc = tm->mark(r.st, MGT_MGR))) return rc;
-    return mg_cycle_level0(r, b, b.q, nullptr, 0, b.zb, 2, tm);
+    return mg_cycle_level0<K>(r, b, b.q, nullptr, 0, b.zb, 2, tm);
 }
 
 }  // namespace

@@ -127,7 +127,7 @@ int launch_spmm(const Run& r, int grid, const SpmmArgs& a) {
     // the vector filter's variants: every mode of the Jacobi path, and the level-0 kernels of the multigrid cycle for
     // (smoothing and residuals on the coupled operator, mg_solve.cuh)
     constexpr bool CG_MODE = MODE == MODE_PLAIN || MODE == MODE_CG1 || MODE == MODE_CG2A || MODE == MODE_CG2B ||
-                             (K == KMAX && (MODE == MODE_AX || MODE == MODE_MGR || MODE == MODE_MGR0));
+                             MODE == MODE_AX || MODE == MODE_MGR || MODE == MODE_MGR0;
     if constexpr (CG_MODE) {
         if (r.vec) {
             k_spmm<K, MODE, true><<<grid, SpmmCfg<K, MODE>::NT, TileSmem<K, MODE, true>::bytes, r.st>>>(r.m, r.w.ctrl, r.w.partials, a);
@@ -287,19 +287,16 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
     const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
     int rc;
     if (r.mg) {   // multigrid path: the column joins the stream, its first iteration forms r0 (k_mg_start)
-        if constexpr (K == KMAX) {
-            const MgBuffers b = mg_layout(h, r.w, r.order_n);
-            k_mg_start<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, d_fields, b.x, b.zb, b.r[0],
-                                                          b.r[1], b.p[0], b.p[1]);
+        const MgBuffers b = mg_layout(h, r.w, r.order_n);
+        k_mg_start<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, d_fields, b.x, b.zb, b.r[0],
+                                                      b.r[1], b.p[0], b.p[1]);
+        IF_LAUNCH_CHECK();
+        const MgLevel& gl = h->mg[h->mg_levels - 1];      // K^-1 of the coarsest level for the new columns' c1
+        if (gl.n <= MG_COARSEST) {
+            k_mg_coarse_factor<<<K, 64, MG_FACTOR_SMEM, r.st>>>(mg_mat(gl), r.w.ctrl, mask, b.coarse_inv);
             IF_LAUNCH_CHECK();
-            const MgLevel& gl = h->mg[h->mg_levels - 1];      // K^-1 of the coarsest level for the new columns' c1
-            if (gl.n <= MG_COARSEST) {
-                k_mg_coarse_factor<<<MGK, 64, MG_FACTOR_SMEM, r.st>>>(mg_mat(gl), r.w.ctrl, mask, b.coarse_inv);
-                IF_LAUNCH_CHECK();
-            }
-            return IF_OK;
         }
-        return IF_EINVAL;
+        return IF_OK;
     }
     k_ingest<K><<<eg, BLOCK, 0, r.st>>>(r.m, sp, mask, d_fields, r.w.x);
     IF_LAUNCH_CHECK();
@@ -450,7 +447,7 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
                 PollState& poll, KernelTimes* times, QueueState& q, bool first, int* compact_to) {
     int rc;
     if ((rc = setup_grids<K>(r))) return rc;
-    if (r.mg && (K != MGK || (rc = mg_setup(r)))) return rc ? rc : IF_EINVAL;
+    if (r.mg && (rc = mg_setup<K>(r))) return rc;
     const size_t R = rhs.size();
     if (compact_to) *compact_to = 0;
     auto assign = [&](unsigned mask, StartParams* sp, unsigned* started) {
@@ -501,7 +498,7 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
         const int timed_it = per_graph > 2 ? 2 : 0;
         for (int i = 0; i < per_graph && rcc == IF_OK; ++i) {
             IterTimer* tm = i == timed_it ? timer : nullptr;
-            rcc = r.mg ? mg_enqueue_iteration(r, tm) : enqueue_iteration<K>(r, tm);
+            rcc = r.mg ? mg_enqueue_iteration<K>(r, tm) : enqueue_iteration<K>(r, tm);
         }
         return rcc;
     });
@@ -516,7 +513,7 @@ int solve_phase(Run& r, Job job, const double* d_fields, const std::vector<Rhs>&
             g_launches += launches_per_graph;
         } else {
             for (int i = 0; i < per_graph; ++i)
-                if ((rc = r.mg ? mg_enqueue_iteration(r, nullptr) : enqueue_iteration<K>(r))) return rc;
+                if ((rc = r.mg ? mg_enqueue_iteration<K>(r, nullptr) : enqueue_iteration<K>(r))) return rc;
         }
         const int slot = (int)(it & 3);
         IF_CUDA_TRY(cudaMemcpyAsync(&poll.snap[slot], reinterpret_cast<const char*>(r.w.ctrl) + offsetof(Ctrl, done),
@@ -629,28 +626,29 @@ int solve_from(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& 
 
 // End and start of columns inside the stream (multigrid path): what k_turn_plan decided is carried out by the same
 // kernels the host-driven refill uses, with their masks read from the control block.
+template <int K>
 int mg_enqueue_turnover(const Run& r, Job job, double* d_out, const double* d_fields, bool first = false) {
     const if_mesh_s* h = r.h;
     const MgBuffers b = mg_layout(h, r.w, r.order_n);
-    k_turn_plan<<<1, 32, 0, r.st>>>(r.w.ctrl, r.w.queue, MGK, first ? 1 : 0, r.w.iters, r.w.status, r.w.relres);
+    k_turn_plan<<<1, 32, 0, r.st>>>(r.w.ctrl, r.w.queue, K, first ? 1 : 0, r.w.iters, r.w.status, r.w.relres);
     IF_LAUNCH_CHECK();
     if (job == JOB_SPECTRUM) {
-        k_energy<MGK><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1,
+        k_energy<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1,
                                                       h->total_area, r.w.energy);
     } else {
         const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
-        k_scatter<MGK><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1, 1, d_out, d_fields,
+        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1, 1, d_out, d_fields,
                                                   (r.opt.flags & IF_FLAG_HIGHPASS) ? 1 : 0);
     }
     IF_LAUNCH_CHECK();
     StartParams none;
     memset(&none, 0, sizeof(none));
-    k_mg_start<MGK><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, none, MASK_TURN_START, d_fields, b.x, b.zb,
+    k_mg_start<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, none, MASK_TURN_START, d_fields, b.x, b.zb,
                                                     b.r[0], b.r[1], b.p[0], b.p[1]);
     IF_LAUNCH_CHECK();
     const MgLevel& gl = h->mg[h->mg_levels - 1];
     if (gl.n <= MG_COARSEST) {
-        k_mg_coarse_factor<<<MGK, 64, MG_FACTOR_SMEM, r.st>>>(mg_mat(gl), r.w.ctrl, MASK_TURN_START, b.coarse_inv);
+        k_mg_coarse_factor<<<K, 64, MG_FACTOR_SMEM, r.st>>>(mg_mat(gl), r.w.ctrl, MASK_TURN_START, b.coarse_inv);
         IF_LAUNCH_CHECK();
     }
     return IF_OK;
@@ -660,11 +658,12 @@ int mg_enqueue_turnover(const Run& r, Job job, double* d_out, const double* d_fi
 // one CUDA graph = one iteration + the turnover, and the host only launches graphs and reads, one launch behind, how
 // many columns still hold a right-hand side.  A stopped column runs its next right-hand side in the very next iteration
 // (the host-driven refill of solve_phase, which sees a stop one launch late, loses an iteration per right-hand side).
+template <int K>
 int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
                         PollState& poll, KernelTimes* times) {
     int rc;
-    if ((rc = setup_grids<MGK>(r))) return rc;
-    if ((rc = mg_setup(r))) return rc;
+    if ((rc = setup_grids<K>(r))) return rc;
+    if ((rc = mg_setup<K>(r))) return rc;
     const size_t R = rhs.size();
     if (R == 0 || R > (size_t)MAX_RHS || !r.w.queue) return IF_EINVAL;
     std::vector<QEntry> hq(R);
@@ -684,17 +683,17 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
     // (pageable sources: both copies are staged by the runtime before the call returns)
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.queue, hq.data(), R * sizeof(QEntry), cudaMemcpyHostToDevice, r.st));
-    if ((rc = mg_enqueue_turnover(r, job, d_out, d_fields, true))) return rc;      // the first MGK right-hand sides
+    if ((rc = mg_enqueue_turnover<K>(r, job, d_out, d_fields, true))) return rc;      // the first K right-hand sides
 
     long long launches_per_graph = 0;
     GraphSet gs;
     rc = capture_graphs(r.st, gs, &launches_per_graph, [&](IterTimer* timer) {
-        const int rcc = mg_enqueue_iteration(r, timer);
-        return rcc != IF_OK ? rcc : mg_enqueue_turnover(r, job, d_out, d_fields);
+        const int rcc = mg_enqueue_iteration<K>(r, timer);
+        return rcc != IF_OK ? rcc : mg_enqueue_turnover<K>(r, job, d_out, d_fields);
     });
     if (rc != IF_OK) return rc;
     const bool use_graph = gs.exec[0] && gs.exec[1];
-    const int64_t slots = r.vec ? MGK / 2 : MGK;
+    const int64_t slots = r.vec ? K / 2 : K;
     const int64_t max_loops = ((int64_t)(R + slots - 1) / slots + 1) * ((int64_t)r.opt.max_iter + 3) + 8;
     int* snap = reinterpret_cast<int*>(poll.snap);      // four slots of four ints in the pinned snapshot buffer
     bool finished = false;
@@ -704,8 +703,8 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
             IF_CUDA_TRY(cudaGraphLaunch(gs.exec[it & 1], r.st));
             g_launches += launches_per_graph;
         } else {
-            if ((rc = mg_enqueue_iteration(r, nullptr))) return rc;
-            if ((rc = mg_enqueue_turnover(r, job, d_out, d_fields))) return rc;
+            if ((rc = mg_enqueue_iteration<K>(r, nullptr))) return rc;
+            if ((rc = mg_enqueue_turnover<K>(r, job, d_out, d_fields))) return rc;
         }
         const int slot = (int)(it & 3);
         IF_CUDA_TRY(cudaMemcpyAsync(snap + 4 * slot, reinterpret_cast<const char*>(r.w.ctrl) + offsetof(Ctrl, snap),
@@ -731,7 +730,7 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
     QueueState q;
     int rc = IF_OK;
     bool on_device = false;
-    if constexpr (K == MGK) {
+    if (r.mg) {
         // multigrid stream: column turnover on the device where an iteration is long enough to pay for the four extra
         // graph nodes (about 12 us per iteration against one idle column-iteration per right-hand side: break-even
         // near 0.5 ms per iteration = 400 k rows for n = 1, a quarter of that for n = 2; measured on configs 2 and 4),
@@ -740,7 +739,7 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
         const bool big = r.h->n_vert * (r.order_n == 1 ? 1 : 4) >= MG_DEVICE_TURNOVER_ROWS;
         const bool host_refill = env != nullptr ? atoi(env) != 0 : !big;
         on_device = r.mg && !host_refill;
-        if (on_device) rc = mg_stream_on_device(r, job, d_fields, rhs, n_ells, d_out, poll, times);
+        if (on_device) rc = mg_stream_on_device<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times);
     }
     if (!on_device) rc = solve_from<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, q, true);
     if (rc != IF_OK) return rc;
@@ -844,14 +843,15 @@ int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields
     // (vector filter: through the scalar hierarchy with the coupled operator on the mesh)
     if (job != JOB_APPLY && r.opt.solver == 1 && order_n <= 2 && r.opt.batch == MGK && r.w.mg_extra && h->mean_edge > 0.0) {
         // default split between the paths (option mg_min_ell = 0), in mean edge lengths: with 12 or more columns in
-        // use the stream takes every scale from 0.5 up; a call with fewer leaves most of the 16 columns of the
-        // multigrid kernels empty, and Jacobi-PCG on 4 or 8 columns is faster at the small scales (measured on config
-        // 4's mesh, one field: 1 / 4 / 8 right-hand sides break even near 6 / 6 / 3 edge lengths for n = 1; n = 2,
-        // whose Jacobi iterations grow with l^2, from about 2.5 / 1.5)
+        // use the stream takes every scale from 0.5 up (tuned on configs 3-5); a call with fewer runs the 4- or
+        // 8-column kernels, or leaves some of the 16 empty, and costs more per right-hand side and iteration, so
+        // Jacobi-PCG keeps the smallest scales.  Measured on config 4's mesh, one field, 1 / 4 / 8 / 10 right-hand
+        // sides: n = 1 breaks even near 2.5 / 2 / 1.5 / 1.3 edge lengths, n = 2 (whose Jacobi iterations grow with
+        // l^2) near 1.2 / 1 / below 1 / below 1.
         const size_t cols = rhs.size() * (r.vec ? 2 : 1);
         const double dflt = cols >= 12 ? (order_n == 1 ? MG_MIN_ELL_N1 : MG_MIN_ELL_N2)
-                          : order_n == 1 ? (cols > 8 ? 1.5 : cols > 4 ? 3.0 : 6.0)
-                                         : (cols > 4 ? 1.5 : 2.5);
+                          : order_n == 1 ? (cols > 4 ? 1.5 : 2.5)
+                                         : 1.0;
         const double min_ell = (r.opt.mg_min_ell > 0.0 ? r.opt.mg_min_ell : dflt) * h->mean_edge;
         size_t n_big = 0;
         while (n_big < rhs.size() && rhs[n_big].ell >= min_ell) ++n_big;
@@ -869,7 +869,11 @@ int run_job_on_device(if_handle h, Job job, const double* d_fields, int n_fields
                 if (sscanf(e, "%d,%d,%d", &a0, &a1, &a2) == 3 && a0 >= 1 && a1 >= 1 && a2 >= 1 && a0 <= MG_MAX_NU &&
                     a1 <= MG_MAX_NU && a2 <= MG_MAX_NU) { rm.mg_nu[0] = a0; rm.mg_nu[1] = a1; rm.mg_nu[2] = a2; }
             }
-            rc = solve_all<MGK>(rm, job, d_fields, big, n_ells, d_out, poll, &mgtimes, &mg_batch_iters);
+            // few right-hand sides: the 8- and 4-column variants of every kernel of the cycle (as on the Jacobi path)
+            const int Kmg = pick_k(MGK, big.size() * (r.vec ? 2 : 1));
+            rc = Kmg == 4 ? solve_all<4>(rm, job, d_fields, big, n_ells, d_out, poll, &mgtimes, &mg_batch_iters)
+               : Kmg == 8 ? solve_all<8>(rm, job, d_fields, big, n_ells, d_out, poll, &mgtimes, &mg_batch_iters)
+                          : solve_all<MGK>(rm, job, d_fields, big, n_ells, d_out, poll, &mgtimes, &mg_batch_iters);
             if (rc != IF_OK) { cudaStreamSynchronize(r.st); return rc; }
             rhs.erase(rhs.begin(), rhs.begin() + (ptrdiff_t)n_big);
             batch_iters += mg_batch_iters;

@@ -800,25 +800,30 @@ def test_multigrid_turnover_on_device_matches_host_refill(ifl, oracle_mod, order
 
 def test_default_split_between_the_paths_depends_on_the_number_of_columns(ifl):
     """mg_min_ell = 0 (default): with 12 or more right-hand sides every scale from 0.5 mean edges goes through the
-    multigrid stream; a call with fewer would leave most of its 16 columns empty, so its small scales stay on
-    Jacobi-PCG (narrower kernels) and only the scales beyond the measured break-even (6 / 3 / 1.5 edge lengths for up
-    to 4 / up to 8 / fewer than 12 columns, n = 1) use the hierarchy.  The answers do not depend on the split."""
-    w = make_config(4, level=5, n_fields=2, n_ells=8, ell_max=32.0)        # scales 1 ... 32 edge lengths
+    multigrid stream; a call with fewer runs the 4- or 8-column variants of the cycle's kernels, which cost more per
+    right-hand side, so its smallest scales stay on Jacobi-PCG up to the measured break-even (2.5 edge lengths for up
+    to 4 columns, 1.5 for up to 11, n = 1; 1 for n = 2).  The answers do not depend on the split nor on the width."""
+    w = make_config(4, level=5, n_fields=2, n_ells=8, ell_max=32.0)        # scales 1, 1.6, 2.7, 4.4, 7.2, 12, 20, 32 h
     h = ifl.if_prepare(w.mesh.coords, w.mesh.tri, None, flags=ifl.IF_FLAG_MULTIGRID)
-    ref, sr = ifl.if_filter(h, w.fields, w.ells, 1)                        # Jacobi-PCG
-    many, sm = ifl.if_filter(h, w.fields, w.ells, 1, solver=1)             # 16 right-hand sides: all through the stream
-    assert sm["code"] == 0 and sm["mg_batch_iters"] == sm["batch_iters"] > 0
-    few_small, s1 = ifl.if_filter(h, w.fields[:1], w.ells[:3], 1, solver=1)      # 3 right-hand sides below 6 edges
-    assert s1["code"] == 0 and s1["mg_batch_iters"] == 0
-    forced, s2 = ifl.if_filter(h, w.fields[:1], w.ells[:3], 1, solver=1, mg_min_ell=0.5)
-    assert s2["mg_batch_iters"] == s2["batch_iters"] > 0
-    few_large, s3 = ifl.if_filter(h, w.fields[:1], w.ells[5:], 1, solver=1)      # 3 right-hand sides beyond 6 edges
-    assert s3["mg_batch_iters"] == s3["batch_iters"] > 0
-    mixed, s4 = ifl.if_filter(h, w.fields[:1], w.ells, 1, solver=1)              # 8 right-hand sides: split at 3 edges
-    assert 0 < s4["mg_batch_iters"] < s4["batch_iters"]
-    scale = float(ref.abs().max())
-    for got, want in ((many, ref), (few_small, ref[:1, :3]), (forced, ref[:1, :3]), (few_large, ref[:1, 5:]), (mixed, ref[:1])):
-        assert float((got - want).abs().max()) <= 1e-9 * scale
+    scale = None
+    for order_n, top in ((1, 8), (2, 6)):
+        ells = w.ells[:top]
+        ref, sr = ifl.if_filter(h, w.fields, ells, order_n)                    # Jacobi-PCG
+        scale = float(ref.abs().max())
+        many, sm = ifl.if_filter(h, w.fields, ells, order_n, solver=1)         # 12-16 right-hand sides: all in the stream
+        assert sm["code"] == 0 and sm["mg_batch_iters"] == sm["batch_iters"] > 0
+        few_small, s1 = ifl.if_filter(h, w.fields[:1], ells[:1], order_n, solver=1)          # one, just below one mean edge
+        assert s1["code"] == 0 and s1["mg_batch_iters"] == 0
+        forced, s2 = ifl.if_filter(h, w.fields[:1], ells[:3], order_n, solver=1, mg_min_ell=0.5)     # 4 columns
+        assert s2["mg_batch_iters"] == s2["batch_iters"] > 0
+        few_large, s3 = ifl.if_filter(h, w.fields[:1], ells[3:6], order_n, solver=1)         # 3 beyond 2.5 edges
+        assert s3["mg_batch_iters"] == s3["batch_iters"] > 0
+        mixed, s4 = ifl.if_filter(h, w.fields[:1], ells, order_n, solver=1)    # 6-8 right-hand sides: 8 columns
+        assert (0 < s4["mg_batch_iters"] < s4["batch_iters"]) if order_n == 1 else s4["mg_batch_iters"] > 0
+        tol = (1e-9 if order_n == 1 else 1e-7) * scale
+        for got, want in ((many, ref), (few_small, ref[:1, :1]), (forced, ref[:1, :3]), (few_large, ref[:1, 3:6]),
+                          (mixed, ref[:1])):
+            assert float((got - want).abs().max()) <= tol, order_n
     h.close()
 
 
@@ -1063,6 +1068,14 @@ def test_vector_filter_through_the_multigrid_path(ifl, oracle_mod, turnover, mon
             xb = np.concatenate([j2[2 * p, j].cpu().numpy(), j2[2 * p + 1, j].cpu().numpy()])
             tol = max(TOL_FIELD, (res[0] + res[1]) * bnorm / area.min() / np.linalg.norm(xb))      # S_2 >= M_2
             assert rel(xa, xb) <= tol, (p, j, rel(xa, xb), tol, res)
+            if p == 0 and j == 0:        # one pair or two alone: the 4- and 8-column variants of the coupled cycle
+                for npairs in (1, 2):
+                    for order_k in (1, 2):
+                        want = (jac if order_k == 1 else j2)[:2 * npairs, 1:3]
+                        ee = (ells if order_k == 1 else ells2)[1:3]
+                        few, sf = ifl.if_filter(h, fields[:2 * npairs], ee, order_k, flags=VEC, solver=1, mg_min_ell=0.5)
+                        assert sf["code"] == 0 and sf["mg_batch_iters"] == sf["batch_iters"] > 0
+                        assert float((few - want).abs().max()) <= (1e-8 if order_k == 1 else 1e-6) * float(want.abs().max())
             if p == 0 and j <= 1:        # and the oracle's joint PCG where it finishes in seconds
                 xu, xv, info = om.solve_vector(fields[0], fields[1], float(ell), 2)
                 xr = np.concatenate([xu, xv])
