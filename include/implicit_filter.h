@@ -104,7 +104,8 @@ typedef struct {
                         2 = Jacobi-PCG explicitly).  1 => right-hand sides with l >= mg_min_ell mean edge lengths are
                         solved by multigrid-preconditioned CG: one V cycle of a smoothed-aggregation hierarchy per
                         iteration for n = 1, the product V M V of two cycles for n = 2 (needs batch = 16 and a handle
-                        prepared with IF_FLAG_MULTIGRID, else ignored); the rest by Jacobi-PCG.  With IF_FLAG_VECTOR
+                        prepared with IF_FLAG_MULTIGRID, else ignored; a call with up to 4 / 8 columns runs the
+                        4- / 8-column variants of the cycle's kernels); the rest by Jacobi-PCG.  With IF_FLAG_VECTOR
                         the same hierarchy preconditions the coupled system: the coupled operator on the mesh,
                         the scalar levels below per component.  Same systems, same
                         start vector, same stop test, same answers within the tolerance (PAPER.md:207 names the
