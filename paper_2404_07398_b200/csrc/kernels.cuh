@@ -103,7 +103,8 @@ struct Ctrl {
     int occupied[KMAX];
     unsigned int turn_fin, turn_start;
     StartParams turn_sp;
-    int snap[4];          // {columns holding a right-hand side, of those still running, q_next, 0} after the turnover
+    int snap[4];          // {slots holding a right-hand side, of those still running, q_next, 0} after the turnover
+    int cmap[KMAX];       // compaction of the stream's tail (k_mg_compact_plan): new column j <- old column cmap[j], -1 = empty
 };
 
 // what the host reads back every check_every iterations
@@ -1471,6 +1472,64 @@ __global__ void k_compact_ctrl(Ctrl* __restrict__ ctrl, ColMap map, int KN) {
         int any = 0;
         for (int k = 0; k < KMAX; ++k) any |= !ctrl->done[k];
         ctrl->all_done = !any;
+    }
+}
+
+// ---- tail of the multigrid stream: when the queue is empty and at most half of the columns still run, the survivors
+// move to the narrower kernels.  Everything is decided on the device, at the iteration boundary the host enqueues it at.
+// k_mg_compact_plan: the column map, occupied slots first in their order (a slot = a column, or a (u, v) pair).
+__global__ void k_mg_compact_plan(Ctrl* __restrict__ ctrl, int KW, int KN) {
+    const unsigned full = 0xffffffffu;
+    const int s = threadIdx.x;
+    const int step = ctrl->pair_mode ? 2 : 1;
+    const bool in = s < KW / step;
+    const bool occ = in && ctrl->occupied[s * step] != 0;
+    const unsigned occm = __ballot_sync(full, occ);
+    if (s < KMAX) ctrl->cmap[s] = -1;
+    __syncwarp();
+    if (occ) {
+        const int rank = __popc(occm & ((1u << s) - 1u));
+        for (int i = 0; i < step; ++i)
+            if (rank * step + i < KN) ctrl->cmap[rank * step + i] = s * step + i;
+    }
+}
+
+// one state vector [nv][KW] -> [nv][KN] through ctrl->cmap; `sel` picks the source of a double-buffered one:
+// 0: src0 ;  1: (src0, src1)[ctrl->cur_r] ;  2: (src0, src1)[ctrl->cur_p]
+template <int KW, int KN>
+__global__ void __launch_bounds__(BLOCK) k_mg_repack(int64_t nv, const Ctrl* __restrict__ ctrl, int sel,
+                                                     const double* __restrict__ src0, const double* __restrict__ src1,
+                                                     double* __restrict__ dst) {
+    const int64_t i = (int64_t)blockIdx.x * BLOCK + threadIdx.x;
+    if (i >= nv * KN) return;
+    const double* __restrict__ src = sel == 1 ? (ctrl->cur_r ? src1 : src0) : sel == 2 ? (ctrl->cur_p ? src1 : src0) : src0;
+    const int64_t row = i / KN;
+    const int s = ctrl->cmap[i % KN];
+    dst[i] = s >= 0 ? src[row * KW + s] : 0.0;
+}
+
+// the control block through the same map; the current buffers of the narrow layout are r'[0] and p'[0]
+__global__ void k_mg_compact_ctrl(Ctrl* __restrict__ ctrl, int KN) {
+    const int j = threadIdx.x;   // one block of KMAX threads
+    const int s = j < KN ? ctrl->cmap[j] : -1;
+    double c = 0.0, c1 = 0.0, al = 0.0, be = 0.0, rho = 0.0, bb = 0.0, rr = 0.0;
+    int field = -1, rhs = 0, done = 1, epoch = 0, status = 0, iters = 0, starting = 0, occupied = 0;
+    if (s >= 0) {
+        c = ctrl->c[s]; c1 = ctrl->c1[s]; al = ctrl->alpha[s]; be = ctrl->beta[s]; rho = ctrl->rho[s]; bb = ctrl->bb[s]; rr = ctrl->rr[s];
+        field = ctrl->field[s]; rhs = ctrl->rhs[s]; done = ctrl->done[s]; epoch = ctrl->epoch[s];
+        status = ctrl->status[s]; iters = ctrl->iters[s]; starting = ctrl->starting[s]; occupied = ctrl->occupied[s];
+    }
+    __syncthreads();
+    ctrl->c[j] = c; ctrl->c1[j] = c1; ctrl->starting[j] = starting; ctrl->alpha[j] = al; ctrl->beta[j] = be; ctrl->rho[j] = rho;
+    ctrl->bb[j] = bb; ctrl->rr[j] = rr; ctrl->field[j] = field; ctrl->rhs[j] = rhs; ctrl->done[j] = done; ctrl->epoch[j] = epoch;
+    ctrl->status[j] = status; ctrl->iters[j] = iters; ctrl->occupied[j] = occupied;
+    __syncthreads();
+    if (j == 0) {
+        int any = 0;
+        for (int k = 0; k < KMAX; ++k) any |= !ctrl->done[k];
+        ctrl->all_done = !any;
+        ctrl->cur_r = 0;
+        ctrl->cur_p = 0;
     }
 }
 

@@ -488,6 +488,11 @@ inline MgBuffers mg_layout(const if_mesh_s* h, const Workspace& w, int order_n) 
     return m;
 }
 
+// the buffers of the phase in progress: the layout of the workspace, or what a compaction of the tail made of it
+inline MgBuffers mg_buffers(const Run& r) {
+    return r.mgb ? *static_cast<const MgBuffers*>(r.mgb) : mg_layout(r.h, r.w, r.order_n);
+}
+
 // level 0: the prolongation kernel can form e = omega r'/d itself (short prolongator rows only)
 inline bool mg_fused_prolongation(const MgLevel& g) { return g.p_nnz < IF_MG_WIDE * g.n; }
 inline MgMat mg_mat(const MgLevel& g) { return MgMat{g.rowptr, g.col, g.sm, g.diag, g.n, g.omega}; }
@@ -740,7 +745,7 @@ int mg_cycle_level0(const Run& r, const MgBuffers& b, const double* R0, const do
 template <int K>
 int mg_enqueue_iteration(const Run& r, IterTimer* tm) {
     const if_mesh_s* h = r.h;
-    const MgBuffers b = mg_layout(h, r.w, r.order_n);
+    const MgBuffers b = mg_buffers(r);
     const int nu = r.mg_nu[0];
     double om[MG_MAX_NU];
     mg_omegas(h->mg[0], nu, om);

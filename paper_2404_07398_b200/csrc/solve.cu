@@ -84,6 +84,7 @@ struct Run {
     bool mg = false;   // this phase runs multigrid-preconditioned CG (mg_solve.cuh) instead of Jacobi-PCG
     MgGrids mgg;
     int mg_nu[3] = {1, 1, 2};   // Jacobi sweeps per side of the V cycle on the mesh, on level 1, below (mg_solve.cuh)
+    const void* mgb = nullptr;  // MgBuffers of the phase in progress once the stream's tail has been compacted (mg_buffers)
 };
 
 template <class Kern>
@@ -287,7 +288,7 @@ int start_columns(const Run& r, unsigned mask, const StartParams& sp, const doub
     const unsigned eg = (unsigned)((h->n_vert * K + BLOCK - 1) / BLOCK);
     int rc;
     if (r.mg) {   // multigrid path: the column joins the stream, its first iteration forms r0 (k_mg_start)
-        const MgBuffers b = mg_layout(h, r.w, r.order_n);
+        const MgBuffers b = mg_buffers(r);
         k_mg_start<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, sp, mask, d_fields, b.x, b.zb, b.r[0],
                                                       b.r[1], b.p[0], b.p[1]);
         IF_LAUNCH_CHECK();
@@ -629,15 +630,15 @@ int solve_from(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& 
 template <int K>
 int mg_enqueue_turnover(const Run& r, Job job, double* d_out, const double* d_fields, bool first = false) {
     const if_mesh_s* h = r.h;
-    const MgBuffers b = mg_layout(h, r.w, r.order_n);
+    const MgBuffers b = mg_buffers(r);
     k_turn_plan<<<1, 32, 0, r.st>>>(r.w.ctrl, r.w.queue, K, first ? 1 : 0, r.w.iters, r.w.status, r.w.relres);
     IF_LAUNCH_CHECK();
     if (job == JOB_SPECTRUM) {
-        k_energy<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1,
-                                                      h->total_area, r.w.energy);
+        k_energy<K><<<r.g.stream, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, r.w.partials, MASK_TURN_FIN, b.x, b.p[0], b.p[1],
+                                                    h->total_area, r.w.energy);
     } else {
         const int sgrid = (int)std::min<int64_t>((h->n_vert + 31) / 32, (int64_t)h->n_sm * 8);
-        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, MASK_TURN_FIN, r.w.x, r.w.p0, r.w.p1, 1, d_out, d_fields,
+        k_scatter<K><<<sgrid, BLOCK, 0, r.st>>>(r.m, r.w.ctrl, MASK_TURN_FIN, b.x, b.p[0], b.p[1], 1, d_out, d_fields,
                                                   (r.opt.flags & IF_FLAG_HIGHPASS) ? 1 : 0);
     }
     IF_LAUNCH_CHECK();
@@ -658,15 +659,20 @@ int mg_enqueue_turnover(const Run& r, Job job, double* d_out, const double* d_fi
 // one CUDA graph = one iteration + the turnover, and the host only launches graphs and reads, one launch behind, how
 // many columns still hold a right-hand side.  A stopped column runs its next right-hand side in the very next iteration
 // (the host-driven refill of solve_phase, which sees a stop one launch late, loses an iteration per right-hand side).
+// `first`: the queue and a fresh control block are set up and the first right-hand sides started; otherwise the state
+// comes from a wider phase (mg_compact).  *compact_to (if given): set to 8 or 4 when the queue is empty and the columns
+// still running fit that width -- the caller compacts after the launch already enqueued and goes on there.
 template <int K>
 int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
-                        PollState& poll, KernelTimes* times) {
+                        PollState& poll, KernelTimes* times, bool first, int* compact_to) {
     int rc;
+    if (compact_to) *compact_to = 0;
     if ((rc = setup_grids<K>(r))) return rc;
     if ((rc = mg_setup<K>(r))) return rc;
     const size_t R = rhs.size();
     if (R == 0 || R > (size_t)MAX_RHS || !r.w.queue) return IF_EINVAL;
-    std::vector<QEntry> hq(R);
+    std::vector<QEntry> hq(first ? R : 0);
+    if (first) {
     for (size_t i = 0; i < R; ++i) {
         const Rhs& s = rhs[i];
         hq[i].c = r.opt.gamma * std::pow(s.ell, 2.0 * r.order_n);
@@ -684,6 +690,7 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.ctrl, &hc, sizeof(Ctrl), cudaMemcpyHostToDevice, r.st));
     IF_CUDA_TRY(cudaMemcpyAsync(r.w.queue, hq.data(), R * sizeof(QEntry), cudaMemcpyHostToDevice, r.st));
     if ((rc = mg_enqueue_turnover<K>(r, job, d_out, d_fields, true))) return rc;      // the first K right-hand sides
+    }
 
     long long launches_per_graph = 0;
     GraphSet gs;
@@ -719,9 +726,81 @@ int mg_stream_on_device(Run& r, Job job, const double* d_fields, const std::vect
         // launch it-1 did full work in every kernel: take its timing sample (graph (it-1)&1 is idle now)
         if (times && use_graph && worked && running > 0) add_timing_sample(*times, gs.tev[(it - 1) & 1]);
         if (occupied == 0) finished = true;      // every right-hand side has been started, stopped and finalised
+        // the tail: the queue is empty and the slots still occupied fit a narrower set of kernels
+        const int occ_cols = occupied * (r.vec ? 2 : 1);
+        if (!finished && compact_to && K > 4 && snap[4 * prev + 2] >= (int)R && occ_cols <= K / 2) {
+            *compact_to = (occ_cols <= 4) ? 4 : 8;
+            return IF_OK;   // the launch already enqueued runs first; the caller repacks after it
+        }
     }
     if (!finished) return IF_ECUDA;   // cannot happen: every column stops at max_iter
     return IF_OK;
+}
+
+// The columns still running move from the KW-wide layout `b` to a KN-wide one (KN <= KW / 2), decided and done on the
+// device at the iteration boundary this is enqueued at: x, the current r and p, and z are repacked into the halves of
+// buffers that are dead there (q, za), the other narrow buffers take the halves of what the repacking freed.
+template <int KW, int KN>
+int mg_compact(const Run& r, const MgBuffers& b, MgBuffers* out) {
+    static_assert(2 * KN <= KW, "compaction at least halves the width");
+    const if_mesh_s* h = r.h;
+    const int64_t nv = h->n_vert;
+    const size_t vn = (size_t)nv * KN;      // doubles per narrow vector: two fit every buffer of the wide layout
+    const unsigned g = (unsigned)((vn + BLOCK - 1) / BLOCK);
+    MgBuffers n = b;
+    n.x = b.q;          n.r[0] = b.q + vn;
+    n.zb = b.za;        n.p[0] = b.za + vn;
+    n.r[1] = b.t;       n.p[1] = b.t + vn;
+    n.q = b.x;          n.za = b.x + vn;
+    n.t = b.zb;
+    k_mg_compact_plan<<<1, 32, 0, r.st>>>(r.w.ctrl, KW, KN);
+    IF_LAUNCH_CHECK();
+    k_mg_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, r.w.ctrl, 0, b.x, nullptr, n.x);
+    IF_LAUNCH_CHECK();
+    k_mg_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, r.w.ctrl, 1, b.r[0], b.r[1], n.r[0]);
+    IF_LAUNCH_CHECK();
+    k_mg_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, r.w.ctrl, 0, b.zb, nullptr, n.zb);
+    IF_LAUNCH_CHECK();
+    k_mg_repack<KW, KN><<<g, BLOCK, 0, r.st>>>(nv, r.w.ctrl, 2, b.p[0], b.p[1], n.p[0]);
+    IF_LAUNCH_CHECK();
+    k_mg_compact_ctrl<<<1, KMAX, 0, r.st>>>(r.w.ctrl, KN);
+    IF_LAUNCH_CHECK();
+    const MgLevel& gl = h->mg[h->mg_levels - 1];      // K^-1 of the coarsest level under the new column numbers
+    if (gl.n <= MG_COARSEST) {
+        IF_CUDA_TRY(cudaFuncSetAttribute(k_mg_coarse_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MG_FACTOR_SMEM));
+        k_mg_coarse_factor<<<KN, 64, MG_FACTOR_SMEM, r.st>>>(mg_mat(gl), r.w.ctrl, (1u << KN) - 1u, n.coarse_inv);
+        IF_LAUNCH_CHECK();
+    }
+    *out = n;
+    return IF_OK;
+}
+
+template <int K>
+int mg_stream_from(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& rhs, int n_ells, double* d_out,
+                   PollState& poll, KernelTimes* times, bool first) {
+    int to = 0;
+    int rc = mg_stream_on_device<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, first, K > 4 ? &to : nullptr);
+    if (rc != IF_OK || to == 0) return rc;
+    const MgBuffers cur = mg_buffers(r);
+    MgBuffers narrow;
+    const void* saved = r.mgb;
+    if constexpr (K == 16) {
+        if (to == 8) {
+            if ((rc = mg_compact<16, 8>(r, cur, &narrow))) return rc;
+            r.mgb = &narrow;
+            rc = mg_stream_from<8>(r, job, d_fields, rhs, n_ells, d_out, poll, nullptr, false);
+        } else {
+            if ((rc = mg_compact<16, 4>(r, cur, &narrow))) return rc;
+            r.mgb = &narrow;
+            rc = mg_stream_from<4>(r, job, d_fields, rhs, n_ells, d_out, poll, nullptr, false);
+        }
+    } else if constexpr (K == 8) {
+        if ((rc = mg_compact<8, 4>(r, cur, &narrow))) return rc;
+        r.mgb = &narrow;
+        rc = mg_stream_from<4>(r, job, d_fields, rhs, n_ells, d_out, poll, nullptr, false);
+    }
+    r.mgb = saved;
+    return rc;
 }
 
 template <int K>
@@ -739,7 +818,7 @@ int solve_all(Run& r, Job job, const double* d_fields, const std::vector<Rhs>& r
         const bool big = r.h->n_vert * (r.order_n == 1 ? 1 : 4) >= MG_DEVICE_TURNOVER_ROWS;
         const bool host_refill = env != nullptr ? atoi(env) != 0 : !big;
         on_device = r.mg && !host_refill;
-        if (on_device) rc = mg_stream_on_device<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times);
+        if (on_device) rc = mg_stream_from<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, true);
     }
     if (!on_device) rc = solve_from<K>(r, job, d_fields, rhs, n_ells, d_out, poll, times, q, true);
     if (rc != IF_OK) return rc;
