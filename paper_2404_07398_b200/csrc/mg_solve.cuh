@@ -9,8 +9,10 @@
 //           (PAPER.md:207 names the loss of convergence of the biharmonic filter at large l as the open problem).
 //   V is a fixed symmetric positive definite operator per column (fixed sweep counts, the same damping before and
 //   after the coarse correction), hence so are B = V and B = V M V, and plain PCG applies.
-// 16 columns at a time, every column with its own c, alpha, beta and stop time; all per-column scalars live in the
-// device control block (Ctrl), so ONE iteration is a fixed launch sequence, captured in a CUDA graph by solve.cu:
+// K = 16 columns at a time (8 or 4 when a call has no more right-hand sides than that, and for the tail of the stream:
+// every kernel here takes the width as a template parameter), every column with its own c, alpha, beta and stop time;
+// all per-column scalars live in the device control block (Ctrl), so ONE iteration is a fixed launch sequence, captured
+// in a CUDA graph by solve.cu (written for K = 16):
 //       k_spmm<16, CG1>  (n = 2: CG2A, CG2B)   p' = z + beta p ; x += alpha p ; q = A p' ; alpha' = rho / p'.q
 //       k_spmm<16, MGR>      r' = r - alpha' q ; e = omega r'/d ; t = r' - K e    (residual update, first sweep of V on
 //                            level 0 and its residual in one pass), then restriction, coarse levels, prolongation
@@ -20,14 +22,17 @@
 // A (re)started column (Ctrl::starting, set by k_mg_start) joins at an iteration boundary with x = 0, z = phi, r = M phi:
 // its first iteration has alpha = 1, which makes kernel A and the fused residual kernel form r0 = M phi - A phi on the
 // way (no pass of its own over the matrix), and ends with rho = r0.z0, beta = 0 -- the start of PCG from x0 = phi -- so
-// columns are refilled from the queue as in the Jacobi path and the host never waits inside the loop.
+// columns are refilled from the queue as in the Jacobi path and the host never waits inside the loop (on large meshes
+// the ending and starting of columns is itself part of every iteration's graph: k_turn_plan, solve.cu).
+// With IF_FLAG_VECTOR the level-0 kernels are the VEC variants (coupled operator D_2 with the metric terms), the levels
+// below work per component.
 // The stop test is the same as in the Jacobi path: recursive ||r||_2 <= tol ||M phi||_2.
 #pragma once
 
 namespace ifl {
 namespace {
 
-constexpr int MGK = 16;               // columns of the multigrid path
+constexpr int MGK = 16;               // columns of the multigrid path at full width (buffers are sized for it)
 constexpr size_t MG_FACTOR_SMEM = 2 * (size_t)MG_COARSEST * (MG_COARSEST + 1) * sizeof(double);   // k_mg_coarse_factor
 constexpr int MG_REFILL_MIN = 1;      // stopped columns are restarted as soon as this many are free (solve.cu)
 // right-hand sides below this many mean edge lengths stay on the Jacobi path (option mg_min_ell = 0)
@@ -56,7 +61,7 @@ struct MgMat {                        // one level's (S, M) pair
     double omega;                     // Jacobi damping of the smoother on this level
 };
 
-// A row is handled by 8 * SL threads: column pair l = tid % 8, entry slice sl = (tid / 8) % SL.  SL = 1 for the
+// A row is handled by TPR * SL threads (TPR = K / 2): column pair l = tid % TPR, entry slice sl = (tid / TPR) % SL.  SL = 1 for the
 // short rows of the fine levels; SL = 4 (one row per warp, slices added with two shuffles) for the coarse levels
 // whose rows have hundreds of entries and would otherwise be walked serially.
 // MODE 0: y = A x ;  MODE 1: y = r - A x ;  MODE 2: y = x + omega (r - A x) / d        with A = M + c S per column
