@@ -784,6 +784,8 @@ int mg_stream_from(Run& r, Job job, const double* d_fields, const std::vector<Rh
     const MgBuffers cur = mg_buffers(r);
     MgBuffers narrow;
     const void* saved = r.mgb;
+    if (const char* v = getenv("IF_VERBOSE"))
+        if (atoi(v) >= 1) fprintf(stderr, "[implicit_filter] multigrid stream: tail moved from %d to %d columns\n", K, to);
     if constexpr (K == 16) {
         if (to == 8) {
             if ((rc = mg_compact<16, 8>(r, cur, &narrow))) return rc;

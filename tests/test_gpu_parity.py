@@ -748,7 +748,7 @@ def test_multigrid_stream_refills_columns_and_is_deterministic(ifl, oracle_mod, 
 
 
 @pytest.mark.parametrize("order_n", [1, 2])
-def test_multigrid_turnover_on_device_matches_host_refill(ifl, oracle_mod, order_n, monkeypatch):
+def test_multigrid_turnover_on_device_matches_host_refill(ifl, oracle_mod, order_n, monkeypatch, capfd):
     """The multigrid stream ends and starts its columns on the device (k_turn_plan inside every iteration's graph;
     the host only watches).  Against the host-driven refill of the Jacobi path's loop (IF_MG_HOST_REFILL=1), which
     sees a stop one launch late: the same per-right-hand-side arithmetic, so the same iteration counts and fields to
@@ -761,7 +761,13 @@ def test_multigrid_turnover_on_device_matches_host_refill(ifl, oracle_mod, order
     for nf, ne in ((1, 3), (2, 8), (5, 9)):                      # 3, 16 and 45 right-hand sides
         fields, ells = w.fields[:nf], w.ells[:ne]
         monkeypatch.setenv("IF_MG_HOST_REFILL", "0")             # (unset: by mesh size, the host on a mesh this small)
+        monkeypatch.setenv("IF_VERBOSE", "1")
+        capfd.readouterr()
         dev, sd = ifl.if_filter(h, fields, ells, order_n, solver=1, mg_min_ell=0.5)
+        trace = capfd.readouterr().err
+        monkeypatch.delenv("IF_VERBOSE")
+        if nf * ne > 8:      # the tail of the stream really moves to the narrower kernels (16 -> 8 or 4, 8 -> 4)
+            assert "tail moved from 16 to" in trace, trace
         spd = ifl.if_spectrum(h, fields, ells, order_n, solver=1, mg_min_ell=0.5)
         monkeypatch.setenv("IF_MG_HOST_REFILL", "1")
         host, sh = ifl.if_filter(h, fields, ells, order_n, solver=1, mg_min_ell=0.5)
